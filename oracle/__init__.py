@@ -1,0 +1,168 @@
+"""CPU oracle for the PVG forward render -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Thin ctypes wrapper over oracle/pvg_oracle.cpp (plain C++, double precision,
+written from the paper; see that file's header for citations and pins). Only
+tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package. It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+SLOTS = dict(mu=slice(0, 3), op=3, pcam=slice(4, 7), sigma=slice(7, 13), cov=slice(13, 16),
+             conic=slice(16, 19), mean=slice(19, 21), ext=slice(21, 23), rgb=slice(23, 26),
+             cull=26, rect=slice(27, 31), count=31)
+CULL_REASONS = {0: "valid", 1: "opacity", 2: "near", 3: "det", 4: "rect", 5: "nonfinite"}
+
+
+class _Cam(C.Structure):
+    _fields_ = [("width", C.c_int), ("height", C.c_int), ("fx", C.c_double), ("fy", C.c_double),
+                ("cx", C.c_double), ("cy", C.c_double), ("w2c", C.c_double * 12),
+                ("znear", C.c_double), ("bg", C.c_double * 3)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        L.oracle_tile_counts.restype = C.c_uint64
+        L.oracle_tile_list.restype = C.c_uint64
+        L.oracle_record_stride.restype = C.c_int
+        L.oracle_num_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _cam(cam) -> _Cam:
+    c = _Cam()
+    c.width, c.height = int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    w2c = np.asarray(cam.world_to_cam, dtype=np.float64).reshape(12)
+    for i in range(12):
+        c.w2c[i] = float(w2c[i])
+    c.znear = float(cam.znear)
+    for i in range(3):
+        c.bg[i] = float(cam.bg[i])
+    return c
+
+
+def _f32(a, shape):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    assert a.shape == shape, (a.shape, shape)
+    return a
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().oracle_set_threads(C.c_int(int(n)))
+
+
+def preprocess(mu, quat, scale, opacity, sh, tau, beta, vel, cycle, sh_degree, cam, t):
+    """Oracle-P. Returns (wide [n,32] float64, rec32 [n,12] float32)."""
+    n = int(np.asarray(mu).shape[0])
+    mu = _f32(mu, (n, 3)); quat = _f32(quat, (n, 4)); scale = _f32(scale, (n, 3))
+    opacity = _f32(opacity, (n,)); sh = _f32(sh, (n, 16, 3)); tau = _f32(tau, (n,))
+    beta = _f32(beta, (n,)); vel = _f32(vel, (n, 3))
+    wide = np.empty((n, 32), dtype=np.float64)
+    rec = np.empty((n, 12), dtype=np.float32)
+    c = _cam(cam)
+    lib().oracle_preprocess(C.c_uint64(n), _p(mu), _p(quat), _p(scale), _p(opacity), _p(sh), _p(tau),
+                            _p(beta), _p(vel), C.c_double(float(cycle)), C.c_int(int(sh_degree)),
+                            C.byref(c), C.c_double(float(t)), _p(wide), _p(rec))
+    return wide, rec
+
+
+def preprocess_scene(scene, cam, t):
+    """Oracle-P on an object with the workloads.Scene attribute names."""
+    return preprocess(scene.mu, scene.quat, scene.scale, scene.opacity, scene.sh, scene.tau,
+                      scene.beta, scene.vel, scene.cycle, scene.sh_degree, cam, t)
+
+
+def sh_basis(d: Sequence[float]) -> np.ndarray:
+    d = np.ascontiguousarray(d, dtype=np.float64)
+    Y = np.empty(16, dtype=np.float64)
+    lib().oracle_sh_basis(_p(d), _p(Y))
+    return Y
+
+
+def tile_counts(rec, width, height):
+    """Integer chain step 1. Returns (rects [n,4] int32 inclusive, counts [n] uint32, M)."""
+    rec = np.ascontiguousarray(rec, dtype=np.float32)
+    n = rec.shape[0]
+    assert rec.shape == (n, 12)
+    rects = np.empty((n, 4), dtype=np.int32)
+    counts = np.empty(n, dtype=np.uint32)
+    M = lib().oracle_tile_counts(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), _p(rects),
+                                 _p(counts))
+    return rects, counts, int(M)
+
+
+def keys(rec, width, height, order_mode=0):
+    """Integer chain step 2 (offsets, unsorted list, std::stable_sort, ranges)."""
+    rec = np.ascontiguousarray(rec, dtype=np.float32)
+    n = rec.shape[0]
+    _, _, M = tile_counts(rec, width, height)
+    ntiles = ((width + 15) // 16) * ((height + 15) // 16)
+    out = dict(M=M,
+               offsets=np.zeros(n, dtype=np.uint64),
+               keys_unsorted=np.zeros(M, dtype=np.uint64), vals_unsorted=np.zeros(M, dtype=np.uint32),
+               keys_sorted=np.zeros(M, dtype=np.uint64), vals_sorted=np.zeros(M, dtype=np.uint32),
+               ranges=np.zeros((ntiles, 2), dtype=np.uint32))
+    lib().oracle_keys(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_int(order_mode),
+                      _p(out["offsets"]), _p(out["keys_unsorted"]), _p(out["vals_unsorted"]),
+                      _p(out["keys_sorted"]), _p(out["vals_sorted"]), _p(out["ranges"]))
+    return out
+
+
+def tile_list(rec, width, height, tile):
+    """Sorted instance list of one tile, computed directly. Returns (keys u64, vals u32)."""
+    rec = np.ascontiguousarray(rec, dtype=np.float32)
+    n = rec.shape[0]
+    L = lib()
+    cnt = int(L.oracle_tile_list(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height),
+                                 C.c_uint32(tile), C.c_uint64(0), None, None))
+    k = np.zeros(cnt, dtype=np.uint64)
+    v = np.zeros(cnt, dtype=np.uint32)
+    if cnt:
+        L.oracle_tile_list(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_uint32(tile),
+                           C.c_uint64(cnt), _p(k), _p(v))
+    return k, v
+
+
+def render(rec, width, height, bg=(0.0, 0.0, 0.0), mode="binned", tiles: Optional[Sequence[int]] = None,
+           tie_budget: bool = False):
+    """Oracle-R on an fp32 record. mode 'brute' or 'binned'. Returns dict of float64
+    images: rgb [3,H,W], depth, alpha, budget, cond [H,W], plus visited / contributed."""
+    rec = np.ascontiguousarray(rec, dtype=np.float32)
+    n = rec.shape[0]
+    assert rec.shape == (n, 12)
+    H, W = int(height), int(width)
+    rgb = np.empty((3, H, W)); depth = np.empty((H, W)); alpha = np.empty((H, W))
+    budget = np.empty((H, W)); cond = np.empty((H, W))
+    stats = np.zeros(2, dtype=np.uint64)
+    bg = np.ascontiguousarray(bg, dtype=np.float64)
+    tl, ntl = None, 0
+    if tiles is not None:
+        tl_arr = np.ascontiguousarray(tiles, dtype=np.uint32)
+        tl, ntl = _p(tl_arr), tl_arr.shape[0]
+    lib().oracle_render(C.c_uint64(n), _p(rec), C.c_int(W), C.c_int(H), _p(bg),
+                        C.c_int({"brute": 0, "binned": 1}[mode]), tl, C.c_uint64(ntl),
+                        C.c_int(1 if tie_budget else 0), _p(rgb), _p(depth), _p(alpha), _p(budget),
+                        _p(cond), _p(stats))
+    return dict(rgb=rgb, depth=depth, alpha=alpha, budget=budget, cond=cond,
+                visited=int(stats[0]), contributed=int(stats[1]))
