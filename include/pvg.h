@@ -1,0 +1,172 @@
+/* pvg.h -- C ABI of the B200-native Periodic Vibration Gaussian forward renderer.
+ *
+ * One hot path of arxiv 2311.18561: the time-conditioned forward splatting render
+ *     I^ = Render({H_i(t)}; E, I)                 (Eq. 8; F_theta(E_o, I_o, t), L57)
+ * with H(t) = {mu~(t), q, s, o~(t), c}            (Eq. 5)
+ *      mu~(t) = mu + l/(2 pi) sin(2 pi (t-tau)/l) v   (Eq. 6)
+ *      o~(t)  = o exp(-(t-tau)^2 / (2 beta^2))        (Eq. 7)
+ * rendered by EWA projection (Eq. 2), depth sort (L70) and front-to-back
+ * alpha compositing (Eq. 3) into colour, normalised depth and opacity (L87, L168).
+ *
+ * Every step runs in hand-written CUDA kernels for sm_100a. There is NO CPU
+ * fallback: without a CUDA device every compute entry point returns PVG_ERR_CUDA.
+ * All functions return 0 (PVG_OK) or a negative pvg_status; nothing throws or
+ * aborts across this boundary. One render at a time per scene; distinct scenes
+ * are independent. Readings of the points the paper leaves open are in DESIGN.md.
+ */
+#ifndef PVG_H_
+#define PVG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum pvg_status {
+  PVG_OK = 0,
+  PVG_ERR_NULL = -1,              /* a required pointer is NULL */
+  PVG_ERR_BAD_DESC = -2,          /* n == 0 or n >= 2^31, cycle <= 0 or NaN, sh_degree outside 0..3 */
+  PVG_ERR_BAD_CAMERA = -3,        /* non-positive or non-finite size / focal length, size > 32768 */
+  PVG_ERR_OOM = -4,               /* device allocation failed */
+  PVG_ERR_INSTANCE_OVERFLOW = -5, /* tile instances M >= 2^32 */
+  PVG_ERR_CUDA = -6,              /* CUDA runtime error (or no device); see pvg_last_cuda_error */
+  PVG_ERR_BAD_OPTION = -7
+} pvg_status;
+
+typedef struct pvg_scene pvg_scene; /* opaque; owns device copies of the model and a growable workspace */
+
+/* The model theta = per-point {mu, q, s, o, c, tau, beta, v} + cycle length l
+ * (PAPER.md:L110). All arrays are dense, row-major float32, read once by
+ * pvg_create_scene (the caller may free them on return). */
+typedef struct pvg_scene_desc {
+  uint64_t n;           /* points, 1 .. 2^31-1 */
+  const float *mu;      /* [n][3]  world position mu  */
+  const float *quat;    /* [n][4]  rotation (w,x,y,z); normalised by the library (L79)      */
+  const float *scale;   /* [n][3]  std-devs s > 0, already activated        (L79)           */
+  const float *opacity; /* [n]     o in [0,1], already activated            (L61)           */
+  const float *sh;      /* [n][16][3] degree-3 real SH, coefficient-major, channel-minor    */
+  const float *tau;     /* [n]     life peak tau                            (L95)           */
+  const float *beta;    /* [n]     lifespan beta > 0; +INF = never fades    (L110, L114)    */
+  const float *vel;     /* [n][3]  v = d mu~/dt at tau                      (L110)          */
+  float cycle;          /* l > 0; +INF selects the linear model mu + (t-tau) v (L336)       */
+  int sh_degree;        /* 0..3: bands above it are ignored */
+  int pointers_on_device; /* 0: host pointers, 1: device pointers (copied either way) */
+} pvg_scene_desc;
+
+/* Camera pose [E_o, I_o]. Pinhole, no distortion.
+ * p_cam = R p_world + T with world_to_cam = row-major 3x4 [R|T]; +z forward,
+ * +x right, +y down. Pixel (i,j) has its centre at (i+0.5, j+0.5). */
+typedef struct pvg_camera {
+  int width, height;      /* 1 .. 32768 */
+  float fx, fy, cx, cy;   /* pixels */
+  float world_to_cam[12];
+  float znear;            /* cull p_cam.z <= znear; <= 0 selects the default 0.2 */
+  float bg[3];            /* constant background colour: rgb = C + (1 - O) bg (L168 with constant f_sky) */
+} pvg_camera;
+
+/* ---- plumbing: device memory and stream come from the caller (PyTorch) -------------------- */
+
+/* Device allocator hooks (process-wide; set before the first pvg_create_scene).
+ * alloc returns a device pointer aligned to >= 256 B or NULL; `stream` is the
+ * cudaStream_t the memory will first be used on. NULL hooks restore cudaMalloc/cudaFree. */
+typedef void *(*pvg_alloc_fn)(size_t bytes, void *stream, void *user);
+typedef void (*pvg_free_fn)(void *ptr, void *user);
+int pvg_set_allocator(pvg_alloc_fn alloc_fn, pvg_free_fn free_fn, void *user);
+
+/* cudaStream_t (as void*) that pvg_render enqueues on; default: the legacy default stream. */
+int pvg_set_stream(pvg_scene *scene, void *cuda_stream);
+
+/* ---- the path ---------------------------------------------------------------------------- */
+
+/* Copies the model to the device and re-lays it out (structure of arrays, float4). */
+int pvg_create_scene(const pvg_scene_desc *desc, pvg_scene **out);
+
+/* Renders the frame at timestamp t. Outputs are caller-owned DEVICE buffers:
+ *   out_rgb [3][H][W], out_depth [H][W] (sum T a z / sum T a, 0 where alpha == 0), out_alpha [H][W] (O = sum T a).
+ * Any of the three may be NULL (not written). Work is enqueued on the scene's stream; the call
+ * blocks once, to read the instance count M back (it sizes the sort buffers), and returns with
+ * the blend kernel still in flight. */
+int pvg_render(pvg_scene *scene, const pvg_camera *cam, float t, float *out_rgb, float *out_depth,
+               float *out_alpha);
+
+/* Same frame into HOST buffers (pinned or pageable): renders into library-owned device images,
+ * copies them back and synchronises the stream before returning. */
+int pvg_render_host(pvg_scene *scene, const pvg_camera *cam, float t, float *host_rgb,
+                    float *host_depth, float *host_alpha);
+
+int pvg_destroy(pvg_scene *scene);
+
+/* ---- options ------------------------------------------------------------------------------ */
+typedef enum pvg_option {
+  /* 1 (default): sort the Gaussians by depth first (n keys, 32 bits), emit tile instances in that
+   *    order, then radix-sort the M instances on the tile-id bits only.
+   * 0: emit in index order and radix-sort all 32 + ceil(log2 tiles) key bits of the M instances.
+   * Both are the same stable LSD sort and give bit-identical sorted lists and ranges. */
+  PVG_OPT_PRESORT_DEPTH = 1,
+  /* 1: keep a copy of the unsorted (key,value) list for pvg_debug_view (default 0). */
+  PVG_OPT_KEEP_UNSORTED = 2,
+  /* 1 (default): record a CUDA event pair around every kernel of the last render
+   * (pvg_kernel_times_ms, pvg_stage_times_ms). 2: keep the records of EVERY render until
+   * pvg_kernel_times_ms reads (and clears) them. 0: no events. */
+  PVG_OPT_KERNEL_EVENTS = 3
+} pvg_option;
+int pvg_set_option(pvg_scene *scene, int option, int64_t value);
+
+/* ---- test and measurement hooks (not part of the paper's problem) ------------------------- */
+
+/* Device views of the last render's intermediates, valid until the next call on the scene. */
+typedef struct pvg_debug {
+  uint64_t n;                    /* points */
+  uint64_t num_instances;        /* M = sum of counts */
+  uint32_t tiles_x, tiles_y;     /* ceil(W/16), ceil(H/16) */
+  uint32_t sort_begin_bit, sort_end_bit; /* key bits the M-instance sort covered */
+  const float *record;           /* [n][12] (mx,my,z,o~ | a,b,c,hx | r,g,b,hy); all 0 if culled */
+  const uint32_t *counts;        /* [n] tiles touched (0 if culled) */
+  const uint32_t *visit_order;   /* [n] Gaussian index visited at position r; NULL = identity (PRESORT_DEPTH=0) */
+  const uint32_t *offsets;       /* [n] exclusive instance offset of visit position r */
+  const uint64_t *keys_unsorted; /* [M] (tile << 32 | fp32 bits of z), NULL unless KEEP_UNSORTED */
+  const uint32_t *vals_unsorted; /* [M] Gaussian index */
+  const uint64_t *keys_sorted;   /* [M] */
+  const uint32_t *vals_sorted;   /* [M] */
+  const uint32_t *ranges;        /* [tiles][2] = [begin, end) of each tile in the sorted list */
+} pvg_debug;
+int pvg_debug_view(pvg_scene *scene, pvg_debug *out);
+
+/* Stages of the last render; ms[] from CUDA events on the scene's stream (synchronises). */
+enum {
+  PVG_STAGE_PREPROCESS = 0, /* a1 */
+  PVG_STAGE_DEPTH_SORT = 1, /* a3, the n-key part (PRESORT_DEPTH=1) */
+  PVG_STAGE_DUPLICATE = 2,  /* a2 scan + key emission */
+  PVG_STAGE_SORT = 3,       /* a3, the M-instance part */
+  PVG_STAGE_RANGES = 4,     /* a4 */
+  PVG_STAGE_BLEND = 5,      /* a5 */
+  PVG_NUM_STAGES = 6
+};
+int pvg_stage_times_ms(pvg_scene *scene, float ms[PVG_NUM_STAGES]);
+
+/* Per-kernel device times of the last render, in launch order. Fills up to `cap` entries of
+ * names (static strings), stage ids and milliseconds; returns the number of launches (>= 0)
+ * or a negative pvg_status. */
+int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stages, float *ms);
+
+/* The onesweep LSD radix sort as a primitive: stable sort of n (key,value) pairs on key bits
+ * [begin_bit, end_bit). All pointers are DEVICE buffers of n elements; the sorted result is
+ * written to keys_out/vals_out, keys_in/vals_in are clobbered. Runs on `cuda_stream` and
+ * synchronises it. */
+int pvg_sort_pairs(uint64_t n, uint64_t *keys_in, uint32_t *vals_in, uint64_t *keys_out,
+                   uint32_t *vals_out, int begin_bit, int end_bit, void *cuda_stream);
+
+/* Debug helper so that bindings need no CUDA runtime of their own: synchronous copy of `bytes`
+ * from a device pointer (e.g. a pvg_debug view) into host memory. */
+int pvg_memcpy_d2h(void *host_dst, const void *device_src, size_t bytes);
+
+const char *pvg_strerror(int code);
+const char *pvg_last_cuda_error(void); /* text of the last CUDA error seen by this thread's calls */
+int pvg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PVG_H_ */

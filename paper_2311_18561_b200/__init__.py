@@ -1,0 +1,286 @@
+"""paper_2311_18561_b200 -- Python binding of libpvg.so (include/pvg.h).
+
+Argument marshalling only: every step of the render runs in the CUDA kernels of
+csrc/. PyTorch provides device memory (caching-allocator hooks), the stream and
+output tensors. There is no CPU fallback: if the library cannot be loaded, or no
+CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpvg.so")
+
+PVG_OK = 0
+STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_BAD_CAMERA",
+          -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION"}
+OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS = 1, 2, 3
+STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
+NUM_STAGES = len(STAGES)
+
+# every symbol include/pvg.h declares
+EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
+           "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms",
+           "pvg_sort_pairs", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
+
+
+class PvgError(RuntimeError):
+    def __init__(self, code: int, detail: str = ""):
+        self.code = code
+        super().__init__(f"{STATUS.get(code, code)}: {detail}")
+
+
+class SceneDesc(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("mu", C.c_void_p), ("quat", C.c_void_p), ("scale", C.c_void_p),
+                ("opacity", C.c_void_p), ("sh", C.c_void_p), ("tau", C.c_void_p), ("beta", C.c_void_p),
+                ("vel", C.c_void_p), ("cycle", C.c_float), ("sh_degree", C.c_int),
+                ("pointers_on_device", C.c_int)]
+
+
+class CameraC(C.Structure):
+    _fields_ = [("width", C.c_int), ("height", C.c_int), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("world_to_cam", C.c_float * 12),
+                ("znear", C.c_float), ("bg", C.c_float * 3)]
+
+
+class DebugC(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("num_instances", C.c_uint64), ("tiles_x", C.c_uint32),
+                ("tiles_y", C.c_uint32), ("sort_begin_bit", C.c_uint32), ("sort_end_bit", C.c_uint32),
+                ("record", C.c_void_p), ("counts", C.c_void_p), ("visit_order", C.c_void_p),
+                ("offsets", C.c_void_p), ("keys_unsorted", C.c_void_p), ("vals_unsorted", C.c_void_p),
+                ("keys_sorted", C.c_void_p), ("vals_sorted", C.c_void_p), ("ranges", C.c_void_p)]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+_lib = None
+_hooks = None  # keeps the ctypes callbacks alive
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libpvg.so (no CUDA call is made). Fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise ImportError(f"{p} is missing: build it with `python -m paper_2311_18561_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(p)
+    L.pvg_strerror.restype = C.c_char_p
+    L.pvg_last_cuda_error.restype = C.c_char_p
+    L.pvg_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    L.pvg_create_scene.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
+    L.pvg_render.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_render_host.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_destroy.argtypes = [C.c_void_p]
+    L.pvg_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
+    L.pvg_debug_view.argtypes = [C.c_void_p, C.POINTER(DebugC)]
+    L.pvg_stage_times_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    L.pvg_kernel_times_ms.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_int),
+                                      C.POINTER(C.c_float)]
+    L.pvg_sort_pairs.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                 C.c_void_p]
+    L.pvg_memcpy_d2h.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+    L.pvg_set_allocator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    if path is None:
+        _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != PVG_OK:
+        L = load_library()
+        detail = L.pvg_strerror(rc).decode()
+        if rc == -6:
+            detail += " | " + L.pvg_last_cuda_error().decode()
+        raise PvgError(rc, detail)
+
+
+def use_torch_allocator(enable: bool = True) -> None:
+    """Route the library's device allocations through PyTorch's caching allocator."""
+    global _hooks
+    import torch
+    L = load_library()
+    if not enable:
+        _check(L.pvg_set_allocator(None, None, None))
+        _hooks = None
+        return
+
+    def _alloc(nbytes, stream, _user):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream) if stream else None)
+        except Exception:
+            return 0
+
+    def _free(ptr, _user):
+        try:
+            torch.cuda.caching_allocator_delete(ptr)
+        except Exception:
+            pass
+
+    a, f = ALLOC_FN(_alloc), FREE_FN(_free)
+    _check(L.pvg_set_allocator(C.cast(a, C.c_void_p), C.cast(f, C.c_void_p), None))
+    _hooks = (a, f)
+
+
+def camera_struct(cam) -> CameraC:
+    """pvg_camera from any object with the fields of workloads.Camera."""
+    c = CameraC()
+    c.width, c.height = int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    w2c = np.asarray(cam.world_to_cam, dtype=np.float32).reshape(12)
+    for i in range(12):
+        c.world_to_cam[i] = float(w2c[i])
+    c.znear = float(getattr(cam, "znear", 0.0))
+    bg = getattr(cam, "bg", (0.0, 0.0, 0.0))
+    for i in range(3):
+        c.bg[i] = float(bg[i])
+    return c
+
+
+def _is_torch(x) -> bool:
+    return type(x).__module__.startswith("torch")
+
+
+class Scene:
+    """Owns a pvg_scene. Arrays may be numpy (host) or torch CUDA tensors (all one kind)."""
+
+    def __init__(self, mu, quat, scale, opacity, sh, tau, beta, vel, cycle: float = 0.2, sh_degree: int = 3,
+                 torch_allocator: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise PvgError(-6, "no CUDA device: this package has no CPU fallback")
+        self._L = load_library()
+        if torch_allocator and _hooks is None:
+            use_torch_allocator(True)
+        arrs = [mu, quat, scale, opacity, sh, tau, beta, vel]
+        shapes = [(3,), (4,), (3,), (), (16, 3), (), (), (3,)]
+        on_dev = all(_is_torch(a) and a.is_cuda for a in arrs)
+        n = int(arrs[0].shape[0])
+        keep = []
+        ptrs = []
+        for a, shp in zip(arrs, shapes):
+            if on_dev:
+                a = a.detach().to(torch.float32).contiguous()
+                assert tuple(a.shape) == (n,) + shp, (tuple(a.shape), shp)
+                ptrs.append(a.data_ptr())
+            else:
+                if _is_torch(a):
+                    a = a.detach().cpu().numpy()
+                a = np.ascontiguousarray(a, dtype=np.float32)
+                assert a.shape == (n,) + shp, (a.shape, shp)
+                ptrs.append(a.ctypes.data)
+            keep.append(a)
+        d = SceneDesc(n, *ptrs, float(cycle), int(sh_degree), 1 if on_dev else 0)
+        h = C.c_void_p()
+        _check(self._L.pvg_create_scene(C.byref(d), C.byref(h)))
+        self._h = h
+        self.n = n
+
+    @classmethod
+    def from_workload_scene(cls, sc, **kw) -> "Scene":
+        return cls(sc.mu, sc.quat, sc.scale, sc.opacity, sc.sh, sc.tau, sc.beta, sc.vel, sc.cycle, sc.sh_degree, **kw)
+
+    # -- the path ---------------------------------------------------------------------------
+    def render(self, cam, t: float, out: Optional[Tuple] = None):
+        """Frame at time t into torch CUDA tensors (rgb [3,H,W], depth [H,W], alpha [H,W])."""
+        import torch
+        c = cam if isinstance(cam, CameraC) else camera_struct(cam)
+        if out is None:
+            out = (torch.empty((3, c.height, c.width), dtype=torch.float32, device="cuda"),
+                   torch.empty((c.height, c.width), dtype=torch.float32, device="cuda"),
+                   torch.empty((c.height, c.width), dtype=torch.float32, device="cuda"))
+        _check(self._L.pvg_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
+        _check(self._L.pvg_render(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
+                                  out[2].data_ptr()))
+        return out
+
+    def render_host(self, cam, t: float, out: Optional[Tuple] = None):
+        """Frame at time t into HOST buffers (torch CPU tensors, pinned if allocated here)."""
+        import torch
+        c = cam if isinstance(cam, CameraC) else camera_struct(cam)
+        if out is None:
+            out = (torch.empty((3, c.height, c.width), dtype=torch.float32, pin_memory=True),
+                   torch.empty((c.height, c.width), dtype=torch.float32, pin_memory=True),
+                   torch.empty((c.height, c.width), dtype=torch.float32, pin_memory=True))
+        _check(self._L.pvg_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
+        _check(self._L.pvg_render_host(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
+                                       out[2].data_ptr()))
+        return out
+
+    # -- options / hooks ----------------------------------------------------------------------
+    def set_option(self, option: int, value: int) -> None:
+        _check(self._L.pvg_set_option(self._h, int(option), int(value)))
+
+    def stage_times_ms(self) -> Dict[str, float]:
+        ms = (C.c_float * NUM_STAGES)()
+        _check(self._L.pvg_stage_times_ms(self._h, ms))
+        return {STAGES[i]: float(ms[i]) for i in range(NUM_STAGES)}
+
+    def kernel_times_ms(self) -> List[Tuple[str, str, float]]:
+        cap = 1 << 16
+        names = (C.c_char_p * cap)()
+        stages = (C.c_int * cap)()
+        ms = (C.c_float * cap)()
+        cnt = self._L.pvg_kernel_times_ms(self._h, cap, names, stages, ms)
+        if cnt < 0:
+            _check(cnt)
+        return [(names[i].decode(), STAGES[stages[i]], float(ms[i])) for i in range(min(cnt, cap))]
+
+    def debug_info(self) -> DebugC:
+        d = DebugC()
+        _check(self._L.pvg_debug_view(self._h, C.byref(d)))
+        return d
+
+    def debug(self, fields: Optional[List[str]] = None) -> Dict[str, np.ndarray]:
+        """Host copies (numpy) of the last render's intermediates."""
+        d = self.debug_info()
+        n, M, tiles = int(d.n), int(d.num_instances), int(d.tiles_x) * int(d.tiles_y)
+        spec = {"record": (d.record, (n, 12), np.float32), "counts": (d.counts, (n,), np.uint32),
+                "visit_order": (d.visit_order, (n,), np.uint32), "offsets": (d.offsets, (n,), np.uint32),
+                "keys_unsorted": (d.keys_unsorted, (M,), np.uint64), "vals_unsorted": (d.vals_unsorted, (M,), np.uint32),
+                "keys_sorted": (d.keys_sorted, (M,), np.uint64), "vals_sorted": (d.vals_sorted, (M,), np.uint32),
+                "ranges": (d.ranges, (tiles, 2), np.uint32)}
+        out: Dict[str, np.ndarray] = {"M": M, "tiles_x": int(d.tiles_x), "tiles_y": int(d.tiles_y),
+                                      "sort_bits": (int(d.sort_begin_bit), int(d.sort_end_bit))}
+        for k, (ptr, shape, dt) in spec.items():
+            if fields is not None and k not in fields:
+                continue
+            if not ptr:
+                out[k] = None if int(np.prod(shape)) else np.zeros(shape, dtype=dt)
+                continue
+            a = np.empty(shape, dtype=dt)
+            _check(self._L.pvg_memcpy_d2h(a.ctypes.data, ptr, a.nbytes))
+            out[k] = a
+        return out
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            self._L.pvg_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def sort_pairs(keys, vals, begin_bit: int = 0, end_bit: int = 64):
+    """Onesweep LSD radix sort of torch CUDA tensors (keys int64 holding uint64 bit patterns,
+    vals int32 holding uint32). Returns new (keys, vals); inputs are clobbered."""
+    import torch
+    L = load_library()
+    assert keys.is_cuda and vals.is_cuda and keys.dtype == torch.int64 and vals.dtype == torch.int32
+    n = keys.numel()
+    ko, vo = torch.empty_like(keys), torch.empty_like(vals)
+    _check(L.pvg_sort_pairs(n, keys.data_ptr(), vals.data_ptr(), ko.data_ptr(), vo.data_ptr(), int(begin_bit),
+                            int(end_bit), torch.cuda.current_stream().cuda_stream))
+    return ko, vo

@@ -1,0 +1,99 @@
+// blend.cuh -- stage a5: per-tile front-to-back alpha compositing
+//   C = sum_i T_i alpha_i c_i,  T_i = prod_{j<i} (1 - alpha_j)      (Eq. 3)
+//   alpha = min(0.99, o~ * exp(-1/2 d^T Sigma'^-1 d))
+//   depth = sum T alpha z / sum T alpha, O = sum T alpha
+// with the 1/255 alpha cutoff, the 0.99 clamp and the T < 1e-4 stop (S9, S10).
+// FP32-pipe bound: no tensor cores (not a dense contraction).
+#pragma once
+
+#include "common.cuh"
+
+namespace pvg {
+
+constexpr int BLEND_THREADS = PVG_TILE_PIXELS;
+constexpr int BLEND_BATCH = 256;
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// One CTA per 16x16 tile, one thread per pixel. The tile's slice of the sorted instance
+// list is consumed in batches: each thread gathers one 48 B record through the sorted
+// index list into shared memory (conic pre-scaled by -log2(e)/2 so the inner loop feeds
+// ex2 directly), then every pixel walks the batch. The tile retires as soon as every
+// pixel's transmittance has dropped below 1e-4.
+__global__ void __launch_bounds__(BLEND_THREADS)
+blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
+             const uint32_t* __restrict__ vals, const float4* __restrict__ record,
+             float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha) {
+  __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
+  __shared__ float4 s_col[BLEND_BATCH];   // c', o~, r, g
+  __shared__ float2 s_bz[BLEND_BATCH];    // b, z
+
+  const uint32_t tid = threadIdx.x;
+  const uint32_t tile = blockIdx.x;
+  const uint32_t tx = tile % P.tiles_x, ty = tile / P.tiles_x;
+  const uint32_t px = tx * PVG_TILE + (tid & 15u), py = ty * PVG_TILE + (tid >> 4);
+  const bool inside = px < (uint32_t)P.width && py < (uint32_t)P.height;
+  const float pxf = (float)px + 0.5f, pyf = (float)py + 0.5f;   // S14
+  const uint2 range = ranges[tile];
+
+  float T = 1.0f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;
+  bool done = !inside;
+
+  for (uint32_t base = range.x; base < range.y; base += BLEND_BATCH) {
+    // all pixels of the tile saturated? (also fences the previous batch's smem reads)
+    if (__syncthreads_count(!done) == 0) break;
+    const uint32_t idx = base + tid;
+    if (idx < range.y) {
+      const uint32_t g = __ldg(vals + idx);
+      const float4 r0 = __ldg(record + 3 * (size_t)g);
+      const float4 r1 = __ldg(record + 3 * (size_t)g + 1);
+      const float4 r2 = __ldg(record + 3 * (size_t)g + 2);
+      const float kh = -0.72134752044448170f;  // -log2(e)/2
+      s_geo[tid] = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
+      s_col[tid] = make_float4(kh * r1.z, r0.w, r2.x, r2.y);
+      s_bz[tid] = make_float2(r2.z, r0.z);
+    }
+    __syncthreads();
+    const uint32_t nb = min((uint32_t)BLEND_BATCH, range.y - base);
+    if (!done) {
+      for (uint32_t j = 0; j < nb; ++j) {
+        const float4 ge = s_geo[j];
+        const float4 co = s_col[j];
+        const float dx = ge.x - pxf, dy = ge.y - pyf;
+        // w = log2(e) * (-1/2 (a dx^2 + c dy^2) - b dx dy)
+        float w = fmaf(dx, fmaf(ge.z, dx, ge.w * dy), (co.x * dy) * dy);
+        w = fminf(w, 0.0f);                       // S16': rounding guard (exact w <= 0)
+        const float alpha = fminf(PVG_ALPHA_MAX, co.y * ex2_approx(w));
+        if (alpha < PVG_ALPHA_MIN) continue;
+        const float Tn = T * (1.0f - alpha);
+        if (Tn < PVG_T_STOP) { done = true; break; }   // S10: not composited
+        const float wgt = alpha * T;
+        const float2 bz = s_bz[j];
+        Cr = fmaf(co.z, wgt, Cr);
+        Cg = fmaf(co.w, wgt, Cg);
+        Cb = fmaf(bz.x, wgt, Cb);
+        D = fmaf(bz.y, wgt, D);
+        T = Tn;
+      }
+    }
+  }
+
+  if (inside) {
+    const size_t HW = (size_t)P.width * P.height;
+    const size_t pi = (size_t)py * P.width + px;
+    const float A = 1.0f - T;
+    if (out_rgb) {
+      out_rgb[pi] = fmaf(T, P.bg[0], Cr);
+      out_rgb[HW + pi] = fmaf(T, P.bg[1], Cg);
+      out_rgb[2 * HW + pi] = fmaf(T, P.bg[2], Cb);
+    }
+    if (out_depth) out_depth[pi] = A > 0.f ? D / A : 0.f;
+    if (out_alpha) out_alpha[pi] = A;
+  }
+}
+
+}  // namespace pvg

@@ -1,0 +1,73 @@
+// common.cuh -- shared device/host definitions of the PVG CUDA path (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define PVG_TILE 16
+#define PVG_TILE_PIXELS 256
+
+// contract constants: S6, S9
+#define PVG_ALPHA_MIN 0.003921569f /* fp32(1/255) */
+#define PVG_ALPHA_MAX 0.99f
+#define PVG_T_STOP 1e-4f
+#define PVG_DILATE 0.3f
+#define PVG_ZNEAR_DEFAULT 0.2f
+
+namespace pvg {
+
+// Per-frame constants, passed by value as a __grid_constant__ kernel parameter.
+struct FrameParams {
+  float R[9];       // world->camera rotation, row-major
+  float T[3];       // world->camera translation
+  float campos[3];  // camera centre in world coordinates (-R^T T)
+  float fx, fy, cx, cy;
+  float limx, limy;  // 1.3 * half-FoV tangents (Jacobian guard)
+  float znear;
+  float t;
+  float two_over_l;   // 2 / l           (sinpi argument scale)
+  float l_over_2pi;   // l / (2 pi)
+  int linear;         // l == +INF: mu~ = mu + (t - tau) v
+  int sh_degree;
+  int width, height, tiles_x, tiles_y;
+  float bg[3];
+};
+
+__device__ __forceinline__ uint32_t lane_id() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%laneid;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t lanemask_lt() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%lanemask_lt;" : "=r"(r));
+  return r;
+}
+
+// 64-bit status words of the decoupled look-back (flag in the top 2 bits, value
+// below): one aligned 64-bit access carries flag and payload together, so relaxed
+// gpu-scope accesses are sufficient.
+__device__ __forceinline__ void st_relaxed_u64(uint64_t* p, uint64_t v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ uint64_t ld_relaxed_u64(const uint64_t* p) {
+  uint64_t v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+constexpr uint64_t LB_FLAG_AGG = 1ull << 62;
+constexpr uint64_t LB_FLAG_PREFIX = 2ull << 62;
+constexpr uint64_t LB_FLAG_MASK = 3ull << 62;
+constexpr uint64_t LB_VALUE_MASK = ~LB_FLAG_MASK;
+
+// streaming (read-once) 128-bit load that does not allocate in L1
+__device__ __forceinline__ float4 ldg_stream_f4(const float4* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+               : "l"(p));
+  return v;
+}
+
+}  // namespace pvg

@@ -1,0 +1,597 @@
+// pvg_api.cu -- host side of the C ABI declared in include/pvg.h.
+// Orchestrates the five stages on one CUDA stream; every step of the path runs in the
+// kernels of this directory. No CPU fallback: CUDA errors surface as PVG_ERR_CUDA.
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/pvg.h"
+#include "blend.cuh"
+#include "common.cuh"
+#include "onesweep.cuh"
+#include "preprocess.cuh"
+#include "ranges.cuh"
+#include "scan_dup.cuh"
+
+using namespace pvg;
+
+namespace {
+
+thread_local char g_cuda_err[512] = "";
+pvg_alloc_fn g_alloc = nullptr;
+pvg_free_fn g_free = nullptr;
+void* g_alloc_user = nullptr;
+
+#define CU(expr)                                                                              \
+  do {                                                                                        \
+    cudaError_t e_ = (expr);                                                                  \
+    if (e_ != cudaSuccess) {                                                                  \
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "%s:%d %s -> %s", __FILE__, __LINE__, #expr,   \
+               cudaGetErrorString(e_));                                                       \
+      return PVG_ERR_CUDA;                                                                    \
+    }                                                                                         \
+  } while (0)
+
+#define TRY(expr)            \
+  do {                       \
+    int rc_ = (expr);        \
+    if (rc_ != PVG_OK) return rc_; \
+  } while (0)
+
+void* dev_alloc(size_t bytes, cudaStream_t st) {
+  if (bytes == 0) bytes = 256;
+  if (g_alloc) return g_alloc(bytes, (void*)st, g_alloc_user);
+  void* p = nullptr;
+  if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  return p;
+}
+void dev_free(void* p) {
+  if (!p) return;
+  if (g_free) g_free(p, g_alloc_user);
+  else cudaFree(p);
+}
+
+// growable device buffer
+struct Buf {
+  void* p = nullptr;
+  size_t cap = 0;
+  int reserve(size_t bytes, cudaStream_t st, double headroom = 1.0) {
+    if (bytes <= cap) return PVG_OK;
+    dev_free(p);
+    p = nullptr;
+    cap = 0;
+    size_t want = (size_t)((double)bytes * headroom);
+    want = (want + 255) & ~(size_t)255;
+    p = dev_alloc(want, st);
+    if (!p && want > bytes) { want = (bytes + 255) & ~(size_t)255; p = dev_alloc(want, st); }
+    if (!p) return PVG_ERR_OOM;
+    cap = want;
+    return PVG_OK;
+  }
+  void release() { dev_free(p); p = nullptr; cap = 0; }
+  template <class T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+struct KernelRec {
+  const char* name;
+  int stage;
+  cudaEvent_t e0, e1;
+};
+
+constexpr int OS_THREADS = 384;
+constexpr int OS_ITEMS = 16;
+constexpr int OS_TILE = OS_THREADS * OS_ITEMS;
+using OsSmem = OnesweepSmem<OS_THREADS, OS_ITEMS>;
+
+// scratch of one sort call
+struct SortScratch {
+  Buf hist;      // [passes][256] u32
+  Buf lookback;  // [passes][tiles][256] u64
+  Buf tickets;   // [passes] u32
+};
+
+struct Timer {
+  bool enabled = true;
+  bool accumulate = false;  // keep the records of every frame until they are read
+  std::vector<KernelRec> recs;     // launches of the current frame
+  std::vector<cudaEvent_t> pool;   // reusable events
+  size_t used = 0;
+  int get(cudaEvent_t* e) {
+    if (used == pool.size()) {
+      cudaEvent_t ev;
+      CU(cudaEventCreate(&ev));
+      pool.push_back(ev);
+    }
+    *e = pool[used++];
+    return PVG_OK;
+  }
+  void reset() { recs.clear(); used = 0; }
+  int begin(const char* name, int stage, cudaStream_t st) {
+    if (!enabled) return PVG_OK;
+    KernelRec r{name, stage, nullptr, nullptr};
+    TRY(get(&r.e0));
+    TRY(get(&r.e1));
+    CU(cudaEventRecord(r.e0, st));
+    recs.push_back(r);
+    return PVG_OK;
+  }
+  int end(cudaStream_t st) {
+    if (!enabled) return PVG_OK;
+    CU(cudaEventRecord(recs.back().e1, st));
+    return PVG_OK;
+  }
+  void destroy() {
+    for (cudaEvent_t e : pool) cudaEventDestroy(e);
+    pool.clear();
+    recs.clear();
+    used = 0;
+  }
+};
+
+int onesweep_configure() {
+  static bool done = false;
+  if (done) return PVG_OK;
+  CU(cudaFuncSetAttribute(onesweep_pass_kernel<OS_THREADS, OS_ITEMS>,
+                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OsSmem)));
+  done = true;
+  return PVG_OK;
+}
+
+// Stable LSD sort of n pairs on key bits [begin_bit, end_bit). Buffers ping-pong; *result
+// tells which side (0: a, 1: b) holds the sorted list.
+int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, int begin_bit,
+                 int end_bit, cudaStream_t st, SortScratch& sc, Timer* tm, int stage, int* result) {
+  *result = 0;
+  if (n == 0 || end_bit <= begin_bit) return PVG_OK;
+  TRY(onesweep_configure());
+  const SortPlan plan = make_sort_plan(begin_bit, end_bit);
+  const uint64_t tiles = (n + OS_TILE - 1) / OS_TILE;
+  TRY(sc.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
+  TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
+  TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, st, 1.25));
+  CU(cudaMemsetAsync(sc.hist.p, 0, (size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
+  CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, st));
+  CU(cudaMemsetAsync(sc.lookback.p, 0, (size_t)plan.num_passes * tiles * OS_RADIX * 8, st));
+
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const uint64_t hist_chunks = (n + (uint64_t)HIST_THREADS * HIST_ITEMS - 1) / ((uint64_t)HIST_THREADS * HIST_ITEMS);
+  const unsigned hist_grid = (unsigned)std::min<uint64_t>(hist_chunks, (uint64_t)sms * 4);
+  if (tm) TRY(tm->begin("onesweep_histogram", stage, st));
+  onesweep_histogram_kernel<<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
+  if (tm) TRY(tm->end(st));
+  if (tm) TRY(tm->begin("onesweep_scan_hist", stage, st));
+  onesweep_scan_hist_kernel<<<plan.num_passes, OS_RADIX, 0, st>>>(sc.hist.as<uint32_t>());
+  if (tm) TRY(tm->end(st));
+
+  uint64_t* kin = ka; uint32_t* vin = va; uint64_t* kout = kb; uint32_t* vout = vb;
+  for (int p = 0; p < plan.num_passes; ++p) {
+    if (tm) TRY(tm->begin("onesweep_pass", stage, st));
+    onesweep_pass_kernel<OS_THREADS, OS_ITEMS><<<(unsigned)tiles, OS_THREADS, sizeof(OsSmem), st>>>(
+        kin, vin, kout, vout, n, plan.shift[p], plan.bits[p], sc.hist.as<uint32_t>() + p * OS_RADIX,
+        sc.lookback.as<uint64_t>() + (size_t)p * tiles * OS_RADIX, sc.tickets.as<uint32_t>() + p);
+    if (tm) TRY(tm->end(st));
+    std::swap(kin, kout);
+    std::swap(vin, vout);
+  }
+  CU(cudaGetLastError());
+  *result = plan.num_passes & 1;
+  return PVG_OK;
+}
+
+}  // namespace
+
+struct pvg_scene {
+  uint32_t n = 0;
+  float cycle = 0.2f;
+  int sh_degree = 3;
+  cudaStream_t stream = nullptr;
+  // options
+  int presort = 1, keep_unsorted = 0;
+  // model (SoA)
+  Buf A0, A1, A2, A3, SH;
+  // per-Gaussian workspace
+  Buf record, tileinfo, counts, offsets, dkeys[2], dvals[2], scan_status, small;  // small: ticket u32 @0, total u64 @8
+  // per-instance workspace
+  Buf keys[2], vals[2], keys_unsorted, vals_unsorted;
+  Buf ranges;
+  Buf img;  // render_host device images
+  SortScratch sort_n, sort_m;
+  uint64_t* h_total = nullptr;  // pinned
+  Timer timer;
+  // last frame
+  uint64_t M = 0;
+  int sorted_side = 0, visit_side = 0;
+  uint32_t tiles_x = 0, tiles_y = 0;
+  int sort_begin = 0, sort_end = 0;
+  bool rendered = false;
+};
+
+namespace {
+
+int ceil_log2(uint32_t v) {
+  int b = 0;
+  while ((1ull << b) < v) ++b;
+  return b;
+}
+
+void release_all(pvg_scene* s) {
+  Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
+                 &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
+                 &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted,
+                 &s->ranges, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
+  for (Buf* b : bufs) b->release();
+  if (s->h_total) cudaFreeHost(s->h_total);
+  s->h_total = nullptr;
+  s->timer.destroy();
+}
+
+int upload(Buf& dst, const float* src, size_t bytes, bool on_device, cudaStream_t st) {
+  TRY(dst.reserve(bytes, st));
+  CU(cudaMemcpyAsync(dst.p, src, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+  return PVG_OK;
+}
+
+int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
+  int ndev = 0;
+  CU(cudaGetDeviceCount(&ndev));
+  if (ndev <= 0) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+    return PVG_ERR_CUDA;
+  }
+  const size_t n = (size_t)d->n;
+  s->n = (uint32_t)n;
+  s->cycle = d->cycle;
+  s->sh_degree = d->sh_degree;
+  cudaStream_t st = s->stream;
+  const bool dev = d->pointers_on_device != 0;
+  Buf t_mu, t_quat, t_scale, t_op, t_sh, t_tau, t_beta, t_vel;
+  int rc = PVG_OK;
+  auto up = [&](Buf& b, const float* src, size_t floats) {
+    if (rc == PVG_OK) rc = upload(b, src, floats * n * 4, dev, st);
+  };
+  up(t_mu, d->mu, 3); up(t_quat, d->quat, 4); up(t_scale, d->scale, 3); up(t_op, d->opacity, 1);
+  up(t_sh, d->sh, 48); up(t_tau, d->tau, 1); up(t_beta, d->beta, 1); up(t_vel, d->vel, 3);
+  auto rs = [&](Buf& b, size_t bytes) { if (rc == PVG_OK) rc = b.reserve(bytes, st); };
+  rs(s->A0, n * 16); rs(s->A1, n * 16); rs(s->A2, n * 16); rs(s->A3, n * 16); rs(s->SH, n * 192);
+  rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4);
+  rs(s->dkeys[0], n * 8); rs(s->dkeys[1], n * 8); rs(s->dvals[0], n * 4); rs(s->dvals[1], n * 4);
+  rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 8); rs(s->small, 256);
+  if (rc == PVG_OK) {
+    relayout_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
+        (uint32_t)n, t_mu.as<float>(), t_quat.as<float>(), t_scale.as<float>(), t_op.as<float>(), t_sh.as<float>(),
+        t_tau.as<float>(), t_beta.as<float>(), t_vel.as<float>(), s->A0.as<float4>(), s->A1.as<float4>(),
+        s->A2.as<float4>(), s->A3.as<float4>(), s->SH.as<float4>());
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "relayout: %s", cudaGetErrorString(e));
+      rc = PVG_ERR_CUDA;
+    }
+  }
+  Buf* tmp[] = {&t_mu, &t_quat, &t_scale, &t_op, &t_sh, &t_tau, &t_beta, &t_vel};
+  for (Buf* b : tmp) b->release();
+  if (rc != PVG_OK) return rc;
+  CU(cudaMallocHost((void**)&s->h_total, 64));
+  return PVG_OK;
+}
+
+int fill_frame(const pvg_scene* s, const pvg_camera* cam, float t, FrameParams* P) {
+  if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
+  if (!(cam->fx > 0.f) || !(cam->fy > 0.f) || !std::isfinite(cam->fx) || !std::isfinite(cam->fy) ||
+      !std::isfinite(cam->cx) || !std::isfinite(cam->cy))
+    return PVG_ERR_BAD_CAMERA;
+  for (int i = 0; i < 12; ++i)
+    if (!std::isfinite(cam->world_to_cam[i])) return PVG_ERR_BAD_CAMERA;
+  const float* E = cam->world_to_cam;
+  for (int r = 0; r < 3; ++r) {
+    for (int c = 0; c < 3; ++c) P->R[3 * r + c] = E[4 * r + c];
+    P->T[r] = E[4 * r + 3];
+  }
+  for (int j = 0; j < 3; ++j)
+    P->campos[j] = (float)-((double)E[j] * E[3] + (double)E[4 + j] * E[7] + (double)E[8 + j] * E[11]);
+  P->fx = cam->fx; P->fy = cam->fy; P->cx = cam->cx; P->cy = cam->cy;
+  P->limx = (float)(1.3 * cam->width / (2.0 * (double)cam->fx));
+  P->limy = (float)(1.3 * cam->height / (2.0 * (double)cam->fy));
+  P->znear = cam->znear > 0.f ? cam->znear : PVG_ZNEAR_DEFAULT;
+  P->t = t;
+  P->linear = std::isinf(s->cycle) ? 1 : 0;
+  P->two_over_l = P->linear ? 0.f : (float)(2.0 / (double)s->cycle);
+  P->l_over_2pi = P->linear ? 0.f : (float)((double)s->cycle / (2.0 * 3.14159265358979323846));
+  P->sh_degree = s->sh_degree;
+  P->width = cam->width; P->height = cam->height;
+  P->tiles_x = (cam->width + PVG_TILE - 1) / PVG_TILE;
+  P->tiles_y = (cam->height + PVG_TILE - 1) / PVG_TILE;
+  for (int j = 0; j < 3; ++j) P->bg[j] = cam->bg[j];
+  return PVG_OK;
+}
+
+int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, float* out_depth, float* out_alpha) {
+  FrameParams P;
+  TRY(fill_frame(s, cam, t, &P));
+  cudaStream_t st = s->stream;
+  Timer& tm = s->timer;
+  if (!tm.accumulate) tm.reset();
+  const uint32_t n = s->n;
+  const uint32_t tiles = (uint32_t)P.tiles_x * (uint32_t)P.tiles_y;
+  s->tiles_x = P.tiles_x; s->tiles_y = P.tiles_y;
+  s->rendered = false;
+  TRY(s->ranges.reserve((size_t)tiles * 8, st));
+
+  // a1 preprocess
+  uint64_t* dk = s->presort ? s->dkeys[0].as<uint64_t>() : nullptr;
+  uint32_t* dv = s->presort ? s->dvals[0].as<uint32_t>() : nullptr;
+  TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
+  preprocess_kernel<<<(n + 255) / 256, 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
+                                                      s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
+                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv);
+  TRY(tm.end(st));
+
+  // a3 (n-key part): depth order of the Gaussians
+  const uint32_t* visit = nullptr;
+  s->visit_side = 0;
+  if (s->presort) {
+    int side = 0;
+    TRY(run_onesweep(n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
+                     s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side));
+    s->visit_side = side;
+    visit = s->dvals[side].as<uint32_t>();
+  }
+
+  // a2 scan
+  const uint32_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 8, st));
+  CU(cudaMemsetAsync(s->small.p, 0, 64, st));
+  uint32_t* ticket = s->small.as<uint32_t>();
+  uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
+  TRY(tm.begin("scan_counts", PVG_STAGE_DUPLICATE, st));
+  scan_counts_kernel<<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), visit, s->offsets.as<uint32_t>(),
+                                                          total, s->scan_status.as<uint64_t>(), ticket);
+  TRY(tm.end(st));
+  CU(cudaMemcpyAsync(s->h_total, total, 8, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));  // the one host read-back: M sizes the instance buffers
+  const uint64_t M = *s->h_total;
+  if (M >= (1ull << 32)) return PVG_ERR_INSTANCE_OVERFLOW;
+  s->M = M;
+
+  const int tile_bits = std::max(1, ceil_log2(tiles));
+  s->sort_begin = s->presort ? 32 : 0;
+  s->sort_end = 32 + tile_bits;
+  s->sorted_side = 0;
+  if (M > 0) {
+    for (int k = 0; k < 2; ++k) {
+      TRY(s->keys[k].reserve((size_t)M * 8, st, 1.125));
+      TRY(s->vals[k].reserve((size_t)M * 4, st, 1.125));
+    }
+    // a2 emit
+    TRY(tm.begin("duplicate", PVG_STAGE_DUPLICATE, st));
+    duplicate_kernel<<<(unsigned)((M + DUP_CHUNK - 1) / DUP_CHUNK), DUP_THREADS, 0, st>>>(
+        n, M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x,
+        s->keys[0].as<uint64_t>(), s->vals[0].as<uint32_t>());
+    TRY(tm.end(st));
+    if (s->keep_unsorted) {
+      TRY(s->keys_unsorted.reserve((size_t)M * 8, st));
+      TRY(s->vals_unsorted.reserve((size_t)M * 4, st));
+      CU(cudaMemcpyAsync(s->keys_unsorted.p, s->keys[0].p, (size_t)M * 8, cudaMemcpyDeviceToDevice, st));
+      CU(cudaMemcpyAsync(s->vals_unsorted.p, s->vals[0].p, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    // a3 (M-instance part)
+    int side = 0;
+    TRY(run_onesweep(M, s->keys[0].as<uint64_t>(), s->vals[0].as<uint32_t>(), s->keys[1].as<uint64_t>(),
+                     s->vals[1].as<uint32_t>(), s->sort_begin, s->sort_end, st, s->sort_m, &tm, PVG_STAGE_SORT, &side));
+    s->sorted_side = side;
+    // a4 ranges
+    TRY(tm.begin("tile_ranges", PVG_STAGE_RANGES, st));
+    tile_ranges_kernel<<<(unsigned)((M + 255) / 256), 256, 0, st>>>(s->keys[side].as<uint64_t>(), M, tiles,
+                                                                    s->ranges.as<uint2>());
+    TRY(tm.end(st));
+  } else {
+    CU(cudaMemsetAsync(s->ranges.p, 0, (size_t)tiles * 8, st));
+  }
+
+  // a5 blend
+  TRY(tm.begin("blend", PVG_STAGE_BLEND, st));
+  blend_kernel<<<tiles, BLEND_THREADS, 0, st>>>(P, s->ranges.as<uint2>(), s->vals[s->sorted_side].as<uint32_t>(),
+                                                s->record.as<float4>(), out_rgb, out_depth, out_alpha);
+  TRY(tm.end(st));
+  CU(cudaGetLastError());
+  s->rendered = true;
+  return PVG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pvg_version(void) { return 100; }
+
+const char* pvg_strerror(int code) {
+  switch (code) {
+    case PVG_OK: return "ok";
+    case PVG_ERR_NULL: return "null pointer argument";
+    case PVG_ERR_BAD_DESC: return "bad scene descriptor";
+    case PVG_ERR_BAD_CAMERA: return "bad camera";
+    case PVG_ERR_OOM: return "device out of memory";
+    case PVG_ERR_INSTANCE_OVERFLOW: return "tile instance count overflows 32 bits";
+    case PVG_ERR_CUDA: return "CUDA error";
+    case PVG_ERR_BAD_OPTION: return "bad option";
+    default: return "unknown error";
+  }
+}
+
+const char* pvg_last_cuda_error(void) { return g_cuda_err; }
+
+int pvg_set_allocator(pvg_alloc_fn alloc_fn, pvg_free_fn free_fn, void* user) {
+  if ((alloc_fn == nullptr) != (free_fn == nullptr)) return PVG_ERR_NULL;
+  g_alloc = alloc_fn;
+  g_free = free_fn;
+  g_alloc_user = user;
+  return PVG_OK;
+}
+
+int pvg_set_stream(pvg_scene* scene, void* cuda_stream) {
+  if (!scene) return PVG_ERR_NULL;
+  scene->stream = (cudaStream_t)cuda_stream;
+  return PVG_OK;
+}
+
+int pvg_create_scene(const pvg_scene_desc* d, pvg_scene** out) {
+  if (!d || !out) return PVG_ERR_NULL;
+  *out = nullptr;
+  if (!d->mu || !d->quat || !d->scale || !d->opacity || !d->sh || !d->tau || !d->beta || !d->vel) return PVG_ERR_NULL;
+  if (d->n == 0 || d->n >= (1ull << 31)) return PVG_ERR_BAD_DESC;
+  if (!(d->cycle > 0.f)) return PVG_ERR_BAD_DESC;  // also rejects NaN
+  if (d->sh_degree < 0 || d->sh_degree > 3) return PVG_ERR_BAD_DESC;
+  pvg_scene* s = new (std::nothrow) pvg_scene();
+  if (!s) return PVG_ERR_OOM;
+  const int rc = create_impl(d, s);
+  if (rc != PVG_OK) {
+    release_all(s);
+    delete s;
+    return rc;
+  }
+  *out = s;
+  return PVG_OK;
+}
+
+int pvg_destroy(pvg_scene* scene) {
+  if (!scene) return PVG_ERR_NULL;
+  cudaStreamSynchronize(scene->stream);
+  release_all(scene);
+  delete scene;
+  return PVG_OK;
+}
+
+int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
+  if (!scene) return PVG_ERR_NULL;
+  switch (option) {
+    case PVG_OPT_PRESORT_DEPTH: scene->presort = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_KEEP_UNSORTED: scene->keep_unsorted = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_KERNEL_EVENTS:
+      scene->timer.enabled = value != 0;
+      scene->timer.accumulate = value == 2;
+      scene->timer.reset();
+      return PVG_OK;
+    default: return PVG_ERR_BAD_OPTION;
+  }
+}
+
+int pvg_render(pvg_scene* scene, const pvg_camera* cam, float t, float* out_rgb, float* out_depth, float* out_alpha) {
+  if (!scene || !cam) return PVG_ERR_NULL;
+  if (!std::isfinite(t)) return PVG_ERR_BAD_CAMERA;
+  return render_impl(scene, cam, t, out_rgb, out_depth, out_alpha);
+}
+
+int pvg_render_host(pvg_scene* scene, const pvg_camera* cam, float t, float* host_rgb, float* host_depth,
+                    float* host_alpha) {
+  if (!scene || !cam) return PVG_ERR_NULL;
+  if (!std::isfinite(t)) return PVG_ERR_BAD_CAMERA;
+  if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
+  const size_t HW = (size_t)cam->width * cam->height;
+  cudaStream_t st = scene->stream;
+  TRY(scene->img.reserve(HW * 5 * 4, st));
+  float* d_rgb = scene->img.as<float>();
+  float* d_depth = d_rgb + 3 * HW;
+  float* d_alpha = d_rgb + 4 * HW;
+  TRY(render_impl(scene, cam, t, host_rgb ? d_rgb : nullptr, host_depth ? d_depth : nullptr,
+                  host_alpha ? d_alpha : nullptr));
+  if (host_rgb) CU(cudaMemcpyAsync(host_rgb, d_rgb, HW * 12, cudaMemcpyDeviceToHost, st));
+  if (host_depth) CU(cudaMemcpyAsync(host_depth, d_depth, HW * 4, cudaMemcpyDeviceToHost, st));
+  if (host_alpha) CU(cudaMemcpyAsync(host_alpha, d_alpha, HW * 4, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  return PVG_OK;
+}
+
+int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
+  if (!s || !out) return PVG_ERR_NULL;
+  memset(out, 0, sizeof(*out));
+  if (!s->rendered) return PVG_OK;
+  out->n = s->n;
+  out->num_instances = s->M;
+  out->tiles_x = s->tiles_x;
+  out->tiles_y = s->tiles_y;
+  out->sort_begin_bit = (uint32_t)s->sort_begin;
+  out->sort_end_bit = (uint32_t)s->sort_end;
+  out->record = s->record.as<float>();
+  out->counts = s->counts.as<uint32_t>();
+  out->visit_order = s->presort ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
+  out->offsets = s->offsets.as<uint32_t>();
+  if (s->keep_unsorted && s->M) {
+    out->keys_unsorted = s->keys_unsorted.as<uint64_t>();
+    out->vals_unsorted = s->vals_unsorted.as<uint32_t>();
+  }
+  if (s->M) {
+    out->keys_sorted = s->keys[s->sorted_side].as<uint64_t>();
+    out->vals_sorted = s->vals[s->sorted_side].as<uint32_t>();
+  }
+  out->ranges = s->ranges.as<uint32_t>();
+  return PVG_OK;
+}
+
+int pvg_kernel_times_ms(pvg_scene* s, int cap, const char** names, int* stages, float* ms) {
+  if (!s) return PVG_ERR_NULL;
+  if (!s->rendered || !s->timer.enabled) return 0;
+  CU(cudaStreamSynchronize(s->stream));
+  const int cnt = (int)s->timer.recs.size();
+  for (int i = 0; i < cnt && i < cap; ++i) {
+    const KernelRec& r = s->timer.recs[i];
+    float v = 0.f;
+    CU(cudaEventElapsedTime(&v, r.e0, r.e1));
+    if (names) names[i] = r.name;
+    if (stages) stages[i] = r.stage;
+    if (ms) ms[i] = v;
+  }
+  if (s->timer.accumulate) s->timer.reset();
+  return cnt;
+}
+
+int pvg_stage_times_ms(pvg_scene* s, float ms[PVG_NUM_STAGES]) {
+  if (!s || !ms) return PVG_ERR_NULL;
+  for (int k = 0; k < PVG_NUM_STAGES; ++k) ms[k] = 0.f;
+  if (!s->rendered || !s->timer.enabled) return PVG_OK;
+  CU(cudaStreamSynchronize(s->stream));
+  // a stage runs from its first launch to its last one's end (includes memsets and the M read-back)
+  for (int k = 0; k < PVG_NUM_STAGES; ++k) {
+    const KernelRec *first = nullptr, *last = nullptr;
+    for (const KernelRec& r : s->timer.recs)
+      if (r.stage == k) { if (!first) first = &r; last = &r; }
+    if (first) CU(cudaEventElapsedTime(&ms[k], first->e0, last->e1));
+  }
+  return PVG_OK;
+}
+
+int pvg_memcpy_d2h(void* host_dst, const void* device_src, size_t bytes) {
+  if (bytes && (!host_dst || !device_src)) return PVG_ERR_NULL;
+  if (bytes) CU(cudaMemcpy(host_dst, device_src, bytes, cudaMemcpyDeviceToHost));
+  return PVG_OK;
+}
+
+int pvg_sort_pairs(uint64_t n, uint64_t* keys_in, uint32_t* vals_in, uint64_t* keys_out, uint32_t* vals_out,
+                   int begin_bit, int end_bit, void* cuda_stream) {
+  if (n && (!keys_in || !vals_in || !keys_out || !vals_out)) return PVG_ERR_NULL;
+  if (begin_bit < 0 || end_bit > 64 || begin_bit > end_bit) return PVG_ERR_BAD_OPTION;
+  if (n >= (1ull << 32)) return PVG_ERR_INSTANCE_OVERFLOW;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  SortScratch sc;
+  int side = 0;
+  int rc = run_onesweep(n, keys_in, vals_in, keys_out, vals_out, begin_bit, end_bit, st, sc, nullptr, 0, &side);
+  if (rc == PVG_OK && n && side == 0) {  // result landed in the input buffers
+    cudaError_t e = cudaMemcpyAsync(keys_out, keys_in, n * 8, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(vals_out, vals_in, n * 4, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof(g_cuda_err), "sort copy: %s", cudaGetErrorString(e)); rc = PVG_ERR_CUDA; }
+  }
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (rc == PVG_OK && e != cudaSuccess) { snprintf(g_cuda_err, sizeof(g_cuda_err), "sort: %s", cudaGetErrorString(e)); rc = PVG_ERR_CUDA; }
+  sc.hist.release(); sc.lookback.release(); sc.tickets.release();
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,138 @@
+"""Parity protocol between the CUDA path (through the C ABI binding) and the CPU oracle.
+
+Three comparisons per frame:
+  (P) GPU per-Gaussian record vs Oracle-P (double), with fragile points listed;
+  (I) bit-exact integer chain: the integer oracle fed the GPU's own fp32 record vs the GPU's
+      counts, offsets, unsorted keys, sorted keys/values and tile ranges;
+  (R) GPU images vs Oracle-R fed the GPU record (isolates stages 2-5), and vs Oracle-R fed
+      Oracle-P's record (end to end, nothing shared), both with the fragile budget.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle
+from oracle import SLOTS
+
+TOL_RGB = 2e-4      # north_star: max-abs per colour channel
+TOL_DEPTH_REL = 1e-3
+
+
+def check_record(gpu_rec: np.ndarray, wide: np.ndarray, cam, scene):
+    """(P). Returns stats; raises AssertionError on a non-fragile mismatch."""
+    n = gpu_rec.shape[0]
+    width, height = int(cam.width), int(cam.height)
+    znear = float(cam.znear) if cam.znear > 0 else 0.2
+    o_valid = wide[:, SLOTS["cull"]] == 0
+    g_valid = gpu_rec[:, 3] > 0
+    # cull-fragile: o~*255, z/znear within 1e-5 of 1, or the tile rectangle within 1e-3 px of flipping empty
+    op, z = wide[:, SLOTS["op"]], wide[:, 6]
+    mx, my, hx, hy = wide[:, 19], wide[:, 20], wide[:, 21], wide[:, 22]
+    TX, TY = (width + 15) // 16, (height + 15) // 16
+    with np.errstate(invalid="ignore"):
+        edge = np.stack([(mx - hx) / 16, (mx + hx) / 16, (my - hy) / 16, (my + hy) / 16], 1)
+        rect_frag = np.any(np.abs(edge - np.round(edge)) < 1e-4, axis=1)
+        cull_frag = (np.abs(op * 255 - 1) < 1e-5) | (np.abs(z / znear - 1) < 1e-5) | rect_frag
+    mism = o_valid != g_valid
+    bad = mism & ~cull_frag
+    assert not bad.any(), f"cull mismatch on non-fragile Gaussians: {np.nonzero(bad)[0][:10]}"
+    both = o_valid & g_valid
+    g = gpu_rec[both].astype(np.float64)
+    w = wide[both]
+    stats = dict(n=n, survivors_gpu=int(g_valid.sum()), survivors_oracle=int(o_valid.sum()),
+                 cull_mismatch_fragile=int(mism.sum()))
+    if not both.any():
+        return stats
+    cov = w[:, SLOTS["cov"]]
+    kappa = cov[:, 0] * cov[:, 2] / (cov[:, 0] * cov[:, 2] - cov[:, 1] ** 2)   # conditioning of the conic
+    err = {}
+    err["mean_px"] = np.abs(g[:, 0:2] - w[:, SLOTS["mean"]]).max(1)
+    err["z_rel"] = np.abs(g[:, 2] - w[:, 6]) / w[:, 6]
+    err["op_rel"] = np.abs(g[:, 3] - w[:, 3]) / w[:, 3]
+    conic = w[:, SLOTS["conic"]]
+    cn = np.sqrt(conic[:, 0] * conic[:, 2])
+    err["conic_rel"] = np.abs(g[:, 4:7] - conic).max(1) / cn / kappa
+    err["ext_rel"] = np.maximum(np.abs(g[:, 7] - w[:, 21]) / w[:, 21], np.abs(g[:, 11] - w[:, 22]) / w[:, 22])
+    err["rgb_abs"] = np.abs(g[:, 8:11] - w[:, SLOTS["rgb"]]).max(1)
+    for k, v in err.items():
+        stats["max_" + k] = float(v.max())
+    # tolerances derived in DESIGN.md "fp32 error budget of the record": the mean inherits the
+    # fp32 rounding of the world position (eps * (|mu| + |v| l/2pi + |T|)) magnified by f/z
+    eps = 2.0 ** -23
+    zc = w[:, 6]
+    f = max(float(cam.fx), float(cam.fy))
+    Tn = float(np.abs(np.asarray(cam.world_to_cam, dtype=np.float64).reshape(3, 4)[:, 3]).max())
+    pos = np.abs(scene.mu[both].astype(np.float64)).max(1) + 0.05 * np.abs(scene.vel[both].astype(np.float64)).max(1) + Tn
+    ray = 1.0 + np.abs(w[:, 4] / zc) + np.abs(w[:, 5] / zc)
+    mean_tol = 8 * eps * f * pos * ray / zc + 4 * eps * (np.abs(w[:, 19]) + np.abs(w[:, 20]) + abs(cam.cx) + abs(cam.cy))
+    stats["max_mean_err_over_tol"] = float((err["mean_px"] / mean_tol).max())
+    assert np.all(err["mean_px"] <= mean_tol), ("mean2d", stats["max_mean_err_over_tol"])
+    assert err["z_rel"].max() <= 2e-6 + 0, ("z", stats["max_z_rel"])
+    assert err["op_rel"].max() <= 2e-5, ("opacity", stats["max_op_rel"])
+    assert err["conic_rel"].max() <= 2e-5, ("conic", stats["max_conic_rel"])
+    # h = sqrt(2 ln(255 o~) Sigma'): near the opacity cutoff the logarithm is ~0 and carries an
+    # absolute fp32 error of ~1e-6, i.e. a relative error 1e-6 / k in k and half that in h
+    kk = 2.0 * np.log(255.0 * w[:, 3])
+    ext_tol = 2e-5 + 2e-6 / np.maximum(kk, 1e-12)
+    assert np.all(err["ext_rel"] <= ext_tol), ("extent", float((err["ext_rel"] / ext_tol).max()))
+    assert err["rgb_abs"].max() <= 5e-6, ("rgb", stats["max_rgb_abs"])
+    return stats
+
+
+def check_integer_chain(dbg: dict, width: int, height: int, presort: bool):
+    """(I): bit-exact. dbg = Scene.debug() of a render with KEEP_UNSORTED=1."""
+    rec = dbg["record"]
+    rects, counts, M = oracle.tile_counts(rec, width, height)
+    assert dbg["M"] == M, (dbg["M"], M)
+    assert np.array_equal(dbg["counts"], counts), "per-Gaussian tile counts"
+    k = oracle.keys(rec, width, height, 1 if presort else 0)
+    n = rec.shape[0]
+    if presort:
+        visit = dbg["visit_order"]
+        # survivors come first in (z bits, index) order; the culled tail is in index order
+        surv = np.nonzero(counts)[0]
+        exp = surv[np.lexsort((surv, rec[surv, 2].view(np.uint32)))]
+        culled = np.nonzero(counts == 0)[0]
+        assert np.array_equal(visit, np.concatenate([exp, culled]).astype(np.uint32)), "depth visit order"
+        off_by_g = np.empty(n, dtype=np.uint64)
+        off_by_g[visit] = dbg["offsets"].astype(np.uint64)
+    else:
+        assert dbg["visit_order"] is None
+        off_by_g = dbg["offsets"].astype(np.uint64)
+    nz = counts > 0
+    assert np.array_equal(off_by_g[nz], k["offsets"][nz]), "exclusive offsets"
+    if dbg.get("keys_unsorted") is not None and M:
+        assert np.array_equal(dbg["keys_unsorted"], k["keys_unsorted"]), "unsorted keys"
+        assert np.array_equal(dbg["vals_unsorted"], k["vals_unsorted"]), "unsorted values"
+    assert np.array_equal(dbg["keys_sorted"], k["keys_sorted"]), "sorted keys"
+    assert np.array_equal(dbg["vals_sorted"], k["vals_sorted"]), "sorted values"
+    assert np.array_equal(dbg["ranges"], k["ranges"]), "tile ranges"
+    return dict(M=M, max_count=int(counts.max()), mean_list=float(M / max(1, k["ranges"].shape[0])))
+
+
+def check_images(gpu, ora, z_max: float, tol_rgb: float = TOL_RGB, with_cond: bool = True, label: str = ""):
+    """(R): per pixel |rgb_gpu - rgb_oracle| <= tol + budget (+ fp32 conditioning allowance),
+    depth within 1e-3 relative + budget * z_max / alpha. gpu = (rgb, depth, alpha) float32 arrays."""
+    rgb, depth, alpha = (np.asarray(x, dtype=np.float64) for x in gpu)
+    allow = ora["budget"] + (ora["cond"] if with_cond else 0.0)
+    e_rgb = np.abs(rgb - ora["rgb"]).max(0)
+    e_alpha = np.abs(alpha - ora["alpha"])
+    a = np.maximum(ora["alpha"], 1.0 / 255.0)
+    e_depth = np.abs(depth - ora["depth"])
+    depth_tol = TOL_DEPTH_REL * ora["depth"] + (allow + tol_rgb) * z_max / a
+    clean = ora["budget"] == 0
+    stats = dict(label=label,
+                 max_rgb_err=float(e_rgb.max()), max_rgb_err_clean=float(e_rgb[clean].max()) if clean.any() else 0.0,
+                 max_alpha_err=float(e_alpha.max()),
+                 max_depth_rel=float((e_depth / np.maximum(ora["depth"], 1e-9))[ora["alpha"] > 0].max()) if (ora["alpha"] > 0).any() else 0.0,
+                 fragile_pixels=int((~clean).sum()), pixels=int(clean.size),
+                 max_cond=float(ora["cond"].max()))
+    bad_rgb = e_rgb > tol_rgb + allow
+    bad_alpha = e_alpha > tol_rgb + allow
+    bad_depth = e_depth > depth_tol
+    stats["bad_rgb"], stats["bad_alpha"], stats["bad_depth"] = int(bad_rgb.sum()), int(bad_alpha.sum()), int(bad_depth.sum())
+    assert not bad_rgb.any(), ("rgb", stats)
+    assert not bad_alpha.any(), ("alpha", stats)
+    assert not bad_depth.any(), ("depth", stats)
+    assert stats["fragile_pixels"] <= 0.01 * stats["pixels"], ("too many fragile pixels", stats)
+    return stats

@@ -1,0 +1,220 @@
+"""GPU parity tests: the CUDA path, called through the C ABI binding, against the CPU oracle
+on the same seeded inputs. Bit-exact for the integer chain; images within 2e-4 (north_star)
+plus the fragile budget. Every test here needs a B200."""
+import json
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2311_18561_b200 as pvg
+from helpers import cam_simple, one_scene
+from parity import check_images, check_integer_chain, check_record
+from workloads import make_config, pinhole_camera
+
+pytestmark = pytest.mark.gpu
+
+
+def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None):
+    """(P), (I), (R) for one frame. Returns the stats of the three comparisons."""
+    own = scene is None
+    sc = scene or pvg.Scene.from_workload_scene(wl_scene)
+    try:
+        sc.set_option(pvg.OPT_PRESORT_DEPTH, 1 if presort else 0)
+        sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
+        rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t))
+        dbg = sc.debug()
+    finally:
+        if own:
+            sc.close()
+    wide, orec = oracle.preprocess_scene(wl_scene, cam, t)
+    stats = {"P": check_record(dbg["record"], wide, cam, wl_scene),
+             "I": check_integer_chain(dbg, cam.width, cam.height, presort)}
+    grec = dbg["record"]
+    zmax = float(max(grec[:, 2].max(), 1.0))
+    mode = "brute" if brute else "binned"
+    ora = oracle.render(grec, cam.width, cam.height, bg=cam.bg, mode=mode)
+    stats["R"] = check_images((rgb, depth, alpha), ora, zmax, label="gpu-record")
+    if end_to_end:
+        ora2 = oracle.render(orec, cam.width, cam.height, bg=cam.bg, mode="binned", tie_budget=True)
+        # end to end the two records differ by fp32 rounding of the preprocess: the tolerance
+        # adds the image-space effect of that
+        stats["E"] = check_images((rgb, depth, alpha), ora2, zmax, tol_rgb=1e-3, label="end-to-end")
+    print(json.dumps(stats))
+    return stats
+
+
+@pytest.mark.parametrize("t", [0.0, 0.37, 0.5])
+@pytest.mark.parametrize("presort", [True, False])
+def test_cfg0_all_timestamps(t, presort):
+    wl = make_config(0)
+    st = full_parity(wl.scene, wl.cameras[0], t, presort=presort, brute=True)
+    assert st["R"]["max_rgb_err_clean"] <= 2e-4
+
+
+def test_cfg1_mid_scene():
+    wl = make_config(1)
+    st = full_parity(wl.scene, wl.cameras[0], 0.5)
+    assert st["I"]["M"] > 1_000_000
+
+
+def test_cfg1_full_width_sort_mode_matches():
+    wl = make_config(1, n=60_000)
+    full_parity(wl.scene, wl.cameras[0], 0.5, presort=False, end_to_end=False)
+
+
+def test_cfg2_mix_reduced_full_resolution():
+    """Config-2 generator at 20k points, full 1920x1280 frame (9600 tiles, 14 tile bits)."""
+    wl = make_config(2, n=20_000)
+    st = full_parity(wl.scene, wl.cameras[0], 0.5)
+    assert st["I"]["max_count"] > 1000          # the skewed counts the duplication must balance
+
+
+def test_cfg4_side_camera_ragged_tiles():
+    """1920x886 side camera: 886 = 55*16 + 6, last tile row is partial; yawed pose."""
+    wl = make_config(4, n=20_000)
+    for cam in (wl.cameras[1], wl.cameras[4]):
+        full_parity(wl.scene, cam, 0.25)
+
+
+def test_background_and_null_outputs():
+    wl = make_config(0)
+    cam = wl.cameras[0]
+    cam.bg = (0.2, 0.5, 0.9)
+    full_parity(wl.scene, cam, 0.37, end_to_end=False)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    import torch
+    rgb = torch.zeros((3, cam.height, cam.width), device="cuda")
+    pvg._check(sc._L.pvg_render(sc._h, pvg.C.byref(pvg.camera_struct(cam)), 0.37, rgb.data_ptr(), None, None))
+    ref = sc.render(cam, 0.37)[0]
+    assert torch.equal(rgb, ref)
+    sc.close()
+
+
+def test_time_pins_on_gpu():
+    """The paper's invariants hold on the CUDA path too: t = tau is static 3DGS; a static scene
+    does not depend on t; l = +inf is linear motion (L336)."""
+    wl = make_config(0)
+    s, cam = wl.scene, wl.cameras[0]
+    n = s.n
+    inf = np.full(n, np.inf, np.float32)
+    static = pvg.Scene(s.mu, s.quat, s.scale, s.opacity, s.sh, s.tau, inf, np.zeros_like(s.vel))
+    a = static.render(cam, 0.1)[0].cpu().numpy()
+    b = static.render(cam, 0.83)[0].cpu().numpy()
+    assert np.array_equal(a, b)
+    at_tau = pvg.Scene(s.mu, s.quat, s.scale, s.opacity, s.sh, np.full(n, 0.375, np.float32), s.beta, s.vel)
+    c = at_tau.render(cam, 0.375)[0].cpu().numpy()
+    assert np.array_equal(a, c)
+    lin = pvg.Scene(s.mu, s.quat, s.scale, s.opacity, s.sh, s.tau, s.beta, s.vel, cycle=float("inf"))
+    lin.render(cam, 0.5)
+    rec = lin.debug(["record"])["record"]
+    wide, _ = oracle.preprocess(s.mu, s.quat, s.scale, s.opacity, s.sh, s.tau, s.beta, s.vel, np.inf, 3, cam, 0.5)
+    check_record(rec, wide, cam, s)
+    for x in (static, at_tau, lin):
+        x.close()
+
+
+def test_edge_cases():
+    cam = cam_simple(64, 48, 50.0)
+    # everything culled -> M = 0, image = background
+    sc = one_scene(mu=[(0, 0, -5), (0, 0, 0.1)], opacity=[0.5, 0.5])
+    cam.bg = (0.1, 0.2, 0.3)
+    g = pvg.Scene.from_workload_scene(sc)
+    rgb, depth, alpha = (x.cpu().numpy() for x in g.render(cam, 0.0))
+    assert g.debug()["M"] == 0 and np.all(alpha == 0) and np.all(depth == 0)
+    assert np.allclose(rgb[:, 3, 3], [0.1, 0.2, 0.3])
+    g.close()
+    cam.bg = (0.0, 0.0, 0.0)
+    # a single Gaussian; a Gaussian covering every tile; n = 1
+    for scene in (one_scene(mu=(0.1, 0.05, 3.0), scale=(0.2, 0.1, 0.1), opacity=0.9, sh=np.full((1, 16, 3), 0.3, np.float32)),
+                  one_scene(mu=(0, 0, 1.0), scale=(5, 5, 5), opacity=0.99)):
+        st = full_parity(scene, cam, 0.0, brute=True)
+    assert st["I"]["max_count"] == 12            # 4 x 3 tiles, all covered
+    # non-finite inputs cull the point and never poison the image
+    bad = one_scene(mu=[(0, 0, 3), (np.nan, 0, 3), (0, np.inf, 3), (0.2, 0, 3)], scale=[(0.1,) * 3, (0.1,) * 3, (0.1,) * 3, (np.nan, 0.1, 0.1)],
+                    opacity=[0.9, 0.9, 0.9, 0.9])
+    g = pvg.Scene.from_workload_scene(bad)
+    rgb, depth, alpha = (x.cpu().numpy() for x in g.render(cam, 0.0))
+    assert np.isfinite(rgb).all() and np.isfinite(depth).all() and list(g.debug()["counts"] > 0) == [True, False, False, False]
+    g.close()
+    # depth ties keep index order (stable sort)
+    tie = one_scene(mu=[(0, 0, 3.0)] * 5, scale=(0.3, 0.3, 0.3), opacity=0.5,
+                    sh=np.stack([np.full((16, 3), 0.1 * k, np.float32) for k in range(5)]))
+    full_parity(tie, cam, 0.0, brute=True, end_to_end=False)   # (ties make every pixel tie-fragile end to end)
+    # errors
+    g = pvg.Scene.from_workload_scene(tie)
+    cam_bad = cam_simple(0, 48, 50.0)
+    with pytest.raises(pvg.PvgError) as e:
+        g.render(cam_bad, 0.0, out=g.render(cam, 0.0))
+    assert e.value.code == -3
+    g.close()
+
+
+def test_render_host_matches_render():
+    wl = make_config(0)
+    cam = wl.cameras[0]
+    g = pvg.Scene.from_workload_scene(wl.scene)
+    d = [x.cpu() for x in g.render(cam, 0.37)]
+    h = g.render_host(cam, 0.37)
+    for a, b in zip(d, h):
+        assert np.array_equal(a.numpy(), b.numpy())
+    g.close()
+
+
+def test_repeatable_and_stream():
+    """Same frame twice on a non-default torch stream: bit-identical (no atomics in the data path)."""
+    import torch
+    wl = make_config(1, n=50_000)
+    cam = wl.cameras[0]
+    g = pvg.Scene.from_workload_scene(wl.scene)
+    a = [x.clone() for x in g.render(cam, 0.5)]
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        b = g.render(cam, 0.5)
+    st.synchronize()
+    for x, y in zip(a, b):
+        assert torch.equal(x, y)
+    times = g.stage_times_ms()
+    assert set(times) == set(pvg.STAGES) and times["blend"] > 0
+    names = [k[0] for k in g.kernel_times_ms()]
+    assert names[0] == "preprocess" and names[-1] == "blend" and "onesweep_pass" in names
+    g.close()
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 6143, 6144, 6145, 100_003, 1_500_000])
+def test_onesweep_sort_pairs_random(n):
+    import torch
+    rng = np.random.default_rng(n + 1)
+    keys = rng.integers(0, 2 ** 63, size=n, dtype=np.int64) ^ (rng.integers(0, 2, size=n, dtype=np.int64) << 63)
+    vals = np.arange(n, dtype=np.int32)
+    ko, vo = pvg.sort_pairs(torch.from_numpy(keys).cuda(), torch.from_numpy(vals).cuda())
+    idx = np.argsort(keys.view(np.uint64), kind="stable")
+    assert np.array_equal(ko.cpu().numpy().view(np.uint64), keys.view(np.uint64)[idx])
+    assert np.array_equal(vo.cpu().numpy(), vals[idx])
+
+
+@pytest.mark.parametrize("bits", [(0, 8), (32, 46), (3, 20), (0, 64), (17, 17), (40, 41)])
+def test_onesweep_bit_ranges_and_stability(bits):
+    """Few distinct digits and many ties: stability is part of the contract (S11)."""
+    import torch
+    n = 300_000
+    rng = np.random.default_rng(5)
+    keys = (rng.integers(0, 7, size=n, dtype=np.int64) << bits[0]) | rng.integers(0, 2 ** 62, size=n, dtype=np.int64)
+    vals = np.arange(n, dtype=np.int32)
+    ko, vo = pvg.sort_pairs(torch.from_numpy(keys).cuda(), torch.from_numpy(vals).cuda(), *bits)
+    width = bits[1] - bits[0]
+    digit = (keys.view(np.uint64) >> np.uint64(bits[0])) & np.uint64((1 << width) - 1 if width < 64 else 2 ** 64 - 1)
+    idx = np.argsort(digit, kind="stable")
+    assert np.array_equal(vo.cpu().numpy(), vals[idx])
+    assert np.array_equal(ko.cpu().numpy(), keys[idx])
+
+
+def test_onesweep_all_equal_and_sorted_inputs():
+    import torch
+    n = 200_000
+    for keys in (np.full(n, 0x1234_5678_9ABC, dtype=np.int64), np.arange(n, dtype=np.int64) * 3,
+                 (np.arange(n, dtype=np.int64)[::-1] * 5).copy()):
+        vals = np.arange(n, dtype=np.int32)
+        ko, vo = pvg.sort_pairs(torch.from_numpy(keys).cuda(), torch.from_numpy(vals).cuda(), 0, 40)
+        idx = np.argsort(keys, kind="stable")
+        assert np.array_equal(vo.cpu().numpy(), vals[idx]) and np.array_equal(ko.cpu().numpy(), keys[idx])
