@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- PVG render FPS at 1920x1280 on B200 (BASELINE.json metric), with roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+A "step" is one pass of the whole hot path (preprocess, depth sort, scan + duplicate, onesweep
+sort, tile ranges, blend) over one frame (camera, t) of the workload: BASELINE.json config 3,
+3M Gaussians, 1920x1280, 50 timestamps in [0,1]. The scene (the model theta) is resident in HBM
+like network weights; the per-step input is (camera, t). N > 1: frames are sharded over ranks,
+no data-path collective, weak scaling.
+
+Prints ONE JSON line on rank 0. `--impl reference` times the CPU oracle (test infrastructure,
+never tuned) on the host cores for the same metric/config and prints the same line shape.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "render_fps_1920x1280"
+UNIT = "frames/s"
+CONFIG_NAMES = {0: "cfg0_tiny_4096g_128x96", 1: "cfg1_mid_200kg_960x640", 2: "cfg2_urban_1Mg_1920x1280",
+                3: "cfg3_timesweep_3Mg_1920x1280_50t", 4: "cfg4_stress_6Mg_5cams"}
+# issue slots per (pixel, list entry) evaluation of the blend
+SLOTS_REJECT, SLOTS_ACCEPT_EXTRA = 11, 6
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--n", type=int, default=None, help="override the point count (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--presort", type=int, default=1)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """dram bytes per launch from the committed ncu --set full capture, if one exists."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
+            d = json.load(f)
+        return d.get(workload, {}).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+        self.t0 = self.t1 = None
+
+    def mark_start(self):
+        self.t0 = time.time()
+
+    def mark_end(self):
+        self.t1 = time.time()
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.12)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        import datetime
+        rows = []
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 10:
+                continue
+            try:
+                ts = datetime.datetime.strptime(parts[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(parts[2]), float(parts[3]), parts[5:10]))
+            except Exception:
+                continue
+        sel = [r for r in rows if self.t0 is not None and self.t0 - 0.05 <= r[0] <= self.t1 + 0.05] or rows
+        if sel:
+            out["sm_mhz"] = statistics.median(r[1] for r in sel)
+            out["sm_max_mhz"] = max(r[2] for r in sel)
+            names = ["active_mask", "hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            seen = set()
+            for r in sel:
+                for nm, v in zip(names[1:], r[3][1:]):
+                    if v.lower().startswith("active"):
+                        seen.add(nm)
+            out["reasons"] = sorted(seen)
+            out["samples"] = len(sel)
+        try:
+            os.unlink(self.f.name)
+        except Exception:
+            pass
+        return out
+
+
+def physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ------------------------------------------------------------------------------------------
+def oracle_frame_time(wl, cam, t, sample_tiles: int, seed: int):
+    """Times the CPU oracle (as it stands) on a bounded sample of one frame: Oracle-P over all N
+    Gaussians + Oracle-R (binned) on `sample_tiles` uniformly sampled tiles; the tile part is
+    scaled to the whole frame. Returns (estimated seconds per frame, detail dict)."""
+    import oracle
+    tiles_total = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    rng = np.random.default_rng(seed)
+    sel = np.sort(rng.choice(tiles_total, size=min(sample_tiles, tiles_total), replace=False)).astype(np.uint32)
+    t0 = time.perf_counter()
+    _, rec = oracle.preprocess_scene(wl.scene, cam, t)
+    t1 = time.perf_counter()
+    oracle.render(rec, cam.width, cam.height, bg=cam.bg, mode="binned", tiles=sel)
+    t2 = time.perf_counter()
+    est = (t1 - t0) + (t2 - t1) * tiles_total / len(sel)
+    return est, dict(preprocess_s=t1 - t0, tiles_s=t2 - t1, tiles=int(len(sel)), tiles_total=int(tiles_total))
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from workloads import make_config
+    wl = make_config(args.config, args.n)
+    frames = list(wl.frames())
+    sample = 24
+    times = []
+    for s in range(args.warmup + args.steps):
+        cam, t = frames[s % len(frames)]
+        est, det = oracle_frame_time(wl, cam, t, sample, seed=s)
+        if s >= args.warmup:
+            times.append(est)
+    sec = float(np.mean(times))
+    fps = 1.0 / sec
+    line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": CONFIG_NAMES[args.config], "n_gaussians": wl.scene.n,
+                       "resolution": f"{frames[0][0].width}x{frames[0][0].height}"},
+            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": f"per step: Oracle-P on all {wl.scene.n} Gaussians + Oracle-R (binned) on {sample} of "
+                                       f"{det['tiles_total']} tiles, tile time scaled to the frame"},
+            "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import paper_2311_18561_b200 as pvg
+    from paper_2311_18561_b200 import build as pvg_build, dist
+    from workloads import make_config
+
+    rank, local_rank, ws = dist.init("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the render path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if rank == 0:
+        pvg_build.build()
+    dist.barrier(local_rank)
+
+    wl = make_config(args.config, args.n)
+    frames = list(wl.frames())
+    sched = dist.frame_schedule(rank, ws, args.steps, frames)
+    warm = dist.frame_schedule(rank, ws, max(args.warmup, 3), frames)
+    scene = pvg.Scene.from_workload_scene(wl.scene)
+    scene.set_option(pvg.OPT_PRESORT_DEPTH, args.presort)
+    cams = {id(c): pvg.camera_struct(c) for c, _ in frames}
+
+    def outs(c):
+        return (torch.empty((3, c.height, c.width), device=dev), torch.empty((c.height, c.width), device=dev),
+                torch.empty((c.height, c.width), device=dev))
+
+    out_by_cam = {k: outs(c) for k, c in {id(c): c for c, _ in frames}.items()}
+
+    # ---- warm-up (also sizes the workspace)
+    for cam, t in warm:
+        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+    torch.cuda.synchronize()
+
+    # ---- timed region: K frames, inputs resident in HBM, device-timed, max over ranks
+    sampler = ClockSampler(physical_gpu_index(local_rank)) if rank == 0 else None
+    time.sleep(0.3 if sampler else 0.0)
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 2)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    Ms = []
+    dist.barrier(local_rank)
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.mark_start()
+    e0.record()
+    for cam, t in sched:
+        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+        Ms.append(int(scene.debug_info().num_instances))
+    e1.record()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.mark_end()
+    dist.barrier(local_rank)
+    elapsed_s = dist.max_over_ranks(e0.elapsed_time(e1) / 1e3, dev)
+    krecs = scene.kernel_times_ms()
+    clocks = sampler.stop() if sampler else None
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 1)
+    total_frames = args.steps * ws
+    fps = total_frames / elapsed_s
+
+    # ---- blend work (pairs) of the same frames, counted in an untimed pass
+    scene.set_option(pvg.OPT_COUNT_PAIRS, 1)
+    pairs_eval = pairs_contrib = 0
+    for cam, t in sched:
+        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+        a, b = scene.blend_counters()
+        pairs_eval += a
+        pairs_contrib += b
+    scene.set_option(pvg.OPT_COUNT_PAIRS, 0)
+
+    # ---- end to end through the C ABI with HOST buffers (D2H of the images inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        host = {k: (torch.empty(v[0].shape, pin_memory=True), torch.empty(v[1].shape, pin_memory=True),
+                    torch.empty(v[2].shape, pin_memory=True)) for k, v in out_by_cam.items()}
+        for cam, t in warm[:2]:
+            scene.render_host(cams[id(cam)], t, host[id(cam)])
+        dist.barrier(local_rank)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        d2h = 0
+        for cam, t in sched:
+            scene.render_host(cams[id(cam)], t, host[id(cam)])
+            d2h += cam.width * cam.height * 5 * 4
+        torch.cuda.synchronize()
+        el = dist.max_over_ranks(time.perf_counter() - t0, dev)
+        dist.barrier(local_rank)
+        e2e = {"value": total_frames / el, "unit": UNIT,
+               "h2d_bytes_per_step": int(pvg.C.sizeof(pvg.CameraC) + 4), "d2h_bytes_per_step": int(d2h // len(sched)),
+               "note": "pvg_render_host: per-step input is (camera, t); rgb+depth+alpha copied to pinned host memory"}
+
+    if rank != 0:
+        scene.close()
+        dist.shutdown()
+        return
+
+    # ---- per-kernel aggregation and roofline
+    hbm_peak, sm_max_mhz, peak_src = measured_peaks()
+    N = wl.scene.n
+    S = int((scene.debug(["counts"])["counts"] > 0).sum())
+    Msum = float(sum(Ms))
+    K = len(sched)
+    agg = {}
+    for name, stage, ms in krecs:
+        a = agg.setdefault((name, stage), [0.0, 0])
+        a[0] += ms
+        a[1] += 1
+    # algorithmic bytes over the timed region, per (kernel, stage)
+    alg = {("preprocess", "preprocess"): K * (64.0 * N + 80.0 * N + 192.0 * S),
+           ("scan_counts", "duplicate"): K * 12.0 * N,
+           ("duplicate", "duplicate"): 12.0 * Msum,
+           ("onesweep_histogram", "sort"): 8.0 * Msum,
+           ("onesweep_pass", "sort"): 0.0,   # filled below: 24 B per instance per launch
+           ("onesweep_histogram", "depth_sort"): K * 8.0 * N,
+           ("onesweep_pass", "depth_sort"): 0.0,
+           ("tile_ranges", "ranges"): 8.0 * Msum,
+           ("tile_prefix", "ranges"): 0.0}
+    for key in (("onesweep_pass", "sort"), ("onesweep_pass", "depth_sort")):
+        if key in agg:
+            per_frame = agg[key][1] / K
+            alg[key] = 24.0 * (Msum if key[1] == "sort" else K * N) * per_frame
+    kernels = {}
+    for (name, stage), (ms, cnt) in agg.items():
+        d = {"launches": cnt, "ms_total": ms, "ms_avg": ms / cnt, "share": ms / (elapsed_s * 1e3)}
+        b = alg.get((name, stage))
+        if b:
+            d["GBps"] = b / (ms * 1e-3) / 1e9
+            d["hbm_frac"] = d["GBps"] / hbm_peak
+        kernels[f"{stage}/{name}"] = d
+    sm_mhz = (clocks or {}).get("sm_mhz") or sm_max_mhz
+    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e12    # T thread-instr/s at the observed SM clock
+    bl = agg.get(("blend", "blend"))
+    if bl:
+        slots = SLOTS_REJECT * pairs_eval + SLOTS_ACCEPT_EXTRA * pairs_contrib
+        k = kernels["blend/blend"]
+        k["pairs_eval_per_frame"] = pairs_eval / K
+        k["pairs_contrib_per_frame"] = pairs_contrib / K
+        k["Tinstr_per_s"] = slots / (bl[0] * 1e-3) / 1e12
+        k["alu_frac"] = k["Tinstr_per_s"] / alu_peak
+    dom = max(agg.items(), key=lambda kv: kv[1][0])[0]
+    dk = kernels[f"{dom[1]}/{dom[0]}"]
+    workload = CONFIG_NAMES[args.config]
+    if dom[0] == "blend":
+        roofline = {"bound": "alu", "achieved": dk["Tinstr_per_s"], "peak": alu_peak, "unit": "Tinstr/s",
+                    "frac": dk["alu_frac"], "traffic": ncu_traffic("blend", workload), "kernel": "blend_kernel",
+                    "peak_source": f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (observed)"}
+    else:
+        roofline = {"bound": "hbm", "achieved": dk["GBps"], "peak": hbm_peak, "unit": "GB/s", "frac": dk["hbm_frac"],
+                    "traffic": ncu_traffic(dom[0], workload), "kernel": f"{dom[0]} ({dom[1]} stage)",
+                    "peak_source": peak_src, "avg_launch_ms": dk["ms_avg"],
+                    "algorithmic_bytes_per_launch": alg[dom] / agg[dom][1]}
+    stage_ms = {}
+    for (name, stage), (ms, cnt) in agg.items():
+        stage_ms[stage] = stage_ms.get(stage, 0.0) + ms / K
+
+    # ---- CPU oracle on a bounded sample (reported baseline, not the target)
+    cpu = None
+    if not args.no_cpu_baseline and ws == 1:
+        import oracle
+        cam, t = frames[len(frames) // 2]
+        est, det = oracle_frame_time(wl, cam, t, 64, seed=0)
+        cpu = {"value": 1.0 / est, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"frame t={t:.3f}: Oracle-P on all {N} Gaussians ({det['preprocess_s']:.2f} s) + Oracle-R (binned) on "
+                         f"{det['tiles']} of {det['tiles_total']} tiles ({det['tiles_s']:.2f} s), tile time scaled to the frame"}
+
+    line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": ws, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": elapsed_s * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload, "n_gaussians": N, "survivors_last_frame": S,
+                       "resolution": f"{frames[0][0].width}x{frames[0][0].height}",
+                       "instances_per_frame_mean": Msum / K, "frames": "one (camera, t) per step, round-robin over the sweep",
+                       "l2_policy": f"inputs larger than L2: model {N * 256 / 1e6:.0f} MB + instance lists {24 * Msum / K / 1e6:.0f} MB "
+                                    "per frame vs 126 MB L2",
+                       "parallelism": f"frames sharded over {ws} rank(s), no collective", "presort_depth": args.presort},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks, "gpu_launches": len(krecs),
+            "gaussians_per_s": N * fps, "stage_ms_per_frame": stage_ms, "kernels": kernels}
+    print(json.dumps(line), flush=True)
+    scene.close()
+    dist.shutdown()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -110,7 +110,10 @@ typedef enum pvg_option {
   /* 1 (default): record a CUDA event pair around every kernel of the last render
    * (pvg_kernel_times_ms, pvg_stage_times_ms). 2: keep the records of EVERY render until
    * pvg_kernel_times_ms reads (and clears) them. 0: no events. */
-  PVG_OPT_KERNEL_EVENTS = 3
+  PVG_OPT_KERNEL_EVENTS = 3,
+  /* 1: the blend also counts its (pixel, list entry) evaluations (pvg_blend_counters); measurement
+   *    only -- the counting variant is a separate kernel instantiation (default 0). */
+  PVG_OPT_COUNT_PAIRS = 4
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 
@@ -150,6 +153,10 @@ int pvg_stage_times_ms(pvg_scene *scene, float ms[PVG_NUM_STAGES]);
  * names (static strings), stage ids and milliseconds; returns the number of launches (>= 0)
  * or a negative pvg_status. */
 int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stages, float *ms);
+
+/* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs
+ * evaluated before the pixel stopped, out[1] = pairs that contributed (alpha >= 1/255). */
+int pvg_blend_counters(pvg_scene *scene, uint64_t out[2]);
 
 /* The onesweep LSD radix sort as a primitive: stable sort of n (key,value) pairs on key bits
  * [begin_bit, end_bit). All pointers are DEVICE buffers of n elements; the sorted result is

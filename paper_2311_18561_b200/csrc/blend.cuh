@@ -24,10 +24,14 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // index list into shared memory (conic pre-scaled by -log2(e)/2 so the inner loop feeds
 // ex2 directly), then every pixel walks the batch. The tile retires as soon as every
 // pixel's transmittance has dropped below 1e-4.
+// COUNT = true additionally counts the (pixel, list entry) evaluations reached and the
+// contributing ones into counters[0..1] (measurement only, never on the product path).
+template <bool COUNT>
 __global__ void __launch_bounds__(BLEND_THREADS)
 blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
              const uint32_t* __restrict__ vals, const float4* __restrict__ record,
-             float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha) {
+             float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
+             unsigned long long* __restrict__ counters) {
   __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
   __shared__ float4 s_col[BLEND_BATCH];   // c', o~, r, g
   __shared__ float2 s_bz[BLEND_BATCH];    // b, z
@@ -42,6 +46,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
 
   float T = 1.0f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;
   bool done = !inside;
+  uint32_t n_eval = 0, n_contrib = 0;
 
   for (uint32_t base = range.x; base < range.y; base += BLEND_BATCH) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
@@ -63,6 +68,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
       for (uint32_t j = 0; j < nb; ++j) {
         const float4 ge = s_geo[j];
         const float4 co = s_col[j];
+        if (COUNT) ++n_eval;
         const float dx = ge.x - pxf, dy = ge.y - pyf;
         // w = log2(e) * (-1/2 (a dx^2 + c dy^2) - b dx dy)
         float w = fmaf(dx, fmaf(ge.z, dx, ge.w * dy), (co.x * dy) * dy);
@@ -78,10 +84,15 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
         Cb = fmaf(bz.x, wgt, Cb);
         D = fmaf(bz.y, wgt, D);
         T = Tn;
+        if (COUNT) ++n_contrib;
       }
     }
   }
 
+  if (COUNT) {
+    atomicAdd(counters, (unsigned long long)n_eval);
+    atomicAdd(counters + 1, (unsigned long long)n_contrib);
+  }
   if (inside) {
     const size_t HW = (size_t)P.width * P.height;
     const size_t pi = (size_t)py * P.width + px;

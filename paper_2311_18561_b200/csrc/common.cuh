@@ -70,4 +70,14 @@ __device__ __forceinline__ float4 ldg_stream_f4(const float4* p) {
   return v;
 }
 
+// corner updates of one rectangle [x0,x1] x [y0,y1] (inclusive) on the (TX+1) x (TY+1) grid
+__device__ __forceinline__ void tilegrid_add_rect(int* __restrict__ grid, int stride, int x0, int y0, int x1, int y1) {
+  atomicAdd(grid + y0 * stride + x0, 1);
+  atomicAdd(grid + y0 * stride + x1 + 1, -1);
+  atomicAdd(grid + (y1 + 1) * stride + x0, -1);
+  atomicAdd(grid + (y1 + 1) * stride + x1 + 1, 1);
+}
+
+__host__ __device__ inline int tilegrid_stride(int tiles_x) { return (tiles_x + 1) | 1; }  // odd: conflict-free rows
+
 }  // namespace pvg

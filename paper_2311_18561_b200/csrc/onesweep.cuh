@@ -36,6 +36,23 @@ inline SortPlan make_sort_plan(int begin_bit, int end_bit) {
   return p;
 }
 
+// Lanes of the warp holding the same digit as the caller. One vote.ballot per digit bit:
+// on sm_100a MATCH.ANY runs on the address-divergence unit at ~64 cycles per warp
+// instruction per SM and caps a sort pass near 40% of HBM bandwidth (profiles/), while
+// ballots issue on the regular pipes. `bits` is warp-uniform.
+__device__ __forceinline__ uint32_t digit_peers(uint32_t d, int bits) {
+  uint32_t peers = 0xffffffffu;
+#pragma unroll
+  for (int b = 0; b < OS_RADIX_BITS; ++b) {
+    if (b < bits) {
+      const bool one = (d >> b) & 1u;
+      const uint32_t m = __ballot_sync(0xffffffffu, one);
+      peers &= one ? m : ~m;
+    }
+  }
+  return peers;
+}
+
 // ---- digit histograms of every pass in one read of the keys ---------------------------
 constexpr int HIST_THREADS = 512;
 constexpr int HIST_ITEMS = 8;
@@ -46,7 +63,7 @@ onesweep_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n, const _
   __shared__ uint32_t s_hist[OS_MAX_PASSES * OS_RADIX];
   for (int k = threadIdx.x; k < plan.num_passes * OS_RADIX; k += HIST_THREADS) s_hist[k] = 0;
   __syncthreads();
-  // block-uniform trip count; equal digits inside a warp are aggregated with match.any
+  // block-uniform trip count; equal digits inside a warp are aggregated before the atomic
   // (tile-id digits of neighbouring instances are nearly always equal)
   constexpr uint64_t CH = (uint64_t)HIST_THREADS * HIST_ITEMS;
   const uint32_t lt = lanemask_lt();
@@ -61,8 +78,9 @@ onesweep_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n, const _
     for (int u = 0; u < HIST_ITEMS; ++u) {
       const bool ok = base + (uint64_t)u * HIST_THREADS + threadIdx.x < n;
       for (int p = 0; p < plan.num_passes; ++p) {
-        const uint32_t d = ok ? ((uint32_t)(k[u] >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u)) : 0xFFFFFFFFu;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t d = (uint32_t)(k[u] >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
+        const uint32_t live = __ballot_sync(0xffffffffu, ok);
+        const uint32_t peers = digit_peers(d, plan.bits[p]) & live;
         if (ok && (peers & lt) == 0) atomicAdd(&s_hist[p * OS_RADIX + d], (uint32_t)__popc(peers));
       }
     }
@@ -109,12 +127,12 @@ struct OnesweepSmem {
 };
 
 // Keys of a tile are read warp-striped (warp w owns ITEMS*32 consecutive keys, lane l its
-// elements l, l+32, ...), ranked inside the warp with match.any (stable: earlier rounds and
+// elements l, l+32, ...), ranked inside the warp with ballots (stable: earlier rounds and
 // lower lanes come first), combined across warps per digit, resolved against earlier
 // tiles by look-back, re-ordered through shared memory and written out in digit runs so
 // that stores are coalesced.
 template <int THREADS, int ITEMS>
-__global__ void __launch_bounds__(THREADS)
+__global__ void __launch_bounds__(THREADS, 2)
 onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                      uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint64_t n,
                      int shift, int bits, const uint32_t* __restrict__ hist_excl /* [256] this pass */,
@@ -139,10 +157,16 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
   //    the last digit and are never written
   const uint32_t wbase = warp * (ITEMS * 32) + lane;
   uint64_t key[ITEMS];
+  uint32_t val[ITEMS];
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
     const uint32_t li = wbase + j * 32;
     key[j] = li < tile_n ? __ldcs(keys_in + tile_base + li) : ~0ull;
+  }
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const uint32_t li = wbase + j * 32;
+    val[j] = li < tile_n ? __ldcs(vals_in + tile_base + li) : 0u;
   }
 
   // 2. rank inside the warp
@@ -152,7 +176,7 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
     const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
-    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t peers = digit_peers(d, bits);
     const uint32_t before = wh[d];
     __syncwarp();
     if ((peers & lt) == 0) wh[d] = before + __popc(peers);
@@ -207,18 +231,12 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
   __syncthreads();
 
   // 6. scatter into shared memory in sorted order
-  uint16_t pos[ITEMS];
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
     const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
     const uint32_t p = s.bin_start[d] + wh[d] + rank[j];
-    pos[j] = (uint16_t)p;
     s.keys[p] = key[j];
-  }
-#pragma unroll
-  for (int j = 0; j < ITEMS; ++j) {
-    const uint32_t li = wbase + j * 32;
-    if (li < tile_n) s.vals[pos[j]] = __ldcs(vals_in + tile_base + li);
+    s.vals[p] = val[j];
   }
   __syncthreads();
 

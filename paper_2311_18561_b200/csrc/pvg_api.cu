@@ -15,6 +15,7 @@
 #include "preprocess.cuh"
 #include "ranges.cuh"
 #include "scan_dup.cuh"
+#include "tilebin.cuh"
 
 using namespace pvg;
 
@@ -146,7 +147,8 @@ int onesweep_configure() {
 // Stable LSD sort of n pairs on key bits [begin_bit, end_bit). Buffers ping-pong; *result
 // tells which side (0: a, 1: b) holds the sorted list.
 int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, int begin_bit,
-                 int end_bit, cudaStream_t st, SortScratch& sc, Timer* tm, int stage, int* result) {
+                 int end_bit, cudaStream_t st, SortScratch& sc, Timer* tm, int stage, int* result,
+                 bool hist_ready = false) {
   *result = 0;
   if (n == 0 || end_bit <= begin_bit) return PVG_OK;
   TRY(onesweep_configure());
@@ -155,7 +157,7 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   TRY(sc.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
   TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
   TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, st, 1.25));
-  CU(cudaMemsetAsync(sc.hist.p, 0, (size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
+  if (!hist_ready) CU(cudaMemsetAsync(sc.hist.p, 0, (size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
   CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, st));
   CU(cudaMemsetAsync(sc.lookback.p, 0, (size_t)plan.num_passes * tiles * OS_RADIX * 8, st));
 
@@ -164,12 +166,14 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const uint64_t hist_chunks = (n + (uint64_t)HIST_THREADS * HIST_ITEMS - 1) / ((uint64_t)HIST_THREADS * HIST_ITEMS);
   const unsigned hist_grid = (unsigned)std::min<uint64_t>(hist_chunks, (uint64_t)sms * 4);
-  if (tm) TRY(tm->begin("onesweep_histogram", stage, st));
-  onesweep_histogram_kernel<<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
-  if (tm) TRY(tm->end(st));
-  if (tm) TRY(tm->begin("onesweep_scan_hist", stage, st));
-  onesweep_scan_hist_kernel<<<plan.num_passes, OS_RADIX, 0, st>>>(sc.hist.as<uint32_t>());
-  if (tm) TRY(tm->end(st));
+  if (!hist_ready) {
+    if (tm) TRY(tm->begin("onesweep_histogram", stage, st));
+    onesweep_histogram_kernel<<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
+    if (tm) TRY(tm->end(st));
+    if (tm) TRY(tm->begin("onesweep_scan_hist", stage, st));
+    onesweep_scan_hist_kernel<<<plan.num_passes, OS_RADIX, 0, st>>>(sc.hist.as<uint32_t>());
+    if (tm) TRY(tm->end(st));
+  }
 
   uint64_t* kin = ka; uint32_t* vin = va; uint64_t* kout = kb; uint32_t* vout = vb;
   for (int p = 0; p < plan.num_passes; ++p) {
@@ -194,14 +198,14 @@ struct pvg_scene {
   int sh_degree = 3;
   cudaStream_t stream = nullptr;
   // options
-  int presort = 1, keep_unsorted = 0;
+  int presort = 1, keep_unsorted = 0, count_pairs = 0;
   // model (SoA)
   Buf A0, A1, A2, A3, SH;
   // per-Gaussian workspace
   Buf record, tileinfo, counts, offsets, dkeys[2], dvals[2], scan_status, small;  // small: ticket u32 @0, total u64 @8
   // per-instance workspace
   Buf keys[2], vals[2], keys_unsorted, vals_unsorted;
-  Buf ranges;
+  Buf ranges, tilegrid;
   Buf img;  // render_host device images
   SortScratch sort_n, sort_m;
   uint64_t* h_total = nullptr;  // pinned
@@ -226,7 +230,7 @@ void release_all(pvg_scene* s) {
   Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted,
-                 &s->ranges, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->ranges, &s->tilegrid, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
@@ -326,14 +330,43 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
   s->rendered = false;
   TRY(s->ranges.reserve((size_t)tiles * 8, st));
 
-  // a1 preprocess
+  const int tile_bits = std::max(1, ceil_log2(tiles));
+  s->sort_begin = s->presort ? 32 : 0;
+  s->sort_end = 32 + tile_bits;
+
+  // a1 preprocess (+ the 2-D difference array of per-tile counts when the depth presort is on)
   uint64_t* dk = s->presort ? s->dkeys[0].as<uint64_t>() : nullptr;
   uint32_t* dv = s->presort ? s->dvals[0].as<uint32_t>() : nullptr;
+  int* grid = nullptr;
+  const size_t grid_bytes = (size_t)tilegrid_stride(P.tiles_x) * (P.tiles_y + 1) * 4;
+  if (s->presort) {
+    TRY(s->tilegrid.reserve(grid_bytes, st));
+    grid = s->tilegrid.as<int>();
+    CU(cudaMemsetAsync(grid, 0, grid_bytes, st));
+  }
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
   preprocess_kernel<<<(n + 255) / 256, 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
                                                       s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
-                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv);
+                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, grid);
   TRY(tm.end(st));
+
+  // a4 + the histograms of a3, from the tile counts alone (no pass over the instances)
+  if (s->presort) {
+    static bool attr_set = false;
+    constexpr size_t kMaxDyn = 200 * 1024;
+    if (!attr_set) {
+      CU(cudaFuncSetAttribute(tile_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
+      attr_set = true;
+    }
+    const int use_smem = grid_bytes <= kMaxDyn ? 1 : 0;
+    TRY(s->sort_m.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
+    uint64_t* total2 = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 16);
+    TRY(tm.begin("tile_prefix", PVG_STAGE_RANGES, st));
+    tile_prefix_kernel<<<1, TB_THREADS, use_smem ? grid_bytes : 0, st>>>(
+        grid, P.tiles_x, P.tiles_y, use_smem, make_sort_plan(s->sort_begin, s->sort_end), s->ranges.as<uint2>(),
+        s->sort_m.hist.as<uint32_t>(), total2);
+    TRY(tm.end(st));
+  }
 
   // a3 (n-key part): depth order of the Gaussians
   const uint32_t* visit = nullptr;
@@ -362,9 +395,6 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
   if (M >= (1ull << 32)) return PVG_ERR_INSTANCE_OVERFLOW;
   s->M = M;
 
-  const int tile_bits = std::max(1, ceil_log2(tiles));
-  s->sort_begin = s->presort ? 32 : 0;
-  s->sort_end = 32 + tile_bits;
   s->sorted_side = 0;
   if (M > 0) {
     for (int k = 0; k < 2; ++k) {
@@ -386,21 +416,31 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
     // a3 (M-instance part)
     int side = 0;
     TRY(run_onesweep(M, s->keys[0].as<uint64_t>(), s->vals[0].as<uint32_t>(), s->keys[1].as<uint64_t>(),
-                     s->vals[1].as<uint32_t>(), s->sort_begin, s->sort_end, st, s->sort_m, &tm, PVG_STAGE_SORT, &side));
+                     s->vals[1].as<uint32_t>(), s->sort_begin, s->sort_end, st, s->sort_m, &tm, PVG_STAGE_SORT, &side,
+                     s->presort != 0));
     s->sorted_side = side;
-    // a4 ranges
-    TRY(tm.begin("tile_ranges", PVG_STAGE_RANGES, st));
-    tile_ranges_kernel<<<(unsigned)((M + 255) / 256), 256, 0, st>>>(s->keys[side].as<uint64_t>(), M, tiles,
-                                                                    s->ranges.as<uint2>());
-    TRY(tm.end(st));
-  } else {
+    if (!s->presort) {
+      // a4 ranges from the sorted keys
+      TRY(tm.begin("tile_ranges", PVG_STAGE_RANGES, st));
+      tile_ranges_kernel<<<(unsigned)((M + 255) / 256), 256, 0, st>>>(s->keys[side].as<uint64_t>(), M, tiles,
+                                                                      s->ranges.as<uint2>());
+      TRY(tm.end(st));
+    }
+  } else if (!s->presort) {
     CU(cudaMemsetAsync(s->ranges.p, 0, (size_t)tiles * 8, st));
   }
 
   // a5 blend
   TRY(tm.begin("blend", PVG_STAGE_BLEND, st));
-  blend_kernel<<<tiles, BLEND_THREADS, 0, st>>>(P, s->ranges.as<uint2>(), s->vals[s->sorted_side].as<uint32_t>(),
-                                                s->record.as<float4>(), out_rgb, out_depth, out_alpha);
+  if (s->count_pairs) {
+    unsigned long long* ctr = reinterpret_cast<unsigned long long*>(s->small.as<unsigned char>() + 64);
+    CU(cudaMemsetAsync(ctr, 0, 16, st));
+    blend_kernel<true><<<tiles, BLEND_THREADS, 0, st>>>(P, s->ranges.as<uint2>(), s->vals[s->sorted_side].as<uint32_t>(),
+                                                        s->record.as<float4>(), out_rgb, out_depth, out_alpha, ctr);
+  } else {
+    blend_kernel<false><<<tiles, BLEND_THREADS, 0, st>>>(P, s->ranges.as<uint2>(), s->vals[s->sorted_side].as<uint32_t>(),
+                                                         s->record.as<float4>(), out_rgb, out_depth, out_alpha, nullptr);
+  }
   TRY(tm.end(st));
   CU(cudaGetLastError());
   s->rendered = true;
@@ -475,6 +515,7 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
   switch (option) {
     case PVG_OPT_PRESORT_DEPTH: scene->presort = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KEEP_UNSORTED: scene->keep_unsorted = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_COUNT_PAIRS: scene->count_pairs = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KERNEL_EVENTS:
       scene->timer.enabled = value != 0;
       scene->timer.accumulate = value == 2;
@@ -565,6 +606,15 @@ int pvg_stage_times_ms(pvg_scene* s, float ms[PVG_NUM_STAGES]) {
       if (r.stage == k) { if (!first) first = &r; last = &r; }
     if (first) CU(cudaEventElapsedTime(&ms[k], first->e0, last->e1));
   }
+  return PVG_OK;
+}
+
+int pvg_blend_counters(pvg_scene* s, uint64_t out[2]) {
+  if (!s || !out) return PVG_ERR_NULL;
+  out[0] = out[1] = 0;
+  if (!s->rendered || !s->count_pairs) return PVG_OK;
+  CU(cudaStreamSynchronize(s->stream));
+  CU(cudaMemcpy(out, s->small.as<unsigned char>() + 64, 16, cudaMemcpyDeviceToHost));
   return PVG_OK;
 }
 
