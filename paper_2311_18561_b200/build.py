@@ -24,14 +24,16 @@ def _deps():
             [os.path.join(os.path.dirname(HERE), "include", "pvg.h"), os.path.abspath(__file__)])
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
-        return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
+def build(force: bool = False, verbose: bool = False, out: str = LIB, defines=()) -> str:
+    """Compile csrc/*.cu into `out`. `defines` (e.g. ["PVG_OSL_THREADS=256"]) are for tuning builds."""
+    if not force and os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(d) for d in _deps()):
+        return out
+    tmp = out + f".tmp{os.getpid()}"
+    cmd = ([NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + [f"-D{d}" for d in defines]
+           + ["-o", tmp] + sources())
     subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, out)
+    return out
 
 
 if __name__ == "__main__":

@@ -12,7 +12,7 @@ namespace pvg {
 
 constexpr int OS_RADIX_BITS = 8;
 constexpr int OS_RADIX = 1 << OS_RADIX_BITS;
-constexpr int OS_MAX_PASSES = 8;
+constexpr int OS_MAX_PASSES = 10;
 
 struct SortPlan {
   int num_passes;
@@ -20,35 +20,50 @@ struct SortPlan {
   int bits[OS_MAX_PASSES];
 };
 
-// Split [begin_bit, end_bit) into ceil(B/8) passes of near-equal width (14 -> 7+7).
+// Split [begin_bit, end_bit) into digit passes of at most 8 bits and near-equal width
+// (14 -> 7+7). No pass straddles bit 32, so a digit always comes from one 32-bit half.
 inline SortPlan make_sort_plan(int begin_bit, int end_bit) {
   SortPlan p{};
-  const int B = end_bit - begin_bit;
-  p.num_passes = (B + OS_RADIX_BITS - 1) / OS_RADIX_BITS;
-  int at = begin_bit;
-  for (int i = 0; i < p.num_passes; ++i) {
-    const int left = end_bit - at, passes_left = p.num_passes - i;
-    const int b = (left + passes_left - 1) / passes_left;
-    p.shift[i] = at;
-    p.bits[i] = b;
-    at += b;
-  }
+  auto seg = [&](int b0, int b1) {
+    const int B = b1 - b0;
+    if (B <= 0) return;
+    const int np = (B + OS_RADIX_BITS - 1) / OS_RADIX_BITS;
+    int at = b0;
+    for (int i = 0; i < np; ++i) {
+      const int left = b1 - at, passes_left = np - i;
+      const int b = (left + passes_left - 1) / passes_left;
+      p.shift[p.num_passes] = at;
+      p.bits[p.num_passes] = b;
+      ++p.num_passes;
+      at += b;
+    }
+  };
+  seg(begin_bit, end_bit < 32 ? end_bit : (begin_bit < 32 ? 32 : begin_bit));
+  seg(begin_bit > 32 ? begin_bit : 32, end_bit);
   return p;
 }
 
-// Lanes of the warp holding the same digit as the caller. One vote.ballot per digit bit:
-// on sm_100a MATCH.ANY runs on the address-divergence unit at ~64 cycles per warp
-// instruction per SM and caps a sort pass near 40% of HBM bandwidth (profiles/), while
-// ballots issue on the regular pipes. `bits` is warp-uniform.
-__device__ __forceinline__ uint32_t digit_peers(uint32_t d, int bits) {
+// Lanes of the warp holding the same digit as the caller: one vote.ballot per digit bit.
+// On sm_100a MATCH.ANY runs on the address-divergence unit at ~64 cycles per warp
+// instruction per SM and capped a sort pass near 40% of HBM bandwidth (profiles/), while
+// ballots issue on the regular pipes.
+template <int BITS>
+__device__ __forceinline__ uint32_t digit_peers(uint32_t d) {
   uint32_t peers = 0xffffffffu;
 #pragma unroll
-  for (int b = 0; b < OS_RADIX_BITS; ++b) {
-    if (b < bits) {
-      const bool one = (d >> b) & 1u;
-      const uint32_t m = __ballot_sync(0xffffffffu, one);
-      peers &= one ? m : ~m;
-    }
+  for (int b = 0; b < BITS; ++b) {
+    // 4 instructions per bit: test (LOP3 with predicate out), ballot, select, and-xor
+    asm("{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .b32 t, m, x;\n\t"
+        "and.b32 t, %1, %2;\n\t"
+        "setp.ne.u32 p, t, 0;\n\t"
+        "vote.sync.ballot.b32 m, p, 0xffffffff;\n\t"
+        "selp.b32 x, 0, -1, p;\n\t"
+        "lop3.b32 %0, %0, m, x, 0x60;\n\t"   // peers & (m ^ x)
+        "}"
+        : "+r"(peers)
+        : "r"(d), "r"(1u << b));
   }
   return peers;
 }
@@ -77,10 +92,10 @@ onesweep_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n, const _
 #pragma unroll
     for (int u = 0; u < HIST_ITEMS; ++u) {
       const bool ok = base + (uint64_t)u * HIST_THREADS + threadIdx.x < n;
+      const uint32_t live = __ballot_sync(0xffffffffu, ok);
       for (int p = 0; p < plan.num_passes; ++p) {
         const uint32_t d = (uint32_t)(k[u] >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
-        const uint32_t live = __ballot_sync(0xffffffffu, ok);
-        const uint32_t peers = digit_peers(d, plan.bits[p]) & live;
+        const uint32_t peers = digit_peers<OS_RADIX_BITS>(d) & live;
         if (ok && (peers & lt) == 0) atomicAdd(&s_hist[p * OS_RADIX + d], (uint32_t)__popc(peers));
       }
     }
@@ -112,139 +127,180 @@ onesweep_scan_hist_kernel(uint32_t* __restrict__ hist) {
   h[threadIdx.x] = wex + incl - v;
 }
 
-// ---- one digit pass -------------------------------------------------------------------
-template <int THREADS, int ITEMS>
-struct OnesweepSmem {
+// ---- the ranking core shared by every digit pass ----------------------------------------
+// A tile of THREADS*ITEMS elements is held warp-striped: warp w owns ITEMS*32 consecutive
+// elements, lane l its elements l, l+32, ... (so a "row" j of a warp is 32 consecutive
+// elements). rank() turns the per-element digits into tile-local sorted positions and
+// resolves, by decoupled look-back over earlier tiles, where each digit's run starts in the
+// output. Stable: earlier rows, lower lanes, lower warps, earlier tiles come first.
+template <int THREADS, int ITEMS, int BITS>
+struct RadixCore {
   static constexpr int WARPS = THREADS / 32;
   static constexpr int TILE = THREADS * ITEMS;
-  uint64_t keys[TILE];
-  uint32_t vals[TILE];
-  uint32_t warp_hist[WARPS * OS_RADIX];  // per-warp digit counts, then per-warp exclusive offsets
-  uint32_t bin_start[OS_RADIX];          // tile-local start of each digit in sorted order
-  uint32_t out_base[OS_RADIX];           // global index of the digit's first key MINUS bin_start
-  uint32_t warp_sums[OS_RADIX / 32];
-  uint32_t tile;
+  static constexpr int RADIX = 1 << BITS;
+  static constexpr int DWARPS = (RADIX + 31) / 32;  // warps that hold the digit threads
+  static_assert(THREADS >= RADIX && TILE < 65536, "digit threads / u16 positions");
+
+  struct Smem {
+    uint32_t warp_off[WARPS * RADIX];  // per-warp digit counts -> tile-local start of (warp, digit)
+    uint32_t out_base[RADIX];          // output index of the digit's run MINUS its tile-local start
+    uint32_t warp_sums[DWARPS];
+    uint32_t tile;
+  };
+
+  __device__ static __forceinline__ uint32_t take_ticket(Smem& s, uint32_t* ticket) {
+    if (threadIdx.x == 0) s.tile = atomicAdd(ticket, 1u);
+    for (int k = threadIdx.x; k < WARPS * RADIX; k += THREADS) s.warp_off[k] = 0;
+    __syncthreads();
+    return s.tile;
+  }
+
+  // In: dp[j] = digit of the thread's j-th element (padding elements carry RADIX-1 and must
+  // be the last elements of the tile). Out: dp[j] = digit | tile-local sorted position << 8
+  // (packed to save registers). Ends with a __syncthreads(); afterwards
+  // s.out_base[digit] + position is the element's output index.
+  __device__ static __forceinline__ void rank(Smem& s, uint32_t tile, uint32_t (&dp)[ITEMS],
+                                              const uint32_t* __restrict__ hist_excl,
+                                              uint64_t* __restrict__ lookback) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    uint32_t* wh = s.warp_off + warp * RADIX;
+    const uint32_t lt = lanemask_lt();
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const uint32_t d = dp[j];
+      const uint32_t peers = digit_peers<BITS>(d);
+      const uint32_t before = wh[d];
+      __syncwarp();
+      if ((peers & lt) == 0) wh[d] = before + __popc(peers);
+      __syncwarp();
+      dp[j] = d | ((before + __popc(peers & lt)) << 8);
+    }
+    __syncthreads();
+
+    if (tid < DWARPS * 32) {  // whole warps, so the shuffles and the named barrier are uniform
+      const bool live = tid < RADIX;
+      // digit thread: exclusive scan of the warp counts over warps -> the tile's digit count
+      uint32_t tile_count = 0;
+      if (live) {
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) tile_count += s.warp_off[w * RADIX + tid];
+      }
+      // publish this tile's digit count before anything else: later tiles look back at it
+      uint64_t* my = lookback + (uint64_t)tile * RADIX + tid;
+      if (live) st_relaxed_u64(my, (tile == 0 ? LB_FLAG_PREFIX : LB_FLAG_AGG) | tile_count);
+      // exclusive scan of the tile counts over digits -> tile-local bin starts
+      uint32_t incl = tile_count;
+#pragma unroll
+      for (int k = 1; k < 32; k <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, k);
+        if (lane >= k) incl += t;
+      }
+      if (lane == 31) s.warp_sums[warp] = incl;
+      asm volatile("bar.sync 1, %0;" ::"n"(DWARPS * 32));
+      uint32_t start = incl - tile_count;
+#pragma unroll
+      for (int w = 0; w < DWARPS; ++w)
+        if (w < (int)warp) start += s.warp_sums[w];
+      if (live) {
+        uint32_t run = start;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) {
+          const uint32_t c = s.warp_off[w * RADIX + tid];
+          s.warp_off[w * RADIX + tid] = run;
+          run += c;
+        }
+        // resolve the exclusive prefix of this digit over earlier tiles
+        uint32_t excl = 0;
+        if (tile != 0) {
+          int64_t p = (int64_t)tile - 1;
+          while (true) {
+            const uint64_t v = ld_relaxed_u64(lookback + (uint64_t)p * RADIX + tid);
+            const uint64_t flag = v & LB_FLAG_MASK;
+            if (flag == 0) continue;  // that tile holds an earlier ticket: it is running
+            excl += (uint32_t)v;
+            if (flag == LB_FLAG_PREFIX) break;
+            --p;
+          }
+          st_relaxed_u64(my, LB_FLAG_PREFIX | (uint64_t)(uint32_t)(excl + tile_count));
+        }
+        s.out_base[tid] = hist_excl[tid] + excl - start;  // mod 2^32 (n < 2^32)
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) dp[j] += wh[dp[j] & 0xFFu] << 8;
+  }
 };
 
-// Keys of a tile are read warp-striped (warp w owns ITEMS*32 consecutive keys, lane l its
-// elements l, l+32, ...), ranked inside the warp with ballots (stable: earlier rounds and
-// lower lanes come first), combined across warps per digit, resolved against earlier
-// tiles by look-back, re-ordered through shared memory and written out in digit runs so
-// that stores are coalesced.
-template <int THREADS, int ITEMS>
-__global__ void __launch_bounds__(THREADS, 2)
+// ---- one digit pass over (u64 key, u32 value) pairs --------------------------------------
+template <int THREADS, int ITEMS, int BITS>
+struct OnesweepSmem {
+  typename RadixCore<THREADS, ITEMS, BITS>::Smem core;
+  uint64_t keys[THREADS * ITEMS];
+  uint32_t vals[THREADS * ITEMS];
+};
+
+// The digit is bits [shift32, shift32+BITS) of the key's upper (HI = 1) or lower 32-bit
+// half (make_sort_plan never lets a pass straddle bit 32). Elements are re-ordered through
+// shared memory and written out in digit runs so that stores are coalesced.
+template <int THREADS, int ITEMS, int BITS, int MINB, int HI>
+__global__ void __launch_bounds__(THREADS, MINB)
 onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
-                     uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint64_t n,
-                     int shift, int bits, const uint32_t* __restrict__ hist_excl /* [256] this pass */,
-                     uint64_t* __restrict__ lookback /* [tiles][256], zeroed */,
+                     uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint32_t n,
+                     int shift32, const uint32_t* __restrict__ hist_excl /* [256] this pass */,
+                     uint64_t* __restrict__ lookback /* [tiles][1 << BITS], zeroed */,
                      uint32_t* __restrict__ ticket /* zeroed */) {
-  using Smem = OnesweepSmem<THREADS, ITEMS>;
-  constexpr int WARPS = Smem::WARPS;
-  constexpr int TILE = Smem::TILE;
+  using Core = RadixCore<THREADS, ITEMS, BITS>;
+  constexpr int TILE = Core::TILE;
+  constexpr uint32_t MASK = (1u << BITS) - 1u;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem& s = *reinterpret_cast<Smem*>(smem_raw);
+  OnesweepSmem<THREADS, ITEMS, BITS>& s = *reinterpret_cast<OnesweepSmem<THREADS, ITEMS, BITS>*>(smem_raw);
 
-  const uint32_t tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
-  if (tid == 0) s.tile = atomicAdd(ticket, 1u);
-  for (int k = tid; k < WARPS * OS_RADIX; k += THREADS) s.warp_hist[k] = 0;
-  __syncthreads();
-  const uint32_t tile = s.tile;
-  const uint64_t tile_base = (uint64_t)tile * TILE;
-  const uint32_t tile_n = (uint32_t)min((uint64_t)TILE, n - tile_base);
-  const uint32_t mask = (1u << bits) - 1u;
+  const uint32_t tile = Core::take_ticket(s.core, ticket);
+  const uint32_t tile_base = tile * TILE;
+  const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
+  const uint32_t tid = threadIdx.x;
+  const uint32_t wbase = (tid >> 5) * (ITEMS * 32) + (tid & 31u);
 
-  // 1. load (warp-striped); padding keys are all-ones: they rank after every real key of
-  //    the last digit and are never written
-  const uint32_t wbase = warp * (ITEMS * 32) + lane;
+  // load (warp-striped); padding keys are all-ones: they rank after every real key of the
+  // last digit and are never written
+  const uint64_t* kp = keys_in + tile_base + wbase;
+  const uint32_t* vp = vals_in + tile_base + wbase;
   uint64_t key[ITEMS];
   uint32_t val[ITEMS];
+  if (tile_n == TILE) {
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) key[j] = __ldcs(kp + j * 32);
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) val[j] = __ldcs(vp + j * 32);
+  } else {
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const bool ok = wbase + j * 32 < tile_n;
+      key[j] = ok ? __ldcs(kp + j * 32) : ~0ull;
+      val[j] = ok ? __ldcs(vp + j * 32) : 0u;
+    }
+  }
+  uint32_t dp[ITEMS];
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
-    const uint32_t li = wbase + j * 32;
-    key[j] = li < tile_n ? __ldcs(keys_in + tile_base + li) : ~0ull;
+    const uint32_t w = HI ? (uint32_t)(key[j] >> 32) : (uint32_t)key[j];
+    dp[j] = (w >> shift32) & MASK;
   }
-#pragma unroll
-  for (int j = 0; j < ITEMS; ++j) {
-    const uint32_t li = wbase + j * 32;
-    val[j] = li < tile_n ? __ldcs(vals_in + tile_base + li) : 0u;
-  }
+  Core::rank(s.core, tile, dp, hist_excl, lookback);
 
-  // 2. rank inside the warp
-  uint32_t* wh = s.warp_hist + warp * OS_RADIX;
-  uint16_t rank[ITEMS];
-  const uint32_t lt = lanemask_lt();
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
-    const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
-    const uint32_t peers = digit_peers(d, bits);
-    const uint32_t before = wh[d];
-    __syncwarp();
-    if ((peers & lt) == 0) wh[d] = before + __popc(peers);
-    __syncwarp();
-    rank[j] = (uint16_t)(before + __popc(peers & lt));
+    s.keys[dp[j] >> 8] = key[j];
+    s.vals[dp[j] >> 8] = val[j];
   }
   __syncthreads();
 
-  // 3. per digit: exclusive scan of the warp counts over warps -> tile count
-  uint32_t tile_count = 0;
-  if (tid < OS_RADIX) {
-#pragma unroll
-    for (int w = 0; w < WARPS; ++w) {
-      const uint32_t c = s.warp_hist[w * OS_RADIX + tid];
-      s.warp_hist[w * OS_RADIX + tid] = tile_count;
-      tile_count += c;
-    }
-    // 4. publish the tile's digit count, then resolve the exclusive prefix over earlier tiles
-    uint64_t* my = lookback + (uint64_t)tile * OS_RADIX + tid;
-    uint64_t excl = 0;
-    if (tile == 0) {
-      st_relaxed_u64(my, LB_FLAG_PREFIX | tile_count);
-    } else {
-      st_relaxed_u64(my, LB_FLAG_AGG | tile_count);
-      int64_t p = (int64_t)tile - 1;
-      while (true) {
-        const uint64_t v = ld_relaxed_u64(lookback + (uint64_t)p * OS_RADIX + tid);
-        const uint64_t flag = v & LB_FLAG_MASK;
-        if (flag == 0) continue;  // that tile holds an earlier ticket: it is running
-        excl += v & LB_VALUE_MASK;
-        if (flag == LB_FLAG_PREFIX) break;
-        --p;
-      }
-      st_relaxed_u64(my, LB_FLAG_PREFIX | (excl + tile_count));
-    }
-    // 5. exclusive scan of the tile counts over digits -> local bin starts
-    uint32_t incl = tile_count;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
-      if (lane >= d) incl += t;
-    }
-    if (lane == 31) s.warp_sums[warp] = incl;
-    // warps 0..7 hold the digits; they meet at a named barrier of 256 threads
-    asm volatile("bar.sync 1, %0;" ::"n"(OS_RADIX));
-    uint32_t wex = 0;
-    for (uint32_t w = 0; w < warp; ++w) wex += s.warp_sums[w];
-    const uint32_t start = wex + incl - tile_count;
-    s.bin_start[tid] = start;
-    s.out_base[tid] = hist_excl[tid] + (uint32_t)excl - start;  // mod 2^32; n < 2^32
-  }
-  __syncthreads();
-
-  // 6. scatter into shared memory in sorted order
-#pragma unroll
-  for (int j = 0; j < ITEMS; ++j) {
-    const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
-    const uint32_t p = s.bin_start[d] + wh[d] + rank[j];
-    s.keys[p] = key[j];
-    s.vals[p] = val[j];
-  }
-  __syncthreads();
-
-  // 7. coalesced write-out of digit runs (real keys occupy local positions [0, tile_n))
+  // coalesced write-out of digit runs (real keys occupy local positions [0, tile_n))
   for (uint32_t p = tid; p < tile_n; p += THREADS) {
     const uint64_t k = s.keys[p];
-    const uint32_t d = (uint32_t)(k >> shift) & mask;
-    const uint32_t o = s.out_base[d] + p;
+    const uint32_t w = HI ? (uint32_t)(k >> 32) : (uint32_t)k;
+    const uint32_t o = s.core.out_base[(w >> shift32) & MASK] + p;
     keys_out[o] = k;
     vals_out[o] = s.vals[p];
   }

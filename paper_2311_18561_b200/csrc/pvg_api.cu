@@ -85,10 +85,16 @@ struct KernelRec {
   cudaEvent_t e0, e1;
 };
 
-constexpr int OS_THREADS = 384;
-constexpr int OS_ITEMS = 16;
-constexpr int OS_TILE = OS_THREADS * OS_ITEMS;
-using OsSmem = OnesweepSmem<OS_THREADS, OS_ITEMS>;
+// Two tile shapes of the onesweep pass: large tiles amortise the look-back for the
+// instance sort, small ones give the n-key depth sort enough CTAs to fill 148 SMs.
+#ifndef PVG_OSL_THREADS
+#define PVG_OSL_THREADS 384
+#define PVG_OSL_ITEMS 16
+#define PVG_OSL_MINB 2
+#endif
+struct OsLarge { static constexpr int THREADS = PVG_OSL_THREADS, ITEMS = PVG_OSL_ITEMS, MINB = PVG_OSL_MINB; };
+struct OsSmall { static constexpr int THREADS = 256, ITEMS = 8, MINB = 4; };
+constexpr uint64_t OS_SMALL_BELOW = 8u << 20;
 
 // scratch of one sort call
 struct SortScratch {
@@ -135,13 +141,34 @@ struct Timer {
   }
 };
 
-int onesweep_configure() {
-  static bool done = false;
-  if (done) return PVG_OK;
-  CU(cudaFuncSetAttribute(onesweep_pass_kernel<OS_THREADS, OS_ITEMS>,
-                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OsSmem)));
-  done = true;
+template <class Cfg, int BITS, int HI>
+int launch_pass_bits(const uint64_t* kin, const uint32_t* vin, uint64_t* kout, uint32_t* vout, uint32_t n, int shift,
+                     const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
+  using Smem = OnesweepSmem<Cfg::THREADS, Cfg::ITEMS, BITS>;
+  auto kern = onesweep_pass_kernel<Cfg::THREADS, Cfg::ITEMS, BITS, Cfg::MINB, HI>;
+  static bool configured = false;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
+    configured = true;
+  }
+  constexpr uint32_t TILE = Cfg::THREADS * Cfg::ITEMS;
+  const uint32_t tiles = (n + TILE - 1) / TILE;
+  kern<<<tiles, Cfg::THREADS, sizeof(Smem), st>>>(kin, vin, kout, vout, n, shift & 31, hist, lookback, ticket);
   return PVG_OK;
+}
+
+template <class Cfg>
+int launch_pass(int bits, const uint64_t* kin, const uint32_t* vin, uint64_t* kout, uint32_t* vout, uint32_t n, int shift,
+                const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
+  switch (bits) {
+#define PVG_CASE(B)                                                                                              \
+  case B:                                                                                                        \
+    return shift >= 32 ? launch_pass_bits<Cfg, B, 1>(kin, vin, kout, vout, n, shift, hist, lookback, ticket, st) \
+                       : launch_pass_bits<Cfg, B, 0>(kin, vin, kout, vout, n, shift, hist, lookback, ticket, st);
+    PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
+#undef PVG_CASE
+    default: return PVG_ERR_BAD_OPTION;
+  }
 }
 
 // Stable LSD sort of n pairs on key bits [begin_bit, end_bit). Buffers ping-pong; *result
@@ -151,9 +178,10 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
                  bool hist_ready = false) {
   *result = 0;
   if (n == 0 || end_bit <= begin_bit) return PVG_OK;
-  TRY(onesweep_configure());
   const SortPlan plan = make_sort_plan(begin_bit, end_bit);
-  const uint64_t tiles = (n + OS_TILE - 1) / OS_TILE;
+  const bool small = n < OS_SMALL_BELOW;
+  const uint64_t tile_sz = small ? OsSmall::THREADS * OsSmall::ITEMS : OsLarge::THREADS * OsLarge::ITEMS;
+  const uint64_t tiles = (n + tile_sz - 1) / tile_sz;
   TRY(sc.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
   TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
   TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, st, 1.25));
@@ -178,9 +206,11 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   uint64_t* kin = ka; uint32_t* vin = va; uint64_t* kout = kb; uint32_t* vout = vb;
   for (int p = 0; p < plan.num_passes; ++p) {
     if (tm) TRY(tm->begin("onesweep_pass", stage, st));
-    onesweep_pass_kernel<OS_THREADS, OS_ITEMS><<<(unsigned)tiles, OS_THREADS, sizeof(OsSmem), st>>>(
-        kin, vin, kout, vout, n, plan.shift[p], plan.bits[p], sc.hist.as<uint32_t>() + p * OS_RADIX,
-        sc.lookback.as<uint64_t>() + (size_t)p * tiles * OS_RADIX, sc.tickets.as<uint32_t>() + p);
+    const uint32_t* hist = sc.hist.as<uint32_t>() + p * OS_RADIX;
+    uint64_t* lb = sc.lookback.as<uint64_t>() + (size_t)p * tiles * OS_RADIX;
+    uint32_t* tk = sc.tickets.as<uint32_t>() + p;
+    if (small) TRY(launch_pass<OsSmall>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st));
+    else TRY(launch_pass<OsLarge>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st));
     if (tm) TRY(tm->end(st));
     std::swap(kin, kout);
     std::swap(vin, vout);
