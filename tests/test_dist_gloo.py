@@ -1,0 +1,68 @@
+"""N > 1 host logic on CPU: world_size-2 gloo processes exercise the frame schedule (frames
+sharded over ranks, no data-path collective) and the barrier / max-over-ranks timing that
+bench.py uses. The render itself needs a GPU and is covered by the -m gpu tests."""
+import os
+import socket
+import sys
+
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank: int, world: int, port: int, steps: int, out_q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    from paper_2311_18561_b200 import dist
+    r, lr, ws = dist.init("gloo")
+    assert (r, lr, ws) == (rank, rank, world)
+    frames = [("cam", k / 49.0) for k in range(50)]
+    sched = dist.frame_schedule(rank, ws, steps, frames)
+    dist.barrier()
+    elapsed = 0.010 * (rank + 1)                      # rank 1 is the slow one
+    mx = dist.max_over_ranks(elapsed)
+    total = dist.sum_over_ranks(len(sched))
+    out_q.put((rank, [f[1] for f in sched], mx, total))
+    dist.barrier()
+    dist.shutdown()
+
+
+def test_frame_sharding_and_max_timing_world2():
+    world, steps = 2, 30
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, steps, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    ts0, ts1 = res[0][1], res[1][1]
+    frames = [k / 49.0 for k in range(50)]
+    # weak scaling: every rank renders `steps` frames; together they walk the sweep in order
+    assert len(ts0) == len(ts1) == steps
+    inter = [t for pair in zip(ts0, ts1) for t in pair]
+    assert inter == [frames[f % 50] for f in range(world * steps)]
+    assert set(ts0).isdisjoint(ts1[:25])              # no frame rendered twice within one sweep
+    # the timed region's duration is the max over ranks; the frame count is summed
+    assert abs(res[0][2] - 0.020) < 1e-12 and abs(res[1][2] - 0.020) < 1e-12
+    assert res[0][3] == res[1][3] == world * steps
+
+
+def test_single_process_defaults():
+    sys.path.insert(0, ROOT)
+    from paper_2311_18561_b200 import dist
+    for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE"):
+        os.environ.pop(k, None)
+    assert dist.world() == (0, 0, 1)
+    assert dist.max_over_ranks(1.5) == 1.5
+    assert dist.frame_schedule(0, 1, 3, ["a", "b"]) == ["a", "b", "a"]
