@@ -11,6 +11,7 @@
 #include "../../include/pvg.h"
 #include "blend.cuh"
 #include "common.cuh"
+#include "expand.cuh"
 #include "onesweep.cuh"
 #include "preprocess.cuh"
 #include "ranges.cuh"
@@ -422,7 +423,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
   CU(cudaMemcpyAsync(s->h_total, total, 8, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));  // the one host read-back: M sizes the instance buffers
   const uint64_t M = *s->h_total;
-  if (M >= (1ull << 32)) return PVG_ERR_INSTANCE_OVERFLOW;
+  if (M >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
   s->M = M;
 
   s->sorted_side = 0;
@@ -433,9 +434,9 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
     }
     // a2 emit
     TRY(tm.begin("duplicate", PVG_STAGE_DUPLICATE, st));
-    duplicate_kernel<<<(unsigned)((M + DUP_CHUNK - 1) / DUP_CHUNK), DUP_THREADS, 0, st>>>(
-        n, M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x,
-        s->keys[0].as<uint64_t>(), s->vals[0].as<uint32_t>());
+    expand_kernel<false><<<(unsigned)((M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
+        n, (uint32_t)M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x,
+        s->keys[0].as<uint64_t>(), nullptr, s->vals[0].as<uint32_t>());
     TRY(tm.end(st));
     if (s->keep_unsorted) {
       TRY(s->keys_unsorted.reserve((size_t)M * 8, st));
