@@ -242,7 +242,7 @@ def run_ours(args):
     e0.record()
     for cam, t in sched:
         scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
-        Ms.append(int(scene.debug_info().num_instances))
+        Ms.append(scene.frame_stats()["M"])
     e1.record()
     torch.cuda.synchronize()
     if sampler:
@@ -305,7 +305,9 @@ def run_ours(args):
     # algorithmic bytes over the timed region, per (kernel, stage)
     alg = {("preprocess", "preprocess"): K * (64.0 * N + 80.0 * N + 192.0 * S),
            ("scan_counts", "duplicate"): K * 12.0 * N,
-           ("duplicate", "duplicate"): 12.0 * Msum,
+           ("duplicate", "duplicate"): (6.0 if any(k[0] == "compact_pass_last" for k in agg) else 12.0) * Msum,
+           ("compact_pass", "sort"): 12.0 * Msum * (agg.get(("compact_pass", "sort"), [0, K])[1] / K),
+           ("compact_pass_last", "sort"): 10.0 * Msum,
            ("onesweep_histogram", "sort"): 8.0 * Msum,
            ("onesweep_pass", "sort"): 0.0,   # filled below: 24 B per instance per launch
            ("onesweep_histogram", "depth_sort"): K * 8.0 * N,

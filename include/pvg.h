@@ -113,13 +113,20 @@ typedef enum pvg_option {
   PVG_OPT_KERNEL_EVENTS = 3,
   /* 1: the blend also counts its (pixel, list entry) evaluations (pvg_blend_counters); measurement
    *    only -- the counting variant is a separate kernel instantiation (default 0). */
-  PVG_OPT_COUNT_PAIRS = 4
+  PVG_OPT_COUNT_PAIRS = 4,
+  /* 1 (default): with PRESORT_DEPTH=1 and at most 65536 tiles, an instance travels through the
+   *    tile-id passes as (u16 tile id, u32 Gaussian index) instead of the 64-bit key + index: its
+   *    depth bits are already in order and would be dead payload. pvg_debug_view rebuilds the
+   *    64-bit keys on demand. 0: always carry the 64-bit keys. Results are identical. */
+  PVG_OPT_COMPACT_KEYS = 5
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 
 /* ---- test and measurement hooks (not part of the paper's problem) ------------------------- */
 
-/* Device views of the last render's intermediates, valid until the next call on the scene. */
+/* Device views of the last render's intermediates, valid until the next call on the scene.
+ * With COMPACT_KEYS in effect this call launches two small kernels that rebuild the 64-bit key
+ * lists and synchronises the stream: a debugging call, not for timed loops (pvg_frame_stats). */
 typedef struct pvg_debug {
   uint64_t n;                    /* points */
   uint64_t num_instances;        /* M = sum of counts */
@@ -153,6 +160,9 @@ int pvg_stage_times_ms(pvg_scene *scene, float ms[PVG_NUM_STAGES]);
  * names (static strings), stage ids and milliseconds; returns the number of launches (>= 0)
  * or a negative pvg_status. */
 int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stages, float *ms);
+
+/* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y}. */
+int pvg_frame_stats(pvg_scene *scene, uint64_t out[4]);
 
 /* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs
  * evaluated before the pixel stopped, out[1] = pairs that contributed (alpha >= 1/255). */

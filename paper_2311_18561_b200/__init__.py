@@ -19,14 +19,14 @@ LIB_PATH = os.environ.get("PVG_LIB") or os.path.join(_HERE, "libpvg.so")   # PVG
 PVG_OK = 0
 STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_BAD_CAMERA",
           -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION"}
-OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS = 1, 2, 3, 4
+OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS = 1, 2, 3, 4, 5
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 
 # every symbol include/pvg.h declares
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
            "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms",
-           "pvg_sort_pairs", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
+           "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
 
 class PvgError(RuntimeError):
@@ -87,6 +87,7 @@ def load_library(path: Optional[str] = None):
                                       C.POINTER(C.c_float)]
     L.pvg_sort_pairs.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                  C.c_void_p]
+    L.pvg_frame_stats.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
     L.pvg_blend_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
     L.pvg_memcpy_d2h.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
     L.pvg_set_allocator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -234,6 +235,12 @@ class Scene:
         if cnt < 0:
             _check(cnt)
         return [(names[i].decode(), STAGES[stages[i]], float(ms[i])) for i in range(min(cnt, cap))]
+
+    def frame_stats(self) -> Dict[str, int]:
+        """Sizes of the last render (no device work)."""
+        out = (C.c_uint64 * 4)()
+        _check(self._L.pvg_frame_stats(self._h, out))
+        return {"n": int(out[0]), "M": int(out[1]), "tiles_x": int(out[2]), "tiles_y": int(out[3])}
 
     def blend_counters(self) -> Tuple[int, int]:
         """(pairs evaluated, pairs contributing) of the last render with OPT_COUNT_PAIRS=1."""

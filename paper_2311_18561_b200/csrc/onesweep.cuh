@@ -306,4 +306,83 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
   }
 }
 
+// ---- digit pass over the compact instance payload -----------------------------------------
+// When the Gaussians were depth-sorted before duplication, the low 32 key bits of the
+// instances are already in order and are dead payload for the remaining tile-id passes, so
+// an instance travels as (u16 tile id, u32 Gaussian index): 6 B instead of 12 B. The LAST
+// pass writes the indices only -- the tile of a position in the sorted list is implied by
+// the tile ranges. (tile << 32 | depth bits) is rebuilt on demand for the debug view.
+template <int THREADS, int ITEMS, int BITS>
+struct CompactSmem {
+  typename RadixCore<THREADS, ITEMS, BITS>::Smem core;
+  uint32_t vals[THREADS * ITEMS];
+  uint16_t tiles[THREADS * ITEMS];
+};
+
+template <int THREADS, int ITEMS, int BITS, int MINB, bool LAST>
+__global__ void __launch_bounds__(THREADS, MINB)
+compact_pass_kernel(const uint16_t* __restrict__ tiles_in, const uint32_t* __restrict__ vals_in,
+                    uint16_t* __restrict__ tiles_out, uint32_t* __restrict__ vals_out, uint32_t n, int shift,
+                    const uint32_t* __restrict__ hist_excl, uint64_t* __restrict__ lookback,
+                    uint32_t* __restrict__ ticket) {
+  using Core = RadixCore<THREADS, ITEMS, BITS>;
+  constexpr int TILE = Core::TILE;
+  constexpr uint32_t MASK = (1u << BITS) - 1u;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  CompactSmem<THREADS, ITEMS, BITS>& s = *reinterpret_cast<CompactSmem<THREADS, ITEMS, BITS>*>(smem_raw);
+
+  const uint32_t tile = Core::take_ticket(s.core, ticket);
+  const uint32_t tile_base = tile * TILE;
+  const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
+  const uint32_t tid = threadIdx.x;
+  const uint32_t wbase = (tid >> 5) * (ITEMS * 32) + (tid & 31u);
+  const uint16_t* tp = tiles_in + tile_base + wbase;
+  const uint32_t* vp = vals_in + tile_base + wbase;
+  uint32_t t[ITEMS], val[ITEMS], dp[ITEMS];
+  if (tile_n == TILE) {
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) t[j] = __ldcs(tp + j * 32);
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) val[j] = __ldcs(vp + j * 32);
+  } else {
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const bool ok = wbase + j * 32 < tile_n;
+      t[j] = ok ? (uint32_t)__ldcs(tp + j * 32) : 0xFFFFu;   // padding ranks last
+      val[j] = ok ? __ldcs(vp + j * 32) : 0u;
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) dp[j] = (t[j] >> shift) & MASK;
+  Core::rank(s.core, tile, dp, hist_excl, lookback);
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    s.tiles[dp[j] >> 8] = (uint16_t)t[j];
+    s.vals[dp[j] >> 8] = val[j];
+  }
+  __syncthreads();
+  for (uint32_t p = tid; p < tile_n; p += THREADS) {
+    const uint32_t tl = s.tiles[p];
+    const uint32_t o = s.core.out_base[(tl >> shift) & MASK] + p;
+    if (!LAST) tiles_out[o] = (uint16_t)tl;
+    vals_out[o] = s.vals[p];
+  }
+}
+
+// debug view: (tile << 32 | depth bits) of the compact payload
+__global__ void __launch_bounds__(256)
+keys_from_tiles16_kernel(const uint16_t* __restrict__ tiles16, const uint32_t* __restrict__ vals,
+                         const uint4* __restrict__ tileinfo, uint32_t M, uint64_t* __restrict__ keys) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < M) keys[i] = ((uint64_t)tiles16[i] << 32) | tileinfo[vals[i]].z;
+}
+
+__global__ void __launch_bounds__(256)
+keys_from_ranges_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
+                        const uint4* __restrict__ tileinfo, uint64_t* __restrict__ keys) {
+  const uint2 r = ranges[blockIdx.x];
+  for (uint32_t i = r.x + threadIdx.x; i < r.y; i += blockDim.x)
+    keys[i] = ((uint64_t)blockIdx.x << 32) | tileinfo[vals[i]].z;
+}
+
 }  // namespace pvg

@@ -221,6 +221,70 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   return PVG_OK;
 }
 
+#ifndef PVG_CP_THREADS
+#define PVG_CP_THREADS 384
+#define PVG_CP_ITEMS 16
+#define PVG_CP_MINB 2
+#endif
+struct CpCfg { static constexpr int THREADS = PVG_CP_THREADS, ITEMS = PVG_CP_ITEMS, MINB = PVG_CP_MINB; };
+
+template <int BITS, bool LAST>
+int launch_compact_bits(const uint16_t* tin, const uint32_t* vin, uint16_t* tout, uint32_t* vout, uint32_t n, int shift,
+                        const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
+  using Smem = CompactSmem<CpCfg::THREADS, CpCfg::ITEMS, BITS>;
+  auto kern = compact_pass_kernel<CpCfg::THREADS, CpCfg::ITEMS, BITS, CpCfg::MINB, LAST>;
+  static bool configured = false;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
+    configured = true;
+  }
+  constexpr uint32_t TILE = CpCfg::THREADS * CpCfg::ITEMS;
+  kern<<<(n + TILE - 1) / TILE, CpCfg::THREADS, sizeof(Smem), st>>>(tin, vin, tout, vout, n, shift, hist, lookback, ticket);
+  return PVG_OK;
+}
+
+// Tile-id passes over the compact (u16 tile, u32 index) payload; histograms come from
+// tile_prefix_kernel. The sorted indices end in v[*result]; t[] ping-pongs alongside.
+int run_compact_sort(uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint32_t* v1, int tile_bits, cudaStream_t st,
+                     SortScratch& sc, Timer* tm, int* result) {
+  *result = 0;
+  if (n == 0) return PVG_OK;
+  const SortPlan plan = make_sort_plan(32, 32 + tile_bits);
+  constexpr uint64_t TILE = CpCfg::THREADS * CpCfg::ITEMS;
+  const uint64_t tiles = (n + TILE - 1) / TILE;
+  TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
+  TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, st, 1.25));
+  CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, st));
+  CU(cudaMemsetAsync(sc.lookback.p, 0, (size_t)plan.num_passes * tiles * OS_RADIX * 8, st));
+  uint16_t* tin = t0; uint32_t* vin = v0; uint16_t* tout = t1; uint32_t* vout = v1;
+  for (int p = 0; p < plan.num_passes; ++p) {
+    const bool last = p == plan.num_passes - 1;
+    const uint32_t* hist = sc.hist.as<uint32_t>() + p * OS_RADIX;
+    uint64_t* lb = sc.lookback.as<uint64_t>() + (size_t)p * tiles * OS_RADIX;
+    uint32_t* tk = sc.tickets.as<uint32_t>() + p;
+    const int shift = plan.shift[p] - 32;
+    if (tm) TRY(tm->begin(last ? "compact_pass_last" : "compact_pass", PVG_STAGE_SORT, st));
+    int rc = PVG_ERR_BAD_OPTION;
+    switch (plan.bits[p]) {
+#define PVG_CASE(B)                                                                                   \
+  case B:                                                                                             \
+    rc = last ? launch_compact_bits<B, true>(tin, vin, tout, vout, n, shift, hist, lb, tk, st)        \
+              : launch_compact_bits<B, false>(tin, vin, tout, vout, n, shift, hist, lb, tk, st);      \
+    break;
+      PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
+#undef PVG_CASE
+      default: break;
+    }
+    TRY(rc);
+    if (tm) TRY(tm->end(st));
+    std::swap(tin, tout);
+    std::swap(vin, vout);
+  }
+  CU(cudaGetLastError());
+  *result = plan.num_passes & 1;
+  return PVG_OK;
+}
+
 }  // namespace
 
 struct pvg_scene {
@@ -229,13 +293,15 @@ struct pvg_scene {
   int sh_degree = 3;
   cudaStream_t stream = nullptr;
   // options
-  int presort = 1, keep_unsorted = 0, count_pairs = 0;
+  int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1;
+  bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
   // model (SoA)
   Buf A0, A1, A2, A3, SH;
   // per-Gaussian workspace
   Buf record, tileinfo, counts, offsets, dkeys[2], dvals[2], scan_status, small;  // small: ticket u32 @0, total u64 @8
   // per-instance workspace
   Buf keys[2], vals[2], keys_unsorted, vals_unsorted;
+  Buf tiles16[2], tiles16_unsorted;
   Buf ranges, tilegrid;
   Buf img;  // render_host device images
   SortScratch sort_n, sort_m;
@@ -260,7 +326,7 @@ int ceil_log2(uint32_t v) {
 void release_all(pvg_scene* s) {
   Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
-                 &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted,
+                 &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->ranges, &s->tilegrid, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
@@ -427,7 +493,29 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
   s->M = M;
 
   s->sorted_side = 0;
-  if (M > 0) {
+  const bool compact = s->presort && s->compact && tile_bits <= 16;
+  s->compact_used = compact;
+  if (M > 0 && compact) {
+    for (int k = 0; k < 2; ++k) {
+      TRY(s->tiles16[k].reserve((size_t)M * 2, st, 1.125));
+      TRY(s->vals[k].reserve((size_t)M * 4, st, 1.125));
+    }
+    TRY(tm.begin("duplicate", PVG_STAGE_DUPLICATE, st));
+    expand_kernel<true><<<(unsigned)((M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
+        n, (uint32_t)M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x, nullptr,
+        s->tiles16[0].as<uint16_t>(), s->vals[0].as<uint32_t>());
+    TRY(tm.end(st));
+    if (s->keep_unsorted) {
+      TRY(s->tiles16_unsorted.reserve((size_t)M * 2, st));
+      TRY(s->vals_unsorted.reserve((size_t)M * 4, st));
+      CU(cudaMemcpyAsync(s->tiles16_unsorted.p, s->tiles16[0].p, (size_t)M * 2, cudaMemcpyDeviceToDevice, st));
+      CU(cudaMemcpyAsync(s->vals_unsorted.p, s->vals[0].p, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    int side = 0;
+    TRY(run_compact_sort((uint32_t)M, s->tiles16[0].as<uint16_t>(), s->vals[0].as<uint32_t>(),
+                         s->tiles16[1].as<uint16_t>(), s->vals[1].as<uint32_t>(), tile_bits, st, s->sort_m, &tm, &side));
+    s->sorted_side = side;
+  } else if (M > 0) {
     for (int k = 0; k < 2; ++k) {
       TRY(s->keys[k].reserve((size_t)M * 8, st, 1.125));
       TRY(s->vals[k].reserve((size_t)M * 4, st, 1.125));
@@ -546,6 +634,7 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
   switch (option) {
     case PVG_OPT_PRESORT_DEPTH: scene->presort = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KEEP_UNSORTED: scene->keep_unsorted = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_COMPACT_KEYS: scene->compact = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_COUNT_PAIRS: scene->count_pairs = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KERNEL_EVENTS:
       scene->timer.enabled = value != 0;
@@ -596,12 +685,29 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->counts = s->counts.as<uint32_t>();
   out->visit_order = s->presort ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
+  if (s->compact_used && s->M) {
+    // rebuild (tile << 32 | depth bits) from the compact payload: debug only
+    cudaStream_t st = s->stream;
+    const uint32_t M32 = (uint32_t)s->M;
+    TRY(s->keys[0].reserve((size_t)s->M * 8, st));
+    keys_from_ranges_kernel<<<s->tiles_x * s->tiles_y, 256, 0, st>>>(s->ranges.as<uint2>(),
+                                                                      s->vals[s->sorted_side].as<uint32_t>(),
+                                                                      s->tileinfo.as<uint4>(), s->keys[0].as<uint64_t>());
+    if (s->keep_unsorted) {
+      TRY(s->keys_unsorted.reserve((size_t)s->M * 8, st));
+      keys_from_tiles16_kernel<<<(M32 + 255) / 256, 256, 0, st>>>(s->tiles16_unsorted.as<uint16_t>(),
+                                                                 s->vals_unsorted.as<uint32_t>(), s->tileinfo.as<uint4>(),
+                                                                 M32, s->keys_unsorted.as<uint64_t>());
+    }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+  }
   if (s->keep_unsorted && s->M) {
     out->keys_unsorted = s->keys_unsorted.as<uint64_t>();
     out->vals_unsorted = s->vals_unsorted.as<uint32_t>();
   }
   if (s->M) {
-    out->keys_sorted = s->keys[s->sorted_side].as<uint64_t>();
+    out->keys_sorted = s->keys[s->compact_used ? 0 : s->sorted_side].as<uint64_t>();
     out->vals_sorted = s->vals[s->sorted_side].as<uint32_t>();
   }
   out->ranges = s->ranges.as<uint32_t>();
@@ -637,6 +743,15 @@ int pvg_stage_times_ms(pvg_scene* s, float ms[PVG_NUM_STAGES]) {
       if (r.stage == k) { if (!first) first = &r; last = &r; }
     if (first) CU(cudaEventElapsedTime(&ms[k], first->e0, last->e1));
   }
+  return PVG_OK;
+}
+
+int pvg_frame_stats(pvg_scene* s, uint64_t out[4]) {
+  if (!s || !out) return PVG_ERR_NULL;
+  out[0] = s->n;
+  out[1] = s->rendered ? s->M : 0;
+  out[2] = s->tiles_x;
+  out[3] = s->tiles_y;
   return PVG_OK;
 }
 

@@ -15,13 +15,14 @@ from workloads import make_config, pinhole_camera
 pytestmark = pytest.mark.gpu
 
 
-def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None):
+def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None, compact=True):
     """(P), (I), (R) for one frame. Returns the stats of the three comparisons."""
     own = scene is None
     sc = scene or pvg.Scene.from_workload_scene(wl_scene)
     try:
         sc.set_option(pvg.OPT_PRESORT_DEPTH, 1 if presort else 0)
         sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
+        sc.set_option(pvg.OPT_COMPACT_KEYS, 1 if compact else 0)
         rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t))
         dbg = sc.debug()
     finally:
@@ -61,6 +62,12 @@ def test_cfg1_mid_scene():
 def test_cfg1_full_width_sort_mode_matches():
     wl = make_config(1, n=60_000)
     full_parity(wl.scene, wl.cameras[0], 0.5, presort=False, end_to_end=False)
+
+
+def test_cfg1_presort_with_64bit_keys_matches():
+    """PRESORT_DEPTH=1 but COMPACT_KEYS=0: the tile-id passes carry the full 64-bit keys."""
+    wl = make_config(1, n=60_000)
+    full_parity(wl.scene, wl.cameras[0], 0.5, compact=False, end_to_end=False)
 
 
 def test_cfg2_mix_reduced_full_resolution():
