@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--presort", type=int, default=1)
+    ap.add_argument("--block-bins", type=int, default=1)
     return ap.parse_args()
 
 
@@ -216,6 +217,7 @@ def run_ours(args):
     warm = dist.frame_schedule(rank, ws, max(args.warmup, 3), frames)
     scene = pvg.Scene.from_workload_scene(wl.scene)
     scene.set_option(pvg.OPT_PRESORT_DEPTH, args.presort)
+    scene.set_option(pvg.OPT_BLOCK_BINS, args.block_bins)
     cams = {id(c): pvg.camera_struct(c) for c, _ in frames}
 
     def outs(c):
@@ -234,7 +236,7 @@ def run_ours(args):
     time.sleep(0.3 if sampler else 0.0)
     scene.set_option(pvg.OPT_KERNEL_EVENTS, 2)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    Ms = []
+    Ms, Mbs = [], []
     dist.barrier(local_rank)
     torch.cuda.synchronize()
     if sampler:
@@ -242,7 +244,9 @@ def run_ours(args):
     e0.record()
     for cam, t in sched:
         scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
-        Ms.append(scene.frame_stats()["M"])
+        fs = scene.frame_stats()
+        Ms.append(fs["M"])
+        Mbs.append(fs["block_entries"])
     e1.record()
     torch.cuda.synchronize()
     if sampler:
@@ -295,8 +299,10 @@ def run_ours(args):
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     N = wl.scene.n
     S = int((scene.debug(["counts"])["counts"] > 0).sum())
-    Msum = float(sum(Ms))
+    Msum, Mbsum = float(sum(Ms)), float(sum(Mbs))
     K = len(sched)
+    list_mode = scene.frame_stats()["list_mode"]
+    chunks = Mbsum / 512 + K * 150
     agg = {}
     for name, stage, ms in krecs:
         a = agg.setdefault((name, stage), [0.0, 0])
@@ -304,7 +310,14 @@ def run_ours(args):
         a[1] += 1
     # algorithmic bytes over the timed region, per (kernel, stage)
     alg = {("preprocess", "preprocess"): K * (64.0 * N + 80.0 * N + 192.0 * S),
-           ("scan_counts", "duplicate"): K * 12.0 * N,
+           ("scan_counts", "duplicate"): K * (24.0 if list_mode == "blocks" else 12.0) * N,
+           # block-entry path (blockbin.cuh): 13 B entries (u8 block, u32 Gaussian, u64 mask)
+           ("bin_expand", "duplicate"): 13.0 * Mbsum + K * 24.0 * S,
+           ("bin_hist", "sort"): 1.0 * Mbsum,
+           ("bin_pass", "sort"): 25.0 * Mbsum,
+           ("bin_count", "sort"): 8.0 * Mbsum + 256.0 * chunks,
+           ("bin_chunk_scan", "sort"): 512.0 * chunks,
+           ("bin_write", "sort"): 12.0 * Mbsum + 4.0 * Msum + 256.0 * chunks,
            ("duplicate", "duplicate"): (6.0 if any(k[0] == "compact_pass_last" for k in agg) else 12.0) * Msum,
            ("compact_pass", "sort"): 12.0 * Msum * (agg.get(("compact_pass", "sort"), [0, K])[1] / K),
            ("compact_pass_last", "sort"): 10.0 * Msum,
@@ -344,7 +357,7 @@ def run_ours(args):
                     "frac": dk["alu_frac"], "traffic": ncu_traffic("blend", workload), "kernel": "blend_kernel",
                     "peak_source": f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (observed)"}
     else:
-        roofline = {"bound": "hbm", "achieved": dk["GBps"], "peak": hbm_peak, "unit": "GB/s", "frac": dk["hbm_frac"],
+        roofline = {"bound": "hbm", "achieved": dk.get("GBps"), "peak": hbm_peak, "unit": "GB/s", "frac": dk.get("hbm_frac"),
                     "traffic": ncu_traffic(dom[0], workload), "kernel": f"{dom[0]} ({dom[1]} stage)",
                     "peak_source": peak_src, "avg_launch_ms": dk["ms_avg"],
                     "algorithmic_bytes_per_launch": alg[dom] / agg[dom][1]}
@@ -367,7 +380,8 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload, "n_gaussians": N, "survivors_last_frame": S,
                        "resolution": f"{frames[0][0].width}x{frames[0][0].height}",
-                       "instances_per_frame_mean": Msum / K, "frames": "one (camera, t) per step, round-robin over the sweep",
+                       "instances_per_frame_mean": Msum / K, "block_entries_per_frame_mean": Mbsum / K,
+                       "list_mode": list_mode, "frames": "one (camera, t) per step, round-robin over the sweep",
                        "l2_policy": f"inputs larger than L2: model {N * 256 / 1e6:.0f} MB + instance lists {24 * Msum / K / 1e6:.0f} MB "
                                     "per frame vs 126 MB L2",
                        "parallelism": f"frames sharded over {ws} rank(s), no collective", "presort_depth": args.presort},

@@ -118,7 +118,16 @@ typedef enum pvg_option {
    *    tile-id passes as (u16 tile id, u32 Gaussian index) instead of the 64-bit key + index: its
    *    depth bits are already in order and would be dead payload. pvg_debug_view rebuilds the
    *    64-bit keys on demand. 0: always carry the 64-bit keys. Results are identical. */
-  PVG_OPT_COMPACT_KEYS = 5
+  PVG_OPT_COMPACT_KEYS = 5,
+  /* 1 (default): with PRESORT_DEPTH=1 and at most 256 blocks of 8x8 tiles (images up to 2048x2048
+   *    pixels or the same area), the per-tile lists are built from one entry per (Gaussian, block)
+   *    -- block id, Gaussian index, 64-bit mask of the covered tiles -- instead of one key per
+   *    (Gaussian, tile): the entries are split by block with one onesweep digit pass and expanded
+   *    into the tile lists by ballots, in depth order. The sorted list and the ranges are
+   *    bit-identical to those of the 64-bit key sort; the unsorted key list and the per-instance
+   *    offsets are not intermediates of this mode (pvg_debug_view produces them on demand).
+   * 0: one key per (Gaussian, tile) as above. */
+  PVG_OPT_BLOCK_BINS = 6
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 
@@ -161,8 +170,9 @@ int pvg_stage_times_ms(pvg_scene *scene, float ms[PVG_NUM_STAGES]);
  * or a negative pvg_status. */
 int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stages, float *ms);
 
-/* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y}. */
-int pvg_frame_stats(pvg_scene *scene, uint64_t out[4]);
+/* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y,
+ * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries}. */
+int pvg_frame_stats(pvg_scene *scene, uint64_t out[6]);
 
 /* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs
  * evaluated before the pixel stopped, out[1] = pairs that contributed (alpha >= 1/255). */

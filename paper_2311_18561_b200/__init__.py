@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("PVG_LIB") or os.path.join(_HERE, "libpvg.so")   # PVG
 PVG_OK = 0
 STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_BAD_CAMERA",
           -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION"}
-OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS = 1, 2, 3, 4, 5
+OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 
@@ -238,9 +238,10 @@ class Scene:
 
     def frame_stats(self) -> Dict[str, int]:
         """Sizes of the last render (no device work)."""
-        out = (C.c_uint64 * 4)()
+        out = (C.c_uint64 * 6)()
         _check(self._L.pvg_frame_stats(self._h, out))
-        return {"n": int(out[0]), "M": int(out[1]), "tiles_x": int(out[2]), "tiles_y": int(out[3])}
+        return {"n": int(out[0]), "M": int(out[1]), "tiles_x": int(out[2]), "tiles_y": int(out[3]),
+                "block_entries": int(out[4]), "list_mode": ("keys64", "compact", "blocks")[int(out[5])]}
 
     def blend_counters(self) -> Tuple[int, int]:
         """(pairs evaluated, pairs contributing) of the last render with OPT_COUNT_PAIRS=1."""

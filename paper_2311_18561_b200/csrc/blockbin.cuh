@@ -1,0 +1,378 @@
+// blockbin.cuh -- stages a2 + a3 (instance part) for depth-presorted Gaussians, without ever
+// materialising or ranking the M individual (tile | depth) keys.
+//
+// The sorted instance list of DESIGN.md S11 is, tile by tile, "the Gaussians whose rectangle
+// covers the tile, in depth order" (PAPER.md:L61 tiles, L70 depth sort). Once the Gaussians are
+// in depth order (the n-key onesweep sort), that list can be produced with one ranked item per
+// (Gaussian, 8x8-tile block) instead of one per (Gaussian, tile) -- 30x fewer at 1920x1280:
+//   1. bin_expand: every Gaussian emits, in depth order, one ENTRY per block its rectangle
+//      touches: (block id, Gaussian index, 64-bit mask of the block's tiles it covers);
+//   2. bin_pass: ONE stable onesweep digit pass splits the entries by block id (<= 256 blocks);
+//      inside a block the entries stay in depth order;
+//   3. bin_count / bin_chunk_scan: per chunk of a block's entries, how many entries cover each
+//      of the 64 tiles; an exclusive scan over the chunks, started at the tile's range begin
+//      (tilebin.cuh), gives every chunk its write position in every tile list;
+//   4. bin_write: a warp owns (chunk, 32 of the block's tiles), a lane holds one entry; for
+//      each tile one ballot of "covers it" ranks the 32 entries, and the covering lanes store
+//      their Gaussian index as one contiguous run of that tile's list.
+// The result is bit-identical to the stable LSD sort of the 64-bit keys: within a tile the
+// order is (depth bits, index), exactly the visiting order of the entries.
+#pragma once
+
+#include "common.cuh"
+#include "onesweep.cuh"
+
+namespace pvg {
+
+constexpr int BB_MAX_BINS = 256;  // one 8-bit digit pass
+constexpr int BB_CHUNK = 512;     // entries per (warp pair) chunk of the count / write walks
+
+__host__ __device__ inline uint32_t bb_blocks(uint32_t tiles) { return (tiles + 7u) >> 3; }
+
+// ---- 1. entry emission ---------------------------------------------------------------------
+constexpr int BE_THREADS = 256;
+constexpr int BE_ITEMS = 8;
+constexpr int BE_CHUNK = BE_THREADS * BE_ITEMS;
+constexpr int BE_SPAN = BE_CHUNK + 64;  // survivors come first in depth order and own >= 1 entry each
+
+struct BinExpandSmem {
+  int4 owner[BE_SPAN];                  // (first entry - chunk start, Gaussian, x0 | y0 << 16, x1 | y1 << 16)
+  alignas(16) uint16_t own[BE_CHUNK];   // owner slot of every entry of the chunk
+  uint32_t warp_max[BE_THREADS / 32];
+  uint32_t lo, hi;
+};
+
+// entry j (row-major over the blocks of the rectangle) of a Gaussian: block id and tile mask
+__device__ __forceinline__ void bb_entry(uint32_t xy0, uint32_t xy1, uint32_t j, uint32_t blocks_x,
+                                         uint32_t& bin, uint64_t& mask) {
+  const uint32_t x0 = xy0 & 0xFFFFu, y0 = xy0 >> 16, x1 = xy1 & 0xFFFFu, y1 = xy1 >> 16;
+  const uint32_t bx0 = x0 >> 3, bw = (x1 >> 3) - bx0 + 1u;
+  // j < 2^16, bw <= 2^8: (j + 0.5) / bw is at least 1/(2 bw) away from an integer, far more than
+  // the rounding of the product, so the truncation is the exact quotient
+  const uint32_t brow = __float2uint_rz(((float)j + 0.5f) * __frcp_rn((float)bw));
+  const uint32_t bx = bx0 + (j - brow * bw), by = (y0 >> 3) + brow;
+  bin = by * blocks_x + bx;
+  const uint32_t lx0 = max(x0, bx * 8u) - bx * 8u, lx1 = min(x1, bx * 8u + 7u) - bx * 8u;
+  const uint32_t ly0 = max(y0, by * 8u) - by * 8u, ly1 = min(y1, by * 8u + 7u) - by * 8u;
+  const uint32_t rowmask = ((2u << (lx1 - lx0)) - 1u) << lx0;   // bits lx0..lx1 of one tile row
+  const uint32_t nrows = ly1 - ly0 + 1u;
+  const uint64_t rows = nrows == 8u ? ~0ull : (((1ull << (8u * nrows)) - 1ull) << (8u * ly0));
+  mask = ((uint64_t)rowmask * 0x0101010101010101ull) & rows;    // bit (ty & 7) * 8 + (tx & 7)
+}
+
+// One CTA owns BE_CHUNK consecutive entries. The owners of the chunk are staged in shared
+// memory, each marks its first entry, and a max-scan spreads the owner slot over the chunk
+// (same scheme as expand.cuh). visit: depth order; boffsets: exclusive scan of bb_count in it.
+__global__ void __launch_bounds__(BE_THREADS)
+bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ visit,
+                  const uint4* __restrict__ tileinfo, uint32_t blocks_x, uint8_t* __restrict__ e_bin,
+                  uint32_t* __restrict__ e_g, uint64_t* __restrict__ e_mask) {
+  __shared__ BinExpandSmem s;
+  const uint32_t tid = threadIdx.x;
+  const uint32_t i0 = blockIdx.x * BE_CHUNK;
+  const uint32_t i1 = min(i0 + (uint32_t)BE_CHUNK, Mb);
+  if (tid == 0 || tid == 32) {
+    // last r in [0, n) with boffsets[r] <= target (boffsets[0] == 0)
+    const uint32_t target = tid == 0 ? i0 : i1 - 1u;
+    uint32_t lo = 0, hi = n;
+    while (hi - lo > 1) {
+      const uint32_t mid = lo + ((hi - lo) >> 1);
+      if (boffsets[mid] <= target) lo = mid; else hi = mid;
+    }
+    if (tid == 0) s.lo = lo; else s.hi = lo;
+  }
+  reinterpret_cast<uint4*>(s.own)[tid] = make_uint4(0u, 0u, 0u, 0u);   // 8 u16 per thread
+  __syncthreads();
+  const uint32_t r_lo = s.lo, span = s.hi - r_lo + 1u;
+
+  if (span <= BE_SPAN) {
+    for (uint32_t k = tid; k < span; k += BE_THREADS) {
+      const uint32_t r = r_lo + k;
+      const uint32_t g = visit[r];
+      const uint4 ti = tileinfo[g];
+      const int start = (int)(boffsets[r] - i0);   // negative only for the owner that began before the chunk
+      const uint32_t xy1 = ((ti.x & 0xFFFFu) + (ti.y & 0xFFFFu) - 1u) | (((ti.x >> 16) + (ti.y >> 16) - 1u) << 16);
+      s.owner[k] = make_int4(start, (int)g, (int)ti.x, (int)xy1);
+      if (ti.w != 0u && start < BE_CHUNK) s.own[max(start, 0)] = (uint16_t)k;
+    }
+    __syncthreads();
+    // inclusive max-scan of the marks (slot numbers increase along the chunk)
+    const uint4 a = reinterpret_cast<uint4*>(s.own)[tid];
+    uint32_t w16[4] = {a.x, a.y, a.z, a.w};
+    uint32_t run = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) run = max(run, max(w16[q] & 0xFFFFu, w16[q] >> 16));
+    uint32_t incl = run;
+    const uint32_t lane = tid & 31u, warp = tid >> 5;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl = max(incl, v);
+    }
+    if (lane == 31) s.warp_max[warp] = incl;
+    uint32_t carry = __shfl_up_sync(0xffffffffu, incl, 1);
+    if (lane == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t wv = 0; wv < warp; ++wv) carry = max(carry, s.warp_max[wv]);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const uint32_t lo16 = max(carry, w16[q] & 0xFFFFu);
+      const uint32_t hi16 = max(lo16, w16[q] >> 16);
+      carry = hi16;
+      w16[q] = lo16 | (hi16 << 16);
+    }
+    reinterpret_cast<uint4*>(s.own)[tid] = make_uint4(w16[0], w16[1], w16[2], w16[3]);
+    __syncthreads();
+#pragma unroll 4
+    for (int k = 0; k < BE_ITEMS; ++k) {
+      const uint32_t p = k * BE_THREADS + tid;
+      if (i0 + p >= i1) break;
+      const int4 o = s.owner[s.own[p]];
+      uint32_t bin;
+      uint64_t mask;
+      bb_entry((uint32_t)o.z, (uint32_t)o.w, (uint32_t)((int)p - o.x), blocks_x, bin, mask);
+      e_bin[i0 + p] = (uint8_t)bin;
+      e_g[i0 + p] = (uint32_t)o.y;
+      e_mask[i0 + p] = mask;
+    }
+  } else {
+    // owners without entries inside the chunk (never the case in depth order): search per entry
+    for (int k = 0; k < BE_ITEMS; ++k) {
+      const uint32_t p = k * BE_THREADS + tid;
+      if (i0 + p >= i1) break;
+      uint32_t lo = 0, hi = span;
+      while (hi - lo > 1) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if (boffsets[r_lo + mid] <= i0 + p) lo = mid; else hi = mid;
+      }
+      const uint32_t r = r_lo + lo;
+      const uint32_t g = visit[r];
+      const uint4 ti = tileinfo[g];
+      const uint32_t xy1 = ((ti.x & 0xFFFFu) + (ti.y & 0xFFFFu) - 1u) | (((ti.x >> 16) + (ti.y >> 16) - 1u) << 16);
+      uint32_t bin;
+      uint64_t mask;
+      bb_entry(ti.x, xy1, i0 + p - boffsets[r], blocks_x, bin, mask);
+      e_bin[i0 + p] = (uint8_t)bin;
+      e_g[i0 + p] = g;
+      e_mask[i0 + p] = mask;
+    }
+  }
+}
+
+// ---- 2. stable split of the entries by block id ---------------------------------------------
+constexpr int BH_THREADS = 256;
+
+// 256-bin histogram of the block ids (16 ids per thread and step)
+__global__ void __launch_bounds__(BH_THREADS)
+bin_hist_kernel(const uint8_t* __restrict__ e_bin, uint32_t Mb, uint32_t* __restrict__ hist /* [256], zeroed */) {
+  __shared__ uint32_t s_hist[BB_MAX_BINS];
+  s_hist[threadIdx.x] = 0;
+  __syncthreads();
+  const uint32_t vecs = Mb >> 4;
+  for (uint32_t v = blockIdx.x * BH_THREADS + threadIdx.x; v < vecs; v += gridDim.x * BH_THREADS) {
+    const uint4 q = __ldcs(reinterpret_cast<const uint4*>(e_bin) + v);
+    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      atomicAdd(&s_hist[w[k] & 0xFFu], 1u);
+      atomicAdd(&s_hist[(w[k] >> 8) & 0xFFu], 1u);
+      atomicAdd(&s_hist[(w[k] >> 16) & 0xFFu], 1u);
+      atomicAdd(&s_hist[w[k] >> 24], 1u);
+    }
+  }
+  if (blockIdx.x == 0)
+    for (uint32_t i = (vecs << 4) + threadIdx.x; i < Mb; i += BH_THREADS) atomicAdd(&s_hist[e_bin[i]], 1u);
+  __syncthreads();
+  const uint32_t c = s_hist[threadIdx.x];
+  if (c) atomicAdd(&hist[threadIdx.x], c);
+}
+
+// Single block of 256 threads: bin_start[b] = first entry of block b in the split list
+// (exclusive scan of the histogram; [256] = Mb) and chunk_start[b] = first chunk of block b
+// when every block's entries are cut into chunks of BB_CHUNK ([256] = number of chunks).
+__global__ void __launch_bounds__(BB_MAX_BINS)
+bin_plan_kernel(const uint32_t* __restrict__ hist, uint32_t* __restrict__ bin_start /* [257] */,
+                uint32_t* __restrict__ chunk_start /* [257] */) {
+  __shared__ uint32_t s_a[BB_MAX_BINS / 32], s_b[BB_MAX_BINS / 32];
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t c = hist[tid];
+  const uint32_t k = (c + BB_CHUNK - 1) / BB_CHUNK;
+  uint32_t ia = c, ib = k;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t ta = __shfl_up_sync(0xffffffffu, ia, d), tb = __shfl_up_sync(0xffffffffu, ib, d);
+    if (lane >= d) { ia += ta; ib += tb; }
+  }
+  if (lane == 31) { s_a[warp] = ia; s_b[warp] = ib; }
+  __syncthreads();
+  uint32_t wa = 0, wb = 0;
+  for (uint32_t w = 0; w < warp; ++w) { wa += s_a[w]; wb += s_b[w]; }
+  bin_start[tid] = wa + ia - c;
+  chunk_start[tid] = wb + ib - k;
+  if (tid == BB_MAX_BINS - 1) { bin_start[BB_MAX_BINS] = wa + ia; chunk_start[BB_MAX_BINS] = wb + ib; }
+}
+
+constexpr int BP_THREADS = 256;
+constexpr int BP_ITEMS = 16;
+
+template <int BITS>
+struct BinPassSmem {
+  typename RadixCore<BP_THREADS, BP_ITEMS, BITS>::Smem core;
+  uint64_t mask[BP_THREADS * BP_ITEMS];
+  uint32_t g[BP_THREADS * BP_ITEMS];
+  uint8_t bin[BP_THREADS * BP_ITEMS];
+};
+
+// One onesweep digit pass (RadixCore, decoupled look-back) over (block id; Gaussian, mask).
+// The block id itself is not written: bin_start[] says where each block's entries live.
+template <int BITS>
+__global__ void __launch_bounds__(BP_THREADS, 2)
+bin_pass_kernel(const uint8_t* __restrict__ bin_in, const uint32_t* __restrict__ g_in, const uint64_t* __restrict__ mask_in,
+                uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, uint32_t n,
+                const uint32_t* __restrict__ bin_start, uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket) {
+  using Core = RadixCore<BP_THREADS, BP_ITEMS, BITS>;
+  constexpr int TILE = Core::TILE;
+  constexpr uint32_t MASK = (1u << BITS) - 1u;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  BinPassSmem<BITS>& s = *reinterpret_cast<BinPassSmem<BITS>*>(smem_raw);
+
+  const uint32_t tile = Core::take_ticket(s.core, ticket);
+  const uint32_t tile_base = tile * TILE;
+  const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
+  const uint32_t tid = threadIdx.x;
+  const uint32_t wbase = (tid >> 5) * (BP_ITEMS * 32) + (tid & 31u);
+  uint32_t dp[BP_ITEMS], bn[BP_ITEMS], g[BP_ITEMS];
+  uint64_t mk[BP_ITEMS];
+#pragma unroll
+  for (int j = 0; j < BP_ITEMS; ++j) {
+    const bool ok = wbase + j * 32 < tile_n;
+    const uint32_t i = tile_base + wbase + j * 32;
+    bn[j] = ok ? (uint32_t)__ldcs(bin_in + i) : MASK;   // padding ranks last
+    g[j] = ok ? __ldcs(g_in + i) : 0u;
+    mk[j] = ok ? __ldcs(mask_in + i) : 0ull;
+    dp[j] = bn[j] & MASK;
+  }
+  Core::rank(s.core, tile, dp, bin_start, lookback);
+#pragma unroll
+  for (int j = 0; j < BP_ITEMS; ++j) {
+    s.bin[dp[j] >> 8] = (uint8_t)bn[j];
+    s.g[dp[j] >> 8] = g[j];
+    s.mask[dp[j] >> 8] = mk[j];
+  }
+  __syncthreads();
+  for (uint32_t p = tid; p < tile_n; p += BP_THREADS) {
+    const uint32_t o = s.core.out_base[s.bin[p] & MASK] + p;
+    g_out[o] = s.g[p];
+    mask_out[o] = s.mask[p];
+  }
+}
+
+// ---- 3./4. the walks over a block's entries --------------------------------------------------
+constexpr int BW_THREADS = 256;                       // 8 warps = 4 chunks x 2 halves of the block
+constexpr int BW_CHUNKS_PER_CTA = BW_THREADS / 64;
+
+// Row `lane` of the transpose of the 32 x 32 bit matrix whose row r is lane r's x.
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, uint32_t lane) {
+#pragma unroll
+  for (int j = 16; j >= 1; j >>= 1) {
+    const uint32_t L = j == 16 ? 0x0000FFFFu : j == 8 ? 0x00FF00FFu : j == 4 ? 0x0F0F0F0Fu : j == 2 ? 0x33333333u : 0x55555555u;
+    const uint32_t o = __shfl_xor_sync(0xffffffffu, x, j);
+    x = (lane & j) ? ((x & ~L) | ((o & ~L) >> j)) : ((x & L) | ((o & L) << j));
+  }
+  return x;
+}
+
+// Which chunk does this warp own? Fills the entry range [e0, e1) and returns false past the end.
+struct BinWalk {
+  uint32_t chunk, half, e0, e1;
+};
+__device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ chunk_start,
+                                               uint32_t* s_cs, BinWalk& w) {
+  for (uint32_t k = threadIdx.x; k <= BB_MAX_BINS; k += BW_THREADS) s_cs[k] = chunk_start[k];
+  __syncthreads();
+  const uint32_t warp = threadIdx.x >> 5;
+  w.chunk = blockIdx.x * BW_CHUNKS_PER_CTA + (warp >> 1);
+  w.half = warp & 1u;
+  if (w.chunk >= s_cs[BB_MAX_BINS]) return false;
+  uint32_t lo = 0, hi = BB_MAX_BINS;   // last b with chunk_start[b] <= chunk: the block that owns it
+  while (hi - lo > 1) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if (s_cs[mid] <= w.chunk) lo = mid; else hi = mid;
+  }
+  w.e0 = bin_start[lo] + (w.chunk - s_cs[lo]) * BB_CHUNK;
+  w.e1 = min(w.e0 + (uint32_t)BB_CHUNK, bin_start[lo + 1]);
+  return true;
+}
+
+// chunk_cnt[chunk][lt] = number of the chunk's entries whose mask covers tile lt of the block
+__global__ void __launch_bounds__(BW_THREADS)
+bin_count_kernel(const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
+                 const uint32_t* __restrict__ chunk_start, uint32_t* __restrict__ chunk_cnt) {
+  __shared__ uint32_t s_cs[BB_MAX_BINS + 1];
+  BinWalk w;
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, w)) return;
+  const uint32_t lane = threadIdx.x & 31u;
+  uint32_t cnt = 0;
+  for (uint32_t e = w.e0; e < w.e1; e += 32) {
+    const uint64_t m64 = e + lane < w.e1 ? __ldcs(masks + e + lane) : 0ull;
+    const uint32_t m = w.half ? (uint32_t)(m64 >> 32) : (uint32_t)m64;
+    cnt += __popc(transpose32(m, lane));
+  }
+  chunk_cnt[w.chunk * 64u + w.half * 32u + lane] = cnt;
+}
+
+// In place: chunk_cnt[chunk][lt] -> position in tile lt's list where the chunk starts writing
+// (the tile's range begin + the counts of the block's earlier chunks). One CTA per block.
+__global__ void __launch_bounds__(64)
+bin_chunk_scan_kernel(uint32_t* __restrict__ chunk_cnt, const uint32_t* __restrict__ chunk_start,
+                      const uint2* __restrict__ ranges, uint32_t tiles_x, uint32_t tiles_y, uint32_t blocks_x) {
+  const uint32_t b = blockIdx.x, lt = threadIdx.x;
+  const uint32_t tx = (b % blocks_x) * 8u + (lt & 7u), ty = (b / blocks_x) * 8u + (lt >> 3);
+  uint32_t run = (tx < tiles_x && ty < tiles_y) ? ranges[ty * tiles_x + tx].x : 0u;
+  const uint32_t c0 = chunk_start[b], c1 = chunk_start[b + 1];
+  uint32_t c = c0;
+  for (; c + 8 <= c1; c += 8) {
+    uint32_t v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = chunk_cnt[(c + k) * 64u + lt];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { chunk_cnt[(c + k) * 64u + lt] = run; run += v[k]; }
+  }
+  for (; c < c1; ++c) {
+    const uint32_t v = chunk_cnt[c * 64u + lt];
+    chunk_cnt[c * 64u + lt] = run;
+    run += v;
+  }
+}
+
+// The sorted value list. A warp owns (chunk, half); lane l holds entry e + l of the batch and,
+// as tile index, the running write position of tile half * 32 + l. For tile l of the half, the
+// ballot of "my entry covers it" ranks the 32 entries; covering lanes store their Gaussian
+// index at consecutive positions of that tile's list.
+__global__ void __launch_bounds__(BW_THREADS)
+bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
+                 const uint32_t* __restrict__ chunk_start, const uint32_t* __restrict__ chunk_pos,
+                 uint32_t* __restrict__ vals) {
+  __shared__ uint32_t s_cs[BB_MAX_BINS + 1];
+  BinWalk w;
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, w)) return;
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t lt = lanemask_lt();
+  uint32_t pos = chunk_pos[w.chunk * 64u + w.half * 32u + lane];
+  for (uint32_t e = w.e0; e < w.e1; e += 32) {
+    const bool ok = e + lane < w.e1;
+    const uint64_t m64 = ok ? __ldcs(masks + e + lane) : 0ull;
+    const uint32_t g = ok ? __ldcs(gs + e + lane) : 0u;
+    const uint32_t m = w.half ? (uint32_t)(m64 >> 32) : (uint32_t)m64;
+#pragma unroll
+    for (int l = 0; l < 32; ++l) {
+      const bool p = (m >> l) & 1u;
+      const uint32_t wl = __ballot_sync(0xffffffffu, p);
+      const uint32_t base = __shfl_sync(0xffffffffu, pos, l);
+      if (p) vals[base + __popc(wl & lt)] = g;
+    }
+    pos += __popc(transpose32(m, lane));
+  }
+}
+
+}  // namespace pvg

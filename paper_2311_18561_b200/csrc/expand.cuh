@@ -69,8 +69,8 @@ expand_kernel(uint32_t n, uint32_t M, const uint32_t* __restrict__ offsets, cons
       const uint32_t g = visit ? visit[r] : r;
       const uint4 ti = tileinfo[g];
       const int start = (int)(offsets[r] - i0);   // negative only for the owner that began before the chunk
-      s.owner[k] = make_int4(start, (int)g, (int)ti.x, (int)ti.y);
-      s.rcp[k] = 1.0f / (float)ti.y;
+      s.owner[k] = make_int4(start, (int)g, (int)ti.x, (int)(ti.y & 0xFFFFu));
+      s.rcp[k] = 1.0f / (float)(ti.y & 0xFFFFu);
       s.zbits[k] = ti.z;
       if (ti.w != 0u && start < EXP_CHUNK) s.own[max(start, 0)] = (uint16_t)k;
     }
@@ -128,7 +128,8 @@ expand_kernel(uint32_t n, uint32_t M, const uint32_t* __restrict__ offsets, cons
       const uint32_t r = r_lo + lo;
       const uint32_t g = visit ? visit[r] : r;
       const uint4 ti = tileinfo[g];
-      const uint32_t tile = rect_tile(ti.x, ti.y, 1.0f / (float)ti.y, i0 + p - offsets[r], tiles_x);
+      const uint32_t rw = ti.y & 0xFFFFu;
+      const uint32_t tile = rect_tile(ti.x, rw, 1.0f / (float)rw, i0 + p - offsets[r], tiles_x);
       if (COMPACT) tiles16[i0 + p] = (uint16_t)tile;
       else keys[i0 + p] = ((uint64_t)tile << 32) | ti.z;
       vals[i0 + p] = g;

@@ -30,7 +30,7 @@ namespace pvg {
 //   SH[p][i], p = 0..11: floats 4p..4p+3 of the point's [16][3] coefficient block
 // Outputs:
 //   record[3 i + {0,1,2}] = (mx,my,z,o~), (a,b,c,hx), (r,g,b,hy)   -- all 0 if culled
-//   tileinfo[i] = (x0 | y0 << 16, rect width, fp32 bits of z, rect count)
+//   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
 //   dkeys[i], dvals[i] (optional) = (fp32 bits of z, or 0xFFFFFFFF if culled), i
 //   tilegrid (optional): 2-D difference array of per-tile instance counts (tilebin.cuh)
@@ -121,7 +121,7 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
       valid = (tx0 <= tx1) && (ty0 <= ty1);
       if (valid) {
         const uint32_t w = (uint32_t)(tx1 - tx0 + 1), h = (uint32_t)(ty1 - ty0 + 1);
-        ti = make_uint4((uint32_t)tx0 | ((uint32_t)ty0 << 16), w, __float_as_uint(pz), w * h);
+        ti = make_uint4((uint32_t)tx0 | ((uint32_t)ty0 << 16), w | (h << 16), __float_as_uint(pz), w * h);
         r0 = make_float4(mx, my, pz, op);
         r1 = make_float4(ca, cb, cc, hx);
       }
@@ -183,7 +183,7 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
   }
   if (tilegrid && valid) {
     const int x0 = (int)(ti.x & 0xFFFFu), y0 = (int)(ti.x >> 16);
-    tilegrid_add_rect(tilegrid, tilegrid_stride(P.tiles_x), x0, y0, x0 + (int)ti.y - 1, y0 + (int)(ti.w / ti.y) - 1);
+    tilegrid_add_rect(tilegrid, tilegrid_stride(P.tiles_x), x0, y0, x0 + (int)(ti.y & 0xFFFFu) - 1, y0 + (int)(ti.y >> 16) - 1);
   }
 }
 

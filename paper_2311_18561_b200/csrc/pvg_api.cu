@@ -10,6 +10,7 @@
 
 #include "../../include/pvg.h"
 #include "blend.cuh"
+#include "blockbin.cuh"
 #include "common.cuh"
 #include "expand.cuh"
 #include "onesweep.cuh"
@@ -293,8 +294,9 @@ struct pvg_scene {
   int sh_degree = 3;
   cudaStream_t stream = nullptr;
   // options
-  int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1;
+  int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1;
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
+  bool block_used = false;    // last frame built the tile lists from 8x8-tile block entries (blockbin.cuh)
   // model (SoA)
   Buf A0, A1, A2, A3, SH;
   // per-Gaussian workspace
@@ -302,13 +304,16 @@ struct pvg_scene {
   // per-instance workspace
   Buf keys[2], vals[2], keys_unsorted, vals_unsorted;
   Buf tiles16[2], tiles16_unsorted;
+  // block-entry workspace (blockbin.cuh)
+  Buf boffsets, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
   Buf ranges, tilegrid;
   Buf img;  // render_host device images
   SortScratch sort_n, sort_m;
   uint64_t* h_total = nullptr;  // pinned
   Timer timer;
   // last frame
-  uint64_t M = 0;
+  uint64_t M = 0, Mb = 0;
+  FrameParams last_P{};
   int sorted_side = 0, visit_side = 0;
   uint32_t tiles_x = 0, tiles_y = 0;
   int sort_begin = 0, sort_end = 0;
@@ -327,6 +332,7 @@ void release_all(pvg_scene* s) {
   Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
+                 &s->boffsets, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
                  &s->ranges, &s->tilegrid, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
@@ -363,7 +369,7 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   up(t_sh, d->sh, 48); up(t_tau, d->tau, 1); up(t_beta, d->beta, 1); up(t_vel, d->vel, 3);
   auto rs = [&](Buf& b, size_t bytes) { if (rc == PVG_OK) rc = b.reserve(bytes, st); };
   rs(s->A0, n * 16); rs(s->A1, n * 16); rs(s->A2, n * 16); rs(s->A3, n * 16); rs(s->SH, n * 192);
-  rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4);
+  rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4); rs(s->boffsets, n * 4);
   rs(s->dkeys[0], n * 8); rs(s->dkeys[1], n * 8); rs(s->dvals[0], n * 4); rs(s->dvals[1], n * 4);
   rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 8); rs(s->small, 256);
   if (rc == PVG_OK) {
@@ -412,6 +418,109 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, float t, FrameParams* 
   P->tiles_x = (cam->width + PVG_TILE - 1) / PVG_TILE;
   P->tiles_y = (cam->height + PVG_TILE - 1) / PVG_TILE;
   for (int j = 0; j < 3; ++j) P->bg[j] = cam->bg[j];
+  return PVG_OK;
+}
+
+// a2 scan of the per-Gaussian item counts in visiting order; the total lands in small @8.
+int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm) {
+  cudaStream_t st = s->stream;
+  const uint32_t n = s->n;
+  const uint32_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 8, st));
+  CU(cudaMemsetAsync(s->small.p, 0, 16, st));
+  uint32_t* ticket = s->small.as<uint32_t>();
+  uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
+  if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
+  if (blocks)
+    scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->tileinfo.as<uint4>(), visit,
+                                                                  out, total, s->scan_status.as<uint64_t>(), ticket);
+  else
+    scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->tileinfo.as<uint4>(), visit,
+                                                                   out, total, s->scan_status.as<uint64_t>(), ticket);
+  if (tm) TRY(tm->end(st));
+  return PVG_OK;
+}
+
+template <int BITS>
+int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64_t* lookback, uint32_t* ticket) {
+  auto kern = bin_pass_kernel<BITS>;
+  static bool configured = false;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BinPassSmem<BITS>)));
+    configured = true;
+  }
+  constexpr uint32_t TILE = BP_THREADS * BP_ITEMS;
+  kern<<<(Mb + TILE - 1) / TILE, BP_THREADS, sizeof(BinPassSmem<BITS>), s->stream>>>(
+      s->e_bin.as<uint8_t>(), s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>(), s->s_g.as<uint32_t>(),
+      s->s_mask.as<uint64_t>(), Mb, bin_start, lookback, ticket);
+  return PVG_OK;
+}
+
+// a2 + a3 (instance part) through 8x8-tile block entries (blockbin.cuh): the sorted value list
+// lands in vals[0]; ranges come from tile_prefix_kernel.
+int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Timer* tm) {
+  cudaStream_t st = s->stream;
+  const uint32_t n = s->n, Mb = (uint32_t)s->Mb;
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  constexpr uint32_t PASS_TILE = BP_THREADS * BP_ITEMS;
+  const uint32_t pass_tiles = (Mb + PASS_TILE - 1) / PASS_TILE;
+  const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
+  TRY(s->vals[0].reserve((size_t)s->M * 4, st, 1.125));
+  TRY(s->e_bin.reserve((size_t)Mb + 16, st, 1.125));
+  TRY(s->e_g.reserve((size_t)Mb * 4, st, 1.125));
+  TRY(s->e_mask.reserve((size_t)Mb * 8, st, 1.125));
+  TRY(s->s_g.reserve((size_t)Mb * 4, st, 1.125));
+  TRY(s->s_mask.reserve((size_t)Mb * 8, st, 1.125));
+  TRY(s->bin_tables.reserve(4096, st));   // hist[256] | bin_start[257] | chunk_start[257] | ticket
+  TRY(s->chunk_cnt.reserve((size_t)max_chunks * 64 * 4, st, 1.125));
+  TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
+  uint32_t* hist = s->bin_tables.as<uint32_t>();
+  uint32_t* bin_start = hist + 256;
+  uint32_t* chunk_start = bin_start + 257;
+  uint32_t* ticket = chunk_start + 257;
+  CU(cudaMemsetAsync(s->bin_tables.p, 0, 4096, st));
+  CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, st));
+
+  TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
+  bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
+      n, Mb, s->boffsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), blocks_x, s->e_bin.as<uint8_t>(),
+      s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>());
+  TRY(tm->end(st));
+
+  TRY(tm->begin("bin_hist", PVG_STAGE_SORT, st));
+  const unsigned hist_grid = (unsigned)std::min<uint64_t>(((uint64_t)Mb / 16 + BH_THREADS - 1) / BH_THREADS + 1, 148 * 4);
+  bin_hist_kernel<<<hist_grid, BH_THREADS, 0, st>>>(s->e_bin.as<uint8_t>(), Mb, hist);
+  TRY(tm->end(st));
+  TRY(tm->begin("bin_plan", PVG_STAGE_SORT, st));
+  bin_plan_kernel<<<1, BB_MAX_BINS, 0, st>>>(hist, bin_start, chunk_start);
+  TRY(tm->end(st));
+
+  TRY(tm->begin("bin_pass", PVG_STAGE_SORT, st));
+  int rc = PVG_ERR_BAD_OPTION;
+  switch (std::max(1, ceil_log2(nbins))) {
+#define PVG_CASE(B) case B: rc = launch_bin_pass<B>(s, Mb, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket); break;
+    PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
+#undef PVG_CASE
+    default: break;
+  }
+  TRY(rc);
+  TRY(tm->end(st));
+
+  const unsigned walk_grid = (max_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
+  TRY(tm->begin("bin_count", PVG_STAGE_SORT, st));
+  bin_count_kernel<<<walk_grid, BW_THREADS, 0, st>>>(s->s_mask.as<uint64_t>(), bin_start, chunk_start,
+                                                     s->chunk_cnt.as<uint32_t>());
+  TRY(tm->end(st));
+  TRY(tm->begin("bin_chunk_scan", PVG_STAGE_SORT, st));
+  bin_chunk_scan_kernel<<<nbins, 64, 0, st>>>(s->chunk_cnt.as<uint32_t>(), chunk_start, s->ranges.as<uint2>(),
+                                              (uint32_t)P.tiles_x, (uint32_t)P.tiles_y, blocks_x);
+  TRY(tm->end(st));
+  TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
+  bin_write_kernel<<<walk_grid, BW_THREADS, 0, st>>>(s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, chunk_start,
+                                                     s->chunk_cnt.as<uint32_t>(), s->vals[0].as<uint32_t>());
+  TRY(tm->end(st));
+  CU(cudaGetLastError());
+  s->sorted_side = 0;
   return PVG_OK;
 }
 
@@ -476,26 +585,26 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
     visit = s->dvals[side].as<uint32_t>();
   }
 
-  // a2 scan
-  const uint32_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 8, st));
-  CU(cudaMemsetAsync(s->small.p, 0, 64, st));
-  uint32_t* ticket = s->small.as<uint32_t>();
-  uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
-  TRY(tm.begin("scan_counts", PVG_STAGE_DUPLICATE, st));
-  scan_counts_kernel<<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), visit, s->offsets.as<uint32_t>(),
-                                                          total, s->scan_status.as<uint64_t>(), ticket);
-  TRY(tm.end(st));
-  CU(cudaMemcpyAsync(s->h_total, total, 8, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));  // the one host read-back: M sizes the instance buffers
-  const uint64_t M = *s->h_total;
-  if (M >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
+  // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), blocks_y = bb_blocks(P.tiles_y);
+  const bool block = s->presort && s->block && blocks_x * blocks_y <= (uint32_t)BB_MAX_BINS;
+  s->block_used = block;
+  s->last_P = P;
+  TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm));
+  // the one host read-back: M (and the entry count) size the per-instance buffers
+  CU(cudaMemcpyAsync(s->h_total, s->small.as<unsigned char>() + 8, 16, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  const uint64_t M = block ? s->h_total[1] : s->h_total[0];
+  s->Mb = block ? s->h_total[0] : 0;
+  if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
   s->M = M;
 
   s->sorted_side = 0;
-  const bool compact = s->presort && s->compact && tile_bits <= 16;
+  const bool compact = !block && s->presort && s->compact && tile_bits <= 16;
   s->compact_used = compact;
-  if (M > 0 && compact) {
+  if (M > 0 && block) {
+    TRY(run_block_bins(s, P, visit, &tm));
+  } else if (M > 0 && compact) {
     for (int k = 0; k < 2; ++k) {
       TRY(s->tiles16[k].reserve((size_t)M * 2, st, 1.125));
       TRY(s->vals[k].reserve((size_t)M * 4, st, 1.125));
@@ -635,6 +744,7 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
     case PVG_OPT_PRESORT_DEPTH: scene->presort = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KEEP_UNSORTED: scene->keep_unsorted = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_COMPACT_KEYS: scene->compact = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_BLOCK_BINS: scene->block = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_COUNT_PAIRS: scene->count_pairs = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KERNEL_EVENTS:
       scene->timer.enabled = value != 0;
@@ -685,6 +795,26 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->counts = s->counts.as<uint32_t>();
   out->visit_order = s->presort ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
+  if (s->block_used) {
+    // the block path never forms per-instance offsets or the unsorted list: produce them here
+    cudaStream_t st = s->stream;
+    const uint32_t* visit = s->dvals[s->visit_side].as<uint32_t>();
+    TRY(run_scan(s, false, s->offsets.as<uint32_t>(), visit, nullptr));
+    if (s->M) {
+      TRY(s->keys[0].reserve((size_t)s->M * 8, st));
+      keys_from_ranges_kernel<<<s->tiles_x * s->tiles_y, 256, 0, st>>>(s->ranges.as<uint2>(), s->vals[0].as<uint32_t>(),
+                                                                        s->tileinfo.as<uint4>(), s->keys[0].as<uint64_t>());
+      if (s->keep_unsorted) {
+        TRY(s->keys_unsorted.reserve((size_t)s->M * 8, st));
+        TRY(s->vals_unsorted.reserve((size_t)s->M * 4, st));
+        expand_kernel<false><<<(unsigned)((s->M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
+            s->n, (uint32_t)s->M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), s->tiles_x,
+            s->keys_unsorted.as<uint64_t>(), nullptr, s->vals_unsorted.as<uint32_t>());
+      }
+    }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+  }
   if (s->compact_used && s->M) {
     // rebuild (tile << 32 | depth bits) from the compact payload: debug only
     cudaStream_t st = s->stream;
@@ -707,7 +837,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     out->vals_unsorted = s->vals_unsorted.as<uint32_t>();
   }
   if (s->M) {
-    out->keys_sorted = s->keys[s->compact_used ? 0 : s->sorted_side].as<uint64_t>();
+    out->keys_sorted = s->keys[(s->compact_used || s->block_used) ? 0 : s->sorted_side].as<uint64_t>();
     out->vals_sorted = s->vals[s->sorted_side].as<uint32_t>();
   }
   out->ranges = s->ranges.as<uint32_t>();
@@ -746,12 +876,14 @@ int pvg_stage_times_ms(pvg_scene* s, float ms[PVG_NUM_STAGES]) {
   return PVG_OK;
 }
 
-int pvg_frame_stats(pvg_scene* s, uint64_t out[4]) {
+int pvg_frame_stats(pvg_scene* s, uint64_t out[6]) {
   if (!s || !out) return PVG_ERR_NULL;
   out[0] = s->n;
   out[1] = s->rendered ? s->M : 0;
   out[2] = s->tiles_x;
   out[3] = s->tiles_y;
+  out[4] = s->rendered ? s->Mb : 0;
+  out[5] = s->block_used ? 2 : (s->compact_used ? 1 : 0);
   return PVG_OK;
 }
 

@@ -1,6 +1,6 @@
-// scan_dup.cuh -- stage a2: exclusive prefix scan of the per-Gaussian tile counts in
-// visiting order, then emission of one (tile | depth) 64-bit key + Gaussian index per
-// tile instance (PAPER.md:L61 tile-based rasterisation, L70 depth sort; S11).
+// scan_dup.cuh -- stage a2, first half: exclusive prefix scan, in visiting order, of the number
+// of items each Gaussian emits -- its tile count, or the number of 8x8-tile blocks its rectangle
+// touches (blockbin.cuh). PAPER.md:L61 tile-based rasterisation; S11.
 #pragma once
 
 #include "common.cuh"
@@ -11,17 +11,28 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 
+// blocks of 8 x 8 tiles touched by a rectangle; tileinfo = (x0 | y0 << 16, w | h << 16, depth bits, count)
+__device__ __forceinline__ uint32_t scan_block_count(const uint4 ti) {
+  if (ti.w == 0u) return 0u;
+  const uint32_t x0 = ti.x & 0xFFFFu, y0 = ti.x >> 16;
+  const uint32_t x1 = x0 + (ti.y & 0xFFFFu) - 1u, y1 = y0 + (ti.y >> 16) - 1u;
+  return ((x1 >> 3) - (x0 >> 3) + 1u) * ((y1 >> 3) - (y0 >> 3) + 1u);
+}
+
 // Single-pass chained scan with decoupled look-back. Warp-aggregated: per-thread
 // serial sums -> warp shuffles -> one partial per warp -> block aggregate, which is
 // published in a 64-bit status word (flag | value) and resolved against predecessor
 // tiles. Tiles are handed out by an atomic ticket so a tile only ever waits on tiles
 // that already started (forward progress without co-residency assumptions).
+//   BLOCKS : false: item count = counts[g]; true: blocks touched by tileinfo[g]'s rectangle
 //   visit  : visiting order (Gaussian index at position r), or nullptr for identity
 //   offsets: [n] exclusive prefix of counts[visit[r]]
 //   total  : [1] 64-bit sum (M), written by the last tile
 //   status : [num_tiles] zeroed; ticket: [1] zeroed
+template <bool BLOCKS>
 __global__ void __launch_bounds__(SCAN_THREADS)
-scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint32_t* __restrict__ visit,
+scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint4* __restrict__ tileinfo,
+                   const uint32_t* __restrict__ visit,
                    uint32_t* __restrict__ offsets, uint64_t* __restrict__ total,
                    uint64_t* __restrict__ status, uint32_t* __restrict__ ticket) {
   __shared__ uint32_t s_tile;
@@ -38,7 +49,10 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint32
   for (int k = 0; k < SCAN_ITEMS; ++k) {
     const uint32_t r = base + k;
     c[k] = 0;
-    if (r < n) c[k] = counts[visit ? visit[r] : r];
+    if (r < n) {
+      const uint32_t g = visit ? visit[r] : r;
+      c[k] = BLOCKS ? scan_block_count(tileinfo[g]) : counts[g];
+    }
     tsum += c[k];  // < 2^32: one Gaussian covers at most 2^22 tiles, 8 of them 2^25
   }
   // warp inclusive scan of the thread sums
@@ -86,72 +100,6 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint32
     const uint32_t r = base + k;
     if (r < n) offsets[r] = (uint32_t)run;  // valid when M < 2^32 (checked on the host)
     run += c[k];
-  }
-}
-
-constexpr int DUP_THREADS = 256;
-constexpr int DUP_ITEMS = 8;
-constexpr int DUP_CHUNK = DUP_THREADS * DUP_ITEMS;
-constexpr int DUP_SPAN = 2048;  // visiting positions cached in shared memory per chunk
-
-// Instance-parallel emission: block b owns output instances [b*CHUNK, (b+1)*CHUNK), so
-// the work per block is uniform no matter how skewed the per-Gaussian counts are (1 ..
-// every tile) and every store is a fully coalesced 256 B (keys) / 128 B (values) line per
-// warp. The owning visiting position of an instance is the last r with offsets[r] <= i,
-// found by binary search (shared-memory copy of the chunk's offset span when it fits).
-__global__ void __launch_bounds__(DUP_THREADS)
-duplicate_kernel(uint32_t n, uint64_t M, const uint32_t* __restrict__ offsets,
-                 const uint32_t* __restrict__ visit, const uint4* __restrict__ tileinfo,
-                 uint32_t tiles_x, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
-  __shared__ uint32_t s_off[DUP_SPAN];
-  __shared__ uint32_t s_lo, s_hi;
-  const uint64_t i0 = (uint64_t)blockIdx.x * DUP_CHUNK;
-  const uint64_t i1 = min(i0 + (uint64_t)DUP_CHUNK, M);  // exclusive
-  if (threadIdx.x < 2) {
-    // last r with offsets[r] <= target
-    const uint32_t target = (uint32_t)(threadIdx.x == 0 ? i0 : i1 - 1);
-    uint32_t lo = 0, hi = n;  // invariant: offsets[lo] <= target (offsets[0] = 0), answer in [lo, hi)
-    while (hi - lo > 1) {
-      const uint32_t mid = lo + ((hi - lo) >> 1);
-      if (offsets[mid] <= target) lo = mid; else hi = mid;
-    }
-    if (threadIdx.x == 0) s_lo = lo; else s_hi = lo;
-  }
-  __syncthreads();
-  const uint32_t r_lo = s_lo, r_hi = s_hi;
-  const uint32_t span = r_hi - r_lo + 1;
-  const bool cached = span <= DUP_SPAN;
-  if (cached)
-    for (uint32_t k = threadIdx.x; k < span; k += DUP_THREADS) s_off[k] = offsets[r_lo + k];
-  __syncthreads();
-
-#pragma unroll
-  for (int k = 0; k < DUP_ITEMS; ++k) {
-    const uint64_t i = i0 + (uint64_t)k * DUP_THREADS + threadIdx.x;
-    if (i >= i1) break;
-    const uint32_t target = (uint32_t)i;
-    uint32_t lo = 0, hi = span;
-    if (cached) {
-      while (hi - lo > 1) {
-        const uint32_t mid = lo + ((hi - lo) >> 1);
-        if (s_off[mid] <= target) lo = mid; else hi = mid;
-      }
-    } else {
-      while (hi - lo > 1) {
-        const uint32_t mid = lo + ((hi - lo) >> 1);
-        if (offsets[r_lo + mid] <= target) lo = mid; else hi = mid;
-      }
-    }
-    const uint32_t r = r_lo + lo;
-    const uint32_t off = cached ? s_off[lo] : offsets[r];
-    const uint32_t g = visit ? visit[r] : r;
-    const uint4 ti = tileinfo[g];
-    const uint32_t j = target - off;          // < ti.w * rect height
-    const uint32_t row = j / ti.y;
-    const uint32_t col = j - row * ti.y;
-    const uint32_t tile = ((ti.x >> 16) + row) * tiles_x + (ti.x & 0xFFFFu) + col;
-    keys[i] = ((uint64_t)tile << 32) | ti.z;
-    vals[i] = g;
   }
 }
 

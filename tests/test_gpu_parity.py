@@ -15,7 +15,7 @@ from workloads import make_config, pinhole_camera
 pytestmark = pytest.mark.gpu
 
 
-def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None, compact=True):
+def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None, compact=True, block=True):
     """(P), (I), (R) for one frame. Returns the stats of the three comparisons."""
     own = scene is None
     sc = scene or pvg.Scene.from_workload_scene(wl_scene)
@@ -23,6 +23,7 @@ def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, sc
         sc.set_option(pvg.OPT_PRESORT_DEPTH, 1 if presort else 0)
         sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
         sc.set_option(pvg.OPT_COMPACT_KEYS, 1 if compact else 0)
+        sc.set_option(pvg.OPT_BLOCK_BINS, 1 if block else 0)
         rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t))
         dbg = sc.debug()
     finally:
@@ -65,9 +66,43 @@ def test_cfg1_full_width_sort_mode_matches():
 
 
 def test_cfg1_presort_with_64bit_keys_matches():
-    """PRESORT_DEPTH=1 but COMPACT_KEYS=0: the tile-id passes carry the full 64-bit keys."""
+    """PRESORT_DEPTH=1 but COMPACT_KEYS=0, BLOCK_BINS=0: the tile-id passes carry the full 64-bit keys."""
     wl = make_config(1, n=60_000)
-    full_parity(wl.scene, wl.cameras[0], 0.5, compact=False, end_to_end=False)
+    full_parity(wl.scene, wl.cameras[0], 0.5, compact=False, block=False, end_to_end=False)
+
+
+@pytest.mark.parametrize("cfg,n,cam_i", [(0, None, 0), (1, 60_000, 0), (2, 20_000, 0), (4, 20_000, 2)])
+def test_compact_key_mode_matches(cfg, n, cam_i):
+    """BLOCK_BINS=0: one (u16 tile, u32 index) instance per (Gaussian, tile), two tile-id digit passes."""
+    wl = make_config(cfg, n=n)
+    full_parity(wl.scene, wl.cameras[cam_i], 0.25, block=False, end_to_end=False)
+
+
+def test_block_mode_is_the_default_and_used():
+    wl = make_config(1, n=30_000)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    sc.render(wl.cameras[0], 0.5)
+    st = sc.frame_stats()
+    assert st["list_mode"] == "blocks" and 0 < st["block_entries"] < st["M"]
+    sc.set_option(pvg.OPT_BLOCK_BINS, 0)
+    sc.render(wl.cameras[0], 0.5)
+    assert sc.frame_stats()["list_mode"] == "compact"
+    sc.close()
+
+
+def test_block_mode_many_chunks_one_block():
+    """A 128x128 image is ONE 8x8-tile block: every entry lands in the same bin, whose list is cut into
+    many chunks; full masks and long tile lists (scales inflated so rectangles cover most tiles)."""
+    wl = make_config(0, n=4096)
+    s = wl.scene
+    big = pvg.Scene(s.mu, s.quat, s.scale * 6.0, s.opacity, s.sh, s.tau, s.beta, s.vel)
+    cam = pinhole_camera(128, 128, 100.0)
+    big.set_option(pvg.OPT_KEEP_UNSORTED, 1)
+    big.render(cam, 0.37)
+    dbg = big.debug()
+    st = check_integer_chain(dbg, 128, 128, True)
+    assert big.frame_stats()["block_entries"] > 4 * 512 and st["mean_list"] > 500
+    big.close()
 
 
 def test_cfg2_mix_reduced_full_resolution():
