@@ -345,34 +345,71 @@ bin_chunk_scan_kernel(uint32_t* __restrict__ chunk_cnt, const uint32_t* __restri
   }
 }
 
-// The sorted value list. A warp owns (chunk, half); lane l holds entry e + l of the batch and,
-// as tile index, the running write position of tile half * 32 + l. For tile l of the half, the
-// ballot of "my entry covers it" ranks the 32 entries; covering lanes store their Gaussian
-// index at consecutive positions of that tile's list.
+// ballot of "bit `bit` of m is set" (test + vote: two instructions)
+__device__ __forceinline__ uint32_t ballot_bit(uint32_t m, uint32_t bit) {
+  uint32_t w;
+  asm volatile("{\n\t"
+               ".reg .pred p;\n\t"
+               ".reg .b32 t;\n\t"
+               "and.b32 t, %1, %2;\n\t"
+               "setp.ne.u32 p, t, 0;\n\t"
+               "vote.sync.ballot.b32 %0, p, 0xffffffff;\n\t"
+               "}"
+               : "=r"(w)
+               : "r"(m), "r"(bit));
+  return w;
+}
+
+// The sorted value list. A warp owns (chunk, half of the block's tiles) and holds the whole chunk in
+// registers: lane j has entries e0 + 32 b + j, b = 0..15. Tile by tile, the ballot of "my entry covers
+// it" ranks the 32 entries of a batch, and the covering lanes store their Gaussian index at consecutive
+// positions of that tile's list. The 16 stores of a tile are issued back to back and extend one
+// contiguous run (~1 KB), so L2 sees whole lines and DRAM whole bursts.
+template <bool FULL>
+__device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 32], const uint32_t (&g)[BB_CHUNK / 32],
+                                                uint32_t nb, uint32_t mypos, uint32_t lt, uint32_t* vp) {
+  for (uint32_t l = 0; l < 32; ++l) {
+    uint32_t run = __shfl_sync(0xffffffffu, mypos, l);
+    const uint32_t bit = 1u << l;
+#pragma unroll
+    for (int b = 0; b < BB_CHUNK / 32; ++b) {
+      if (FULL || b < nb) {
+        const uint32_t wl = ballot_bit(m[b], bit);
+        if (m[b] & bit) asm volatile("st.global.u32 [%0], %1;" ::"l"(vp + (run + __popc(wl & lt))), "r"(g[b]) : "memory");
+        run += __popc(wl);
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(BW_THREADS)
 bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
                  const uint32_t* __restrict__ chunk_start, const uint32_t* __restrict__ chunk_pos,
                  uint32_t* __restrict__ vals) {
   __shared__ uint32_t s_cs[BB_MAX_BINS + 1];
+  // the base pointer round-trips through shared memory so that it lives in registers; taken from the
+  // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
+  __shared__ uint32_t* s_vals;
+  if (threadIdx.x == 0) s_vals = vals;
   BinWalk w;
-  if (!bin_walk_setup(bin_start, chunk_start, s_cs, w)) return;
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, w)) return;   // (contains the barrier)
+  uint32_t* const vp = s_vals;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t lt = lanemask_lt();
-  uint32_t pos = chunk_pos[w.chunk * 64u + w.half * 32u + lane];
-  for (uint32_t e = w.e0; e < w.e1; e += 32) {
-    const bool ok = e + lane < w.e1;
-    const uint64_t m64 = ok ? __ldcs(masks + e + lane) : 0ull;
-    const uint32_t g = ok ? __ldcs(gs + e + lane) : 0u;
-    const uint32_t m = w.half ? (uint32_t)(m64 >> 32) : (uint32_t)m64;
+  constexpr int NB = BB_CHUNK / 32;
+  const uint32_t* mp = reinterpret_cast<const uint32_t*>(masks) + w.half;   // this half's 32 mask bits
+  uint32_t m[NB], g[NB];
 #pragma unroll
-    for (int l = 0; l < 32; ++l) {
-      const bool p = (m >> l) & 1u;
-      const uint32_t wl = __ballot_sync(0xffffffffu, p);
-      const uint32_t base = __shfl_sync(0xffffffffu, pos, l);
-      if (p) vals[base + __popc(wl & lt)] = g;
-    }
-    pos += __popc(transpose32(m, lane));
+  for (int b = 0; b < NB; ++b) {
+    const uint32_t e = w.e0 + b * 32 + lane;
+    const bool ok = e < w.e1;
+    m[b] = ok ? __ldcs(mp + 2 * (size_t)e) : 0u;
+    g[b] = ok ? __ldcs(gs + e) : 0u;
   }
+  const uint32_t mypos = chunk_pos[w.chunk * 64u + w.half * 32u + lane];
+  const uint32_t nb = (w.e1 - w.e0 + 31u) >> 5;
+  if (nb == NB) bin_write_tiles<true>(m, g, nb, mypos, lt, vp);
+  else bin_write_tiles<false>(m, g, nb, mypos, lt, vp);
 }
 
 }  // namespace pvg
