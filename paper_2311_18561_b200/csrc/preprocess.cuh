@@ -33,14 +33,13 @@ namespace pvg {
 //   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
 //   dkeys[i], dvals[i] (optional) = (fp32 bits of z, or 0xFFFFFFFF if culled), i
-//   tilegrid (optional): 2-D difference array of per-tile instance counts (tilebin.cuh)
 __global__ void __launch_bounds__(256)
 preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
                   const float4* __restrict__ A0, const float4* __restrict__ A1,
                   const float4* __restrict__ A2, const float4* __restrict__ A3,
                   const float4* __restrict__ SH, float4* __restrict__ record,
                   uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
-                  uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, int* __restrict__ tilegrid) {
+                  uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
 
@@ -180,10 +179,6 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
   if (dkeys) {
     dkeys[i] = valid ? (uint64_t)ti.z : 0xFFFFFFFFull;
     dvals[i] = i;
-  }
-  if (tilegrid && valid) {
-    const int x0 = (int)(ti.x & 0xFFFFu), y0 = (int)(ti.x >> 16);
-    tilegrid_add_rect(tilegrid, tilegrid_stride(P.tiles_x), x0, y0, x0 + (int)(ti.y & 0xFFFFu) - 1, y0 + (int)(ti.y >> 16) - 1);
   }
 }
 

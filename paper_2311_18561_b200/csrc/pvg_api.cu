@@ -553,18 +553,24 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
   preprocess_kernel<<<(n + 255) / 256, 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
                                                       s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
-                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, grid);
+                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv);
   TRY(tm.end(st));
 
   // a4 + the histograms of a3, from the tile counts alone (no pass over the instances)
   if (s->presort) {
     static bool attr_set = false;
     constexpr size_t kMaxDyn = 200 * 1024;
-    if (!attr_set) {
-      CU(cudaFuncSetAttribute(tile_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
-      attr_set = true;
-    }
+    if (!attr_set) CU(cudaFuncSetAttribute(tile_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
     const int use_smem = grid_bytes <= kMaxDyn ? 1 : 0;
+    if (!attr_set) CU(cudaFuncSetAttribute(tile_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    TRY(tm.begin("tile_grid", PVG_STAGE_RANGES, st));
+    tile_grid_kernel<<<std::min<unsigned>((n + TG_THREADS - 1) / TG_THREADS, (unsigned)sms), TG_THREADS, use_smem ? grid_bytes : 0, st>>>(
+        s->tileinfo.as<uint4>(), n, P.tiles_x, P.tiles_y, use_smem, grid);
+    TRY(tm.end(st));
+    attr_set = true;
     TRY(s->sort_m.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
     uint64_t* total2 = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 16);
     TRY(tm.begin("tile_prefix", PVG_STAGE_RANGES, st));

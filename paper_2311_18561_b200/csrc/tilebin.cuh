@@ -1,8 +1,8 @@
 // tilebin.cuh -- per-tile instance counts without touching the instance list.
 //
 // Every surviving Gaussian adds +1 to each tile of its rectangle. Instead of M atomic
-// increments (or a pass over the M sorted keys), preprocess adds the rectangle's four
-// corners to a 2-D difference array (4 integer atomics per Gaussian) and this kernel
+// increments (or a pass over the M sorted keys), tile_grid_kernel adds the rectangle's four
+// corners to a 2-D difference array (4 integer atomics per Gaussian) and tile_prefix_kernel
 // integrates it: a 2-D prefix sum gives the exact number of instances of every tile.
 // From those counts follow, with no further HBM traffic,
 //   * the per-tile ranges  range[tile] = [lower_bound(tile<<32), lower_bound((tile+1)<<32))
@@ -15,6 +15,38 @@
 #include "onesweep.cuh"
 
 namespace pvg {
+
+constexpr int TG_THREADS = 1024;
+
+// The difference array. One persistent CTA per SM accumulates the four corner updates of its share
+// of the rectangles in a shared-memory copy of the grid (they are heavily contended: clamped
+// rectangles all hit the border cells) and then adds its non-zero cells to the global grid.
+// use_smem = 0 (grid larger than shared memory): update the global grid directly.
+__global__ void __launch_bounds__(TG_THREADS)
+tile_grid_kernel(const uint4* __restrict__ tileinfo, uint32_t n, int TX, int TY, int use_smem, int* __restrict__ grid) {
+  extern __shared__ int s_grid[];
+  const int stride = tilegrid_stride(TX);
+  const int cells = stride * (TY + 1);
+  int* g = grid;
+  if (use_smem) {
+    for (int k = threadIdx.x; k < cells; k += TG_THREADS) s_grid[k] = 0;
+    __syncthreads();
+    g = s_grid;
+  }
+  for (uint32_t i = blockIdx.x * TG_THREADS + threadIdx.x; i < n; i += gridDim.x * TG_THREADS) {
+    const uint4 ti = tileinfo[i];
+    if (ti.w == 0u) continue;
+    const int x0 = (int)(ti.x & 0xFFFFu), y0 = (int)(ti.x >> 16);
+    tilegrid_add_rect(g, stride, x0, y0, x0 + (int)(ti.y & 0xFFFFu) - 1, y0 + (int)(ti.y >> 16) - 1);
+  }
+  if (use_smem) {
+    __syncthreads();
+    for (int k = threadIdx.x; k < cells; k += TG_THREADS) {
+      const int v = s_grid[k];
+      if (v) atomicAdd(grid + k, v);
+    }
+  }
+}
 
 constexpr int TB_THREADS = 1024;
 
