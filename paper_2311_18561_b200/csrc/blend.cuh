@@ -12,6 +12,8 @@ namespace pvg {
 
 constexpr int BLEND_THREADS = PVG_TILE_PIXELS;
 constexpr int BLEND_BATCH = 256;
+constexpr int BLEND_BATCH_FIRST = 64;
+constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -21,9 +23,13 @@ __device__ __forceinline__ float ex2_approx(float x) {
 
 // One CTA per 16x16 tile, one thread per pixel. The tile's slice of the sorted instance
 // list is consumed in batches: each thread gathers one 48 B record through the sorted
-// index list into shared memory (conic pre-scaled by -log2(e)/2 so the inner loop feeds
-// ex2 directly), then every pixel walks the batch. The tile retires as soon as every
-// pixel's transmittance has dropped below 1e-4.
+// index list into shared memory, pre-digested so that the inner loop is straight-line:
+//   conic scaled by -log2(e)/2 and log2(o~) carried as the constant term, so that
+//   alpha = min(0.99, ex2(a' dx^2 + b' dx dy + c' dy^2 + log2 o~)) needs no multiply by o~.
+// The per-pixel decisions (1/255 cutoff, T stop) are predicates, not branches: 71% of the
+// evaluations contribute at config 3, so a warp practically always has a contributing lane and
+// branching only added reconvergence overhead. A warp leaves the batch as soon as none of its
+// pixels is alive; the tile retires when every pixel's transmittance has dropped below 1e-4.
 // COUNT = true additionally counts the (pixel, list entry) evaluations reached and the
 // contributing ones into counters[0..1] (measurement only, never on the product path).
 template <bool COUNT>
@@ -33,7 +39,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
              float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
              unsigned long long* __restrict__ counters) {
   __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
-  __shared__ float4 s_col[BLEND_BATCH];   // c', o~, r, g
+  __shared__ float4 s_col[BLEND_BATCH];   // c', log2 o~, r, g
   __shared__ float2 s_bz[BLEND_BATCH];    // b, z
 
   const uint32_t tid = threadIdx.x;
@@ -45,46 +51,64 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   const uint2 range = ranges[tile];
 
   float T = 1.0f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;
-  bool done = !inside;
+  bool alive = inside;
   uint32_t n_eval = 0, n_contrib = 0;
 
-  for (uint32_t base = range.x; base < range.y; base += BLEND_BATCH) {
+  // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
+  // saturates, so a fixed 256-entry first batch gathers mostly records that are never used
+  uint32_t bs = BLEND_BATCH_FIRST;
+  for (uint32_t base = range.x; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
-    if (__syncthreads_count(!done) == 0) break;
+    if (__syncthreads_count(alive) == 0) break;
     const uint32_t idx = base + tid;
-    if (idx < range.y) {
+    if (tid >= bs) {
+    } else if (idx < range.y) {
       const uint32_t g = __ldg(vals + idx);
       const float4 r0 = __ldg(record + 3 * (size_t)g);
       const float4 r1 = __ldg(record + 3 * (size_t)g + 1);
       const float4 r2 = __ldg(record + 3 * (size_t)g + 2);
       const float kh = -0.72134752044448170f;  // -log2(e)/2
       s_geo[tid] = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
-      s_col[tid] = make_float4(kh * r1.z, r0.w, r2.x, r2.y);
+      s_col[tid] = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
       s_bz[tid] = make_float2(r2.z, r0.z);
+    } else {
+      // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0
+      s_geo[tid] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_col[tid] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
+      s_bz[tid] = make_float2(0.f, 0.f);
     }
     __syncthreads();
-    const uint32_t nb = min((uint32_t)BLEND_BATCH, range.y - base);
-    if (!done) {
-      for (uint32_t j = 0; j < nb; ++j) {
-        const float4 ge = s_geo[j];
-        const float4 co = s_col[j];
-        if (COUNT) ++n_eval;
-        const float dx = ge.x - pxf, dy = ge.y - pyf;
-        // w = log2(e) * (-1/2 (a dx^2 + c dy^2) - b dx dy)
-        float w = fmaf(dx, fmaf(ge.z, dx, ge.w * dy), (co.x * dy) * dy);
-        w = fminf(w, 0.0f);                       // S16': rounding guard (exact w <= 0)
-        const float alpha = fminf(PVG_ALPHA_MAX, co.y * ex2_approx(w));
-        if (alpha < PVG_ALPHA_MIN) continue;
-        const float Tn = T * (1.0f - alpha);
-        if (Tn < PVG_T_STOP) { done = true; break; }   // S10: not composited
-        const float wgt = alpha * T;
-        const float2 bz = s_bz[j];
-        Cr = fmaf(co.z, wgt, Cr);
-        Cg = fmaf(co.w, wgt, Cg);
-        Cb = fmaf(bz.x, wgt, Cb);
-        D = fmaf(bz.y, wgt, D);
-        T = Tn;
-        if (COUNT) ++n_contrib;
+    const uint32_t nb = min(bs, range.y - base);
+    if (__any_sync(0xffffffffu, alive)) {
+      for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
+#pragma unroll
+        for (int u = 0; u < BLEND_UNROLL; ++u) {
+          const uint32_t j = j0 + u;
+          const float4 ge = s_geo[j];
+          const float4 co = s_col[j];
+          const float2 bz = s_bz[j];
+          if (COUNT) n_eval += alive && j < nb;
+          const float dx = ge.x - pxf, dy = ge.y - pyf;
+          // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy); the quadratic form is <= 0 exactly (S16')
+          const float t1 = fmaf(ge.w, dy, ge.z * dx);
+          float w = fmaf(co.x * dy, dy, fmaf(t1, dx, co.y));
+          w = fminf(w, co.y);
+          const float alpha = fminf(PVG_ALPHA_MAX, ex2_approx(w));
+          const bool acc = alive && alpha >= PVG_ALPHA_MIN;
+          const float wgt = alpha * T;
+          const float Tn = T - wgt;                      // T (1 - alpha)
+          const bool use = acc && Tn >= PVG_T_STOP;      // S10: the one that would cross the stop is not composited
+          alive = alive && (use || !acc);
+          if (use) {
+            Cr = fmaf(co.z, wgt, Cr);
+            Cg = fmaf(co.w, wgt, Cg);
+            Cb = fmaf(bz.x, wgt, Cb);
+            D = fmaf(bz.y, wgt, D);
+            T = Tn;
+          }
+          if (COUNT) n_contrib += use;
+        }
+        if (!__any_sync(0xffffffffu, alive)) break;
       }
     }
   }
