@@ -310,10 +310,10 @@ def run_ours(args):
         a[1] += 1
     # algorithmic bytes over the timed region, per (kernel, stage)
     alg = {("preprocess", "preprocess"): K * (64.0 * N + 80.0 * N + 192.0 * S),
-           ("scan_counts", "duplicate"): K * (24.0 if list_mode == "blocks" else 12.0) * N,
+           ("scan_counts", "duplicate"): K * 12.0 * N,   # 8 B sorted key (or 4 B visit + 4 B count) + 4 B offset
            # block-entry path (blockbin.cuh): 13 B entries (u8 block, u32 Gaussian, u64 mask)
-           ("bin_expand", "duplicate"): 13.0 * Mbsum + K * 24.0 * S,
-           ("bin_hist", "sort"): 1.0 * Mbsum,
+           ("bin_expand", "duplicate"): 13.0 * Mbsum + K * 16.0 * S,
+           ("tile_grid", "ranges"): K * 16.0 * N,
            ("bin_pass", "sort"): 25.0 * Mbsum,
            ("bin_count", "sort"): 8.0 * Mbsum + 256.0 * chunks,
            ("bin_chunk_scan", "sort"): 512.0 * chunks,

@@ -9,6 +9,7 @@
 //      touches: (block id, Gaussian index, 64-bit mask of the block's tiles it covers);
 //   2. bin_pass: ONE stable onesweep digit pass splits the entries by block id (<= 256 blocks);
 //      inside a block the entries stay in depth order;
+//   (the entries per block, hence bin_start / chunk_start, come from tilebin.cuh's block grid)
 //   3. bin_count / bin_chunk_scan: per chunk of a block's entries, how many entries cover each
 //      of the 64 tiles; an exclusive scan over the chunks, started at the tile's range begin
 //      (tilebin.cuh), gives every chunk its write position in every tile list;
@@ -62,10 +63,11 @@ __device__ __forceinline__ void bb_entry(uint32_t xy0, uint32_t xy1, uint32_t j,
 
 // One CTA owns BE_CHUNK consecutive entries. The owners of the chunk are staged in shared
 // memory, each marks its first entry, and a max-scan spreads the owner slot over the chunk
-// (same scheme as expand.cuh). visit: depth order; boffsets: exclusive scan of bb_count in it.
+// (same scheme as expand.cuh). keys/visit: the depth-sorted (rect | depth, Gaussian) pairs;
+// boffsets: exclusive scan of the blocks touched, in that order.
 __global__ void __launch_bounds__(BE_THREADS)
-bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ visit,
-                  const uint4* __restrict__ tileinfo, uint32_t blocks_x, uint8_t* __restrict__ e_bin,
+bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint64_t* __restrict__ keys,
+                  const uint32_t* __restrict__ visit, uint32_t blocks_x, uint8_t* __restrict__ e_bin,
                   uint32_t* __restrict__ e_g, uint64_t* __restrict__ e_mask) {
   __shared__ BinExpandSmem s;
   const uint32_t tid = threadIdx.x;
@@ -88,12 +90,12 @@ bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets
   if (span <= BE_SPAN) {
     for (uint32_t k = tid; k < span; k += BE_THREADS) {
       const uint32_t r = r_lo + k;
-      const uint32_t g = visit[r];
-      const uint4 ti = tileinfo[g];
+      const uint64_t key = keys[r];
+      const uint32_t rc = (uint32_t)(key >> 32);   // (x0, y0, x1, y1), 8 bits each
       const int start = (int)(boffsets[r] - i0);   // negative only for the owner that began before the chunk
-      const uint32_t xy1 = ((ti.x & 0xFFFFu) + (ti.y & 0xFFFFu) - 1u) | (((ti.x >> 16) + (ti.y >> 16) - 1u) << 16);
-      s.owner[k] = make_int4(start, (int)g, (int)ti.x, (int)xy1);
-      if (ti.w != 0u && start < BE_CHUNK) s.own[max(start, 0)] = (uint16_t)k;
+      s.owner[k] = make_int4(start, (int)visit[r], (int)((rc & 0xFFu) | ((rc & 0xFF00u) << 8)),
+                             (int)(((rc >> 16) & 0xFFu) | ((rc >> 24) << 16)));
+      if ((uint32_t)key != 0xFFFFFFFFu && start < BE_CHUNK) s.own[max(start, 0)] = (uint16_t)k;
     }
     __syncthreads();
     // inclusive max-scan of the marks (slot numbers increase along the chunk)
@@ -147,11 +149,11 @@ bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets
       }
       const uint32_t r = r_lo + lo;
       const uint32_t g = visit[r];
-      const uint4 ti = tileinfo[g];
-      const uint32_t xy1 = ((ti.x & 0xFFFFu) + (ti.y & 0xFFFFu) - 1u) | (((ti.x >> 16) + (ti.y >> 16) - 1u) << 16);
+      const uint32_t rc = (uint32_t)(keys[r] >> 32);
       uint32_t bin;
       uint64_t mask;
-      bb_entry(ti.x, xy1, i0 + p - boffsets[r], blocks_x, bin, mask);
+      bb_entry((rc & 0xFFu) | ((rc & 0xFF00u) << 8), ((rc >> 16) & 0xFFu) | ((rc >> 24) << 16), i0 + p - boffsets[r], blocks_x,
+               bin, mask);
       e_bin[i0 + p] = (uint8_t)bin;
       e_g[i0 + p] = g;
       e_mask[i0 + p] = mask;
@@ -160,58 +162,6 @@ bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets
 }
 
 // ---- 2. stable split of the entries by block id ---------------------------------------------
-constexpr int BH_THREADS = 256;
-
-// 256-bin histogram of the block ids (16 ids per thread and step)
-__global__ void __launch_bounds__(BH_THREADS)
-bin_hist_kernel(const uint8_t* __restrict__ e_bin, uint32_t Mb, uint32_t* __restrict__ hist /* [256], zeroed */) {
-  __shared__ uint32_t s_hist[BB_MAX_BINS];
-  s_hist[threadIdx.x] = 0;
-  __syncthreads();
-  const uint32_t vecs = Mb >> 4;
-  for (uint32_t v = blockIdx.x * BH_THREADS + threadIdx.x; v < vecs; v += gridDim.x * BH_THREADS) {
-    const uint4 q = __ldcs(reinterpret_cast<const uint4*>(e_bin) + v);
-    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      atomicAdd(&s_hist[w[k] & 0xFFu], 1u);
-      atomicAdd(&s_hist[(w[k] >> 8) & 0xFFu], 1u);
-      atomicAdd(&s_hist[(w[k] >> 16) & 0xFFu], 1u);
-      atomicAdd(&s_hist[w[k] >> 24], 1u);
-    }
-  }
-  if (blockIdx.x == 0)
-    for (uint32_t i = (vecs << 4) + threadIdx.x; i < Mb; i += BH_THREADS) atomicAdd(&s_hist[e_bin[i]], 1u);
-  __syncthreads();
-  const uint32_t c = s_hist[threadIdx.x];
-  if (c) atomicAdd(&hist[threadIdx.x], c);
-}
-
-// Single block of 256 threads: bin_start[b] = first entry of block b in the split list
-// (exclusive scan of the histogram; [256] = Mb) and chunk_start[b] = first chunk of block b
-// when every block's entries are cut into chunks of BB_CHUNK ([256] = number of chunks).
-__global__ void __launch_bounds__(BB_MAX_BINS)
-bin_plan_kernel(const uint32_t* __restrict__ hist, uint32_t* __restrict__ bin_start /* [257] */,
-                uint32_t* __restrict__ chunk_start /* [257] */) {
-  __shared__ uint32_t s_a[BB_MAX_BINS / 32], s_b[BB_MAX_BINS / 32];
-  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  const uint32_t c = hist[tid];
-  const uint32_t k = (c + BB_CHUNK - 1) / BB_CHUNK;
-  uint32_t ia = c, ib = k;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t ta = __shfl_up_sync(0xffffffffu, ia, d), tb = __shfl_up_sync(0xffffffffu, ib, d);
-    if (lane >= d) { ia += ta; ib += tb; }
-  }
-  if (lane == 31) { s_a[warp] = ia; s_b[warp] = ib; }
-  __syncthreads();
-  uint32_t wa = 0, wb = 0;
-  for (uint32_t w = 0; w < warp; ++w) { wa += s_a[w]; wb += s_b[w]; }
-  bin_start[tid] = wa + ia - c;
-  chunk_start[tid] = wb + ib - k;
-  if (tid == BB_MAX_BINS - 1) { bin_start[BB_MAX_BINS] = wa + ia; chunk_start[BB_MAX_BINS] = wb + ib; }
-}
-
 constexpr int BP_THREADS = 256;
 constexpr int BP_ITEMS = 16;
 

@@ -31,6 +31,7 @@ struct FrameParams {
   int linear;         // l == +INF: mu~ = mu + (t - tau) v
   int sh_degree;
   int width, height, tiles_x, tiles_y;
+  int pack_rect;      // tiles_x, tiles_y <= 256: the depth key carries the tile rectangle in its upper half
   float bg[3];
 };
 

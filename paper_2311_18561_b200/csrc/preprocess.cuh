@@ -32,7 +32,7 @@ namespace pvg {
 //   record[3 i + {0,1,2}] = (mx,my,z,o~), (a,b,c,hx), (r,g,b,hy)   -- all 0 if culled
 //   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
-//   dkeys[i], dvals[i] (optional) = (fp32 bits of z, or 0xFFFFFFFF if culled), i
+//   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | fp32 bits of z, or 0xFFFFFFFF if culled), i
 __global__ void __launch_bounds__(256)
 preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
                   const float4* __restrict__ A0, const float4* __restrict__ A1,
@@ -177,7 +177,14 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
   tileinfo[i] = ti;
   counts[i] = ti.w;
   if (dkeys) {
-    dkeys[i] = valid ? (uint64_t)ti.z : 0xFFFFFFFFull;
+    // upper half: (x0, y0, x1, y1) of the tile rectangle, 8 bits each -- payload that rides through the
+    // depth sort, so the block-entry scan and emission read it sequentially instead of gathering tileinfo
+    uint32_t rect = 0;
+    if (P.pack_rect) {
+      const uint32_t x0 = ti.x & 0xFFFFu, y0 = ti.x >> 16;
+      rect = x0 | (y0 << 8) | ((x0 + (ti.y & 0xFFFFu) - 1u) << 16) | ((y0 + (ti.y >> 16) - 1u) << 24);
+    }
+    dkeys[i] = valid ? (((uint64_t)rect << 32) | ti.z) : 0xFFFFFFFFull;
     dvals[i] = i;
   }
 }

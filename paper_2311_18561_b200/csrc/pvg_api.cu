@@ -310,6 +310,8 @@ struct pvg_scene {
   Buf img;  // render_host device images
   SortScratch sort_n, sort_m;
   uint64_t* h_total = nullptr;  // pinned
+  cudaStream_t side = nullptr;  // tile grid + prefix run here, beside the depth sort
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   Timer timer;
   // last frame
   uint64_t M = 0, Mb = 0;
@@ -338,6 +340,11 @@ void release_all(pvg_scene* s) {
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
   s->h_total = nullptr;
+  if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+  if (s->ev_join) cudaEventDestroy(s->ev_join);
+  if (s->side) cudaStreamDestroy(s->side);
+  s->ev_fork = s->ev_join = nullptr;
+  s->side = nullptr;
   s->timer.destroy();
 }
 
@@ -388,6 +395,9 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   for (Buf* b : tmp) b->release();
   if (rc != PVG_OK) return rc;
   CU(cudaMallocHost((void**)&s->h_total, 64));
+  CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
+  CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
   return PVG_OK;
 }
 
@@ -417,6 +427,7 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, float t, FrameParams* 
   P->width = cam->width; P->height = cam->height;
   P->tiles_x = (cam->width + PVG_TILE - 1) / PVG_TILE;
   P->tiles_y = (cam->height + PVG_TILE - 1) / PVG_TILE;
+  P->pack_rect = (P->tiles_x <= 256 && P->tiles_y <= 256) ? 1 : 0;
   for (int j = 0; j < 3; ++j) P->bg[j] = cam->bg[j];
   return PVG_OK;
 }
@@ -432,11 +443,11 @@ int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Ti
   uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
   if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
   if (blocks)
-    scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->tileinfo.as<uint4>(), visit,
-                                                                  out, total, s->scan_status.as<uint64_t>(), ticket);
+    scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(),
+                                                                  visit, out, total, s->scan_status.as<uint64_t>(), ticket);
   else
-    scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->tileinfo.as<uint4>(), visit,
-                                                                   out, total, s->scan_status.as<uint64_t>(), ticket);
+    scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), nullptr, visit, out, total,
+                                                                   s->scan_status.as<uint64_t>(), ticket);
   if (tm) TRY(tm->end(st));
   return PVG_OK;
 }
@@ -471,28 +482,19 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(s->e_mask.reserve((size_t)Mb * 8, st, 1.125));
   TRY(s->s_g.reserve((size_t)Mb * 4, st, 1.125));
   TRY(s->s_mask.reserve((size_t)Mb * 8, st, 1.125));
-  TRY(s->bin_tables.reserve(4096, st));   // hist[256] | bin_start[257] | chunk_start[257] | ticket
   TRY(s->chunk_cnt.reserve((size_t)max_chunks * 64 * 4, st, 1.125));
   TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
-  uint32_t* hist = s->bin_tables.as<uint32_t>();
-  uint32_t* bin_start = hist + 256;
+  TRY(s->sort_m.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
+  uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
   uint32_t* chunk_start = bin_start + 257;
-  uint32_t* ticket = chunk_start + 257;
-  CU(cudaMemsetAsync(s->bin_tables.p, 0, 4096, st));
+  uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
+  CU(cudaMemsetAsync(ticket, 0, 4, st));
   CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, st));
 
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
-      n, Mb, s->boffsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), blocks_x, s->e_bin.as<uint8_t>(),
+      n, Mb, s->boffsets.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x, s->e_bin.as<uint8_t>(),
       s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>());
-  TRY(tm->end(st));
-
-  TRY(tm->begin("bin_hist", PVG_STAGE_SORT, st));
-  const unsigned hist_grid = (unsigned)std::min<uint64_t>(((uint64_t)Mb / 16 + BH_THREADS - 1) / BH_THREADS + 1, 148 * 4);
-  bin_hist_kernel<<<hist_grid, BH_THREADS, 0, st>>>(s->e_bin.as<uint8_t>(), Mb, hist);
-  TRY(tm->end(st));
-  TRY(tm->begin("bin_plan", PVG_STAGE_SORT, st));
-  bin_plan_kernel<<<1, BB_MAX_BINS, 0, st>>>(hist, bin_start, chunk_start);
   TRY(tm->end(st));
 
   TRY(tm->begin("bin_pass", PVG_STAGE_SORT, st));
@@ -540,68 +542,85 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
   s->sort_begin = s->presort ? 32 : 0;
   s->sort_end = 32 + tile_bits;
 
-  // a1 preprocess (+ the 2-D difference array of per-tile counts when the depth presort is on)
+  // which list builder (blockbin.cuh needs the depth order, <= 256 blocks and 8-bit tile coordinates)
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), blocks_y = bb_blocks(P.tiles_y);
+  const bool block = s->presort && s->block && P.pack_rect && blocks_x * blocks_y <= (uint32_t)BB_MAX_BINS;
+  s->block_used = block;
+  s->last_P = P;
+
+  // a1 preprocess
   uint64_t* dk = s->presort ? s->dkeys[0].as<uint64_t>() : nullptr;
   uint32_t* dv = s->presort ? s->dvals[0].as<uint32_t>() : nullptr;
-  int* grid = nullptr;
-  const size_t grid_bytes = (size_t)tilegrid_stride(P.tiles_x) * (P.tiles_y + 1) * 4;
-  if (s->presort) {
-    TRY(s->tilegrid.reserve(grid_bytes, st));
-    grid = s->tilegrid.as<int>();
-    CU(cudaMemsetAsync(grid, 0, grid_bytes, st));
-  }
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
   preprocess_kernel<<<(n + 255) / 256, 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
                                                       s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
                                                       s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv);
   TRY(tm.end(st));
 
-  // a4 + the histograms of a3, from the tile counts alone (no pass over the instances)
+  const uint32_t* visit = nullptr;
+  s->visit_side = 0;
+  uint64_t M = 0;
+  s->Mb = 0;
   if (s->presort) {
+    // a4 + the histograms of a3 + the block tables, from the rectangles alone (no pass over the
+    // instances), on the side stream: they overlap the depth sort, and the host reads M and Mb
+    // (they size the frame's buffers) while the depth sort is still running
+    cudaStream_t sd = s->side;
+    CU(cudaEventRecord(s->ev_fork, st));
+    CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
     static bool attr_set = false;
     constexpr size_t kMaxDyn = 200 * 1024;
-    if (!attr_set) CU(cudaFuncSetAttribute(tile_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
+    if (!attr_set) {
+      CU(cudaFuncSetAttribute(tile_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
+      CU(cudaFuncSetAttribute(tile_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
+      attr_set = true;
+    }
+    const size_t grid_bytes = ((size_t)tilegrid_cells(P.tiles_x, P.tiles_y) +
+                               (block ? (size_t)tilegrid_cells((int)blocks_x, (int)blocks_y) : 0)) * 4;
     const int use_smem = grid_bytes <= kMaxDyn ? 1 : 0;
-    if (!attr_set) CU(cudaFuncSetAttribute(tile_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
+    TRY(s->tilegrid.reserve(grid_bytes, st));
+    TRY(s->sort_m.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
+    TRY(s->bin_tables.reserve(4096, st));   // bin_start[257] | chunk_start[257]
+    int* grid = s->tilegrid.as<int>();
+    CU(cudaMemsetAsync(grid, 0, grid_bytes, sd));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    TRY(tm.begin("tile_grid", PVG_STAGE_RANGES, st));
-    tile_grid_kernel<<<std::min<unsigned>((n + TG_THREADS - 1) / TG_THREADS, (unsigned)sms), TG_THREADS, use_smem ? grid_bytes : 0, st>>>(
-        s->tileinfo.as<uint4>(), n, P.tiles_x, P.tiles_y, use_smem, grid);
-    TRY(tm.end(st));
-    attr_set = true;
-    TRY(s->sort_m.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
-    uint64_t* total2 = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 16);
-    TRY(tm.begin("tile_prefix", PVG_STAGE_RANGES, st));
-    tile_prefix_kernel<<<1, TB_THREADS, use_smem ? grid_bytes : 0, st>>>(
-        grid, P.tiles_x, P.tiles_y, use_smem, make_sort_plan(s->sort_begin, s->sort_end), s->ranges.as<uint2>(),
-        s->sort_m.hist.as<uint32_t>(), total2);
-    TRY(tm.end(st));
-  }
+    TRY(tm.begin("tile_grid", PVG_STAGE_RANGES, sd));
+    tile_grid_kernel<<<std::min<unsigned>((n + TG_THREADS - 1) / TG_THREADS, (unsigned)sms), TG_THREADS,
+                       use_smem ? grid_bytes : 0, sd>>>(s->tileinfo.as<uint4>(), n, P.tiles_x, P.tiles_y, use_smem,
+                                                        block ? 1 : 0, grid);
+    TRY(tm.end(sd));
+    uint64_t* totals = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 16);
+    TRY(tm.begin("tile_prefix", PVG_STAGE_RANGES, sd));
+    tile_prefix_kernel<<<1, TB_THREADS, use_smem ? grid_bytes : 0, sd>>>(
+        grid, P.tiles_x, P.tiles_y, use_smem, block ? 1 : 0, make_sort_plan(s->sort_begin, s->sort_end),
+        s->ranges.as<uint2>(), s->sort_m.hist.as<uint32_t>(), totals, s->bin_tables.as<uint32_t>(),
+        s->bin_tables.as<uint32_t>() + 257);
+    TRY(tm.end(sd));
+    CU(cudaMemcpyAsync(s->h_total, totals, 16, cudaMemcpyDeviceToHost, sd));
+    CU(cudaEventRecord(s->ev_join, sd));
 
-  // a3 (n-key part): depth order of the Gaussians
-  const uint32_t* visit = nullptr;
-  s->visit_side = 0;
-  if (s->presort) {
+    // a3 (n-key part): depth order of the Gaussians
     int side = 0;
     TRY(run_onesweep(n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
                      s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side));
     s->visit_side = side;
     visit = s->dvals[side].as<uint32_t>();
-  }
 
-  // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
-  const uint32_t blocks_x = bb_blocks(P.tiles_x), blocks_y = bb_blocks(P.tiles_y);
-  const bool block = s->presort && s->block && blocks_x * blocks_y <= (uint32_t)BB_MAX_BINS;
-  s->block_used = block;
-  s->last_P = P;
-  TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm));
-  // the one host read-back: M (and the entry count) size the per-instance buffers
-  CU(cudaMemcpyAsync(s->h_total, s->small.as<unsigned char>() + 8, 16, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));
-  const uint64_t M = block ? s->h_total[1] : s->h_total[0];
-  s->Mb = block ? s->h_total[0] : 0;
+    // the one host wait of the frame, hidden behind the depth sort
+    CU(cudaEventSynchronize(s->ev_join));
+    CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+    M = s->h_total[0];
+    s->Mb = block ? s->h_total[1] : 0;
+    // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
+    TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm));
+  } else {
+    TRY(run_scan(s, false, s->offsets.as<uint32_t>(), nullptr, &tm));
+    CU(cudaMemcpyAsync(s->h_total, s->small.as<unsigned char>() + 8, 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));   // index-order path: M is only known after the scan
+    M = s->h_total[0];
+  }
   if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
   s->M = M;
 

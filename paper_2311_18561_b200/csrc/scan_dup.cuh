@@ -11,11 +11,12 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 
-// blocks of 8 x 8 tiles touched by a rectangle; tileinfo = (x0 | y0 << 16, w | h << 16, depth bits, count)
-__device__ __forceinline__ uint32_t scan_block_count(const uint4 ti) {
-  if (ti.w == 0u) return 0u;
-  const uint32_t x0 = ti.x & 0xFFFFu, y0 = ti.x >> 16;
-  const uint32_t x1 = x0 + (ti.y & 0xFFFFu) - 1u, y1 = y0 + (ti.y >> 16) - 1u;
+// blocks of 8 x 8 tiles touched by the rectangle packed in the upper half of a sorted depth key
+// (x0, y0, x1, y1, 8 bits each; preprocess.cuh); culled Gaussians carry depth bits 0xFFFFFFFF
+__device__ __forceinline__ uint32_t scan_block_count(uint64_t key) {
+  if ((uint32_t)key == 0xFFFFFFFFu) return 0u;
+  const uint32_t r = (uint32_t)(key >> 32);
+  const uint32_t x0 = r & 0xFFu, y0 = (r >> 8) & 0xFFu, x1 = (r >> 16) & 0xFFu, y1 = r >> 24;
   return ((x1 >> 3) - (x0 >> 3) + 1u) * ((y1 >> 3) - (y0 >> 3) + 1u);
 }
 
@@ -24,14 +25,15 @@ __device__ __forceinline__ uint32_t scan_block_count(const uint4 ti) {
 // published in a 64-bit status word (flag | value) and resolved against predecessor
 // tiles. Tiles are handed out by an atomic ticket so a tile only ever waits on tiles
 // that already started (forward progress without co-residency assumptions).
-//   BLOCKS : false: item count = counts[g]; true: blocks touched by tileinfo[g]'s rectangle
+//   BLOCKS : false: item count = counts[visit[r]]; true: blocks touched by the rectangle in keys[r]
+//            (keys = the depth-sorted keys, already in visiting order)
 //   visit  : visiting order (Gaussian index at position r), or nullptr for identity
 //   offsets: [n] exclusive prefix of counts[visit[r]]
 //   total  : [1] 64-bit sum (M), written by the last tile
 //   status : [num_tiles] zeroed; ticket: [1] zeroed
 template <bool BLOCKS>
 __global__ void __launch_bounds__(SCAN_THREADS)
-scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint4* __restrict__ tileinfo,
+scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64_t* __restrict__ keys,
                    const uint32_t* __restrict__ visit,
                    uint32_t* __restrict__ offsets, uint64_t* __restrict__ total,
                    uint64_t* __restrict__ status, uint32_t* __restrict__ ticket) {
@@ -49,10 +51,7 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint4*
   for (int k = 0; k < SCAN_ITEMS; ++k) {
     const uint32_t r = base + k;
     c[k] = 0;
-    if (r < n) {
-      const uint32_t g = visit ? visit[r] : r;
-      c[k] = BLOCKS ? scan_block_count(tileinfo[g]) : counts[g];
-    }
+    if (r < n) c[k] = BLOCKS ? scan_block_count(keys[r]) : counts[visit ? visit[r] : r];
     tsum += c[k];  // < 2^32: one Gaussian covers at most 2^22 tiles, 8 of them 2^25
   }
   // warp inclusive scan of the thread sums
