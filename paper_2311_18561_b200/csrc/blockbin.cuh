@@ -10,12 +10,12 @@
 //   2. bin_pass: ONE stable onesweep digit pass splits the entries by block id (<= 256 blocks);
 //      inside a block the entries stay in depth order;
 //   (the entries per block, hence bin_start / chunk_start, come from tilebin.cuh's block grid)
-//   3. bin_count / bin_chunk_scan: per chunk of a block's entries, how many entries cover each
-//      of the 64 tiles; an exclusive scan over the chunks, started at the tile's range begin
-//      (tilebin.cuh), gives every chunk its write position in every tile list;
-//   4. bin_write: a warp owns (chunk, 32 of the block's tiles), a lane holds one entry; for
-//      each tile one ballot of "covers it" ranks the 32 entries, and the covering lanes store
-//      their Gaussian index as one contiguous run of that tile's list.
+//   3. bin_write: a warp owns (chunk of 512 entries of a block, 32 of the block's tiles). It counts
+//      how many of its entries cover each tile, and a decoupled look-back over the block's earlier
+//      chunks, started at the tile's range begin (tilebin.cuh), gives its write position in every
+//      tile list. Then, with a lane holding one entry, one ballot of "covers it" per tile ranks 32
+//      entries, and the covering lanes store their Gaussian index as one contiguous run of that
+//      tile's list.
 // The result is bit-identical to the stable LSD sort of the 64-bit keys: within a tile the
 // order is (depth bits, index), exactly the visiting order of the entries.
 #pragma once
@@ -232,16 +232,20 @@ __device__ __forceinline__ uint32_t transpose32(uint32_t x, uint32_t lane) {
   return x;
 }
 
-// Which chunk does this warp own? Fills the entry range [e0, e1) and returns false past the end.
+// Which chunk does this warp own? CTAs take tickets so that a chunk only ever waits (look-back)
+// on chunks whose CTA has already started. Fills the entry range [e0, e1), the block and whether
+// the chunk is the block's first; returns false past the end.
 struct BinWalk {
-  uint32_t chunk, half, e0, e1;
+  uint32_t chunk, half, e0, e1, bin;
+  bool first;
 };
 __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ chunk_start,
-                                               uint32_t* s_cs, BinWalk& w) {
+                                               uint32_t* s_cs, uint32_t* __restrict__ ticket, BinWalk& w) {
+  if (threadIdx.x == 0) s_cs[BB_MAX_BINS + 1] = atomicAdd(ticket, 1u);
   for (uint32_t k = threadIdx.x; k <= BB_MAX_BINS; k += BW_THREADS) s_cs[k] = chunk_start[k];
   __syncthreads();
   const uint32_t warp = threadIdx.x >> 5;
-  w.chunk = blockIdx.x * BW_CHUNKS_PER_CTA + (warp >> 1);
+  w.chunk = s_cs[BB_MAX_BINS + 1] * BW_CHUNKS_PER_CTA + (warp >> 1);
   w.half = warp & 1u;
   if (w.chunk >= s_cs[BB_MAX_BINS]) return false;
   uint32_t lo = 0, hi = BB_MAX_BINS;   // last b with chunk_start[b] <= chunk: the block that owns it
@@ -249,50 +253,11 @@ __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_
     const uint32_t mid = (lo + hi) >> 1;
     if (s_cs[mid] <= w.chunk) lo = mid; else hi = mid;
   }
+  w.bin = lo;
+  w.first = w.chunk == s_cs[lo];
   w.e0 = bin_start[lo] + (w.chunk - s_cs[lo]) * BB_CHUNK;
   w.e1 = min(w.e0 + (uint32_t)BB_CHUNK, bin_start[lo + 1]);
   return true;
-}
-
-// chunk_cnt[chunk][lt] = number of the chunk's entries whose mask covers tile lt of the block
-__global__ void __launch_bounds__(BW_THREADS)
-bin_count_kernel(const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
-                 const uint32_t* __restrict__ chunk_start, uint32_t* __restrict__ chunk_cnt) {
-  __shared__ uint32_t s_cs[BB_MAX_BINS + 1];
-  BinWalk w;
-  if (!bin_walk_setup(bin_start, chunk_start, s_cs, w)) return;
-  const uint32_t lane = threadIdx.x & 31u;
-  uint32_t cnt = 0;
-  for (uint32_t e = w.e0; e < w.e1; e += 32) {
-    const uint64_t m64 = e + lane < w.e1 ? __ldcs(masks + e + lane) : 0ull;
-    const uint32_t m = w.half ? (uint32_t)(m64 >> 32) : (uint32_t)m64;
-    cnt += __popc(transpose32(m, lane));
-  }
-  chunk_cnt[w.chunk * 64u + w.half * 32u + lane] = cnt;
-}
-
-// In place: chunk_cnt[chunk][lt] -> position in tile lt's list where the chunk starts writing
-// (the tile's range begin + the counts of the block's earlier chunks). One CTA per block.
-__global__ void __launch_bounds__(64)
-bin_chunk_scan_kernel(uint32_t* __restrict__ chunk_cnt, const uint32_t* __restrict__ chunk_start,
-                      const uint2* __restrict__ ranges, uint32_t tiles_x, uint32_t tiles_y, uint32_t blocks_x) {
-  const uint32_t b = blockIdx.x, lt = threadIdx.x;
-  const uint32_t tx = (b % blocks_x) * 8u + (lt & 7u), ty = (b / blocks_x) * 8u + (lt >> 3);
-  uint32_t run = (tx < tiles_x && ty < tiles_y) ? ranges[ty * tiles_x + tx].x : 0u;
-  const uint32_t c0 = chunk_start[b], c1 = chunk_start[b + 1];
-  uint32_t c = c0;
-  for (; c + 8 <= c1; c += 8) {
-    uint32_t v[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) v[k] = chunk_cnt[(c + k) * 64u + lt];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) { chunk_cnt[(c + k) * 64u + lt] = run; run += v[k]; }
-  }
-  for (; c < c1; ++c) {
-    const uint32_t v = chunk_cnt[c * 64u + lt];
-    chunk_cnt[c * 64u + lt] = run;
-    run += v;
-  }
 }
 
 // ballot of "bit `bit` of m is set" (test + vote: two instructions)
@@ -332,17 +297,22 @@ __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 3
   }
 }
 
+// status[chunk][64]: 64-bit look-back words (flag | position), zeroed. A chunk first counts, per tile,
+// how many of its entries cover it (bit-matrix transpose + popcount), publishes the counts, resolves
+// where it starts in every tile list by looking back over the earlier chunks of its block (the block's
+// first chunk starts at the tile's range begin), and then writes.
 __global__ void __launch_bounds__(BW_THREADS)
 bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
-                 const uint32_t* __restrict__ chunk_start, const uint32_t* __restrict__ chunk_pos,
+                 const uint32_t* __restrict__ chunk_start, const uint2* __restrict__ ranges, uint32_t tiles_x,
+                 uint32_t tiles_y, uint32_t blocks_x, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
                  uint32_t* __restrict__ vals) {
-  __shared__ uint32_t s_cs[BB_MAX_BINS + 1];
+  __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
   // the base pointer round-trips through shared memory so that it lives in registers; taken from the
   // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
   __shared__ uint32_t* s_vals;
   if (threadIdx.x == 0) s_vals = vals;
   BinWalk w;
-  if (!bin_walk_setup(bin_start, chunk_start, s_cs, w)) return;   // (contains the barrier)
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w)) return;   // (contains the barrier)
   uint32_t* const vp = s_vals;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t lt = lanemask_lt();
@@ -356,7 +326,31 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
     m[b] = ok ? __ldcs(mp + 2 * (size_t)e) : 0u;
     g[b] = ok ? __ldcs(gs + e) : 0u;
   }
-  const uint32_t mypos = chunk_pos[w.chunk * 64u + w.half * 32u + lane];
+  // lane = tile (half * 32 + lane) of the block from here to the end of the look-back
+  uint32_t cnt = 0;
+#pragma unroll
+  for (int b = 0; b < NB; ++b) cnt += __popc(transpose32(m[b], lane));
+  uint64_t* my = status + (size_t)w.chunk * 64u + w.half * 32u + lane;
+  uint32_t mypos;
+  if (w.first) {
+    const uint32_t ltile = w.half * 32u + lane;
+    const uint32_t tx = (w.bin % blocks_x) * 8u + (ltile & 7u), ty = (w.bin / blocks_x) * 8u + (ltile >> 3);
+    mypos = (tx < tiles_x && ty < tiles_y) ? ranges[ty * tiles_x + tx].x : 0u;
+  } else {
+    st_relaxed_u64(my, LB_FLAG_AGG | cnt);
+    mypos = 0;
+    const uint64_t* p = my - 64;
+    while (true) {
+      const uint64_t v = ld_relaxed_u64(p);
+      const uint64_t flag = v & LB_FLAG_MASK;
+      if (flag == 0) continue;   // that chunk's CTA holds an earlier ticket: it is running
+      mypos += (uint32_t)v;
+      if (flag == LB_FLAG_PREFIX) break;
+      p -= 64;
+    }
+  }
+  st_relaxed_u64(my, LB_FLAG_PREFIX | (uint64_t)(mypos + cnt));
+  __syncwarp();
   const uint32_t nb = (w.e1 - w.e0 + 31u) >> 5;
   if (nb == NB) bin_write_tiles<true>(m, g, nb, mypos, lt, vp);
   else bin_write_tiles<false>(m, g, nb, mypos, lt, vp);

@@ -482,13 +482,14 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(s->e_mask.reserve((size_t)Mb * 8, st, 1.125));
   TRY(s->s_g.reserve((size_t)Mb * 4, st, 1.125));
   TRY(s->s_mask.reserve((size_t)Mb * 8, st, 1.125));
-  TRY(s->chunk_cnt.reserve((size_t)max_chunks * 64 * 4, st, 1.125));
+  TRY(s->chunk_cnt.reserve((size_t)max_chunks * 64 * 8, st, 1.125));   // look-back words of bin_write
   TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
   TRY(s->sort_m.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
   uint32_t* chunk_start = bin_start + 257;
   uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
-  CU(cudaMemsetAsync(ticket, 0, 4, st));
+  CU(cudaMemsetAsync(ticket, 0, 8, st));
+  CU(cudaMemsetAsync(s->chunk_cnt.p, 0, (size_t)max_chunks * 64 * 8, st));
   CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, st));
 
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
@@ -509,17 +510,10 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(tm->end(st));
 
   const unsigned walk_grid = (max_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
-  TRY(tm->begin("bin_count", PVG_STAGE_SORT, st));
-  bin_count_kernel<<<walk_grid, BW_THREADS, 0, st>>>(s->s_mask.as<uint64_t>(), bin_start, chunk_start,
-                                                     s->chunk_cnt.as<uint32_t>());
-  TRY(tm->end(st));
-  TRY(tm->begin("bin_chunk_scan", PVG_STAGE_SORT, st));
-  bin_chunk_scan_kernel<<<nbins, 64, 0, st>>>(s->chunk_cnt.as<uint32_t>(), chunk_start, s->ranges.as<uint2>(),
-                                              (uint32_t)P.tiles_x, (uint32_t)P.tiles_y, blocks_x);
-  TRY(tm->end(st));
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
   bin_write_kernel<<<walk_grid, BW_THREADS, 0, st>>>(s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, chunk_start,
-                                                     s->chunk_cnt.as<uint32_t>(), s->vals[0].as<uint32_t>());
+                                                     s->ranges.as<uint2>(), (uint32_t)P.tiles_x, (uint32_t)P.tiles_y, blocks_x,
+                                                     s->chunk_cnt.as<uint64_t>(), ticket + 1, s->vals[0].as<uint32_t>());
   TRY(tm->end(st));
   CU(cudaGetLastError());
   s->sorted_side = 0;
