@@ -236,7 +236,7 @@ __device__ __forceinline__ uint32_t transpose32(uint32_t x, uint32_t lane) {
 // on chunks whose CTA has already started. Fills the entry range [e0, e1), the block and whether
 // the chunk is the block's first; returns false past the end.
 struct BinWalk {
-  uint32_t chunk, half, e0, e1, bin;
+  uint32_t chunk, half, e0, e1, bin, kin;   // kin: index of the chunk inside its block
   bool first;
 };
 __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ chunk_start,
@@ -254,7 +254,8 @@ __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_
     if (s_cs[mid] <= w.chunk) lo = mid; else hi = mid;
   }
   w.bin = lo;
-  w.first = w.chunk == s_cs[lo];
+  w.kin = w.chunk - s_cs[lo];
+  w.first = w.kin == 0;
   w.e0 = bin_start[lo] + (w.chunk - s_cs[lo]) * BB_CHUNK;
   w.e1 = min(w.e0 + (uint32_t)BB_CHUNK, bin_start[lo + 1]);
   return true;
@@ -280,18 +281,31 @@ __device__ __forceinline__ uint32_t ballot_bit(uint32_t m, uint32_t bit) {
 // it" ranks the 32 entries of a batch, and the covering lanes store their Gaussian index at consecutive
 // positions of that tile's list. The 16 stores of a tile are issued back to back and extend one
 // contiguous run (~1 KB), so L2 sees whole lines and DRAM whole bursts.
+// s_ptr[l][b]: where batch b's covering entries of tile l go (a pointer into the tile's list), laid down
+// by lane l after the look-back. A step is then: test my mask bit, ballot, rank = popcount below my lane,
+// address, store -- six instructions plus half a broadcast shared load.
+// Measured alternatives (cfg 3, profiles/): a running position advanced by a second popcount per step
+// (XU pipe 80% busy), per-batch offsets fetched by shuffles (0.34 ms), the transposed coverage word
+// fetched by a shuffle instead of the ballot (0.55 ms: the shuffle path saturates first), compacting each
+// tile's run in shared memory and storing whole aligned lines (0.43 ms: more instructions, and the
+// partial-line stores were never the limiter -- L2 merges them).
 template <bool FULL>
 __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 32], const uint32_t (&g)[BB_CHUNK / 32],
-                                                uint32_t nb, uint32_t mypos, uint32_t lt, uint32_t* vp) {
+                                                const uint4* s_ptr /* [32 tiles][8] of this warp */, uint32_t nb,
+                                                uint32_t lt) {
   for (uint32_t l = 0; l < 32; ++l) {
-    uint32_t run = __shfl_sync(0xffffffffu, mypos, l);
     const uint32_t bit = 1u << l;
 #pragma unroll
-    for (int b = 0; b < BB_CHUNK / 32; ++b) {
-      if (FULL || b < nb) {
-        const uint32_t wl = ballot_bit(m[b], bit);
-        if (m[b] & bit) asm volatile("st.global.u32 [%0], %1;" ::"l"(vp + (run + __popc(wl & lt))), "r"(g[b]) : "memory");
-        run += __popc(wl);
+    for (int k = 0; k < BB_CHUNK / 64; ++k) {
+      const uint4 q = s_ptr[8 * l + k];   // two pointers, broadcast
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int b = 2 * k + h;
+        if (FULL || b < nb) {
+          const uint32_t wl = ballot_bit(m[b], bit);
+          uint32_t* dst = reinterpret_cast<uint32_t*>(h ? ((uint64_t)q.w << 32 | q.z) : ((uint64_t)q.y << 32 | q.x));
+          if (m[b] & bit) asm volatile("st.global.u32 [%0], %1;" ::"l"(dst + __popc(wl & lt)), "r"(g[b]) : "memory");
+        }
       }
     }
   }
@@ -301,7 +315,7 @@ __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 3
 // how many of its entries cover it (bit-matrix transpose + popcount), publishes the counts, resolves
 // where it starts in every tile list by looking back over the earlier chunks of its block (the block's
 // first chunk starts at the tile's range begin), and then writes.
-__global__ void __launch_bounds__(BW_THREADS)
+__global__ void __launch_bounds__(BW_THREADS, 4)
 bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
                  const uint32_t* __restrict__ chunk_start, const uint2* __restrict__ ranges, uint32_t tiles_x,
                  uint32_t tiles_y, uint32_t blocks_x, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
@@ -310,6 +324,7 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
   // the base pointer round-trips through shared memory so that it lives in registers; taken from the
   // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
   __shared__ uint32_t* s_vals;
+  __shared__ uint4 s_ptr[BW_THREADS / 32][32 * BB_CHUNK / 64];
   if (threadIdx.x == 0) s_vals = vals;
   BinWalk w;
   if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w)) return;   // (contains the barrier)
@@ -328,8 +343,12 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
   }
   // lane = tile (half * 32 + lane) of the block from here to the end of the look-back
   uint32_t cnt = 0;
+  uint32_t pre[NB];   // covering entries of my tile in the batches before batch b
 #pragma unroll
-  for (int b = 0; b < NB; ++b) cnt += __popc(transpose32(m[b], lane));
+  for (int b = 0; b < NB; ++b) {
+    pre[b] = cnt;
+    cnt += __popc(transpose32(m[b], lane));
+  }
   uint64_t* my = status + (size_t)w.chunk * 64u + w.half * 32u + lane;
   uint32_t mypos;
   if (w.first) {
@@ -339,21 +358,47 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
   } else {
     st_relaxed_u64(my, LB_FLAG_AGG | cnt);
     mypos = 0;
+    // windowed look-back: the status words of the next LB_WINDOW predecessors are fetched together (the
+    // chunks of a wave start at the same time, so their prefixes lag and the walk can be long), then
+    // consumed in order up to the first one that is not published yet
+    constexpr int LB_WINDOW = 4;
     const uint64_t* p = my - 64;
-    while (true) {
-      const uint64_t v = ld_relaxed_u64(p);
-      const uint64_t flag = v & LB_FLAG_MASK;
-      if (flag == 0) continue;   // that chunk's CTA holds an earlier ticket: it is running
-      mypos += (uint32_t)v;
-      if (flag == LB_FLAG_PREFIX) break;
-      p -= 64;
+    uint32_t left = w.kin;   // predecessors inside the block; the block's first chunk always ends the walk
+    bool done = false;
+    while (!done) {
+      uint64_t v[LB_WINDOW];
+#pragma unroll
+      for (int k = 0; k < LB_WINDOW; ++k) v[k] = (uint32_t)k < left ? ld_relaxed_u64(p - 64 * k) : 0ull;
+      uint32_t used = 0;
+      bool open = true;
+#pragma unroll
+      for (int k = 0; k < LB_WINDOW; ++k) {
+        const uint64_t flag = v[k] & LB_FLAG_MASK;
+        open = open && flag != 0;   // a zero flag: that chunk's CTA holds an earlier ticket, it is running
+        if (open) {
+          mypos += (uint32_t)v[k];
+          ++used;
+          if (flag == LB_FLAG_PREFIX) { done = true; open = false; }
+        }
+      }
+      p -= 64 * used;
+      left -= used;
     }
   }
   st_relaxed_u64(my, LB_FLAG_PREFIX | (uint64_t)(mypos + cnt));
+  uint4* sp = s_ptr[threadIdx.x >> 5];
+  {
+    const uint64_t base = reinterpret_cast<uint64_t>(vp + mypos);
+#pragma unroll
+    for (int k = 0; k < NB / 2; ++k) {
+      const uint64_t a = base + 4ull * pre[2 * k], c = base + 4ull * pre[2 * k + 1];
+      sp[8 * lane + k] = make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)c, (uint32_t)(c >> 32));
+    }
+  }
   __syncwarp();
   const uint32_t nb = (w.e1 - w.e0 + 31u) >> 5;
-  if (nb == NB) bin_write_tiles<true>(m, g, nb, mypos, lt, vp);
-  else bin_write_tiles<false>(m, g, nb, mypos, lt, vp);
+  if (nb == NB) bin_write_tiles<true>(m, g, sp, nb, lt);
+  else bin_write_tiles<false>(m, g, sp, nb, lt);
 }
 
 }  // namespace pvg
