@@ -212,14 +212,30 @@ struct RadixCore {
         // resolve the exclusive prefix of this digit over earlier tiles
         uint32_t excl = 0;
         if (tile != 0) {
-          int64_t p = (int64_t)tile - 1;
-          while (true) {
-            const uint64_t v = ld_relaxed_u64(lookback + (uint64_t)p * RADIX + tid);
-            const uint64_t flag = v & LB_FLAG_MASK;
-            if (flag == 0) continue;  // that tile holds an earlier ticket: it is running
-            excl += (uint32_t)v;
-            if (flag == LB_FLAG_PREFIX) break;
-            --p;
+          // windowed: the status words of the next LB_WINDOW predecessors are fetched together (one L2
+          // round trip), then consumed in order up to the first one that is not published yet
+          constexpr int LB_WINDOW = 4;
+          uint32_t left = tile;   // predecessors not yet consumed; tile 0 always ends the walk
+          const uint64_t* p = lookback + (uint64_t)(tile - 1) * RADIX + tid;
+          bool done = false;
+          while (!done) {
+            uint64_t v[LB_WINDOW];
+#pragma unroll
+            for (int k = 0; k < LB_WINDOW; ++k) v[k] = (uint32_t)k < left ? ld_relaxed_u64(p - (size_t)k * RADIX) : 0ull;
+            uint32_t used = 0;
+            bool open = true;
+#pragma unroll
+            for (int k = 0; k < LB_WINDOW; ++k) {
+              const uint64_t flag = v[k] & LB_FLAG_MASK;
+              open = open && flag != 0;   // zero: that tile holds an earlier ticket, it is running
+              if (open) {
+                excl += (uint32_t)v[k];
+                ++used;
+                if (flag == LB_FLAG_PREFIX) { done = true; open = false; }
+              }
+            }
+            p -= (size_t)used * RADIX;
+            left -= used;
           }
           st_relaxed_u64(my, LB_FLAG_PREFIX | (uint64_t)(uint32_t)(excl + tile_count));
         }
@@ -243,7 +259,9 @@ struct OnesweepSmem {
 // The digit is bits [shift32, shift32+BITS) of the key's upper (HI = 1) or lower 32-bit
 // half (make_sort_plan never lets a pass straddle bit 32). Elements are re-ordered through
 // shared memory and written out in digit runs so that stores are coalesced.
-template <int THREADS, int ITEMS, int BITS, int MINB, int HI>
+// STREAM: read the pairs with evict-first loads (lists far larger than L2); otherwise leave them in L2
+// for the next pass (the n-key depth sort: 36 MB at 3M Gaussians).
+template <int THREADS, int ITEMS, int BITS, int MINB, int HI, bool STREAM>
 __global__ void __launch_bounds__(THREADS, MINB)
 onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                      uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint32_t n,
@@ -270,15 +288,15 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
   uint32_t val[ITEMS];
   if (tile_n == TILE) {
 #pragma unroll
-    for (int j = 0; j < ITEMS; ++j) key[j] = __ldcs(kp + j * 32);
+    for (int j = 0; j < ITEMS; ++j) key[j] = STREAM ? __ldcs(kp + j * 32) : __ldcg(kp + j * 32);
 #pragma unroll
-    for (int j = 0; j < ITEMS; ++j) val[j] = __ldcs(vp + j * 32);
+    for (int j = 0; j < ITEMS; ++j) val[j] = STREAM ? __ldcs(vp + j * 32) : __ldcg(vp + j * 32);
   } else {
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
       const bool ok = wbase + j * 32 < tile_n;
-      key[j] = ok ? __ldcs(kp + j * 32) : ~0ull;
-      val[j] = ok ? __ldcs(vp + j * 32) : 0u;
+      key[j] = ok ? (STREAM ? __ldcs(kp + j * 32) : __ldcg(kp + j * 32)) : ~0ull;
+      val[j] = ok ? (STREAM ? __ldcs(vp + j * 32) : __ldcg(vp + j * 32)) : 0u;
     }
   }
   uint32_t dp[ITEMS];

@@ -94,8 +94,8 @@ struct KernelRec {
 #define PVG_OSL_ITEMS 16
 #define PVG_OSL_MINB 2
 #endif
-struct OsLarge { static constexpr int THREADS = PVG_OSL_THREADS, ITEMS = PVG_OSL_ITEMS, MINB = PVG_OSL_MINB; };
-struct OsSmall { static constexpr int THREADS = 256, ITEMS = 8, MINB = 4; };
+struct OsLarge { static constexpr int THREADS = PVG_OSL_THREADS, ITEMS = PVG_OSL_ITEMS, MINB = PVG_OSL_MINB; static constexpr bool STREAM = true; };
+struct OsSmall { static constexpr int THREADS = 256, ITEMS = 8, MINB = 4; static constexpr bool STREAM = false; };
 constexpr uint64_t OS_SMALL_BELOW = 8u << 20;
 
 // scratch of one sort call
@@ -147,7 +147,7 @@ template <class Cfg, int BITS, int HI>
 int launch_pass_bits(const uint64_t* kin, const uint32_t* vin, uint64_t* kout, uint32_t* vout, uint32_t n, int shift,
                      const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
   using Smem = OnesweepSmem<Cfg::THREADS, Cfg::ITEMS, BITS>;
-  auto kern = onesweep_pass_kernel<Cfg::THREADS, Cfg::ITEMS, BITS, Cfg::MINB, HI>;
+  auto kern = onesweep_pass_kernel<Cfg::THREADS, Cfg::ITEMS, BITS, Cfg::MINB, HI, Cfg::STREAM>;
   static bool configured = false;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
