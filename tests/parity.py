@@ -69,7 +69,17 @@ def check_record(gpu_rec: np.ndarray, wide: np.ndarray, cam, scene):
     assert np.all(err["mean_px"] <= mean_tol), ("mean2d", stats["max_mean_err_over_tol"])
     assert err["z_rel"].max() <= 2e-6 + 0, ("z", stats["max_z_rel"])
     assert err["op_rel"].max() <= 2e-5, ("opacity", stats["max_op_rel"])
-    assert err["conic_rel"].max() <= 2e-5, ("conic", stats["max_conic_rel"])
+    # conic: the fp32 covariance U U^T (U = J W R(q) diag(s)) carries an absolute error of C eps |T_row|^2 s_max^2
+    # per entry, |T_row|^2 <= (f/z)^2 (1 + tx^2 + ty^2); relative to the smaller diagonal entry that is
+    # C eps amp with amp >= 1 large for needles seen end-on. Measured C = 11.7 over 3M Gaussians (cfg 3) and
+    # 10.2 over 200k (cfg 1): the model holds across sizes; the bound uses C = 24.
+    smax = scene.scale[both].astype(np.float64).max(1)
+    limx, limy = 1.3 * width / (2.0 * float(cam.fx)), 1.3 * height / (2.0 * float(cam.fy))
+    txc, tyc = np.clip(w[:, 4] / zc, -limx, limx), np.clip(w[:, 5] / zc, -limy, limy)
+    amp = (f / zc) ** 2 * (1.0 + txc ** 2 + tyc ** 2) * smax ** 2 / np.minimum(cov[:, 0], cov[:, 2])
+    conic_tol = 24 * eps * np.maximum(amp, 1.0)
+    stats["max_conic_err_over_tol"] = float((err["conic_rel"] / conic_tol).max())
+    assert np.all(err["conic_rel"] <= conic_tol), ("conic", stats["max_conic_rel"], stats["max_conic_err_over_tol"])
     # h = sqrt(2 ln(255 o~) Sigma'): near the opacity cutoff the logarithm is ~0 and carries an
     # absolute fp32 error of ~1e-6, i.e. a relative error 1e-6 / k in k and half that in h
     kk = 2.0 * np.log(255.0 * w[:, 3])
@@ -110,7 +120,8 @@ def check_integer_chain(dbg: dict, width: int, height: int, presort: bool):
     return dict(M=M, max_count=int(counts.max()), mean_list=float(M / max(1, k["ranges"].shape[0])))
 
 
-def check_images(gpu, ora, z_max: float, tol_rgb: float = TOL_RGB, with_cond: bool = True, label: str = ""):
+def check_images(gpu, ora, z_max: float, tol_rgb: float = TOL_RGB, with_cond: bool = True, label: str = "",
+                 max_fragile_frac: float = 0.01):
     """(R): per pixel |rgb_gpu - rgb_oracle| <= tol + budget (+ fp32 conditioning allowance),
     depth within 1e-3 relative + budget * z_max / alpha. gpu = (rgb, depth, alpha) float32 arrays."""
     rgb, depth, alpha = (np.asarray(x, dtype=np.float64) for x in gpu)
@@ -134,5 +145,7 @@ def check_images(gpu, ora, z_max: float, tol_rgb: float = TOL_RGB, with_cond: bo
     assert not bad_rgb.any(), ("rgb", stats)
     assert not bad_alpha.any(), ("alpha", stats)
     assert not bad_depth.any(), ("depth", stats)
-    assert stats["fragile_pixels"] <= 0.01 * stats["pixels"], ("too many fragile pixels", stats)
+    # the share of pixels with a non-zero budget grows with the number of candidates per pixel (each one is a
+    # chance to land within 1e-4 of a threshold): 0.4-0.6 % at configs 0-3, a few % at the stress config
+    assert stats["fragile_pixels"] <= max_fragile_frac * stats["pixels"], ("too many fragile pixels", stats)
     return stats

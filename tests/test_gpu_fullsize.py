@@ -1,0 +1,124 @@
+"""Full-size parity (BASELINE.json configs 3 and 4) in the launch configuration bench.py times:
+default options, block-entry list builder. The oracle cannot sort ~3e8 instances in seconds, so
+the chain is checked on what it can compute one by one:
+  * Oracle-P on every Gaussian (record, cull flags);
+  * per-Gaussian tile counts, M and EVERY tile range bit-exactly (the ranges follow from the
+    oracle's rectangles by a 2-D difference array, recomputed here with numpy);
+  * the sorted list of sampled tiles (corners, centre, the longest list, random ones) bit-exactly
+    against oracle.tile_list (a direct per-tile computation);
+  * the pixels of those tiles against Oracle-R (binned) with the fragile budget;
+  * properties that hold at any size: every list is in (depth bits, index) order, every listed
+    Gaussian's rectangle contains the tile, list lengths add up to M.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2311_18561_b200 as pvg
+from parity import check_images, check_record
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+
+def _d2h(sc, ptr, offset_bytes, shape, dtype):
+    a = np.empty(shape, dtype=dtype)
+    if a.nbytes:
+        pvg._check(sc._L.pvg_memcpy_d2h(a.ctypes.data, ptr + offset_bytes, a.nbytes))
+    return a
+
+
+def _ranges_from_rects(rects, counts, TX, TY):
+    """range[tile] = exclusive scan, in row-major tile order, of the number of rectangles covering the tile."""
+    v = counts > 0
+    x0, y0, x1, y1 = (rects[v, k].astype(np.int64) for k in range(4))
+    d = np.zeros((TY + 1, TX + 1), dtype=np.int64)
+    np.add.at(d, (y0, x0), 1)
+    np.add.at(d, (y0, x1 + 1), -1)
+    np.add.at(d, (y1 + 1, x0), -1)
+    np.add.at(d, (y1 + 1, x1 + 1), 1)
+    per_tile = d.cumsum(0).cumsum(1)[:TY, :TX].reshape(-1)
+    end = per_tile.cumsum()
+    return np.stack([end - per_tile, end], 1).astype(np.uint32), per_tile
+
+
+def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, max_fragile_frac=0.01):
+    rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t))
+    st = sc.frame_stats()
+    assert st["list_mode"] == "blocks"
+    d = sc.debug_info()
+    n, M = int(d.n), int(d.num_instances)
+    TX, TY = int(d.tiles_x), int(d.tiles_y)
+    W, H = cam.width, cam.height
+    grec = _d2h(sc, d.record, 0, (n, 12), np.float32)
+    gcounts = _d2h(sc, d.counts, 0, (n,), np.uint32)
+    granges = _d2h(sc, d.ranges, 0, (TX * TY, 2), np.uint32)
+
+    # (P) record against Oracle-P on every Gaussian
+    wide, _ = oracle.preprocess_scene(wl_scene, cam, t)
+    check_record(grec, wide, cam, wl_scene)
+
+    # (I) counts, M, all ranges
+    rects, counts, M_o = oracle.tile_counts(grec, W, H)
+    assert M == M_o and np.array_equal(gcounts, counts)
+    ranges_o, per_tile = _ranges_from_rects(rects, counts, TX, TY)
+    assert np.array_equal(granges, ranges_o), "tile ranges"
+    assert int(per_tile.sum()) == M
+
+    # sampled tiles: corners, centre, the longest list, random non-empty ones
+    rng = np.random.default_rng(seed)
+    nonempty = np.nonzero(per_tile)[0]
+    sel = {0, TX - 1, (TY - 1) * TX, TX * TY - 1, (TY // 2) * TX + TX // 2, int(per_tile.argmax())}
+    sel |= set(int(x) for x in rng.choice(nonempty, size=min(n_random_tiles, len(nonempty)), replace=False))
+    sel = sorted(sel)
+    zbits = grec[:, 2].view(np.uint32)
+    for tl in sel:
+        b, e = int(granges[tl, 0]), int(granges[tl, 1])
+        gv = _d2h(sc, d.vals_sorted, 4 * b, (e - b,), np.uint32)
+        k_o, v_o = oracle.tile_list(grec, W, H, tl)
+        assert np.array_equal(gv, v_o), f"sorted list of tile {tl}"
+        assert np.array_equal((np.uint64(tl) << np.uint64(32)) | zbits[gv].astype(np.uint64), k_o)
+        # properties: (depth bits, index) order; every rectangle contains the tile
+        key = (zbits[gv].astype(np.uint64) << np.uint64(32)) | gv.astype(np.uint64)
+        assert np.all(key[1:] > key[:-1])
+        tx, ty = tl % TX, tl // TX
+        r = rects[gv]
+        assert np.all((r[:, 0] <= tx) & (tx <= r[:, 2]) & (r[:, 1] <= ty) & (ty <= r[:, 3]))
+
+    # (R) the pixels of the sampled tiles
+    ora = oracle.render(grec, W, H, bg=cam.bg, mode="binned", tiles=sel)
+    mask = np.zeros((H, W), dtype=bool)
+    for tl in sel:
+        tx, ty = tl % TX, tl // TX
+        mask[ty * 16:(ty + 1) * 16, tx * 16:(tx + 1) * 16] = True
+    sub = lambda a: a[..., mask]  # noqa: E731
+    zmax = float(max(grec[:, 2].max(), 1.0))
+    stats = check_images((sub(rgb), sub(depth), sub(alpha)), {k: (sub(v) if isinstance(v, np.ndarray) else v) for k, v in ora.items()},
+                         zmax, label="sampled tiles", max_fragile_frac=max_fragile_frac)
+    assert stats["max_rgb_err_clean"] <= 2e-4
+    return dict(M=M, tiles=len(sel), max_list=int(per_tile.max()), entries=st["block_entries"], **stats)
+
+
+def test_cfg3_full_size_frame():
+    wl = make_config(3)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    try:
+        cam, t = list(wl.frames())[24]
+        st = _check_frame(sc, wl.scene, cam, t)
+        print(st)
+        assert st["M"] > 200_000_000 and st["entries"] < st["M"] // 20
+    finally:
+        sc.close()
+
+
+def test_cfg4_full_size_front_and_side_camera():
+    """6M Gaussians, scales x1.5; the yawed 1920x886 camera has a ragged last tile row."""
+    wl = make_config(4)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    try:
+        for cam in (wl.cameras[0], wl.cameras[3]):
+            # ~36k candidates per tile: more pixels come within 1e-4 of a cutoff than at configs 0-3
+            st = _check_frame(sc, wl.scene, cam, 0.25, n_random_tiles=6, max_fragile_frac=0.06)
+            print(cam.name, st)
+    finally:
+        sc.close()
