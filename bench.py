@@ -298,7 +298,7 @@ def run_ours(args):
     # ---- per-kernel aggregation and roofline
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     N = wl.scene.n
-    S = int((scene.debug(["counts"])["counts"] > 0).sum())
+    S = scene.frame_stats()["survivors"] or N
     Msum, Mbsum = float(sum(Ms)), float(sum(Mbs))
     K = len(sched)
     list_mode = scene.frame_stats()["list_mode"]

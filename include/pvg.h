@@ -171,8 +171,9 @@ int pvg_stage_times_ms(pvg_scene *scene, float ms[PVG_NUM_STAGES]);
 int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stages, float *ms);
 
 /* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y,
- * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries}. */
-int pvg_frame_stats(pvg_scene *scene, uint64_t out[6]);
+ * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries,
+ * surviving Gaussians S (PRESORT_DEPTH=1, else 0), reserved}. */
+int pvg_frame_stats(pvg_scene *scene, uint64_t out[8]);
 
 /* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs
  * evaluated before the pixel stopped, out[1] = pairs that contributed (alpha >= 1/255). */

@@ -238,10 +238,11 @@ class Scene:
 
     def frame_stats(self) -> Dict[str, int]:
         """Sizes of the last render (no device work)."""
-        out = (C.c_uint64 * 6)()
+        out = (C.c_uint64 * 8)()
         _check(self._L.pvg_frame_stats(self._h, out))
         return {"n": int(out[0]), "M": int(out[1]), "tiles_x": int(out[2]), "tiles_y": int(out[3]),
-                "block_entries": int(out[4]), "list_mode": ("keys64", "compact", "blocks")[int(out[5])]}
+                "block_entries": int(out[4]), "list_mode": ("keys64", "compact", "blocks")[int(out[5])],
+                "survivors": int(out[6])}
 
     def blend_counters(self) -> Tuple[int, int]:
         """(pairs evaluated, pairs contributing) of the last render with OPT_COUNT_PAIRS=1."""

@@ -297,7 +297,7 @@ __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 3
     const uint32_t bit = 1u << l;
 #pragma unroll
     for (int k = 0; k < BB_CHUNK / 64; ++k) {
-      const uint4 q = s_ptr[8 * l + k];   // two pointers, broadcast
+      const uint4 q = s_ptr[8 * l + (k ^ (l & 7u))];   // two pointers, broadcast (slot swizzled: conflict-free writes)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const int b = 2 * k + h;
@@ -392,7 +392,7 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
 #pragma unroll
     for (int k = 0; k < NB / 2; ++k) {
       const uint64_t a = base + 4ull * pre[2 * k], c = base + 4ull * pre[2 * k + 1];
-      sp[8 * lane + k] = make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)c, (uint32_t)(c >> 32));
+      sp[8 * lane + (k ^ (lane & 7u))] = make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)c, (uint32_t)(c >> 32));
     }
   }
   __syncwarp();

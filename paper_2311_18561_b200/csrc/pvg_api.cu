@@ -314,7 +314,7 @@ struct pvg_scene {
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   Timer timer;
   // last frame
-  uint64_t M = 0, Mb = 0;
+  uint64_t M = 0, Mb = 0, survivors = 0;
   FrameParams last_P{};
   int sorted_side = 0, visit_side = 0;
   uint32_t tiles_x = 0, tiles_y = 0;
@@ -570,13 +570,13 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
       attr_set = true;
     }
     const size_t grid_bytes = ((size_t)tilegrid_cells(P.tiles_x, P.tiles_y) +
-                               (block ? (size_t)tilegrid_cells((int)blocks_x, (int)blocks_y) : 0)) * 4;
+                               (block ? (size_t)tilegrid_cells((int)blocks_x, (int)blocks_y) : 0)) * 4;   // + 1 cell: survivor count
     const int use_smem = grid_bytes <= kMaxDyn ? 1 : 0;
-    TRY(s->tilegrid.reserve(grid_bytes, st));
+    TRY(s->tilegrid.reserve(grid_bytes + 4, st));
     TRY(s->sort_m.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
     TRY(s->bin_tables.reserve(4096, st));   // bin_start[257] | chunk_start[257]
     int* grid = s->tilegrid.as<int>();
-    CU(cudaMemsetAsync(grid, 0, grid_bytes, sd));
+    CU(cudaMemsetAsync(grid, 0, grid_bytes + 4, sd));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -592,7 +592,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
         s->ranges.as<uint2>(), s->sort_m.hist.as<uint32_t>(), totals, s->bin_tables.as<uint32_t>(),
         s->bin_tables.as<uint32_t>() + 257);
     TRY(tm.end(sd));
-    CU(cudaMemcpyAsync(s->h_total, totals, 16, cudaMemcpyDeviceToHost, sd));
+    CU(cudaMemcpyAsync(s->h_total, totals, 24, cudaMemcpyDeviceToHost, sd));
     CU(cudaEventRecord(s->ev_join, sd));
 
     // a3 (n-key part): depth order of the Gaussians
@@ -607,6 +607,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, fl
     CU(cudaStreamWaitEvent(st, s->ev_join, 0));
     M = s->h_total[0];
     s->Mb = block ? s->h_total[1] : 0;
+    s->survivors = s->h_total[2];
     // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
     TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm));
   } else {
@@ -895,7 +896,7 @@ int pvg_stage_times_ms(pvg_scene* s, float ms[PVG_NUM_STAGES]) {
   return PVG_OK;
 }
 
-int pvg_frame_stats(pvg_scene* s, uint64_t out[6]) {
+int pvg_frame_stats(pvg_scene* s, uint64_t out[8]) {
   if (!s || !out) return PVG_ERR_NULL;
   out[0] = s->n;
   out[1] = s->rendered ? s->M : 0;
@@ -903,6 +904,8 @@ int pvg_frame_stats(pvg_scene* s, uint64_t out[6]) {
   out[3] = s->tiles_y;
   out[4] = s->rendered ? s->Mb : 0;
   out[5] = s->block_used ? 2 : (s->compact_used ? 1 : 0);
+  out[6] = (s->rendered && s->presort) ? s->survivors : 0;
+  out[7] = 0;
   return PVG_OK;
 }
 

@@ -50,9 +50,11 @@ tile_grid_kernel(const uint4* __restrict__ tileinfo, uint32_t n, int TX, int TY,
     g = s_grid;
   }
   int* gb = g + cells;
+  uint32_t survivors = 0;
   for (uint32_t i = blockIdx.x * TG_THREADS + threadIdx.x; i < n; i += gridDim.x * TG_THREADS) {
     const uint4 ti = tileinfo[i];
     if (ti.w == 0u) continue;
+    ++survivors;
     const int x0 = (int)(ti.x & 0xFFFFu), y0 = (int)(ti.x >> 16);
     const int x1 = x0 + (int)(ti.y & 0xFFFFu) - 1, y1 = y0 + (int)(ti.y >> 16) - 1;
     tilegrid_add_rect(g, stride, x0, y0, x1, y1);
@@ -65,6 +67,9 @@ tile_grid_kernel(const uint4* __restrict__ tileinfo, uint32_t n, int TX, int TY,
       if (v) atomicAdd(grid + k, v);
     }
   }
+  // number of surviving Gaussians S (a statistic for pvg_frame_stats): one extra cell after the grids
+  survivors = __reduce_add_sync(0xffffffffu, survivors);
+  if ((threadIdx.x & 31u) == 0 && survivors) atomicAdd(grid + cells + bcells, (int)survivors);
 }
 
 constexpr int TB_THREADS = 1024;
@@ -89,7 +94,7 @@ __device__ __forceinline__ void grid_prefix_2d(int* g, int rows, int cols, int s
 // plan.shift[] are KEY bit positions (tile id sits at bit 32).
 //   ranges[tile]            = [begin, end) of the tile in the sorted list
 //   hist[pass][256]         = exclusive digit histograms of the tile-id passes
-//   totals[0] = M (tile instances), totals[1] = Mb (block entries; with_blocks)
+//   totals[0] = M (tile instances), totals[1] = Mb (block entries; with_blocks), totals[2] = S (survivors)
 //   bin_start[257], chunk_start[257] (with_blocks): see blockbin.cuh
 __global__ void __launch_bounds__(TB_THREADS)
 tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int with_blocks, const __grid_constant__ SortPlan plan,
@@ -145,7 +150,7 @@ tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int wit
       }
     run += c;
   }
-  if (tid == 0) totals[0] = all;
+  if (tid == 0) { totals[0] = all; totals[2] = (uint32_t)grid[cells + bcells]; }
   __syncthreads();
   // exclusive scan of each pass's histogram (256 threads per pass)
   for (int p = 0; p < plan.num_passes; ++p) {
