@@ -10,10 +10,10 @@
 
 namespace pvg {
 
-constexpr int BLEND_THREADS = PVG_TILE_PIXELS;
+constexpr int BLEND_THREADS = PVG_TILE_PIXELS / 2;   // two horizontally adjacent pixels per thread
 constexpr int BLEND_BATCH = 256;
 constexpr int BLEND_BATCH_FIRST = 64;
-constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH
+constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH_FIRST
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -21,9 +21,36 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
-// One CTA per 16x16 tile, one thread per pixel. The tile's slice of the sorted instance
-// list is consumed in batches: each thread gathers one 48 B record through the sorted
-// index list into shared memory, pre-digested so that the inner loop is straight-line:
+// Per-pixel compositing state and one front-to-back step. The cutoffs are predicates (selects),
+// not branches: alpha < 1/255 skips, T' = T - alpha T < 1e-4 stops the pixel WITHOUT compositing
+// the Gaussian that crosses the threshold (S10).
+struct BlendPixel {
+  float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;
+  bool alive = false;
+  // w: log2 of o~ G(x); L = log2 o~ (exact quadratic form <= 0, so w <= L: the S16' guard)
+  __device__ __forceinline__ bool step(float w, float L, float r, float g, float b, float z) {
+    w = fminf(w, L);
+    const float alpha = fminf(PVG_ALPHA_MAX, ex2_approx(w));
+    const bool acc = alive && alpha >= PVG_ALPHA_MIN;
+    const float wgt = alpha * T;
+    const float Tn = T - wgt;                      // T (1 - alpha)
+    const bool use = acc && Tn >= PVG_T_STOP;
+    alive = alive && (use || !acc);
+    if (use) {
+      Cr = fmaf(r, wgt, Cr);
+      Cg = fmaf(g, wgt, Cg);
+      Cb = fmaf(b, wgt, Cb);
+      D = fmaf(z, wgt, D);
+      T = Tn;
+    }
+    return use;
+  }
+};
+
+// One CTA per 16x16 tile, one thread per pair of horizontally adjacent pixels (they share dy and
+// with it 4 of the 10 operations of the exponent, and every shared-memory load). The tile's slice
+// of the sorted instance list is consumed in batches: each thread gathers 48 B records through the
+// sorted index list into shared memory, pre-digested so that the inner loop is straight-line:
 //   conic scaled by -log2(e)/2 and log2(o~) carried as the constant term, so that
 //   alpha = min(0.99, ex2(a' dx^2 + b' dx dy + c' dy^2 + log2 o~)) needs no multiply by o~.
 // The per-pixel decisions (1/255 cutoff, T stop) are predicates, not branches: 71% of the
@@ -45,13 +72,14 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   const uint32_t tid = threadIdx.x;
   const uint32_t tile = blockIdx.x;
   const uint32_t tx = tile % P.tiles_x, ty = tile / P.tiles_x;
-  const uint32_t px = tx * PVG_TILE + (tid & 15u), py = ty * PVG_TILE + (tid >> 4);
-  const bool inside = px < (uint32_t)P.width && py < (uint32_t)P.height;
-  const float pxf = (float)px + 0.5f, pyf = (float)py + 0.5f;   // S14
+  const uint32_t px = tx * PVG_TILE + 2u * (tid & 7u), py = ty * PVG_TILE + (tid >> 3);
+  const float px0 = (float)px + 0.5f, px1 = (float)px + 1.5f, pyf = (float)py + 0.5f;   // S14
   const uint2 range = ranges[tile];
 
-  float T = 1.0f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;
-  bool alive = inside;
+  BlendPixel A, B;
+  A.alive = px < (uint32_t)P.width && py < (uint32_t)P.height;
+  B.alive = px + 1u < (uint32_t)P.width && py < (uint32_t)P.height;
+  const bool in0 = A.alive, in1 = B.alive;
   uint32_t n_eval = 0, n_contrib = 0;
 
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
@@ -59,27 +87,28 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   uint32_t bs = BLEND_BATCH_FIRST;
   for (uint32_t base = range.x; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
-    if (__syncthreads_count(alive) == 0) break;
-    const uint32_t idx = base + tid;
-    if (tid >= bs) {
-    } else if (idx < range.y) {
-      const uint32_t g = __ldg(vals + idx);
-      const float4 r0 = __ldg(record + 3 * (size_t)g);
-      const float4 r1 = __ldg(record + 3 * (size_t)g + 1);
-      const float4 r2 = __ldg(record + 3 * (size_t)g + 2);
-      const float kh = -0.72134752044448170f;  // -log2(e)/2
-      s_geo[tid] = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
-      s_col[tid] = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
-      s_bz[tid] = make_float2(r2.z, r0.z);
-    } else {
-      // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0
-      s_geo[tid] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_col[tid] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
-      s_bz[tid] = make_float2(0.f, 0.f);
+    if (__syncthreads_count(A.alive || B.alive) == 0) break;
+    for (uint32_t k = tid; k < bs; k += BLEND_THREADS) {
+      const uint32_t idx = base + k;
+      if (idx < range.y) {
+        const uint32_t g = __ldg(vals + idx);
+        const float4 r0 = __ldg(record + 3 * (size_t)g);
+        const float4 r1 = __ldg(record + 3 * (size_t)g + 1);
+        const float4 r2 = __ldg(record + 3 * (size_t)g + 2);
+        const float kh = -0.72134752044448170f;  // -log2(e)/2
+        s_geo[k] = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
+        s_col[k] = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
+        s_bz[k] = make_float2(r2.z, r0.z);
+      } else {
+        // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0
+        s_geo[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        s_col[k] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
+        s_bz[k] = make_float2(0.f, 0.f);
+      }
     }
     __syncthreads();
     const uint32_t nb = min(bs, range.y - base);
-    if (__any_sync(0xffffffffu, alive)) {
+    if (__any_sync(0xffffffffu, A.alive || B.alive)) {
       for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
 #pragma unroll
         for (int u = 0; u < BLEND_UNROLL; ++u) {
@@ -87,28 +116,19 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
           const float4 ge = s_geo[j];
           const float4 co = s_col[j];
           const float2 bz = s_bz[j];
-          if (COUNT) n_eval += alive && j < nb;
-          const float dx = ge.x - pxf, dy = ge.y - pyf;
-          // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy); the quadratic form is <= 0 exactly (S16')
-          const float t1 = fmaf(ge.w, dy, ge.z * dx);
-          float w = fmaf(co.x * dy, dy, fmaf(t1, dx, co.y));
-          w = fminf(w, co.y);
-          const float alpha = fminf(PVG_ALPHA_MAX, ex2_approx(w));
-          const bool acc = alive && alpha >= PVG_ALPHA_MIN;
-          const float wgt = alpha * T;
-          const float Tn = T - wgt;                      // T (1 - alpha)
-          const bool use = acc && Tn >= PVG_T_STOP;      // S10: the one that would cross the stop is not composited
-          alive = alive && (use || !acc);
-          if (use) {
-            Cr = fmaf(co.z, wgt, Cr);
-            Cg = fmaf(co.w, wgt, Cg);
-            Cb = fmaf(bz.x, wgt, Cb);
-            D = fmaf(bz.y, wgt, D);
-            T = Tn;
-          }
-          if (COUNT) n_contrib += use;
+          if (COUNT) n_eval += (j < nb) ? (uint32_t)A.alive + (uint32_t)B.alive : 0u;
+          // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
+          const float dy = ge.y - pyf;
+          const float q = ge.w * dy;
+          const float rr = fmaf(co.x * dy, dy, co.y);
+          const float dx0 = ge.x - px0, dx1 = ge.x - px1;
+          const float w0 = fmaf(fmaf(ge.z, dx0, q), dx0, rr);
+          const float w1 = fmaf(fmaf(ge.z, dx1, q), dx1, rr);
+          const bool u0 = A.step(w0, co.y, co.z, co.w, bz.x, bz.y);
+          const bool u1 = B.step(w1, co.y, co.z, co.w, bz.x, bz.y);
+          if (COUNT) n_contrib += (uint32_t)u0 + (uint32_t)u1;
         }
-        if (!__any_sync(0xffffffffu, alive)) break;
+        if (!__any_sync(0xffffffffu, A.alive || B.alive)) break;
       }
     }
   }
@@ -117,17 +137,20 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
     atomicAdd(counters, (unsigned long long)n_eval);
     atomicAdd(counters + 1, (unsigned long long)n_contrib);
   }
-  if (inside) {
-    const size_t HW = (size_t)P.width * P.height;
-    const size_t pi = (size_t)py * P.width + px;
-    const float A = 1.0f - T;
+  const size_t HW = (size_t)P.width * P.height;
+  const size_t pi = (size_t)py * P.width + px;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const BlendPixel& X = k ? B : A;
+    if (!(k ? in1 : in0)) continue;
+    const float Al = 1.0f - X.T;
     if (out_rgb) {
-      out_rgb[pi] = fmaf(T, P.bg[0], Cr);
-      out_rgb[HW + pi] = fmaf(T, P.bg[1], Cg);
-      out_rgb[2 * HW + pi] = fmaf(T, P.bg[2], Cb);
+      out_rgb[pi + k] = fmaf(X.T, P.bg[0], X.Cr);
+      out_rgb[HW + pi + k] = fmaf(X.T, P.bg[1], X.Cg);
+      out_rgb[2 * HW + pi + k] = fmaf(X.T, P.bg[2], X.Cb);
     }
-    if (out_depth) out_depth[pi] = A > 0.f ? D / A : 0.f;
-    if (out_alpha) out_alpha[pi] = A;
+    if (out_depth) out_depth[pi + k] = Al > 0.f ? X.D / Al : 0.f;
+    if (out_alpha) out_alpha[pi + k] = Al;
   }
 }
 
