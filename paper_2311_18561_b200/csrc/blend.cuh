@@ -10,7 +10,11 @@
 
 namespace pvg {
 
-constexpr int BLEND_THREADS = PVG_TILE_PIXELS / 2;   // two horizontally adjacent pixels per thread
+#ifndef PVG_BLEND_NPX
+#define PVG_BLEND_NPX 4
+#endif
+constexpr int BLEND_NPX = PVG_BLEND_NPX;                   // horizontally adjacent pixels per thread (2 or 4)
+constexpr int BLEND_THREADS = PVG_TILE_PIXELS / BLEND_NPX;
 constexpr int BLEND_BATCH = 256;
 constexpr int BLEND_BATCH_FIRST = 64;
 constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH_FIRST
@@ -47,8 +51,8 @@ struct BlendPixel {
   }
 };
 
-// One CTA per 16x16 tile, one thread per pair of horizontally adjacent pixels (they share dy and
-// with it 4 of the 10 operations of the exponent, and every shared-memory load). The tile's slice
+// One CTA per 16x16 tile, one thread per BLEND_NPX horizontally adjacent pixels (they share dy and
+// with it 4 of the operations of the exponent, and every shared-memory load). The tile's slice
 // of the sorted instance list is consumed in batches: each thread gathers 48 B records through the
 // sorted index list into shared memory, pre-digested so that the inner loop is straight-line:
 //   conic scaled by -log2(e)/2 and log2(o~) carried as the constant term, so that
@@ -72,14 +76,21 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   const uint32_t tid = threadIdx.x;
   const uint32_t tile = blockIdx.x;
   const uint32_t tx = tile % P.tiles_x, ty = tile / P.tiles_x;
-  const uint32_t px = tx * PVG_TILE + 2u * (tid & 7u), py = ty * PVG_TILE + (tid >> 3);
-  const float px0 = (float)px + 0.5f, px1 = (float)px + 1.5f, pyf = (float)py + 0.5f;   // S14
+  constexpr uint32_t TPR = PVG_TILE / BLEND_NPX;   // threads per tile row
+  const uint32_t px = tx * PVG_TILE + BLEND_NPX * (tid % TPR), py = ty * PVG_TILE + tid / TPR;
+  const float pxf = (float)px + 0.5f, pyf = (float)py + 0.5f;   // S14
   const uint2 range = ranges[tile];
 
-  BlendPixel A, B;
-  A.alive = px < (uint32_t)P.width && py < (uint32_t)P.height;
-  B.alive = px + 1u < (uint32_t)P.width && py < (uint32_t)P.height;
-  const bool in0 = A.alive, in1 = B.alive;
+  BlendPixel X[BLEND_NPX];
+  bool in[BLEND_NPX];
+#pragma unroll
+  for (int k = 0; k < BLEND_NPX; ++k) X[k].alive = in[k] = px + k < (uint32_t)P.width && py < (uint32_t)P.height;
+  auto any_alive = [&]() {
+    bool a = false;
+#pragma unroll
+    for (int k = 0; k < BLEND_NPX; ++k) a = a || X[k].alive;
+    return a;
+  };
   uint32_t n_eval = 0, n_contrib = 0;
 
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
@@ -87,7 +98,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   uint32_t bs = BLEND_BATCH_FIRST;
   for (uint32_t base = range.x; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
-    if (__syncthreads_count(A.alive || B.alive) == 0) break;
+    if (__syncthreads_count(any_alive()) == 0) break;
     for (uint32_t k = tid; k < bs; k += BLEND_THREADS) {
       const uint32_t idx = base + k;
       if (idx < range.y) {
@@ -108,7 +119,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
     }
     __syncthreads();
     const uint32_t nb = min(bs, range.y - base);
-    if (__any_sync(0xffffffffu, A.alive || B.alive)) {
+    if (__any_sync(0xffffffffu, any_alive())) {
       for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
 #pragma unroll
         for (int u = 0; u < BLEND_UNROLL; ++u) {
@@ -116,19 +127,19 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
           const float4 ge = s_geo[j];
           const float4 co = s_col[j];
           const float2 bz = s_bz[j];
-          if (COUNT) n_eval += (j < nb) ? (uint32_t)A.alive + (uint32_t)B.alive : 0u;
           // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
           const float dy = ge.y - pyf;
           const float q = ge.w * dy;
           const float rr = fmaf(co.x * dy, dy, co.y);
-          const float dx0 = ge.x - px0, dx1 = ge.x - px1;
-          const float w0 = fmaf(fmaf(ge.z, dx0, q), dx0, rr);
-          const float w1 = fmaf(fmaf(ge.z, dx1, q), dx1, rr);
-          const bool u0 = A.step(w0, co.y, co.z, co.w, bz.x, bz.y);
-          const bool u1 = B.step(w1, co.y, co.z, co.w, bz.x, bz.y);
-          if (COUNT) n_contrib += (uint32_t)u0 + (uint32_t)u1;
+#pragma unroll
+          for (int k = 0; k < BLEND_NPX; ++k) {
+            if (COUNT) n_eval += (j < nb && X[k].alive) ? 1u : 0u;
+            const float dx = ge.x - (pxf + (float)k);
+            const bool used = X[k].step(fmaf(fmaf(ge.z, dx, q), dx, rr), co.y, co.z, co.w, bz.x, bz.y);
+            if (COUNT) n_contrib += used ? 1u : 0u;
+          }
         }
-        if (!__any_sync(0xffffffffu, A.alive || B.alive)) break;
+        if (!__any_sync(0xffffffffu, any_alive())) break;
       }
     }
   }
@@ -140,16 +151,15 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   const size_t HW = (size_t)P.width * P.height;
   const size_t pi = (size_t)py * P.width + px;
 #pragma unroll
-  for (int k = 0; k < 2; ++k) {
-    const BlendPixel& X = k ? B : A;
-    if (!(k ? in1 : in0)) continue;
-    const float Al = 1.0f - X.T;
+  for (int k = 0; k < BLEND_NPX; ++k) {
+    if (!in[k]) continue;
+    const float Al = 1.0f - X[k].T;
     if (out_rgb) {
-      out_rgb[pi + k] = fmaf(X.T, P.bg[0], X.Cr);
-      out_rgb[HW + pi + k] = fmaf(X.T, P.bg[1], X.Cg);
-      out_rgb[2 * HW + pi + k] = fmaf(X.T, P.bg[2], X.Cb);
+      out_rgb[pi + k] = fmaf(X[k].T, P.bg[0], X[k].Cr);
+      out_rgb[HW + pi + k] = fmaf(X[k].T, P.bg[1], X[k].Cg);
+      out_rgb[2 * HW + pi + k] = fmaf(X[k].T, P.bg[2], X[k].Cb);
     }
-    if (out_depth) out_depth[pi + k] = Al > 0.f ? X.D / Al : 0.f;
+    if (out_depth) out_depth[pi + k] = Al > 0.f ? X[k].D / Al : 0.f;
     if (out_alpha) out_alpha[pi + k] = Al;
   }
 }
