@@ -66,22 +66,20 @@ __device__ __forceinline__ void bb_entry(uint32_t xy0, uint32_t xy1, uint32_t j,
 // (same scheme as expand.cuh). keys/visit: the depth-sorted (rect | depth, Gaussian) pairs;
 // boffsets: exclusive scan of the blocks touched, in that order.
 __global__ void __launch_bounds__(BE_THREADS)
-bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint64_t* __restrict__ keys,
-                  const uint32_t* __restrict__ visit, uint32_t blocks_x, uint8_t* __restrict__ e_bin,
+bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
+                  const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x, uint8_t* __restrict__ e_bin,
                   uint32_t* __restrict__ e_g, uint64_t* __restrict__ e_mask) {
   __shared__ BinExpandSmem s;
   const uint32_t tid = threadIdx.x;
   const uint32_t i0 = blockIdx.x * BE_CHUNK;
   const uint32_t i1 = min(i0 + (uint32_t)BE_CHUNK, Mb);
-  if (tid == 0 || tid == 32) {
-    // last r in [0, n) with boffsets[r] <= target (boffsets[0] == 0)
-    const uint32_t target = tid == 0 ? i0 : i1 - 1u;
-    uint32_t lo = 0, hi = n;
-    while (hi - lo > 1) {
-      const uint32_t mid = lo + ((hi - lo) >> 1);
-      if (boffsets[mid] <= target) lo = mid; else hi = mid;
-    }
-    if (tid == 0) s.lo = lo; else s.hi = lo;
+  if (tid == 0) {
+    // owners of the chunk: from the one that contains its first entry (written by the scan) to the one that
+    // contains the next chunk's first entry; the last chunk stages up to the span limit (owners that start
+    // beyond the chunk leave no mark)
+    const uint32_t lo = chunk_owner[blockIdx.x];
+    s.lo = lo;
+    s.hi = (uint64_t)(blockIdx.x + 1) * BE_CHUNK < Mb ? chunk_owner[blockIdx.x + 1] : min(lo + (uint32_t)BE_SPAN, n) - 1u;
   }
   reinterpret_cast<uint4*>(s.own)[tid] = make_uint4(0u, 0u, 0u, 0u);   // 8 u16 per thread
   __syncthreads();

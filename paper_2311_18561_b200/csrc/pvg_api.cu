@@ -305,7 +305,7 @@ struct pvg_scene {
   Buf keys[2], vals[2], keys_unsorted, vals_unsorted;
   Buf tiles16[2], tiles16_unsorted;
   // block-entry workspace (blockbin.cuh)
-  Buf boffsets, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
+  Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
   Buf ranges, tilegrid;
   Buf img;  // render_host device images
   SortScratch sort_n, sort_m;
@@ -334,7 +334,7 @@ void release_all(pvg_scene* s) {
   Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
-                 &s->boffsets, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
+                 &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
                  &s->ranges, &s->tilegrid, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
@@ -442,12 +442,14 @@ int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Ti
   uint32_t* ticket = s->small.as<uint32_t>();
   uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
   if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
+  if (blocks) TRY(s->chunk_owner.reserve(((size_t)s->Mb / BE_CHUNK + 2) * 4, st, 1.125));
   if (blocks)
     scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(),
-                                                                  visit, out, total, s->scan_status.as<uint64_t>(), ticket);
+                                                                  visit, out, total, s->scan_status.as<uint64_t>(), ticket,
+                                                                  s->chunk_owner.as<uint32_t>(), (uint32_t)BE_CHUNK);
   else
     scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), nullptr, visit, out, total,
-                                                                   s->scan_status.as<uint64_t>(), ticket);
+                                                                   s->scan_status.as<uint64_t>(), ticket, nullptr, 0u);
   if (tm) TRY(tm->end(st));
   return PVG_OK;
 }
@@ -494,7 +496,8 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
-      n, Mb, s->boffsets.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x, s->e_bin.as<uint8_t>(),
+      n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x,
+      s->e_bin.as<uint8_t>(),
       s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>());
   TRY(tm->end(st));
 
