@@ -7,7 +7,7 @@
 
 namespace pvg {
 
-constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_THREADS = 512;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 
@@ -76,25 +76,35 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
     block_sum += v;
   }
 
-  if (threadIdx.x == 0) {
+  if (warp == 0) {
+    // warp-wide look-back: lane l inspects predecessor tile - 1 - l; the walk ends at the nearest tile
+    // that has published its inclusive prefix (tile -1 counts as a prefix of 0)
     uint64_t excl = 0;
     if (tile == 0) {
-      st_relaxed_u64(status, LB_FLAG_PREFIX | block_sum);
+      if (lane == 0) st_relaxed_u64(status, LB_FLAG_PREFIX | block_sum);
     } else {
-      st_relaxed_u64(status + tile, LB_FLAG_AGG | block_sum);
-      int64_t p = (int64_t)tile - 1;
+      if (lane == 0) st_relaxed_u64(status + tile, LB_FLAG_AGG | block_sum);
+      int64_t p = (int64_t)tile - 1 - (int64_t)lane;
       while (true) {
-        const uint64_t s = ld_relaxed_u64(status + p);
-        const uint64_t flag = s & LB_FLAG_MASK;
-        if (flag == 0) continue;  // predecessor has a ticket, so it is running: spin
-        excl += s & LB_VALUE_MASK;
-        if (flag == LB_FLAG_PREFIX) break;
-        --p;
+        const uint64_t sv = p >= 0 ? ld_relaxed_u64(status + p) : LB_FLAG_PREFIX;
+        const uint64_t flag = sv & LB_FLAG_MASK;
+        const uint32_t ready = __ballot_sync(0xffffffffu, flag != 0);
+        const uint32_t pref = __ballot_sync(0xffffffffu, flag == LB_FLAG_PREFIX);
+        const uint32_t upto = pref ? (0xffffffffu >> (31 - (__ffs(pref) - 1))) : 0xffffffffu;   // lanes 0..first prefix
+        if ((ready & upto) != upto) continue;   // a tile in the window holds an earlier ticket: it is running
+        uint64_t v = ((upto >> lane) & 1u) ? (sv & LB_VALUE_MASK) : 0ull;
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+        excl += v;
+        if (pref) break;
+        p -= 32;
       }
-      st_relaxed_u64(status + tile, LB_FLAG_PREFIX | (excl + block_sum));
+      if (lane == 0) st_relaxed_u64(status + tile, LB_FLAG_PREFIX | (excl + block_sum));
     }
-    s_prefix = excl;
-    if ((uint64_t)(tile + 1) * SCAN_TILE >= n) *total = excl + block_sum;
+    if (lane == 0) {
+      s_prefix = excl;
+      if ((uint64_t)(tile + 1) * SCAN_TILE >= n) *total = excl + block_sum;
+    }
   }
   __syncthreads();
   uint64_t run = s_prefix + warp_excl + (incl - tsum);
