@@ -95,7 +95,12 @@ struct KernelRec {
 #define PVG_OSL_MINB 2
 #endif
 struct OsLarge { static constexpr int THREADS = PVG_OSL_THREADS, ITEMS = PVG_OSL_ITEMS, MINB = PVG_OSL_MINB; static constexpr bool STREAM = true; };
-struct OsSmall { static constexpr int THREADS = 256, ITEMS = 8, MINB = 4; static constexpr bool STREAM = false; };
+#ifndef PVG_OSS_THREADS
+#define PVG_OSS_THREADS 384
+#define PVG_OSS_ITEMS 8
+#define PVG_OSS_MINB 2
+#endif
+struct OsSmall { static constexpr int THREADS = PVG_OSS_THREADS, ITEMS = PVG_OSS_ITEMS, MINB = PVG_OSS_MINB; static constexpr bool STREAM = false; };
 constexpr uint64_t OS_SMALL_BELOW = 8u << 20;
 
 // scratch of one sort call
@@ -198,7 +203,8 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   const unsigned hist_grid = (unsigned)std::min<uint64_t>(hist_chunks, (uint64_t)sms * 4);
   if (!hist_ready) {
     if (tm) TRY(tm->begin("onesweep_histogram", stage, st));
-    onesweep_histogram_kernel<<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
+    if (small) onesweep_histogram_kernel<false><<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
+    else onesweep_histogram_kernel<true><<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
     if (tm) TRY(tm->end(st));
     if (tm) TRY(tm->begin("onesweep_scan_hist", stage, st));
     onesweep_scan_hist_kernel<<<plan.num_passes, OS_RADIX, 0, st>>>(sc.hist.as<uint32_t>());
