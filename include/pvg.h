@@ -96,6 +96,16 @@ int pvg_render(pvg_scene *scene, const pvg_camera *cam, float t, float *out_rgb,
 int pvg_render_host(pvg_scene *scene, const pvg_camera *cam, float t, float *host_rgb,
                     float *host_depth, float *host_alpha);
 
+/* Pipelined variant for frame streams: enqueues the render and the device-to-host copies (on an
+ * internal copy stream, from one of two library-owned device images) and returns without waiting,
+ * so the copy of frame k overlaps the render of frame k + 1. The host buffers should be pinned
+ * (pageable memory makes the copies synchronous) and must not be read before pvg_wait_host, which
+ * blocks until every pending copy of the scene has landed. At most two frames are in flight: the
+ * third call reuses the first one's device image after its copy has left. */
+int pvg_render_host_async(pvg_scene *scene, const pvg_camera *cam, float t, float *host_rgb,
+                          float *host_depth, float *host_alpha);
+int pvg_wait_host(pvg_scene *scene);
+
 int pvg_destroy(pvg_scene *scene);
 
 /* ---- options ------------------------------------------------------------------------------ */

@@ -25,6 +25,7 @@ NUM_STAGES = len(STAGES)
 
 # every symbol include/pvg.h declares
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
+           "pvg_render_host_async", "pvg_wait_host",
            "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms",
            "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
@@ -79,6 +80,8 @@ def load_library(path: Optional[str] = None):
     L.pvg_create_scene.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.pvg_render.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_render_host.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_render_host_async.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_wait_host.argtypes = [C.c_void_p]
     L.pvg_destroy.argtypes = [C.c_void_p]
     L.pvg_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
     L.pvg_debug_view.argtypes = [C.c_void_p, C.POINTER(DebugC)]
@@ -216,6 +219,18 @@ class Scene:
         _check(self._L.pvg_render_host(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
                                        out[2].data_ptr()))
         return out
+
+    def render_host_async(self, cam, t: float, out: Tuple):
+        """Pipelined render into pinned HOST tensors; read them only after wait_host()."""
+        import torch
+        c = cam if isinstance(cam, CameraC) else camera_struct(cam)
+        _check(self._L.pvg_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
+        _check(self._L.pvg_render_host_async(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
+                                             out[2].data_ptr()))
+        return out
+
+    def wait_host(self) -> None:
+        _check(self._L.pvg_wait_host(self._h))
 
     # -- options / hooks ----------------------------------------------------------------------
     def set_option(self, option: int, value: int) -> None:

@@ -313,7 +313,11 @@ struct pvg_scene {
   // block-entry workspace (blockbin.cuh)
   Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
   Buf ranges, tilegrid;
-  Buf img;  // render_host device images
+  Buf img[2];  // render_host device images (double-buffered: the copy of frame k overlaps frame k + 1)
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_rendered = nullptr, ev_copied[2] = {nullptr, nullptr};
+  bool copy_pending[2] = {false, false};
+  int img_next = 0;
   SortScratch sort_n, sort_m;
   uint64_t* h_total = nullptr;  // pinned
   cudaStream_t side = nullptr;  // tile grid + prefix run here, beside the depth sort
@@ -341,7 +345,7 @@ void release_all(pvg_scene* s) {
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
-                 &s->ranges, &s->tilegrid, &s->img, &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->ranges, &s->tilegrid, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
@@ -349,6 +353,10 @@ void release_all(pvg_scene* s) {
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->side) cudaStreamDestroy(s->side);
+  if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+  if (s->ev_rendered) cudaEventDestroy(s->ev_rendered);
+  for (int k = 0; k < 2; ++k) if (s->ev_copied[k]) cudaEventDestroy(s->ev_copied[k]);
+  s->copy_stream = nullptr; s->ev_rendered = nullptr; s->ev_copied[0] = s->ev_copied[1] = nullptr;
   s->ev_fork = s->ev_join = nullptr;
   s->side = nullptr;
   s->timer.destroy();
@@ -404,6 +412,9 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+  CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+  CU(cudaEventCreateWithFlags(&s->ev_rendered, cudaEventDisableTiming));
+  for (int k = 0; k < 2; ++k) CU(cudaEventCreateWithFlags(&s->ev_copied[k], cudaEventDisableTiming));
   return PVG_OK;
 }
 
@@ -762,6 +773,7 @@ int pvg_create_scene(const pvg_scene_desc* d, pvg_scene** out) {
 int pvg_destroy(pvg_scene* scene) {
   if (!scene) return PVG_ERR_NULL;
   cudaStreamSynchronize(scene->stream);
+  if (scene->copy_stream) cudaStreamSynchronize(scene->copy_stream);
   release_all(scene);
   delete scene;
   return PVG_OK;
@@ -790,24 +802,52 @@ int pvg_render(pvg_scene* scene, const pvg_camera* cam, float t, float* out_rgb,
   return render_impl(scene, cam, t, out_rgb, out_depth, out_alpha);
 }
 
-int pvg_render_host(pvg_scene* scene, const pvg_camera* cam, float t, float* host_rgb, float* host_depth,
-                    float* host_alpha) {
+int pvg_wait_host(pvg_scene* scene) {
+  if (!scene) return PVG_ERR_NULL;
+  for (int k = 0; k < 2; ++k)
+    if (scene->copy_pending[k]) {
+      CU(cudaEventSynchronize(scene->ev_copied[k]));
+      scene->copy_pending[k] = false;
+    }
+  return PVG_OK;
+}
+
+int pvg_render_host_async(pvg_scene* scene, const pvg_camera* cam, float t, float* host_rgb, float* host_depth,
+                          float* host_alpha) {
   if (!scene || !cam) return PVG_ERR_NULL;
   if (!std::isfinite(t)) return PVG_ERR_BAD_CAMERA;
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
   const size_t HW = (size_t)cam->width * cam->height;
   cudaStream_t st = scene->stream;
-  TRY(scene->img.reserve(HW * 5 * 4, st));
-  float* d_rgb = scene->img.as<float>();
+  const int slot = scene->img_next;
+  scene->img_next ^= 1;
+  // the frame rendered two calls ago used this device image: its copy must have left before the blend rewrites it
+  if (scene->copy_pending[slot]) CU(cudaStreamWaitEvent(st, scene->ev_copied[slot], 0));
+  if (HW * 5 * 4 > scene->img[slot].cap && scene->copy_pending[slot]) {   // growing frees the old buffer
+    CU(cudaEventSynchronize(scene->ev_copied[slot]));
+    scene->copy_pending[slot] = false;
+  }
+  TRY(scene->img[slot].reserve(HW * 5 * 4, st));
+  float* d_rgb = scene->img[slot].as<float>();
   float* d_depth = d_rgb + 3 * HW;
   float* d_alpha = d_rgb + 4 * HW;
   TRY(render_impl(scene, cam, t, host_rgb ? d_rgb : nullptr, host_depth ? d_depth : nullptr,
                   host_alpha ? d_alpha : nullptr));
-  if (host_rgb) CU(cudaMemcpyAsync(host_rgb, d_rgb, HW * 12, cudaMemcpyDeviceToHost, st));
-  if (host_depth) CU(cudaMemcpyAsync(host_depth, d_depth, HW * 4, cudaMemcpyDeviceToHost, st));
-  if (host_alpha) CU(cudaMemcpyAsync(host_alpha, d_alpha, HW * 4, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));
+  CU(cudaEventRecord(scene->ev_rendered, st));
+  cudaStream_t cs = scene->copy_stream;
+  CU(cudaStreamWaitEvent(cs, scene->ev_rendered, 0));
+  if (host_rgb) CU(cudaMemcpyAsync(host_rgb, d_rgb, HW * 12, cudaMemcpyDeviceToHost, cs));
+  if (host_depth) CU(cudaMemcpyAsync(host_depth, d_depth, HW * 4, cudaMemcpyDeviceToHost, cs));
+  if (host_alpha) CU(cudaMemcpyAsync(host_alpha, d_alpha, HW * 4, cudaMemcpyDeviceToHost, cs));
+  CU(cudaEventRecord(scene->ev_copied[slot], cs));
+  scene->copy_pending[slot] = true;
   return PVG_OK;
+}
+
+int pvg_render_host(pvg_scene* scene, const pvg_camera* cam, float t, float* host_rgb, float* host_depth,
+                    float* host_alpha) {
+  TRY(pvg_render_host_async(scene, cam, t, host_rgb, host_depth, host_alpha));
+  return pvg_wait_host(scene);
 }
 
 int pvg_debug_view(pvg_scene* s, pvg_debug* out) {

@@ -203,6 +203,25 @@ def test_render_host_matches_render():
     g.close()
 
 
+def test_render_host_async_pipeline():
+    """Four frames in flight through the two-deep pipeline; each equals the synchronous render."""
+    import torch
+    wl = make_config(1, n=40_000)
+    cam = wl.cameras[0]
+    g = pvg.Scene.from_workload_scene(wl.scene)
+    ts = [0.1, 0.35, 0.6, 0.85]
+    bufs = [tuple(torch.zeros(shape, pin_memory=True) for shape in ((3, cam.height, cam.width), (cam.height, cam.width), (cam.height, cam.width)))
+            for _ in ts]
+    for t, b in zip(ts, bufs):
+        g.render_host_async(cam, t, b)
+    g.wait_host()
+    for t, b in zip(ts, bufs):
+        ref = [x.cpu() for x in g.render(cam, t)]
+        for a, r in zip(b, ref):
+            assert torch.equal(a, r)
+    g.close()
+
+
 def test_repeatable_and_stream():
     """Same frame twice on a non-default torch stream: bit-identical (no atomics in the data path)."""
     import torch
