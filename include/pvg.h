@@ -32,7 +32,8 @@ typedef enum pvg_status {
   PVG_ERR_OOM = -4,               /* device allocation failed */
   PVG_ERR_INSTANCE_OVERFLOW = -5, /* tile instances M >= 2^32 */
   PVG_ERR_CUDA = -6,              /* CUDA runtime error (or no device); see pvg_last_cuda_error */
-  PVG_ERR_BAD_OPTION = -7
+  PVG_ERR_BAD_OPTION = -7,
+  PVG_ERR_BAD_STATE = -8          /* non-finite t or dt, rho_min < 0, rho_max < rho_min */
 } pvg_status;
 
 typedef struct pvg_scene pvg_scene; /* opaque; owns device copies of the model and a growable workspace */
@@ -90,6 +91,20 @@ int pvg_create_scene(const pvg_scene_desc *desc, pvg_scene **out);
  * the blend kernel still in flight. */
 int pvg_render(pvg_scene *scene, const pvg_camera *cam, float t, float *out_rgb, float *out_depth,
                float *out_alpha);
+
+/* Which state of the model is rendered:
+ *   dt == 0: H(t) = { mu~(t), q, s, o~(t), c } (Eq. 5-7) -- what pvg_render draws.
+ *   dt != 0: the temporal-smoothing estimate of the state at t from the state at t1 = t - dt,
+ *            H^(t) = { mu~(t1) + vbar dt, q, s, o~(t1), c } (Eq. 12), with the average velocity
+ *            vbar = v exp(-rho / 2) (Eq. 10) and the staticness rho = beta / l (L112).
+ *   rho_min, rho_max: only points with rho_min <= rho <= rho_max are drawn; {0, +INF} draws all. The paper
+ *            removes rho < 1 to keep the static part of a scene (L192) and thresholds rho to tell dynamic
+ *            points (L118). beta = +INF counts as rho = +INF; cycle = +INF with finite beta as rho = 0. */
+typedef struct pvg_state {
+  float t, dt, rho_min, rho_max;
+} pvg_state;
+int pvg_render_state(pvg_scene *scene, const pvg_camera *cam, const pvg_state *state, float *out_rgb,
+                     float *out_depth, float *out_alpha);
 
 /* Same frame into HOST buffers (pinned or pageable): renders into library-owned device images,
  * copies them back and synchronises the stream before returning. */

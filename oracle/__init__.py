@@ -17,7 +17,7 @@ from . import build as _build
 SLOTS = dict(mu=slice(0, 3), op=3, pcam=slice(4, 7), sigma=slice(7, 13), cov=slice(13, 16),
              conic=slice(16, 19), mean=slice(19, 21), ext=slice(21, 23), rgb=slice(23, 26),
              cull=26, rect=slice(27, 31), count=31)
-CULL_REASONS = {0: "valid", 1: "opacity", 2: "near", 3: "det", 4: "rect", 5: "nonfinite"}
+CULL_REASONS = {0: "valid", 1: "opacity", 2: "near", 3: "det", 4: "rect", 5: "nonfinite", 6: "staticness"}
 
 
 class _Cam(C.Structure):
@@ -72,8 +72,10 @@ def set_threads(n: int) -> None:
     lib().oracle_set_threads(C.c_int(int(n)))
 
 
-def preprocess(mu, quat, scale, opacity, sh, tau, beta, vel, cycle, sh_degree, cam, t):
-    """Oracle-P. Returns (wide [n,32] float64, rec32 [n,12] float32)."""
+def preprocess(mu, quat, scale, opacity, sh, tau, beta, vel, cycle, sh_degree, cam, t, dt=0.0, rho_min=0.0,
+               rho_max=float("inf")):
+    """Oracle-P. Returns (wide [n,32] float64, rec32 [n,12] float32).
+    dt != 0: the temporal-smoothing state H^(t) built from t - dt (Eq. 12); rho_min / rho_max: staticness filter."""
     n = int(np.asarray(mu).shape[0])
     mu = _f32(mu, (n, 3)); quat = _f32(quat, (n, 4)); scale = _f32(scale, (n, 3))
     opacity = _f32(opacity, (n,)); sh = _f32(sh, (n, 16, 3)); tau = _f32(tau, (n,))
@@ -81,16 +83,17 @@ def preprocess(mu, quat, scale, opacity, sh, tau, beta, vel, cycle, sh_degree, c
     wide = np.empty((n, 32), dtype=np.float64)
     rec = np.empty((n, 12), dtype=np.float32)
     c = _cam(cam)
-    lib().oracle_preprocess(C.c_uint64(n), _p(mu), _p(quat), _p(scale), _p(opacity), _p(sh), _p(tau),
-                            _p(beta), _p(vel), C.c_double(float(cycle)), C.c_int(int(sh_degree)),
-                            C.byref(c), C.c_double(float(t)), _p(wide), _p(rec))
+    lib().oracle_preprocess_state(C.c_uint64(n), _p(mu), _p(quat), _p(scale), _p(opacity), _p(sh), _p(tau),
+                                  _p(beta), _p(vel), C.c_double(float(cycle)), C.c_int(int(sh_degree)),
+                                  C.byref(c), C.c_double(float(t)), C.c_double(float(dt)), C.c_double(float(rho_min)),
+                                  C.c_double(float(rho_max)), _p(wide), _p(rec))
     return wide, rec
 
 
-def preprocess_scene(scene, cam, t):
+def preprocess_scene(scene, cam, t, dt=0.0, rho_min=0.0, rho_max=float("inf")):
     """Oracle-P on an object with the workloads.Scene attribute names."""
     return preprocess(scene.mu, scene.quat, scene.scale, scene.opacity, scene.sh, scene.tau,
-                      scene.beta, scene.vel, scene.cycle, scene.sh_degree, cam, t)
+                      scene.beta, scene.vel, scene.cycle, scene.sh_degree, cam, t, dt, rho_min, rho_max)
 
 
 def sh_basis(d: Sequence[float]) -> np.ndarray:

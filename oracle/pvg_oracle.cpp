@@ -17,7 +17,8 @@
 //
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed forms T1..T8 of the
 // paper, single-Gaussian image, stop/clamp/cutoff rules, brute force == binned,
-// std::stable_sort equivalence on tiny scenes. "Absolute values on real data"
+// std::stable_sort equivalence on tiny scenes; for oracle_preprocess_state (Eq. 10 / 12,
+// staticness filter) TestTemporalSmoothingState. "Absolute values on real data"
 // is parity unpinned (the paper prints no worked numeric example).
 
 #include <algorithm>
@@ -203,10 +204,32 @@ int oracle_record_stride() { return S_STRIDE; }
 // Eq. 2, H(t) PAPER.md:L101/L120).
 //   wide  [n][32] double : every intermediate (enum Slot)
 //   rec32 [n][12] float  : (mx,my,z,op | a,b,c,hx | r,g,b,hy), zeros if culled
+//
+// oracle_preprocess_state adds the two variants of SURVEY.md 8(f-1):
+//   dts != 0: the temporal-smoothing state H^(t2 = t) = { mu~(t1) + vbar dts, q, s, o~(t1), c } with
+//             t1 = t - dts (Eq. 12) and vbar = v exp(-rho/2), rho = beta / l (Eq. 10; L112);
+//   staticness filter: only points with rho_min <= rho <= rho_max are kept ("we remove the PVG points
+//             whose rho < 1 to preserve the static part"; threshold on rho, L118).
+//             beta = +INF is rho = +INF (3DGS, L114); l = +INF with finite beta is rho = 0.
+void oracle_preprocess_state(uint64_t n, const float* mu, const float* quat, const float* scale,
+                             const float* opacity, const float* sh, const float* tau,
+                             const float* beta, const float* vel, double cycle, int sh_degree,
+                             const Cam* cam, double t, double dts, double rho_min, double rho_max,
+                             double* wide, float* rec32);
+
 void oracle_preprocess(uint64_t n, const float* mu, const float* quat, const float* scale,
                        const float* opacity, const float* sh, const float* tau,
                        const float* beta, const float* vel, double cycle, int sh_degree,
                        const Cam* cam, double t, double* wide, float* rec32) {
+  oracle_preprocess_state(n, mu, quat, scale, opacity, sh, tau, beta, vel, cycle, sh_degree, cam, t, 0.0, 0.0,
+                          std::numeric_limits<double>::infinity(), wide, rec32);
+}
+
+void oracle_preprocess_state(uint64_t n, const float* mu, const float* quat, const float* scale,
+                             const float* opacity, const float* sh, const float* tau,
+                             const float* beta, const float* vel, double cycle, int sh_degree,
+                             const Cam* cam, double t, double dts, double rho_min, double rho_max,
+                             double* wide, float* rec32) {
   const double* R = cam->w2c;
   const int TX = (cam->width + kTile - 1) / kTile, TY = (cam->height + kTile - 1) / kTile;
   const double znear = cam->znear > 0.0 ? cam->znear : 0.2;  // S5
@@ -228,12 +251,21 @@ void oracle_preprocess(uint64_t n, const float* mu, const float* quat, const flo
     w[S_RECT + 2] = w[S_RECT + 3] = -1.0;
 
     // P1: Eq. 6; l = +INF is the linear model
-    const double dt = t - (double)tau[i];
+    // (Eq. 12: the state is evaluated at t1 = t - dts; dts = 0 is H(t) itself)
+    const double dt = (t - dts) - (double)tau[i];
     const double m = std::isinf(cycle) ? dt : (cycle / (2.0 * kPi)) * std::sin(2.0 * kPi * dt / cycle);
     double mt[3];
     for (int j = 0; j < 3; ++j) mt[j] = (double)mu[i * 3 + j] + m * (double)vel[i * 3 + j];
     // P2: Eq. 7; beta = +INF => o~ = o
     const double be = beta[i];
+    // staticness rho = beta / l
+    const double rho = std::isinf(be) ? std::numeric_limits<double>::infinity() : (std::isinf(cycle) ? 0.0 : be / cycle);
+    if (dts != 0.0) {
+      // Eq. 10: vbar = v exp(-rho / 2); Eq. 12 (L162): flow translation vbar * dts
+      const double e = std::exp(-0.5 * rho);
+      for (int j = 0; j < 3; ++j) mt[j] += (double)vel[i * 3 + j] * e * dts;
+    }
+    if (!(rho >= rho_min) || rho > rho_max) { w[S_CULL] = 6; continue; }
     const double ot = std::isinf(be) ? (double)opacity[i]
                                      : (double)opacity[i] * std::exp(-0.5 * dt * dt / (be * be));
     for (int j = 0; j < 3; ++j) w[S_MU + j] = mt[j];

@@ -18,14 +18,14 @@ LIB_PATH = os.environ.get("PVG_LIB") or os.path.join(_HERE, "libpvg.so")   # PVG
 
 PVG_OK = 0
 STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_BAD_CAMERA",
-          -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION"}
+          -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION", -8: "PVG_ERR_BAD_STATE"}
 OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 
 # every symbol include/pvg.h declares
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
-           "pvg_render_host_async", "pvg_wait_host",
+           "pvg_render_host_async", "pvg_wait_host", "pvg_render_state",
            "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms",
            "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
@@ -47,6 +47,10 @@ class CameraC(C.Structure):
     _fields_ = [("width", C.c_int), ("height", C.c_int), ("fx", C.c_float), ("fy", C.c_float),
                 ("cx", C.c_float), ("cy", C.c_float), ("world_to_cam", C.c_float * 12),
                 ("znear", C.c_float), ("bg", C.c_float * 3)]
+
+
+class StateC(C.Structure):
+    _fields_ = [("t", C.c_float), ("dt", C.c_float), ("rho_min", C.c_float), ("rho_max", C.c_float)]
 
 
 class DebugC(C.Structure):
@@ -79,6 +83,7 @@ def load_library(path: Optional[str] = None):
     L.pvg_set_stream.argtypes = [C.c_void_p, C.c_void_p]
     L.pvg_create_scene.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.pvg_render.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_render_state.argtypes = [C.c_void_p, C.POINTER(CameraC), C.POINTER(StateC), C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_render_host.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_render_host_async.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_wait_host.argtypes = [C.c_void_p]
@@ -194,8 +199,11 @@ class Scene:
         return cls(sc.mu, sc.quat, sc.scale, sc.opacity, sc.sh, sc.tau, sc.beta, sc.vel, sc.cycle, sc.sh_degree, **kw)
 
     # -- the path ---------------------------------------------------------------------------
-    def render(self, cam, t: float, out: Optional[Tuple] = None):
-        """Frame at time t into torch CUDA tensors (rgb [3,H,W], depth [H,W], alpha [H,W])."""
+    def render(self, cam, t: float, out: Optional[Tuple] = None, dt: float = 0.0, rho_min: float = 0.0,
+               rho_max: float = float("inf")):
+        """Frame at time t into torch CUDA tensors (rgb [3,H,W], depth [H,W], alpha [H,W]).
+        dt != 0 renders the temporal-smoothing state H^(t) built from t - dt (Eq. 12); rho_min / rho_max
+        keep only the points whose staticness beta / l lies in [rho_min, rho_max]."""
         import torch
         c = cam if isinstance(cam, CameraC) else camera_struct(cam)
         if out is None:
@@ -203,8 +211,13 @@ class Scene:
                    torch.empty((c.height, c.width), dtype=torch.float32, device="cuda"),
                    torch.empty((c.height, c.width), dtype=torch.float32, device="cuda"))
         _check(self._L.pvg_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
-        _check(self._L.pvg_render(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
-                                  out[2].data_ptr()))
+        if dt == 0.0 and rho_min == 0.0 and rho_max == float("inf"):
+            _check(self._L.pvg_render(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
+                                      out[2].data_ptr()))
+        else:
+            st = StateC(float(t), float(dt), float(rho_min), float(rho_max))
+            _check(self._L.pvg_render_state(self._h, C.byref(c), C.byref(st), out[0].data_ptr(), out[1].data_ptr(),
+                                            out[2].data_ptr()))
         return out
 
     def render_host(self, cam, t: float, out: Optional[Tuple] = None):

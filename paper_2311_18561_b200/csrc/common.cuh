@@ -25,7 +25,11 @@ struct FrameParams {
   float fx, fy, cx, cy;
   float limx, limy;  // 1.3 * half-FoV tangents (Jacobian guard)
   float znear;
-  float t;
+  float t;            // time at which Eq. 6 / Eq. 7 are evaluated (t - dts for the temporal-smoothing state)
+  float dts;          // Eq. 12 flow translation interval (0: the plain state H(t))
+  float inv_l;        // 1 / l (0 for the linear model): rho = beta / l
+  float rho_min, rho_max;  // staticness filter (only when `filter` is set)
+  int filter;
   float two_over_l;   // 2 / l           (sinpi argument scale)
   float l_over_2pi;   // l / (2 pi)
   int linear;         // l == +INF: mu~ = mu + (t - tau) v

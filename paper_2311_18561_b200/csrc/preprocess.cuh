@@ -3,7 +3,8 @@
 // One thread per Gaussian. HBM-bound: 4 coalesced 128-bit loads of the SoA model
 // (64 B), 3..12 more for the SH planes of survivors only (<= 192 B), one 48 B record
 // + 16 B tile info + 4 B count out. Steps P1..P12 of DESIGN.md:
-//   Eq. 6 mu~(t), Eq. 7 (L105) o~(t), culls, Sigma from (q, s) (L79),
+//   Eq. 6 mu~(t), Eq. 7 (L105) o~(t) -- or the temporal-smoothing state of Eq. 12 (L162) and
+//   the staticness filter on rho = beta / l (L118, L192) --, culls, Sigma from (q, s) (L79),
 //   Eq. 2 (L68) EWA projection with 0.3 px^2 dilation, conic, exact-cutoff extents,
 //   tile rectangle, degree-3 SH colour viewed from mu~(t).
 #pragma once
@@ -55,11 +56,18 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
   // P1: Eq. 6. sinpi gives an exact range reduction of 2 pi (t - tau) / l.
   const float dt = P.t - a0.w;
   const float m = P.linear ? dt : P.l_over_2pi * sinpif(P.two_over_l * dt);
-  const float wx = fmaf(m, a1.x, a0.x), wy = fmaf(m, a1.y, a0.y), wz = fmaf(m, a1.z, a0.z);
+  // staticness rho = beta / l; beta = +INF is rho = +INF whatever l
+  const float rho = a1.w > 3.0e38f ? a1.w : a1.w * P.inv_l;
+  // Eq. 12: temporal-smoothing state mu~(t1) + vbar dts, vbar = v exp(-rho/2) (Eq. 10)
+  float mm = m;
+  if (P.dts != 0.f) mm = fmaf(expf(-0.5f * rho), P.dts, m);
+  const float wx = fmaf(mm, a1.x, a0.x), wy = fmaf(mm, a1.y, a0.y), wz = fmaf(mm, a1.z, a0.z);
   // P2: Eq. 7 (beta = +INF gives exp(-0) = 1)
   const float op = a3.w * expf(-0.5f * (dt * dt) / (a1.w * a1.w));
   // P3: opacity cull; the comparison is false for NaN
   valid = (op >= PVG_ALPHA_MIN) && (op <= 3.0e38f);
+  // staticness filter: keep rho_min <= rho <= rho_max
+  if (P.filter) valid = valid && (rho >= P.rho_min) && !(rho > P.rho_max);
   // P4: camera space + near cull
   const float px = fmaf(P.R[0], wx, fmaf(P.R[1], wy, fmaf(P.R[2], wz, P.T[0])));
   const float py = fmaf(P.R[3], wx, fmaf(P.R[4], wy, fmaf(P.R[5], wz, P.T[1])));

@@ -418,7 +418,8 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   return PVG_OK;
 }
 
-int fill_frame(const pvg_scene* s, const pvg_camera* cam, float t, FrameParams* P) {
+int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state, FrameParams* P) {
+  const float t = (float)((double)state->t - (double)state->dt);
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
   if (!(cam->fx > 0.f) || !(cam->fy > 0.f) || !std::isfinite(cam->fx) || !std::isfinite(cam->fy) ||
       !std::isfinite(cam->cx) || !std::isfinite(cam->cy))
@@ -437,7 +438,12 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, float t, FrameParams* 
   P->limy = (float)(1.3 * cam->height / (2.0 * (double)cam->fy));
   P->znear = cam->znear > 0.f ? cam->znear : PVG_ZNEAR_DEFAULT;
   P->t = t;
+  P->dts = state->dt;
+  P->rho_min = state->rho_min;
+  P->rho_max = state->rho_max;
+  P->filter = (state->rho_min > 0.f || state->rho_max < INFINITY) ? 1 : 0;
   P->linear = std::isinf(s->cycle) ? 1 : 0;
+  P->inv_l = P->linear ? 0.f : (float)(1.0 / (double)s->cycle);
   P->two_over_l = P->linear ? 0.f : (float)(2.0 / (double)s->cycle);
   P->l_over_2pi = P->linear ? 0.f : (float)((double)s->cycle / (2.0 * 3.14159265358979323846));
   P->sh_degree = s->sh_degree;
@@ -540,9 +546,10 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   return PVG_OK;
 }
 
-int render_impl(pvg_scene* s, const pvg_camera* cam, float t, float* out_rgb, float* out_depth, float* out_alpha) {
+int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, float* out_rgb, float* out_depth,
+                float* out_alpha) {
   FrameParams P;
-  TRY(fill_frame(s, cam, t, &P));
+  TRY(fill_frame(s, cam, state, &P));
   cudaStream_t st = s->stream;
   Timer& tm = s->timer;
   if (!tm.accumulate) tm.reset();
@@ -731,6 +738,7 @@ const char* pvg_strerror(int code) {
     case PVG_ERR_INSTANCE_OVERFLOW: return "tile instance count overflows 32 bits";
     case PVG_ERR_CUDA: return "CUDA error";
     case PVG_ERR_BAD_OPTION: return "bad option";
+    case PVG_ERR_BAD_STATE: return "bad state (non-finite t or dt, negative rho_min, rho_max < rho_min)";
     default: return "unknown error";
   }
 }
@@ -796,10 +804,20 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
   }
 }
 
+static bool state_ok(const pvg_state* st) {
+  return std::isfinite(st->t) && std::isfinite(st->dt) && !(st->rho_min < 0.f) && !(st->rho_max < st->rho_min);
+}
+
+int pvg_render_state(pvg_scene* scene, const pvg_camera* cam, const pvg_state* state, float* out_rgb, float* out_depth,
+                     float* out_alpha) {
+  if (!scene || !cam || !state) return PVG_ERR_NULL;
+  if (!state_ok(state)) return PVG_ERR_BAD_STATE;
+  return render_impl(scene, cam, state, out_rgb, out_depth, out_alpha);
+}
+
 int pvg_render(pvg_scene* scene, const pvg_camera* cam, float t, float* out_rgb, float* out_depth, float* out_alpha) {
-  if (!scene || !cam) return PVG_ERR_NULL;
-  if (!std::isfinite(t)) return PVG_ERR_BAD_CAMERA;
-  return render_impl(scene, cam, t, out_rgb, out_depth, out_alpha);
+  const pvg_state st = {t, 0.f, 0.f, INFINITY};
+  return pvg_render_state(scene, cam, &st, out_rgb, out_depth, out_alpha);
 }
 
 int pvg_wait_host(pvg_scene* scene) {
@@ -815,7 +833,8 @@ int pvg_wait_host(pvg_scene* scene) {
 int pvg_render_host_async(pvg_scene* scene, const pvg_camera* cam, float t, float* host_rgb, float* host_depth,
                           float* host_alpha) {
   if (!scene || !cam) return PVG_ERR_NULL;
-  if (!std::isfinite(t)) return PVG_ERR_BAD_CAMERA;
+  const pvg_state state = {t, 0.f, 0.f, INFINITY};
+  if (!state_ok(&state)) return PVG_ERR_BAD_STATE;
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
   const size_t HW = (size_t)cam->width * cam->height;
   cudaStream_t st = scene->stream;
@@ -831,7 +850,7 @@ int pvg_render_host_async(pvg_scene* scene, const pvg_camera* cam, float t, floa
   float* d_rgb = scene->img[slot].as<float>();
   float* d_depth = d_rgb + 3 * HW;
   float* d_alpha = d_rgb + 4 * HW;
-  TRY(render_impl(scene, cam, t, host_rgb ? d_rgb : nullptr, host_depth ? d_depth : nullptr,
+  TRY(render_impl(scene, cam, &state, host_rgb ? d_rgb : nullptr, host_depth ? d_depth : nullptr,
                   host_alpha ? d_alpha : nullptr));
   CU(cudaEventRecord(scene->ev_rendered, st));
   cudaStream_t cs = scene->copy_stream;

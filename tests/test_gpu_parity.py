@@ -15,7 +15,8 @@ from workloads import make_config, pinhole_camera
 pytestmark = pytest.mark.gpu
 
 
-def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None, compact=True, block=True):
+def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, scene=None, compact=True, block=True,
+                state=None):
     """(P), (I), (R) for one frame. Returns the stats of the three comparisons."""
     own = scene is None
     sc = scene or pvg.Scene.from_workload_scene(wl_scene)
@@ -24,12 +25,13 @@ def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, sc
         sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
         sc.set_option(pvg.OPT_COMPACT_KEYS, 1 if compact else 0)
         sc.set_option(pvg.OPT_BLOCK_BINS, 1 if block else 0)
-        rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t))
+        kw = state or {}
+        rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t, **kw))
         dbg = sc.debug()
     finally:
         if own:
             sc.close()
-    wide, orec = oracle.preprocess_scene(wl_scene, cam, t)
+    wide, orec = oracle.preprocess_scene(wl_scene, cam, t, **(state or {}))
     stats = {"P": check_record(dbg["record"], wide, cam, wl_scene),
              "I": check_integer_chain(dbg, cam.width, cam.height, presort)}
     grec = dbg["record"]
@@ -189,6 +191,36 @@ def test_edge_cases():
     with pytest.raises(pvg.PvgError) as e:
         g.render(cam_bad, 0.0, out=g.render(cam, 0.0))
     assert e.value.code == -3
+    g.close()
+
+
+@pytest.mark.parametrize("state", [dict(dt=0.02), dict(dt=-0.013, rho_min=1.0), dict(rho_min=1.0),
+                                   dict(rho_max=0.999), dict(dt=0.005, rho_min=0.5, rho_max=4.0)])
+def test_temporal_smoothing_state_and_staticness_filter(state):
+    """H^(t) from t - dt (Eq. 12) and the rho filter (L118, L192), full parity."""
+    wl = make_config(1, n=60_000)
+    st = full_parity(wl.scene, wl.cameras[0], 0.5, state=state)
+    assert st["P"]["survivors_gpu"] > 1000
+
+
+def test_state_dt_zero_is_render_and_filter_partitions():
+    import torch
+    wl = make_config(0)
+    cam = wl.cameras[0]
+    g = pvg.Scene.from_workload_scene(wl.scene)
+    a = [x.clone() for x in g.render(cam, 0.37)]
+    b = g.render(cam, 0.37, rho_min=0.0, rho_max=3.0e38)            # goes through pvg_render_state, keeps every point
+    for x, y in zip(a, b):
+        assert torch.equal(x, y)
+    n_all = g.frame_stats()["survivors"]
+    g.render(cam, 0.37, rho_min=1.0)
+    n_static = g.frame_stats()["survivors"]
+    g.render(cam, 0.37, rho_max=float(np.nextafter(np.float32(1.0), np.float32(0.0))))
+    n_dyn = g.frame_stats()["survivors"]
+    assert n_static + n_dyn == n_all and 0 < n_dyn < n_all
+    with pytest.raises(pvg.PvgError) as e:
+        g.render(cam, 0.37, dt=float("nan"))
+    assert e.value.code == -8
     g.close()
 
 

@@ -606,3 +606,83 @@ class TestIntegerChain:
             s, e = k["ranges"][tl]
             if e > s:
                 assert list(k["vals_sorted"][s:e]) == [0, 1, 2, 3, 4]
+
+
+# ----------------------------------------------------------------------------- f-1: Eq. 10 / Eq. 12, staticness filter
+class TestTemporalSmoothingState:
+    """H^(t2) = { mu~(t1) + vbar (t2 - t1), q, s, o~(t1), c }, vbar = v exp(-rho/2), rho = beta/l
+    (Eq. 10, Eq. 12, rho L112); filter on rho (L118, L192)."""
+    mu = np.array([0.5, -0.25, 6.0])
+    v = np.array([1.5, -0.75, 0.5])
+    tau = 0.25
+    cam = cam_simple()
+
+    def state(self, t, dt, beta, cycle=L, **kw):
+        sc = one_scene(mu=self.mu, vel=self.v, tau=self.tau, beta=beta, cycle=cycle, opacity=0.8)
+        w = oracle.preprocess_scene(sc, self.cam, t, dt, **kw)[0][0]
+        return w[SLOTS["mu"]], w[SLOTS["op"]], int(w[SLOTS["cull"]])
+
+    def test_dt_zero_is_the_plain_state(self):       # "assign a probability of eta to set dt as 0 (no estimation)", L166
+        wl = make_config(0)
+        a = oracle.preprocess_scene(wl.scene, wl.cameras[0], 0.37)
+        b = oracle.preprocess_scene(wl.scene, wl.cameras[0], 0.37, 0.0)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+    def test_opacity_is_taken_at_t1(self):           # Eq. 12: o~(t1), not o~(t2)
+        for dt in (-0.03, 0.02):
+            _, op_hat, _ = self.state(0.3, dt, beta=0.1)
+            _, op_t1, _ = self.state(0.3 - dt, 0.0, beta=0.1)
+            assert op_hat == op_t1
+
+    def test_flow_translation(self):                 # Eq. 12 minus the plain state at t1 is vbar * dt; Eq. 10 for vbar
+        for beta, dt in ((0.05, 0.02), (0.3, -0.015), (0.02, 0.01)):
+            mu_hat, _, _ = self.state(0.31, dt, beta)
+            mu_t1, _, _ = self.state(0.31 - dt, 0.0, beta)
+            rho = float(np.float32(beta)) / L          # the model stores beta in fp32
+            assert np.allclose(mu_hat - mu_t1, self.v * math.exp(-rho / 2) * dt, rtol=1e-11, atol=1e-16)
+
+    def test_limits_of_the_average_velocity(self):   # T8, PAPER.md:L156: rho -> inf: vbar -> 0; rho -> 0: vbar -> v
+        dt = 0.02
+        mu_hat, _, _ = self.state(0.3, dt, beta=np.inf)
+        mu_t1, _, _ = self.state(0.3 - dt, 0.0, beta=np.inf)
+        assert np.array_equal(mu_hat, mu_t1)                                  # vbar = 0 exactly
+        mu_hat, _, _ = self.state(0.3, dt, beta=1e-9)
+        mu_t1, _, _ = self.state(0.3 - dt, 0.0, beta=1e-9)
+        assert np.allclose(mu_hat - mu_t1, self.v * dt, rtol=1e-8)           # vbar = v
+
+    def test_estimates_the_next_state_of_a_fast_point(self):
+        """L160: 'dynamic objects often maintain a constant speed within a short time interval': for rho -> 0 and
+        t1, t2 near tau the estimate equals the true state up to the curvature of the sine, |v| |D|^3 (2 pi / l)^2 / 6
+        summed over the two ends."""
+        beta, dt, t2 = 1e-6, 0.004, self.tau + 0.006
+        mu_hat, _, _ = self.state(t2, dt, beta)
+        mu_true, _, _ = self.state(t2, 0.0, beta)
+        k = (2 * math.pi / L) ** 2 / 6
+        bound = np.linalg.norm(self.v) * k * (abs(t2 - self.tau) ** 3 + abs(t2 - dt - self.tau) ** 3)
+        assert 0 < np.linalg.norm(mu_hat - mu_true) <= bound * (1 + 1e-6)
+
+    def test_linear_model_has_rho_zero(self):        # l = +inf: rho = beta / l = 0, vbar = v, and mu + v (t1 - tau) + v dt = mu + v (t2 - tau)
+        mu_hat, _, _ = self.state(0.4, 0.05, beta=0.1, cycle=np.inf)
+        assert np.allclose(mu_hat, self.mu + self.v * (0.4 - self.tau), rtol=1e-14)
+
+    def test_staticness_filter(self):                # L192: "remove the PVG points whose rho < 1"
+        assert self.state(0.25, 0.0, beta=0.19, rho_min=1.0)[2] == 6          # rho = 0.95: removed
+        assert self.state(0.25, 0.0, beta=0.2, rho_min=1.0)[2] == 0           # rho = 1: kept (fp32 0.2 / 0.2)
+        assert self.state(0.25, 0.0, beta=np.inf, rho_min=1.0)[2] == 0        # 3DGS point: rho = +inf (L114)
+        assert self.state(0.25, 0.0, beta=0.5, rho_max=1.0)[2] == 6           # dynamic-only view drops static points
+        assert self.state(0.25, 0.0, beta=0.1, rho_max=1.0)[2] == 0
+        assert self.state(0.25, 0.0, beta=50.0, cycle=np.inf, rho_min=1e-3)[2] == 6   # l = inf: rho = 0
+
+    def test_filter_partitions_the_scene(self):
+        """rho < 1 and rho >= 1 partition the points: the two filtered records are disjoint and their union is the
+        unfiltered record, row by row."""
+        wl = make_config(0)
+        cam = wl.cameras[0]
+        full = oracle.preprocess_scene(wl.scene, cam, 0.37)[1]
+        stat = oracle.preprocess_scene(wl.scene, cam, 0.37, 0.0, 1.0)[1]
+        rho = wl.scene.beta.astype(np.float64) / wl.scene.cycle
+        dyn = oracle.preprocess_scene(wl.scene, cam, 0.37, 0.0, 0.0, float(np.nextafter(1.0, 0.0)))[1]
+        keep = rho >= 1.0
+        assert np.array_equal(stat[keep], full[keep]) and not stat[~keep].any()
+        assert np.array_equal(dyn[~keep], full[~keep]) and not dyn[keep].any()
+        assert 0 < keep.sum() < len(keep)
