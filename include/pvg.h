@@ -106,6 +106,16 @@ typedef struct pvg_state {
 int pvg_render_state(pvg_scene *scene, const pvg_camera *cam, const pvg_state *state, float *out_rgb,
                      float *out_depth, float *out_alpha);
 
+/* Sky: "a high-resolution learnable environment cube map f_sky(d) = c_sky as the background.
+ * The final color is C_f = C + (1 - O) f_sky(d)". cube = [6][res][res][3] floats (host or
+ * device; copied), NULL switches the sky off (the camera's constant bg is used again). d is the pixel-centre
+ * ray in WORLD coordinates, R^T ((x - cx)/fx, (y - cy)/fy, 1). Layout (the paper fixes none): face =
+ * 2 a + (d_a < 0) for the axis a of largest |d_a| (faces +x, -x, +y, -y, +z, -z; ties: lowest axis);
+ * u = d_b / |d_a|, v = d_c / |d_a| with (b, c) the next two axes in cyclic order; texel (i, j) = cube[face][j][i]
+ * has its centre at u = (2 i + 1)/res - 1, v = (2 j + 1)/res - 1; bilinear between the four nearest centres,
+ * clamped to the face (no filtering across faces). Synchronises the scene's stream. */
+int pvg_set_sky(pvg_scene *scene, const float *cube, int res, int on_device);
+
 /* Same frame into HOST buffers (pinned or pageable): renders into library-owned device images,
  * copies them back and synchronises the stream before returning. */
 int pvg_render_host(pvg_scene *scene, const pvg_camera *cam, float t, float *host_rgb,

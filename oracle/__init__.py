@@ -169,3 +169,26 @@ def render(rec, width, height, bg=(0.0, 0.0, 0.0), mode="binned", tiles: Optiona
                         _p(cond), _p(stats))
     return dict(rgb=rgb, depth=depth, alpha=alpha, budget=budget, cond=cond,
                 visited=int(stats[0]), contributed=int(stats[1]))
+
+
+def sky_sample(cube, d):
+    """f_sky(d): bilinear lookup in a cube map [6][R][R][3] (face = 2 axis + (d_axis < 0))."""
+    cube = np.ascontiguousarray(cube, dtype=np.float32)
+    res = cube.shape[1]
+    assert cube.shape == (6, res, res, 3)
+    d = np.ascontiguousarray(d, dtype=np.float64)
+    out = np.empty(3, dtype=np.float64)
+    lib().oracle_sky_sample(_p(cube), C.c_int(res), _p(d), _p(out))
+    return out
+
+
+def sky_composite(cam, cube, rgb, alpha):
+    """C_f = C + (1 - O) f_sky(d) on an Oracle-R image rendered with bg = 0. Returns a new rgb."""
+    cube = np.ascontiguousarray(cube, dtype=np.float32)
+    res = cube.shape[1]
+    assert cube.shape == (6, res, res, 3)
+    out = np.array(rgb, dtype=np.float64, order="C", copy=True)
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64)
+    c = _cam(cam)
+    lib().oracle_sky_composite(C.byref(c), _p(cube), C.c_int(res), _p(out), _p(alpha))
+    return out

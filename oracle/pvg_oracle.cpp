@@ -18,7 +18,8 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed forms T1..T8 of the
 // paper, single-Gaussian image, stop/clamp/cutoff rules, brute force == binned,
 // std::stable_sort equivalence on tiny scenes; for oracle_preprocess_state (Eq. 10 / 12,
-// staticness filter) TestTemporalSmoothingState. "Absolute values on real data"
+// staticness filter) TestTemporalSmoothingState; for the sky cube map (oracle_sky_*) TestSky.
+// "Absolute values on real data"
 // is parity unpinned (the paper prints no worked numeric example).
 
 #include <algorithm>
@@ -525,6 +526,56 @@ void oracle_render(uint64_t n, const float* rec, int width, int height, const do
       }
   }
   if (stats) { stats[0] = visited; stats[1] = contributed; }
+}
+
+// f-3: sky. "we utilize a high-resolution learnable environment cube map f_sky(d) = c_sky as
+// the background. The final color is C_f = C + (1 - O) f_sky(d)"; "the sky color depends
+// solely on the viewing direction". The paper fixes neither the cube-map layout nor the filter; readings
+// (S20-S22):
+//   d     = R^T ((px + 0.5 - cx) / fx, (py + 0.5 - cy) / fy, 1): the pixel-centre ray in world coordinates;
+//   face  = 2 a + (d_a < 0), a = the axis of largest |d_a| (ties: lowest axis); the other two axes in cyclic
+//           order (x -> y,z; y -> z,x; z -> x,y) give u = d_b / |d_a|, v = d_c / |d_a| in [-1, 1];
+//   texel (i, j) of a face of resolution R has its centre at u = (2 i + 1) / R - 1, v = (2 j + 1) / R - 1;
+//           cube[face][j][i][ch]; bilinear between the four nearest centres, clamped to the face.
+// sky_sample is the definition written out; oracle_sky_composite applies C_f to an Oracle-R image rendered
+// with bg = 0 (then rgb = C and alpha = O).
+void oracle_sky_sample(const float* cube, int res, const double d[3], double out[3]) {
+  int a = 0;
+  if (std::fabs(d[1]) > std::fabs(d[a])) a = 1;
+  if (std::fabs(d[2]) > std::fabs(d[a])) a = 2;
+  const int b = (a + 1) % 3, c = (a + 2) % 3;
+  const double m = std::fabs(d[a]);
+  const int face = 2 * a + (d[a] < 0.0 ? 1 : 0);
+  const double u = d[b] / m, v = d[c] / m;
+  // continuous texel coordinates: centre of texel i is at s = i
+  double sx = (u + 1.0) * 0.5 * res - 0.5, sy = (v + 1.0) * 0.5 * res - 0.5;
+  sx = std::fmin(std::fmax(sx, 0.0), (double)(res - 1));
+  sy = std::fmin(std::fmax(sy, 0.0), (double)(res - 1));
+  const int i0 = (int)std::floor(sx), j0 = (int)std::floor(sy);
+  const int i1 = std::min(i0 + 1, res - 1), j1 = std::min(j0 + 1, res - 1);
+  const double fx = sx - i0, fy = sy - j0;
+  const float* F = cube + (size_t)face * res * res * 3;
+  for (int ch = 0; ch < 3; ++ch) {
+    const double c00 = F[((size_t)j0 * res + i0) * 3 + ch], c10 = F[((size_t)j0 * res + i1) * 3 + ch];
+    const double c01 = F[((size_t)j1 * res + i0) * 3 + ch], c11 = F[((size_t)j1 * res + i1) * 3 + ch];
+    out[ch] = (1.0 - fy) * ((1.0 - fx) * c00 + fx * c10) + fy * ((1.0 - fx) * c01 + fx * c11);
+  }
+}
+
+// rgb [3][H][W] (= C, rendered with bg = 0) and alpha [H][W] (= O) -> rgb += (1 - O) f_sky(d), in place
+void oracle_sky_composite(const Cam* cam, const float* cube, int res, double* rgb, const double* alpha) {
+  const double* R = cam->w2c;
+  const uint64_t HW = (uint64_t)cam->width * cam->height;
+  for (int py = 0; py < cam->height; ++py)
+    for (int px = 0; px < cam->width; ++px) {
+      const double dc[3] = {(px + 0.5 - cam->cx) / cam->fx, (py + 0.5 - cam->cy) / cam->fy, 1.0};
+      double d[3];
+      for (int j = 0; j < 3; ++j) d[j] = R[0 + j] * dc[0] + R[4 + j] * dc[1] + R[8 + j] * dc[2];   // R^T d_cam
+      double sky[3];
+      oracle_sky_sample(cube, res, d, sky);
+      const uint64_t pi = (uint64_t)py * cam->width + px;
+      for (int ch = 0; ch < 3; ++ch) rgb[ch * HW + pi] += (1.0 - alpha[pi]) * sky[ch];
+    }
 }
 
 int oracle_num_threads() {

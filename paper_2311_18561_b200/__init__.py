@@ -25,7 +25,7 @@ NUM_STAGES = len(STAGES)
 
 # every symbol include/pvg.h declares
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
-           "pvg_render_host_async", "pvg_wait_host", "pvg_render_state",
+           "pvg_render_host_async", "pvg_wait_host", "pvg_render_state", "pvg_set_sky",
            "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms",
            "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
@@ -84,6 +84,7 @@ def load_library(path: Optional[str] = None):
     L.pvg_create_scene.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.pvg_render.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_render_state.argtypes = [C.c_void_p, C.POINTER(CameraC), C.POINTER(StateC), C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_set_sky.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int]
     L.pvg_render_host.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_render_host_async.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_wait_host.argtypes = [C.c_void_p]
@@ -232,6 +233,23 @@ class Scene:
         _check(self._L.pvg_render_host(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
                                        out[2].data_ptr()))
         return out
+
+    def set_sky(self, cube) -> None:
+        """Sky cube map [6, R, R, 3] (numpy or torch CUDA tensor; copied), or None to switch it off:
+        rgb = C + (1 - O) f_sky(d) (PAPER.md:L168)."""
+        import torch
+        _check(self._L.pvg_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
+        if cube is None:
+            _check(self._L.pvg_set_sky(self._h, None, 0, 0))
+            return
+        if _is_torch(cube) and cube.is_cuda:
+            c = cube.detach().to(torch.float32).contiguous()
+            assert c.dim() == 4 and c.shape[0] == 6 and c.shape[1] == c.shape[2] and c.shape[3] == 3
+            _check(self._L.pvg_set_sky(self._h, c.data_ptr(), int(c.shape[1]), 1))
+        else:
+            c = np.ascontiguousarray(cube.detach().cpu().numpy() if _is_torch(cube) else cube, dtype=np.float32)
+            assert c.ndim == 4 and c.shape[0] == 6 and c.shape[1] == c.shape[2] and c.shape[3] == 3
+            _check(self._L.pvg_set_sky(self._h, c.ctypes.data, int(c.shape[1]), 0))
 
     def render_host_async(self, cam, t: float, out: Tuple):
         """Pipelined render into pinned HOST tensors; read them only after wait_host()."""

@@ -25,6 +25,37 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
+// f_sky(d) (layout and filter: DESIGN.md S20-S22): face = 2 a + (d_a < 0) with a the axis of
+// largest |d_a| (ties: lowest axis), u = d_b / |d_a|, v = d_c / |d_a| for (b, c) the next two axes in cyclic
+// order, texel centres at (2 i + 1) / res - 1, bilinear between the four nearest centres, clamped to the face.
+__device__ __forceinline__ void sky_sample(const float* __restrict__ cube, int res, float dx, float dy, float dz, float (&out)[3]) {
+  const float ax = fabsf(dx), ay = fabsf(dy), az = fabsf(dz);
+  int a = 0;
+  float m = ax, da = dx, u = dy, v = dz;
+  if (ay > m) { a = 1; m = ay; da = dy; u = dz; v = dx; }
+  if (az > m) { a = 2; m = az; da = dz; u = dx; v = dy; }
+  const int face = 2 * a + (da < 0.f ? 1 : 0);
+  const float inv = 1.0f / m;
+  const float r = (float)res;
+  float sx = fmaf(fmaf(u, inv, 1.0f), 0.5f * r, -0.5f), sy = fmaf(fmaf(v, inv, 1.0f), 0.5f * r, -0.5f);
+  sx = fminf(fmaxf(sx, 0.f), r - 1.0f);
+  sy = fminf(fmaxf(sy, 0.f), r - 1.0f);
+  const int i0 = (int)sx, j0 = (int)sy;   // sx, sy >= 0: truncation is the floor
+  const int i1 = min(i0 + 1, res - 1), j1 = min(j0 + 1, res - 1);
+  const float fx = sx - (float)i0, fy = sy - (float)j0;
+  const float* F = cube + (size_t)face * res * res * 3;
+  const float* p00 = F + ((size_t)j0 * res + i0) * 3;
+  const float* p10 = F + ((size_t)j0 * res + i1) * 3;
+  const float* p01 = F + ((size_t)j1 * res + i0) * 3;
+  const float* p11 = F + ((size_t)j1 * res + i1) * 3;
+#pragma unroll
+  for (int ch = 0; ch < 3; ++ch) {
+    const float top = fmaf(fx, __ldg(p10 + ch) - __ldg(p00 + ch), __ldg(p00 + ch));
+    const float bot = fmaf(fx, __ldg(p11 + ch) - __ldg(p01 + ch), __ldg(p01 + ch));
+    out[ch] = fmaf(fy, bot - top, top);
+  }
+}
+
 // Per-pixel compositing state and one front-to-back step. The cutoffs are predicates (selects),
 // not branches: alpha < 1/255 skips, T' = T - alpha T < 1e-4 stops the pixel WITHOUT compositing
 // the Gaussian that crosses the threshold (S10).
@@ -63,7 +94,9 @@ struct BlendPixel {
 // pixels is alive; the tile retires when every pixel's transmittance has dropped below 1e-4.
 // COUNT = true additionally counts the (pixel, list entry) evaluations reached and the
 // contributing ones into counters[0..1] (measurement only, never on the product path).
-template <bool COUNT>
+// SKY = true: the background is the cube map f_sky(d) instead of the constant bg (its own instantiation, so
+// that the lookup's registers do not cost the plain kernel occupancy: 69 against 62 registers).
+template <bool COUNT, bool SKY>
 __global__ void __launch_bounds__(BLEND_THREADS)
 blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
              const uint32_t* __restrict__ vals, const float4* __restrict__ record,
@@ -155,9 +188,16 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
     if (!in[k]) continue;
     const float Al = 1.0f - X[k].T;
     if (out_rgb) {
-      out_rgb[pi + k] = fmaf(X[k].T, P.bg[0], X[k].Cr);
-      out_rgb[HW + pi + k] = fmaf(X[k].T, P.bg[1], X[k].Cg);
-      out_rgb[2 * HW + pi + k] = fmaf(X[k].T, P.bg[2], X[k].Cb);
+      float bg[3] = {P.bg[0], P.bg[1], P.bg[2]};
+      if (SKY) {
+        // the pixel-centre ray in world coordinates: R^T ((x - cx) / fx, (y - cy) / fy, 1)
+        const float cxr = (pxf + (float)k - P.cx) / P.fx, cyr = (pyf - P.cy) / P.fy;
+        sky_sample(P.sky, P.sky_res, fmaf(P.R[0], cxr, fmaf(P.R[3], cyr, P.R[6])),
+                   fmaf(P.R[1], cxr, fmaf(P.R[4], cyr, P.R[7])), fmaf(P.R[2], cxr, fmaf(P.R[5], cyr, P.R[8])), bg);
+      }
+      out_rgb[pi + k] = fmaf(X[k].T, bg[0], X[k].Cr);
+      out_rgb[HW + pi + k] = fmaf(X[k].T, bg[1], X[k].Cg);
+      out_rgb[2 * HW + pi + k] = fmaf(X[k].T, bg[2], X[k].Cb);
     }
     if (out_depth) out_depth[pi + k] = Al > 0.f ? X[k].D / Al : 0.f;
     if (out_alpha) out_alpha[pi + k] = Al;

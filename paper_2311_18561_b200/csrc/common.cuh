@@ -37,6 +37,8 @@ struct FrameParams {
   int width, height, tiles_x, tiles_y;
   int pack_rect;      // tiles_x, tiles_y <= 256: the depth key carries the tile rectangle in its upper half
   float bg[3];
+  const float* sky;   // cube map [6][res][res][3] or nullptr: rgb = C + (1 - O) f_sky(d)
+  int sky_res;
 };
 
 __device__ __forceinline__ uint32_t lane_id() {

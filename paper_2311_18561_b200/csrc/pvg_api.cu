@@ -313,6 +313,8 @@ struct pvg_scene {
   // block-entry workspace (blockbin.cuh)
   Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
   Buf ranges, tilegrid;
+  Buf sky;     // cube map [6][res][res][3] (pvg_set_sky)
+  int sky_res = 0;
   Buf img[2];  // render_host device images (double-buffered: the copy of frame k overlaps frame k + 1)
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_rendered = nullptr, ev_copied[2] = {nullptr, nullptr};
@@ -345,7 +347,7 @@ void release_all(pvg_scene* s) {
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
-                 &s->ranges, &s->tilegrid, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->ranges, &s->tilegrid, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
@@ -452,6 +454,8 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   P->tiles_y = (cam->height + PVG_TILE - 1) / PVG_TILE;
   P->pack_rect = (P->tiles_x <= 256 && P->tiles_y <= 256) ? 1 : 0;
   for (int j = 0; j < 3; ++j) P->bg[j] = cam->bg[j];
+  P->sky = s->sky_res > 0 ? s->sky.as<float>() : nullptr;
+  P->sky_res = s->sky_res;
   return PVG_OK;
 }
 
@@ -707,14 +711,22 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
 
   // a5 blend
   TRY(tm.begin("blend", PVG_STAGE_BLEND, st));
-  if (s->count_pairs) {
-    unsigned long long* ctr = reinterpret_cast<unsigned long long*>(s->small.as<unsigned char>() + 64);
-    CU(cudaMemsetAsync(ctr, 0, 16, st));
-    blend_kernel<true><<<tiles, BLEND_THREADS, 0, st>>>(P, s->ranges.as<uint2>(), s->vals[s->sorted_side].as<uint32_t>(),
-                                                        s->record.as<float4>(), out_rgb, out_depth, out_alpha, ctr);
-  } else {
-    blend_kernel<false><<<tiles, BLEND_THREADS, 0, st>>>(P, s->ranges.as<uint2>(), s->vals[s->sorted_side].as<uint32_t>(),
-                                                         s->record.as<float4>(), out_rgb, out_depth, out_alpha, nullptr);
+  {
+    unsigned long long* ctr = nullptr;
+    if (s->count_pairs) {
+      ctr = reinterpret_cast<unsigned long long*>(s->small.as<unsigned char>() + 64);
+      CU(cudaMemsetAsync(ctr, 0, 16, st));
+    }
+    const uint2* rg = s->ranges.as<uint2>();
+    const uint32_t* vl = s->vals[s->sorted_side].as<uint32_t>();
+    const float4* rec = s->record.as<float4>();
+    const int variant = (s->count_pairs ? 2 : 0) | (P.sky ? 1 : 0);
+    switch (variant) {
+      case 0: blend_kernel<false, false><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
+      case 1: blend_kernel<false, true><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
+      case 2: blend_kernel<true, false><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
+      default: blend_kernel<true, true><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
+    }
   }
   TRY(tm.end(st));
   CU(cudaGetLastError());
@@ -784,6 +796,25 @@ int pvg_destroy(pvg_scene* scene) {
   if (scene->copy_stream) cudaStreamSynchronize(scene->copy_stream);
   release_all(scene);
   delete scene;
+  return PVG_OK;
+}
+
+int pvg_set_sky(pvg_scene* scene, const float* cube, int res, int on_device) {
+  if (!scene) return PVG_ERR_NULL;
+  cudaStream_t st = scene->stream;
+  CU(cudaStreamSynchronize(st));   // frames in flight may still read the old map
+  if (scene->copy_stream) CU(cudaStreamSynchronize(scene->copy_stream));
+  if (!cube) {
+    scene->sky_res = 0;
+    return PVG_OK;
+  }
+  if (res < 1 || res > 16384) return PVG_ERR_BAD_OPTION;
+  const size_t bytes = (size_t)6 * res * res * 3 * sizeof(float);
+  scene->sky_res = 0;
+  TRY(scene->sky.reserve(bytes, st));
+  CU(cudaMemcpyAsync(scene->sky.p, cube, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+  CU(cudaStreamSynchronize(st));
+  scene->sky_res = res;
   return PVG_OK;
 }
 

@@ -224,6 +224,37 @@ def test_state_dt_zero_is_render_and_filter_partitions():
     g.close()
 
 
+@pytest.mark.parametrize("cfg,n,cam_i,res", [(1, 40_000, 0, 256), (4, 20_000, 1, 64), (4, 20_000, 4, 1024)])
+def test_sky_cube_map(cfg, n, cam_i, res):
+    """rgb = C + (1 - O) f_sky(d) against the oracle's sky composite on Oracle-R's
+    image of the GPU record; yawed cameras look at other faces and across face seams."""
+    from workloads import sky_cubemap
+    wl = make_config(cfg, n=n)
+    cam = wl.cameras[cam_i]
+    cube = sky_cubemap(res, seed=cfg)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    plain = [x.cpu().numpy() for x in sc.render(cam, 0.25)]
+    sc.set_sky(cube)
+    rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, 0.25))
+    grec = sc.debug(["record"])["record"]
+    sc.set_sky(None)
+    again = [x.cpu().numpy() for x in sc.render(cam, 0.25)]
+    sc.close()
+    assert all(np.array_equal(a, b) for a, b in zip(plain, again))           # switching the sky off restores bg
+    assert np.array_equal(depth, plain[1]) and np.array_equal(alpha, plain[2])
+    ora = oracle.render(grec, cam.width, cam.height, bg=(0, 0, 0), mode="binned")
+    ora["rgb"] = oracle.sky_composite(cam, cube, ora["rgb"], ora["alpha"])
+    # fp32 ray and texel coordinates: the lookup position is off by <= 4e-4 texel (0.5 res * a few ulps of u),
+    # i.e. by that share of the largest difference between neighbouring texels; a ray within that distance of a
+    # face seam may land on the neighbouring face, whose edge texels differ by about one texel step as well
+    step = max(np.abs(np.diff(cube, axis=1)).max(), np.abs(np.diff(cube, axis=2)).max())
+    ora["cond"] = ora["cond"] + (1 - ora["alpha"]) * step * 1e-3
+    zmax = float(max(grec[:, 2].max(), 1.0))
+    st = check_images((rgb, depth, alpha), ora, zmax, label="sky")
+    assert st["max_rgb_err_clean"] <= 2e-4
+    assert np.abs(rgb - plain[0]).max() > 1e-3                                # the sky shows through (barely at the dense config 4)
+
+
 def test_render_host_matches_render():
     wl = make_config(0)
     cam = wl.cameras[0]

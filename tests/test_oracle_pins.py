@@ -686,3 +686,88 @@ class TestTemporalSmoothingState:
         assert np.array_equal(stat[keep], full[keep]) and not stat[~keep].any()
         assert np.array_equal(dyn[~keep], full[~keep]) and not dyn[keep].any()
         assert 0 < keep.sum() < len(keep)
+
+
+# ----------------------------------------------------------------------------- f-3: sky cube map
+class TestSky:
+    """C_f = C + (1 - O) f_sky(d); cube-map layout and filter: DESIGN.md S20-S22."""
+
+    @staticmethod
+    def direction(face, u, v):
+        a, sign = face // 2, (1.0 if face % 2 == 0 else -1.0)
+        d = np.zeros(3)
+        d[a], d[(a + 1) % 3], d[(a + 2) % 3] = sign, u, v
+        return d
+
+    def test_constant_map(self):
+        cube = np.full((6, 8, 8, 3), 0.0, np.float32)
+        cube[..., 0], cube[..., 1], cube[..., 2] = 0.25, 0.5, 0.75
+        rng = np.random.default_rng(0)
+        for d in rng.normal(size=(50, 3)):
+            assert np.array_equal(oracle.sky_sample(cube, d), [0.25, 0.5, 0.75])
+
+    def test_axis_directions_pick_their_face(self):
+        cube = np.zeros((6, 4, 4, 3), np.float32)
+        for f in range(6):
+            cube[f] = f + 1
+        for f in range(6):
+            assert np.array_equal(oracle.sky_sample(cube, self.direction(f, 0.0, 0.0)), [f + 1] * 3)
+            assert np.array_equal(oracle.sky_sample(cube, 7.5 * self.direction(f, 0.3, -0.8)), [f + 1] * 3)   # |d| irrelevant
+
+    def test_texel_centres_return_the_texel(self):
+        rng = np.random.default_rng(1)
+        res = 16
+        cube = rng.random((6, res, res, 3)).astype(np.float32)
+        for _ in range(200):
+            f, i, j = rng.integers(6), rng.integers(res), rng.integers(res)
+            d = self.direction(f, (2 * i + 1) / res - 1, (2 * j + 1) / res - 1)
+            assert np.allclose(oracle.sky_sample(cube, d), cube[f, j, i], rtol=0, atol=1e-12)
+
+    def test_bilinear_reproduces_affine_faces(self):
+        res = 32
+        i, j = np.meshgrid(np.arange(res), np.arange(res), indexing="xy")
+        cube = np.zeros((6, res, res, 3), np.float32)
+        for f in range(6):
+            cube[f, ..., 0], cube[f, ..., 1], cube[f, ..., 2] = i, j, 0.5 * i - 0.25 * j + f   # exact in fp32
+        rng = np.random.default_rng(2)
+        lim = 1 - 1 / res                                   # between the outermost texel centres
+        for _ in range(200):
+            f, u, v = rng.integers(6), rng.uniform(-lim, lim), rng.uniform(-lim, lim)
+            si, sj = (u + 1) / 2 * res - 0.5, (v + 1) / 2 * res - 0.5
+            got = oracle.sky_sample(cube, self.direction(f, u, v))
+            assert np.allclose(got, [si, sj, 0.5 * si - 0.25 * sj + f], rtol=0, atol=1e-10)
+
+    def test_clamped_at_the_face_edge(self):
+        res = 8
+        i, j = np.meshgrid(np.arange(res), np.arange(res), indexing="xy")
+        cube = np.zeros((6, res, res, 3), np.float32)
+        cube[0, ..., 0], cube[0, ..., 1] = i, j
+        got = oracle.sky_sample(cube, self.direction(0, 0.999999, 0.0))      # beyond the last centre: edge value
+        assert np.allclose(got[:2], [res - 1, (0 + 1) / 2 * res - 0.5], atol=1e-9)
+
+    def test_composite_weights_by_one_minus_opacity(self):
+        cam = cam_simple(64, 48, 50.0)
+        rec = np.stack([record_row(32.3, 24.2, 3.0, 0.7, 0.02, 0.0, 0.02, rgb=(0.2, 0.4, 0.6))])
+        base = oracle.render(rec, cam.width, cam.height, mode="brute")
+        cube = np.zeros((6, 4, 4, 3), np.float32)
+        cube[4] = (0.1, 0.3, 0.9)                          # +z face: identity pose looks down +z, FoV < 45 deg
+        out = oracle.sky_composite(cam, cube, base["rgb"], base["alpha"])
+        sky = np.array([0.1, 0.3, 0.9], np.float32).astype(np.float64)       # the map holds fp32 values
+        expect = base["rgb"] + (1 - base["alpha"])[None] * sky[:, None, None]
+        assert np.allclose(out, expect, rtol=0, atol=1e-15)
+        # a constant map is a constant background: ties the sky to the pinned bg path (S13)
+        const = np.zeros((6, 4, 4, 3), np.float32)
+        const[...] = (0.5, 0.25, 0.125)
+        with_bg = oracle.render(rec, cam.width, cam.height, bg=(0.5, 0.25, 0.125), mode="brute")
+        assert np.allclose(oracle.sky_composite(cam, const, base["rgb"], base["alpha"]), with_bg["rgb"], rtol=0, atol=1e-15)
+
+    def test_direction_is_in_world_coordinates(self):
+        """Camera yawed by +90 deg (camera->world = R_y: camera +z points along world +x): an empty frame shows the +x face."""
+        cube = np.zeros((6, 4, 4, 3), np.float32)
+        for f in range(6):
+            cube[f] = f + 1
+        zero = np.zeros((3, 48, 64)), np.zeros((48, 64))
+        for yaw, face in ((0.0, 4), (90.0, 0), (-90.0, 1), (180.0, 5)):
+            cam = pinhole_camera(64, 48, 50.0, yaw_deg=yaw)
+            out = oracle.sky_composite(cam, cube, *zero)
+            assert np.all(out[:, 20:28, 28:36] == face + 1), (yaw, out[0, 24, 32])

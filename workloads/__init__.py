@@ -14,5 +14,6 @@ from .gen import (  # noqa: F401
     pinhole_camera,
     rng_uniform,
     rng_normal,
+    sky_cubemap,
     splitmix64,
 )

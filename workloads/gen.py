@@ -232,3 +232,29 @@ def make_config(config_id: int, n: Optional[int] = None, seed: Optional[int] = N
     if n is not None:
         desc += f" [n overridden to {scene.n}]"
     return Workload(config_id, seed, scene, cams, ts, desc)
+
+
+def sky_cubemap(res: int = 256, seed: int = 0) -> np.ndarray:
+    """Synthetic sky for the cube-map background (the trained map is not available): a smooth
+    function of the world direction -- horizon-to-zenith gradient (+y is down, so up is -y) plus a sun lobe --
+    sampled at the texel centres of the layout include/pvg.h documents: cube[face][j][i], face = 2 a + (d_a < 0),
+    u = d_b / |d_a| = (2 i + 1) / res - 1, v = d_c / |d_a| = (2 j + 1) / res - 1, (b, c) = next axes in cyclic order.
+    Returns float32 [6, res, res, 3]."""
+    c = (2.0 * np.arange(res, dtype=np.float64) + 1.0) / res - 1.0
+    u, v = np.meshgrid(c, c, indexing="xy")            # u varies along i (last index), v along j
+    sun = np.array([0.3 + 0.1 * seed, -0.5, 0.8])
+    sun /= np.linalg.norm(sun)
+    cube = np.empty((6, res, res, 3), dtype=np.float32)
+    for face in range(6):
+        a, sign = face // 2, (1.0 if face % 2 == 0 else -1.0)
+        d = np.empty((res, res, 3))
+        d[..., a] = sign
+        d[..., (a + 1) % 3] = u
+        d[..., (a + 2) % 3] = v
+        d /= np.linalg.norm(d, axis=-1, keepdims=True)
+        up = -d[..., 1]
+        t = np.clip(0.5 + 0.5 * up, 0.0, 1.0)
+        base = np.stack([0.75 - 0.45 * t, 0.82 - 0.32 * t, 0.95 - 0.10 * t], -1)
+        lobe = np.clip((d * sun).sum(-1), 0.0, 1.0) ** 64
+        cube[face] = (base + lobe[..., None] * np.array([1.0, 0.9, 0.6])).astype(np.float32)
+    return cube
