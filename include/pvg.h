@@ -33,7 +33,7 @@ typedef enum pvg_status {
   PVG_ERR_INSTANCE_OVERFLOW = -5, /* tile instances M >= 2^32 */
   PVG_ERR_CUDA = -6,              /* CUDA runtime error (or no device); see pvg_last_cuda_error */
   PVG_ERR_BAD_OPTION = -7,
-  PVG_ERR_BAD_STATE = -8          /* non-finite t or dt, rho_min < 0, rho_max < rho_min */
+  PVG_ERR_BAD_STATE = -8          /* non-finite t or dt, rho_min < 0, rho_max < rho_min, unknown target */
 } pvg_status;
 
 typedef struct pvg_scene pvg_scene; /* opaque; owns device copies of the model and a growable workspace */
@@ -100,8 +100,19 @@ int pvg_render(pvg_scene *scene, const pvg_camera *cam, float t, float *out_rgb,
  *   rho_min, rho_max: only points with rho_min <= rho <= rho_max are drawn; {0, +INF} draws all. The paper
  *            removes rho < 1 to keep the static part of a scene (L192) and thresholds rho to tell dynamic
  *            points (L118). beta = +INF counts as rho = +INF; cycle = +INF with finite beta as rho = 0. */
+typedef enum pvg_target {
+  PVG_TARGET_COLOR = 0,   /* out_rgb = C + (1 - O) background, out_depth = sum T a z / sum T a */
+  /* SURVEY 8(f-2), "flexible rendering ... by replacing the color c in Eq. (3)" with the
+   * quantities of the paper's dynamic element analysis (L298): out_rgb = sum T a vbar_cam, the average velocity
+   * vbar = v exp(-rho/2) (Eq. 10) rotated into camera axes (x right, y down, z forward; its x, y components are
+   * the projection onto the plane parallel to the camera plane that the paper colour-codes); out_depth =
+   * sum T a clamp(rho, 0, 2), the staticness map. Plain sums of Eq. 3: no background, no normalisation;
+   * out_alpha = O as always. The record's colour slot holds vbar_cam in this mode. */
+  PVG_TARGET_DYNAMICS = 1
+} pvg_target;
 typedef struct pvg_state {
   float t, dt, rho_min, rho_max;
+  int target; /* pvg_target */
 } pvg_state;
 int pvg_render_state(pvg_scene *scene, const pvg_camera *cam, const pvg_state *state, float *out_rgb,
                      float *out_depth, float *out_alpha);

@@ -192,3 +192,13 @@ def sky_composite(cam, cube, rgb, alpha):
     c = _cam(cam)
     lib().oracle_sky_composite(C.byref(c), _p(cube), C.c_int(res), _p(out), _p(alpha))
     return out
+
+
+def dynamics(scene, cam):
+    """(vbar in camera axes, clamp(rho, 0, 2)) per point: float64 [n, 4] (Eq. 10)."""
+    n = int(scene.mu.shape[0])
+    beta = _f32(scene.beta, (n,)); vel = _f32(scene.vel, (n, 3))
+    out = np.empty((n, 4), dtype=np.float64)
+    c = _cam(cam)
+    lib().oracle_dynamics(C.c_uint64(n), _p(beta), _p(vel), C.c_double(float(scene.cycle)), C.byref(c), _p(out))
+    return out

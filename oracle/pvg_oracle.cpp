@@ -18,7 +18,8 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed forms T1..T8 of the
 // paper, single-Gaussian image, stop/clamp/cutoff rules, brute force == binned,
 // std::stable_sort equivalence on tiny scenes; for oracle_preprocess_state (Eq. 10 / 12,
-// staticness filter) TestTemporalSmoothingState; for the sky cube map (oracle_sky_*) TestSky.
+// staticness filter) TestTemporalSmoothingState; for the sky cube map (oracle_sky_*) TestSky; for
+// oracle_dynamics TestDynamicsTarget.
 // "Absolute values on real data"
 // is parity unpinned (the paper prints no worked numeric example).
 
@@ -576,6 +577,24 @@ void oracle_sky_composite(const Cam* cam, const float* cube, int res, double* rg
       const uint64_t pi = (uint64_t)py * cam->width + px;
       for (int ch = 0; ch < 3; ++ch) rgb[ch * HW + pi] += (1.0 - alpha[pi]) * sky[ch];
     }
+}
+
+// f-2: the per-point quantities of the paper's dynamic element analysis, rendered by "replacing
+// the color c in Eq. (3)": "we first transform vbar ... from the world coordinate system to the
+// camera coordinate system" (L298), vbar = v exp(-rho / 2) (Eq. 10), rho = beta / l (L112); "we need to
+// clamp each point's rho to the range of [0,2] and render" (L298). out[i] = (vbar_cam.x, .y, .z, clamp(rho, 0, 2));
+// a velocity is a direction: only the rotation part of E applies. Rendering them is Oracle-R on a record whose
+// colour slot holds these values, with bg = 0 (the sums of Eq. 3, no normalisation).
+void oracle_dynamics(uint64_t n, const float* beta, const float* vel, double cycle, const Cam* cam, double* out) {
+  const double* R = cam->w2c;
+  for (uint64_t i = 0; i < n; ++i) {
+    const double be = beta[i];
+    const double rho = std::isinf(be) ? std::numeric_limits<double>::infinity() : (std::isinf(cycle) ? 0.0 : be / cycle);
+    const double e = std::exp(-0.5 * rho);
+    const double vb[3] = {vel[i * 3] * e, vel[i * 3 + 1] * e, vel[i * 3 + 2] * e};
+    for (int j = 0; j < 3; ++j) out[i * 4 + j] = R[4 * j] * vb[0] + R[4 * j + 1] * vb[1] + R[4 * j + 2] * vb[2];
+    out[i * 4 + 3] = std::fmin(std::fmax(rho, 0.0), 2.0);
+  }
 }
 
 int oracle_num_threads() {

@@ -50,7 +50,8 @@ class CameraC(C.Structure):
 
 
 class StateC(C.Structure):
-    _fields_ = [("t", C.c_float), ("dt", C.c_float), ("rho_min", C.c_float), ("rho_max", C.c_float)]
+    _fields_ = [("t", C.c_float), ("dt", C.c_float), ("rho_min", C.c_float), ("rho_max", C.c_float),
+                ("target", C.c_int)]
 
 
 class DebugC(C.Structure):
@@ -201,10 +202,11 @@ class Scene:
 
     # -- the path ---------------------------------------------------------------------------
     def render(self, cam, t: float, out: Optional[Tuple] = None, dt: float = 0.0, rho_min: float = 0.0,
-               rho_max: float = float("inf")):
+               rho_max: float = float("inf"), target: str = "color"):
         """Frame at time t into torch CUDA tensors (rgb [3,H,W], depth [H,W], alpha [H,W]).
         dt != 0 renders the temporal-smoothing state H^(t) built from t - dt (Eq. 12); rho_min / rho_max
-        keep only the points whose staticness beta / l lies in [rho_min, rho_max]."""
+        keep only the points whose staticness beta / l lies in [rho_min, rho_max]. target="dynamics": the first
+        tensor holds sum T a vbar (camera axes) and the second sum T a clamp(rho, 0, 2)."""
         import torch
         c = cam if isinstance(cam, CameraC) else camera_struct(cam)
         if out is None:
@@ -212,11 +214,12 @@ class Scene:
                    torch.empty((c.height, c.width), dtype=torch.float32, device="cuda"),
                    torch.empty((c.height, c.width), dtype=torch.float32, device="cuda"))
         _check(self._L.pvg_set_stream(self._h, torch.cuda.current_stream().cuda_stream))
-        if dt == 0.0 and rho_min == 0.0 and rho_max == float("inf"):
+        tg = {"color": 0, "dynamics": 1}[target]
+        if dt == 0.0 and rho_min == 0.0 and rho_max == float("inf") and tg == 0:
             _check(self._L.pvg_render(self._h, C.byref(c), float(t), out[0].data_ptr(), out[1].data_ptr(),
                                       out[2].data_ptr()))
         else:
-            st = StateC(float(t), float(dt), float(rho_min), float(rho_max))
+            st = StateC(float(t), float(dt), float(rho_min), float(rho_max), tg)
             _check(self._L.pvg_render_state(self._h, C.byref(c), C.byref(st), out[0].data_ptr(), out[1].data_ptr(),
                                             out[2].data_ptr()))
         return out

@@ -94,14 +94,18 @@ struct BlendPixel {
 // pixels is alive; the tile retires when every pixel's transmittance has dropped below 1e-4.
 // COUNT = true additionally counts the (pixel, list entry) evaluations reached and the
 // contributing ones into counters[0..1] (measurement only, never on the product path).
-// SKY = true: the background is the cube map f_sky(d) instead of the constant bg (its own instantiation, so
-// that the lookup's registers do not cost the plain kernel occupancy: 69 against 62 registers).
-template <bool COUNT, bool SKY>
+// MODE: BLEND_COLOR -- rgb = C + T bg, depth = D / (1 - T); BLEND_SKY -- the background is the cube map f_sky(d)
+// (its own instantiation, so that the lookup's registers do not cost the plain kernel occupancy);
+// BLEND_FEATURE -- "flexible rendering": the record's colour slot holds another per-Gaussian
+// quantity (here vbar in camera axes) and `featw` a fourth one (clamp(rho, 0, 2)); the outputs are the plain sums
+// sum T alpha f of Eq. 3, without background and without normalisation, in out_rgb and out_depth.
+enum { BLEND_COLOR = 0, BLEND_SKY = 1, BLEND_FEATURE = 2 };
+template <bool COUNT, int MODE>
 __global__ void __launch_bounds__(BLEND_THREADS)
 blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
              const uint32_t* __restrict__ vals, const float4* __restrict__ record,
              float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
-             unsigned long long* __restrict__ counters) {
+             unsigned long long* __restrict__ counters, const float* __restrict__ featw) {
   __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
   __shared__ float4 s_col[BLEND_BATCH];   // c', log2 o~, r, g
   __shared__ float2 s_bz[BLEND_BATCH];    // b, z
@@ -142,7 +146,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
         const float kh = -0.72134752044448170f;  // -log2(e)/2
         s_geo[k] = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
         s_col[k] = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
-        s_bz[k] = make_float2(r2.z, r0.z);
+        s_bz[k] = make_float2(r2.z, MODE == BLEND_FEATURE ? __ldg(featw + g) : r0.z);
       } else {
         // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0
         s_geo[k] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -189,7 +193,8 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
     const float Al = 1.0f - X[k].T;
     if (out_rgb) {
       float bg[3] = {P.bg[0], P.bg[1], P.bg[2]};
-      if (SKY) {
+      if (MODE == BLEND_FEATURE) bg[0] = bg[1] = bg[2] = 0.f;
+      if (MODE == BLEND_SKY) {
         // the pixel-centre ray in world coordinates: R^T ((x - cx) / fx, (y - cy) / fy, 1)
         const float cxr = (pxf + (float)k - P.cx) / P.fx, cyr = (pyf - P.cy) / P.fy;
         sky_sample(P.sky, P.sky_res, fmaf(P.R[0], cxr, fmaf(P.R[3], cyr, P.R[6])),
@@ -199,7 +204,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
       out_rgb[HW + pi + k] = fmaf(X[k].T, bg[1], X[k].Cg);
       out_rgb[2 * HW + pi + k] = fmaf(X[k].T, bg[2], X[k].Cb);
     }
-    if (out_depth) out_depth[pi + k] = Al > 0.f ? X[k].D / Al : 0.f;
+    if (out_depth) out_depth[pi + k] = MODE == BLEND_FEATURE ? X[k].D : (Al > 0.f ? X[k].D / Al : 0.f);
     if (out_alpha) out_alpha[pi + k] = Al;
   }
 }

@@ -30,7 +30,8 @@ namespace pvg {
 //   A2[i] = unit quaternion (w,x,y,z)   A3[i] = (s.x, s.y, s.z, o)
 //   SH[p][i], p = 0..11: floats 4p..4p+3 of the point's [16][3] coefficient block
 // Outputs:
-//   record[3 i + {0,1,2}] = (mx,my,z,o~), (a,b,c,hx), (r,g,b,hy)   -- all 0 if culled
+//   record[3 i + {0,1,2}] = (mx,my,z,o~), (a,b,c,hx), (r,g,b,hy)   -- all 0 if culled; with P.target == 1 the
+//                           colour slot holds vbar in camera axes and featw[i] = clamp(rho, 0, 2)
 //   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
 //   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | fp32 bits of z, or 0xFFFFFFFF if culled), i
@@ -40,7 +41,7 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
                   const float4* __restrict__ A2, const float4* __restrict__ A3,
                   const float4* __restrict__ SH, float4* __restrict__ record,
                   uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
-                  uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals) {
+                  uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, float* __restrict__ featw) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
 
@@ -135,7 +136,21 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
     }
   }
 
-  if (valid) {
+  if (valid && P.target == 1) {
+    // "Flexible rendering ... by replacing the color c in Eq. (3)" with the quantities of the
+    // dynamic element analysis (L298): the average velocity vbar = v exp(-rho/2) (Eq. 10) in camera axes, and the
+    // staticness clamped to [0, 2]. No SH read in this mode.
+    const float e = expf(-0.5f * rho);
+    const float vx = e * a1.x, vy = e * a1.y, vz = e * a1.z;
+    r2 = make_float4(fmaf(P.R[0], vx, fmaf(P.R[1], vy, P.R[2] * vz)), fmaf(P.R[3], vx, fmaf(P.R[4], vy, P.R[5] * vz)),
+                     fmaf(P.R[6], vx, fmaf(P.R[7], vy, P.R[8] * vz)), hy);
+    featw[i] = fminf(fmaxf(rho, 0.f), 2.0f);
+    if (!((fabsf(r2.x) <= 3.0e38f) && (fabsf(r2.y) <= 3.0e38f) && (fabsf(r2.z) <= 3.0e38f))) {
+      valid = false;
+      r0 = make_float4(0.f, 0.f, 0.f, 0.f); r1 = r0; r2 = r0;
+      ti = make_uint4(0u, 0u, 0u, 0u);
+    }
+  } else if (valid) {
     // P11: SH colour; only survivors touch the 192 B of coefficients
     float dx = wx - P.campos[0], dy = wy - P.campos[1], dz = wz - P.campos[2];
     const float inv = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);

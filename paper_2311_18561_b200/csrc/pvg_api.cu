@@ -313,6 +313,7 @@ struct pvg_scene {
   // block-entry workspace (blockbin.cuh)
   Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
   Buf ranges, tilegrid;
+  Buf featw;   // clamp(rho, 0, 2) per Gaussian (dynamics target)
   Buf sky;     // cube map [6][res][res][3] (pvg_set_sky)
   int sky_res = 0;
   Buf img[2];  // render_host device images (double-buffered: the copy of frame k overlaps frame k + 1)
@@ -347,7 +348,7 @@ void release_all(pvg_scene* s) {
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
-                 &s->ranges, &s->tilegrid, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
@@ -444,6 +445,7 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   P->rho_min = state->rho_min;
   P->rho_max = state->rho_max;
   P->filter = (state->rho_min > 0.f || state->rho_max < INFINITY) ? 1 : 0;
+  P->target = state->target;
   P->linear = std::isinf(s->cycle) ? 1 : 0;
   P->inv_l = P->linear ? 0.f : (float)(1.0 / (double)s->cycle);
   P->two_over_l = P->linear ? 0.f : (float)(2.0 / (double)s->cycle);
@@ -576,10 +578,15 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   // a1 preprocess
   uint64_t* dk = s->presort ? s->dkeys[0].as<uint64_t>() : nullptr;
   uint32_t* dv = s->presort ? s->dvals[0].as<uint32_t>() : nullptr;
+  float* featw = nullptr;
+  if (P.target == 1) {
+    TRY(s->featw.reserve((size_t)n * 4, st));
+    featw = s->featw.as<float>();
+  }
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
   preprocess_kernel<<<(n + 255) / 256, 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
                                                       s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
-                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv);
+                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, featw);
   TRY(tm.end(st));
 
   const uint32_t* visit = nullptr;
@@ -720,13 +727,18 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     const uint2* rg = s->ranges.as<uint2>();
     const uint32_t* vl = s->vals[s->sorted_side].as<uint32_t>();
     const float4* rec = s->record.as<float4>();
-    const int variant = (s->count_pairs ? 2 : 0) | (P.sky ? 1 : 0);
-    switch (variant) {
-      case 0: blend_kernel<false, false><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
-      case 1: blend_kernel<false, true><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
-      case 2: blend_kernel<true, false><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
-      default: blend_kernel<true, true><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr); break;
+    const int mode = P.target == 1 ? BLEND_FEATURE : (P.sky ? BLEND_SKY : BLEND_COLOR);
+#define PVG_BLEND(C, M) blend_kernel<C, M><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw)
+    if (s->count_pairs) {
+      if (mode == BLEND_FEATURE) PVG_BLEND(true, BLEND_FEATURE);
+      else if (mode == BLEND_SKY) PVG_BLEND(true, BLEND_SKY);
+      else PVG_BLEND(true, BLEND_COLOR);
+    } else {
+      if (mode == BLEND_FEATURE) PVG_BLEND(false, BLEND_FEATURE);
+      else if (mode == BLEND_SKY) PVG_BLEND(false, BLEND_SKY);
+      else PVG_BLEND(false, BLEND_COLOR);
     }
+#undef PVG_BLEND
   }
   TRY(tm.end(st));
   CU(cudaGetLastError());
@@ -836,7 +848,8 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
 }
 
 static bool state_ok(const pvg_state* st) {
-  return std::isfinite(st->t) && std::isfinite(st->dt) && !(st->rho_min < 0.f) && !(st->rho_max < st->rho_min);
+  return std::isfinite(st->t) && std::isfinite(st->dt) && !(st->rho_min < 0.f) && !(st->rho_max < st->rho_min) &&
+         (st->target == PVG_TARGET_COLOR || st->target == PVG_TARGET_DYNAMICS);
 }
 
 int pvg_render_state(pvg_scene* scene, const pvg_camera* cam, const pvg_state* state, float* out_rgb, float* out_depth,
@@ -847,7 +860,7 @@ int pvg_render_state(pvg_scene* scene, const pvg_camera* cam, const pvg_state* s
 }
 
 int pvg_render(pvg_scene* scene, const pvg_camera* cam, float t, float* out_rgb, float* out_depth, float* out_alpha) {
-  const pvg_state st = {t, 0.f, 0.f, INFINITY};
+  const pvg_state st = {t, 0.f, 0.f, INFINITY, PVG_TARGET_COLOR};
   return pvg_render_state(scene, cam, &st, out_rgb, out_depth, out_alpha);
 }
 
@@ -864,7 +877,7 @@ int pvg_wait_host(pvg_scene* scene) {
 int pvg_render_host_async(pvg_scene* scene, const pvg_camera* cam, float t, float* host_rgb, float* host_depth,
                           float* host_alpha) {
   if (!scene || !cam) return PVG_ERR_NULL;
-  const pvg_state state = {t, 0.f, 0.f, INFINITY};
+  const pvg_state state = {t, 0.f, 0.f, INFINITY, PVG_TARGET_COLOR};
   if (!state_ok(&state)) return PVG_ERR_BAD_STATE;
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
   const size_t HW = (size_t)cam->width * cam->height;

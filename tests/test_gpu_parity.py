@@ -255,6 +255,40 @@ def test_sky_cube_map(cfg, n, cam_i, res):
     assert np.abs(rgb - plain[0]).max() > 1e-3                                # the sky shows through (barely at the dense config 4)
 
 
+@pytest.mark.parametrize("cfg,n,cam_i,kw", [(1, 40_000, 0, {}), (2, 30_000, 0, dict(dt=0.01)), (4, 20_000, 2, dict(rho_max=3.0))])
+def test_dynamics_target(cfg, n, cam_i, kw):
+    """velocity map sum T a vbar_cam and staticness map sum T a clamp(rho, 0, 2)."""
+    wl = make_config(cfg, n=n)
+    cam = wl.cameras[cam_i]
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    color = [x.cpu().numpy() for x in sc.render(cam, 0.25, **kw)]
+    vel, rho, alpha = (x.cpu().numpy() for x in sc.render(cam, 0.25, target="dynamics", **kw))
+    grec = sc.debug(["record"])["record"]
+    sc.close()
+    assert np.array_equal(alpha, color[2])                      # same Gaussians, same opacity image
+    f = oracle.dynamics(wl.scene, cam)
+    valid = grec[:, 3] > 0
+    # (P) the record's colour slot holds vbar in camera axes (fp32 rounding of exp and of the 3x3 product)
+    scale = np.abs(wl.scene.vel).max(1)[valid] + 1e-30
+    assert (np.abs(grec[valid, 8:11] - f[valid, :3]).max(1) / scale).max() <= 1e-6
+    # (R) Oracle-R on the GPU record = Eq. 3 with the colour replaced; budgets from the magnitudes
+    zmax = float(max(grec[:, 2].max(), 1.0))
+    mag = grec.copy()
+    mag[:, 8:11] = np.abs(grec[:, 8:11])
+    bud = oracle.render(mag, cam.width, cam.height, mode="binned")
+    ora = oracle.render(grec, cam.width, cam.height, mode="binned")
+    ora["budget"], ora["cond"] = bud["budget"], bud["cond"]
+    cmax = float(max(1.0, np.abs(grec[:, 8:11]).max()))
+    st = check_images((vel, ora["depth"], alpha), ora, zmax, tol_rgb=2e-4 * cmax, label="velocity map")
+    r2 = grec.copy()
+    r2[:, 8:11] = 0
+    r2[valid, 8] = f[valid, 3]
+    ora2 = oracle.render(r2, cam.width, cam.height, mode="binned")
+    st2 = check_images((np.stack([rho, rho * 0, rho * 0]), ora2["depth"], alpha), ora2, zmax, tol_rgb=4e-4, label="staticness map")
+    assert np.abs(vel).max() > 0.05 and 0.05 < rho.max() <= 2.0 + 1e-5
+    print(st, st2)
+
+
 def test_render_host_matches_render():
     wl = make_config(0)
     cam = wl.cameras[0]

@@ -771,3 +771,45 @@ class TestSky:
             cam = pinhole_camera(64, 48, 50.0, yaw_deg=yaw)
             out = oracle.sky_composite(cam, cube, *zero)
             assert np.all(out[:, 20:28, 28:36] == face + 1), (yaw, out[0, 24, 32])
+
+
+# ----------------------------------------------------------------------------- f-2: velocity / staticness targets
+class TestDynamicsTarget:
+    """vbar = v exp(-rho/2) in camera axes and clamp(rho, 0, 2), rendered by replacing c in Eq. 3."""
+
+    def test_limits_and_clamp(self):                 # T8 (L156) and the [0, 2] clamp (L298)
+        cam = cam_simple()
+        sc = one_scene(mu=[(0, 0, 5)] * 4, vel=[(1.0, -2.0, 0.5)] * 4, beta=[np.inf, 1e-9, 0.1, 0.7])
+        f = oracle.dynamics(sc, cam)
+        assert np.array_equal(f[0], [0, 0, 0, 2.0])                                   # rho = inf: vbar = 0, clamp at 2
+        assert np.allclose(f[1], [1.0, -2.0, 0.5, 0.0], rtol=1e-8, atol=5e-9)         # rho -> 0: vbar = v
+        assert np.allclose(f[2, :3], np.array([1.0, -2.0, 0.5]) * math.exp(-float(np.float32(0.1)) / L / 2), rtol=1e-13)
+        assert f[2, 3] == float(np.float32(0.1)) / L and f[3, 3] == 2.0               # 0.5 inside, 3.5 clamped
+
+    def test_velocity_rotates_but_does_not_translate(self):
+        sc = one_scene(mu=(0, 0, 5), vel=(3.0, 0.0, 0.0), beta=1e-9)
+        # camera yawed +90 deg looks along world +x: a world +x velocity points INTO that camera (+z), no x/y part
+        f = oracle.dynamics(sc, pinhole_camera(64, 48, 50.0, yaw_deg=90.0))[0]
+        assert np.allclose(f[:3], [0.0, 0.0, 3.0], atol=1e-6)
+        cam = cam_simple()
+        moved = cam_simple()
+        moved.world_to_cam = cam.world_to_cam.copy()
+        moved.world_to_cam[[3, 7, 11]] = (5.0, -2.0, 9.0)                             # translation only
+        assert np.array_equal(oracle.dynamics(sc, cam), oracle.dynamics(sc, moved))
+
+    def test_rendering_is_eq3_with_the_colour_replaced(self):
+        """One Gaussian: the velocity image is alpha(x) * vbar_cam, the staticness image alpha(x) * clamp(rho)."""
+        cam = cam_simple(64, 48, 50.0)
+        sc = one_scene(mu=(0.1, 0.05, 3.0), scale=(0.2, 0.1, 0.1), opacity=0.9, vel=(-1.5, 0.25, 2.0), beta=0.06)
+        _, rec = oracle.preprocess_scene(sc, cam, 0.0)
+        f = oracle.dynamics(sc, cam)
+        plain = oracle.render(rec, cam.width, cam.height, mode="brute")              # alpha image of the single Gaussian
+        r = rec.copy()
+        r[:, 8:11] = f[:, :3]
+        vel_img = oracle.render(r, cam.width, cam.height, mode="brute")["rgb"]
+        r[:, 8] = f[:, 3]
+        rho_img = oracle.render(r, cam.width, cam.height, mode="brute")["rgb"][0]
+        a = plain["alpha"]
+        for ch in range(3):
+            assert np.allclose(vel_img[ch], a * float(np.float32(f[0, ch])), rtol=1e-12, atol=1e-15)
+        assert np.allclose(rho_img, a * float(np.float32(f[0, 3])), rtol=1e-12, atol=1e-15) and a.max() > 0.8
