@@ -289,6 +289,21 @@ def test_dynamics_target(cfg, n, cam_i, kw):
     print(st, st2)
 
 
+@pytest.mark.parametrize("w,h,f,mode", [(4112, 48, 300.0, "compact"), (3008, 2992, 1500.0, "compact"), (2048, 2048, 1000.0, "blocks")])
+def test_large_images_pick_the_right_list_builder(w, h, f, mode):
+    """257 tiles on an axis (no 8-bit rectangle in the depth key) and 24 x 24 = 576 blocks (> 256) fall back to the
+    compact-key passes; 16 x 16 = 256 blocks is the largest image of the block path. All bit-exact."""
+    wl = make_config(1, n=30_000)
+    cam = pinhole_camera(w, h, f)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
+    sc.render(cam, 0.5)
+    assert sc.frame_stats()["list_mode"] == mode
+    st = check_integer_chain(sc.debug(), w, h, True)
+    assert st["M"] > 50_000
+    sc.close()
+
+
 def test_render_host_matches_render():
     wl = make_config(0)
     cam = wl.cameras[0]
