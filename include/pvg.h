@@ -173,7 +173,13 @@ typedef enum pvg_option {
    *    bit-identical to those of the 64-bit key sort; the unsorted key list and the per-instance
    *    offsets are not intermediates of this mode (pvg_debug_view produces them on demand).
    * 0: one key per (Gaussian, tile) as above. */
-  PVG_OPT_BLOCK_BINS = 6
+  PVG_OPT_BLOCK_BINS = 6,
+  /* 1 (default): while it stages a batch of its list, the blend drops the entries whose ellipse
+   *    { alpha >= 1/255 } cannot reach any pixel centre of the tile (the lists are built from axis-aligned
+   *    rectangles; a quarter to a half of the entries a tile consumes only cover it with their rectangle).
+   *    Such an entry is rejected at every pixel anyway, so the images are bit-identical; the test is
+   *    conservative by a rounding margin. 0: every listed entry is evaluated at every pixel. */
+  PVG_OPT_BLEND_CULL = 7
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 

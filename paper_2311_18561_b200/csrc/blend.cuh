@@ -17,7 +17,7 @@ constexpr int BLEND_NPX = PVG_BLEND_NPX;                   // horizontally adjac
 constexpr int BLEND_THREADS = PVG_TILE_PIXELS / BLEND_NPX;
 constexpr int BLEND_BATCH = 256;
 constexpr int BLEND_BATCH_FIRST = 64;
-constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH_FIRST
+constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH_FIRST / (BLEND_THREADS / 32)
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -54,6 +54,32 @@ __device__ __forceinline__ void sky_sample(const float* __restrict__ cube, int r
     const float bot = fmaf(fx, __ldg(p11 + ch) - __ldg(p01 + ch), __ldg(p01 + ch));
     out[ch] = fmaf(fy, bot - top, top);
   }
+}
+
+// Can the Gaussian reach alpha >= 1/255 at any pixel centre of the box [x0, x1] x [y0, y1]? Its exponent
+// w(x) = a' dx^2 + b' dx dy + c' dy^2 + L (log2 units; a', c' < 0, concave) is maximised over the box: 0 + L if
+// the centre is inside, else on one of the four edges at the clamped stationary point of the 1-D restriction.
+// Conservative: the margin covers the fp32 rounding of this evaluation and of the per-pixel one (a few ulps
+// of the sum of the term magnitudes, which cancel for needles) and ex2.approx; anything non-finite keeps.
+__device__ __forceinline__ bool blend_reaches_tile(float mx, float my, float a, float b, float c, float L,
+                                                   float x0, float x1, float y0, float y1) {
+  const float dx0 = x0 - mx, dx1 = x1 - mx, dy0 = y0 - my, dy1 = y1 - my;
+  if (dx0 <= 0.f && dx1 >= 0.f && dy0 <= 0.f && dy1 >= 0.f) return true;
+  const float hb_c = -0.5f * b / c, hb_a = -0.5f * b / a;   // stationary dy per dx, dx per dy
+  float best = -3.0e38f;
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const float dx = e ? dx1 : dx0;
+    const float dy = fminf(fmaxf(hb_c * dx, dy0), dy1);
+    best = fmaxf(best, fmaf(fmaf(a, dx, b * dy), dx, (c * dy) * dy));
+    const float ey = e ? dy1 : dy0;
+    const float ex = fminf(fmaxf(hb_a * ey, dx0), dx1);
+    best = fmaxf(best, fmaf(fmaf(a, ex, b * ey), ex, (c * ey) * ey));
+  }
+  const float Dx = fmaxf(fabsf(dx0), fabsf(dx1)), Dy = fmaxf(fabsf(dy0), fabsf(dy1));
+  const float S = fabsf(a) * Dx * Dx + fabsf(b) * Dx * Dy + fabsf(c) * Dy * Dy;
+  const float bound = L + best + fmaf(S, 2e-6f, 1e-3f);
+  return !(bound < -7.994353436858858f);   // log2(1/255); NaN keeps
 }
 
 // Per-pixel compositing state and one front-to-back step. The cutoffs are predicates (selects),
@@ -109,6 +135,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
   __shared__ float4 s_col[BLEND_BATCH];   // c', log2 o~, r, g
   __shared__ float2 s_bz[BLEND_BATCH];    // b, z
+  __shared__ uint32_t s_kept[BLEND_THREADS / 32];
 
   const uint32_t tid = threadIdx.x;
   const uint32_t tile = blockIdx.x;
@@ -130,53 +157,84 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   };
   uint32_t n_eval = 0, n_contrib = 0;
 
+  // The tile's box of pixel centres, for the staging-time test below.
+  const float bx0 = (float)(tx * PVG_TILE) + 0.5f, bx1 = bx0 + (float)(PVG_TILE - 1);
+  const float by0 = (float)(ty * PVG_TILE) + 0.5f, by1 = by0 + (float)(PVG_TILE - 1);
+  const uint32_t lane = tid & 31u, wid = tid >> 5;
+  constexpr uint32_t WARPS = BLEND_THREADS / 32;
+
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
   // saturates, so a fixed 256-entry first batch gathers mostly records that are never used
   uint32_t bs = BLEND_BATCH_FIRST;
   for (uint32_t base = range.x; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
     if (__syncthreads_count(any_alive()) == 0) break;
-    for (uint32_t k = tid; k < bs; k += BLEND_THREADS) {
-      const uint32_t idx = base + k;
+    // Staging. Warp w gathers the w-th segment of the batch and keeps, in order, only the entries whose
+    // ellipse { alpha >= 1/255 } can reach the tile at all: the lists are built from axis-aligned
+    // rectangles (S7), and 26% (config 3) to 48% (config 4) of the entries a tile consumes cover it with
+    // their rectangle only. A dropped entry would have been rejected at every pixel, so the image is
+    // unchanged bit for bit (blend_reaches_tile is conservative by a margin).
+    const uint32_t seg = bs / WARPS, seg0 = wid * seg;
+    uint32_t kept = 0;
+    for (uint32_t r = 0; r < seg; r += 32) {
+      const uint32_t idx = base + seg0 + r + lane;
+      bool keep = false;
+      float4 ge, co;
+      float2 bz;
       if (idx < range.y) {
         const uint32_t g = __ldg(vals + idx);
         const float4 r0 = __ldg(record + 3 * (size_t)g);
         const float4 r1 = __ldg(record + 3 * (size_t)g + 1);
         const float4 r2 = __ldg(record + 3 * (size_t)g + 2);
         const float kh = -0.72134752044448170f;  // -log2(e)/2
-        s_geo[k] = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
-        s_col[k] = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
-        s_bz[k] = make_float2(r2.z, MODE == BLEND_FEATURE ? __ldg(featw + g) : r0.z);
-      } else {
-        // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0
-        s_geo[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-        s_col[k] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
-        s_bz[k] = make_float2(0.f, 0.f);
+        ge = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
+        co = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
+        bz = make_float2(r2.z, MODE == BLEND_FEATURE ? __ldg(featw + g) : r0.z);
+        keep = !P.cull || blend_reaches_tile(ge.x, ge.y, ge.z, ge.w, co.x, co.y, bx0, bx1, by0, by1);
       }
+      const uint32_t m = __ballot_sync(0xffffffffu, keep);
+      if (keep) {
+        const uint32_t slot = seg0 + kept + __popc(m & ((1u << lane) - 1u));
+        s_geo[slot] = ge;
+        s_col[slot] = co;
+        s_bz[slot] = bz;
+      }
+      kept += __popc(m);
     }
+    // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0 (kept < seg leaves room: seg % 4 == 0)
+    if (lane < ((0u - kept) & (BLEND_UNROLL - 1u))) {
+      s_geo[seg0 + kept + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_col[seg0 + kept + lane] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
+      s_bz[seg0 + kept + lane] = make_float2(0.f, 0.f);
+    }
+    if (lane == 0) s_kept[wid] = kept;
     __syncthreads();
-    const uint32_t nb = min(bs, range.y - base);
     if (__any_sync(0xffffffffu, any_alive())) {
-      for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
+      for (uint32_t sg = 0; sg < WARPS; ++sg) {
+        const uint32_t nb = s_kept[sg], j00 = sg * seg;
+        bool stop = false;
+        for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
 #pragma unroll
-        for (int u = 0; u < BLEND_UNROLL; ++u) {
-          const uint32_t j = j0 + u;
-          const float4 ge = s_geo[j];
-          const float4 co = s_col[j];
-          const float2 bz = s_bz[j];
-          // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
-          const float dy = ge.y - pyf;
-          const float q = ge.w * dy;
-          const float rr = fmaf(co.x * dy, dy, co.y);
+          for (int u = 0; u < BLEND_UNROLL; ++u) {
+            const uint32_t j = j00 + j0 + u;
+            const float4 ge = s_geo[j];
+            const float4 co = s_col[j];
+            const float2 bz = s_bz[j];
+            // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
+            const float dy = ge.y - pyf;
+            const float q = ge.w * dy;
+            const float rr = fmaf(co.x * dy, dy, co.y);
 #pragma unroll
-          for (int k = 0; k < BLEND_NPX; ++k) {
-            if (COUNT) n_eval += (j < nb && X[k].alive) ? 1u : 0u;
-            const float dx = ge.x - (pxf + (float)k);
-            const bool used = X[k].step(fmaf(fmaf(ge.z, dx, q), dx, rr), co.y, co.z, co.w, bz.x, bz.y);
-            if (COUNT) n_contrib += used ? 1u : 0u;
+            for (int k = 0; k < BLEND_NPX; ++k) {
+              if (COUNT) n_eval += (j0 + u < nb && X[k].alive) ? 1u : 0u;
+              const float dx = ge.x - (pxf + (float)k);
+              const bool used = X[k].step(fmaf(fmaf(ge.z, dx, q), dx, rr), co.y, co.z, co.w, bz.x, bz.y);
+              if (COUNT) n_contrib += used ? 1u : 0u;
+            }
           }
+          if (!__any_sync(0xffffffffu, any_alive())) { stop = true; break; }
         }
-        if (!__any_sync(0xffffffffu, any_alive())) break;
+        if (stop) break;
       }
     }
   }

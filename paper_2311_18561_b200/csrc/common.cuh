@@ -30,6 +30,7 @@ struct FrameParams {
   float inv_l;        // 1 / l (0 for the linear model): rho = beta / l
   float rho_min, rho_max;  // staticness filter (only when `filter` is set)
   int filter;
+  int cull;           // blend: drop list entries whose ellipse cannot reach the tile (bit-identical images)
   int target;         // 0: colour (SH) + depth; 1: dynamics -- colour := vbar in camera axes, 4th channel := clamp(rho, 0, 2)
   float two_over_l;   // 2 / l           (sinpi argument scale)
   float l_over_2pi;   // l / (2 pi)

@@ -300,7 +300,7 @@ struct pvg_scene {
   int sh_degree = 3;
   cudaStream_t stream = nullptr;
   // options
-  int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1;
+  int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1, blend_cull = 1;
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
   bool block_used = false;    // last frame built the tile lists from 8x8-tile block entries (blockbin.cuh)
   // model (SoA)
@@ -446,6 +446,7 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   P->rho_max = state->rho_max;
   P->filter = (state->rho_min > 0.f || state->rho_max < INFINITY) ? 1 : 0;
   P->target = state->target;
+  P->cull = s->blend_cull;
   P->linear = std::isinf(s->cycle) ? 1 : 0;
   P->inv_l = P->linear ? 0.f : (float)(1.0 / (double)s->cycle);
   P->two_over_l = P->linear ? 0.f : (float)(2.0 / (double)s->cycle);
@@ -837,6 +838,7 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
     case PVG_OPT_KEEP_UNSORTED: scene->keep_unsorted = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_COMPACT_KEYS: scene->compact = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_BLOCK_BINS: scene->block = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_BLEND_CULL: scene->blend_cull = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_COUNT_PAIRS: scene->count_pairs = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_KERNEL_EVENTS:
       scene->timer.enabled = value != 0;

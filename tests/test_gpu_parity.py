@@ -304,6 +304,28 @@ def test_large_images_pick_the_right_list_builder(w, h, f, mode):
     sc.close()
 
 
+@pytest.mark.parametrize("cfg,n,cam_i", [(0, None, 0), (1, None, 0), (2, 200_000, 0), (4, 300_000, 1), (4, 300_000, 4)])
+def test_blend_cull_is_bit_identical(cfg, n, cam_i):
+    """BLEND_CULL drops list entries whose ellipse cannot reach the tile: the images must not change by one bit,
+    while the number of (pixel, entry) evaluations falls."""
+    import torch
+    wl = make_config(cfg, n=n)
+    cam = wl.cameras[cam_i]
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    sc.set_option(pvg.OPT_COUNT_PAIRS, 1)
+    res = {}
+    for cull in (0, 1):
+        sc.set_option(pvg.OPT_BLEND_CULL, cull)
+        img = [x.clone() for x in sc.render(cam, 0.25)]
+        res[cull] = (img, sc.blend_counters())
+    sc.close()
+    for a, b in zip(res[0][0], res[1][0]):
+        assert torch.equal(a, b)
+    (e0, c0), (e1, c1) = res[0][1], res[1][1]
+    assert c0 == c1 and e1 <= e0                      # same contributions, fewer evaluations
+    print(cfg, cam_i, "evaluations", e0, "->", e1, "contributing", c0)
+
+
 def test_render_host_matches_render():
     wl = make_config(0)
     cam = wl.cameras[0]
