@@ -16,7 +16,10 @@ namespace pvg {
 constexpr int BLEND_NPX = PVG_BLEND_NPX;                   // horizontally adjacent pixels per thread (2 or 4)
 constexpr int BLEND_THREADS = PVG_TILE_PIXELS / BLEND_NPX;
 constexpr int BLEND_BATCH = 256;
-constexpr int BLEND_BATCH_FIRST = 64;
+#ifndef PVG_BLEND_FIRST
+#define PVG_BLEND_FIRST 64
+#endif
+constexpr int BLEND_BATCH_FIRST = PVG_BLEND_FIRST;
 constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH_FIRST / (BLEND_THREADS / 32)
 
 __device__ __forceinline__ float ex2_approx(float x) {
