@@ -101,7 +101,10 @@ struct OsLarge { static constexpr int THREADS = PVG_OSL_THREADS, ITEMS = PVG_OSL
 #define PVG_OSS_MINB 2
 #endif
 struct OsSmall { static constexpr int THREADS = PVG_OSS_THREADS, ITEMS = PVG_OSS_ITEMS, MINB = PVG_OSS_MINB; static constexpr bool STREAM = false; };
-constexpr uint64_t OS_SMALL_BELOW = 8u << 20;
+#ifndef PVG_OS_SMALL_BELOW
+#define PVG_OS_SMALL_BELOW (8u << 20)
+#endif
+constexpr uint64_t OS_SMALL_BELOW = PVG_OS_SMALL_BELOW;
 
 // scratch of one sort call
 struct SortScratch {
