@@ -189,21 +189,20 @@ bin_pass_kernel(const uint8_t* __restrict__ bin_in, const uint32_t* __restrict__
   const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
   const uint32_t tid = threadIdx.x;
   const uint32_t wbase = (tid >> 5) * (BP_ITEMS * 32) + (tid & 31u);
-  uint32_t dp[BP_ITEMS], bn[BP_ITEMS], g[BP_ITEMS];
+  uint32_t dp[BP_ITEMS], g[BP_ITEMS];
   uint64_t mk[BP_ITEMS];
 #pragma unroll
   for (int j = 0; j < BP_ITEMS; ++j) {
     const bool ok = wbase + j * 32 < tile_n;
     const uint32_t i = tile_base + wbase + j * 32;
-    bn[j] = ok ? (uint32_t)__ldcs(bin_in + i) : MASK;   // padding ranks last
+    dp[j] = ok ? (uint32_t)__ldcs(bin_in + i) & MASK : MASK;   // block ids < 2^BITS; padding ranks last
     g[j] = ok ? __ldcs(g_in + i) : 0u;
     mk[j] = ok ? __ldcs(mask_in + i) : 0ull;
-    dp[j] = bn[j] & MASK;
   }
   Core::rank(s.core, tile, dp, bin_start, lookback);
 #pragma unroll
   for (int j = 0; j < BP_ITEMS; ++j) {
-    s.bin[dp[j] >> 8] = (uint8_t)bn[j];
+    s.bin[dp[j] >> 8] = (uint8_t)dp[j];   // rank() keeps the digit in the low 8 bits
     s.g[dp[j] >> 8] = g[j];
     s.mask[dp[j] >> 8] = mk[j];
   }

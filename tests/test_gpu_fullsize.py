@@ -43,7 +43,15 @@ def _ranges_from_rects(rects, counts, TX, TY):
 
 
 def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, max_fragile_frac=0.01):
-    rgb, depth, alpha = (x.cpu().numpy() for x in sc.render(cam, t))
+    # the staging-time ellipse cull of the blend must not change one bit of the frame
+    sc.set_option(pvg.OPT_BLEND_CULL, 0)
+    plain = [x.clone() for x in sc.render(cam, t)]
+    sc.set_option(pvg.OPT_BLEND_CULL, 1)
+    out = sc.render(cam, t)
+    import torch
+    assert all(torch.equal(a, b) for a, b in zip(plain, out)), "BLEND_CULL changed the image"
+    del plain
+    rgb, depth, alpha = (x.cpu().numpy() for x in out)
     st = sc.frame_stats()
     assert st["list_mode"] == "blocks"
     d = sc.debug_info()
