@@ -350,6 +350,25 @@ def test_fuzz_resolutions_and_poses_bit_exact():
         check_images((rgb, depth, alpha), ora, float(max(grec[:, 2].max(), 1.0)), label=f"fuzz {it}", max_fragile_frac=1.0)
 
 
+def test_instance_overflow_is_an_error_not_a_crash():
+    """460k Gaussians that each cover all 9600 tiles: M = 4.4e9 >= 2^32 -> PVG_ERR_INSTANCE_OVERFLOW before any
+    instance buffer is sized; the scene stays usable."""
+    n = 460_000
+    rng = np.random.default_rng(3)
+    mu = np.zeros((n, 3), np.float32)
+    mu[:, 2] = rng.uniform(1.0, 2.0, n)
+    sc = one_scene(mu=mu, scale=(40.0, 40.0, 40.0), opacity=0.9)
+    g = pvg.Scene.from_workload_scene(sc)
+    cam = pinhole_camera(1920, 1280, 2000.0)
+    with pytest.raises(pvg.PvgError) as e:
+        g.render(cam, 0.0)
+    assert e.value.code == -5
+    small = pinhole_camera(256, 256, 300.0)            # 256 tiles x 460k = 1.2e8 instances: fine
+    rgb, depth, alpha = g.render(small, 0.0)
+    assert g.frame_stats()["M"] == 256 * n and float(alpha.min()) > 0.98
+    g.close()
+
+
 def test_render_host_matches_render():
     wl = make_config(0)
     cam = wl.cameras[0]
