@@ -26,7 +26,10 @@
 namespace pvg {
 
 constexpr int BB_MAX_BINS = 256;  // one 8-bit digit pass
-constexpr int BB_CHUNK = 512;     // entries per (warp pair) chunk of the count / write walks
+#ifndef PVG_BB_CHUNK
+#define PVG_BB_CHUNK 512
+#endif
+constexpr int BB_CHUNK = PVG_BB_CHUNK;   // entries per (warp pair) chunk of the write walk (tilebin.cuh cuts the lists)
 
 __host__ __device__ inline uint32_t bb_blocks(uint32_t tiles) { return (tiles + 7u) >> 3; }
 
@@ -295,7 +298,7 @@ __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 3
     const uint32_t bit = 1u << l;
 #pragma unroll
     for (int k = 0; k < BB_CHUNK / 64; ++k) {
-      const uint4 q = s_ptr[8 * l + (k ^ (l & 7u))];   // two pointers, broadcast (slot swizzled: conflict-free writes)
+      const uint4 q = s_ptr[(BB_CHUNK / 64) * l + (k ^ (l & (BB_CHUNK / 64 - 1)))];   // two pointers, broadcast (slot swizzled: conflict-free writes)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const int b = 2 * k + h;
@@ -390,7 +393,7 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
 #pragma unroll
     for (int k = 0; k < NB / 2; ++k) {
       const uint64_t a = base + 4ull * pre[2 * k], c = base + 4ull * pre[2 * k + 1];
-      sp[8 * lane + (k ^ (lane & 7u))] = make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)c, (uint32_t)(c >> 32));
+      sp[(NB / 2) * lane + (k ^ (lane & (NB / 2 - 1)))] = make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)c, (uint32_t)(c >> 32));
     }
   }
   __syncwarp();

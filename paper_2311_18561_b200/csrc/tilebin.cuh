@@ -23,7 +23,10 @@ namespace pvg {
 
 constexpr int TG_THREADS = 1024;
 constexpr int TB_MAX_BINS = 256;   // == BB_MAX_BINS (blockbin.cuh)
-constexpr int TB_CHUNK = 512;      // == BB_CHUNK
+#ifndef PVG_BB_CHUNK
+#define PVG_BB_CHUNK 512
+#endif
+constexpr int TB_CHUNK = PVG_BB_CHUNK;   // == BB_CHUNK
 
 // Layout of the global grid buffer: the tile difference array, then the block difference array.
 __host__ __device__ inline int tilegrid_cells(int tiles_x, int tiles_y) { return tilegrid_stride(tiles_x) * (tiles_y + 1); }
