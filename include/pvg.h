@@ -222,6 +222,10 @@ int pvg_stage_times_ms(pvg_scene *scene, float ms[PVG_NUM_STAGES]);
  * or a negative pvg_status. */
 int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stages, float *ms);
 
+/* The same launches as a timeline: start (relative to the first launch of the frame) and duration of each, in
+ * launch order, so that gaps and the overlap of the side stream are visible. Same return convention. */
+int pvg_kernel_timeline_ms(pvg_scene *scene, int cap, const char **names, float *start_ms, float *dur_ms);
+
 /* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y,
  * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries,
  * surviving Gaussians S (PRESORT_DEPTH=1, else 0), reserved}. */

@@ -27,7 +27,7 @@ NUM_STAGES = len(STAGES)
 # every symbol include/pvg.h declares
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
            "pvg_render_host_async", "pvg_wait_host", "pvg_render_state", "pvg_set_sky",
-           "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms",
+           "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms", "pvg_kernel_timeline_ms",
            "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
 
@@ -96,6 +96,8 @@ def load_library(path: Optional[str] = None):
     L.pvg_stage_times_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
     L.pvg_kernel_times_ms.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_int),
                                       C.POINTER(C.c_float)]
+    L.pvg_kernel_timeline_ms.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float),
+                                         C.POINTER(C.c_float)]
     L.pvg_sort_pairs.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                  C.c_void_p]
     L.pvg_frame_stats.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
@@ -285,6 +287,17 @@ class Scene:
         if cnt < 0:
             _check(cnt)
         return [(names[i].decode(), STAGES[stages[i]], float(ms[i])) for i in range(min(cnt, cap))]
+
+    def kernel_timeline_ms(self) -> List[Tuple[str, float, float]]:
+        """(kernel, start relative to the frame's first launch, duration) of the last render, in launch order."""
+        cap = 4096
+        names = (C.c_char_p * cap)()
+        start = (C.c_float * cap)()
+        dur = (C.c_float * cap)()
+        cnt = self._L.pvg_kernel_timeline_ms(self._h, cap, names, start, dur)
+        if cnt < 0:
+            _check(cnt)
+        return [(names[i].decode(), float(start[i]), float(dur[i])) for i in range(min(cnt, cap))]
 
     def frame_stats(self) -> Dict[str, int]:
         """Sizes of the last render (no device work)."""

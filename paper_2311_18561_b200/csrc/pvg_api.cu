@@ -183,21 +183,34 @@ int launch_pass(int bits, const uint64_t* kin, const uint32_t* vin, uint64_t* ko
 
 // Stable LSD sort of n pairs on key bits [begin_bit, end_bit). Buffers ping-pong; *result
 // tells which side (0: a, 1: b) holds the sorted list.
+// Sizes and zeroes the scratch of one sort call (histograms, tickets, look-back words) on stream zs -- the
+// renderer does this on its side stream while preprocess runs, so the memsets are off the critical path.
+int prep_onesweep(uint64_t n, int begin_bit, int end_bit, cudaStream_t alloc_st, cudaStream_t zs, SortScratch& sc,
+                  bool hist_ready) {
+  if (n == 0 || end_bit <= begin_bit) return PVG_OK;
+  const SortPlan plan = make_sort_plan(begin_bit, end_bit);
+  const bool small = n < OS_SMALL_BELOW;
+  const uint64_t tile_sz = small ? OsSmall::THREADS * OsSmall::ITEMS : OsLarge::THREADS * OsLarge::ITEMS;
+  const uint64_t tiles = (n + tile_sz - 1) / tile_sz;
+  TRY(sc.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, alloc_st));
+  TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, alloc_st));
+  TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, alloc_st, 1.25));
+  if (!hist_ready) CU(cudaMemsetAsync(sc.hist.p, 0, (size_t)OS_MAX_PASSES * OS_RADIX * 4, zs));
+  CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, zs));
+  CU(cudaMemsetAsync(sc.lookback.p, 0, (size_t)plan.num_passes * tiles * OS_RADIX * 8, zs));
+  return PVG_OK;
+}
+
 int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, int begin_bit,
                  int end_bit, cudaStream_t st, SortScratch& sc, Timer* tm, int stage, int* result,
-                 bool hist_ready = false) {
+                 bool hist_ready = false, bool scratch_ready = false) {
   *result = 0;
   if (n == 0 || end_bit <= begin_bit) return PVG_OK;
   const SortPlan plan = make_sort_plan(begin_bit, end_bit);
   const bool small = n < OS_SMALL_BELOW;
   const uint64_t tile_sz = small ? OsSmall::THREADS * OsSmall::ITEMS : OsLarge::THREADS * OsLarge::ITEMS;
   const uint64_t tiles = (n + tile_sz - 1) / tile_sz;
-  TRY(sc.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
-  TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
-  TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, st, 1.25));
-  if (!hist_ready) CU(cudaMemsetAsync(sc.hist.p, 0, (size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
-  CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, st));
-  CU(cudaMemsetAsync(sc.lookback.p, 0, (size_t)plan.num_passes * tiles * OS_RADIX * 8, st));
+  if (!scratch_ready) TRY(prep_onesweep(n, begin_bit, end_bit, st, st, sc, hist_ready));
 
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
@@ -327,7 +340,7 @@ struct pvg_scene {
   SortScratch sort_n, sort_m;
   uint64_t* h_total = nullptr;  // pinned
   cudaStream_t side = nullptr;  // tile grid + prefix run here, beside the depth sort
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_start = nullptr, ev_zero = nullptr;
   Timer timer;
   // last frame
   uint64_t M = 0, Mb = 0, survivors = 0;
@@ -358,6 +371,9 @@ void release_all(pvg_scene* s) {
   s->h_total = nullptr;
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
+  if (s->ev_start) cudaEventDestroy(s->ev_start);
+  if (s->ev_zero) cudaEventDestroy(s->ev_zero);
+  s->ev_start = s->ev_zero = nullptr;
   if (s->side) cudaStreamDestroy(s->side);
   if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
   if (s->ev_rendered) cudaEventDestroy(s->ev_rendered);
@@ -418,6 +434,8 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_start, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_zero, cudaEventDisableTiming));
   CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_rendered, cudaEventDisableTiming));
   for (int k = 0; k < 2; ++k) CU(cudaEventCreateWithFlags(&s->ev_copied[k], cudaEventDisableTiming));
@@ -466,16 +484,21 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
 }
 
 // a2 scan of the per-Gaussian item counts in visiting order; the total lands in small @8.
-int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm) {
+int prep_scan(pvg_scene* s, cudaStream_t zs) {
+  const uint32_t scan_tiles = (s->n + SCAN_TILE - 1) / SCAN_TILE;
+  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 8, zs));
+  CU(cudaMemsetAsync(s->small.p, 0, 16, zs));
+  return PVG_OK;
+}
+
+int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm, bool scratch_ready = false) {
   cudaStream_t st = s->stream;
   const uint32_t n = s->n;
   const uint32_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 8, st));
-  CU(cudaMemsetAsync(s->small.p, 0, 16, st));
+  if (!scratch_ready) TRY(prep_scan(s, st));
   uint32_t* ticket = s->small.as<uint32_t>();
   uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
   if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
-  if (blocks) TRY(s->chunk_owner.reserve(((size_t)s->Mb / BE_CHUNK + 2) * 4, st, 1.125));
   if (blocks)
     scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(),
                                                                   visit, out, total, s->scan_status.as<uint64_t>(), ticket,
@@ -504,10 +527,12 @@ int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64
 
 // a2 + a3 (instance part) through 8x8-tile block entries (blockbin.cuh): the sorted value list
 // lands in vals[0]; ranges come from tile_prefix_kernel.
-int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Timer* tm) {
+// Sizes the buffers of the block path from M and Mb and zeroes its tickets and look-back words on stream zs
+// (the side stream, while the depth sort is still running on the main one).
+int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
   cudaStream_t st = s->stream;
-  const uint32_t n = s->n, Mb = (uint32_t)s->Mb;
-  const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  const uint32_t Mb = (uint32_t)s->Mb;
+  const uint32_t nbins = bb_blocks(P.tiles_x) * bb_blocks(P.tiles_y);
   constexpr uint32_t PASS_TILE = BP_THREADS * BP_ITEMS;
   const uint32_t pass_tiles = (Mb + PASS_TILE - 1) / PASS_TILE;
   const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
@@ -520,12 +545,23 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(s->chunk_cnt.reserve((size_t)max_chunks * 64 * 8, st, 1.125));   // look-back words of bin_write
   TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
   TRY(s->sort_m.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
+  TRY(s->chunk_owner.reserve(((size_t)Mb / BE_CHUNK + 2) * 4, st, 1.125));
+  CU(cudaMemsetAsync(s->sort_m.tickets.p, 0, 8, zs));
+  CU(cudaMemsetAsync(s->chunk_cnt.p, 0, (size_t)max_chunks * 64 * 8, zs));
+  CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, zs));
+  return PVG_OK;
+}
+
+// a2 + a3 (instance part) through 8x8-tile block entries (blockbin.cuh), after prep_block_bins: the sorted value
+// list lands in vals[0]; ranges come from tile_prefix_kernel.
+int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Timer* tm) {
+  cudaStream_t st = s->stream;
+  const uint32_t n = s->n, Mb = (uint32_t)s->Mb;
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
   uint32_t* chunk_start = bin_start + 257;
   uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
-  CU(cudaMemsetAsync(ticket, 0, 8, st));
-  CU(cudaMemsetAsync(s->chunk_cnt.p, 0, (size_t)max_chunks * 64 * 8, st));
-  CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, st));
 
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
@@ -579,6 +615,16 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   s->block_used = block;
   s->last_P = P;
 
+  // scratch of the depth sort and of the scan: sized by n, zeroed on the side stream while preprocess runs
+  if (s->presort) {
+    cudaStream_t sd = s->side;
+    CU(cudaEventRecord(s->ev_start, st));
+    CU(cudaStreamWaitEvent(sd, s->ev_start, 0));
+    TRY(prep_onesweep(n, 0, 32, st, sd, s->sort_n, false));
+    TRY(prep_scan(s, sd));
+    CU(cudaEventRecord(s->ev_zero, sd));
+  }
+
   // a1 preprocess
   uint64_t* dk = s->presort ? s->dkeys[0].as<uint64_t>() : nullptr;
   uint32_t* dv = s->presort ? s->dvals[0].as<uint32_t>() : nullptr;
@@ -602,6 +648,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     // instances), on the side stream: they overlap the depth sort, and the host reads M and Mb
     // (they size the frame's buffers) while the depth sort is still running
     cudaStream_t sd = s->side;
+    CU(cudaStreamWaitEvent(st, s->ev_zero, 0));
     CU(cudaEventRecord(s->ev_fork, st));
     CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
     static bool attr_set = false;
@@ -640,7 +687,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     // a3 (n-key part): depth order of the Gaussians
     int side = 0;
     TRY(run_onesweep(n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
-                     s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side));
+                     s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side, false, true));
     s->visit_side = side;
     visit = s->dvals[side].as<uint32_t>();
 
@@ -650,8 +697,14 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     M = s->h_total[0];
     s->Mb = block ? s->h_total[1] : 0;
     s->survivors = s->h_total[2];
+    if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
+    s->M = M;
+    if (block && M > 0) {   // the side stream is idle now: size and zero the block path's scratch beside the depth sort
+      TRY(prep_block_bins(s, P, sd));
+      CU(cudaEventRecord(s->ev_zero, sd));
+    }
     // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
-    TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm));
+    TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm, true));
   } else {
     TRY(run_scan(s, false, s->offsets.as<uint32_t>(), nullptr, &tm));
     CU(cudaMemcpyAsync(s->h_total, s->small.as<unsigned char>() + 8, 8, cudaMemcpyDeviceToHost, st));
@@ -665,6 +718,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   const bool compact = !block && s->presort && s->compact && tile_bits <= 16;
   s->compact_used = compact;
   if (M > 0 && block) {
+    CU(cudaStreamWaitEvent(st, s->ev_zero, 0));
     TRY(run_block_bins(s, P, visit, &tm));
   } else if (M > 0 && compact) {
     for (int k = 0; k < 2; ++k) {
@@ -995,6 +1049,25 @@ int pvg_kernel_times_ms(pvg_scene* s, int cap, const char** names, int* stages, 
     if (ms) ms[i] = v;
   }
   if (s->timer.accumulate) s->timer.reset();
+  return cnt;
+}
+
+int pvg_kernel_timeline_ms(pvg_scene* s, int cap, const char** names, float* start_ms, float* dur_ms) {
+  if (!s) return PVG_ERR_NULL;
+  if (!s->rendered || !s->timer.enabled || s->timer.recs.empty()) return 0;
+  CU(cudaStreamSynchronize(s->stream));
+  if (s->side) CU(cudaStreamSynchronize(s->side));
+  const int cnt = (int)s->timer.recs.size();
+  const cudaEvent_t origin = s->timer.recs[0].e0;
+  for (int i = 0; i < cnt && i < cap; ++i) {
+    const KernelRec& r = s->timer.recs[i];
+    float a = 0.f, d = 0.f;
+    CU(cudaEventElapsedTime(&a, origin, r.e0));
+    CU(cudaEventElapsedTime(&d, r.e0, r.e1));
+    if (names) names[i] = r.name;
+    if (start_ms) start_ms[i] = a;
+    if (dur_ms) dur_ms[i] = d;
+  }
   return cnt;
 }
 
