@@ -78,7 +78,8 @@ constexpr int HIST_ITEMS = 8;
 template <bool AGGREGATE>
 __global__ void __launch_bounds__(HIST_THREADS)
 onesweep_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n, const __grid_constant__ SortPlan plan,
-                          uint32_t* __restrict__ hist /* [passes][256] */) {
+                          uint32_t* __restrict__ hist /* [passes][256]: counts, then exclusive prefixes */,
+                          uint32_t* __restrict__ done /* zeroed: CTAs that have added their counts */) {
   __shared__ uint32_t s_hist[OS_MAX_PASSES * OS_RADIX];
   for (int k = threadIdx.x; k < plan.num_passes * OS_RADIX; k += HIST_THREADS) s_hist[k] = 0;
   __syncthreads();
@@ -112,26 +113,36 @@ onesweep_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n, const _
     const uint32_t v = s_hist[k];
     if (v) atomicAdd(&hist[k], v);
   }
-}
-
-// exclusive scan of each pass's 256-bin histogram (one block per pass, 256 threads)
-__global__ void __launch_bounds__(OS_RADIX)
-onesweep_scan_hist_kernel(uint32_t* __restrict__ hist) {
+  // the last CTA to arrive turns the counts into exclusive prefixes (saves a launch: the scan is 1 KB per pass)
+  __shared__ bool s_last;
   __shared__ uint32_t s_warp[OS_RADIX / 32];
-  uint32_t* h = hist + blockIdx.x * OS_RADIX;
-  const uint32_t v = h[threadIdx.x];
-  uint32_t incl = v;
-  const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
-    if (lane >= d) incl += t;
-  }
-  if (lane == 31) s_warp[warp] = incl;
+  __threadfence();
   __syncthreads();
-  uint32_t wex = 0;
-  for (uint32_t w = 0; w < warp; ++w) wex += s_warp[w];
-  h[threadIdx.x] = wex + incl - v;
+  if (threadIdx.x == 0) s_last = atomicAdd(done, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+  for (int p = 0; p < plan.num_passes; ++p) {
+    uint32_t v = 0, incl = 0;
+    if (threadIdx.x < OS_RADIX) {
+      v = __ldcg(hist + p * OS_RADIX + threadIdx.x);
+      incl = v;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+      }
+      if (lane == 31) s_warp[warp] = incl;
+    }
+    __syncthreads();
+    if (threadIdx.x < OS_RADIX) {
+      uint32_t wex = 0;
+      for (uint32_t w = 0; w < warp; ++w) wex += s_warp[w];
+      hist[p * OS_RADIX + threadIdx.x] = wex + incl - v;
+    }
+    __syncthreads();
+  }
 }
 
 // ---- the ranking core shared by every digit pass ----------------------------------------

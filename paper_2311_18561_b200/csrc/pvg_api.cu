@@ -219,11 +219,9 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   const unsigned hist_grid = (unsigned)std::min<uint64_t>(hist_chunks, (uint64_t)sms * 4);
   if (!hist_ready) {
     if (tm) TRY(tm->begin("onesweep_histogram", stage, st));
-    if (small) onesweep_histogram_kernel<false><<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
-    else onesweep_histogram_kernel<true><<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>());
-    if (tm) TRY(tm->end(st));
-    if (tm) TRY(tm->begin("onesweep_scan_hist", stage, st));
-    onesweep_scan_hist_kernel<<<plan.num_passes, OS_RADIX, 0, st>>>(sc.hist.as<uint32_t>());
+    uint32_t* done = sc.tickets.as<uint32_t>() + (OS_MAX_PASSES - 1);   // last ticket slot: never a pass's (<= 8 passes)
+    if (small) onesweep_histogram_kernel<false><<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>(), done);
+    else onesweep_histogram_kernel<true><<<hist_grid, HIST_THREADS, 0, st>>>(ka, n, plan, sc.hist.as<uint32_t>(), done);
     if (tm) TRY(tm->end(st));
   }
 
