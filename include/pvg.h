@@ -179,7 +179,11 @@ typedef enum pvg_option {
    *    rectangles; a quarter to a half of the entries a tile consumes only cover it with their rectangle).
    *    Such an entry is rejected at every pixel anyway, so the images are bit-identical; the test is
    *    conservative by a rounding margin. 0: every listed entry is evaluated at every pixel. */
-  PVG_OPT_BLEND_CULL = 7
+  PVG_OPT_BLEND_CULL = 7,
+  /* k >= 1 (default 1): with KERNEL_EVENTS on, record the launches of every k-th render only, counted from the
+   *    call that sets this option or KERNEL_EVENTS (renders 0, k, 2k, ...). An event record between two kernels
+   *    costs about 2 us of stream time -- 3.6% of a 1 ms frame with ~16 records -- so a long timed loop samples. */
+  PVG_OPT_EVENT_STRIDE = 8
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 

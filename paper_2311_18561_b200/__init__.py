@@ -20,7 +20,7 @@ PVG_OK = 0
 STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_BAD_CAMERA",
           -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION", -8: "PVG_ERR_BAD_STATE"}
 OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
-OPT_BLEND_CULL = 7
+OPT_BLEND_CULL, OPT_EVENT_STRIDE = 7, 8
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 

@@ -116,6 +116,10 @@ struct SortScratch {
 struct Timer {
   bool enabled = true;
   bool accumulate = false;  // keep the records of every frame until they are read
+  int stride = 1;           // record the launches of every stride-th render only (PVG_OPT_EVENT_STRIDE)
+  uint64_t renders = 0;     // renders since the options were last set
+  bool frame_on = true;     // this render records
+  void next_frame() { frame_on = enabled && (renders++ % (uint64_t)stride == 0); }
   std::vector<KernelRec> recs;     // launches of the current frame
   std::vector<cudaEvent_t> pool;   // reusable events
   size_t used = 0;
@@ -128,19 +132,32 @@ struct Timer {
     *e = pool[used++];
     return PVG_OK;
   }
-  void reset() { recs.clear(); used = 0; }
+  // Back-to-back kernels of one stream share their boundary event (the end of one is the start of the next):
+  // every event record between two kernels costs ~2 us of stream time, 28 records were 5% of a 1 ms frame.
+  // A shared start includes the ~1 us launch gap in the next kernel's time. Anything else enqueued on the
+  // stream (a wait on another stream, a memset, a copy) must call cut() so that it is not billed to a kernel.
+  cudaStream_t chain_stream = nullptr;
+  cudaEvent_t chain_event = nullptr;
+  void cut() { chain_event = nullptr; }
+  void reset() { recs.clear(); used = 0; cut(); }
   int begin(const char* name, int stage, cudaStream_t st) {
-    if (!enabled) return PVG_OK;
+    if (!frame_on) return PVG_OK;
     KernelRec r{name, stage, nullptr, nullptr};
-    TRY(get(&r.e0));
+    if (chain_event && chain_stream == st) {
+      r.e0 = chain_event;
+    } else {
+      TRY(get(&r.e0));
+      CU(cudaEventRecord(r.e0, st));
+    }
     TRY(get(&r.e1));
-    CU(cudaEventRecord(r.e0, st));
     recs.push_back(r);
     return PVG_OK;
   }
   int end(cudaStream_t st) {
-    if (!enabled) return PVG_OK;
+    if (!frame_on) return PVG_OK;
     CU(cudaEventRecord(recs.back().e1, st));
+    chain_stream = st;
+    chain_event = recs.back().e1;
     return PVG_OK;
   }
   void destroy() {
@@ -210,7 +227,10 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   const bool small = n < OS_SMALL_BELOW;
   const uint64_t tile_sz = small ? OsSmall::THREADS * OsSmall::ITEMS : OsLarge::THREADS * OsLarge::ITEMS;
   const uint64_t tiles = (n + tile_sz - 1) / tile_sz;
-  if (!scratch_ready) TRY(prep_onesweep(n, begin_bit, end_bit, st, st, sc, hist_ready));
+  if (!scratch_ready) {
+    TRY(prep_onesweep(n, begin_bit, end_bit, st, st, sc, hist_ready));
+    if (tm) tm->cut();
+  }
 
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
@@ -277,6 +297,7 @@ int run_compact_sort(uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint3
   TRY(sc.lookback.reserve((size_t)plan.num_passes * tiles * OS_RADIX * 8, st, 1.25));
   CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, st));
   CU(cudaMemsetAsync(sc.lookback.p, 0, (size_t)plan.num_passes * tiles * OS_RADIX * 8, st));
+  if (tm) tm->cut();
   uint16_t* tin = t0; uint32_t* vin = v0; uint16_t* tout = t1; uint32_t* vout = v1;
   for (int p = 0; p < plan.num_passes; ++p) {
     const bool last = p == plan.num_passes - 1;
@@ -493,7 +514,10 @@ int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Ti
   cudaStream_t st = s->stream;
   const uint32_t n = s->n;
   const uint32_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-  if (!scratch_ready) TRY(prep_scan(s, st));
+  if (!scratch_ready) {
+    TRY(prep_scan(s, st));
+    if (tm) tm->cut();
+  }
   uint32_t* ticket = s->small.as<uint32_t>();
   uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
   if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
@@ -596,7 +620,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   TRY(fill_frame(s, cam, state, &P));
   cudaStream_t st = s->stream;
   Timer& tm = s->timer;
-  if (!tm.accumulate) tm.reset();
+  tm.next_frame();
+  if (!tm.accumulate) { if (tm.frame_on) tm.reset(); } else tm.cut();
   const uint32_t n = s->n;
   const uint32_t tiles = (uint32_t)P.tiles_x * (uint32_t)P.tiles_y;
   s->tiles_x = P.tiles_x; s->tiles_y = P.tiles_y;
@@ -664,6 +689,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     TRY(s->bin_tables.reserve(4096, st));   // bin_start[257] | chunk_start[257]
     int* grid = s->tilegrid.as<int>();
     CU(cudaMemsetAsync(grid, 0, grid_bytes + 4, sd));
+    tm.cut();
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -681,6 +707,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     TRY(tm.end(sd));
     CU(cudaMemcpyAsync(s->h_total, totals, 24, cudaMemcpyDeviceToHost, sd));
     CU(cudaEventRecord(s->ev_join, sd));
+    tm.cut();
 
     // a3 (n-key part): depth order of the Gaussians
     int side = 0;
@@ -692,6 +719,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     // the one host wait of the frame, hidden behind the depth sort
     CU(cudaEventSynchronize(s->ev_join));
     CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+    tm.cut();
     M = s->h_total[0];
     s->Mb = block ? s->h_total[1] : 0;
     s->survivors = s->h_total[2];
@@ -707,6 +735,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     TRY(run_scan(s, false, s->offsets.as<uint32_t>(), nullptr, &tm));
     CU(cudaMemcpyAsync(s->h_total, s->small.as<unsigned char>() + 8, 8, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));   // index-order path: M is only known after the scan
+    tm.cut();
     M = s->h_total[0];
   }
   if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
@@ -717,6 +746,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   s->compact_used = compact;
   if (M > 0 && block) {
     CU(cudaStreamWaitEvent(st, s->ev_zero, 0));
+    tm.cut();
     TRY(run_block_bins(s, P, visit, &tm));
   } else if (M > 0 && compact) {
     for (int k = 0; k < 2; ++k) {
@@ -733,6 +763,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       TRY(s->vals_unsorted.reserve((size_t)M * 4, st));
       CU(cudaMemcpyAsync(s->tiles16_unsorted.p, s->tiles16[0].p, (size_t)M * 2, cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(s->vals_unsorted.p, s->vals[0].p, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
+      tm.cut();
     }
     int side = 0;
     TRY(run_compact_sort((uint32_t)M, s->tiles16[0].as<uint16_t>(), s->vals[0].as<uint32_t>(),
@@ -754,6 +785,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       TRY(s->vals_unsorted.reserve((size_t)M * 4, st));
       CU(cudaMemcpyAsync(s->keys_unsorted.p, s->keys[0].p, (size_t)M * 8, cudaMemcpyDeviceToDevice, st));
       CU(cudaMemcpyAsync(s->vals_unsorted.p, s->vals[0].p, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
+      tm.cut();
     }
     // a3 (M-instance part)
     int side = 0;
@@ -770,6 +802,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     }
   } else if (!s->presort) {
     CU(cudaMemsetAsync(s->ranges.p, 0, (size_t)tiles * 8, st));
+    tm.cut();
   }
 
   // a5 blend
@@ -779,6 +812,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     if (s->count_pairs) {
       ctr = reinterpret_cast<unsigned long long*>(s->small.as<unsigned char>() + 64);
       CU(cudaMemsetAsync(ctr, 0, 16, st));
+      tm.cut();
     }
     const uint2* rg = s->ranges.as<uint2>();
     const uint32_t* vl = s->vals[s->sorted_side].as<uint32_t>();
@@ -898,7 +932,13 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
     case PVG_OPT_KERNEL_EVENTS:
       scene->timer.enabled = value != 0;
       scene->timer.accumulate = value == 2;
+      scene->timer.renders = 0;
       scene->timer.reset();
+      return PVG_OK;
+    case PVG_OPT_EVENT_STRIDE:
+      if (value < 1 || value > (1 << 20)) return PVG_ERR_BAD_OPTION;
+      scene->timer.stride = (int)value;
+      scene->timer.renders = 0;
       return PVG_OK;
     default: return PVG_ERR_BAD_OPTION;
   }
