@@ -167,8 +167,11 @@ def render(rec, width, height, bg=(0.0, 0.0, 0.0), mode="binned", tiles: Optiona
                         C.c_int({"brute": 0, "binned": 1}[mode]), tl, C.c_uint64(ntl),
                         C.c_int(1 if tie_budget else 0), _p(rgb), _p(depth), _p(alpha), _p(budget),
                         _p(cond), _p(stats))
+    # c_max: the colour scale of budget and cond (largest colour of a non-culled Gaussian or of the background)
+    live = rec[:, 3] > 0
+    c_max = float(max(rec[live, 8:11].max(initial=0.0), float(np.max(bg))))
     return dict(rgb=rgb, depth=depth, alpha=alpha, budget=budget, cond=cond,
-                visited=int(stats[0]), contributed=int(stats[1]))
+                visited=int(stats[0]), contributed=int(stats[1]), c_max=c_max)
 
 
 def sky_sample(cube, d):

@@ -126,11 +126,13 @@ def check_images(gpu, ora, z_max: float, tol_rgb: float = TOL_RGB, with_cond: bo
     depth within 1e-3 relative + budget * z_max / alpha. gpu = (rgb, depth, alpha) float32 arrays."""
     rgb, depth, alpha = (np.asarray(x, dtype=np.float64) for x in gpu)
     allow = ora["budget"] + (ora["cond"] if with_cond else 0.0)
+    # budget and cond are weights (alpha T) times the colour scale c_max; alpha and depth flip by the bare weight
+    allow_w = allow / ora["c_max"] if ora.get("c_max", 0.0) > 0 else allow
     e_rgb = np.abs(rgb - ora["rgb"]).max(0)
     e_alpha = np.abs(alpha - ora["alpha"])
     a = np.maximum(ora["alpha"], 1.0 / 255.0)
     e_depth = np.abs(depth - ora["depth"])
-    depth_tol = TOL_DEPTH_REL * ora["depth"] + (allow + tol_rgb) * z_max / a
+    depth_tol = TOL_DEPTH_REL * ora["depth"] + (np.maximum(allow, allow_w) + tol_rgb) * z_max / a
     clean = ora["budget"] == 0
     stats = dict(label=label,
                  max_rgb_err=float(e_rgb.max()), max_rgb_err_clean=float(e_rgb[clean].max()) if clean.any() else 0.0,
@@ -139,7 +141,7 @@ def check_images(gpu, ora, z_max: float, tol_rgb: float = TOL_RGB, with_cond: bo
                  fragile_pixels=int((~clean).sum()), pixels=int(clean.size),
                  max_cond=float(ora["cond"].max()))
     bad_rgb = e_rgb > tol_rgb + allow
-    bad_alpha = e_alpha > tol_rgb + allow
+    bad_alpha = e_alpha > tol_rgb + np.maximum(allow, allow_w)
     bad_depth = e_depth > depth_tol
     stats["bad_rgb"], stats["bad_alpha"], stats["bad_depth"] = int(bad_rgb.sum()), int(bad_alpha.sum()), int(bad_depth.sum())
     assert not bad_rgb.any(), ("rgb", stats)

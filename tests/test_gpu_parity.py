@@ -277,7 +277,7 @@ def test_dynamics_target(cfg, n, cam_i, kw):
     mag[:, 8:11] = np.abs(grec[:, 8:11])
     bud = oracle.render(mag, cam.width, cam.height, mode="binned")
     ora = oracle.render(grec, cam.width, cam.height, mode="binned")
-    ora["budget"], ora["cond"] = bud["budget"], bud["cond"]
+    ora["budget"], ora["cond"], ora["c_max"] = bud["budget"], bud["cond"], bud["c_max"]
     cmax = float(max(1.0, np.abs(grec[:, 8:11]).max()))
     st = check_images((vel, ora["depth"], alpha), ora, zmax, tol_rgb=2e-4 * cmax, label="velocity map")
     r2 = grec.copy()
