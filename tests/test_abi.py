@@ -56,6 +56,7 @@ int main(void) {
   printf("%zu %zu %zu %zu\n", sizeof(pvg_camera), offsetof(pvg_camera, world_to_cam), offsetof(pvg_camera, znear), offsetof(pvg_camera, bg));
   printf("%zu %zu %zu %zu\n", sizeof(pvg_debug), offsetof(pvg_debug, record), offsetof(pvg_debug, keys_sorted), offsetof(pvg_debug, ranges));
   printf("%d %d\n", PVG_NUM_STAGES, PVG_ERR_BAD_OPTION);
+  printf("%zu %zu %zu %d\n", sizeof(pvg_state), offsetof(pvg_state, rho_max), offsetof(pvg_state, target), PVG_ERR_BAD_STATE);
   return 0;
 }'''
     with tempfile.TemporaryDirectory() as d:
@@ -68,6 +69,8 @@ int main(void) {
     assert rows[1] == [C.sizeof(Cm), Cm.world_to_cam.offset, Cm.znear.offset, Cm.bg.offset]
     assert rows[2] == [C.sizeof(D), D.record.offset, D.keys_sorted.offset, D.ranges.offset]
     assert rows[3] == [pvg.NUM_STAGES, -7]
+    St = pvg.StateC
+    assert rows[4] == [C.sizeof(St), St.rho_max.offset, St.target.offset, -8]
 
 
 def test_argument_validation_without_device(lib):
