@@ -49,6 +49,12 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--presort", type=int, default=1)
     ap.add_argument("--block-bins", type=int, default=1)
+    ap.add_argument("--split", default="frames", choices=["frames", "band"],
+                    help="frames (default, the contract's line): every rank renders its own frames, no collective; "
+                         "band: all ranks render tile-row bands of the SAME frame + one all-gather (strong scaling)")
+    ap.add_argument("--bands", type=int, default=0,
+                    help="with --split band on ONE GPU: time the bands of a K-way split one after another and "
+                         "report the slowest band per frame (what one of K GPUs would compute; no collective)")
     ap.add_argument("--event-stride", type=int, default=5,
                     help="record per-kernel CUDA events on every k-th timed frame (each record costs ~2 us of stream time)")
     return ap.parse_args()
@@ -426,9 +432,79 @@ def run_ours(args):
     dist.shutdown()
 
 
+def run_band_split(args):
+    """Within-frame split; NOT the contract's line (that is run_ours). Every rank holds the
+    scene, renders its band of tile rows of the same frame and the bands are all-gathered, so every rank ends
+    each step with the whole frame. Strong scaling: value = frames/s of the job."""
+    import torch
+    import paper_2311_18561_b200 as pvg
+    from paper_2311_18561_b200 import build as pvg_build, dist
+    from workloads import make_config
+
+    rank, local_rank, ws = dist.init("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the render path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if rank == 0:
+        pvg_build.build()
+    dist.barrier(local_rank)
+    wl = make_config(args.config, args.n)
+    frames = list(wl.frames())
+    sched = [frames[s % len(frames)] for s in range(args.steps)]
+    warm = [frames[s % len(frames)] for s in range(max(args.warmup, 3))]
+    scene = pvg.Scene.from_workload_scene(wl.scene)
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 0)
+    cams = {id(c): pvg.camera_struct(c) for c, _ in frames}
+    out_by_cam = {id(c): (torch.zeros((3, c.height, c.width), device=dev), torch.zeros((c.height, c.width), device=dev),
+                          torch.zeros((c.height, c.width), device=dev)) for c, _ in frames}
+    parts = ws if ws > 1 else max(args.bands, 1)
+
+    def step(cam, t, part):
+        ty = (cam.height + 15) // 16
+        b, e = dist.band_rows(part, parts, ty)
+        if e > b:
+            scene.set_tile_rows(b, e)
+            scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+        if ws > 1:
+            dist.gather_bands(out_by_cam[id(cam)], ty)
+
+    per_band = []
+    for part in ([rank] if ws > 1 else range(parts)):
+        for cam, t in warm:
+            step(cam, t, part)
+        torch.cuda.synchronize()
+        dist.barrier(local_rank)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for cam, t in sched:
+            step(cam, t, part)
+        e1.record()
+        torch.cuda.synchronize()
+        dist.barrier(local_rank)
+        per_band.append(e0.elapsed_time(e1) / 1e3)
+    elapsed_s = dist.max_over_ranks(max(per_band), dev)
+    if rank == 0:
+        c0 = frames[0][0]
+        line = {"metric": METRIC, "value": args.steps / elapsed_s, "unit": UNIT, "n_gpus": ws, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": elapsed_s * 1e3 / args.steps, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": f"config {args.config}", "n_gaussians": wl.scene.n,
+                           "resolution": f"{c0.width}x{c0.height}",
+                           "parallelism": (f"tile-row bands over {ws} ranks + one all-gather of the bands per frame" if ws > 1 else
+                                           f"ONE GPU timing each band of a {parts}-way split in turn; value = slowest band, "
+                                           "no collective (a projection of the per-rank compute, not a multi-GPU result)"),
+                           "band_ms_per_frame": [x * 1e3 / args.steps for x in per_band]}}
+        print(json.dumps(line), flush=True)
+    scene.close()
+    dist.shutdown()
+
+
 if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.split == "band":
+        run_band_split(a)
     else:
         run_ours(a)

@@ -183,7 +183,16 @@ typedef enum pvg_option {
   /* k >= 1 (default 1): with KERNEL_EVENTS on, record the launches of every k-th render only, counted from the
    *    call that sets this option or KERNEL_EVENTS (renders 0, k, 2k, ...). An event record between two kernels
    *    costs about 2 us of stream time -- 3.6% of a 1 ms frame with ~16 records -- so a long timed loop samples. */
-  PVG_OPT_EVENT_STRIDE = 8
+  PVG_OPT_EVENT_STRIDE = 8,
+  /* The band of tile rows [BEGIN, END) a render covers (the within-frame multi-GPU split --
+   *    every GPU holds the scene, preprocesses all N Gaussians but duplicates only into the tiles of its own band,
+   *    and writes only the pixel rows [16*BEGIN, min(16*END, H)) of the output images; the other rows are left
+   *    untouched, so bands rendered one after another into the same images add up to the full frame bit for bit).
+   *    Defaults 0 and 0; END = 0 (or beyond the image) means "to the last tile row". A band that is empty for the
+   *    camera of a render (BEGIN >= its tile rows) makes that render return PVG_ERR_BAD_STATE.
+   *    In a band render the per-Gaussian counts, M and the ranges describe the band's tiles only. */
+  PVG_OPT_TILE_ROW_BEGIN = 9,
+  PVG_OPT_TILE_ROW_END = 10
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 

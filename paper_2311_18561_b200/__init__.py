@@ -21,6 +21,7 @@ STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_
           -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION", -8: "PVG_ERR_BAD_STATE"}
 OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
 OPT_BLEND_CULL, OPT_EVENT_STRIDE = 7, 8
+OPT_TILE_ROW_BEGIN, OPT_TILE_ROW_END = 9, 10
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 
@@ -226,6 +227,12 @@ class Scene:
             _check(self._L.pvg_render_state(self._h, C.byref(c), C.byref(st), out[0].data_ptr(), out[1].data_ptr(),
                                             out[2].data_ptr()))
         return out
+
+    def set_tile_rows(self, begin: int = 0, end: int = 0) -> None:
+        """Restrict the following renders to the tile rows [begin, end) (end = 0: to the last row): only the
+        pixel rows [16 begin, 16 end) of the output images are written (include/pvg.h PVG_OPT_TILE_ROW_BEGIN)."""
+        self.set_option(OPT_TILE_ROW_BEGIN, int(begin))
+        self.set_option(OPT_TILE_ROW_END, int(end))
 
     def render_host(self, cam, t: float, out: Optional[Tuple] = None):
         """Frame at time t into HOST buffers (torch CPU tensors, pinned if allocated here)."""

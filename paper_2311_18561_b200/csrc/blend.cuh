@@ -141,7 +141,7 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   __shared__ uint32_t s_kept[BLEND_THREADS / 32];
 
   const uint32_t tid = threadIdx.x;
-  const uint32_t tile = blockIdx.x;
+  const uint32_t tile = blockIdx.x + (uint32_t)P.band_y0 * (uint32_t)P.tiles_x;   // only the band's tiles are launched
   const uint32_t tx = tile % P.tiles_x, ty = tile / P.tiles_x;
   constexpr uint32_t TPR = PVG_TILE / BLEND_NPX;   // threads per tile row
   const uint32_t px = tx * PVG_TILE + BLEND_NPX * (tid % TPR), py = ty * PVG_TILE + tid / TPR;

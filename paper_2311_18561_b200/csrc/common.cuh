@@ -38,6 +38,7 @@ struct FrameParams {
   int sh_degree;
   int width, height, tiles_x, tiles_y;
   int pack_rect;      // tiles_x, tiles_y <= 256: the depth key carries the tile rectangle in its upper half
+  int band_y0, band_y1;  // tile rows [band_y0, band_y1) this render covers (the whole image: 0, tiles_y)
   float bg[3];
   const float* sky;   // cube map [6][res][res][3] or nullptr: rgb = C + (1 - O) f_sky(d)
   int sky_res;

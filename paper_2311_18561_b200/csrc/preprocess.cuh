@@ -125,7 +125,8 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
       x0 = fminf(fmaxf(x0, -1.0f), TXf); x1 = fminf(fmaxf(x1, -1.0f), TXf);
       y0 = fminf(fmaxf(y0, -1.0f), TYf); y1 = fminf(fmaxf(y1, -1.0f), TYf);
       const int tx0 = max((int)floorf(x0), 0), tx1 = min((int)floorf(x1), P.tiles_x - 1);
-      const int ty0 = max((int)floorf(y0), 0), ty1 = min((int)floorf(y1), P.tiles_y - 1);
+      // the band of tile rows of this render: duplicate into own tiles only
+      const int ty0 = max((int)floorf(y0), P.band_y0), ty1 = min((int)floorf(y1), P.band_y1 - 1);
       valid = (tx0 <= tx1) && (ty0 <= ty1);
       if (valid) {
         const uint32_t w = (uint32_t)(tx1 - tx0 + 1), h = (uint32_t)(ty1 - ty0 + 1);

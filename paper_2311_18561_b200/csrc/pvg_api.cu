@@ -336,6 +336,7 @@ struct pvg_scene {
   cudaStream_t stream = nullptr;
   // options
   int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1, blend_cull = 1;
+  int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
   bool block_used = false;    // last frame built the tile lists from 8x8-tile block entries (blockbin.cuh)
   // model (SoA)
@@ -496,6 +497,9 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   P->tiles_x = (cam->width + PVG_TILE - 1) / PVG_TILE;
   P->tiles_y = (cam->height + PVG_TILE - 1) / PVG_TILE;
   P->pack_rect = (P->tiles_x <= 256 && P->tiles_y <= 256) ? 1 : 0;
+  P->band_y0 = s->band_begin;
+  P->band_y1 = (s->band_end <= 0 || s->band_end > P->tiles_y) ? P->tiles_y : s->band_end;
+  if (P->band_y0 >= P->band_y1) return PVG_ERR_BAD_STATE;
   for (int j = 0; j < 3; ++j) P->bg[j] = cam->bg[j];
   P->sky = s->sky_res > 0 ? s->sky.as<float>() : nullptr;
   P->sky_res = s->sky_res;
@@ -818,7 +822,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     const uint32_t* vl = s->vals[s->sorted_side].as<uint32_t>();
     const float4* rec = s->record.as<float4>();
     const int mode = P.target == 1 ? BLEND_FEATURE : (P.sky ? BLEND_SKY : BLEND_COLOR);
-#define PVG_BLEND(C, M) blend_kernel<C, M><<<tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw)
+    const uint32_t band_tiles = (uint32_t)P.tiles_x * (uint32_t)(P.band_y1 - P.band_y0);
+#define PVG_BLEND(C, M) blend_kernel<C, M><<<band_tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw)
     if (s->count_pairs) {
       if (mode == BLEND_FEATURE) PVG_BLEND(true, BLEND_FEATURE);
       else if (mode == BLEND_SKY) PVG_BLEND(true, BLEND_SKY);
@@ -934,6 +939,14 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
       scene->timer.accumulate = value == 2;
       scene->timer.renders = 0;
       scene->timer.reset();
+      return PVG_OK;
+    case PVG_OPT_TILE_ROW_BEGIN:
+      if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
+      scene->band_begin = (int)value;
+      return PVG_OK;
+    case PVG_OPT_TILE_ROW_END:
+      if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
+      scene->band_end = (int)value;
       return PVG_OK;
     case PVG_OPT_EVENT_STRIDE:
       if (value < 1 || value > (1 << 20)) return PVG_ERR_BAD_OPTION;

@@ -66,3 +66,53 @@ def test_single_process_defaults():
     assert dist.world() == (0, 0, 1)
     assert dist.max_over_ranks(1.5) == 1.5
     assert dist.frame_schedule(0, 1, 3, ["a", "b"]) == ["a", "b", "a"]
+
+
+def test_band_rows_partition():
+    sys.path.insert(0, ROOT)
+    from paper_2311_18561_b200 import dist
+    for ty in (1, 7, 56, 80):
+        for ws in (1, 2, 3, 8, 16):
+            rows = [dist.band_rows(r, ws, ty) for r in range(ws)]
+            assert rows[0][0] == 0 and rows[-1][1] == ty
+            assert all(rows[k][1] == rows[k + 1][0] for k in range(ws - 1))
+            h = [e - b for b, e in rows]
+            assert max(h) - min(h) <= 1 and min(h) >= 0
+
+
+def _band_worker(rank: int, world: int, port: int, H: int, W: int, out_q):
+    import torch
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    from paper_2311_18561_b200 import dist
+    dist.init("gloo")
+    TY = (H + 15) // 16
+    g = torch.Generator().manual_seed(7)
+    full = (torch.rand((3, H, W), generator=g), torch.rand((H, W), generator=g), torch.rand((H, W), generator=g))
+    b, e = dist.band_rows(rank, world, TY)
+    mine = tuple(torch.full_like(x, float("nan")) for x in full)      # only the own band is valid
+    for m, f in zip(mine, full):
+        m[..., b * 16:min(e * 16, H), :] = f[..., b * 16:min(e * 16, H), :]
+    dist.gather_bands(mine, TY)
+    out_q.put((rank, all(torch.equal(m, f) for m, f in zip(mine, full))))
+    dist.barrier()
+    dist.shutdown()
+
+
+def test_gather_bands_world2_ragged_last_row():
+    """Within-frame split: each rank holds its band of a 3-image frame; one all-gather assembles the frame on
+    every rank. H = 886 = 55 tile rows + 6 pixels (the ragged last row of config 4's side cameras); 56 rows
+    over 2 ranks."""
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_band_worker, args=(r, world, port, 886, 96, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(0, True), (1, True)]
