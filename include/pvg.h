@@ -153,9 +153,11 @@ typedef enum pvg_option {
   PVG_OPT_PRESORT_DEPTH = 1,
   /* 1: keep a copy of the unsorted (key,value) list for pvg_debug_view (default 0). */
   PVG_OPT_KEEP_UNSORTED = 2,
-  /* 1 (default): record a CUDA event pair around every kernel of the last render
-   * (pvg_kernel_times_ms, pvg_stage_times_ms). 2: keep the records of EVERY render until
-   * pvg_kernel_times_ms reads (and clears) them. 0: no events. */
+  /* 0 (default): no events. 1: record CUDA events around every kernel of the last render
+   * (pvg_kernel_times_ms, pvg_stage_times_ms; without it they report nothing). 2: keep the records of
+   * EVERY render until pvg_kernel_times_ms reads (and clears) them. A measurement hook: the records cost
+   * ~4% of a 1 ms frame, and far more (measured +34%) in the pvg_render_host_async pipeline, where they
+   * interleave with the image copies. */
   PVG_OPT_KERNEL_EVENTS = 3,
   /* 1: the blend also counts its (pixel, list entry) evaluations (pvg_blend_counters); measurement
    *    only -- the counting variant is a separate kernel instantiation (default 0). */

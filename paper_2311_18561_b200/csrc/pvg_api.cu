@@ -114,7 +114,7 @@ struct SortScratch {
 };
 
 struct Timer {
-  bool enabled = true;
+  bool enabled = false;      // PVG_OPT_KERNEL_EVENTS (default off: a measurement hook)
   bool accumulate = false;  // keep the records of every frame until they are read
   int stride = 1;           // record the launches of every stride-th render only (PVG_OPT_EVENT_STRIDE)
   uint64_t renders = 0;     // renders since the options were last set
@@ -358,7 +358,8 @@ struct pvg_scene {
   bool copy_pending[2] = {false, false};
   int img_next = 0;
   SortScratch sort_n, sort_m;
-  uint64_t* h_total = nullptr;  // pinned
+  uint64_t* h_total = nullptr;  // pinned, mapped
+  uint64_t* d_total = nullptr;  // device alias of h_total (tile_prefix_kernel stores the totals through it)
   cudaStream_t side = nullptr;  // tile grid + prefix run here, beside the depth sort
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_start = nullptr, ev_zero = nullptr;
   Timer timer;
@@ -450,7 +451,8 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   Buf* tmp[] = {&t_mu, &t_quat, &t_scale, &t_op, &t_sh, &t_tau, &t_beta, &t_vel};
   for (Buf* b : tmp) b->release();
   if (rc != PVG_OK) return rc;
-  CU(cudaMallocHost((void**)&s->h_total, 64));
+  CU(cudaHostAlloc((void**)&s->h_total, 64, cudaHostAllocMapped));
+  CU(cudaHostGetDevicePointer((void**)&s->d_total, s->h_total, 0));
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
@@ -707,9 +709,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     tile_prefix_kernel<<<1, TB_THREADS, use_smem ? grid_bytes : 0, sd>>>(
         grid, P.tiles_x, P.tiles_y, use_smem, block ? 1 : 0, make_sort_plan(s->sort_begin, s->sort_end),
         s->ranges.as<uint2>(), s->sort_m.hist.as<uint32_t>(), totals, s->bin_tables.as<uint32_t>(),
-        s->bin_tables.as<uint32_t>() + 257);
+        s->bin_tables.as<uint32_t>() + 257, s->d_total);
     TRY(tm.end(sd));
-    CU(cudaMemcpyAsync(s->h_total, totals, 24, cudaMemcpyDeviceToHost, sd));
     CU(cudaEventRecord(s->ev_join, sd));
     tm.cut();
 

@@ -97,12 +97,14 @@ __device__ __forceinline__ void grid_prefix_2d(int* g, int rows, int cols, int s
 // plan.shift[] are KEY bit positions (tile id sits at bit 32).
 //   ranges[tile]            = [begin, end) of the tile in the sorted list
 //   hist[pass][256]         = exclusive digit histograms of the tile-id passes
-//   totals[0] = M (tile instances), totals[1] = Mb (block entries; with_blocks), totals[2] = S (survivors)
+//   totals[0] = M (tile instances), totals[1] = Mb (block entries; with_blocks), totals[2] = S (survivors);
+//   totals_host[0..2]: the same, in mapped host memory
 //   bin_start[257], chunk_start[257] (with_blocks): see blockbin.cuh
 __global__ void __launch_bounds__(TB_THREADS)
 tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int with_blocks, const __grid_constant__ SortPlan plan,
                    uint2* __restrict__ ranges, uint32_t* __restrict__ hist, uint64_t* __restrict__ totals,
-                   uint32_t* __restrict__ bin_start, uint32_t* __restrict__ chunk_start) {
+                   uint32_t* __restrict__ bin_start, uint32_t* __restrict__ chunk_start,
+                   volatile uint64_t* __restrict__ totals_host) {
   extern __shared__ int s_dyn[];
   __shared__ uint32_t s_hist[OS_MAX_PASSES * OS_RADIX];
   __shared__ uint64_t s_part[TB_THREADS / 32];
@@ -153,7 +155,13 @@ tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int wit
       }
     run += c;
   }
-  if (tid == 0) { totals[0] = all; totals[2] = (uint32_t)grid[cells + bcells]; }
+  // totals_host: the same three words in mapped pinned host memory, stored by this thread block itself -- a
+  // copy-engine readback would queue behind the image copy of the previous frame (pvg_render_host_async)
+  if (tid == 0) {
+    const uint64_t surv = (uint32_t)grid[cells + bcells];
+    totals[0] = all; totals[2] = surv;
+    totals_host[0] = all; totals_host[2] = surv;
+  }
   __syncthreads();
   // exclusive scan of each pass's histogram (256 threads per pass)
   for (int p = 0; p < plan.num_passes; ++p) {
@@ -199,6 +207,7 @@ tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int wit
       bin_start[TB_MAX_BINS] = wa + ia;
       chunk_start[TB_MAX_BINS] = wb + ib;
       totals[1] = wa + ia;
+      totals_host[1] = wa + ia;
     }
   }
 }

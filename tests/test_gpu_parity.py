@@ -406,6 +406,8 @@ def test_repeatable_and_stream():
     cam = wl.cameras[0]
     g = pvg.Scene.from_workload_scene(wl.scene)
     a = [x.clone() for x in g.render(cam, 0.5)]
+    assert g.kernel_times_ms() == [] and g.stage_times_ms()["blend"] == 0.0     # the timing hook is off by default
+    g.set_option(pvg.OPT_KERNEL_EVENTS, 1)
     st = torch.cuda.Stream()
     with torch.cuda.stream(st):
         b = g.render(cam, 0.5)
