@@ -356,6 +356,7 @@ def run_ours(args):
            ("bin_expand", "duplicate"): 13.0 * Mbsum + K * 16.0 * S,
            ("tile_grid", "ranges"): K * 16.0 * N,
            ("bin_pass", "sort"): 25.0 * Mbsum,
+           ("bin_emit", "sort"): 12.0 * Mbsum + K * 16.0 * S,   # fused expand + split: 16 B per survivor read, (u32 g, u64 mask) written
            ("bin_count", "sort"): 8.0 * Mbsum + 256.0 * chunks,
            ("bin_chunk_scan", "sort"): 512.0 * chunks,
            ("bin_write", "sort"): 12.0 * Mbsum + 4.0 * Msum + 256.0 * chunks,

@@ -9,6 +9,9 @@
 //      touches: (block id, Gaussian index, 64-bit mask of the block's tiles it covers);
 //   2. bin_pass: ONE stable onesweep digit pass splits the entries by block id (<= 256 blocks);
 //      inside a block the entries stay in depth order;
+//      (1 and 2 run as ONE kernel, bin_emit_kernel: the CTA that ranks a tile of entries forms them
+//      in registers, so the unsplit entries never exist in HBM; the two-kernel form is kept behind
+//      PVG_BIN_FUSED=0)
 //   (the entries per block, hence bin_start / chunk_start, come from tilebin.cuh's block grid)
 //   3. bin_write: a warp owns (chunk of 512 entries of a block, 32 of the block's tiles). It counts
 //      how many of its entries cover each tile, and a decoupled look-back over the block's earlier
@@ -163,8 +166,13 @@ bin_expand_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets
 }
 
 // ---- 2. stable split of the entries by block id ---------------------------------------------
-constexpr int BP_THREADS = 256;
-constexpr int BP_ITEMS = 16;
+#ifndef PVG_BP_THREADS
+#define PVG_BP_THREADS 512   // cfg 3, fused: 512 x 8 0.128 ms, 256 x 16 0.132, 384 x 8 0.134, 256 x 8 (3 CTAs/SM) 0.143
+#define PVG_BP_ITEMS 8
+#define PVG_BP_MINB 2
+#endif
+constexpr int BP_THREADS = PVG_BP_THREADS;
+constexpr int BP_ITEMS = PVG_BP_ITEMS;   // a multiple of 8
 
 template <int BITS>
 struct BinPassSmem {
@@ -177,7 +185,7 @@ struct BinPassSmem {
 // One onesweep digit pass (RadixCore, decoupled look-back) over (block id; Gaussian, mask).
 // The block id itself is not written: bin_start[] says where each block's entries live.
 template <int BITS>
-__global__ void __launch_bounds__(BP_THREADS, 2)
+__global__ void __launch_bounds__(BP_THREADS, PVG_BP_MINB)
 bin_pass_kernel(const uint8_t* __restrict__ bin_in, const uint32_t* __restrict__ g_in, const uint64_t* __restrict__ mask_in,
                 uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, uint32_t n,
                 const uint32_t* __restrict__ bin_start, uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket) {
@@ -214,6 +222,150 @@ bin_pass_kernel(const uint8_t* __restrict__ bin_in, const uint32_t* __restrict__
     const uint32_t o = s.core.out_base[s.bin[p] & MASK] + p;
     g_out[o] = s.g[p];
     mask_out[o] = s.mask[p];
+  }
+}
+
+// ---- 1 + 2 fused: the entries of a tile are formed in registers and split at once ------------
+// bin_expand writes 13 B per entry only for bin_pass to read them back. Here the CTA that ranks a tile of
+// BP_THREADS * BP_ITEMS entries forms them itself: the owners are staged as in bin_expand_kernel, every
+// thread derives its BP_ITEMS entries (warp-striped, the order RadixCore ranks in), and the staging arrays of
+// the split then reuse the shared memory of the owner table.
+constexpr int BF_TILE = BP_THREADS * BP_ITEMS;
+constexpr int BF_SPAN = BF_TILE + 64;
+
+template <int BITS>
+struct BinEmitSmem {
+  typename RadixCore<BP_THREADS, BP_ITEMS, BITS>::Smem core;
+  uint32_t warp_max[BP_THREADS / 32];
+  uint32_t lo, hi;
+  union {
+    struct {
+      int4 owner[BF_SPAN];
+      alignas(16) uint16_t own[BF_TILE];
+    } a;
+    struct {
+      uint64_t mask[BF_TILE];
+      uint32_t g[BF_TILE];
+      uint8_t bin[BF_TILE];
+    } b;
+  };
+};
+
+template <int BITS>
+__global__ void __launch_bounds__(BP_THREADS, PVG_BP_MINB)
+bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
+                const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x,
+                uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, const uint32_t* __restrict__ bin_start,
+                uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket) {
+  using Core = RadixCore<BP_THREADS, BP_ITEMS, BITS>;
+  constexpr uint32_t MASK = (1u << BITS) - 1u;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  BinEmitSmem<BITS>& s = *reinterpret_cast<BinEmitSmem<BITS>*>(smem_raw);
+
+  const uint32_t tile = Core::take_ticket(s.core, ticket);
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t i0 = tile * BF_TILE;
+  const uint32_t tile_n = min((uint32_t)BF_TILE, Mb - i0);
+  if (tid == 0) {
+    const uint32_t lo = chunk_owner[tile];
+    s.lo = lo;
+    s.hi = (uint64_t)(tile + 1) * BF_TILE < Mb ? chunk_owner[tile + 1] : min(lo + (uint32_t)BF_SPAN, n) - 1u;
+  }
+  constexpr int OV = BP_ITEMS / 8;   // uint4 (8 u16 marks) per thread
+#pragma unroll
+  for (int q = 0; q < OV; ++q) reinterpret_cast<uint4*>(s.a.own)[OV * tid + q] = make_uint4(0u, 0u, 0u, 0u);
+  __syncthreads();
+  const uint32_t r_lo = s.lo, span = s.hi - r_lo + 1u;
+  const uint32_t wbase = warp * (BP_ITEMS * 32) + lane;
+  uint32_t dp[BP_ITEMS], g[BP_ITEMS];
+  uint64_t mk[BP_ITEMS];
+
+  if (span <= BF_SPAN) {
+    for (uint32_t k = tid; k < span; k += BP_THREADS) {
+      const uint32_t r = r_lo + k;
+      const uint64_t key = keys[r];
+      const uint32_t rc = (uint32_t)(key >> 32);   // (x0, y0, x1, y1), 8 bits each
+      const int start = (int)(boffsets[r] - i0);   // negative only for the owner that began before the tile
+      s.a.owner[k] = make_int4(start, (int)visit[r], (int)((rc & 0xFFu) | ((rc & 0xFF00u) << 8)),
+                               (int)(((rc >> 16) & 0xFFu) | ((rc >> 24) << 16)));
+      if ((uint32_t)key != 0xFFFFFFFFu && start < BF_TILE) s.a.own[max(start, 0)] = (uint16_t)k;
+    }
+    __syncthreads();
+    // inclusive max-scan of the marks (slot numbers increase along the tile)
+    uint32_t w16[4 * OV];
+#pragma unroll
+    for (int q = 0; q < OV; ++q) {
+      const uint4 a = reinterpret_cast<uint4*>(s.a.own)[OV * tid + q];
+      w16[4 * q] = a.x; w16[4 * q + 1] = a.y; w16[4 * q + 2] = a.z; w16[4 * q + 3] = a.w;
+    }
+    uint32_t run = 0;
+#pragma unroll
+    for (int q = 0; q < 4 * OV; ++q) run = max(run, max(w16[q] & 0xFFFFu, w16[q] >> 16));
+    uint32_t incl = run;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl = max(incl, v);
+    }
+    if (lane == 31) s.warp_max[warp] = incl;
+    uint32_t carry = __shfl_up_sync(0xffffffffu, incl, 1);
+    if (lane == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t wv = 0; wv < warp; ++wv) carry = max(carry, s.warp_max[wv]);
+#pragma unroll
+    for (int q = 0; q < 4 * OV; ++q) {
+      const uint32_t lo16 = max(carry, w16[q] & 0xFFFFu);
+      const uint32_t hi16 = max(lo16, w16[q] >> 16);
+      carry = hi16;
+      w16[q] = lo16 | (hi16 << 16);
+    }
+#pragma unroll
+    for (int q = 0; q < OV; ++q)
+      reinterpret_cast<uint4*>(s.a.own)[OV * tid + q] = make_uint4(w16[4 * q], w16[4 * q + 1], w16[4 * q + 2], w16[4 * q + 3]);
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < BP_ITEMS; ++j) {
+      const uint32_t p = wbase + j * 32;
+      dp[j] = MASK; g[j] = 0u; mk[j] = 0ull;   // padding ranks last
+      if (p < tile_n) {
+        const int4 o = s.a.owner[s.a.own[p]];
+        bb_entry((uint32_t)o.z, (uint32_t)o.w, (uint32_t)((int)p - o.x), blocks_x, dp[j], mk[j]);
+        g[j] = (uint32_t)o.y;
+      }
+    }
+  } else {
+    // owners without entries inside the tile (never the case in depth order): search per entry
+#pragma unroll
+    for (int j = 0; j < BP_ITEMS; ++j) {
+      const uint32_t p = wbase + j * 32;
+      dp[j] = MASK; g[j] = 0u; mk[j] = 0ull;
+      if (p < tile_n) {
+        uint32_t lo = 0, hi = span;
+        while (hi - lo > 1) {
+          const uint32_t mid = lo + ((hi - lo) >> 1);
+          if (boffsets[r_lo + mid] <= i0 + p) lo = mid; else hi = mid;
+        }
+        const uint32_t r = r_lo + lo;
+        const uint32_t rc = (uint32_t)(keys[r] >> 32);
+        bb_entry((rc & 0xFFu) | ((rc & 0xFF00u) << 8), ((rc >> 16) & 0xFFu) | ((rc >> 24) << 16), i0 + p - boffsets[r],
+                 blocks_x, dp[j], mk[j]);
+        g[j] = visit[r];
+      }
+    }
+  }
+  __syncthreads();   // the owner table is dead: s.b reuses it
+  Core::rank(s.core, tile, dp, bin_start, lookback);
+#pragma unroll
+  for (int j = 0; j < BP_ITEMS; ++j) {
+    s.b.bin[dp[j] >> 8] = (uint8_t)dp[j];   // rank() keeps the digit in the low 8 bits
+    s.b.g[dp[j] >> 8] = g[j];
+    s.b.mask[dp[j] >> 8] = mk[j];
+  }
+  __syncthreads();
+  for (uint32_t p = tid; p < tile_n; p += BP_THREADS) {
+    const uint32_t o = s.core.out_base[s.b.bin[p] & MASK] + p;
+    g_out[o] = s.b.g[p];
+    mask_out[o] = s.b.mask[p];
   }
 }
 

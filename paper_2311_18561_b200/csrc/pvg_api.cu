@@ -508,6 +508,13 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   return PVG_OK;
 }
 
+// PVG_BIN_FUSED=1: bin_emit_kernel forms the entries inside the split (no e_* round trip through HBM);
+// 0: bin_expand_kernel + bin_pass_kernel.
+#ifndef PVG_BIN_FUSED
+#define PVG_BIN_FUSED 1
+#endif
+constexpr uint32_t kOwnerChunk = PVG_BIN_FUSED ? (uint32_t)BF_TILE : (uint32_t)BE_CHUNK;   // granularity of chunk_owner[]
+
 // a2 scan of the per-Gaussian item counts in visiting order; the total lands in small @8.
 int prep_scan(pvg_scene* s, cudaStream_t zs) {
   const uint32_t scan_tiles = (s->n + SCAN_TILE - 1) / SCAN_TILE;
@@ -530,7 +537,7 @@ int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Ti
   if (blocks)
     scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(),
                                                                   visit, out, total, s->scan_status.as<uint64_t>(), ticket,
-                                                                  s->chunk_owner.as<uint32_t>(), (uint32_t)BE_CHUNK);
+                                                                  s->chunk_owner.as<uint32_t>(), kOwnerChunk);
   else
     scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), nullptr, visit, out, total,
                                                                    s->scan_status.as<uint64_t>(), ticket, nullptr, 0u);
@@ -553,6 +560,21 @@ int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64
   return PVG_OK;
 }
 
+template <int BITS>
+int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t blocks_x, const uint32_t* bin_start,
+                    uint64_t* lookback, uint32_t* ticket) {
+  auto kern = bin_emit_kernel<BITS>;
+  static bool configured = false;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BinEmitSmem<BITS>)));
+    configured = true;
+  }
+  kern<<<(Mb + BF_TILE - 1) / BF_TILE, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
+      s->n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
+      blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket);
+  return PVG_OK;
+}
+
 // a2 + a3 (instance part) through 8x8-tile block entries (blockbin.cuh): the sorted value list
 // lands in vals[0]; ranges come from tile_prefix_kernel.
 // Sizes the buffers of the block path from M and Mb and zeroes its tickets and look-back words on stream zs
@@ -565,15 +587,17 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
   const uint32_t pass_tiles = (Mb + PASS_TILE - 1) / PASS_TILE;
   const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
   TRY(s->vals[0].reserve((size_t)s->M * 4, st, 1.125));
-  TRY(s->e_bin.reserve((size_t)Mb + 16, st, 1.125));
-  TRY(s->e_g.reserve((size_t)Mb * 4, st, 1.125));
-  TRY(s->e_mask.reserve((size_t)Mb * 8, st, 1.125));
+  if (!PVG_BIN_FUSED) {
+    TRY(s->e_bin.reserve((size_t)Mb + 16, st, 1.125));
+    TRY(s->e_g.reserve((size_t)Mb * 4, st, 1.125));
+    TRY(s->e_mask.reserve((size_t)Mb * 8, st, 1.125));
+  }
   TRY(s->s_g.reserve((size_t)Mb * 4, st, 1.125));
   TRY(s->s_mask.reserve((size_t)Mb * 8, st, 1.125));
   TRY(s->chunk_cnt.reserve((size_t)max_chunks * 64 * 8, st, 1.125));   // look-back words of bin_write
   TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
   TRY(s->sort_m.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
-  TRY(s->chunk_owner.reserve(((size_t)Mb / BE_CHUNK + 2) * 4, st, 1.125));
+  TRY(s->chunk_owner.reserve(((size_t)Mb / kOwnerChunk + 2) * 4, st, 1.125));
   CU(cudaMemsetAsync(s->sort_m.tickets.p, 0, 8, zs));
   CU(cudaMemsetAsync(s->chunk_cnt.p, 0, (size_t)max_chunks * 64 * 8, zs));
   CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, zs));
@@ -591,6 +615,19 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   uint32_t* chunk_start = bin_start + 257;
   uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
 
+  int rc = PVG_ERR_BAD_OPTION;
+  const int bits = std::max(1, ceil_log2(nbins));
+#if PVG_BIN_FUSED
+  TRY(tm->begin("bin_emit", PVG_STAGE_SORT, st));
+  switch (bits) {
+#define PVG_CASE(B) case B: rc = launch_bin_emit<B>(s, Mb, visit, blocks_x, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket); break;
+    PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
+#undef PVG_CASE
+    default: break;
+  }
+  TRY(rc);
+  TRY(tm->end(st));
+#else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
       n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x,
@@ -599,8 +636,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(tm->end(st));
 
   TRY(tm->begin("bin_pass", PVG_STAGE_SORT, st));
-  int rc = PVG_ERR_BAD_OPTION;
-  switch (std::max(1, ceil_log2(nbins))) {
+  switch (bits) {
 #define PVG_CASE(B) case B: rc = launch_bin_pass<B>(s, Mb, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket); break;
     PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
 #undef PVG_CASE
@@ -608,6 +644,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   }
   TRY(rc);
   TRY(tm->end(st));
+#endif
 
   const unsigned walk_grid = (max_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
