@@ -608,7 +608,7 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
 // list lands in vals[0]; ranges come from tile_prefix_kernel.
 int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Timer* tm) {
   cudaStream_t st = s->stream;
-  const uint32_t n = s->n, Mb = (uint32_t)s->Mb;
+  const uint32_t Mb = (uint32_t)s->Mb;
   const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
   const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
@@ -630,7 +630,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
-      n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x,
+      s->n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x,
       s->e_bin.as<uint8_t>(),
       s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>());
   TRY(tm->end(st));
