@@ -7,8 +7,12 @@
 
 namespace pvg {
 
-constexpr int SCAN_THREADS = 512;
-constexpr int SCAN_ITEMS = 8;
+#ifndef PVG_SCAN_THREADS
+#define PVG_SCAN_THREADS 512
+#define PVG_SCAN_ITEMS 8
+#endif
+constexpr int SCAN_THREADS = PVG_SCAN_THREADS;
+constexpr int SCAN_ITEMS = PVG_SCAN_ITEMS;   // a multiple of 4 (128-bit loads and stores)
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 
 // blocks of 8 x 8 tiles touched by the rectangle packed in the upper half of a sorted depth key
@@ -51,13 +55,24 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
 
   uint32_t c[SCAN_ITEMS];
   uint32_t tsum = 0;
+  const bool whole = base + SCAN_ITEMS <= n;   // this thread's items are all inside: 128-bit accesses
+  if (BLOCKS && whole) {
 #pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) {
-    const uint32_t r = base + k;
-    c[k] = 0;
-    if (r < n) c[k] = BLOCKS ? scan_block_count(keys[r]) : counts[visit ? visit[r] : r];
-    tsum += c[k];  // < 2^32: one Gaussian covers at most 2^22 tiles, 8 of them 2^25
+    for (int k = 0; k < SCAN_ITEMS; k += 2) {
+      const ulonglong2 kk = *reinterpret_cast<const ulonglong2*>(keys + base + k);
+      c[k] = scan_block_count(kk.x);
+      c[k + 1] = scan_block_count(kk.y);
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+      const uint32_t r = base + k;
+      c[k] = 0;
+      if (r < n) c[k] = BLOCKS ? scan_block_count(keys[r]) : counts[visit ? visit[r] : r];
+    }
   }
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) tsum += c[k];  // < 2^32: one Gaussian covers at most 2^22 tiles, 8 of them 2^25
   // warp inclusive scan of the thread sums
   const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
   uint64_t incl = tsum;
@@ -108,11 +123,20 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
   }
   __syncthreads();
   uint64_t run = s_prefix + warp_excl + (incl - tsum);
+  if (whole) {
+    uint32_t o = (uint32_t)run;   // valid when M < 2^32 (checked on the host)
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; k += 4) {
+      const uint4 v = make_uint4(o, o + c[k], o + c[k] + c[k + 1], o + c[k] + c[k + 1] + c[k + 2]);
+      *reinterpret_cast<uint4*>(offsets + base + k) = v;
+      o = v.w + c[k + 3];
+    }
+  }
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k) {
     const uint32_t r = base + k;
     if (r < n) {
-      offsets[r] = (uint32_t)run;  // valid when M < 2^32 (checked on the host)
+      if (!whole) offsets[r] = (uint32_t)run;
       if (BLOCKS && chunk_owner && c[k]) {
         const uint64_t first = (run + chunk - 1) / chunk;   // first chunk boundary at or after my first item
         if (first * chunk < run + c[k]) chunk_owner[first] = r;   // c[k] <= 256 < chunk: at most one boundary
