@@ -35,15 +35,14 @@ namespace pvg {
 //   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
 //   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | fp32 bits of z, or 0xFFFFFFFF if culled), i
-__global__ void __launch_bounds__(256)
-preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
-                  const float4* __restrict__ A0, const float4* __restrict__ A1,
-                  const float4* __restrict__ A2, const float4* __restrict__ A3,
-                  const float4* __restrict__ SH, float4* __restrict__ record,
-                  uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
-                  uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, float* __restrict__ featw) {
-  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+// Returns the low half of the depth-sort key: the fp32 bits of z, 0xFFFFFFFF if culled.
+__device__ __forceinline__ uint32_t
+preprocess_point(const FrameParams& P, uint32_t n, uint32_t i,
+                 const float4* __restrict__ A0, const float4* __restrict__ A1,
+                 const float4* __restrict__ A2, const float4* __restrict__ A3,
+                 const float4* __restrict__ SH, float4* __restrict__ record,
+                 uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
+                 uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, float* __restrict__ featw) {
 
   const float4 a0 = ldg_stream_f4(A0 + i);
   const float4 a1 = ldg_stream_f4(A1 + i);
@@ -210,6 +209,72 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
     }
     dkeys[i] = valid ? (((uint64_t)rect << 32) | ti.z) : 0xFFFFFFFFull;
     dvals[i] = i;
+  }
+  return valid ? ti.z : 0xFFFFFFFFu;
+}
+
+// PRE_CHUNKS consecutive groups of 256 Gaussians per CTA. With dhist != nullptr the CTA also counts the four
+// 8-bit digits of its depth keys in shared memory, adds them to dhist[4][256] (zeroed) and the last CTA to
+// finish (dhist[1024] counts them) turns the counts into the exclusive prefixes the onesweep passes of the
+// depth sort start from -- the keys are in registers here; a histogram kernel would read them back from HBM.
+#ifndef PVG_PRE_CHUNKS
+#define PVG_PRE_CHUNKS 4
+#endif
+constexpr int PRE_CHUNKS = PVG_PRE_CHUNKS;
+__global__ void __launch_bounds__(256)
+preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
+                  const float4* __restrict__ A0, const float4* __restrict__ A1,
+                  const float4* __restrict__ A2, const float4* __restrict__ A3,
+                  const float4* __restrict__ SH, float4* __restrict__ record,
+                  uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
+                  uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, float* __restrict__ featw,
+                  uint32_t* __restrict__ dhist) {
+  __shared__ uint32_t s_hist[4 * 256];
+  if (dhist) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s_hist[k * 256 + threadIdx.x] = 0;
+    __syncthreads();
+  }
+#pragma unroll 1
+  for (int c = 0; c < PRE_CHUNKS; ++c) {
+    const uint32_t i = (blockIdx.x * PRE_CHUNKS + c) * 256u + threadIdx.x;
+    if (i >= n) break;
+    const uint32_t z = preprocess_point(P, n, i, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
+    if (dhist) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) atomicAdd(&s_hist[k * 256 + ((z >> (8 * k)) & 0xFFu)], 1u);
+    }
+  }
+  if (!dhist) return;
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint32_t v = s_hist[k * 256 + threadIdx.x];
+    if (v) atomicAdd(&dhist[k * 256 + threadIdx.x], v);
+  }
+  __shared__ bool s_last;
+  __shared__ uint32_t s_warp[8];
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = atomicAdd(dhist + 1024, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  for (int k = 0; k < 4; ++k) {
+    const uint32_t v = __ldcg(dhist + k * 256 + threadIdx.x);
+    uint32_t incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    uint32_t wex = 0;
+    for (uint32_t w = 0; w < warp; ++w) wex += s_warp[w];
+    dhist[k * 256 + threadIdx.x] = wex + incl - v;
+    __syncthreads();
   }
 }
 

@@ -107,6 +107,8 @@ struct OsSmall { static constexpr int THREADS = PVG_OSS_THREADS, ITEMS = PVG_OSS
 constexpr uint64_t OS_SMALL_BELOW = PVG_OS_SMALL_BELOW;
 
 // scratch of one sort call
+constexpr size_t kDhistWords = 1032;   // 4 x 256 counts + the CTA counter, padded to 16 B
+
 struct SortScratch {
   Buf hist;      // [passes][256] u32
   Buf lookback;  // [passes][tiles][256] u64
@@ -220,7 +222,7 @@ int prep_onesweep(uint64_t n, int begin_bit, int end_bit, cudaStream_t alloc_st,
 
 int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, int begin_bit,
                  int end_bit, cudaStream_t st, SortScratch& sc, Timer* tm, int stage, int* result,
-                 bool hist_ready = false, bool scratch_ready = false) {
+                 bool hist_ready = false, bool scratch_ready = false, const uint32_t* hist_at = nullptr) {
   *result = 0;
   if (n == 0 || end_bit <= begin_bit) return PVG_OK;
   const SortPlan plan = make_sort_plan(begin_bit, end_bit);
@@ -248,7 +250,7 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
   uint64_t* kin = ka; uint32_t* vin = va; uint64_t* kout = kb; uint32_t* vout = vb;
   for (int p = 0; p < plan.num_passes; ++p) {
     if (tm) TRY(tm->begin("onesweep_pass", stage, st));
-    const uint32_t* hist = sc.hist.as<uint32_t>() + p * OS_RADIX;
+    const uint32_t* hist = (hist_at ? hist_at : sc.hist.as<uint32_t>()) + p * OS_RADIX;
     uint64_t* lb = sc.lookback.as<uint64_t>() + (size_t)p * tiles * OS_RADIX;
     uint32_t* tk = sc.tickets.as<uint32_t>() + p;
     if (small) TRY(launch_pass<OsSmall>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st));
@@ -348,6 +350,8 @@ struct pvg_scene {
   Buf tiles16[2], tiles16_unsorted;
   // block-entry workspace (blockbin.cuh)
   Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
+  Buf dhist;          // 2 x (4 x 256 digit counts + 1 CTA counter) u32: the depth histogram preprocess accumulates, double-buffered
+  int dhist_side = 0;
   Buf ranges, tilegrid;
   Buf featw;   // clamp(rho, 0, 2) per Gaussian (dynamics target)
   Buf sky;     // cube map [6][res][res][3] (pvg_set_sky)
@@ -384,7 +388,7 @@ void release_all(pvg_scene* s) {
   Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
-                 &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
+                 &s->dhist, &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
                  &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
@@ -436,6 +440,8 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4); rs(s->boffsets, n * 4);
   rs(s->dkeys[0], n * 8); rs(s->dkeys[1], n * 8); rs(s->dvals[0], n * 4); rs(s->dvals[1], n * 4);
   rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 8); rs(s->small, 256);
+  rs(s->dhist, 2 * kDhistWords * 4);
+  if (rc == PVG_OK && cudaMemsetAsync(s->dhist.p, 0, 2 * kDhistWords * 4, st) != cudaSuccess) rc = PVG_ERR_CUDA;
   if (rc == PVG_OK) {
     relayout_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
         (uint32_t)n, t_mu.as<float>(), t_quat.as<float>(), t_scale.as<float>(), t_op.as<float>(), t_sh.as<float>(),
@@ -684,9 +690,14 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   // scratch of the depth sort and of the scan: sized by n, zeroed on the side stream while preprocess runs
   if (s->presort) {
     cudaStream_t sd = s->side;
+    CU(cudaStreamWaitEvent(st, s->ev_zero, 0));   // normally long past; matters only after a frame that stopped early
     CU(cudaEventRecord(s->ev_start, st));
     CU(cudaStreamWaitEvent(sd, s->ev_start, 0));
-    TRY(prep_onesweep(n, 0, 32, st, sd, s->sort_n, false));
+    TRY(prep_onesweep(n, 0, 32, st, sd, s->sort_n, true));
+    // the depth histogram is accumulated by preprocess into one half of dhist; the other half is zeroed here for
+    // the next frame (its last readers, the previous frame's passes, are behind ev_start)
+    s->dhist_side ^= 1;
+    CU(cudaMemsetAsync(s->dhist.as<uint32_t>() + (s->dhist_side ^ 1) * kDhistWords, 0, kDhistWords * 4, sd));
     TRY(prep_scan(s, sd));
     CU(cudaEventRecord(s->ev_zero, sd));
   }
@@ -700,9 +711,10 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     featw = s->featw.as<float>();
   }
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
-  preprocess_kernel<<<(n + 255) / 256, 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
+  preprocess_kernel<<<(n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS), 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
                                                       s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
-                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, featw);
+                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, featw,
+                                                      s->presort ? s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords : nullptr);
   TRY(tm.end(st));
 
   const uint32_t* visit = nullptr;
@@ -754,7 +766,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     // a3 (n-key part): depth order of the Gaussians
     int side = 0;
     TRY(run_onesweep(n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
-                     s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side, false, true));
+                     s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side, true, true,
+                     s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords));
     s->visit_side = side;
     visit = s->dvals[side].as<uint32_t>();
 
