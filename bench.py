@@ -47,6 +47,7 @@ def parse_args():
     ap.add_argument("--n", type=int, default=None, help="override the point count (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-pipelined", action="store_true")
     ap.add_argument("--presort", type=int, default=1)
     ap.add_argument("--block-bins", type=int, default=1)
     ap.add_argument("--split", default="frames", choices=["frames", "band"],
@@ -298,34 +299,71 @@ def run_ours(args):
         pairs_contrib += b
     scene.set_option(pvg.OPT_COUNT_PAIRS, 0)
 
+    # ---- two frames in flight: the same K frames through the scene and a fork of it (shared model), on two streams
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 0)      # the per-kernel timing hook is a measurement aid, not the user's call
+    handles = [scene, scene.fork()]
+    lanes = [torch.cuda.Stream(), torch.cuda.Stream()]
+    out2 = [out_by_cam, {k: outs(c) for k, c in {id(c): c for c, _ in frames}.items()}]
+    cur = torch.cuda.current_stream()
+
+    def in_flight(seq):
+        for i, (cam, t) in enumerate(seq):
+            with torch.cuda.stream(lanes[i % 2]):
+                handles[i % 2].render(cams[id(cam)], t, out2[i % 2][id(cam)])
+
+    pipelined = None
+    if not args.no_pipelined:
+        in_flight(warm[:4])
+        torch.cuda.synchronize()
+        dist.barrier(local_rank)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record()
+        for ln in lanes:
+            ln.wait_stream(cur)
+        in_flight(sched)
+        for ln in lanes:
+            cur.wait_stream(ln)
+        p1.record()
+        torch.cuda.synchronize()
+        dist.barrier(local_rank)
+        pel = dist.max_over_ranks(p0.elapsed_time(p1) / 1e3, dev)
+        pipelined = {"value": total_frames / pel, "unit": UNIT, "frames_in_flight": 2, "ms_per_step": pel * 1e3 / args.steps,
+                     "note": "the same K frames, alternately through the scene and a pvg_fork_scene of it (shared model, two "
+                             "workspaces) on two streams; `value`, the per-kernel times and the roofline above are one frame at a time"}
+
     # ---- end to end through the C ABI with HOST buffers (D2H of the images inside the timed region)
     e2e = None
     if not args.no_e2e:
         def pinned(v):
             return (torch.empty(v[0].shape, pin_memory=True), torch.empty(v[1].shape, pin_memory=True),
                     torch.empty(v[2].shape, pin_memory=True))
-        # two host image sets per camera: frame k is copied out while frame k + 1 renders
-        host = {k: (pinned(v), pinned(v)) for k, v in out_by_cam.items()}
-        scene.set_option(pvg.OPT_KERNEL_EVENTS, 0)      # the per-kernel timing hook is a measurement aid, not the user's call
-        for i, (cam, t) in enumerate(warm[:2]):
-            scene.render_host_async(cams[id(cam)], t, host[id(cam)][i % 2])
-        scene.wait_host()
+        # two frames in flight (scene + fork), two host image sets per handle and camera: frame k is copied out while
+        # the next frames render
+        host = [{k: (pinned(v), pinned(v)) for k, v in out_by_cam.items()} for _ in handles]
+
+        def e2e_loop(seq):
+            for i, (cam, t) in enumerate(seq):
+                with torch.cuda.stream(lanes[i % 2]):
+                    handles[i % 2].render_host_async(cams[id(cam)], t, host[i % 2][id(cam)][(i // 2) % 2])
+            for h in handles:
+                h.wait_host()
+
+        e2e_loop(warm[:4])
         dist.barrier(local_rank)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        d2h = 0
-        for i, (cam, t) in enumerate(sched):
-            scene.render_host_async(cams[id(cam)], t, host[id(cam)][i % 2])
-            d2h += cam.width * cam.height * 5 * 4
-        scene.wait_host()
+        e2e_loop(sched)
         torch.cuda.synchronize()
         el = dist.max_over_ranks(time.perf_counter() - t0, dev)
         dist.barrier(local_rank)
-        scene.set_option(pvg.OPT_KERNEL_EVENTS, 1)
+        d2h = sum(cam.width * cam.height * 5 * 4 for cam, _ in sched)
         e2e = {"value": total_frames / el, "unit": UNIT,
                "h2d_bytes_per_step": int(pvg.C.sizeof(pvg.CameraC) + 4), "d2h_bytes_per_step": int(d2h // len(sched)),
-               "note": "pvg_render_host_async + pvg_wait_host: per-step input is (camera, t); every frame's rgb+depth+alpha is copied "
-                       "to pinned host memory inside the timed region, the copy of frame k overlapping the render of frame k+1"}
+               "note": "pvg_render_host_async + pvg_wait_host, two frames in flight (scene + pvg_fork_scene): per-step input is "
+                       "(camera, t); every frame's rgb+depth+alpha is copied to pinned host memory inside the timed region, the "
+                       "copies overlapping the following renders"}
+    handles[1].close()
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 1)
 
     if rank != 0:
         scene.close()
@@ -427,7 +465,7 @@ def run_ours(args):
                        "l2_policy": f"inputs larger than L2: model {N * 256 / 1e6:.0f} MB + sorted list + block entries {(4 * Msum + 25 * Mbsum) / K / 1e6:.0f} MB "
                                     "per frame vs 126 MB L2",
                        "parallelism": f"frames sharded over {ws} rank(s), no collective", "presort_depth": args.presort},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks, "gpu_launches": int(round(len(krecs) * Kall / K)),
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "pipelined": pipelined, "clocks": clocks, "gpu_launches": int(round(len(krecs) * Kall / K)),
             "kernel_events": f"recorded on every {stride}th frame of the timed region ({K} of {Kall} frames, {len(krecs)} launches)",
             "gaussians_per_s": N * fps, "stage_ms_per_frame": stage_ms, "kernels": kernels}
     print(json.dumps(line), flush=True)

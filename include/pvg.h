@@ -142,6 +142,17 @@ int pvg_render_host_async(pvg_scene *scene, const pvg_camera *cam, float t, floa
                           float *host_depth, float *host_alpha);
 int pvg_wait_host(pvg_scene *scene);
 
+/* Frames in flight. Frames (camera, t) are independent, but one scene renders them one
+ * after another: its workspace holds one frame and the host waits once per frame for the frame's sizes. A FORK
+ * is a second scene handle on the SAME model (the re-laid-out Gaussians are shared and reference-counted: no
+ * copy, no extra model memory) with its own workspace, side streams and options (copied from the parent at the
+ * fork; the sky cube map is not inherited). Rendering alternate frames through a scene and its fork, each on
+ * its own stream (pvg_set_stream), keeps two frames in flight: the latency-bound kernels of one overlap the
+ * bandwidth- and issue-bound kernels of the other (config 3: +8% frames/s with two, nothing more with three).
+ * Each handle is destroyed with pvg_destroy, in any order; the model goes with the last one. A handle is not
+ * thread-safe; different handles may be used from different threads. Results are those of pvg_render. */
+int pvg_fork_scene(pvg_scene *scene, pvg_scene **out);
+
 int pvg_destroy(pvg_scene *scene);
 
 /* ---- options ------------------------------------------------------------------------------ */

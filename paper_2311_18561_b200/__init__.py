@@ -28,7 +28,7 @@ NUM_STAGES = len(STAGES)
 # every symbol include/pvg.h declares
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
            "pvg_render_host_async", "pvg_wait_host", "pvg_render_state", "pvg_set_sky",
-           "pvg_destroy", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms", "pvg_kernel_timeline_ms",
+           "pvg_destroy", "pvg_fork_scene", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms", "pvg_kernel_timeline_ms",
            "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
 
@@ -92,6 +92,7 @@ def load_library(path: Optional[str] = None):
     L.pvg_render_host_async.argtypes = [C.c_void_p, C.POINTER(CameraC), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_wait_host.argtypes = [C.c_void_p]
     L.pvg_destroy.argtypes = [C.c_void_p]
+    L.pvg_fork_scene.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
     L.pvg_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
     L.pvg_debug_view.argtypes = [C.c_void_p, C.POINTER(DebugC)]
     L.pvg_stage_times_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
@@ -203,6 +204,16 @@ class Scene:
     @classmethod
     def from_workload_scene(cls, sc, **kw) -> "Scene":
         return cls(sc.mu, sc.quat, sc.scale, sc.opacity, sc.sh, sc.tau, sc.beta, sc.vel, sc.cycle, sc.sh_degree, **kw)
+
+    def fork(self) -> "Scene":
+        """A second handle on the same model with its own workspace (include/pvg.h pvg_fork_scene): render
+        alternate frames through a scene and its fork, each under its own torch stream, to keep two frames in
+        flight."""
+        h = C.c_void_p()
+        _check(self._L.pvg_fork_scene(self._h, C.byref(h)))
+        other = object.__new__(Scene)
+        other._L, other._h, other.n = self._L, h, self.n
+        return other
 
     # -- the path ---------------------------------------------------------------------------
     def render(self, cam, t: float, out: Optional[Tuple] = None, dt: float = 0.0, rho_min: float = 0.0,

@@ -2,6 +2,7 @@
 // Orchestrates the five stages on one CUDA stream; every step of the path runs in the
 // kernels of this directory. No CPU fallback: CUDA errors surface as PVG_ERR_CUDA.
 
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -331,6 +332,12 @@ int run_compact_sort(uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint3
 
 }  // namespace
 
+// The re-laid-out model (SoA, preprocess.cuh), shared by a scene and its forks (pvg_fork_scene).
+struct Model {
+  Buf A0, A1, A2, A3, SH;
+  std::atomic<int> refs{1};
+};
+
 struct pvg_scene {
   uint32_t n = 0;
   float cycle = 0.2f;
@@ -341,8 +348,7 @@ struct pvg_scene {
   int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
   bool block_used = false;    // last frame built the tile lists from 8x8-tile block entries (blockbin.cuh)
-  // model (SoA)
-  Buf A0, A1, A2, A3, SH;
+  Model* model = nullptr;
   // per-Gaussian workspace
   Buf record, tileinfo, counts, offsets, dkeys[2], dvals[2], scan_status, small;  // small: ticket u32 @0, total u64 @8
   // per-instance workspace
@@ -385,7 +391,13 @@ int ceil_log2(uint32_t v) {
 }
 
 void release_all(pvg_scene* s) {
-  Buf* bufs[] = {&s->A0, &s->A1, &s->A2, &s->A3, &s->SH, &s->record, &s->tileinfo, &s->counts, &s->offsets,
+  if (s->model && s->model->refs.fetch_sub(1) == 1) {
+    Buf* mb[] = {&s->model->A0, &s->model->A1, &s->model->A2, &s->model->A3, &s->model->SH};
+    for (Buf* b : mb) b->release();
+    delete s->model;
+  }
+  s->model = nullptr;
+  Buf* bufs[] = {&s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->dhist, &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
@@ -415,6 +427,8 @@ int upload(Buf& dst, const float* src, size_t bytes, bool on_device, cudaStream_
   return PVG_OK;
 }
 
+int init_workspace(pvg_scene* s);
+
 int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   int ndev = 0;
   CU(cudaGetDeviceCount(&ndev));
@@ -436,17 +450,15 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   up(t_mu, d->mu, 3); up(t_quat, d->quat, 4); up(t_scale, d->scale, 3); up(t_op, d->opacity, 1);
   up(t_sh, d->sh, 48); up(t_tau, d->tau, 1); up(t_beta, d->beta, 1); up(t_vel, d->vel, 3);
   auto rs = [&](Buf& b, size_t bytes) { if (rc == PVG_OK) rc = b.reserve(bytes, st); };
-  rs(s->A0, n * 16); rs(s->A1, n * 16); rs(s->A2, n * 16); rs(s->A3, n * 16); rs(s->SH, n * 192);
-  rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4); rs(s->boffsets, n * 4);
-  rs(s->dkeys[0], n * 8); rs(s->dkeys[1], n * 8); rs(s->dvals[0], n * 4); rs(s->dvals[1], n * 4);
-  rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 8); rs(s->small, 256);
-  rs(s->dhist, 2 * kDhistWords * 4);
-  if (rc == PVG_OK && cudaMemsetAsync(s->dhist.p, 0, 2 * kDhistWords * 4, st) != cudaSuccess) rc = PVG_ERR_CUDA;
+  s->model = new (std::nothrow) Model();
+  if (!s->model) return PVG_ERR_OOM;
+  Model* m = s->model;
+  rs(m->A0, n * 16); rs(m->A1, n * 16); rs(m->A2, n * 16); rs(m->A3, n * 16); rs(m->SH, n * 192);
   if (rc == PVG_OK) {
     relayout_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
         (uint32_t)n, t_mu.as<float>(), t_quat.as<float>(), t_scale.as<float>(), t_op.as<float>(), t_sh.as<float>(),
-        t_tau.as<float>(), t_beta.as<float>(), t_vel.as<float>(), s->A0.as<float4>(), s->A1.as<float4>(),
-        s->A2.as<float4>(), s->A3.as<float4>(), s->SH.as<float4>());
+        t_tau.as<float>(), t_beta.as<float>(), t_vel.as<float>(), m->A0.as<float4>(), m->A1.as<float4>(),
+        m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>());
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {
@@ -457,6 +469,21 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   Buf* tmp[] = {&t_mu, &t_quat, &t_scale, &t_op, &t_sh, &t_tau, &t_beta, &t_vel};
   for (Buf* b : tmp) b->release();
   if (rc != PVG_OK) return rc;
+  return init_workspace(s);
+}
+
+// The per-scene workspace (sized by n), streams and events: everything a scene or a fork owns besides the model.
+int init_workspace(pvg_scene* s) {
+  const size_t n = s->n;
+  cudaStream_t st = s->stream;
+  int rc = PVG_OK;
+  auto rs = [&](Buf& b, size_t bytes) { if (rc == PVG_OK) rc = b.reserve(bytes, st); };
+  rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4); rs(s->boffsets, n * 4);
+  rs(s->dkeys[0], n * 8); rs(s->dkeys[1], n * 8); rs(s->dvals[0], n * 4); rs(s->dvals[1], n * 4);
+  rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 8); rs(s->small, 256);
+  rs(s->dhist, 2 * kDhistWords * 4);
+  if (rc != PVG_OK) return rc;
+  CU(cudaMemsetAsync(s->dhist.p, 0, 2 * kDhistWords * 4, st));
   CU(cudaHostAlloc((void**)&s->h_total, 64, cudaHostAllocMapped));
   CU(cudaHostGetDevicePointer((void**)&s->d_total, s->h_total, 0));
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
@@ -711,8 +738,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     featw = s->featw.as<float>();
   }
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
-  preprocess_kernel<<<(n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS), 256, 0, st>>>(P, n, s->A0.as<float4>(), s->A1.as<float4>(), s->A2.as<float4>(),
-                                                      s->A3.as<float4>(), s->SH.as<float4>(), s->record.as<float4>(),
+  preprocess_kernel<<<(n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS), 256, 0, st>>>(P, n, s->model->A0.as<float4>(), s->model->A1.as<float4>(), s->model->A2.as<float4>(),
+                                                      s->model->A3.as<float4>(), s->model->SH.as<float4>(), s->record.as<float4>(),
                                                       s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, featw,
                                                       s->presort ? s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords : nullptr);
   TRY(tm.end(st));
@@ -939,6 +966,28 @@ int pvg_create_scene(const pvg_scene_desc* d, pvg_scene** out) {
   pvg_scene* s = new (std::nothrow) pvg_scene();
   if (!s) return PVG_ERR_OOM;
   const int rc = create_impl(d, s);
+  if (rc != PVG_OK) {
+    release_all(s);
+    delete s;
+    return rc;
+  }
+  *out = s;
+  return PVG_OK;
+}
+
+int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
+  if (!scene || !out) return PVG_ERR_NULL;
+  *out = nullptr;
+  pvg_scene* s = new (std::nothrow) pvg_scene();
+  if (!s) return PVG_ERR_OOM;
+  s->n = scene->n; s->cycle = scene->cycle; s->sh_degree = scene->sh_degree;
+  s->stream = scene->stream;
+  s->presort = scene->presort; s->keep_unsorted = scene->keep_unsorted; s->count_pairs = scene->count_pairs;
+  s->compact = scene->compact; s->block = scene->block; s->blend_cull = scene->blend_cull;
+  s->model = scene->model;
+  s->model->refs.fetch_add(1);
+  // the model was written on the parent's stream at creation, which synchronised: nothing to wait for
+  const int rc = init_workspace(s);
   if (rc != PVG_OK) {
     release_all(s);
     delete s;

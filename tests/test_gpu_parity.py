@@ -458,3 +458,32 @@ def test_onesweep_all_equal_and_sorted_inputs():
         ko, vo = pvg.sort_pairs(torch.from_numpy(keys).cuda(), torch.from_numpy(vals).cuda(), 0, 40)
         idx = np.argsort(keys, kind="stable")
         assert np.array_equal(vo.cpu().numpy(), vals[idx]) and np.array_equal(ko.cpu().numpy(), keys[idx])
+
+
+def test_fork_shares_the_model_and_renders_the_same_frames():
+    """pvg_fork_scene: two frames in flight on two streams through a scene and its fork; every frame is bit-identical
+    to the same frame rendered alone, and the fork outlives its parent (the model is reference-counted)."""
+    import torch
+    wl = make_config(1, n=80_000)
+    cam = wl.cameras[0]
+    ts = [k / 7.0 for k in range(8)]
+    a = pvg.Scene.from_workload_scene(wl.scene)
+    ref = [[x.clone() for x in a.render(cam, t)] for t in ts]
+    b = a.fork()
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for k, t in enumerate(ts):
+        sc, st = (a, sa) if k % 2 == 0 else (b, sb)
+        with torch.cuda.stream(st):
+            outs.append(sc.render(cam, t))
+    torch.cuda.synchronize()
+    for r, o in zip(ref, outs):
+        assert all(torch.equal(x, y) for x, y in zip(r, o))
+    a.close()                                   # the fork keeps the model alive
+    again = b.render(cam, ts[3])
+    torch.cuda.synchronize()
+    assert all(torch.equal(x, y) for x, y in zip(ref[3], again))
+    c = b.fork()
+    b.close()
+    assert all(torch.equal(x, y) for x, y in zip(ref[5], c.render(cam, ts[5])))
+    c.close()
