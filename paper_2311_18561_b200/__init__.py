@@ -9,7 +9,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
-from typing import Dict, List, Optional, Tuple
+from typing import Dict, List, Optional, Sequence, Tuple
 
 import numpy as np
 
@@ -215,6 +215,35 @@ class Scene:
         other._L, other._h, other.n = self._L, h, self.n
         return other
 
+    def render_many(self, frames: Sequence, outs: Optional[Sequence] = None, in_flight: int = 2) -> List[Tuple]:
+        """Frames [(cam, t), ...] with `in_flight` of them overlapping (this scene and in_flight - 1 forks of it,
+        round-robin, each under its own torch stream). Returns the per-frame (rgb, depth, alpha); the calling
+        stream waits for all of them. Only stream and handle bookkeeping happens here."""
+        import torch
+        in_flight = max(1, min(int(in_flight), len(frames)))
+        forks = getattr(self, "_forks", None) or []
+        while len(forks) < in_flight - 1:
+            forks.append(self.fork())
+        self._forks = forks
+        lanes = getattr(self, "_lanes", None) or []
+        while len(lanes) < in_flight:
+            lanes.append(torch.cuda.Stream())
+        self._lanes = lanes
+        handles = [self] + forks
+        cur = torch.cuda.current_stream()
+        for ln in lanes[:in_flight]:
+            ln.wait_stream(cur)
+        res = []
+        for i, (cam, t) in enumerate(frames):
+            with torch.cuda.stream(lanes[i % in_flight]):
+                o = handles[i % in_flight].render(cam, t, None if outs is None else outs[i])
+            for x in o:
+                x.record_stream(cur)
+            res.append(o)
+        for ln in lanes[:in_flight]:
+            cur.wait_stream(ln)
+        return res
+
     # -- the path ---------------------------------------------------------------------------
     def render(self, cam, t: float, out: Optional[Tuple] = None, dt: float = 0.0, rho_min: float = 0.0,
                rho_max: float = float("inf"), target: str = "color"):
@@ -359,6 +388,9 @@ class Scene:
         return out
 
     def close(self) -> None:
+        for f in getattr(self, "_forks", None) or []:
+            f.close()
+        self._forks = []
         if getattr(self, "_h", None):
             self._L.pvg_destroy(self._h)
             self._h = None

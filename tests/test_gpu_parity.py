@@ -487,3 +487,17 @@ def test_fork_shares_the_model_and_renders_the_same_frames():
     b.close()
     assert all(torch.equal(x, y) for x, y in zip(ref[5], c.render(cam, ts[5])))
     c.close()
+
+
+def test_render_many_matches_single_frames():
+    import torch
+    wl = make_config(1, n=50_000)
+    frames = [(wl.cameras[0], k / 5.0) for k in range(6)]
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    ref = [[x.clone() for x in sc.render(c, t)] for c, t in frames]
+    for k in (1, 2, 3):
+        got = sc.render_many(frames, in_flight=k)
+        torch.cuda.current_stream().synchronize()
+        for r, o in zip(ref, got):
+            assert all(torch.equal(x, y) for x, y in zip(r, o))
+    sc.close()
