@@ -501,3 +501,27 @@ def test_render_many_matches_single_frames():
         for r, o in zip(ref, got):
             assert all(torch.equal(x, y) for x, y in zip(r, o))
     sc.close()
+
+
+def test_render_host_async_through_a_scene_and_its_fork():
+    """bench.py's end-to-end leg: alternate frames through two handles on two streams into pinned host buffers."""
+    import torch
+    wl = make_config(1, n=40_000)
+    cam = wl.cameras[0]
+    a = pvg.Scene.from_workload_scene(wl.scene)
+    handles = [a, a.fork()]
+    lanes = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ts = [k / 9.0 for k in range(10)]
+    bufs = [tuple(torch.zeros(shape, pin_memory=True) for shape in ((3, cam.height, cam.width), (cam.height, cam.width), (cam.height, cam.width)))
+            for _ in ts]
+    for k, (t, b) in enumerate(zip(ts, bufs)):
+        with torch.cuda.stream(lanes[k % 2]):
+            handles[k % 2].render_host_async(cam, t, b)
+    for h in handles:
+        h.wait_host()
+    for t, b in zip(ts, bufs):
+        ref = [x.cpu() for x in a.render(cam, t)]
+        for x, r in zip(b, ref):
+            assert torch.equal(x, r)
+    handles[1].close()
+    a.close()
