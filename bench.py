@@ -56,6 +56,7 @@ def parse_args():
     ap.add_argument("--bands", type=int, default=0,
                     help="with --split band on ONE GPU: time the bands of a K-way split one after another and "
                          "report the slowest band per frame (what one of K GPUs would compute; no collective)")
+    ap.add_argument("--lazy-chunks", type=int, default=-1, help="PVG_OPT_LAZY_CHUNKS (-1: the library default)")
     ap.add_argument("--event-stride", type=int, default=5,
                     help="record per-kernel CUDA events on every k-th timed frame (each record costs ~2 us of stream time)")
     return ap.parse_args()
@@ -245,6 +246,8 @@ def run_ours(args):
     scene = pvg.Scene.from_workload_scene(wl.scene)
     scene.set_option(pvg.OPT_PRESORT_DEPTH, args.presort)
     scene.set_option(pvg.OPT_BLOCK_BINS, args.block_bins)
+    if args.lazy_chunks >= 0:
+        scene.set_option(pvg.OPT_LAZY_CHUNKS, args.lazy_chunks)
     cams = {id(c): pvg.camera_struct(c) for c, _ in frames}
 
     def outs(c):

@@ -205,7 +205,17 @@ typedef enum pvg_option {
    *    camera of a render (BEGIN >= its tile rows) makes that render return PVG_ERR_BAD_STATE.
    *    In a band render the per-Gaussian counts, M and the ranges describe the band's tiles only. */
   PVG_OPT_TILE_ROW_BEGIN = 9,
-  PVG_OPT_TILE_ROW_END = 10
+  PVG_OPT_TILE_ROW_END = 10,
+  /* k > 0 (default 2), BLOCK_BINS mode: lazy tile lists. Front-to-back compositing stops a pixel at T < 1e-4, so a
+   *    tile reads its depth-sorted list only as far as its last live pixel needs -- at config 3 a few hundred of
+   *    its ~30 000 entries. The lists are therefore first written only as far as the first k chunks (512 block
+   *    entries each, in depth order) of every 8x8-tile block reach; the blend runs on these prefixes; the tiles
+   *    that still have a live pixel at the end of their prefix park their per-pixel state, get the REST of their
+   *    lists written (only those tiles), and resume. Every pixel sees the same entries in the same order with the
+   *    same arithmetic: the images are bit-identical to k = 0, and every list position that is written holds what
+   *    the complete list holds there. pvg_debug_view writes the remainder on demand, so vals_sorted is always
+   *    every tile's whole list. 0: write the complete lists before the blend. */
+  PVG_OPT_LAZY_CHUNKS = 11
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 
@@ -254,7 +264,8 @@ int pvg_kernel_timeline_ms(pvg_scene *scene, int cap, const char **names, float 
 
 /* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y,
  * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries,
- * surviving Gaussians S (PRESORT_DEPTH=1, else 0), reserved}. */
+ * surviving Gaussians S (PRESORT_DEPTH=1, else 0), tiles the first blend phase of the lazy lists parked (LAZY_CHUNKS;
+ * valid once the frame has completed on the stream)}. */
 int pvg_frame_stats(pvg_scene *scene, uint64_t out[8]);
 
 /* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs

@@ -129,29 +129,85 @@ struct BlendPixel {
 // quantity (here vbar in camera axes) and `featw` a fourth one (clamp(rho, 0, 2)); the outputs are the plain sums
 // sum T alpha f of Eq. 3, without background and without normalisation, in out_rgb and out_depth.
 enum { BLEND_COLOR = 0, BLEND_SKY = 1, BLEND_FEATURE = 2 };
-template <bool COUNT, int MODE>
-__global__ void __launch_bounds__(BLEND_THREADS)
-blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
-             const uint32_t* __restrict__ vals, const float4* __restrict__ record,
-             float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
-             unsigned long long* __restrict__ counters, const float* __restrict__ featw) {
+
+// Lazy lists (blockbin.cuh, PVG_OPT_LAZY_CHUNKS): a tile's list is first written only as far as the first c0
+// chunks of its block reach; most tiles saturate inside that prefix and the rest of their list is never needed.
+//   PHASE 0: the whole list at once (the lists are complete).
+//   PHASE 1: the prefix [begin, lim). A tile that still has a live pixel at lim < end parks its per-pixel state
+//            (T, C, D; the sign of T carries `alive`) and marks itself in unf_tile / unf_mask; every other tile
+//            writes its pixels.
+//   PHASE 2: only the marked tiles: they take their state back and go on from lim to the end, by then written
+//            by the second bin_write round. Same entries, same order, same arithmetic: the image is bit-identical.
+// lim[tile] is the position after chunk min(c0, chunks of the block) - 1 of the tile's block, stored by the warp
+// of bin_write's first round that owns that chunk. Phase 2 is a persistent launch over the list of parked tiles.
+struct BlendLazy {
+  const uint32_t* lim;             // [tiles] end of the written prefix of every non-empty list (bin_write, round 0)
+  float* state;                    // [5][H * W]
+  unsigned long long* unf_mask;    // [blocks] bit (ty & 7) * 8 + (tx & 7), zeroed
+  uint32_t* unf_count;             // [1] zeroed: number of parked tiles
+  uint32_t* unf_list;              // [tiles] the parked tiles, in parking order
+  volatile uint64_t* parked_host;  // mapped host word: the count, for pvg_frame_stats
+  uint32_t blocks_x;
+};
+
+// Parks a tile (first blend phase of the lazy lists): out of line, so that the rare path costs the common one nothing.
+__device__ __noinline__ void blend_park(const BlendLazy& Z, uint32_t tile, uint32_t bin, uint32_t ltile, size_t HW, size_t pi,
+                                        uint32_t inmask, const float (&st)[BLEND_NPX][5]) {
+#pragma unroll
+  for (int k = 0; k < BLEND_NPX; ++k) {
+    if (!((inmask >> k) & 1u)) continue;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) Z.state[c * HW + pi + k] = st[k][c];
+  }
+  if (threadIdx.x == 0) {
+    Z.unf_list[atomicAdd(Z.unf_count, 1u)] = tile;
+    atomicOr(Z.unf_mask + bin, 1ull << ltile);
+  }
+}
+
+template <bool COUNT, int MODE, int PHASE>
+__device__ __forceinline__ void
+blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ ranges,
+           const uint32_t* __restrict__ vals, const float4* __restrict__ record,
+           float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
+           unsigned long long* __restrict__ counters, const float* __restrict__ featw, const BlendLazy& Z) {
   __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
   __shared__ float4 s_col[BLEND_BATCH];   // c', log2 o~, r, g
   __shared__ float2 s_bz[BLEND_BATCH];    // b, z
   __shared__ uint32_t s_kept[BLEND_THREADS / 32];
 
   const uint32_t tid = threadIdx.x;
-  const uint32_t tile = blockIdx.x + (uint32_t)P.band_y0 * (uint32_t)P.tiles_x;   // only the band's tiles are launched
   const uint32_t tx = tile % P.tiles_x, ty = tile / P.tiles_x;
   constexpr uint32_t TPR = PVG_TILE / BLEND_NPX;   // threads per tile row
   const uint32_t px = tx * PVG_TILE + BLEND_NPX * (tid % TPR), py = ty * PVG_TILE + tid / TPR;
   const float pxf = (float)px + 0.5f, pyf = (float)py + 0.5f;   // S14
-  const uint2 range = ranges[tile];
+  uint2 range = ranges[tile];
+  const uint32_t list_end = range.y;
+  (void)list_end;
+  if (PHASE != 0) {
+    const uint32_t lim = range.x == range.y ? range.y : Z.lim[tile];
+    if (PHASE == 1) range.y = lim; else range.x = lim;
+  }
 
   BlendPixel X[BLEND_NPX];
   bool in[BLEND_NPX];
 #pragma unroll
   for (int k = 0; k < BLEND_NPX; ++k) X[k].alive = in[k] = px + k < (uint32_t)P.width && py < (uint32_t)P.height;
+  if (PHASE == 2) {
+    const size_t HW = (size_t)P.width * P.height;
+    const size_t pi = (size_t)py * P.width + px;
+#pragma unroll
+    for (int k = 0; k < BLEND_NPX; ++k) {
+      if (!in[k]) continue;
+      const float t = Z.state[pi + k];
+      X[k].alive = !signbit(t);
+      X[k].T = fabsf(t);
+      X[k].Cr = Z.state[HW + pi + k];
+      X[k].Cg = Z.state[2 * HW + pi + k];
+      X[k].Cb = Z.state[3 * HW + pi + k];
+      X[k].D = Z.state[4 * HW + pi + k];
+    }
+  }
   auto any_alive = [&]() {
     bool a = false;
 #pragma unroll
@@ -169,9 +225,10 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
   // saturates, so a fixed 256-entry first batch gathers mostly records that are never used
   uint32_t bs = BLEND_BATCH_FIRST;
+  bool all_dead = false;   // block-uniform: the loop ended because every pixel of the tile had stopped
   for (uint32_t base = range.x; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
-    if (__syncthreads_count(any_alive()) == 0) break;
+    if (__syncthreads_count(any_alive()) == 0) { all_dead = true; break; }
     // Staging. Warp w gathers the w-th segment of the batch and keeps, in order, only the entries whose
     // ellipse { alpha >= 1/255 } can reach the tile at all: the lists are built from axis-aligned
     // rectangles (S7), and 26% (config 3) to 48% (config 4) of the entries a tile consumes cover it with
@@ -248,6 +305,23 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
   }
   const size_t HW = (size_t)P.width * P.height;
   const size_t pi = (size_t)py * P.width + px;
+  if (PHASE == 1 && !all_dead && range.y < list_end) {
+    // the written prefix is used up without the tile being known dead: park it if a pixel is still alive
+    // (block-uniform decision; rare -- a saturating tile leaves the loop through the check at its top)
+    if (__syncthreads_or(any_alive())) {
+      float st[BLEND_NPX][5];
+#pragma unroll
+      for (int k = 0; k < BLEND_NPX; ++k) {
+        st[k][0] = X[k].alive ? X[k].T : -X[k].T;
+        st[k][1] = X[k].Cr; st[k][2] = X[k].Cg; st[k][3] = X[k].Cb; st[k][4] = X[k].D;
+      }
+      uint32_t inmask = 0;
+#pragma unroll
+      for (int k = 0; k < BLEND_NPX; ++k) inmask |= in[k] ? 1u << k : 0u;
+      blend_park(Z, tile, (ty >> 3) * Z.blocks_x + (tx >> 3), (ty & 7u) * 8u + (tx & 7u), HW, pi, inmask, st);
+      return;
+    }
+  }
 #pragma unroll
   for (int k = 0; k < BLEND_NPX; ++k) {
     if (!in[k]) continue;
@@ -267,6 +341,27 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
     }
     if (out_depth) out_depth[pi + k] = MODE == BLEND_FEATURE ? X[k].D : (Al > 0.f ? X[k].D / Al : 0.f);
     if (out_alpha) out_alpha[pi + k] = Al;
+  }
+}
+
+template <bool COUNT, int MODE, int PHASE>
+__global__ void __launch_bounds__(BLEND_THREADS)
+blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
+             const uint32_t* __restrict__ vals, const float4* __restrict__ record,
+             float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
+             unsigned long long* __restrict__ counters, const float* __restrict__ featw,
+             const __grid_constant__ BlendLazy Z) {
+  if (PHASE != 2) {
+    // one CTA per tile; only the band's tiles are launched
+    blend_tile<COUNT, MODE, PHASE>(P, blockIdx.x + (uint32_t)P.band_y0 * (uint32_t)P.tiles_x, ranges, vals, record, out_rgb,
+                                   out_depth, out_alpha, counters, featw, Z);
+  } else {
+    const uint32_t parked = *Z.unf_count;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *Z.parked_host = parked;
+    for (uint32_t it = blockIdx.x; it < parked; it += gridDim.x) {
+      blend_tile<COUNT, MODE, 2>(P, Z.unf_list[it], ranges, vals, record, out_rgb, out_depth, out_alpha, counters, featw, Z);
+      __syncthreads();   // the next tile's staging reuses the shared-memory batch
+    }
   }
 }
 

@@ -391,24 +391,40 @@ struct BinWalk {
   uint32_t chunk, half, e0, e1, bin, kin;   // kin: index of the chunk inside its block
   bool first;
 };
+// kin_lo, kin_hi: only the chunks kin_lo <= kin < kin_hi of every block are walked (lazy lists: the first
+// kin_hi chunks, later the rest). With kin_lo == 0 and kin_hi < 2^30 the launch enumerates (block, kin) pairs
+// directly -- chunk t of the launch is chunk t % kin_hi of block t / kin_hi -- so that its grid is nblocks *
+// kin_hi chunks instead of all of them; inside a block kin still ascends with the ticket.
 __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ chunk_start,
-                                               uint32_t* s_cs, uint32_t* __restrict__ ticket, BinWalk& w) {
+                                               uint32_t* s_cs, uint32_t* __restrict__ ticket, BinWalk& w,
+                                               uint32_t kin_lo, uint32_t kin_hi) {
   if (threadIdx.x == 0) s_cs[BB_MAX_BINS + 1] = atomicAdd(ticket, 1u);
   for (uint32_t k = threadIdx.x; k <= BB_MAX_BINS; k += BW_THREADS) s_cs[k] = chunk_start[k];
   __syncthreads();
   const uint32_t warp = threadIdx.x >> 5;
-  w.chunk = s_cs[BB_MAX_BINS + 1] * BW_CHUNKS_PER_CTA + (warp >> 1);
+  const uint32_t t = s_cs[BB_MAX_BINS + 1] * BW_CHUNKS_PER_CTA + (warp >> 1);
   w.half = warp & 1u;
-  if (w.chunk >= s_cs[BB_MAX_BINS]) return false;
-  uint32_t lo = 0, hi = BB_MAX_BINS;   // last b with chunk_start[b] <= chunk: the block that owns it
-  while (hi - lo > 1) {
-    const uint32_t mid = (lo + hi) >> 1;
-    if (s_cs[mid] <= w.chunk) lo = mid; else hi = mid;
+  uint32_t lo;
+  if (kin_lo == 0 && kin_hi < (1u << 30)) {
+    lo = t / kin_hi;
+    w.kin = t - lo * kin_hi;
+    if (lo >= BB_MAX_BINS || w.kin >= s_cs[lo + 1] - s_cs[lo]) return false;
+    w.chunk = s_cs[lo] + w.kin;
+  } else {
+    w.chunk = t;
+    if (w.chunk >= s_cs[BB_MAX_BINS]) return false;
+    lo = 0;
+    uint32_t hi = BB_MAX_BINS;   // last b with chunk_start[b] <= chunk: the block that owns it
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (s_cs[mid] <= w.chunk) lo = mid; else hi = mid;
+    }
+    w.kin = w.chunk - s_cs[lo];
+    if (w.kin < kin_lo || w.kin >= kin_hi) return false;
   }
   w.bin = lo;
-  w.kin = w.chunk - s_cs[lo];
   w.first = w.kin == 0;
-  w.e0 = bin_start[lo] + (w.chunk - s_cs[lo]) * BB_CHUNK;
+  w.e0 = bin_start[lo] + w.kin * BB_CHUNK;
   w.e1 = min(w.e0 + (uint32_t)BB_CHUNK, bin_start[lo + 1]);
   return true;
 }
@@ -450,9 +466,10 @@ constexpr int BW_PTR_ROW = BB_CHUNK / 64 + 1;   // uint4 per tile row, padded by
 template <bool FULL>
 __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 32], const uint32_t (&g)[BB_CHUNK / 32],
                                                 const ulonglong2* s_ptr /* [32 tiles][BW_PTR_ROW] of this warp */, uint32_t nb,
-                                                uint32_t lt) {
+                                                uint32_t lt, uint32_t want /* tiles to write (bit l = tile l) */) {
   for (uint32_t l = 0; l < 32; ++l, s_ptr += BW_PTR_ROW) {
     const uint32_t bit = 1u << l;
+    if (!(want & bit)) continue;
 #pragma unroll
     for (int k = 0; k < BB_CHUNK / 64; ++k) {
       const ulonglong2 q = s_ptr[k];   // two pointers, broadcast; row + constant offset: no address arithmetic per load
@@ -477,15 +494,23 @@ __global__ void __launch_bounds__(BW_THREADS, 4)
 bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
                  const uint32_t* __restrict__ chunk_start, const uint2* __restrict__ ranges, uint32_t tiles_x,
                  uint32_t tiles_y, uint32_t blocks_x, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
-                 uint32_t* __restrict__ vals) {
+                 uint32_t* __restrict__ vals, uint32_t kin_lo, uint32_t kin_hi,
+                 const unsigned long long* __restrict__ want_mask /* [blocks] tiles still wanted, or nullptr: all */,
+                 const uint32_t* __restrict__ want_count /* with want_mask: nothing to do at all if 0 */,
+                 uint32_t* __restrict__ lim /* [tiles] or nullptr: where each tile's list stands after chunk kin_hi - 1 */) {
   __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
   // the base pointer round-trips through shared memory so that it lives in registers; taken from the
   // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
   __shared__ uint32_t* s_vals;
   __shared__ ulonglong2 s_ptr[BW_THREADS / 32][32 * BW_PTR_ROW];
+  if (want_mask && *want_count == 0u) return;   // lazy lists: no tile was parked
   if (threadIdx.x == 0) s_vals = vals;
   BinWalk w;
-  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w)) return;   // (contains the barrier)
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w, kin_lo, kin_hi)) return;   // (contains the barrier)
+  // lazy lists, second round: only the tiles the blend has not finished; a block without any is skipped by all of
+  // its chunks alike (the mask is fixed for the whole launch), so nobody waits for a skipped chunk's look-back word
+  const uint32_t want = want_mask ? (uint32_t)(want_mask[w.bin] >> (32u * w.half)) : 0xFFFFFFFFu;
+  if (want_mask && want_mask[w.bin] == 0ull) return;
   uint32_t* const vp = s_vals;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t lt = lanemask_lt();
@@ -547,6 +572,12 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
     }
   }
   st_relaxed_u64(my, LB_FLAG_PREFIX | (uint64_t)(mypos + cnt));
+  if (lim && (w.kin + 1u == kin_hi || w.e1 == bin_start[w.bin + 1])) {
+    // the last chunk of the block this round writes: the blend's first phase reads each list up to here
+    const uint32_t ltile = w.half * 32u + lane;
+    const uint32_t tx = (w.bin % blocks_x) * 8u + (ltile & 7u), ty = (w.bin / blocks_x) * 8u + (ltile >> 3);
+    if (tx < tiles_x && ty < tiles_y) lim[ty * tiles_x + tx] = mypos + cnt;
+  }
   ulonglong2* sp = s_ptr[threadIdx.x >> 5];
   {
     const uint64_t base = reinterpret_cast<uint64_t>(vp + mypos);
@@ -558,8 +589,8 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
   }
   __syncwarp();
   const uint32_t nb = (w.e1 - w.e0 + 31u) >> 5;
-  if (nb == NB) bin_write_tiles<true>(m, g, sp, nb, lt);
-  else bin_write_tiles<false>(m, g, sp, nb, lt);
+  if (nb == NB) bin_write_tiles<true>(m, g, sp, nb, lt, want);
+  else bin_write_tiles<false>(m, g, sp, nb, lt, want);
 }
 
 }  // namespace pvg

@@ -108,6 +108,8 @@ struct OsSmall { static constexpr int THREADS = PVG_OSS_THREADS, ITEMS = PVG_OSS
 constexpr uint64_t OS_SMALL_BELOW = PVG_OS_SMALL_BELOW;
 
 // scratch of one sort call
+// layout of pvg_scene::unf: [256] u64 block masks | u32 parked count (+ pad) | [tiles] u32 lim | [tiles] u32 parked list
+constexpr size_t kUnfHead = 2048 + 64;
 constexpr size_t kDhistWords = 1032;   // 4 x 256 counts + the CTA counter, padded to 16 B
 
 struct SortScratch {
@@ -346,6 +348,9 @@ struct pvg_scene {
   // options
   int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1, blend_cull = 1;
   int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
+  int lazy_chunks = 2;                // PVG_OPT_LAZY_CHUNKS (0: always write the complete lists)
+  bool lazy_used = false;             // last frame wrote list prefixes + what the unfinished tiles needed
+  bool lists_complete = true;         // vals[] holds every tile's whole list (pvg_debug_view completes them on demand)
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
   bool block_used = false;    // last frame built the tile lists from 8x8-tile block entries (blockbin.cuh)
   Model* model = nullptr;
@@ -356,6 +361,7 @@ struct pvg_scene {
   Buf tiles16[2], tiles16_unsorted;
   // block-entry workspace (blockbin.cuh)
   Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
+  Buf lazy_state, unf;   // blend state of parked tiles [5][H W]; unfinished flags: [256] u64 block masks, then [tiles] u32
   Buf dhist;          // 2 x (4 x 256 digit counts + 1 CTA counter) u32: the depth histogram preprocess accumulates, double-buffered
   int dhist_side = 0;
   Buf ranges, tilegrid;
@@ -400,7 +406,7 @@ void release_all(pvg_scene* s) {
   Buf* bufs[] = {&s->record, &s->tileinfo, &s->counts, &s->offsets,
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
-                 &s->dhist, &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
+                 &s->lazy_state, &s->unf, &s->dhist, &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
                  &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
@@ -631,9 +637,33 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
   TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
   TRY(s->sort_m.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
   TRY(s->chunk_owner.reserve(((size_t)Mb / kOwnerChunk + 2) * 4, st, 1.125));
-  CU(cudaMemsetAsync(s->sort_m.tickets.p, 0, 8, zs));
+  CU(cudaMemsetAsync(s->sort_m.tickets.p, 0, 16, zs));   // emit, write (round 0), write (round 1), write (completion)
   CU(cudaMemsetAsync(s->chunk_cnt.p, 0, (size_t)max_chunks * 64 * 8, zs));
+  if (s->lazy_chunks > 0) {
+    const size_t tiles = (size_t)P.tiles_x * P.tiles_y;
+    TRY(s->unf.reserve(kUnfHead + tiles * 8, st));
+    TRY(s->lazy_state.reserve((size_t)5 * P.width * P.height * 4, st));
+    CU(cudaMemsetAsync(s->unf.p, 0, kUnfHead, zs));   // masks and count; lim and the list are written before they are read
+  }
   CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, zs));
+  return PVG_OK;
+}
+
+// bin_write over the chunks kin_lo <= kin < kin_hi of every block; only_unfinished: the tiles the first blend
+// phase marked. ticket_slot: which zeroed ticket of sort_m.tickets this launch consumes.
+int launch_bin_write(pvg_scene* s, const FrameParams& P, uint32_t kin_lo, uint32_t kin_hi, bool only_unfinished, int ticket_slot) {
+  const uint32_t Mb = (uint32_t)s->Mb;
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
+  uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
+  const uint32_t launch_chunks = (kin_lo == 0 && kin_hi < (1u << 30)) ? std::min<uint64_t>((uint64_t)nbins * kin_hi, 0x7FFFFFFFull) : max_chunks;
+  const unsigned grid = (launch_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
+  bin_write_kernel<<<grid, BW_THREADS, 0, s->stream>>>(
+      s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, bin_start + 257, s->ranges.as<uint2>(), (uint32_t)P.tiles_x,
+      (uint32_t)P.tiles_y, blocks_x, s->chunk_cnt.as<uint64_t>(), s->sort_m.tickets.as<uint32_t>() + ticket_slot,
+      s->vals[0].as<uint32_t>(), kin_lo, kin_hi, only_unfinished ? s->unf.as<unsigned long long>() : nullptr,
+      reinterpret_cast<const uint32_t*>(s->unf.as<unsigned char>() + 2048),
+      (kin_lo == 0 && kin_hi < (1u << 30)) ? reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) : nullptr);
   return PVG_OK;
 }
 
@@ -643,9 +673,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   cudaStream_t st = s->stream;
   const uint32_t Mb = (uint32_t)s->Mb;
   const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
-  const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
-  uint32_t* chunk_start = bin_start + 257;
   uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
 
   int rc = PVG_ERR_BAD_OPTION;
@@ -679,11 +707,12 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(tm->end(st));
 #endif
 
-  const unsigned walk_grid = (max_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
+  // the tile lists: all of them, or (lazy) only as far as the first lazy_chunks chunks of every block reach --
+  // render_impl runs the second round after the first blend phase
+  s->lazy_used = s->lazy_chunks > 0;
+  s->lists_complete = !s->lazy_used;
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
-  bin_write_kernel<<<walk_grid, BW_THREADS, 0, st>>>(s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, chunk_start,
-                                                     s->ranges.as<uint2>(), (uint32_t)P.tiles_x, (uint32_t)P.tiles_y, blocks_x,
-                                                     s->chunk_cnt.as<uint64_t>(), ticket + 1, s->vals[0].as<uint32_t>());
+  TRY(launch_bin_write(s, P, 0u, s->lazy_used ? (uint32_t)s->lazy_chunks : 0xFFFFFFFFu, false, 1));
   TRY(tm->end(st));
   CU(cudaGetLastError());
   s->sorted_side = 0;
@@ -901,16 +930,42 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     const float4* rec = s->record.as<float4>();
     const int mode = P.target == 1 ? BLEND_FEATURE : (P.sky ? BLEND_SKY : BLEND_COLOR);
     const uint32_t band_tiles = (uint32_t)P.tiles_x * (uint32_t)(P.band_y1 - P.band_y0);
-#define PVG_BLEND(C, M) blend_kernel<C, M><<<band_tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw)
-    if (s->count_pairs) {
-      if (mode == BLEND_FEATURE) PVG_BLEND(true, BLEND_FEATURE);
-      else if (mode == BLEND_SKY) PVG_BLEND(true, BLEND_SKY);
-      else PVG_BLEND(true, BLEND_COLOR);
-    } else {
-      if (mode == BLEND_FEATURE) PVG_BLEND(false, BLEND_FEATURE);
-      else if (mode == BLEND_SKY) PVG_BLEND(false, BLEND_SKY);
-      else PVG_BLEND(false, BLEND_COLOR);
+    const bool lazy = M > 0 && s->block_used && s->lazy_used;
+    BlendLazy Z = {};
+    if (lazy) {
+      const size_t ntiles = (size_t)P.tiles_x * P.tiles_y;
+      Z.state = s->lazy_state.as<float>();
+      Z.unf_mask = s->unf.as<unsigned long long>();
+      Z.unf_count = reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + 2048);
+      Z.lim = reinterpret_cast<const uint32_t*>(s->unf.as<unsigned char>() + kUnfHead);
+      Z.unf_list = reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) + ntiles;
+      Z.parked_host = s->d_total + 3;
+      Z.blocks_x = bb_blocks(P.tiles_x);
     }
+#define PVG_BLEND(C, M, PH) blend_kernel<C, M, PH><<<(PH) == 2 ? std::min(band_tiles, 148u * 8u) : band_tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw, Z)
+#define PVG_BLEND_ALL(PH)                                        \
+    if (s->count_pairs) {                                        \
+      if (mode == BLEND_FEATURE) PVG_BLEND(true, BLEND_FEATURE, PH); \
+      else if (mode == BLEND_SKY) PVG_BLEND(true, BLEND_SKY, PH);    \
+      else PVG_BLEND(true, BLEND_COLOR, PH);                         \
+    } else {                                                     \
+      if (mode == BLEND_FEATURE) PVG_BLEND(false, BLEND_FEATURE, PH); \
+      else if (mode == BLEND_SKY) PVG_BLEND(false, BLEND_SKY, PH);    \
+      else PVG_BLEND(false, BLEND_COLOR, PH);                         \
+    }
+    if (!lazy) {
+      PVG_BLEND_ALL(0)
+    } else {
+      // phase 1 on the list prefixes; the tiles it could not finish get the rest of their lists, then phase 2
+      PVG_BLEND_ALL(1)
+      TRY(tm.end(st));
+      TRY(tm.begin("bin_write", PVG_STAGE_SORT, st));
+      TRY(launch_bin_write(s, P, (uint32_t)s->lazy_chunks, 0xFFFFFFFFu, true, 2));
+      TRY(tm.end(st));
+      TRY(tm.begin("blend", PVG_STAGE_BLEND, st));
+      PVG_BLEND_ALL(2)
+    }
+#undef PVG_BLEND_ALL
 #undef PVG_BLEND
   }
   TRY(tm.end(st));
@@ -984,6 +1039,7 @@ int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
   s->stream = scene->stream;
   s->presort = scene->presort; s->keep_unsorted = scene->keep_unsorted; s->count_pairs = scene->count_pairs;
   s->compact = scene->compact; s->block = scene->block; s->blend_cull = scene->blend_cull;
+  s->lazy_chunks = scene->lazy_chunks;
   s->model = scene->model;
   s->model->refs.fetch_add(1);
   // the model was written on the parent's stream at creation, which synchronised: nothing to wait for
@@ -1039,6 +1095,10 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
       scene->timer.accumulate = value == 2;
       scene->timer.renders = 0;
       scene->timer.reset();
+      return PVG_OK;
+    case PVG_OPT_LAZY_CHUNKS:
+      if (value < 0 || value > (1 << 20)) return PVG_ERR_BAD_OPTION;
+      scene->lazy_chunks = (int)value;
       return PVG_OK;
     case PVG_OPT_TILE_ROW_BEGIN:
       if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
@@ -1137,6 +1197,13 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->counts = s->counts.as<uint32_t>();
   out->visit_order = s->presort ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
+  if (s->block_used && s->lazy_used && !s->lists_complete && s->M) {
+    // lazy lists: write what the frame never needed, so that vals_sorted is every tile's whole list
+    CU(cudaMemsetAsync(s->sort_m.tickets.as<uint32_t>() + 3, 0, 4, s->stream));
+    TRY(launch_bin_write(s, s->last_P, (uint32_t)s->lazy_chunks, 0xFFFFFFFFu, false, 3));
+    CU(cudaGetLastError());
+    s->lists_complete = true;
+  }
   if (s->block_used) {
     // the block path never forms per-instance offsets or the unsorted list: produce them here
     cudaStream_t st = s->stream;
@@ -1246,7 +1313,9 @@ int pvg_frame_stats(pvg_scene* s, uint64_t out[8]) {
   out[4] = s->rendered ? s->Mb : 0;
   out[5] = s->block_used ? 2 : (s->compact_used ? 1 : 0);
   out[6] = (s->rendered && s->presort) ? s->survivors : 0;
-  out[7] = 0;
+  // tiles the lazy lists' first blend phase parked (stored by the second phase through mapped host memory: it is
+  // the last frame's figure once that frame has completed on the stream; the word is only read here)
+  out[7] = (s->rendered && s->block_used && s->lazy_used && s->M) ? s->h_total[3] : 0;
   return PVG_OK;
 }
 
