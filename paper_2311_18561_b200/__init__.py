@@ -22,7 +22,7 @@ STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_
 OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
 OPT_BLEND_CULL, OPT_EVENT_STRIDE = 7, 8
 OPT_TILE_ROW_BEGIN, OPT_TILE_ROW_END = 9, 10
-OPT_LAZY_CHUNKS = 11
+OPT_LAZY_CHUNKS, OPT_LAZY_SLAB = 11, 12
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 

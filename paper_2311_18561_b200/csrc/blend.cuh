@@ -185,7 +185,8 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   const uint32_t list_end = range.y;
   (void)list_end;
   if (PHASE != 0) {
-    const uint32_t lim = range.x == range.y ? range.y : Z.lim[tile];
+    // lim[] is zeroed: a tile whose block has no complete chunk yet stands at its list's begin
+    const uint32_t lim = range.x == range.y ? range.y : max(Z.lim[tile], range.x);
     if (PHASE == 1) range.y = lim; else range.x = lim;
   }
 

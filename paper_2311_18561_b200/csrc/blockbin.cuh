@@ -256,11 +256,15 @@ __global__ void __launch_bounds__(BP_THREADS, PVG_BP_MINB)
 bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
                 const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x,
                 uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, const uint32_t* __restrict__ bin_start,
-                uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket) {
+                uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket,
+                const uint32_t* __restrict__ only_if /* nullptr, or: do nothing when *only_if == 0 */) {
   using Core = RadixCore<BP_THREADS, BP_ITEMS, BITS>;
   constexpr uint32_t MASK = (1u << BITS) - 1u;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   BinEmitSmem<BITS>& s = *reinterpret_cast<BinEmitSmem<BITS>*>(smem_raw);
+  // lazy lists: the launch that emits the entries behind the first slab runs only if a tile was parked. The
+  // tiles are handed out by the ticket, which simply goes on counting from the first launch.
+  if (only_if && *only_if == 0u) return;
 
   const uint32_t tile = Core::take_ticket(s.core, ticket);
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -388,16 +392,29 @@ __device__ __forceinline__ uint32_t transpose32(uint32_t x, uint32_t lane) {
 // on chunks whose CTA has already started. Fills the entry range [e0, e1), the block and whether
 // the chunk is the block's first; returns false past the end.
 struct BinWalk {
-  uint32_t chunk, half, e0, e1, bin, kin;   // kin: index of the chunk inside its block
+  uint32_t chunk, half, e0, e1, bin, kin, limit;   // kin: index of the chunk inside its block; limit: chunks of the block this round
   bool first;
 };
 // kin_lo, kin_hi: only the chunks kin_lo <= kin < kin_hi of every block are walked (lazy lists: the first
 // kin_hi chunks, later the rest). With kin_lo == 0 and kin_hi < 2^30 the launch enumerates (block, kin) pairs
 // directly -- chunk t of the launch is chunk t % kin_hi of block t / kin_hi -- so that its grid is nblocks *
 // kin_hi chunks instead of all of them; inside a block kin still ascends with the ticket.
+// avail (lazy emission): avail[b] (low 62 bits) = entries of block b that exist so far; a chunk counts only if all
+// of its entries do. The first round then stops at min(kin_hi, whole chunks available) per block, and the round
+// after it (kin_lo > 0) starts there.
+__device__ __forceinline__ uint32_t bin_round0_chunks(const uint32_t* __restrict__ bin_start, const uint64_t* __restrict__ avail,
+                                                      uint32_t bin, uint32_t nch, uint32_t c0) {
+  uint32_t have = nch;
+  if (avail) {
+    const uint32_t a = (uint32_t)(avail[bin] & LB_VALUE_MASK), total = bin_start[bin + 1] - bin_start[bin];
+    have = a >= total ? nch : a / (uint32_t)BB_CHUNK;
+  }
+  return min(c0, have);
+}
+
 __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ chunk_start,
                                                uint32_t* s_cs, uint32_t* __restrict__ ticket, BinWalk& w,
-                                               uint32_t kin_lo, uint32_t kin_hi) {
+                                               uint32_t kin_lo, uint32_t kin_hi, const uint64_t* __restrict__ avail) {
   if (threadIdx.x == 0) s_cs[BB_MAX_BINS + 1] = atomicAdd(ticket, 1u);
   for (uint32_t k = threadIdx.x; k <= BB_MAX_BINS; k += BW_THREADS) s_cs[k] = chunk_start[k];
   __syncthreads();
@@ -408,7 +425,9 @@ __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_
   if (kin_lo == 0 && kin_hi < (1u << 30)) {
     lo = t / kin_hi;
     w.kin = t - lo * kin_hi;
-    if (lo >= BB_MAX_BINS || w.kin >= s_cs[lo + 1] - s_cs[lo]) return false;
+    if (lo >= BB_MAX_BINS) return false;
+    w.limit = bin_round0_chunks(bin_start, avail, lo, s_cs[lo + 1] - s_cs[lo], kin_hi);
+    if (w.kin >= w.limit) return false;
     w.chunk = s_cs[lo] + w.kin;
   } else {
     w.chunk = t;
@@ -420,7 +439,9 @@ __device__ __forceinline__ bool bin_walk_setup(const uint32_t* __restrict__ bin_
       if (s_cs[mid] <= w.chunk) lo = mid; else hi = mid;
     }
     w.kin = w.chunk - s_cs[lo];
-    if (w.kin < kin_lo || w.kin >= kin_hi) return false;
+    w.limit = kin_hi;
+    if (w.kin >= kin_hi) return false;
+    if (kin_lo && w.kin < bin_round0_chunks(bin_start, avail, lo, s_cs[lo + 1] - s_cs[lo], kin_lo)) return false;
   }
   w.bin = lo;
   w.first = w.kin == 0;
@@ -497,7 +518,8 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
                  uint32_t* __restrict__ vals, uint32_t kin_lo, uint32_t kin_hi,
                  const unsigned long long* __restrict__ want_mask /* [blocks] tiles still wanted, or nullptr: all */,
                  const uint32_t* __restrict__ want_count /* with want_mask: nothing to do at all if 0 */,
-                 uint32_t* __restrict__ lim /* [tiles] or nullptr: where each tile's list stands after chunk kin_hi - 1 */) {
+                 uint32_t* __restrict__ lim /* [tiles] or nullptr: where each tile's list stands after this round */,
+                 const uint64_t* __restrict__ avail /* [blocks] or nullptr: entries emitted so far (bin_round0_chunks) */) {
   __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
   // the base pointer round-trips through shared memory so that it lives in registers; taken from the
   // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
@@ -506,7 +528,7 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
   if (want_mask && *want_count == 0u) return;   // lazy lists: no tile was parked
   if (threadIdx.x == 0) s_vals = vals;
   BinWalk w;
-  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w, kin_lo, kin_hi)) return;   // (contains the barrier)
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w, kin_lo, kin_hi, avail)) return;   // (contains the barrier)
   // lazy lists, second round: only the tiles the blend has not finished; a block without any is skipped by all of
   // its chunks alike (the mask is fixed for the whole launch), so nobody waits for a skipped chunk's look-back word
   const uint32_t want = want_mask ? (uint32_t)(want_mask[w.bin] >> (32u * w.half)) : 0xFFFFFFFFu;
@@ -572,7 +594,7 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
     }
   }
   st_relaxed_u64(my, LB_FLAG_PREFIX | (uint64_t)(mypos + cnt));
-  if (lim && (w.kin + 1u == kin_hi || w.e1 == bin_start[w.bin + 1])) {
+  if (lim && w.kin + 1u == w.limit) {
     // the last chunk of the block this round writes: the blend's first phase reads each list up to here
     const uint32_t ltile = w.half * 32u + lane;
     const uint32_t tx = (w.bin % blocks_x) * 8u + (ltile & 7u), ty = (w.bin / blocks_x) * 8u + (ltile >> 3);

@@ -349,6 +349,9 @@ struct pvg_scene {
   int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1, blend_cull = 1;
   int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
   int lazy_chunks = 2;                // PVG_OPT_LAZY_CHUNKS (0: always write the complete lists)
+  int lazy_slab = 8;                  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front
+  uint32_t emit_first = 0, emit_tiles = 0, emit_radix = 256;   // bin_emit tiles in the first launch / in all; its look-back row length
+  const uint32_t* visit_last = nullptr;
   bool lazy_used = false;             // last frame wrote list prefixes + what the unfinished tiles needed
   bool lists_complete = true;         // vals[] holds every tile's whole list (pvg_debug_view completes them on demand)
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
@@ -601,16 +604,16 @@ int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64
 
 template <int BITS>
 int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t blocks_x, const uint32_t* bin_start,
-                    uint64_t* lookback, uint32_t* ticket) {
+                    uint64_t* lookback, uint32_t* ticket, uint32_t grid, const uint32_t* only_if) {
   auto kern = bin_emit_kernel<BITS>;
   static bool configured = false;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BinEmitSmem<BITS>)));
     configured = true;
   }
-  kern<<<(Mb + BF_TILE - 1) / BF_TILE, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
+  kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
       s->n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
-      blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket);
+      blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if);
   return PVG_OK;
 }
 
@@ -643,11 +646,28 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
     const size_t tiles = (size_t)P.tiles_x * P.tiles_y;
     TRY(s->unf.reserve(kUnfHead + tiles * 8, st));
     TRY(s->lazy_state.reserve((size_t)5 * P.width * P.height * 4, st));
-    CU(cudaMemsetAsync(s->unf.p, 0, kUnfHead, zs));   // masks and count; lim and the list are written before they are read
+    CU(cudaMemsetAsync(s->unf.p, 0, kUnfHead + tiles * 4, zs));   // masks, count and lim; the list is written before it is read
   }
   CU(cudaMemsetAsync(s->sort_m.lookback.p, 0, (size_t)pass_tiles * OS_RADIX * 8, zs));
   return PVG_OK;
 }
+
+#if PVG_BIN_FUSED
+// bin_emit over the next `grid` tiles of 4096 entries (the ticket goes on counting across launches)
+int run_bin_emit(pvg_scene* s, const FrameParams& P, const uint32_t* visit, uint32_t grid, const uint32_t* only_if) {
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  uint32_t* bin_start = s->bin_tables.as<uint32_t>();
+  uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
+  int rc = PVG_ERR_BAD_OPTION;
+  switch (std::max(1, ceil_log2(nbins))) {
+#define PVG_CASE(B) case B: rc = launch_bin_emit<B>(s, (uint32_t)s->Mb, visit, blocks_x, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket, grid, only_if); break;
+    PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
+#undef PVG_CASE
+    default: break;
+  }
+  return rc;
+}
+#endif
 
 // bin_write over the chunks kin_lo <= kin < kin_hi of every block; only_unfinished: the tiles the first blend
 // phase marked. ticket_slot: which zeroed ticket of sort_m.tickets this launch consumes.
@@ -663,7 +683,9 @@ int launch_bin_write(pvg_scene* s, const FrameParams& P, uint32_t kin_lo, uint32
       (uint32_t)P.tiles_y, blocks_x, s->chunk_cnt.as<uint64_t>(), s->sort_m.tickets.as<uint32_t>() + ticket_slot,
       s->vals[0].as<uint32_t>(), kin_lo, kin_hi, only_unfinished ? s->unf.as<unsigned long long>() : nullptr,
       reinterpret_cast<const uint32_t*>(s->unf.as<unsigned char>() + 2048),
-      (kin_lo == 0 && kin_hi < (1u << 30)) ? reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) : nullptr);
+      (kin_lo == 0 && kin_hi < (1u << 30)) ? reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) : nullptr,
+      (s->lazy_used && s->emit_first && s->emit_first < s->emit_tiles)
+          ? s->sort_m.lookback.as<uint64_t>() + (size_t)(s->emit_first - 1) * s->emit_radix : nullptr);
   return PVG_OK;
 }
 
@@ -679,14 +701,16 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   int rc = PVG_ERR_BAD_OPTION;
   const int bits = std::max(1, ceil_log2(nbins));
 #if PVG_BIN_FUSED
+  // lazy lists: only the first slab of the entries (in depth order) is formed now; render_impl emits the rest if
+  // the first blend phase parks a tile
+  s->lazy_used = s->lazy_chunks > 0;
+  const uint32_t emit_tiles = (Mb + BF_TILE - 1) / BF_TILE;
+  s->emit_first = s->lazy_used ? std::min(emit_tiles, std::max(1u, (emit_tiles + (uint32_t)s->lazy_slab - 1) / (uint32_t)s->lazy_slab)) : emit_tiles;
+  s->emit_tiles = emit_tiles;
+  s->emit_radix = 1u << bits;
   TRY(tm->begin("bin_emit", PVG_STAGE_SORT, st));
-  switch (bits) {
-#define PVG_CASE(B) case B: rc = launch_bin_emit<B>(s, Mb, visit, blocks_x, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket); break;
-    PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
-#undef PVG_CASE
-    default: break;
-  }
-  TRY(rc);
+  TRY(run_bin_emit(s, P, visit, s->emit_first, nullptr));
+  rc = PVG_OK;
   TRY(tm->end(st));
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
@@ -709,8 +733,12 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 
   // the tile lists: all of them, or (lazy) only as far as the first lazy_chunks chunks of every block reach --
   // render_impl runs the second round after the first blend phase
+#if !PVG_BIN_FUSED
   s->lazy_used = s->lazy_chunks > 0;
+  s->emit_first = s->emit_tiles = 0;
+#endif
   s->lists_complete = !s->lazy_used;
+  s->visit_last = visit;
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
   TRY(launch_bin_write(s, P, 0u, s->lazy_used ? (uint32_t)s->lazy_chunks : 0xFFFFFFFFu, false, 1));
   TRY(tm->end(st));
@@ -959,6 +987,13 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       // phase 1 on the list prefixes; the tiles it could not finish get the rest of their lists, then phase 2
       PVG_BLEND_ALL(1)
       TRY(tm.end(st));
+#if PVG_BIN_FUSED
+      if (s->emit_first < s->emit_tiles) {
+        TRY(tm.begin("bin_emit", PVG_STAGE_SORT, st));
+        TRY(run_bin_emit(s, P, s->visit_last, s->emit_tiles - s->emit_first, Z.unf_count));
+        TRY(tm.end(st));
+      }
+#endif
       TRY(tm.begin("bin_write", PVG_STAGE_SORT, st));
       TRY(launch_bin_write(s, P, (uint32_t)s->lazy_chunks, 0xFFFFFFFFu, true, 2));
       TRY(tm.end(st));
@@ -1039,7 +1074,7 @@ int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
   s->stream = scene->stream;
   s->presort = scene->presort; s->keep_unsorted = scene->keep_unsorted; s->count_pairs = scene->count_pairs;
   s->compact = scene->compact; s->block = scene->block; s->blend_cull = scene->blend_cull;
-  s->lazy_chunks = scene->lazy_chunks;
+  s->lazy_chunks = scene->lazy_chunks; s->lazy_slab = scene->lazy_slab;
   s->model = scene->model;
   s->model->refs.fetch_add(1);
   // the model was written on the parent's stream at creation, which synchronised: nothing to wait for
@@ -1099,6 +1134,10 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
     case PVG_OPT_LAZY_CHUNKS:
       if (value < 0 || value > (1 << 20)) return PVG_ERR_BAD_OPTION;
       scene->lazy_chunks = (int)value;
+      return PVG_OK;
+    case PVG_OPT_LAZY_SLAB:
+      if (value < 1 || value > 4096) return PVG_ERR_BAD_OPTION;
+      scene->lazy_slab = (int)value;
       return PVG_OK;
     case PVG_OPT_TILE_ROW_BEGIN:
       if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
@@ -1199,6 +1238,16 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->offsets = s->offsets.as<uint32_t>();
   if (s->block_used && s->lazy_used && !s->lists_complete && s->M) {
     // lazy lists: write what the frame never needed, so that vals_sorted is every tile's whole list
+#if PVG_BIN_FUSED
+    if (s->emit_first < s->emit_tiles) {
+      // the entries behind the first slab, unless the frame's second round has formed them already (then the
+      // ticket stands at emit_tiles; forming them twice would be harmless but the ticket must not run on)
+      uint32_t tk = 0;
+      CU(cudaMemcpyAsync(&tk, s->sort_m.tickets.as<uint32_t>(), 4, cudaMemcpyDeviceToHost, s->stream));
+      CU(cudaStreamSynchronize(s->stream));
+      if (tk < s->emit_tiles) TRY(run_bin_emit(s, s->last_P, s->visit_last, s->emit_tiles - tk, nullptr));
+    }
+#endif
     CU(cudaMemsetAsync(s->sort_m.tickets.as<uint32_t>() + 3, 0, 4, s->stream));
     TRY(launch_bin_write(s, s->last_P, (uint32_t)s->lazy_chunks, 0xFFFFFFFFu, false, 3));
     CU(cudaGetLastError());
