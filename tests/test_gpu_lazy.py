@@ -22,8 +22,9 @@ def _scene(wl, opacity_scale=1.0, scale_scale=1.0):
                      s.sh, s.tau, s.beta, s.vel, s.cycle, s.sh_degree)
 
 
-def _render(sc, k, cam, t, **kw):
+def _render(sc, k, cam, t, slab=8, **kw):
     sc.set_option(pvg.OPT_LAZY_CHUNKS, k)
+    sc.set_option(pvg.OPT_LAZY_SLAB, slab)
     sc.set_option(pvg.OPT_COUNT_PAIRS, 1)
     out = [x.clone() for x in sc.render(cam, t, **kw)]
     torch.cuda.synchronize()
@@ -45,7 +46,7 @@ def test_lazy_lists_give_bit_identical_images(cfg, n, cam_i, op, sc_scale):
         full, ctr_full, _ = _render(sc, 0, cam, t)
         parked = []
         for k in (1, 2, 5):
-            lazy, ctr, p = _render(sc, k, cam, t)
+            lazy, ctr, p = _render(sc, k, cam, t, slab=1)      # every entry formed up front
             parked.append(p)
             for a, b in zip(full, lazy):
                 assert torch.equal(a, b), f"k={k}"
@@ -54,6 +55,13 @@ def test_lazy_lists_give_bit_identical_images(cfg, n, cam_i, op, sc_scale):
         if op < 0.05:
             assert parked[0] > 0
         assert parked[0] >= parked[1] >= parked[2]
+        # lazy emission: only the first 1/slab of the entries exists in the first round
+        for k, slab in ((2, 8), (1, 64), (5, 3), (2, 4096)):
+            lazy, ctr, p = _render(sc, k, cam, t, slab=slab)
+            for a, b in zip(full, lazy):
+                assert torch.equal(a, b), f"k={k} slab={slab}"
+            assert ctr == ctr_full
+            print(f"k={k} slab={slab}: parked {p}")
     finally:
         sc.close()
 
@@ -71,7 +79,7 @@ def test_lazy_lists_park_some_tiles_and_the_lists_complete_on_demand():
     try:
         full, _, _ = _render(sc, 0, cam, t)
         dbg_full = sc.debug(["vals_sorted", "ranges"])
-        lazy, _, parked = _render(sc, 1, cam, t)
+        lazy, _, parked = _render(sc, 1, cam, t, slab=1)
         tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
         assert 0 < parked < tiles, parked
         for a, b in zip(full, lazy):
@@ -79,6 +87,12 @@ def test_lazy_lists_park_some_tiles_and_the_lists_complete_on_demand():
         dbg = sc.debug(["vals_sorted", "ranges"])
         assert np.array_equal(dbg["ranges"], dbg_full["ranges"])
         assert np.array_equal(dbg["vals_sorted"], dbg_full["vals_sorted"])
+        # the same with lazy emission, whether or not the frame itself had to form the remaining entries
+        for slab in (16, 4096):
+            lazy, _, _ = _render(sc, 1, cam, t, slab=slab)
+            for a, b in zip(full, lazy):
+                assert torch.equal(a, b)
+            assert np.array_equal(sc.debug(["vals_sorted"])["vals_sorted"], dbg_full["vals_sorted"])
     finally:
         sc.close()
 
