@@ -36,8 +36,15 @@ namespace pvg {
 //   counts[i]   = rect count (0 if culled)
 //   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | fp32 bits of z, or 0xFFFFFFFF if culled), i
 // Returns the low half of the depth-sort key: the fp32 bits of z, 0xFFFFFFFF if culled.
+// PART: PRE_ALL -- everything. PRE_GEO -- what the list building needs (tile info, counts, depth pair) without the
+// record: the 192 B of SH coefficients are not read (lazy lists: most Gaussians are never composited). Whether a
+// Gaussian survives depends on its colour only through the non-finite-colour cull, which needs non-finite or
+// astronomically large coefficients: relayout_kernel flags those Gaussians (shflag) and only they evaluate their
+// colour here. PRE_REC -- recompute the same values and write the record only (shade_kernel).
+enum { PRE_ALL = 0, PRE_GEO = 1, PRE_REC = 2 };
+template <int PART>
 __device__ __forceinline__ uint32_t
-preprocess_point(const FrameParams& P, uint32_t n, uint32_t i,
+preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __restrict__ shflag,
                  const float4* __restrict__ A0, const float4* __restrict__ A1,
                  const float4* __restrict__ A2, const float4* __restrict__ A3,
                  const float4* __restrict__ SH, float4* __restrict__ record,
@@ -144,13 +151,13 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i,
     const float vx = e * a1.x, vy = e * a1.y, vz = e * a1.z;
     r2 = make_float4(fmaf(P.R[0], vx, fmaf(P.R[1], vy, P.R[2] * vz)), fmaf(P.R[3], vx, fmaf(P.R[4], vy, P.R[5] * vz)),
                      fmaf(P.R[6], vx, fmaf(P.R[7], vy, P.R[8] * vz)), hy);
-    featw[i] = fminf(fmaxf(rho, 0.f), 2.0f);
+    if (PART != PRE_GEO) featw[i] = fminf(fmaxf(rho, 0.f), 2.0f);
     if (!((fabsf(r2.x) <= 3.0e38f) && (fabsf(r2.y) <= 3.0e38f) && (fabsf(r2.z) <= 3.0e38f))) {
       valid = false;
       r0 = make_float4(0.f, 0.f, 0.f, 0.f); r1 = r0; r2 = r0;
       ti = make_uint4(0u, 0u, 0u, 0u);
     }
-  } else if (valid) {
+  } else if (valid && (PART != PRE_GEO || shflag[i])) {
     // P11: SH colour; only survivors touch the 192 B of coefficients
     float dx = wx - P.campos[0], dy = wy - P.campos[1], dz = wz - P.campos[2];
     const float inv = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
@@ -194,9 +201,12 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i,
     }
   }
 
-  record[3 * (size_t)i] = r0;
-  record[3 * (size_t)i + 1] = r1;
-  record[3 * (size_t)i + 2] = r2;
+  if (PART != PRE_GEO) {
+    record[3 * (size_t)i] = r0;
+    record[3 * (size_t)i + 1] = r1;
+    record[3 * (size_t)i + 2] = r2;
+  }
+  if (PART == PRE_REC) return valid ? ti.z : 0xFFFFFFFFu;
   tileinfo[i] = ti;
   counts[i] = ti.w;
   if (dkeys) {
@@ -221,8 +231,9 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i,
 #define PVG_PRE_CHUNKS 4
 #endif
 constexpr int PRE_CHUNKS = PVG_PRE_CHUNKS;
+template <int PART>
 __global__ void __launch_bounds__(256)
-preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
+preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8_t* __restrict__ shflag,
                   const float4* __restrict__ A0, const float4* __restrict__ A1,
                   const float4* __restrict__ A2, const float4* __restrict__ A3,
                   const float4* __restrict__ SH, float4* __restrict__ record,
@@ -239,7 +250,7 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
   for (int c = 0; c < PRE_CHUNKS; ++c) {
     const uint32_t i = (blockIdx.x * PRE_CHUNKS + c) * 256u + threadIdx.x;
     if (i >= n) break;
-    const uint32_t z = preprocess_point(P, n, i, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
+    const uint32_t z = preprocess_point<PART>(P, n, i, shflag, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
     if (dhist) {
 #pragma unroll
       for (int k = 0; k < 4; ++k) atomicAdd(&s_hist[k * 256 + ((z >> (8 * k)) & 0xFFu)], 1u);
@@ -278,6 +289,29 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n,
   }
 }
 
+// The records PRE_GEO left out, for the Gaussians at depth ranks [*r_lo (or 0), *r_hi + 1 (or n)) of the sorted
+// order: the same arithmetic as preprocess_kernel<PRE_ALL>, so the records are bit-identical to an eager frame.
+// only_if: nothing to do when *only_if == 0 (lazy lists: the second round runs only if a tile was parked).
+__global__ void __launch_bounds__(256)
+shade_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit,
+             const uint32_t* __restrict__ r_lo, const uint32_t* __restrict__ r_hi, const uint32_t* __restrict__ only_if,
+             const float4* __restrict__ A0, const float4* __restrict__ A1, const float4* __restrict__ A2,
+             const float4* __restrict__ A3, const float4* __restrict__ SH, float4* __restrict__ record, float* __restrict__ featw,
+             int zero_culled /* pvg_debug_view: the culled Gaussians' records read as zero */) {
+  if (only_if && *only_if == 0u) return;
+  const uint32_t lo = r_lo ? *r_lo + 1u : 0u, hi = r_hi ? min(*r_hi + 1u, n) : n;
+  const uint32_t r = lo + blockIdx.x * 256u + threadIdx.x;
+  if (r >= hi) return;
+  if ((uint32_t)keys[r] == 0xFFFFFFFFu) {   // culled (they sort last): nobody composites them
+    if (zero_culled) {
+      const size_t g = visit[r];
+      record[3 * g] = record[3 * g + 1] = record[3 * g + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    return;
+  }
+  preprocess_point<PRE_REC>(P, n, visit[r], nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
+}
+
 // One-off re-layout of the caller's arrays into the SoA float4 model (pvg_create_scene).
 __global__ void __launch_bounds__(256)
 relayout_kernel(uint32_t n, const float* __restrict__ mu, const float* __restrict__ quat,
@@ -285,9 +319,14 @@ relayout_kernel(uint32_t n, const float* __restrict__ mu, const float* __restric
                 const float* __restrict__ sh, const float* __restrict__ tau,
                 const float* __restrict__ beta, const float* __restrict__ vel,
                 float4* __restrict__ A0, float4* __restrict__ A1, float4* __restrict__ A2,
-                float4* __restrict__ A3, float4* __restrict__ SH) {
+                float4* __restrict__ A3, float4* __restrict__ SH, uint8_t* __restrict__ shflag) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  // shflag: could the colour 0.5 + sum Y_k f_k be non-finite? |Y_k| < 3, so not while the coefficients are finite
+  // and their absolute sum stays below 1e37
+  float asum = 0.f;
+  for (int k = 0; k < 48; ++k) asum += fabsf(sh[48 * (size_t)i + k]);
+  shflag[i] = (asum < 1.0e37f) ? 0 : 1;   // NaN and inf fail the comparison
   A0[i] = make_float4(mu[3 * (size_t)i], mu[3 * (size_t)i + 1], mu[3 * (size_t)i + 2], tau[i]);
   A1[i] = make_float4(vel[3 * (size_t)i], vel[3 * (size_t)i + 1], vel[3 * (size_t)i + 2], beta[i]);
   const float qw = quat[4 * (size_t)i], qx = quat[4 * (size_t)i + 1], qy = quat[4 * (size_t)i + 2], qz = quat[4 * (size_t)i + 3];

@@ -336,7 +336,7 @@ int run_compact_sort(uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint3
 
 // The re-laid-out model (SoA, preprocess.cuh), shared by a scene and its forks (pvg_fork_scene).
 struct Model {
-  Buf A0, A1, A2, A3, SH;
+  Buf A0, A1, A2, A3, SH, shflag;
   std::atomic<int> refs{1};
 };
 
@@ -352,6 +352,9 @@ struct pvg_scene {
   int lazy_slab = 8;                  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front
   uint32_t emit_first = 0, emit_tiles = 0, emit_radix = 256;   // bin_emit tiles in the first launch / in all; its look-back row length
   const uint32_t* visit_last = nullptr;
+  bool light = false;                 // this frame's preprocess left the records to shade_kernel
+  bool records_complete = true;       // record[] holds every Gaussian's record (pvg_debug_view completes them on demand)
+  float* featw_last = nullptr;
   bool lazy_used = false;             // last frame wrote list prefixes + what the unfinished tiles needed
   bool lists_complete = true;         // vals[] holds every tile's whole list (pvg_debug_view completes them on demand)
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
@@ -401,7 +404,7 @@ int ceil_log2(uint32_t v) {
 
 void release_all(pvg_scene* s) {
   if (s->model && s->model->refs.fetch_sub(1) == 1) {
-    Buf* mb[] = {&s->model->A0, &s->model->A1, &s->model->A2, &s->model->A3, &s->model->SH};
+    Buf* mb[] = {&s->model->A0, &s->model->A1, &s->model->A2, &s->model->A3, &s->model->SH, &s->model->shflag};
     for (Buf* b : mb) b->release();
     delete s->model;
   }
@@ -462,12 +465,12 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
   s->model = new (std::nothrow) Model();
   if (!s->model) return PVG_ERR_OOM;
   Model* m = s->model;
-  rs(m->A0, n * 16); rs(m->A1, n * 16); rs(m->A2, n * 16); rs(m->A3, n * 16); rs(m->SH, n * 192);
+  rs(m->A0, n * 16); rs(m->A1, n * 16); rs(m->A2, n * 16); rs(m->A3, n * 16); rs(m->SH, n * 192); rs(m->shflag, n);
   if (rc == PVG_OK) {
     relayout_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
         (uint32_t)n, t_mu.as<float>(), t_quat.as<float>(), t_scale.as<float>(), t_op.as<float>(), t_sh.as<float>(),
         t_tau.as<float>(), t_beta.as<float>(), t_vel.as<float>(), m->A0.as<float4>(), m->A1.as<float4>(),
-        m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>());
+        m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(), m->shflag.as<uint8_t>());
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {
@@ -669,6 +672,16 @@ int run_bin_emit(pvg_scene* s, const FrameParams& P, const uint32_t* visit, uint
 }
 #endif
 
+// shade_kernel over the depth ranks (r_lo, r_hi] given by device words (nullptr: from the start / to the end)
+int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const uint32_t* r_hi, const uint32_t* only_if, int zero_culled) {
+  const Model* m = s->model;
+  shade_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(P, s->n, s->dkeys[s->visit_side].as<uint64_t>(), s->visit_last, r_lo, r_hi,
+                                                          only_if, m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(),
+                                                          m->A3.as<float4>(), m->SH.as<float4>(), s->record.as<float4>(),
+                                                          s->featw_last, zero_culled);
+  return PVG_OK;
+}
+
 // bin_write over the chunks kin_lo <= kin < kin_hi of every block; only_unfinished: the tiles the first blend
 // phase marked. ticket_slot: which zeroed ticket of sort_m.tickets this launch consumes.
 int launch_bin_write(pvg_scene* s, const FrameParams& P, uint32_t kin_lo, uint32_t kin_hi, bool only_unfinished, int ticket_slot) {
@@ -708,10 +721,17 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   s->emit_first = s->lazy_used ? std::min(emit_tiles, std::max(1u, (emit_tiles + (uint32_t)s->lazy_slab - 1) / (uint32_t)s->lazy_slab)) : emit_tiles;
   s->emit_tiles = emit_tiles;
   s->emit_radix = 1u << bits;
+  s->visit_last = visit;
   TRY(tm->begin("bin_emit", PVG_STAGE_SORT, st));
   TRY(run_bin_emit(s, P, visit, s->emit_first, nullptr));
   rc = PVG_OK;
   TRY(tm->end(st));
+  if (s->light) {
+    // the records of the Gaussians that own the first slab's entries: depth ranks 0 .. owner of the slab's end
+    TRY(tm->begin("shade", PVG_STAGE_PREPROCESS, st));
+    TRY(run_shade(s, P, nullptr, s->emit_first < s->emit_tiles ? s->chunk_owner.as<uint32_t>() + s->emit_first : nullptr, nullptr, 0));
+    TRY(tm->end(st));
+  }
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
@@ -794,11 +814,27 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     TRY(s->featw.reserve((size_t)n * 4, st));
     featw = s->featw.as<float>();
   }
+  s->featw_last = featw;
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
-  preprocess_kernel<<<(n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS), 256, 0, st>>>(P, n, s->model->A0.as<float4>(), s->model->A1.as<float4>(), s->model->A2.as<float4>(),
-                                                      s->model->A3.as<float4>(), s->model->SH.as<float4>(), s->record.as<float4>(),
-                                                      s->tileinfo.as<uint4>(), s->counts.as<uint32_t>(), dk, dv, featw,
-                                                      s->presort ? s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords : nullptr);
+  // lazy lists: the records (conic, colour: 48 B written, 192 B of SH read per survivor) are left to shade_kernel,
+  // which forms them for the Gaussians in front only -- unless a tile parks
+  s->light = block && s->lazy_chunks > 0 && PVG_BIN_FUSED;
+  s->records_complete = !s->light;
+  {
+    const unsigned pgrid = (n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS);
+    uint32_t* dh = s->presort ? s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords : nullptr;
+    const Model* m = s->model;
+    if (s->light)
+      preprocess_kernel<PRE_GEO><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
+                                                          m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
+                                                          s->record.as<float4>(), s->tileinfo.as<uint4>(),
+                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh);
+    else
+      preprocess_kernel<PRE_ALL><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
+                                                          m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
+                                                          s->record.as<float4>(), s->tileinfo.as<uint4>(),
+                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh);
+  }
   TRY(tm.end(st));
 
   const uint32_t* visit = nullptr;
@@ -880,6 +916,11 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
   s->M = M;
 
+  if (s->light && M == 0) {   // nothing survives: every record reads as zero
+    CU(cudaMemsetAsync(s->record.p, 0, (size_t)n * 48, st));
+    tm.cut();
+    s->records_complete = true;
+  }
   s->sorted_side = 0;
   const bool compact = !block && s->presort && s->compact && tile_bits <= 16;
   s->compact_used = compact;
@@ -992,6 +1033,11 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
         TRY(tm.begin("bin_emit", PVG_STAGE_SORT, st));
         TRY(run_bin_emit(s, P, s->visit_last, s->emit_tiles - s->emit_first, Z.unf_count));
         TRY(tm.end(st));
+        if (s->light) {
+          TRY(tm.begin("shade", PVG_STAGE_PREPROCESS, st));
+          TRY(run_shade(s, P, s->chunk_owner.as<uint32_t>() + s->emit_first, nullptr, Z.unf_count, 0));
+          TRY(tm.end(st));
+        }
       }
 #endif
       TRY(tm.begin("bin_write", PVG_STAGE_SORT, st));
@@ -1236,6 +1282,12 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->counts = s->counts.as<uint32_t>();
   out->visit_order = s->presort ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
+  if (s->block_used && s->light && !s->records_complete && s->M) {
+    // lazy lists: the records the frame never needed (and zeros for the culled Gaussians)
+    TRY(run_shade(s, s->last_P, nullptr, nullptr, nullptr, 1));
+    CU(cudaGetLastError());
+    s->records_complete = true;
+  }
   if (s->block_used && s->lazy_used && !s->lists_complete && s->M) {
     // lazy lists: write what the frame never needed, so that vals_sorted is every tile's whole list
 #if PVG_BIN_FUSED
