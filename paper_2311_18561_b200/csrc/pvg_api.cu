@@ -673,9 +673,10 @@ int run_bin_emit(pvg_scene* s, const FrameParams& P, const uint32_t* visit, uint
 #endif
 
 // shade_kernel over the depth ranks (r_lo, r_hi] given by device words (nullptr: from the start / to the end)
-int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const uint32_t* r_hi, const uint32_t* only_if, int zero_culled) {
+int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const uint32_t* r_hi, const uint32_t* only_if, int zero_culled,
+              cudaStream_t on = nullptr) {
   const Model* m = s->model;
-  shade_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(P, s->n, s->dkeys[s->visit_side].as<uint64_t>(), s->visit_last, r_lo, r_hi,
+  shade_kernel<<<(s->n + 255) / 256, 256, 0, on ? on : s->stream>>>(P, s->n, s->dkeys[s->visit_side].as<uint64_t>(), s->visit_last, r_lo, r_hi,
                                                           only_if, m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(),
                                                           m->A3.as<float4>(), m->SH.as<float4>(), s->record.as<float4>(),
                                                           s->featw_last, zero_culled);
@@ -722,16 +723,22 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   s->emit_tiles = emit_tiles;
   s->emit_radix = 1u << bits;
   s->visit_last = visit;
+  if (s->light) {
+    // the records of the Gaussians that own the first slab's entries (depth ranks 0 .. owner of the slab's end), on
+    // the side stream: a latency-bound gather that overlaps the equally latency-bound bin_emit and bin_write
+    cudaStream_t sd = s->side;
+    CU(cudaEventRecord(s->ev_fork, st));
+    CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
+    tm->cut();
+    TRY(tm->begin("shade", PVG_STAGE_PREPROCESS, sd));
+    TRY(run_shade(s, P, nullptr, s->emit_first < s->emit_tiles ? s->chunk_owner.as<uint32_t>() + s->emit_first : nullptr, nullptr, 0, sd));
+    TRY(tm->end(sd));
+    CU(cudaEventRecord(s->ev_join, sd));
+  }
   TRY(tm->begin("bin_emit", PVG_STAGE_SORT, st));
   TRY(run_bin_emit(s, P, visit, s->emit_first, nullptr));
   rc = PVG_OK;
   TRY(tm->end(st));
-  if (s->light) {
-    // the records of the Gaussians that own the first slab's entries: depth ranks 0 .. owner of the slab's end
-    TRY(tm->begin("shade", PVG_STAGE_PREPROCESS, st));
-    TRY(run_shade(s, P, nullptr, s->emit_first < s->emit_tiles ? s->chunk_owner.as<uint32_t>() + s->emit_first : nullptr, nullptr, 0));
-    TRY(tm->end(st));
-  }
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
@@ -762,6 +769,10 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
   TRY(launch_bin_write(s, P, 0u, s->lazy_used ? (uint32_t)s->lazy_chunks : 0xFFFFFFFFu, false, 1));
   TRY(tm->end(st));
+  if (s->light) {   // the blend reads the records
+    CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+    tm->cut();
+  }
   CU(cudaGetLastError());
   s->sorted_side = 0;
   return PVG_OK;
