@@ -412,6 +412,8 @@ def run_ours(args):
            ("tile_prefix", "ranges"): 0.0}
     lazy = list_mode == "blocks" and args.lazy_chunks != 0
     if lazy:
+        # deferred records: preprocess reads the 64 B model + 1 B flag and writes tile info, count and depth pair (32 B)
+        alg[("preprocess", "preprocess")] = K * 97.0 * N
         # lazy lists: bin_emit forms the first 1/8 of the entries and bin_write the first chunks of every block -- what
         # they move depends on where the tiles saturate, so no algorithmic-byte figure is claimed for them
         alg.pop(("bin_emit", "sort"), None)
