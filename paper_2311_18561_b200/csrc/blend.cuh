@@ -226,10 +226,10 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
   // saturates, so a fixed 256-entry first batch gathers mostly records that are never used
   uint32_t bs = BLEND_BATCH_FIRST;
-  bool all_dead = false;   // block-uniform: the loop ended because every pixel of the tile had stopped
-  for (uint32_t base = range.x; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
+  uint32_t base = range.x;   // after the loop: base < range.y iff it ended because every pixel of the tile had stopped
+  for (; base < range.y; base += bs, bs = min(2u * bs, (uint32_t)BLEND_BATCH)) {
     // all pixels of the tile saturated? (also fences the previous batch's smem reads)
-    if (__syncthreads_count(any_alive()) == 0) { all_dead = true; break; }
+    if (__syncthreads_count(any_alive()) == 0) break;
     // Staging. Warp w gathers the w-th segment of the batch and keeps, in order, only the entries whose
     // ellipse { alpha >= 1/255 } can reach the tile at all: the lists are built from axis-aligned
     // rectangles (S7), and 26% (config 3) to 48% (config 4) of the entries a tile consumes cover it with
@@ -306,7 +306,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   }
   const size_t HW = (size_t)P.width * P.height;
   const size_t pi = (size_t)py * P.width + px;
-  if (PHASE == 1 && !all_dead && range.y < list_end) {
+  if (PHASE == 1 && base >= range.y && range.y < list_end) {
     // the written prefix is used up without the tile being known dead: park it if a pixel is still alive
     // (block-uniform decision; rare -- a saturating tile leaves the loop through the check at its top)
     if (__syncthreads_or(any_alive())) {
@@ -318,14 +318,14 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
       }
       uint32_t inmask = 0;
 #pragma unroll
-      for (int k = 0; k < BLEND_NPX; ++k) inmask |= in[k] ? 1u << k : 0u;
+      for (int k = 0; k < BLEND_NPX; ++k) inmask |= (px + k < (uint32_t)P.width && py < (uint32_t)P.height) ? 1u << k : 0u;
       blend_park(Z, tile, (ty >> 3) * Z.blocks_x + (tx >> 3), (ty & 7u) * 8u + (tx & 7u), HW, pi, inmask, st);
       return;
     }
   }
 #pragma unroll
   for (int k = 0; k < BLEND_NPX; ++k) {
-    if (!in[k]) continue;
+    if (!(px + k < (uint32_t)P.width && py < (uint32_t)P.height)) continue;   // recomputed: not kept live through the loop
     const float Al = 1.0f - X[k].T;
     if (out_rgb) {
       float bg[3] = {P.bg[0], P.bg[1], P.bg[2]};
