@@ -97,8 +97,8 @@ struct KernelRec {
 #endif
 struct OsLarge { static constexpr int THREADS = PVG_OSL_THREADS, ITEMS = PVG_OSL_ITEMS, MINB = PVG_OSL_MINB; static constexpr bool STREAM = true; };
 #ifndef PVG_OSS_THREADS
-#define PVG_OSS_THREADS 384
-#define PVG_OSS_ITEMS 8
+#define PVG_OSS_THREADS 256   // cfg 3 depth passes: 256 x 16 0.141 ms, 384 x 8 0.149, 256 x 24 0.146, 512 x 8 0.154, 256 x 8 (3 CTAs/SM) 0.158
+#define PVG_OSS_ITEMS 16
 #define PVG_OSS_MINB 2
 #endif
 struct OsSmall { static constexpr int THREADS = PVG_OSS_THREADS, ITEMS = PVG_OSS_ITEMS, MINB = PVG_OSS_MINB; static constexpr bool STREAM = false; };
@@ -709,11 +709,12 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   cudaStream_t st = s->stream;
   const uint32_t Mb = (uint32_t)s->Mb;
   const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  const int bits = std::max(1, ceil_log2(nbins));
+#if !PVG_BIN_FUSED
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
   uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
-
   int rc = PVG_ERR_BAD_OPTION;
-  const int bits = std::max(1, ceil_log2(nbins));
+#endif
 #if PVG_BIN_FUSED
   // lazy lists: only the first slab of the entries (in depth order) is formed now; render_impl emits the rest if
   // the first blend phase parks a tile
@@ -737,7 +738,6 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   }
   TRY(tm->begin("bin_emit", PVG_STAGE_SORT, st));
   TRY(run_bin_emit(s, P, visit, s->emit_first, nullptr));
-  rc = PVG_OK;
   TRY(tm->end(st));
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
