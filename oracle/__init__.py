@@ -148,15 +148,22 @@ def tile_list(rec, width, height, tile):
 
 
 def render(rec, width, height, bg=(0.0, 0.0, 0.0), mode="binned", tiles: Optional[Sequence[int]] = None,
-           tie_budget: bool = False):
+           tie_budget: bool = False, slack=None):
     """Oracle-R on an fp32 record. mode 'brute' or 'binned'. Returns dict of float64
-    images: rgb [3,H,W], depth, alpha, budget, cond [H,W], plus visited / contributed."""
+    images: rgb [3,H,W], depth, alpha, budget, cond, derived [H,W], plus visited / contributed.
+    slack [n,6] (end-to-end comparison only): how far another fp32 record of the same scene may lie from `rec`,
+    per Gaussian (d mx, d my, d conic, d ln o~, d colour, d z in ulps); `derived` is the per-pixel allowance it
+    propagates to, and the fragile windows (alpha cutoff, T stop, depth ties) widen by the same uncertainty."""
     rec = np.ascontiguousarray(rec, dtype=np.float32)
     n = rec.shape[0]
     assert rec.shape == (n, 12)
     H, W = int(height), int(width)
     rgb = np.empty((3, H, W)); depth = np.empty((H, W)); alpha = np.empty((H, W))
-    budget = np.empty((H, W)); cond = np.empty((H, W))
+    budget = np.empty((H, W)); cond = np.empty((H, W)); derived = np.zeros((H, W))
+    sl = None
+    if slack is not None:
+        sl = np.ascontiguousarray(slack, dtype=np.float64)
+        assert sl.shape == (n, 6), sl.shape
     stats = np.zeros(2, dtype=np.uint64)
     bg = np.ascontiguousarray(bg, dtype=np.float64)
     tl, ntl = None, 0
@@ -166,11 +173,11 @@ def render(rec, width, height, bg=(0.0, 0.0, 0.0), mode="binned", tiles: Optiona
     lib().oracle_render(C.c_uint64(n), _p(rec), C.c_int(W), C.c_int(H), _p(bg),
                         C.c_int({"brute": 0, "binned": 1}[mode]), tl, C.c_uint64(ntl),
                         C.c_int(1 if tie_budget else 0), _p(rgb), _p(depth), _p(alpha), _p(budget),
-                        _p(cond), _p(stats))
+                        _p(cond), _p(stats), _p(sl) if sl is not None else None, _p(derived))
     # c_max: the colour scale of budget and cond (largest colour of a non-culled Gaussian or of the background)
     live = rec[:, 3] > 0
     c_max = float(max(rec[live, 8:11].max(initial=0.0), float(np.max(bg))))
-    return dict(rgb=rgb, depth=depth, alpha=alpha, budget=budget, cond=cond,
+    return dict(rgb=rgb, depth=depth, alpha=alpha, budget=budget, cond=cond, derived=derived,
                 visited=int(stats[0]), contributed=int(stats[1]), c_max=c_max)
 
 

@@ -143,19 +143,36 @@ std::vector<uint32_t> depth_order(uint64_t n, const float* rec) {
 }
 
 struct PixelOut {
-  double rgb[3], depth, alpha, budget, cond;
+  double rgb[3], depth, alpha, budget, cond, derived;
   uint64_t visited, contributed;
 };
+
+// End-to-end comparison: the image of ANOTHER fp32 record of the same scene (the CUDA
+// path's own a1 output) is compared with the image of this record. Per Gaussian the caller states how far that
+// other record may lie from this one -- slack[g] = { d mx, d my [px], d conic [absolute, each of a, b, c],
+// d ln o~ [relative], d colour [absolute], d z [fp32 ulps] } -- and composite_pixel turns the statement into a per-pixel allowance
+// by first-order propagation through Eq. 3:
+//   d w      = |dw/dmx| d mx + |dw/dmy| d my + (dx^2/2 + dy^2/2 + |dx dy|) d conic + d ln o~     (w = ln alpha)
+//   |dC/d alpha_i| <= T_i c_max   (C = sum_j T_j alpha_j c_j: the two terms of the derivative, T_i c_i and
+//                                  -sum_{j>i} T_j alpha_j c_j / (1 - alpha_i), are each within [0, T_i c_max])
+//   derived  = sum_i T_i alpha_i (c_max expm1(d w_i) + d colour_i)
+// and widens the two fragile windows by the same uncertainty (alpha by d w, T' by the accumulated one). Depth order:
+// two consecutive contributors may swap in the other record only if their z bit patterns are closer than the sum of
+// their d z (equal bits with d z = 0 on both keep their index order on both sides); without slack the tie window is
+// the flat 4 ulps of SURVEY.md 8(c).
+constexpr int kSlack = 6;
 
 // Oracle-R for one pixel over an ordered candidate list (Eq. 3, PAPER.md:L72;
 // alpha PAPER.md:L79; depth / opacity targets PAPER.md:L87, L168; S9, S10, S12,
 // S13, S16'). `budget` is the fragile-point allowance of DESIGN.md; `cond` is the
 // fp32 conditioning allowance of the quadratic form.
 PixelOut composite_pixel(const float* rec, const uint32_t* cand, size_t ncand, double px,
-                         double py, const double bg[3], double c_max, bool tie_budget) {
+                         double py, const double bg[3], double c_max, bool tie_budget,
+                         const double* slack = nullptr) {
   PixelOut o{};
   double T = 1.0, C[3] = {0, 0, 0}, D = 0.0;
-  double prev_alpha = 0.0;
+  double relT = 0.0;   // accumulated relative uncertainty of T (end-to-end only)
+  double prev_alpha = 0.0, prev_dz = 0.0;
   uint32_t prev_zbits = 0;
   bool have_prev = false;
   for (size_t k = 0; k < ncand; ++k) {
@@ -166,18 +183,32 @@ PixelOut composite_pixel(const float* rec, const uint32_t* cand, size_t ncand, d
     double w = -0.5 * (a * dx * dx + c * dy * dy) - b * dx * dy;
     if (w > 0.0) w = 0.0;  // S16': rounding guard, continuous (exact w <= 0)
     const double alpha = std::fmin(kAlphaMax, (double)r[3] * std::exp(w));
-    if (std::fabs(255.0 * alpha - 1.0) < 1e-4) o.budget += alpha * T * c_max;
+    double dw = 0.0, dcol = 0.0, dz = 0.0;
+    if (slack) {
+      const double* sl = slack + (uint64_t)cand[k] * kSlack;
+      dw = std::fabs(a * dx + b * dy) * sl[0] + std::fabs(c * dy + b * dx) * sl[1] +
+           (0.5 * dx * dx + 0.5 * dy * dy + std::fabs(dx * dy)) * sl[2] + sl[3];
+      dcol = sl[4];
+      dz = sl[5];
+    }
+    if (std::fabs(255.0 * alpha - 1.0) < 1e-4 + dw) o.budget += alpha * T * c_max;
     if (alpha < kAlphaMin) continue;
     const double Tn = T * (1.0 - alpha);
-    if (std::fabs(Tn / kTStop - 1.0) < 1e-4) o.budget += T * c_max;
+    const double dTn = relT + alpha * dw / (1.0 - alpha);   // relative uncertainty of T'
+    if (std::fabs(Tn / kTStop - 1.0) < 1e-4 + dTn) o.budget += T * c_max;
     if (Tn < kTStop) break;  // S10: the Gaussian that would cross the stop is NOT composited
     const double wgt = alpha * T;
+    o.derived += wgt * (c_max * std::expm1(dw) + dcol);
+    relT = dTn;
     // fp32 evaluation of the quadratic form loses ~2^-22 of the sum of magnitudes
     o.cond += wgt * c_max * 2.384185791015625e-07 *
               (0.5 * (std::fabs(a) * dx * dx + std::fabs(c) * dy * dy) + std::fabs(b * dx * dy));
     if (tie_budget && have_prev) {
       const uint32_t zb = f32_bits(r[2]);
-      if (zb - prev_zbits <= 4u) o.budget += prev_alpha * alpha * T * c_max;
+      const bool tie = slack ? (dz + prev_dz > 0.0 && (double)(zb - prev_zbits) <= dz + prev_dz) : (zb - prev_zbits <= 4u);
+      // swapping two adjacent layers changes C by alpha_i alpha_j T_before (c_j - c_i), T_before = the
+      // transmittance in front of BOTH = T / (1 - alpha_i)
+      if (tie) o.budget += prev_alpha * alpha * (T / (1.0 - prev_alpha)) * c_max;
     }
     C[0] += (double)r[8] * wgt;
     C[1] += (double)r[9] * wgt;
@@ -187,6 +218,7 @@ PixelOut composite_pixel(const float* rec, const uint32_t* cand, size_t ncand, d
     ++o.contributed;
     prev_alpha = alpha;
     prev_zbits = f32_bits(r[2]);
+    prev_dz = dz;
     have_prev = true;
   }
   o.alpha = 1.0 - T;
@@ -464,11 +496,12 @@ uint64_t oracle_tile_list(uint64_t n, const float* rec, int width, int height, u
 // depth order); mode 1 = binned (a pixel visits only the Gaussians whose P10
 // rectangle contains its tile, same order). tiles == nullptr renders the whole
 // image, else only the listed tile ids (other pixels stay 0).
-// Outputs are double: rgb [3][H][W], depth/alpha/budget/cond [H][W].
+// Outputs are double: rgb [3][H][W], depth/alpha/budget/cond/derived [H][W].
 // stats[0] = visited pairs, stats[1] = contributing pairs.
 void oracle_render(uint64_t n, const float* rec, int width, int height, const double* bg, int mode,
                    const uint32_t* tiles, uint64_t ntiles_sel, int tie_budget, double* rgb,
-                   double* depth, double* alpha, double* budget, double* cond, uint64_t* stats) {
+                   double* depth, double* alpha, double* budget, double* cond, uint64_t* stats,
+                   const double* slack /* [n][6] or nullptr: see kSlack */, double* derived /* [H][W] or nullptr */) {
   const int TX = (width + kTile - 1) / kTile, TY = (height + kTile - 1) / kTile;
   const uint64_t HW = (uint64_t)width * height;
   std::fill(rgb, rgb + 3 * HW, 0.0);
@@ -476,6 +509,7 @@ void oracle_render(uint64_t n, const float* rec, int width, int height, const do
   std::fill(alpha, alpha + HW, 0.0);
   if (budget) std::fill(budget, budget + HW, 0.0);
   if (cond) std::fill(cond, cond + HW, 0.0);
+  if (derived) std::fill(derived, derived + HW, 0.0);
   const std::vector<uint32_t> order = depth_order(n, rec);
   double c_max = 0.0;
   for (uint32_t g : order)
@@ -515,13 +549,14 @@ void oracle_render(uint64_t n, const float* rec, int width, int height, const do
     for (int py = ty * kTile; py < std::min((ty + 1) * kTile, height); ++py)
       for (int px = tx * kTile; px < std::min((tx + 1) * kTile, width); ++px) {
         // S14: pixel centres at half-integers
-        const PixelOut o = composite_pixel(rec, cand, ncand, px + 0.5, py + 0.5, bg, c_max, tie_budget != 0);
+        const PixelOut o = composite_pixel(rec, cand, ncand, px + 0.5, py + 0.5, bg, c_max, tie_budget != 0, slack);
         const uint64_t pi = (uint64_t)py * width + px;
         for (int ch = 0; ch < 3; ++ch) rgb[ch * HW + pi] = o.rgb[ch];
         depth[pi] = o.depth;
         alpha[pi] = o.alpha;
         if (budget) budget[pi] = o.budget;
         if (cond) cond[pi] = o.cond;
+        if (derived) derived[pi] = o.derived;
         visited += o.visited;
         contributed += o.contributed;
       }

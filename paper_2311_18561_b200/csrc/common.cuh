@@ -13,27 +13,33 @@
 #define PVG_ALPHA_MAX 0.99f
 #define PVG_T_STOP 1e-4f
 #define PVG_DILATE 0.3f
+#define PVG_DILATE_D 0.3 /* the same reading (S6) for the double-precision conic: 0.3 px^2, not fp32(0.3) */
 #define PVG_ZNEAR_DEFAULT 0.2f
 
 namespace pvg {
 
 // Per-frame constants, passed by value as a __grid_constant__ kernel parameter.
 struct FrameParams {
+  // The position chain mu~(t) -> p_cam -> (mx, my) runs in double (preprocess.cuh): the time the state is evaluated
+  // at (t - dts, exact) and the two constants of Eq. 6, computed by the host in double.
+  double t1;          // t - dts
+  double two_over_l;  // 2 / l: sin(2 pi dt / l) = sinpi(two_over_l * dt)   (0 for the linear model)
+  double l_over_2pi;  // l / (2 pi)
+  double inv_l_d;     // 1 / l (0 for the linear model), for the flow translation of Eq. 12
+  double Rd[9], Td[3], fxd, fyd, cxd, cyd;   // the camera once more, as doubles (exact copies of the fp32 fields below)
+  double limxd, limyd;                       // 1.3 * half-FoV tangents, unrounded
   float R[9];       // world->camera rotation, row-major
   float T[3];       // world->camera translation
   float campos[3];  // camera centre in world coordinates (-R^T T)
   float fx, fy, cx, cy;
   float limx, limy;  // 1.3 * half-FoV tangents (Jacobian guard)
   float znear;
-  float t;            // time at which Eq. 6 / Eq. 7 are evaluated (t - dts for the temporal-smoothing state)
   float dts;          // Eq. 12 flow translation interval (0: the plain state H(t))
   float inv_l;        // 1 / l (0 for the linear model): rho = beta / l
   float rho_min, rho_max;  // staticness filter (only when `filter` is set)
   int filter;
   int cull;           // blend: drop list entries whose ellipse cannot reach the tile (bit-identical images)
   int target;         // 0: colour (SH) + depth; 1: dynamics -- colour := vbar in camera axes, 4th channel := clamp(rho, 0, 2)
-  float two_over_l;   // 2 / l           (sinpi argument scale)
-  float l_over_2pi;   // l / (2 pi)
   int linear;         // l == +INF: mu~ = mu + (t - tau) v
   int sh_degree;
   int width, height, tiles_x, tiles_y;

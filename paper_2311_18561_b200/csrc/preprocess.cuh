@@ -25,9 +25,28 @@ namespace pvg {
 #define SH_C3D 0.3731763325901154f
 #define SH_C3E 1.445305721320277f
 
+// sin(pi x) in double, |error| < 1e-13: x is reduced to [-1, 1] by the nearest even integer (exact), folded to
+// [-1/2, 1/2] by sin(pi (s - x)) = sin(pi x) for s = +-1 (exact), and summed as the odd Taylor polynomial of degree
+// 17 (its remainder at 1/2 is 4e-14).
+__device__ __forceinline__ double sinpi_reduced(double x) {
+  x = fma(-2.0, rint(0.5 * x), x);
+  if (fabs(x) > 0.5) x = copysign(1.0, x) - x;
+  const double x2 = x * x;
+  double p = 7.952054001475513e-07;
+  p = fma(p, x2, -2.1915353447830217e-05);
+  p = fma(p, x2, 0.00046630280576761255);
+  p = fma(p, x2, -0.0073704309457143504);
+  p = fma(p, x2, 0.08214588661112823);
+  p = fma(p, x2, -0.5992645293207921);
+  p = fma(p, x2, 2.5501640398773455);
+  p = fma(p, x2, -5.16771278004997);
+  p = fma(p, x2, 3.141592653589793);
+  return p * x;
+}
+
 // Model layout in HBM (built once by relayout_kernel):
 //   A0[i] = (mu.x, mu.y, mu.z, tau)     A1[i] = (v.x, v.y, v.z, beta)
-//   A2[i] = unit quaternion (w,x,y,z)   A3[i] = (s.x, s.y, s.z, o)
+//   A2[i] = quaternion (w,x,y,z) as given (normalised inside R(q))   A3[i] = (s.x, s.y, s.z, o)
 //   SH[p][i], p = 0..11: floats 4p..4p+3 of the point's [16][3] coefficient block
 // Outputs:
 //   record[3 i + {0,1,2}] = (mx,my,z,o~), (a,b,c,hx), (r,g,b,hy)   -- all 0 if culled; with P.target == 1 the
@@ -60,37 +79,59 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
   float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0, r2 = r0;
   uint4 ti = make_uint4(0u, 0u, 0u, 0u);
 
-  // P1: Eq. 6. sinpi gives an exact range reduction of 2 pi (t - tau) / l.
-  const float dt = P.t - a0.w;
-  const float m = P.linear ? dt : P.l_over_2pi * sinpif(P.two_over_l * dt);
+  // P1, P4, P8 -- the chain mu~(t) -> p_cam -> (mx, my) -- run in DOUBLE. In fp32 the rounding of t - tau alone
+  // (3e-8) moves a fast, near Gaussian (|v| = 20 m/s at z = 2 m, f = 2000 px) by 6e-4 px, and the three dot products
+  // and the division of the projection add a few ulps of coordinates of up to 2000 px (1.2e-4 px each): together up
+  // to 3e-4 px in the mean, which through d alpha / d mean <= 0.6 o~ / sigma was the whole end-to-end image error
+  // (6e-4 against the oracle's own record). In double the record's (mx, my, z) are the
+  // correctly rounded fp32 values of the exact ones. B200 issues FP64 at half the FP32 rate and this kernel is
+  // HBM-bound; the chain is kept to ~45 double instructions (polynomial sine, Newton reciprocal).
+  // P1: Eq. 6, sin(2 pi dt / l) = sin(pi x) with x = 2 dt / l reduced to [-1/2, 1/2] exactly.
+  const double dtd = P.t1 - (double)a0.w;   // exact
+  double md = dtd;
+  if (!P.linear) md = P.l_over_2pi * sinpi_reduced(P.two_over_l * dtd);
   // staticness rho = beta / l; beta = +INF is rho = +INF whatever l
   const float rho = a1.w > 3.0e38f ? a1.w : a1.w * P.inv_l;
   // Eq. 12: temporal-smoothing state mu~(t1) + vbar dts, vbar = v exp(-rho/2) (Eq. 10)
-  float mm = m;
-  if (P.dts != 0.f) mm = fmaf(expf(-0.5f * rho), P.dts, m);
-  const float wx = fmaf(mm, a1.x, a0.x), wy = fmaf(mm, a1.y, a0.y), wz = fmaf(mm, a1.z, a0.z);
-  // P2: Eq. 7 (beta = +INF gives exp(-0) = 1)
-  const float op = a3.w * expf(-0.5f * (dt * dt) / (a1.w * a1.w));
+  if (P.dts != 0.f) {
+    const double rhod = a1.w > 3.0e38f ? (double)a1.w : (double)a1.w * P.inv_l_d;
+    md = fma(exp(-0.5 * rhod), (double)P.dts, md);
+  }
+  const double wxd = fma(md, (double)a1.x, (double)a0.x), wyd = fma(md, (double)a1.y, (double)a0.y),
+               wzd = fma(md, (double)a1.z, (double)a0.z);
+  const float wx = (float)wxd, wy = (float)wyd, wz = (float)wzd;
+  // P2: Eq. 7 (beta = +INF gives exp(-0) = 1), fp32 on the exact t - tau: the exponent of a survivor is above
+  // ln(1/255) = -5.5, three roundings of it are 1e-6 absolute
+  const float dtb = (float)dtd / a1.w;
+  const float op = a3.w * expf(-0.5f * dtb * dtb);
   // P3: opacity cull; the comparison is false for NaN
   valid = (op >= PVG_ALPHA_MIN) && (op <= 3.0e38f);
   // staticness filter: keep rho_min <= rho <= rho_max
   if (P.filter) valid = valid && (rho >= P.rho_min) && !(rho > P.rho_max);
   // P4: camera space + near cull
-  const float px = fmaf(P.R[0], wx, fmaf(P.R[1], wy, fmaf(P.R[2], wz, P.T[0])));
-  const float py = fmaf(P.R[3], wx, fmaf(P.R[4], wy, fmaf(P.R[5], wz, P.T[1])));
-  const float pz = fmaf(P.R[6], wx, fmaf(P.R[7], wy, fmaf(P.R[8], wz, P.T[2])));
+  const double pxd = fma(P.Rd[0], wxd, fma(P.Rd[1], wyd, fma(P.Rd[2], wzd, P.Td[0])));
+  const double pyd = fma(P.Rd[3], wxd, fma(P.Rd[4], wyd, fma(P.Rd[5], wzd, P.Td[1])));
+  const double pzd = fma(P.Rd[6], wxd, fma(P.Rd[7], wyd, fma(P.Rd[8], wzd, P.Td[2])));
+  const float px = (float)pxd, py = (float)pyd, pz = (float)pzd;
   valid = valid && (pz > P.znear) && (pz <= 3.0e38f) && (fabsf(px) <= 3.0e38f) && (fabsf(py) <= 3.0e38f);
 
   float mx = 0.f, my = 0.f, hx = 0.f, hy = 0.f;
   if (valid) {
-    // P5: M = R(q) diag(s); Sigma = M M^T (never formed)
+    // P5: M = R(q) diag(s); Sigma = M M^T (never formed). q is stored as given: R(q / |q|) = I + (2 / |q|^2) (...)
+    // needs no square root.
     const float qw = a2.x, qx = a2.y, qy = a2.z, qz = a2.w;
-    const float R00 = 1.f - 2.f * (qy * qy + qz * qz), R01 = 2.f * (qx * qy - qw * qz), R02 = 2.f * (qx * qz + qw * qy);
-    const float R10 = 2.f * (qx * qy + qw * qz), R11 = 1.f - 2.f * (qx * qx + qz * qz), R12 = 2.f * (qy * qz - qw * qx);
-    const float R20 = 2.f * (qx * qz - qw * qy), R21 = 2.f * (qy * qz + qw * qx), R22 = 1.f - 2.f * (qx * qx + qy * qy);
+    const float q2 = 2.0f / (qw * qw + qx * qx + qy * qy + qz * qz);
+    const float R00 = 1.f - q2 * (qy * qy + qz * qz), R01 = q2 * (qx * qy - qw * qz), R02 = q2 * (qx * qz + qw * qy);
+    const float R10 = q2 * (qx * qy + qw * qz), R11 = 1.f - q2 * (qx * qx + qz * qz), R12 = q2 * (qy * qz - qw * qx);
+    const float R20 = q2 * (qx * qz - qw * qy), R21 = q2 * (qy * qz + qw * qx), R22 = 1.f - q2 * (qx * qx + qy * qy);
     // P6: T = J W with the Jacobian guard (S15)
     const float iz = 1.0f / pz;
-    const float xz = px / pz, yz = py / pz;
+    // 1 / z in double from the fp32 reciprocal by two Newton steps (relative error 1e-7 -> 1e-14 -> 1e-28: rounding)
+    double izd = (double)iz;
+    izd = izd * fma(-pzd, izd, 2.0);
+    izd = izd * fma(-pzd, izd, 2.0);
+    const double xzd = pxd * izd, yzd = pyd * izd;
+    const float xz = (float)xzd, yz = (float)yzd;
     const float tx = fminf(P.limx, fmaxf(-P.limx, xz));
     const float ty = fminf(P.limy, fmaxf(-P.limy, yz));
     const float j00 = P.fx * iz, j02 = -P.fx * tx * iz;  // -fx * xbar / z^2 with xbar = tx * z
@@ -112,13 +153,45 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
     const float det0 = c0 * c0 + c1 * c1 + c2 * c2;
     const float cxx = sxx + PVG_DILATE, cyy = syy + PVG_DILATE;
     const float det = det0 + PVG_DILATE * (sxx + syy) + PVG_DILATE * PVG_DILATE;
-    // P7: conic
+    // P7: conic. The survival decision and the extents below use the fp32 covariance (the geometry pass and the
+    // record pass must take them identically); the record's conic itself is computed in double (record passes only:
+    // in the lazy mode ~12 % of the Gaussians): in fp32 U U^T loses C eps (f/z)^2 s_max^2 per entry -- for a needle
+    // seen end-on a large multiple of the entry itself --, in double the conic is the correctly rounded one.
     valid = (det > 0.f) && (det <= 3.0e38f);
-    const float idet = 1.0f / det;
-    const float ca = cyy * idet, cb = -sxy * idet, cc = cxx * idet;
+    float ca = 0.f, cb = 0.f, cc = 0.f;
+    if (PART != PRE_GEO) {
+      const double dqw = a2.x, dqx = a2.y, dqz = a2.w, dqy = a2.z;
+      const double n2 = fma(dqw, dqw, fma(dqx, dqx, fma(dqy, dqy, dqz * dqz)));
+      double s2 = (double)(1.0f / (float)n2);
+      s2 = s2 * fma(-n2, s2, 2.0);
+      s2 = s2 * fma(-n2, s2, 2.0);
+      s2 += s2;   // 2 / |q|^2
+      const double D00 = fma(-s2, fma(dqy, dqy, dqz * dqz), 1.0), D01 = s2 * fma(dqx, dqy, -dqw * dqz), D02 = s2 * fma(dqx, dqz, dqw * dqy);
+      const double D10 = s2 * fma(dqx, dqy, dqw * dqz), D11 = fma(-s2, fma(dqx, dqx, dqz * dqz), 1.0), D12 = s2 * fma(dqy, dqz, -dqw * dqx);
+      const double D20 = s2 * fma(dqx, dqz, -dqw * dqy), D21 = s2 * fma(dqy, dqz, dqw * dqx), D22 = fma(-s2, fma(dqx, dqx, dqy * dqy), 1.0);
+      const double txd = fmin(P.limxd, fmax(-P.limxd, xzd)), tyd = fmin(P.limyd, fmax(-P.limyd, yzd));
+      const double e00 = P.fxd * izd, e02 = -e00 * txd, e11 = P.fyd * izd, e12 = -e11 * tyd;
+      const double T00 = fma(e00, P.Rd[0], e02 * P.Rd[6]), T01 = fma(e00, P.Rd[1], e02 * P.Rd[7]), T02 = fma(e00, P.Rd[2], e02 * P.Rd[8]);
+      const double T10 = fma(e11, P.Rd[3], e12 * P.Rd[6]), T11 = fma(e11, P.Rd[4], e12 * P.Rd[7]), T12 = fma(e11, P.Rd[5], e12 * P.Rd[8]);
+      const double sx = a3.x, sy = a3.y, sz = a3.z;
+      const double U00 = fma(T00, D00, fma(T01, D10, T02 * D20)) * sx, U01 = fma(T00, D01, fma(T01, D11, T02 * D21)) * sy,
+                   U02 = fma(T00, D02, fma(T01, D12, T02 * D22)) * sz;
+      const double U10 = fma(T10, D00, fma(T11, D10, T12 * D20)) * sx, U11 = fma(T10, D01, fma(T11, D11, T12 * D21)) * sy,
+                   U12 = fma(T10, D02, fma(T11, D12, T12 * D22)) * sz;
+      const double Sxx = fma(U00, U00, fma(U01, U01, U02 * U02)) + (double)PVG_DILATE_D;
+      const double Sxy = fma(U00, U10, fma(U01, U11, U02 * U12));
+      const double Syy = fma(U10, U10, fma(U11, U11, U12 * U12)) + (double)PVG_DILATE_D;
+      const double detd = fma(Sxx, Syy, -Sxy * Sxy);
+      double idd = (double)(1.0f / (float)detd);
+      idd = idd * fma(-detd, idd, 2.0);
+      idd = idd * fma(-detd, idd, 2.0);
+      ca = (float)(Syy * idd);
+      cb = (float)(-Sxy * idd);
+      cc = (float)(Sxx * idd);
+    }
     // P8, P9
-    mx = fmaf(P.fx, xz, P.cx);
-    my = fmaf(P.fy, yz, P.cy);
+    mx = (float)fma(P.fxd, xzd, P.cxd);
+    my = (float)fma(P.fyd, yzd, P.cyd);
     const float kk = 2.0f * logf(255.0f * op);
     hx = sqrtf(kk * cxx);
     hy = sqrtf(kk * cyy);
@@ -330,8 +403,7 @@ relayout_kernel(uint32_t n, const float* __restrict__ mu, const float* __restric
   A0[i] = make_float4(mu[3 * (size_t)i], mu[3 * (size_t)i + 1], mu[3 * (size_t)i + 2], tau[i]);
   A1[i] = make_float4(vel[3 * (size_t)i], vel[3 * (size_t)i + 1], vel[3 * (size_t)i + 2], beta[i]);
   const float qw = quat[4 * (size_t)i], qx = quat[4 * (size_t)i + 1], qy = quat[4 * (size_t)i + 2], qz = quat[4 * (size_t)i + 3];
-  const float qn = 1.0f / sqrtf(qw * qw + qx * qx + qy * qy + qz * qz);
-  A2[i] = make_float4(qw * qn, qx * qn, qy * qn, qz * qn);
+  A2[i] = make_float4(qw, qx, qy, qz);
   A3[i] = make_float4(scale[3 * (size_t)i], scale[3 * (size_t)i + 1], scale[3 * (size_t)i + 2], opacity[i]);
   const float4* src = reinterpret_cast<const float4*>(sh + 48 * (size_t)i);  // 192 B rows: 16 B aligned
 #pragma unroll

@@ -45,6 +45,37 @@ void* g_alloc_user = nullptr;
     if (rc_ != PVG_OK) return rc_; \
   } while (0)
 
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: remember per (call site, device), thread-safe.
+#define PVG_ENSURE_SMEM(kern, bytes, dev)                                                              \
+  do {                                                                                                 \
+    static std::atomic<uint64_t> done_[4];                                                             \
+    const unsigned d_ = (unsigned)(dev) & 255u;                                                        \
+    if (!(done_[d_ >> 6].load(std::memory_order_acquire) & (1ull << (d_ & 63u)))) {                    \
+      CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes)));       \
+      done_[d_ >> 6].fetch_or(1ull << (d_ & 63u), std::memory_order_release);                          \
+    }                                                                                                  \
+  } while (0)
+
+// The caller's current device for the duration of an entry point (a scene lives on the device it was created on).
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    int cur = -1;
+    if (dev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != dev && cudaSetDevice(dev) == cudaSuccess) prev = cur;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+// device ordinal and SM count, looked up once (pvg_create_scene) instead of on every frame
+struct Dev {
+  int ordinal = 0, sms = 1;
+  int query() {
+    CU(cudaGetDevice(&ordinal));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ordinal));
+    return PVG_OK;
+  }
+};
+
 void* dev_alloc(size_t bytes, cudaStream_t st) {
   if (bytes == 0) bytes = 256;
   if (g_alloc) return g_alloc(bytes, (void*)st, g_alloc_user);
@@ -67,7 +98,13 @@ struct Buf {
   size_t cap = 0;
   int reserve(size_t bytes, cudaStream_t st, double headroom = 1.0) {
     if (bytes <= cap) return PVG_OK;
-    dev_free(p);
+    if (p) {
+      // Growing a live buffer: a caching allocator (the torch hooks) would re-issue the block at once to work on the
+      // stream it was allocated for, while kernels of this scene -- on its current, side or copy stream, possibly
+      // another stream than the one of the allocation -- may still read it. Growth is rare (headroom): wait.
+      cudaDeviceSynchronize();
+      dev_free(p);
+    }
     p = nullptr;
     cap = 0;
     size_t want = (size_t)((double)bytes * headroom);
@@ -175,14 +212,10 @@ struct Timer {
 
 template <class Cfg, int BITS, int HI>
 int launch_pass_bits(const uint64_t* kin, const uint32_t* vin, uint64_t* kout, uint32_t* vout, uint32_t n, int shift,
-                     const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
+                     const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev) {
   using Smem = OnesweepSmem<Cfg::THREADS, Cfg::ITEMS, BITS>;
   auto kern = onesweep_pass_kernel<Cfg::THREADS, Cfg::ITEMS, BITS, Cfg::MINB, HI, Cfg::STREAM>;
-  static bool configured = false;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
-    configured = true;
-  }
+  PVG_ENSURE_SMEM(kern, sizeof(Smem), dev);
   constexpr uint32_t TILE = Cfg::THREADS * Cfg::ITEMS;
   const uint32_t tiles = (n + TILE - 1) / TILE;
   kern<<<tiles, Cfg::THREADS, sizeof(Smem), st>>>(kin, vin, kout, vout, n, shift & 31, hist, lookback, ticket);
@@ -191,12 +224,12 @@ int launch_pass_bits(const uint64_t* kin, const uint32_t* vin, uint64_t* kout, u
 
 template <class Cfg>
 int launch_pass(int bits, const uint64_t* kin, const uint32_t* vin, uint64_t* kout, uint32_t* vout, uint32_t n, int shift,
-                const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
+                const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev) {
   switch (bits) {
 #define PVG_CASE(B)                                                                                              \
   case B:                                                                                                        \
-    return shift >= 32 ? launch_pass_bits<Cfg, B, 1>(kin, vin, kout, vout, n, shift, hist, lookback, ticket, st) \
-                       : launch_pass_bits<Cfg, B, 0>(kin, vin, kout, vout, n, shift, hist, lookback, ticket, st);
+    return shift >= 32 ? launch_pass_bits<Cfg, B, 1>(kin, vin, kout, vout, n, shift, hist, lookback, ticket, st, dev) \
+                       : launch_pass_bits<Cfg, B, 0>(kin, vin, kout, vout, n, shift, hist, lookback, ticket, st, dev);
     PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
 #undef PVG_CASE
     default: return PVG_ERR_BAD_OPTION;
@@ -223,7 +256,7 @@ int prep_onesweep(uint64_t n, int begin_bit, int end_bit, cudaStream_t alloc_st,
   return PVG_OK;
 }
 
-int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, int begin_bit,
+int run_onesweep(const Dev& dv, uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, int begin_bit,
                  int end_bit, cudaStream_t st, SortScratch& sc, Timer* tm, int stage, int* result,
                  bool hist_ready = false, bool scratch_ready = false, const uint32_t* hist_at = nullptr) {
   *result = 0;
@@ -237,11 +270,8 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
     if (tm) tm->cut();
   }
 
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const uint64_t hist_chunks = (n + (uint64_t)HIST_THREADS * HIST_ITEMS - 1) / ((uint64_t)HIST_THREADS * HIST_ITEMS);
-  const unsigned hist_grid = (unsigned)std::min<uint64_t>(hist_chunks, (uint64_t)sms * 4);
+  const unsigned hist_grid = (unsigned)std::min<uint64_t>(hist_chunks, (uint64_t)dv.sms * 4);
   if (!hist_ready) {
     if (tm) TRY(tm->begin("onesweep_histogram", stage, st));
     uint32_t* done = sc.tickets.as<uint32_t>() + (OS_MAX_PASSES - 1);   // last ticket slot: never a pass's (<= 8 passes)
@@ -256,8 +286,8 @@ int run_onesweep(uint64_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t*
     const uint32_t* hist = (hist_at ? hist_at : sc.hist.as<uint32_t>()) + p * OS_RADIX;
     uint64_t* lb = sc.lookback.as<uint64_t>() + (size_t)p * tiles * OS_RADIX;
     uint32_t* tk = sc.tickets.as<uint32_t>() + p;
-    if (small) TRY(launch_pass<OsSmall>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st));
-    else TRY(launch_pass<OsLarge>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st));
+    if (small) TRY(launch_pass<OsSmall>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st, dv.ordinal));
+    else TRY(launch_pass<OsLarge>(plan.bits[p], kin, vin, kout, vout, (uint32_t)n, plan.shift[p], hist, lb, tk, st, dv.ordinal));
     if (tm) TRY(tm->end(st));
     std::swap(kin, kout);
     std::swap(vin, vout);
@@ -276,14 +306,10 @@ struct CpCfg { static constexpr int THREADS = PVG_CP_THREADS, ITEMS = PVG_CP_ITE
 
 template <int BITS, bool LAST>
 int launch_compact_bits(const uint16_t* tin, const uint32_t* vin, uint16_t* tout, uint32_t* vout, uint32_t n, int shift,
-                        const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st) {
+                        const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev) {
   using Smem = CompactSmem<CpCfg::THREADS, CpCfg::ITEMS, BITS>;
   auto kern = compact_pass_kernel<CpCfg::THREADS, CpCfg::ITEMS, BITS, CpCfg::MINB, LAST>;
-  static bool configured = false;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
-    configured = true;
-  }
+  PVG_ENSURE_SMEM(kern, sizeof(Smem), dev);
   constexpr uint32_t TILE = CpCfg::THREADS * CpCfg::ITEMS;
   kern<<<(n + TILE - 1) / TILE, CpCfg::THREADS, sizeof(Smem), st>>>(tin, vin, tout, vout, n, shift, hist, lookback, ticket);
   return PVG_OK;
@@ -291,7 +317,7 @@ int launch_compact_bits(const uint16_t* tin, const uint32_t* vin, uint16_t* tout
 
 // Tile-id passes over the compact (u16 tile, u32 index) payload; histograms come from
 // tile_prefix_kernel. The sorted indices end in v[*result]; t[] ping-pongs alongside.
-int run_compact_sort(uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint32_t* v1, int tile_bits, cudaStream_t st,
+int run_compact_sort(const Dev& dv, uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint32_t* v1, int tile_bits, cudaStream_t st,
                      SortScratch& sc, Timer* tm, int* result) {
   *result = 0;
   if (n == 0) return PVG_OK;
@@ -315,8 +341,8 @@ int run_compact_sort(uint32_t n, uint16_t* t0, uint32_t* v0, uint16_t* t1, uint3
     switch (plan.bits[p]) {
 #define PVG_CASE(B)                                                                                   \
   case B:                                                                                             \
-    rc = last ? launch_compact_bits<B, true>(tin, vin, tout, vout, n, shift, hist, lb, tk, st)        \
-              : launch_compact_bits<B, false>(tin, vin, tout, vout, n, shift, hist, lb, tk, st);      \
+    rc = last ? launch_compact_bits<B, true>(tin, vin, tout, vout, n, shift, hist, lb, tk, st, dv.ordinal)   \
+              : launch_compact_bits<B, false>(tin, vin, tout, vout, n, shift, hist, lb, tk, st, dv.ordinal); \
     break;
       PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
 #undef PVG_CASE
@@ -345,6 +371,8 @@ struct pvg_scene {
   float cycle = 0.2f;
   int sh_degree = 3;
   cudaStream_t stream = nullptr;
+  cudaEvent_t ev_switch = nullptr;    // orders a new stream (pvg_set_stream) behind the work still in flight on the old one
+  Dev dev;                            // the device the scene lives on
   // options
   int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1, blend_cull = 1;
   int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
@@ -355,6 +383,8 @@ struct pvg_scene {
   bool light = false;                 // this frame's preprocess left the records to shade_kernel
   bool records_complete = true;       // record[] holds every Gaussian's record (pvg_debug_view completes them on demand)
   float* featw_last = nullptr;
+  // the option values the last render ran with: pvg_debug_view completes THAT frame, whatever was set since
+  int presort_used = 1, keep_unsorted_used = 0, lazy_chunks_used = 0;
   bool lazy_used = false;             // last frame wrote list prefixes + what the unfinished tiles needed
   bool lists_complete = true;         // vals[] holds every tile's whole list (pvg_debug_view completes them on demand)
   bool compact_used = false;  // last frame carried (u16 tile, u32 index) instances
@@ -418,6 +448,8 @@ void release_all(pvg_scene* s) {
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
   s->h_total = nullptr;
+  if (s->ev_switch) cudaEventDestroy(s->ev_switch);
+  s->ev_switch = nullptr;
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->ev_start) cudaEventDestroy(s->ev_start);
@@ -448,6 +480,7 @@ int create_impl(const pvg_scene_desc* d, pvg_scene* s) {
     snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
     return PVG_ERR_CUDA;
   }
+  TRY(s->dev.query());
   const size_t n = (size_t)d->n;
   s->n = (uint32_t)n;
   s->cycle = d->cycle;
@@ -496,6 +529,8 @@ int init_workspace(pvg_scene* s) {
   rs(s->dhist, 2 * kDhistWords * 4);
   if (rc != PVG_OK) return rc;
   CU(cudaMemsetAsync(s->dhist.p, 0, 2 * kDhistWords * 4, st));
+  CU(cudaStreamSynchronize(st));   // the first render may run on another stream: the zeroes must have landed
+  CU(cudaEventCreateWithFlags(&s->ev_switch, cudaEventDisableTiming));
   CU(cudaHostAlloc((void**)&s->h_total, 64, cudaHostAllocMapped));
   CU(cudaHostGetDevicePointer((void**)&s->d_total, s->h_total, 0));
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
@@ -510,7 +545,6 @@ int init_workspace(pvg_scene* s) {
 }
 
 int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state, FrameParams* P) {
-  const float t = (float)((double)state->t - (double)state->dt);
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
   if (!(cam->fx > 0.f) || !(cam->fy > 0.f) || !std::isfinite(cam->fx) || !std::isfinite(cam->fy) ||
       !std::isfinite(cam->cx) || !std::isfinite(cam->cy))
@@ -525,10 +559,15 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   for (int j = 0; j < 3; ++j)
     P->campos[j] = (float)-((double)E[j] * E[3] + (double)E[4 + j] * E[7] + (double)E[8 + j] * E[11]);
   P->fx = cam->fx; P->fy = cam->fy; P->cx = cam->cx; P->cy = cam->cy;
+  for (int k = 0; k < 9; ++k) P->Rd[k] = (double)P->R[k];
+  for (int k = 0; k < 3; ++k) P->Td[k] = (double)P->T[k];
+  P->fxd = cam->fx; P->fyd = cam->fy; P->cxd = cam->cx; P->cyd = cam->cy;
   P->limx = (float)(1.3 * cam->width / (2.0 * (double)cam->fx));
   P->limy = (float)(1.3 * cam->height / (2.0 * (double)cam->fy));
+  P->limxd = 1.3 * cam->width / (2.0 * (double)cam->fx);
+  P->limyd = 1.3 * cam->height / (2.0 * (double)cam->fy);
   P->znear = cam->znear > 0.f ? cam->znear : PVG_ZNEAR_DEFAULT;
-  P->t = t;
+  P->t1 = (double)state->t - (double)state->dt;
   P->dts = state->dt;
   P->rho_min = state->rho_min;
   P->rho_max = state->rho_max;
@@ -537,8 +576,9 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   P->cull = s->blend_cull;
   P->linear = std::isinf(s->cycle) ? 1 : 0;
   P->inv_l = P->linear ? 0.f : (float)(1.0 / (double)s->cycle);
-  P->two_over_l = P->linear ? 0.f : (float)(2.0 / (double)s->cycle);
-  P->l_over_2pi = P->linear ? 0.f : (float)((double)s->cycle / (2.0 * 3.14159265358979323846));
+  P->inv_l_d = P->linear ? 0.0 : 1.0 / (double)s->cycle;
+  P->two_over_l = P->linear ? 0.0 : 2.0 / (double)s->cycle;
+  P->l_over_2pi = P->linear ? 0.0 : (double)s->cycle / (2.0 * 3.14159265358979323846);
   P->sh_degree = s->sh_degree;
   P->width = cam->width; P->height = cam->height;
   P->tiles_x = (cam->width + PVG_TILE - 1) / PVG_TILE;
@@ -593,11 +633,7 @@ int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Ti
 template <int BITS>
 int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64_t* lookback, uint32_t* ticket) {
   auto kern = bin_pass_kernel<BITS>;
-  static bool configured = false;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BinPassSmem<BITS>)));
-    configured = true;
-  }
+  PVG_ENSURE_SMEM(kern, sizeof(BinPassSmem<BITS>), s->dev.ordinal);
   constexpr uint32_t TILE = BP_THREADS * BP_ITEMS;
   kern<<<(Mb + TILE - 1) / TILE, BP_THREADS, sizeof(BinPassSmem<BITS>), s->stream>>>(
       s->e_bin.as<uint8_t>(), s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>(), s->s_g.as<uint32_t>(),
@@ -609,11 +645,7 @@ template <int BITS>
 int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t blocks_x, const uint32_t* bin_start,
                     uint64_t* lookback, uint32_t* ticket, uint32_t grid, const uint32_t* only_if) {
   auto kern = bin_emit_kernel<BITS>;
-  static bool configured = false;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BinEmitSmem<BITS>)));
-    configured = true;
-  }
+  PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
   kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
       s->n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
       blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if);
@@ -782,8 +814,10 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
                 float* out_alpha) {
   FrameParams P;
   TRY(fill_frame(s, cam, state, &P));
+  DeviceGuard guard(s->dev.ordinal);
   cudaStream_t st = s->stream;
   Timer& tm = s->timer;
+  s->presort_used = s->presort; s->keep_unsorted_used = s->keep_unsorted; s->lazy_chunks_used = s->lazy_chunks;
   tm.next_frame();
   if (!tm.accumulate) { if (tm.frame_on) tm.reset(); } else tm.cut();
   const uint32_t n = s->n;
@@ -860,13 +894,9 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     CU(cudaStreamWaitEvent(st, s->ev_zero, 0));
     CU(cudaEventRecord(s->ev_fork, st));
     CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
-    static bool attr_set = false;
     constexpr size_t kMaxDyn = 200 * 1024;
-    if (!attr_set) {
-      CU(cudaFuncSetAttribute(tile_prefix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
-      CU(cudaFuncSetAttribute(tile_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDyn));
-      attr_set = true;
-    }
+    PVG_ENSURE_SMEM(tile_prefix_kernel, kMaxDyn, s->dev.ordinal);
+    PVG_ENSURE_SMEM(tile_grid_kernel, kMaxDyn, s->dev.ordinal);
     const size_t grid_bytes = ((size_t)tilegrid_cells(P.tiles_x, P.tiles_y) +
                                (block ? (size_t)tilegrid_cells((int)blocks_x, (int)blocks_y) : 0)) * 4;   // + 1 cell: survivor count
     const int use_smem = grid_bytes <= kMaxDyn ? 1 : 0;
@@ -876,11 +906,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     int* grid = s->tilegrid.as<int>();
     CU(cudaMemsetAsync(grid, 0, grid_bytes + 4, sd));
     tm.cut();
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     TRY(tm.begin("tile_grid", PVG_STAGE_RANGES, sd));
-    tile_grid_kernel<<<std::min<unsigned>((n + TG_THREADS - 1) / TG_THREADS, (unsigned)sms), TG_THREADS,
+    tile_grid_kernel<<<std::min<unsigned>((n + TG_THREADS - 1) / TG_THREADS, (unsigned)s->dev.sms), TG_THREADS,
                        use_smem ? grid_bytes : 0, sd>>>(s->tileinfo.as<uint4>(), n, P.tiles_x, P.tiles_y, use_smem,
                                                         block ? 1 : 0, grid);
     TRY(tm.end(sd));
@@ -896,7 +923,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
 
     // a3 (n-key part): depth order of the Gaussians
     int side = 0;
-    TRY(run_onesweep(n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
+    TRY(run_onesweep(s->dev, n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
                      s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side, true, true,
                      s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords));
     s->visit_side = side;
@@ -957,7 +984,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       tm.cut();
     }
     int side = 0;
-    TRY(run_compact_sort((uint32_t)M, s->tiles16[0].as<uint16_t>(), s->vals[0].as<uint32_t>(),
+    TRY(run_compact_sort(s->dev, (uint32_t)M, s->tiles16[0].as<uint16_t>(), s->vals[0].as<uint32_t>(),
                          s->tiles16[1].as<uint16_t>(), s->vals[1].as<uint32_t>(), tile_bits, st, s->sort_m, &tm, &side));
     s->sorted_side = side;
   } else if (M > 0) {
@@ -980,7 +1007,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     }
     // a3 (M-instance part)
     int side = 0;
-    TRY(run_onesweep(M, s->keys[0].as<uint64_t>(), s->vals[0].as<uint32_t>(), s->keys[1].as<uint64_t>(),
+    TRY(run_onesweep(s->dev, M, s->keys[0].as<uint64_t>(), s->vals[0].as<uint32_t>(), s->keys[1].as<uint64_t>(),
                      s->vals[1].as<uint32_t>(), s->sort_begin, s->sort_end, st, s->sort_m, &tm, PVG_STAGE_SORT, &side,
                      s->presort != 0));
     s->sorted_side = side;
@@ -1022,7 +1049,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       Z.parked_host = s->d_total + 3;
       Z.blocks_x = bb_blocks(P.tiles_x);
     }
-#define PVG_BLEND(C, M, PH) blend_kernel<C, M, PH><<<(PH) == 2 ? std::min(band_tiles, 148u * 8u) : band_tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw, Z)
+#define PVG_BLEND(C, M, PH) blend_kernel<C, M, PH><<<(PH) == 2 ? std::min(band_tiles, (uint32_t)s->dev.sms * 8u) : band_tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw, Z)
 #define PVG_BLEND_ALL(PH)                                        \
     if (s->count_pairs) {                                        \
       if (mode == BLEND_FEATURE) PVG_BLEND(true, BLEND_FEATURE, PH); \
@@ -1099,7 +1126,20 @@ int pvg_set_allocator(pvg_alloc_fn alloc_fn, pvg_free_fn free_fn, void* user) {
 
 int pvg_set_stream(pvg_scene* scene, void* cuda_stream) {
   if (!scene) return PVG_ERR_NULL;
-  scene->stream = (cudaStream_t)cuda_stream;
+  cudaStream_t next = (cudaStream_t)cuda_stream;
+  if (next == scene->stream) return PVG_OK;
+  // The workspace (record, ranges, vals, histograms, ...) belongs to the frames already enqueued on the old
+  // stream: the new stream -- and through ev_start / ev_rendered the side and copy streams -- must run behind them.
+  DeviceGuard guard(scene->dev.ordinal);
+  if (scene->ev_switch) {
+    if (cudaEventRecord(scene->ev_switch, scene->stream) == cudaSuccess) {
+      CU(cudaStreamWaitEvent(next, scene->ev_switch, 0));
+    } else {   // the old stream is gone (destroyed by its owner): nothing finer to wait on
+      cudaGetLastError();
+      CU(cudaDeviceSynchronize());
+    }
+  }
+  scene->stream = next;
   return PVG_OK;
 }
 
@@ -1127,11 +1167,15 @@ int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
   *out = nullptr;
   pvg_scene* s = new (std::nothrow) pvg_scene();
   if (!s) return PVG_ERR_OOM;
+  DeviceGuard guard(scene->dev.ordinal);
   s->n = scene->n; s->cycle = scene->cycle; s->sh_degree = scene->sh_degree;
   s->stream = scene->stream;
+  s->dev = scene->dev;
   s->presort = scene->presort; s->keep_unsorted = scene->keep_unsorted; s->count_pairs = scene->count_pairs;
   s->compact = scene->compact; s->block = scene->block; s->blend_cull = scene->blend_cull;
   s->lazy_chunks = scene->lazy_chunks; s->lazy_slab = scene->lazy_slab;
+  s->band_begin = scene->band_begin; s->band_end = scene->band_end;
+  s->timer.enabled = scene->timer.enabled; s->timer.accumulate = scene->timer.accumulate; s->timer.stride = scene->timer.stride;
   s->model = scene->model;
   s->model->refs.fetch_add(1);
   // the model was written on the parent's stream at creation, which synchronised: nothing to wait for
@@ -1147,7 +1191,9 @@ int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
 
 int pvg_destroy(pvg_scene* scene) {
   if (!scene) return PVG_ERR_NULL;
+  DeviceGuard guard(scene->dev.ordinal);
   cudaStreamSynchronize(scene->stream);
+  if (scene->side) cudaStreamSynchronize(scene->side);
   if (scene->copy_stream) cudaStreamSynchronize(scene->copy_stream);
   release_all(scene);
   delete scene;
@@ -1156,6 +1202,7 @@ int pvg_destroy(pvg_scene* scene) {
 
 int pvg_set_sky(pvg_scene* scene, const float* cube, int res, int on_device) {
   if (!scene) return PVG_ERR_NULL;
+  DeviceGuard guard(scene->dev.ordinal);
   cudaStream_t st = scene->stream;
   CU(cudaStreamSynchronize(st));   // frames in flight may still read the old map
   if (scene->copy_stream) CU(cudaStreamSynchronize(scene->copy_stream));
@@ -1247,6 +1294,7 @@ int pvg_render_host_async(pvg_scene* scene, const pvg_camera* cam, float t, floa
   if (!state_ok(&state)) return PVG_ERR_BAD_STATE;
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 32768 || cam->height > 32768) return PVG_ERR_BAD_CAMERA;
   const size_t HW = (size_t)cam->width * cam->height;
+  DeviceGuard guard(scene->dev.ordinal);
   cudaStream_t st = scene->stream;
   const int slot = scene->img_next;
   scene->img_next ^= 1;
@@ -1283,6 +1331,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   if (!s || !out) return PVG_ERR_NULL;
   memset(out, 0, sizeof(*out));
   if (!s->rendered) return PVG_OK;
+  DeviceGuard guard(s->dev.ordinal);
   out->n = s->n;
   out->num_instances = s->M;
   out->tiles_x = s->tiles_x;
@@ -1291,7 +1340,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->sort_end_bit = (uint32_t)s->sort_end;
   out->record = s->record.as<float>();
   out->counts = s->counts.as<uint32_t>();
-  out->visit_order = s->presort ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
+  out->visit_order = s->presort_used ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
   if (s->block_used && s->light && !s->records_complete && s->M) {
     // lazy lists: the records the frame never needed (and zeros for the culled Gaussians)
@@ -1312,7 +1361,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     }
 #endif
     CU(cudaMemsetAsync(s->sort_m.tickets.as<uint32_t>() + 3, 0, 4, s->stream));
-    TRY(launch_bin_write(s, s->last_P, (uint32_t)s->lazy_chunks, 0xFFFFFFFFu, false, 3));
+    TRY(launch_bin_write(s, s->last_P, (uint32_t)s->lazy_chunks_used, 0xFFFFFFFFu, false, 3));
     CU(cudaGetLastError());
     s->lists_complete = true;
   }
@@ -1325,7 +1374,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
       TRY(s->keys[0].reserve((size_t)s->M * 8, st));
       keys_from_ranges_kernel<<<s->tiles_x * s->tiles_y, 256, 0, st>>>(s->ranges.as<uint2>(), s->vals[0].as<uint32_t>(),
                                                                         s->tileinfo.as<uint4>(), s->keys[0].as<uint64_t>());
-      if (s->keep_unsorted) {
+      if (s->keep_unsorted_used) {
         TRY(s->keys_unsorted.reserve((size_t)s->M * 8, st));
         TRY(s->vals_unsorted.reserve((size_t)s->M * 4, st));
         expand_kernel<false><<<(unsigned)((s->M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
@@ -1344,7 +1393,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     keys_from_ranges_kernel<<<s->tiles_x * s->tiles_y, 256, 0, st>>>(s->ranges.as<uint2>(),
                                                                       s->vals[s->sorted_side].as<uint32_t>(),
                                                                       s->tileinfo.as<uint4>(), s->keys[0].as<uint64_t>());
-    if (s->keep_unsorted) {
+    if (s->keep_unsorted_used) {
       TRY(s->keys_unsorted.reserve((size_t)s->M * 8, st));
       keys_from_tiles16_kernel<<<(M32 + 255) / 256, 256, 0, st>>>(s->tiles16_unsorted.as<uint16_t>(),
                                                                  s->vals_unsorted.as<uint32_t>(), s->tileinfo.as<uint4>(),
@@ -1353,7 +1402,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(st));
   }
-  if (s->keep_unsorted && s->M) {
+  if (s->keep_unsorted_used && s->M) {
     out->keys_unsorted = s->keys_unsorted.as<uint64_t>();
     out->vals_unsorted = s->vals_unsorted.as<uint32_t>();
   }
@@ -1424,7 +1473,7 @@ int pvg_frame_stats(pvg_scene* s, uint64_t out[8]) {
   out[3] = s->tiles_y;
   out[4] = s->rendered ? s->Mb : 0;
   out[5] = s->block_used ? 2 : (s->compact_used ? 1 : 0);
-  out[6] = (s->rendered && s->presort) ? s->survivors : 0;
+  out[6] = (s->rendered && s->presort_used) ? s->survivors : 0;
   // tiles the lazy lists' first blend phase parked (stored by the second phase through mapped host memory: it is
   // the last frame's figure once that frame has completed on the stream; the word is only read here)
   out[7] = (s->rendered && s->block_used && s->lazy_used && s->M) ? s->h_total[3] : 0;
@@ -1454,7 +1503,9 @@ int pvg_sort_pairs(uint64_t n, uint64_t* keys_in, uint32_t* vals_in, uint64_t* k
   cudaStream_t st = (cudaStream_t)cuda_stream;
   SortScratch sc;
   int side = 0;
-  int rc = run_onesweep(n, keys_in, vals_in, keys_out, vals_out, begin_bit, end_bit, st, sc, nullptr, 0, &side);
+  Dev dv;
+  TRY(dv.query());
+  int rc = run_onesweep(dv, n, keys_in, vals_in, keys_out, vals_out, begin_bit, end_bit, st, sc, nullptr, 0, &side);
   if (rc == PVG_OK && n && side == 0) {  // result landed in the input buffers
     cudaError_t e = cudaMemcpyAsync(keys_out, keys_in, n * 8, cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(vals_out, vals_in, n * 4, cudaMemcpyDeviceToDevice, st);

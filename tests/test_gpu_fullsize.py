@@ -1,21 +1,25 @@
-"""Full-size parity (BASELINE.json configs 3 and 4) in the launch configuration bench.py times:
-default options, block-entry list builder. The oracle cannot sort ~3e8 instances in seconds, so
-the chain is checked on what it can compute one by one:
-  * Oracle-P on every Gaussian (record, cull flags);
-  * per-Gaussian tile counts, M and EVERY tile range bit-exactly (the ranges follow from the
-    oracle's rectangles by a 2-D difference array, recomputed here with numpy);
-  * the sorted list of sampled tiles (corners, centre, the longest list, random ones) bit-exactly
-    against oracle.tile_list (a direct per-tile computation);
-  * the pixels of those tiles against Oracle-R (binned) with the fragile budget;
-  * properties that hold at any size: every list is in (depth bits, index) order, every listed
-    Gaussian's rectangle contains the tile, list lengths add up to M.
-"""
+"""Full-size parity on EVERY BASELINE.json config, in the launch configuration bench.py times (default options:
+block-entry list builder, lazy lists). The oracle cannot sort ~3e8 instances in seconds, so the integer chain is
+checked on what it can compute one by one, and the images on the WHOLE frame:
+  * (P) Oracle-P on every Gaussian (record, cull flags; mean and depth bit-equal to the oracle's rounded record);
+  * (I) per-Gaussian tile counts, M and EVERY tile range bit-exactly (the ranges follow from the oracle's rectangles
+    by a 2-D difference array, recomputed here with numpy); the sorted list of sampled tiles (corners, centre, the
+    longest list, random ones) bit-exactly against oracle.tile_list (a direct per-tile computation); properties that
+    hold at any size: every list in (depth bits, index) order, every listed rectangle contains the tile, lengths add
+    up to M;
+  * (R) every pixel of the frame against Oracle-R (binned) fed the GPU record: 2e-4 + fragile budget + cond;
+  * (E) every pixel against Oracle-R fed Oracle-P's OWN record (nothing shared): 2e-4 + budget + cond + the allowance
+    derived from the record tolerances of (P) (parity.e2e_slack).
+Config 2: the 1M frame. Config 3: timestamps k = 0, 24, 49 of the sweep. Config 4: all 5 cameras x 2 timestamps
+((E) on the front and one side camera; the other renders stop at (R))."""
+import json
+
 import numpy as np
 import pytest
 
 import oracle
 import paper_2311_18561_b200 as pvg
-from parity import check_images, check_record
+from parity import check_images, check_record, e2e_slack, fragile_cap, oracle_preprocess
 from workloads import make_config
 
 pytestmark = pytest.mark.gpu
@@ -42,15 +46,17 @@ def _ranges_from_rects(rects, counts, TX, TY):
     return np.stack([end - per_tile, end], 1).astype(np.uint32), per_tile
 
 
-def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, max_fragile_frac=0.01):
-    # the staging-time ellipse cull of the blend must not change one bit of the frame
-    sc.set_option(pvg.OPT_BLEND_CULL, 0)
-    plain = [x.clone() for x in sc.render(cam, t)]
-    sc.set_option(pvg.OPT_BLEND_CULL, 1)
-    out = sc.render(cam, t)
+def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, end_to_end=True, check_cull=True):
     import torch
-    assert all(torch.equal(a, b) for a, b in zip(plain, out)), "BLEND_CULL changed the image"
-    del plain
+    if check_cull:
+        # the staging-time ellipse cull of the blend must not change one bit of the frame
+        sc.set_option(pvg.OPT_BLEND_CULL, 0)
+        plain = [x.clone() for x in sc.render(cam, t)]
+        sc.set_option(pvg.OPT_BLEND_CULL, 1)
+    out = sc.render(cam, t)
+    if check_cull:
+        assert all(torch.equal(a, b) for a, b in zip(plain, out)), "BLEND_CULL changed the image"
+        del plain
     rgb, depth, alpha = (x.cpu().numpy() for x in out)
     st = sc.frame_stats()
     assert st["list_mode"] == "blocks"
@@ -63,8 +69,8 @@ def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, max_fragile_fr
     granges = _d2h(sc, d.ranges, 0, (TX * TY, 2), np.uint32)
 
     # (P) record against Oracle-P on every Gaussian
-    wide, _ = oracle.preprocess_scene(wl_scene, cam, t)
-    check_record(grec, wide, cam, wl_scene)
+    wide, orec = oracle_preprocess(wl_scene, cam, t)
+    pstats = check_record(grec, wide, cam, wl_scene)
 
     # (I) counts, M, all ranges
     rects, counts, M_o = oracle.tile_counts(grec, W, H)
@@ -93,40 +99,58 @@ def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, max_fragile_fr
         r = rects[gv]
         assert np.all((r[:, 0] <= tx) & (tx <= r[:, 2]) & (r[:, 1] <= ty) & (ty <= r[:, 3]))
 
-    # (R) the pixels of the sampled tiles
-    ora = oracle.render(grec, W, H, bg=cam.bg, mode="binned", tiles=sel)
-    mask = np.zeros((H, W), dtype=bool)
-    for tl in sel:
-        tx, ty = tl % TX, tl // TX
-        mask[ty * 16:(ty + 1) * 16, tx * 16:(tx + 1) * 16] = True
-    sub = lambda a: a[..., mask]  # noqa: E731
+    # (R) every pixel of the frame against Oracle-R fed the GPU record
     zmax = float(max(grec[:, 2].max(), 1.0))
-    stats = check_images((sub(rgb), sub(depth), sub(alpha)), {k: (sub(v) if isinstance(v, np.ndarray) else v) for k, v in ora.items()},
-                         zmax, label="sampled tiles", max_fragile_frac=max_fragile_frac)
+    ora = oracle.render(grec, W, H, bg=cam.bg, mode="binned")
+    cap = fragile_cap(grec, ora, W * H)
+    stats = check_images((rgb, depth, alpha), ora, zmax, label="whole frame, gpu record", max_fragile_frac=cap)
     assert stats["max_rgb_err_clean"] <= 2e-4
-    return dict(M=M, tiles=len(sel), max_list=int(per_tile.max()), entries=st["block_entries"], **stats)
+    res = dict(M=M, tiles=len(sel), max_list=int(per_tile.max()), entries=st["block_entries"], fragile_cap=cap, P=pstats, R=stats)
+    print(json.dumps(res))
+    if end_to_end:
+        # (E) every pixel against Oracle-R fed Oracle-P's own record
+        ora2 = oracle.render(orec, W, H, bg=cam.bg, mode="binned", tie_budget=True, slack=e2e_slack(wide, wl_scene, cam))
+        cap2 = fragile_cap(orec, ora2, W * H, end_to_end=True)
+        res["E"] = check_images((rgb, depth, alpha), ora2, zmax, label="whole frame, end to end", max_fragile_frac=cap2)
+        res["fragile_cap_e2e"] = cap2
+    print(json.dumps(res))
+    return res
 
 
-def test_cfg3_full_size_frame():
+def test_cfg2_full_size_frame():
+    """BASELINE.json config 2: 1M Gaussians, 1920x1280, t = 0.5 -- the whole frame."""
+    wl = make_config(2)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    try:
+        cam, t = list(wl.frames())[0]
+        st = _check_frame(sc, wl.scene, cam, t)
+        assert st["M"] > 50_000_000
+    finally:
+        sc.close()
+
+
+@pytest.mark.parametrize("k", [0, 24, 49])
+def test_cfg3_full_size_frames(k):
+    """BASELINE.json config 3 (the configuration bench.py times): first, middle and last timestamp of the sweep."""
     wl = make_config(3)
     sc = pvg.Scene.from_workload_scene(wl.scene)
     try:
-        cam, t = list(wl.frames())[24]
-        st = _check_frame(sc, wl.scene, cam, t)
-        print(st)
+        cam, t = list(wl.frames())[k]
+        st = _check_frame(sc, wl.scene, cam, t, check_cull=(k == 24))
         assert st["M"] > 200_000_000 and st["entries"] < st["M"] // 20
     finally:
         sc.close()
 
 
-def test_cfg4_full_size_front_and_side_camera():
-    """6M Gaussians, scales x1.5; the yawed 1920x886 camera has a ragged last tile row."""
+def test_cfg4_full_size_all_cameras_and_timestamps():
+    """6M Gaussians, scales x1.5, five cameras x two timestamps; the yawed 1920x886 cameras have a ragged last tile row."""
     wl = make_config(4)
     sc = pvg.Scene.from_workload_scene(wl.scene)
     try:
-        for cam in (wl.cameras[0], wl.cameras[3]):
-            # ~36k candidates per tile: more pixels come within 1e-4 of a cutoff than at configs 0-3
-            st = _check_frame(sc, wl.scene, cam, 0.25, n_random_tiles=6, max_fragile_frac=0.06)
-            print(cam.name, st)
+        for ci, cam in enumerate(wl.cameras):
+            for ti, t in enumerate(wl.timestamps):
+                st = _check_frame(sc, wl.scene, cam, t, n_random_tiles=4, end_to_end=(ci in (0, 3) and ti == 0),
+                                  check_cull=(ci in (0, 3) and ti == 0))
+                assert st["M"] > 100_000_000, (cam.name, t)
     finally:
         sc.close()

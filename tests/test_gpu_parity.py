@@ -9,7 +9,7 @@ import pytest
 import oracle
 import paper_2311_18561_b200 as pvg
 from helpers import cam_simple, one_scene
-from parity import check_images, check_integer_chain, check_record
+from parity import check_images, check_integer_chain, check_record, e2e_slack, fragile_cap, oracle_preprocess
 from workloads import make_config, pinhole_camera
 
 pytestmark = pytest.mark.gpu
@@ -31,19 +31,22 @@ def full_parity(wl_scene, cam, t, presort=True, end_to_end=True, brute=False, sc
     finally:
         if own:
             sc.close()
-    wide, orec = oracle.preprocess_scene(wl_scene, cam, t, **(state or {}))
+    wide, orec = oracle_preprocess(wl_scene, cam, t, **(state or {}))
     stats = {"P": check_record(dbg["record"], wide, cam, wl_scene),
              "I": check_integer_chain(dbg, cam.width, cam.height, presort)}
     grec = dbg["record"]
     zmax = float(max(grec[:, 2].max(), 1.0))
     mode = "brute" if brute else "binned"
     ora = oracle.render(grec, cam.width, cam.height, bg=cam.bg, mode=mode)
-    stats["R"] = check_images((rgb, depth, alpha), ora, zmax, label="gpu-record")
+    npx = cam.width * cam.height
+    stats["R"] = check_images((rgb, depth, alpha), ora, zmax, label="gpu-record", max_fragile_frac=fragile_cap(grec, ora, npx))
     if end_to_end:
-        ora2 = oracle.render(orec, cam.width, cam.height, bg=cam.bg, mode="binned", tie_budget=True)
-        # end to end the two records differ by fp32 rounding of the preprocess: the tolerance
-        # adds the image-space effect of that
-        stats["E"] = check_images((rgb, depth, alpha), ora2, zmax, tol_rgb=1e-3, label="end-to-end")
+        # end to end (nothing shared): Oracle-R on Oracle-P's own record. The contract tolerance 2e-4 plus the fragile
+        # budget plus the allowance DERIVED per pixel from how far (P) lets the two records differ
+        ora2 = oracle.render(orec, cam.width, cam.height, bg=cam.bg, mode="binned", tie_budget=True,
+                             slack=e2e_slack(wide, wl_scene, cam))
+        stats["E"] = check_images((rgb, depth, alpha), ora2, zmax, label="end-to-end",
+                                  max_fragile_frac=fragile_cap(orec, ora2, npx, end_to_end=True))
     print(json.dumps(stats))
     return stats
 
@@ -152,7 +155,7 @@ def test_time_pins_on_gpu():
     lin = pvg.Scene(s.mu, s.quat, s.scale, s.opacity, s.sh, s.tau, s.beta, s.vel, cycle=float("inf"))
     lin.render(cam, 0.5)
     rec = lin.debug(["record"])["record"]
-    wide, _ = oracle.preprocess(s.mu, s.quat, s.scale, s.opacity, s.sh, s.tau, s.beta, s.vel, np.inf, 3, cam, 0.5)
+    wide, _ = oracle.preprocess(s.mu, s.quat, s.scale, s.opacity, s.sh, s.tau, s.beta, s.vel, np.inf, 3, cam, 0.5)   # 0.5, inf: fp32 numbers
     check_record(rec, wide, cam, s)
     for x in (static, at_tau, lin):
         x.close()
@@ -347,7 +350,7 @@ def test_fuzz_resolutions_and_poses_bit_exact():
         check_integer_chain(dbg, w, h, True)
         grec = dbg["record"]
         ora = oracle.render(grec, w, h, bg=cam.bg, mode="binned")
-        check_images((rgb, depth, alpha), ora, float(max(grec[:, 2].max(), 1.0)), label=f"fuzz {it}", max_fragile_frac=1.0)
+        check_images((rgb, depth, alpha), ora, float(max(grec[:, 2].max(), 1.0)), label=f"fuzz {it}", max_fragile_frac=fragile_cap(grec, ora, w * h))
 
 
 def test_instance_overflow_is_an_error_not_a_crash():
@@ -525,3 +528,51 @@ def test_render_host_async_through_a_scene_and_its_fork():
             assert torch.equal(x, r)
     handles[1].close()
     a.close()
+
+
+def test_stream_switch_orders_frames_on_the_shared_workspace():
+    """Consecutive frames of ONE scene under different torch streams (pvg_set_stream): the second frame must run
+    behind the first on the scene's workspace, so every frame equals the same frame rendered alone."""
+    import torch
+    wl = make_config(1, n=150_000)
+    cam = wl.cameras[0]
+    ts = [k / 11.0 for k in range(12)]
+    g = pvg.Scene.from_workload_scene(wl.scene)
+    ref = [[x.clone() for x in g.render(cam, t)] for t in ts]
+    torch.cuda.synchronize()
+    lanes = [torch.cuda.Stream() for _ in range(3)]
+    outs = []
+    for k, t in enumerate(ts):
+        with torch.cuda.stream(lanes[k % 3]):
+            outs.append(g.render(cam, t))
+    torch.cuda.synchronize()
+    for r, o in zip(ref, outs):
+        assert all(torch.equal(x, y) for x, y in zip(r, o))
+    g.close()
+
+
+def test_debug_view_follows_the_options_of_the_last_render():
+    """Options changed between a render and pvg_debug_view must not be applied to the finished frame: the view
+    completes THAT frame (lazy lists written with the frame's chunk count; no unsorted list that was never kept)."""
+    wl = make_config(1, n=60_000)
+    cam = wl.cameras[0]
+    g = pvg.Scene.from_workload_scene(wl.scene)
+    g.set_option(pvg.OPT_KEEP_UNSORTED, 1)
+    g.render(cam, 0.5)
+    ref = g.debug()
+    for mode in ("blocks", "compact", "keys64"):
+        g.set_option(pvg.OPT_BLOCK_BINS, 1 if mode == "blocks" else 0)
+        g.set_option(pvg.OPT_COMPACT_KEYS, 0 if mode == "keys64" else 1)
+        g.set_option(pvg.OPT_KEEP_UNSORTED, 0)
+        g.set_option(pvg.OPT_LAZY_CHUNKS, 2)
+        g.render(cam, 0.5)
+        assert g.frame_stats()["list_mode"] == mode
+        g.set_option(pvg.OPT_KEEP_UNSORTED, 1)      # after the render: nothing was kept
+        g.set_option(pvg.OPT_LAZY_CHUNKS, 7)
+        g.set_option(pvg.OPT_PRESORT_DEPTH, 0)
+        d = g.debug()
+        g.set_option(pvg.OPT_PRESORT_DEPTH, 1)
+        assert d["keys_unsorted"] is None and d["vals_unsorted"] is None
+        assert np.array_equal(d["vals_sorted"], ref["vals_sorted"]) and np.array_equal(d["keys_sorted"], ref["keys_sorted"])
+        assert np.array_equal(d["visit_order"], ref["visit_order"])
+    g.close()

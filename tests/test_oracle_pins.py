@@ -813,3 +813,96 @@ class TestDynamicsTarget:
         for ch in range(3):
             assert np.allclose(vel_img[ch], a * float(np.float32(f[0, ch])), rtol=1e-12, atol=1e-15)
         assert np.allclose(rho_img, a * float(np.float32(f[0, 3])), rtol=1e-12, atol=1e-15) and a.max() > 0.8
+
+
+# ----------------------------------------------------------------------------- end-to-end allowance
+class TestEndToEndAllowance:
+    """oracle.render(slack=...): the per-pixel allowance `derived` must bound what the image of
+    ANOTHER record does when that record lies within the stated per-Gaussian slack of this one. Pinned by brute
+    force: perturb a record inside its slack (random signs, the worst corner of the box) and render both."""
+
+    def _records(self, seed=3, n=600):
+        wl = make_config(0, n=n, seed=seed)
+        cam = wl.cameras[0]
+        _, rec = oracle.preprocess_scene(wl.scene, cam, 0.37)
+        return rec, cam
+
+    def test_zero_slack_changes_nothing(self):
+        rec, cam = self._records()
+        a = oracle.render(rec, cam.width, cam.height)
+        b = oracle.render(rec, cam.width, cam.height, slack=np.zeros((rec.shape[0], 6)))
+        assert np.array_equal(a["rgb"], b["rgb"]) and np.array_equal(a["budget"], b["budget"])
+        assert np.all(b["derived"] == 0) and np.all(a["derived"] == 0)
+
+    @pytest.mark.parametrize("which", ["mean", "conic", "opacity", "colour", "all"])
+    def test_derived_bounds_the_image_of_a_perturbed_record(self, which):
+        rec, cam = self._records()
+        n = rec.shape[0]
+        rng = np.random.default_rng(11)
+        live = rec[:, 3] > 0
+        sl = np.zeros((n, 6))
+        if which in ("mean", "all"):
+            sl[:, 0] = sl[:, 1] = 2e-4
+        if which in ("conic", "all"):
+            sl[:, 2] = 1e-5 * np.sqrt(np.abs(rec[:, 4] * rec[:, 6]))
+        if which in ("opacity", "all"):
+            sl[:, 3] = 3e-5
+        if which in ("colour", "all"):
+            sl[:, 4] = 2e-5
+        sl[~live] = 0
+        base = oracle.render(rec, cam.width, cam.height, slack=sl)
+        assert base["derived"].max() > 0
+        worst = 0.0
+        for trial in range(6):
+            sg = rng.choice([-1.0, 1.0], size=(n, 8))
+            p = rec.astype(np.float64).copy()
+            p[:, 0] += sg[:, 0] * sl[:, 0]
+            p[:, 1] += sg[:, 1] * sl[:, 1]
+            for j, col in enumerate((4, 5, 6)):
+                p[:, col] += sg[:, 2 + j] * sl[:, 2]
+            p[:, 3] *= np.exp(sg[:, 5] * sl[:, 3])
+            p[:, 8:11] += sg[:, 6:7] * sl[:, 4:5]
+            p32 = p.astype(np.float32)
+            p32[~live] = rec[~live]
+            # the perturbed record is itself rounded to fp32: one more half ulp of every field, far below the slack
+            other = oracle.render(p32, cam.width, cam.height)
+            err = np.abs(other["rgb"] - base["rgb"]).max(0)
+            allow = 1e-7 + base["derived"] + base["budget"]
+            assert np.all(err <= allow), (which, trial, float((err - allow).max()))
+            ea = np.abs(other["alpha"] - base["alpha"])
+            assert np.all(ea <= 1e-7 + (base["derived"] + base["budget"]) / min(1.0, base["c_max"]))
+            clean = base["budget"] == 0
+            worst = max(worst, float((err[clean] / np.maximum(base["derived"][clean], 1e-30)).max()))
+        # the bound is not vacuous: random sign patterns reach a fair share of it
+        assert worst > 0.02, worst
+
+    def test_slack_widens_the_cutoff_window(self):
+        """A Gaussian whose alpha at a pixel is 1e-3 relative below 1/255 is not fragile on its own, but is once the
+        other record's opacity may be 2e-3 higher (it would then pass the cutoff there)."""
+        rows = np.stack([record_row(8.5, 8.5, 3.0, (1.0 / 255.0) * (1 - 1e-3), 0.02, 0.0, 0.02)])
+        a = oracle.render(rows, 16, 16)
+        assert a["budget"][8, 8] == 0
+        sl = np.zeros((1, 6))
+        sl[0, 3] = 2e-3
+        b = oracle.render(rows, 16, 16, slack=sl)
+        assert b["budget"][8, 8] > 0
+
+    def test_depth_slack_flags_only_reachable_swaps(self):
+        """Two overlapping layers whose depth bits differ by one ulp: with d z = 0 on both the other record visits them
+        in the same order (no flag); with d z = 1 ulp on either, a swap is possible and the pixel is flagged with
+        alpha_1 alpha_2 T c_max. Equal bits with d z = 0 keep index order on both sides: no flag."""
+        z0 = np.float32(3.0)
+        z1 = np.nextafter(z0, np.float32(4.0))
+        for zb, dz, want in ((z1, 0.0, False), (z1, 1.0, True), (z0, 0.0, False), (np.float32(3.5), 1.0, False)):
+            rows = np.stack([record_row(8.5, 8.5, z0, 0.5, 0.02, 0.0, 0.02, rgb=(1, 0, 0)),
+                             record_row(8.5, 8.5, zb, 0.5, 0.02, 0.0, 0.02, rgb=(0, 1, 0))])
+            sl = np.zeros((2, 6))
+            sl[1, 5] = dz
+            o = oracle.render(rows, 16, 16, tie_budget=True, slack=sl)
+            assert (o["budget"][8, 8] > 0) == want, (zb, dz)
+            if want:
+                assert np.isclose(o["budget"][8, 8], 0.5 * 0.5 * 1.0 * 1.0)      # = |C(swapped) - C| per channel here
+                swapped = rows.copy()
+                swapped[0, 2], swapped[1, 2] = rows[1, 2], rows[0, 2]      # the other depth order
+                sw = oracle.render(swapped, 16, 16)
+                assert np.isclose(np.abs(sw["rgb"][:, 8, 8] - o["rgb"][:, 8, 8]).max(), 0.25)
