@@ -57,6 +57,11 @@ def parse_args():
                     help="with --split band on ONE GPU: time the bands of a K-way split one after another and "
                          "report the slowest band per frame (what one of K GPUs would compute; no collective)")
     ap.add_argument("--lazy-chunks", type=int, default=-1, help="PVG_OPT_LAZY_CHUNKS (-1: the library default)")
+    ap.add_argument("--no-legs", action="store_true", help="skip the complete_lists / parked / sustained legs")
+    ap.add_argument("--sustained-seconds", type=float, default=2.5)
+    ap.add_argument("--selftest-spawn", action="store_true",
+                    help="CPU self-test of the --gpus N launch path: the ranks rendezvous over gloo, take the max of a "
+                         "dummy time and rank 0 prints a line with n_gpus (no CUDA work)")
     ap.add_argument("--event-stride", type=int, default=5,
                     help="record per-kernel CUDA events on every k-th timed frame (each record costs ~2 us of stream time)")
     return ap.parse_args()
@@ -158,56 +163,41 @@ def physical_gpu_index(local_rank: int) -> int:
 
 
 # ------------------------------------------------------------------------------------------
-_ORACLE_FIXED = {}
-
-
-def oracle_frame_time(wl, cam, t, sample_tiles: int, seed: int):
-    """Times the CPU oracle (as it stands) on one frame. sample_tiles <= 0: the whole frame, Oracle-P on all N
-    Gaussians + Oracle-R (binned) on every tile -- no extrapolation. Otherwise a bounded sample: Oracle-P on all N +
-    Oracle-R (binned) on `sample_tiles` uniformly sampled tiles; Oracle-R's cost that does not depend on the selection
-    (depth order of all Gaussians, the walk over every rectangle: measured once with an empty selection) is counted
-    once and only the remainder is scaled to the frame. Returns (seconds per frame, detail dict)."""
+def oracle_frame_time(wl, cam, t, sample_tiles: int = 0, seed: int = 0):
+    """Times the CPU oracle (as it stands) on ONE WHOLE frame: Oracle-P on all N Gaussians + Oracle-R (binned) on
+    every tile. Nothing is sampled or extrapolated. Returns (seconds, detail dict)."""
     import oracle
     tiles_total = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
     t0 = time.perf_counter()
     _, rec = oracle.preprocess_scene(wl.scene, cam, t)
     t1 = time.perf_counter()
-    if sample_tiles <= 0 or sample_tiles >= tiles_total:
-        oracle.render(rec, cam.width, cam.height, bg=cam.bg, mode="binned")
-        t2 = time.perf_counter()
-        return t2 - t0, dict(preprocess_s=t1 - t0, tiles_s=t2 - t1, tiles=int(tiles_total), tiles_total=int(tiles_total),
-                             fixed_s=0.0)
-    key = (wl.scene.n, cam.width, cam.height)
-    if key not in _ORACLE_FIXED:
-        f0 = time.perf_counter()
-        oracle.render(rec, cam.width, cam.height, bg=cam.bg, mode="binned", tiles=np.zeros(0, dtype=np.uint32))
-        _ORACLE_FIXED[key] = time.perf_counter() - f0
-    fixed = _ORACLE_FIXED[key]
-    rng = np.random.default_rng(seed)
-    sel = np.sort(rng.choice(tiles_total, size=sample_tiles, replace=False)).astype(np.uint32)
-    t1 = time.perf_counter()
-    oracle.render(rec, cam.width, cam.height, bg=cam.bg, mode="binned", tiles=sel)
+    oracle.render(rec, cam.width, cam.height, bg=cam.bg, mode="binned")
     t2 = time.perf_counter()
-    est = (t1 - t0) + fixed + max(0.0, (t2 - t1) - fixed) * tiles_total / len(sel)
-    return est, dict(preprocess_s=t1 - t0, tiles_s=t2 - t1, tiles=int(len(sel)), tiles_total=int(tiles_total), fixed_s=fixed)
+    return t2 - t0, dict(preprocess_s=t1 - t0, tiles_s=t2 - t1, tiles=int(tiles_total), tiles_total=int(tiles_total))
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores; rank 0 only."""
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only. Every step is ONE WHOLE FRAME
+    (Oracle-P on all N Gaussians + Oracle-R binned on every tile): nothing is sampled or extrapolated, so the figure
+    agrees with the `cpu_baseline` the GPU arm measures on the same box (3 s per config-3 frame on 16 cores: the default
+    50 + 3 steps take under three minutes)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
     from workloads import make_config
+    if "WORLD_SIZE" in os.environ:
+        # torchrun exports OMP_NUM_THREADS=1 to its workers; the oracle is timed on all the host cores it may use
+        oracle.set_threads(len(os.sched_getaffinity(0)))
     wl = make_config(args.config, args.n)
     frames = list(wl.frames())
-    sample = 480 if args.steps + args.warmup > 8 else 0   # few steps: whole frames, no extrapolation
     times = []
+    det = None
     for s in range(args.warmup + args.steps):
         cam, t = frames[s % len(frames)]
-        est, det = oracle_frame_time(wl, cam, t, sample, seed=s)
+        sec, det = oracle_frame_time(wl, cam, float(np.float32(t)), 0, seed=s)
         if s >= args.warmup:
-            times.append(est)
+            times.append(sec)
     sec = float(np.mean(times))
     fps = 1.0 / sec
     line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -216,14 +206,155 @@ def run_reference(args):
             "config": {"workload": CONFIG_NAMES[args.config], "n_gaussians": wl.scene.n,
                        "resolution": f"{frames[0][0].width}x{frames[0][0].height}"},
             "cpu_baseline": {"value": fps, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                             "sample": (f"per step: Oracle-P on all {wl.scene.n} Gaussians + Oracle-R (binned) on {det['tiles']} of "
-                                        f"{det['tiles_total']} tiles; Oracle-R's selection-independent part "
-                                        f"({det['fixed_s']:.2f} s) counted once, the rest scaled to the frame")},
+                             "sample": (f"every step one whole frame: Oracle-P on all {wl.scene.n} Gaussians + Oracle-R (binned) "
+                                        f"on all {det['tiles_total']} tiles; no sampling, no extrapolation")},
             "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
 
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without a torchrun environment: start the N ranks here (one process per GPU, the
+    launch line the driver uses) and pass their output through; rank 0 prints the one JSON line."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_selftest_spawn(args):
+    """The plumbing of an N-rank run without CUDA: gloo rendezvous, barrier, max over ranks, one line from rank 0."""
+    from paper_2311_18561_b200 import dist
+    rank, local_rank, ws = dist.init("gloo")
+    frames = [("cam", k / 49.0) for k in range(50)]
+    sched = dist.frame_schedule(rank, ws, args.steps, frames)
+    dist.barrier()
+    elapsed = dist.max_over_ranks(1e-3 * (rank + 1))
+    total = dist.sum_over_ranks(len(sched))
+    dist.barrier()
+    if rank == 0:
+        print(json.dumps({"selftest": "spawn", "n_gpus": ws, "steps": args.steps, "frames_total": int(total),
+                          "elapsed_max_s": elapsed}), flush=True)
+    dist.shutdown()
+
+
 # ------------------------------------------------------------------------------------------
+def algorithmic_bytes(agg, K, N, S, Msum, Mbsum, chunks, lazy):
+    """Algorithmic HBM bytes over the K sampled frames, per (kernel, stage)."""
+    alg = {("preprocess", "preprocess"): K * (64.0 * N + 80.0 * N + 192.0 * S),
+           ("scan_counts", "duplicate"): K * 12.0 * N,   # 8 B sorted key (or 4 B visit + 4 B count) + 4 B offset
+           # block-entry path (blockbin.cuh): 13 B entries (u8 block, u32 Gaussian, u64 mask)
+           ("bin_expand", "duplicate"): 13.0 * Mbsum + K * 16.0 * S,
+           ("tile_grid", "ranges"): K * 16.0 * N,
+           ("bin_pass", "sort"): 25.0 * Mbsum,
+           ("bin_emit", "sort"): 12.0 * Mbsum + K * 16.0 * S,   # fused expand + split: 16 B per survivor read, (u32 g, u64 mask) written
+           ("bin_write", "sort"): 12.0 * Mbsum + 4.0 * Msum + 256.0 * chunks,
+           ("duplicate", "duplicate"): (6.0 if any(k[0] == "compact_pass_last" for k in agg) else 12.0) * Msum,
+           ("compact_pass", "sort"): 12.0 * Msum * (agg.get(("compact_pass", "sort"), [0, K])[1] / K),
+           ("compact_pass_last", "sort"): 10.0 * Msum,
+           ("onesweep_histogram", "sort"): 8.0 * Msum,
+           ("onesweep_histogram", "depth_sort"): K * 8.0 * N,
+           ("tile_ranges", "ranges"): 8.0 * Msum}
+    if lazy:
+        # deferred records: preprocess reads the 64 B model + 1 B flag and writes tile info, count and depth pair (32 B)
+        alg[("preprocess", "preprocess")] = K * 97.0 * N
+        # lazy lists: bin_emit forms the first 1/8 of the entries and bin_write the first chunks of every block -- what
+        # they move depends on where the tiles saturate, so no algorithmic-byte figure is claimed for them
+        alg.pop(("bin_emit", "sort"), None)
+        alg.pop(("bin_write", "sort"), None)
+    for key in (("onesweep_pass", "sort"), ("onesweep_pass", "depth_sort")):
+        if key in agg:
+            per_frame = agg[key][1] / K
+            alg[key] = 24.0 * (Msum if key[1] == "sort" else K * N) * per_frame
+    return alg
+
+
+def timed_frames(pvg, torch, dist, scene, sched, cams, out_by_cam, local_rank, dev, stride, on_start=None, on_end=None):
+    """K frames, inputs resident in HBM, device-timed with CUDA events on the current stream, barrier + synchronize on
+    both sides, max over ranks. Per-kernel CUDA-event records on every stride-th frame."""
+    scene.set_option(pvg.OPT_EVENT_STRIDE, stride)
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 2)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    Ms, Mbs, parked = [], [], []
+    dist.barrier(local_rank)
+    torch.cuda.synchronize()
+    if on_start:
+        on_start()
+    e0.record()
+    for cam, t in sched:
+        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+        fs = scene.frame_stats()
+        Ms.append(fs["M"])
+        Mbs.append(fs["block_entries"])
+    e1.record()
+    torch.cuda.synchronize()
+    if on_end:
+        on_end()
+    dist.barrier(local_rank)
+    elapsed_s = dist.max_over_ranks(e0.elapsed_time(e1) / 1e3, dev)
+    krecs = scene.kernel_times_ms()
+    scene.set_option(pvg.OPT_EVENT_STRIDE, 1)
+    scene.set_option(pvg.OPT_KERNEL_EVENTS, 0)
+    return dict(elapsed_s=elapsed_s, krecs=krecs, Ms=Ms, Mbs=Mbs, parked=scene.frame_stats()["parked_tiles"])
+
+
+def count_pairs(pvg, scene, sched, cams, out_by_cam):
+    """Blend work (pairs evaluated / contributing) of the same frames, counted in an untimed pass."""
+    scene.set_option(pvg.OPT_COUNT_PAIRS, 1)
+    ev = co = 0
+    for cam, t in sched:
+        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+        a, b = scene.blend_counters()
+        ev += a
+        co += b
+    scene.set_option(pvg.OPT_COUNT_PAIRS, 0)
+    return ev, co
+
+
+def kernel_table(run, stride, N, S, lazy, hbm_peak, alu_peak, pairs=None):
+    """Per-kernel aggregation of one timed loop: times, shares, achieved GB/s or thread-instructions/s, and per-stage
+    ms and Gaussians/s (north_star: 'frames/sec and Gaussians/sec per stage')."""
+    Kall = len(run["Ms"])
+    sampled = list(range(0, Kall, stride))
+    K = len(sampled)
+    Msum, Mbsum = float(sum(run["Ms"][i] for i in sampled)), float(sum(run["Mbs"][i] for i in sampled))
+    chunks = Mbsum / 512 + K * 150
+    agg = {}
+    for name, stage, ms in run["krecs"]:
+        a = agg.setdefault((name, stage), [0.0, 0])
+        a[0] += ms
+        a[1] += 1
+    alg = algorithmic_bytes(agg, K, N, S, Msum, Mbsum, chunks, lazy)
+    frame_ms = run["elapsed_s"] * 1e3 / Kall
+    kernels = {}
+    for (name, stage), (ms, cnt) in agg.items():
+        d = {"launches": cnt, "ms_total": ms, "ms_avg": ms / cnt, "ms_per_frame": ms / K, "share": (ms / K) / frame_ms}
+        b = alg.get((name, stage))
+        if b:
+            d["GBps"] = b / (ms * 1e-3) / 1e9
+            d["hbm_frac"] = d["GBps"] / hbm_peak
+            d["algorithmic_bytes_per_launch"] = b / cnt
+        kernels[f"{stage}/{name}"] = d
+    bl = agg.get(("blend", "blend"))
+    if bl and pairs:
+        ev, co = pairs
+        slots = (SLOTS_REJECT * ev + SLOTS_ACCEPT_EXTRA * co) * K / Kall   # pairs were counted on all frames
+        k = kernels["blend/blend"]
+        k["pairs_eval_per_frame"] = ev / Kall
+        k["pairs_contrib_per_frame"] = co / Kall
+        k["Tinstr_per_s"] = slots / (bl[0] * 1e-3) / 1e12
+        k["alu_frac"] = k["Tinstr_per_s"] / alu_peak
+    stage_ms, stage_gps = {}, {}
+    for (name, stage), (ms, cnt) in agg.items():
+        stage_ms[stage] = stage_ms.get(stage, 0.0) + ms / K
+    for stage, ms in stage_ms.items():
+        stage_gps[stage] = N / (ms * 1e-3) if ms > 0 else None
+    return dict(kernels=kernels, agg=agg, alg=alg, stage_ms=stage_ms, stage_gaussians_per_s=stage_gps, K=K, Kall=Kall,
+                Msum=Msum, Mbsum=Mbsum, launches_per_frame=len(run["krecs"]) / K)
+
+
 def run_ours(args):
     import torch
     import paper_2311_18561_b200 as pvg
@@ -256,54 +387,34 @@ def run_ours(args):
 
     out_by_cam = {k: outs(c) for k, c in {id(c): c for c, _ in frames}.items()}
 
+    def warm_up(sc):
+        for cam, t in warm:
+            sc.render(cams[id(cam)], t, out_by_cam[id(cam)])
+        torch.cuda.synchronize()
+
     # ---- warm-up (also sizes the workspace)
-    for cam, t in warm:
-        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
-    torch.cuda.synchronize()
+    warm_up(scene)
+
+    # ---- the ALU / issue peak of this device, measured: FFMA only, FFMA + LOP3, packed FFMA2
+    calib = {}
+    for mode, name in ((0, "ffma"), (1, "ffma_lop3"), (2, "ffma2")):
+        rate, sms = pvg.calibrate_fp32(mode)
+        calib[name] = rate / 1e12
+    calib["sms"] = sms
 
     # ---- timed region: K frames, inputs resident in HBM, device-timed, max over ranks
     sampler = ClockSampler(physical_gpu_index(local_rank)) if rank == 0 else None
     time.sleep(0.3 if sampler else 0.0)
     stride = max(1, min(args.event_stride, len(sched)))
-    scene.set_option(pvg.OPT_EVENT_STRIDE, stride)
-    scene.set_option(pvg.OPT_KERNEL_EVENTS, 2)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    Ms, Mbs = [], []
-    dist.barrier(local_rank)
-    torch.cuda.synchronize()
-    if sampler:
-        sampler.mark_start()
-    e0.record()
-    for cam, t in sched:
-        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
-        fs = scene.frame_stats()
-        Ms.append(fs["M"])
-        Mbs.append(fs["block_entries"])
-    e1.record()
-    torch.cuda.synchronize()
-    if sampler:
-        sampler.mark_end()
-    dist.barrier(local_rank)
-    elapsed_s = dist.max_over_ranks(e0.elapsed_time(e1) / 1e3, dev)
-    krecs = scene.kernel_times_ms()
+    main = timed_frames(pvg, torch, dist, scene, sched, cams, out_by_cam, local_rank, dev, stride,
+                        on_start=sampler.mark_start if sampler else None, on_end=sampler.mark_end if sampler else None)
     clocks = sampler.stop() if sampler else None
-    scene.set_option(pvg.OPT_EVENT_STRIDE, 1)
-    scene.set_option(pvg.OPT_KERNEL_EVENTS, 1)
+    elapsed_s = main["elapsed_s"]
     total_frames = args.steps * ws
     fps = total_frames / elapsed_s
-
-    # ---- blend work (pairs) of the same frames, counted in an untimed pass
-    scene.set_option(pvg.OPT_COUNT_PAIRS, 1)
-    pairs_eval = pairs_contrib = 0
-    for cam, t in sched:
-        scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
-        a, b = scene.blend_counters()
-        pairs_eval += a
-        pairs_contrib += b
-    scene.set_option(pvg.OPT_COUNT_PAIRS, 0)
+    pairs = count_pairs(pvg, scene, sched, cams, out_by_cam)
 
     # ---- two frames in flight: the same K frames through the scene and a fork of it (shared model), on two streams
-    scene.set_option(pvg.OPT_KERNEL_EVENTS, 0)      # the per-kernel timing hook is a measurement aid, not the user's call
     handles = [scene, scene.fork()]
     lanes = [torch.cuda.Stream(), torch.cuda.Stream()]
     out2 = [out_by_cam, {k: outs(c) for k, c in {id(c): c for c, _ in frames}.items()}]
@@ -365,8 +476,9 @@ def run_ours(args):
                "note": "pvg_render_host_async + pvg_wait_host, two frames in flight (scene + pvg_fork_scene): per-step input is "
                        "(camera, t); every frame's rgb+depth+alpha is copied to pinned host memory inside the timed region, the "
                        "copies overlapping the following renders"}
+        del host
     handles[1].close()
-    scene.set_option(pvg.OPT_KERNEL_EVENTS, 1)
+    torch.cuda.synchronize()
 
     if rank != 0:
         scene.close()
@@ -377,91 +489,100 @@ def run_ours(args):
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     N = wl.scene.n
     S = scene.frame_stats()["survivors"] or N
-    # per-kernel events were recorded on frames 0, stride, 2 stride, ... of the timed region: the per-kernel sums below
-    # (and the algorithmic bytes they are divided into) are over those frames; K counts them
-    Kall = len(sched)
-    sampled = list(range(0, Kall, stride))
-    Msum, Mbsum = float(sum(Ms[i] for i in sampled)), float(sum(Mbs[i] for i in sampled))
-    K = len(sampled)
     list_mode = scene.frame_stats()["list_mode"]
-    chunks = Mbsum / 512 + K * 150
-    agg = {}
-    for name, stage, ms in krecs:
-        a = agg.setdefault((name, stage), [0.0, 0])
-        a[0] += ms
-        a[1] += 1
-    # algorithmic bytes over the timed region, per (kernel, stage)
-    alg = {("preprocess", "preprocess"): K * (64.0 * N + 80.0 * N + 192.0 * S),
-           ("scan_counts", "duplicate"): K * 12.0 * N,   # 8 B sorted key (or 4 B visit + 4 B count) + 4 B offset
-           # block-entry path (blockbin.cuh): 13 B entries (u8 block, u32 Gaussian, u64 mask)
-           ("bin_expand", "duplicate"): 13.0 * Mbsum + K * 16.0 * S,
-           ("tile_grid", "ranges"): K * 16.0 * N,
-           ("bin_pass", "sort"): 25.0 * Mbsum,
-           ("bin_emit", "sort"): 12.0 * Mbsum + K * 16.0 * S,   # fused expand + split: 16 B per survivor read, (u32 g, u64 mask) written
-           ("bin_count", "sort"): 8.0 * Mbsum + 256.0 * chunks,
-           ("bin_chunk_scan", "sort"): 512.0 * chunks,
-           ("bin_write", "sort"): 12.0 * Mbsum + 4.0 * Msum + 256.0 * chunks,
-           ("duplicate", "duplicate"): (6.0 if any(k[0] == "compact_pass_last" for k in agg) else 12.0) * Msum,
-           ("compact_pass", "sort"): 12.0 * Msum * (agg.get(("compact_pass", "sort"), [0, K])[1] / K),
-           ("compact_pass_last", "sort"): 10.0 * Msum,
-           ("onesweep_histogram", "sort"): 8.0 * Msum,
-           ("onesweep_pass", "sort"): 0.0,   # filled below: 24 B per instance per launch
-           ("onesweep_histogram", "depth_sort"): K * 8.0 * N,
-           ("onesweep_pass", "depth_sort"): 0.0,
-           ("tile_ranges", "ranges"): 8.0 * Msum,
-           ("tile_prefix", "ranges"): 0.0}
     lazy = list_mode == "blocks" and args.lazy_chunks != 0
-    if lazy:
-        # deferred records: preprocess reads the 64 B model + 1 B flag and writes tile info, count and depth pair (32 B)
-        alg[("preprocess", "preprocess")] = K * 97.0 * N
-        # lazy lists: bin_emit forms the first 1/8 of the entries and bin_write the first chunks of every block -- what
-        # they move depends on where the tiles saturate, so no algorithmic-byte figure is claimed for them
-        alg.pop(("bin_emit", "sort"), None)
-        alg.pop(("bin_write", "sort"), None)
-    for key in (("onesweep_pass", "sort"), ("onesweep_pass", "depth_sort")):
-        if key in agg:
-            per_frame = agg[key][1] / K
-            alg[key] = 24.0 * (Msum if key[1] == "sort" else K * N) * per_frame
-    kernels = {}
-    for (name, stage), (ms, cnt) in agg.items():
-        d = {"launches": cnt, "ms_total": ms, "ms_avg": ms / cnt, "share": (ms / K) / (elapsed_s * 1e3 / Kall)}
-        b = alg.get((name, stage))
-        if b:
-            d["GBps"] = b / (ms * 1e-3) / 1e9
-            d["hbm_frac"] = d["GBps"] / hbm_peak
-        kernels[f"{stage}/{name}"] = d
     sm_mhz = (clocks or {}).get("sm_mhz") or sm_max_mhz
-    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e12    # T thread-instr/s at the observed SM clock
-    bl = agg.get(("blend", "blend"))
-    if bl:
-        slots = (SLOTS_REJECT * pairs_eval + SLOTS_ACCEPT_EXTRA * pairs_contrib) * K / Kall   # pairs were counted on all frames
-        k = kernels["blend/blend"]
-        k["pairs_eval_per_frame"] = pairs_eval / Kall
-        k["pairs_contrib_per_frame"] = pairs_contrib / Kall
-        k["Tinstr_per_s"] = slots / (bl[0] * 1e-3) / 1e12
-        k["alu_frac"] = k["Tinstr_per_s"] / alu_peak
+    nominal = calib["sms"] * 128 * sm_mhz * 1e6 / 1e12    # T thread-instr/s at the observed SM clock
+    # the denominator of the ALU roofline: the best issue rate the microbenchmark reached on this device
+    alu_peak = max(calib["ffma"], calib["ffma_lop3"])
+    tab = kernel_table(main, stride, N, S, lazy, hbm_peak, alu_peak, pairs)
+    kernels, agg, alg, K, Kall = tab["kernels"], tab["agg"], tab["alg"], tab["K"], tab["Kall"]
     dom = max(agg.items(), key=lambda kv: kv[1][0])[0]
     dk = kernels[f"{dom[1]}/{dom[0]}"]
     workload = CONFIG_NAMES[args.config]
+    alu_src = (f"pvg_calibrate_fp32 on this device ({calib['sms']} SMs from cudaDeviceGetAttribute): FFMA+LOP3 {calib['ffma_lop3']:.2f}, "
+               f"FFMA {calib['ffma']:.2f}, packed FFMA2 {calib['ffma2']:.2f} T thread-instr/s (an FFMA2 counts once); nominal "
+               f"{calib['sms']} x 128 lanes x {sm_mhz:.0f} MHz = {nominal:.2f}")
     if dom[0] == "blend":
         roofline = {"bound": "alu", "achieved": dk["Tinstr_per_s"], "peak": alu_peak, "unit": "Tinstr/s",
                     "frac": dk["alu_frac"], "traffic": ncu_traffic("blend", workload), "kernel": "blend_kernel",
-                    "peak_source": f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (observed)"}
+                    "peak_source": alu_src, "frac_of_nominal": dk["Tinstr_per_s"] / nominal}
     else:
         roofline = {"bound": "hbm", "achieved": dk.get("GBps"), "peak": hbm_peak, "unit": "GB/s", "frac": dk.get("hbm_frac"),
                     "traffic": ncu_traffic(dom[0], workload), "kernel": f"{dom[0]} ({dom[1]} stage)",
                     "peak_source": peak_src, "avg_launch_ms": dk["ms_avg"],
                     "algorithmic_bytes_per_launch": alg[dom] / agg[dom][1]}
-    stage_ms = {}
-    for (name, stage), (ms, cnt) in agg.items():
-        stage_ms[stage] = stage_ms.get(stage, 0.0) + ms / K
 
-    # ---- CPU oracle on a bounded sample (reported baseline, not the target)
+    # ---- extra legs (1 GPU only): complete lists, a scene whose tiles park, a sustained loop
+    legs = {}
+    if ws == 1 and not args.no_legs and list_mode == "blocks":
+        # (1) complete lists + eager records (PVG_OPT_LAZY_CHUNKS = 0): every list entry is formed, split and written
+        scene.set_option(pvg.OPT_LAZY_CHUNKS, 0)
+        warm_up(scene)
+        sm1 = ClockSampler(physical_gpu_index(local_rank))
+        time.sleep(0.3)
+        run1 = timed_frames(pvg, torch, dist, scene, sched, cams, out_by_cam, local_rank, dev, stride, sm1.mark_start, sm1.mark_end)
+        ck1 = sm1.stop()
+        pairs1 = count_pairs(pvg, scene, sched, cams, out_by_cam)
+        t1 = kernel_table(run1, stride, N, S, False, hbm_peak, alu_peak, pairs1)
+        legs["complete_lists"] = {
+            "value": total_frames / run1["elapsed_s"], "unit": UNIT, "ms_per_step": run1["elapsed_s"] * 1e3 / args.steps,
+            "clocks": ck1, "stage_ms_per_frame": t1["stage_ms"],
+            "kernels": {k: {a: v[a] for a in ("ms_per_frame", "launches", "GBps", "hbm_frac", "alu_frac", "Tinstr_per_s") if a in v}
+                        for k, v in t1["kernels"].items()},
+            "note": "PVG_OPT_LAZY_CHUNKS=0: full preprocess (records, SH), every block entry emitted and split, every tile list "
+                    "written whole; same frames, same images bit for bit"}
+        scene.set_option(pvg.OPT_LAZY_CHUNKS, args.lazy_chunks if args.lazy_chunks >= 0 else 2)
+
+        # (2) a scene whose tiles do NOT saturate inside the list prefixes: opacity x 0.05 -> tiles park, the second
+        #     round forms the remaining entries and writes the rest of the parked tiles' lists
+        s0 = wl.scene
+        thin = pvg.Scene(s0.mu, s0.quat, s0.scale, (s0.opacity * 0.05).astype(np.float32), s0.sh, s0.tau, s0.beta, s0.vel,
+                         s0.cycle, s0.sh_degree)
+        warm_up(thin)
+        run2 = timed_frames(pvg, torch, dist, thin, sched, cams, out_by_cam, local_rank, dev, stride)
+        t2 = kernel_table(run2, stride, N, thin.frame_stats()["survivors"] or N, True, hbm_peak, alu_peak)
+        legs["parked"] = {
+            "value": total_frames / run2["elapsed_s"], "unit": UNIT, "ms_per_step": run2["elapsed_s"] * 1e3 / args.steps,
+            "parked_tiles_last_frame": run2["parked"], "tiles": int(frames[0][0].width // 16 * (frames[0][0].height // 16)),
+            "instances_per_frame_mean": t2["Msum"] / t2["K"], "stage_ms_per_frame": t2["stage_ms"],
+            "kernels": {k: {"ms_per_frame": v["ms_per_frame"], "launches": v["launches"]} for k, v in t2["kernels"].items()},
+            "note": "the same scene with every opacity x 0.05 (default lazy options): pixels do not saturate inside the list "
+                    "prefixes, the tiles park and the second round completes their lists"}
+        thin.close()
+        del thin
+        torch.cuda.synchronize()
+
+        # (3) sustained: the 50-frame sweep looped for >= sustained_seconds of device time, clocks sampled throughout
+        warm_up(scene)
+        sm3 = ClockSampler(physical_gpu_index(local_rank))
+        time.sleep(0.3)
+        sweep = [frames[k % len(frames)] for k in range(max(len(frames), 50))]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        sm3.mark_start()
+        w0 = time.perf_counter()
+        nfr = 0
+        e0.record()
+        while time.perf_counter() - w0 < args.sustained_seconds:
+            for cam, t in sweep:
+                scene.render(cams[id(cam)], t, out_by_cam[id(cam)])
+            nfr += len(sweep)
+        e1.record()
+        torch.cuda.synchronize()
+        sm3.mark_end()
+        sus_s = e0.elapsed_time(e1) / 1e3
+        legs["sustained"] = {"value": nfr / sus_s, "unit": UNIT, "frames": nfr, "seconds": sus_s, "ms_per_step": sus_s * 1e3 / nfr,
+                             "clocks": sm3.stop(),
+                             "note": "the time sweep looped back to back (one frame at a time, no per-kernel events) for the stated "
+                                     "seconds of device time"}
+
+    # ---- CPU oracle on ONE whole frame (reported baseline, not the target)
     cpu = None
     if not args.no_cpu_baseline and ws == 1:
         import oracle
         cam, t = frames[len(frames) // 2]
-        est, det = oracle_frame_time(wl, cam, t, 0, seed=0)
+        est, det = oracle_frame_time(wl, cam, float(np.float32(t)))
         cpu = {"value": 1.0 / est, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                "sample": f"frame t={t:.3f}: Oracle-P on all {N} Gaussians ({det['preprocess_s']:.2f} s) + Oracle-R (binned) on "
                          f"all {det['tiles_total']} tiles ({det['tiles_s']:.2f} s): one whole frame, no extrapolation"}
@@ -471,18 +592,23 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload, "n_gaussians": N, "survivors_last_frame": S,
                        "resolution": f"{frames[0][0].width}x{frames[0][0].height}",
-                       "instances_per_frame_mean": Msum / K, "block_entries_per_frame_mean": Mbsum / K,
+                       "instances_per_frame_mean": tab["Msum"] / K, "block_entries_per_frame_mean": tab["Mbsum"] / K,
                        "list_mode": list_mode,
                        "lists": ("lazy (PVG_OPT_LAZY_CHUNKS/SLAB defaults): list prefixes, the remainder only for parked tiles; "
-                                 f"parked tiles in the last frame: {scene.frame_stats()['parked_tiles']}") if lazy else "complete",
+                                 f"parked tiles in the last frame: {main['parked']}") if lazy else "complete",
                        "frames": "one (camera, t) per step, round-robin over the sweep",
                        "l2_policy": (f"inputs larger than L2: the model, {N * 256 / 1e6:.0f} MB read every frame, vs 126 MB L2" if lazy else
                                      f"inputs larger than L2: model {N * 256 / 1e6:.0f} MB + sorted list + block entries "
-                                     f"{(4 * Msum + 25 * Mbsum) / K / 1e6:.0f} MB per frame vs 126 MB L2"),
+                                     f"{(4 * tab['Msum'] + 25 * tab['Mbsum']) / K / 1e6:.0f} MB per frame vs 126 MB L2"),
+                       "arithmetic": "fp32; the position chain mu~(t) -> p_cam -> mean2D and the record's conic in fp64 (DESIGN.md 5)",
                        "parallelism": f"frames sharded over {ws} rank(s), no collective", "presort_depth": args.presort},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "pipelined": pipelined, "clocks": clocks, "gpu_launches": int(round(len(krecs) * Kall / K)),
-            "kernel_events": f"recorded on every {stride}th frame of the timed region ({K} of {Kall} frames, {len(krecs)} launches)",
-            "gaussians_per_s": N * fps, "stage_ms_per_frame": stage_ms, "kernels": kernels}
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "pipelined": pipelined, "clocks": clocks,
+            "gpu_launches": int(round(len(main["krecs"]) * Kall / K)),
+            "kernel_events": f"recorded on every {stride}th frame of the timed region ({K} of {Kall} frames, {len(main['krecs'])} launches)",
+            "gaussians_per_s": N * fps, "stage_ms_per_frame": tab["stage_ms"],
+            "stage_gaussians_per_s": tab["stage_gaussians_per_s"], "alu_calibration_Tinstr_per_s": calib,
+            "kernels": kernels}
+    line.update(legs)
     print(json.dumps(line), flush=True)
     scene.close()
     dist.shutdown()
@@ -558,7 +684,12 @@ def run_band_split(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    if a.impl == "reference":
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: start the ranks ourselves (one process per GPU), so that `--gpus N` is real
+        sys.exit(spawn_ranks(a))
+    if a.selftest_spawn:
+        run_selftest_spawn(a)
+    elif a.impl == "reference":
         run_reference(a)
     elif a.split == "band":
         run_band_split(a)

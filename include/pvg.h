@@ -284,6 +284,14 @@ int pvg_blend_counters(pvg_scene *scene, uint64_t out[2]);
 int pvg_sort_pairs(uint64_t n, uint64_t *keys_in, uint32_t *vals_in, uint64_t *keys_out,
                    uint32_t *vals_out, int begin_bit, int end_bit, void *cuda_stream);
 
+/* Measurement hook for the roofline of the ALU-bound blend ("calibrate with an FFMA microbenchmark on
+ * the box"): runs a register-only kernel on the current device (8 CTAs of 256 threads per SM, 8 independent chains
+ * per thread, a few ms) and reports the best of four timed launches as thread-level instructions per second.
+ *   mode 0: FFMA only (three register operands);  mode 1: FFMA and LOP3 alternating (FMA pipe + ALU pipe: the issue
+ *   rate an instruction mix like the blend's can reach);  mode 2: packed FFMA2 (fma.rn.f32x2; one instruction = two FMAs,
+ *   counted once). sm_count (may be NULL) receives cudaDevAttrMultiProcessorCount. Synchronises `cuda_stream`. */
+int pvg_calibrate_fp32(int mode, void *cuda_stream, double *thread_instr_per_s, int *sm_count);
+
 /* Debug helper so that bindings need no CUDA runtime of their own: synchronous copy of `bytes`
  * from a device pointer (e.g. a pvg_debug view) into host memory. */
 int pvg_memcpy_d2h(void *host_dst, const void *device_src, size_t bytes);

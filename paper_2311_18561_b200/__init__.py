@@ -30,7 +30,7 @@ NUM_STAGES = len(STAGES)
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
            "pvg_render_host_async", "pvg_wait_host", "pvg_render_state", "pvg_set_sky",
            "pvg_destroy", "pvg_fork_scene", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms", "pvg_kernel_timeline_ms",
-           "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
+           "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_calibrate_fp32", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
 
 class PvgError(RuntimeError):
@@ -107,6 +107,7 @@ def load_library(path: Optional[str] = None):
     L.pvg_blend_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
     L.pvg_memcpy_d2h.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
     L.pvg_set_allocator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.pvg_calibrate_fp32.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     if path is None:
         _lib = L
     return L
@@ -414,3 +415,13 @@ def sort_pairs(keys, vals, begin_bit: int = 0, end_bit: int = 64):
     _check(L.pvg_sort_pairs(n, keys.data_ptr(), vals.data_ptr(), ko.data_ptr(), vo.data_ptr(), int(begin_bit),
                             int(end_bit), torch.cuda.current_stream().cuda_stream))
     return ko, vo
+
+
+def calibrate_fp32(mode: int = 1):
+    """(thread-level instructions per second, SM count) of the current CUDA device, measured by the library's
+    register-only microbenchmark (include/pvg.h pvg_calibrate_fp32): mode 0 FFMA, 1 FFMA + LOP3, 2 packed FFMA2."""
+    import torch
+    L = load_library()
+    rate, sms = C.c_double(0.0), C.c_int(0)
+    _check(L.pvg_calibrate_fp32(int(mode), torch.cuda.current_stream().cuda_stream, C.byref(rate), C.byref(sms)))
+    return float(rate.value), int(sms.value)

@@ -147,7 +147,6 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
     const float u11 = (t10 * R01 + t11 * R11 + t12 * R21) * a3.y;
     const float u12 = (t10 * R02 + t11 * R12 + t12 * R22) * a3.z;
     const float sxx = u00 * u00 + u01 * u01 + u02 * u02;
-    const float sxy = u00 * u10 + u01 * u11 + u02 * u12;
     const float syy = u10 * u10 + u11 * u11 + u12 * u12;
     const float c0 = u01 * u12 - u02 * u11, c1 = u02 * u10 - u00 * u12, c2 = u00 * u11 - u01 * u10;
     const float det0 = c0 * c0 + c1 * c1 + c2 * c2;

@@ -12,6 +12,7 @@
 #include "../../include/pvg.h"
 #include "blend.cuh"
 #include "blockbin.cuh"
+#include "calib.cuh"
 #include "common.cuh"
 #include "expand.cuh"
 #include "onesweep.cuh"
@@ -1487,6 +1488,41 @@ int pvg_blend_counters(pvg_scene* s, uint64_t out[2]) {
   CU(cudaStreamSynchronize(s->stream));
   CU(cudaMemcpy(out, s->small.as<unsigned char>() + 64, 16, cudaMemcpyDeviceToHost));
   return PVG_OK;
+}
+
+int pvg_calibrate_fp32(int mode, void* cuda_stream, double* thread_instr_per_s, int* sm_count) {
+  if (!thread_instr_per_s) return PVG_ERR_NULL;
+  if (mode < 0 || mode > 2) return PVG_ERR_BAD_OPTION;
+  Dev dv;
+  TRY(dv.query());
+  if (sm_count) *sm_count = dv.sms;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const unsigned grid = (unsigned)dv.sms * 8u;   // 8 CTAs of 256 threads per SM: 16 warps per scheduler
+  const int trips = 4096;
+  float* sink = nullptr;
+  CU(cudaMalloc(&sink, (size_t)grid * CALIB_THREADS * sizeof(float)));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  int rc = PVG_OK;
+  float best = 0.f;
+  do {
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { rc = PVG_ERR_CUDA; break; }
+    for (int rep = 0; rep < 6 && rc == PVG_OK; ++rep) {   // first launches warm up; the best of the rest counts
+      cudaEventRecord(e0, st);
+      if (mode == 0) calib_kernel<0><<<grid, CALIB_THREADS, 0, st>>>(sink, trips, 0.999f, 1e-3f, 0x5bd1e995u, 0x1b873593u);
+      else if (mode == 1) calib_kernel<1><<<grid, CALIB_THREADS, 0, st>>>(sink, trips, 0.999f, 1e-3f, 0x5bd1e995u, 0x1b873593u);
+      else calib_kernel<2><<<grid, CALIB_THREADS, 0, st>>>(sink, trips, 0.999f, 1e-3f, 0x5bd1e995u, 0x1b873593u);
+      cudaEventRecord(e1, st);
+      float ms = 0.f;
+      if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) { rc = PVG_ERR_CUDA; break; }
+      if (rep >= 2 && ms > 0.f && (best == 0.f || ms < best)) best = ms;
+    }
+  } while (false);
+  if (rc != PVG_OK) snprintf(g_cuda_err, sizeof(g_cuda_err), "calibrate: %s", cudaGetErrorString(cudaGetLastError()));
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (rc == PVG_OK) *thread_instr_per_s = best > 0.f ? calib_instructions(mode, grid, trips) / ((double)best * 1e-3) : 0.0;
+  return rc;
 }
 
 int pvg_memcpy_d2h(void* host_dst, const void* device_src, size_t bytes) {

@@ -116,3 +116,35 @@ def test_gather_bands_world2_ragged_last_row():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert res == [(0, True), (1, True)]
+
+
+def test_bench_gpus_n_starts_its_own_ranks():
+    """`python bench.py --gpus 2` outside torchrun must start two ranks itself (torch.distributed.run, 127.0.0.1) and
+    print ONE line from rank 0 with n_gpus = 2. --selftest-spawn runs the rendezvous, barrier and max-over-ranks over
+    gloo without any CUDA work, so the launch path is covered on a CPU box."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-spawn", "--steps", "9"],
+                       capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["frames_total"] == 18 and abs(d["elapsed_max_s"] - 2e-3) < 1e-12
+
+
+def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
+    """--impl reference under a 2-rank launch: rank 0 alone runs the oracle (whole frames) and prints the line, the
+    other rank exits 0 without work."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "0",
+                        "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
+    assert "no extrapolation" in d["cpu_baseline"]["sample"] and d["cpu_baseline"]["cores"] >= 1
