@@ -85,29 +85,54 @@ __device__ __forceinline__ bool blend_reaches_tile(float mx, float my, float a, 
   return !(bound < -7.994353436858858f);   // log2(1/255); NaN keeps
 }
 
-// Per-pixel compositing state and one front-to-back step. The cutoffs are predicates (selects),
-// not branches: alpha < 1/255 skips, T' = T - alpha T < 1e-4 stops the pixel WITHOUT compositing
-// the Gaussian that crosses the threshold (S10).
+// Per-pixel compositing state and one front-to-back step.
+//
+// What bounds this kernel (ncu, round 1: ALU pipe 57 % + FMA pipe 43 % = 100 %; the FFMA / FFMA+LOP3 / FFMA2 rates
+// of pvg_calibrate_fp32 say the same): of an SM sub-partition's two 16-lane fp32 datapaths one is shared with the
+// integer / compare / select unit. An FFMA, FMUL or FADD takes both for one cycle, an FMNMX, FSETP, PLOP3 or SEL
+// the shared one for two -- and a packed FFMA2 both for two, so packing buys issue slots, not datapath cycles.
+// The step is therefore written to minimise (FMA-pipe instructions + 2 x ALU-pipe instructions):
+//   * no `alive` predicate: a stopped pixel carries its final transmittance NEGATED (T < 0). Then T' = T (1 - alpha)
+//     < 0 fails `T' >= 1e-4` by itself, nothing is ever composited again, and the stop is idempotent: two FSETP
+//     (listed, composite) instead of two FSETP + PLOP3 + predicated FSETP;
+//   * the contribution and the T update are predicated FFMAs (FMA pipe), not selects;
+//   * the two clamps -- w <= log2 o~ (S16': the exact quadratic form is <= 0) and alpha <= 0.99 -- are applied only to
+//     entries that can need them (o~ > 0.98, or a conic that is not safely positive definite in fp32: the staging
+//     code decides per entry, below); for every other entry w <= log2 o~ + rounding < log2 0.99 holds by itself.
+// 11 FMA-pipe + 2 ALU-pipe + 1 MUFU instructions per (pixel, entry) evaluation = 15 cycles of the shared datapath,
+// against 9 + 7 (23 cycles) before.
 struct BlendPixel {
-  float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;
-  bool alive = false;
-  // w: log2 of o~ G(x); L = log2 o~ (exact quadratic form <= 0, so w <= L: the S16' guard)
-  __device__ __forceinline__ bool step(float w, float L, float r, float g, float b, float z) {
-    w = fminf(w, L);
-    const float alpha = fminf(PVG_ALPHA_MAX, ex2_approx(w));
-    const bool acc = alive && alpha >= PVG_ALPHA_MIN;
+  float T = -1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;   // T > 0: live; T < 0: stopped, |T| final (outside the image: -1)
+  __device__ __forceinline__ bool alive() const { return T > 0.f; }
+  // alpha: opacity of this entry at this pixel, clamps already applied.
+  // T' = T - alpha T as ONE fma (tested and, if it passes, stored: the same expression twice, so the same bits).
+  // The T logic stays on the FMA pipe: "@listed T = -|T|" (as |T| * -2 + |T|, exact), then "@composite T = T'"
+  // rebuilt from the negated value (alpha * (-T) + T) -- ptxas turns a predicated MOV into an FSEL (ALU pipe, two
+  // cycles) but leaves a predicated FFMA alone.
+  template <bool WANT_FLAG>
+  __device__ __forceinline__ uint32_t step(float alpha, float r, float g, float b, float z) {
     const float wgt = alpha * T;
-    const float Tn = T - wgt;                      // T (1 - alpha)
-    const bool use = acc && Tn >= PVG_T_STOP;
-    alive = alive && (use || !acc);
-    if (use) {
-      Cr = fmaf(r, wgt, Cr);
-      Cg = fmaf(g, wgt, Cg);
-      Cb = fmaf(b, wgt, Cb);
-      D = fmaf(z, wgt, D);
-      T = Tn;
-    }
-    return use;
+    uint32_t used = 0;
+    asm("{\n\t"
+        ".reg .pred pa, pu;\n\t"
+        ".reg .f32 ta, nt, tn;\n\t"
+        "abs.f32 ta, %4;\n\t"
+        "neg.f32 nt, %4;\n\t"
+        "fma.rn.f32 tn, %6, nt, %4;\n\t"                  // T' = T (1 - alpha)
+        "setp.ge.f32 pa, %6, 0f3B808081;\n\t"             // listed: alpha >= 1/255 (false for NaN)
+        "setp.ge.and.f32 pu, tn, 0f38D1B717, pa;\n\t"     // composite: T' >= 1e-4; listed and not composite = stop (S10)
+        "@pu fma.rn.f32 %0, %7, %11, %0;\n\t"
+        "@pu fma.rn.f32 %1, %8, %11, %1;\n\t"
+        "@pu fma.rn.f32 %2, %9, %11, %2;\n\t"
+        "@pu fma.rn.f32 %3, %10, %11, %3;\n\t"
+        "@pa fma.rn.f32 %4, ta, 0fC0000000, ta;\n\t"      // T = -|T| (a stopped pixel keeps its value)
+        "neg.f32 nt, %4;\n\t"
+        "@pu fma.rn.f32 %4, %6, %4, nt;\n\t"              // T = alpha (-T0) + T0 = T'
+        "selp.u32 %5, 1, 0, pu;\n\t"
+        "}"
+        : "+f"(Cr), "+f"(Cg), "+f"(Cb), "+f"(D), "+f"(T), "=r"(used)
+        : "f"(alpha), "f"(r), "f"(g), "f"(b), "f"(z), "f"(wgt));
+    return WANT_FLAG ? used : 0u;
   }
 };
 
@@ -151,6 +176,7 @@ struct BlendLazy {
 };
 
 // Parks a tile (first blend phase of the lazy lists): out of line, so that the rare path costs the common one nothing.
+// st[k] = (T signed: negative = stopped, Cr, Cg, Cb, D).
 __device__ __noinline__ void blend_park(const BlendLazy& Z, uint32_t tile, uint32_t bin, uint32_t ltile, size_t HW, size_t pi,
                                         uint32_t inmask, const float (&st)[BLEND_NPX][5]) {
 #pragma unroll
@@ -165,6 +191,10 @@ __device__ __noinline__ void blend_park(const BlendLazy& Z, uint32_t tile, uint3
   }
 }
 
+// log2(0.98): entries with o~ above it take the clamped evaluation (the 0.99 clamp can bind only above log2 0.99;
+// the margin covers the rounding of w)
+#define PVG_L_CLAMPED -0.029146346f
+
 template <bool COUNT, int MODE, int PHASE>
 __device__ __forceinline__ void
 blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ ranges,
@@ -173,8 +203,9 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
            unsigned long long* __restrict__ counters, const float* __restrict__ featw, const BlendLazy& Z) {
   __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
   __shared__ float4 s_col[BLEND_BATCH];   // c', log2 o~, r, g
-  __shared__ float2 s_bz[BLEND_BATCH];    // b, z
+  __shared__ float4 s_bz[BLEND_BATCH];    // b, z, upper clamp of w (+inf: none), upper clamp of alpha (+inf: none)
   __shared__ uint32_t s_kept[BLEND_THREADS / 32];
+  __shared__ uint32_t s_plain[BLEND_BATCH / BLEND_UNROLL];   // per group of BLEND_UNROLL staged entries: none of them is clamped
 
   const uint32_t tid = threadIdx.x;
   const uint32_t tx = tile % P.tiles_x, ty = tile / P.tiles_x;
@@ -191,29 +222,27 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   }
 
   BlendPixel X[BLEND_NPX];
-  bool in[BLEND_NPX];
 #pragma unroll
-  for (int k = 0; k < BLEND_NPX; ++k) X[k].alive = in[k] = px + k < (uint32_t)P.width && py < (uint32_t)P.height;
+  for (int k = 0; k < BLEND_NPX; ++k) X[k].T = (px + k < (uint32_t)P.width && py < (uint32_t)P.height) ? 1.f : -1.f;
   if (PHASE == 2) {
     const size_t HW = (size_t)P.width * P.height;
     const size_t pi = (size_t)py * P.width + px;
 #pragma unroll
     for (int k = 0; k < BLEND_NPX; ++k) {
-      if (!in[k]) continue;
-      const float t = Z.state[pi + k];
-      X[k].alive = !signbit(t);
-      X[k].T = fabsf(t);
+      if (!(px + k < (uint32_t)P.width && py < (uint32_t)P.height)) continue;
+      X[k].T = Z.state[pi + k];
       X[k].Cr = Z.state[HW + pi + k];
       X[k].Cg = Z.state[2 * HW + pi + k];
       X[k].Cb = Z.state[3 * HW + pi + k];
       X[k].D = Z.state[4 * HW + pi + k];
     }
   }
+  // a pixel is live while its T is positive: some pixel of the thread is live iff the AND of the sign bits is clear
   auto any_alive = [&]() {
-    bool a = false;
+    uint32_t m = __float_as_uint(X[0].T);
 #pragma unroll
-    for (int k = 0; k < BLEND_NPX; ++k) a = a || X[k].alive;
-    return a;
+    for (int k = 1; k < BLEND_NPX; ++k) m &= __float_as_uint(X[k].T);
+    return (int)m >= 0;
   };
   uint32_t n_eval = 0, n_contrib = 0;
 
@@ -222,6 +251,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   const float by0 = (float)(ty * PVG_TILE) + 0.5f, by1 = by0 + (float)(PVG_TILE - 1);
   const uint32_t lane = tid & 31u, wid = tid >> 5;
   constexpr uint32_t WARPS = BLEND_THREADS / 32;
+  const float kInf = __int_as_float(0x7f800000);
 
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
   // saturates, so a fixed 256-entry first batch gathers mostly records that are never used
@@ -240,8 +270,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     for (uint32_t r = 0; r < seg; r += 32) {
       const uint32_t idx = base + seg0 + r + lane;
       bool keep = false;
-      float4 ge, co;
-      float2 bz;
+      float4 ge, co, bz;
       if (idx < range.y) {
         const uint32_t g = __ldg(vals + idx);
         const float4 r0 = __ldg(record + 3 * (size_t)g);
@@ -250,7 +279,13 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
         const float kh = -0.72134752044448170f;  // -log2(e)/2
         ge = make_float4(r0.x, r0.y, kh * r1.x, 2.0f * kh * r1.y);
         co = make_float4(kh * r1.z, __log2f(r0.w), r2.x, r2.y);
-        bz = make_float2(r2.z, MODE == BLEND_FEATURE ? __ldg(featw + g) : r0.z);
+        // Which entries need the clamps evaluated (a property of the entry alone, so that a (pixel, entry) evaluation
+        // does not depend on how the list was cut into batches): alpha <= 0.99 can only bind when o~ is near 1, and
+        // w <= log2 o~ holds up to rounding whenever the conic is positive definite with a margin in fp32
+        // (4 a' c' - b'^2 = 4 kh^2 (a c - b^2)); everything else -- needles whose rounded conic is indefinite, NaN --
+        // takes the clamped path.
+        const bool safe = co.y <= PVG_L_CLAMPED && 4.0f * ge.z * co.x > 1.00001f * ge.w * ge.w;
+        bz = make_float4(r2.z, MODE == BLEND_FEATURE ? __ldg(featw + g) : r0.z, safe ? kInf : co.y, safe ? kInf : PVG_ALPHA_MAX);
         keep = !P.cull || blend_reaches_tile(ge.x, ge.y, ge.z, ge.w, co.x, co.y, bx0, bx1, by0, by1);
       }
       const uint32_t m = __ballot_sync(0xffffffffu, keep);
@@ -266,31 +301,64 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     if (lane < ((0u - kept) & (BLEND_UNROLL - 1u))) {
       s_geo[seg0 + kept + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
       s_col[seg0 + kept + lane] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
-      s_bz[seg0 + kept + lane] = make_float2(0.f, 0.f);
+      s_bz[seg0 + kept + lane] = make_float4(0.f, 0.f, kInf, kInf);
     }
     if (lane == 0) s_kept[wid] = kept;
+    __syncwarp();
+    // group flags of this warp's segment (a group is what one trip of the unrolled loop below consumes)
+    for (uint32_t gq = lane; BLEND_UNROLL * gq < kept; gq += 32) {
+      uint32_t m = 0x7f800000u;
+#pragma unroll
+      for (int u = 0; u < BLEND_UNROLL; ++u) m &= __float_as_uint(s_bz[seg0 + BLEND_UNROLL * gq + u].z);
+      s_plain[seg0 / BLEND_UNROLL + gq] = m == 0x7f800000u ? 1u : 0u;   // +inf's bit pattern survives the AND iff all four are +inf
+    }
     __syncthreads();
     if (__any_sync(0xffffffffu, any_alive())) {
       for (uint32_t sg = 0; sg < WARPS; ++sg) {
         const uint32_t nb = s_kept[sg], j00 = sg * seg;
         bool stop = false;
         for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
+          // warp-uniform (every lane looks at the same entries): the clamped evaluation is the plain one plus two
+          // FMNMX per (pixel, entry), and a no-op on the group's unclamped entries (their clamps are +inf)
+          if (s_plain[(j00 + j0) / BLEND_UNROLL]) {
 #pragma unroll
-          for (int u = 0; u < BLEND_UNROLL; ++u) {
-            const uint32_t j = j00 + j0 + u;
-            const float4 ge = s_geo[j];
-            const float4 co = s_col[j];
-            const float2 bz = s_bz[j];
-            // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
-            const float dy = ge.y - pyf;
-            const float q = ge.w * dy;
-            const float rr = fmaf(co.x * dy, dy, co.y);
+            for (int u = 0; u < BLEND_UNROLL; ++u) {
+              const uint32_t j = j00 + j0 + u;
+              const float4 ge = s_geo[j];
+              const float4 co = s_col[j];
+              const float2 bz = *reinterpret_cast<const float2*>(&s_bz[j]);
+              // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
+              const float dy = ge.y - pyf;
+              const float q = ge.w * dy;
+              const float rr = fmaf(co.x * dy, dy, co.y);
 #pragma unroll
-            for (int k = 0; k < BLEND_NPX; ++k) {
-              if (COUNT) n_eval += (j0 + u < nb && X[k].alive) ? 1u : 0u;
-              const float dx = ge.x - (pxf + (float)k);
-              const bool used = X[k].step(fmaf(fmaf(ge.z, dx, q), dx, rr), co.y, co.z, co.w, bz.x, bz.y);
-              if (COUNT) n_contrib += used ? 1u : 0u;
+              for (int k = 0; k < BLEND_NPX; ++k) {
+                if (COUNT) n_eval += (j0 + u < nb && X[k].alive()) ? 1u : 0u;
+                const float dx = ge.x - (pxf + (float)k);
+                const float alpha = ex2_approx(fmaf(fmaf(ge.z, dx, q), dx, rr));
+                const uint32_t used = X[k].template step<COUNT>(alpha, co.z, co.w, bz.x, bz.y);
+                if (COUNT) n_contrib += used;
+              }
+            }
+          } else {
+#pragma unroll
+            for (int u = 0; u < BLEND_UNROLL; ++u) {
+              const uint32_t j = j00 + j0 + u;
+              const float4 ge = s_geo[j];
+              const float4 co = s_col[j];
+              const float4 bz = s_bz[j];
+              const float dy = ge.y - pyf;
+              const float q = ge.w * dy;
+              const float rr = fmaf(co.x * dy, dy, co.y);
+#pragma unroll
+              for (int k = 0; k < BLEND_NPX; ++k) {
+                if (COUNT) n_eval += (j0 + u < nb && X[k].alive()) ? 1u : 0u;
+                const float dx = ge.x - (pxf + (float)k);
+                const float w = fminf(fmaf(fmaf(ge.z, dx, q), dx, rr), bz.z);   // S16'
+                const float alpha = fminf(ex2_approx(w), bz.w);                 // S9
+                const uint32_t used = X[k].template step<COUNT>(alpha, co.z, co.w, bz.x, bz.y);
+                if (COUNT) n_contrib += used;
+              }
             }
           }
           if (!__any_sync(0xffffffffu, any_alive())) { stop = true; break; }
@@ -313,7 +381,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
       float st[BLEND_NPX][5];
 #pragma unroll
       for (int k = 0; k < BLEND_NPX; ++k) {
-        st[k][0] = X[k].alive ? X[k].T : -X[k].T;
+        st[k][0] = X[k].T;
         st[k][1] = X[k].Cr; st[k][2] = X[k].Cg; st[k][3] = X[k].Cb; st[k][4] = X[k].D;
       }
       uint32_t inmask = 0;
@@ -326,7 +394,8 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
 #pragma unroll
   for (int k = 0; k < BLEND_NPX; ++k) {
     if (!(px + k < (uint32_t)P.width && py < (uint32_t)P.height)) continue;   // recomputed: not kept live through the loop
-    const float Al = 1.0f - X[k].T;
+    const float Tk = fabsf(X[k].T);
+    const float Al = 1.0f - Tk;
     if (out_rgb) {
       float bg[3] = {P.bg[0], P.bg[1], P.bg[2]};
       if (MODE == BLEND_FEATURE) bg[0] = bg[1] = bg[2] = 0.f;
@@ -336,9 +405,9 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
         sky_sample(P.sky, P.sky_res, fmaf(P.R[0], cxr, fmaf(P.R[3], cyr, P.R[6])),
                    fmaf(P.R[1], cxr, fmaf(P.R[4], cyr, P.R[7])), fmaf(P.R[2], cxr, fmaf(P.R[5], cyr, P.R[8])), bg);
       }
-      out_rgb[pi + k] = fmaf(X[k].T, bg[0], X[k].Cr);
-      out_rgb[HW + pi + k] = fmaf(X[k].T, bg[1], X[k].Cg);
-      out_rgb[2 * HW + pi + k] = fmaf(X[k].T, bg[2], X[k].Cb);
+      out_rgb[pi + k] = fmaf(Tk, bg[0], X[k].Cr);
+      out_rgb[HW + pi + k] = fmaf(Tk, bg[1], X[k].Cg);
+      out_rgb[2 * HW + pi + k] = fmaf(Tk, bg[2], X[k].Cb);
     }
     if (out_depth) out_depth[pi + k] = MODE == BLEND_FEATURE ? X[k].D : (Al > 0.f ? X[k].D / Al : 0.f);
     if (out_alpha) out_alpha[pi + k] = Al;
