@@ -15,12 +15,21 @@ namespace pvg {
 #endif
 constexpr int BLEND_NPX = PVG_BLEND_NPX;                   // horizontally adjacent pixels per thread (2 or 4)
 constexpr int BLEND_THREADS = PVG_TILE_PIXELS / BLEND_NPX;
-constexpr int BLEND_BATCH = 256;
+#ifndef PVG_BLEND_BATCH
+#define PVG_BLEND_BATCH 128
+#endif
+constexpr int BLEND_BATCH = PVG_BLEND_BATCH;   // 88 B of (duplicated) shared memory per staged entry
 #ifndef PVG_BLEND_FIRST
-#define PVG_BLEND_FIRST 64
+#define PVG_BLEND_FIRST 128
 #endif
 constexpr int BLEND_BATCH_FIRST = PVG_BLEND_FIRST;
-constexpr int BLEND_UNROLL = 4;   // divides BLEND_BATCH_FIRST / (BLEND_THREADS / 32)
+#ifndef PVG_BLEND_UNROLL
+#define PVG_BLEND_UNROLL 4
+#endif
+constexpr int BLEND_UNROLL = PVG_BLEND_UNROLL;   // divides BLEND_BATCH_FIRST / (BLEND_THREADS / 32)
+#ifndef PVG_BLEND_MINB
+#define PVG_BLEND_MINB 12   // resident CTAs per SM the register allocation must allow
+#endif
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -85,54 +94,68 @@ __device__ __forceinline__ bool blend_reaches_tile(float mx, float my, float a, 
   return !(bound < -7.994353436858858f);   // log2(1/255); NaN keeps
 }
 
-// Per-pixel compositing state and one front-to-back step.
-//
-// What bounds this kernel (ncu, round 1: ALU pipe 57 % + FMA pipe 43 % = 100 %; the FFMA / FFMA+LOP3 / FFMA2 rates
-// of pvg_calibrate_fp32 say the same): of an SM sub-partition's two 16-lane fp32 datapaths one is shared with the
-// integer / compare / select unit. An FFMA, FMUL or FADD takes both for one cycle, an FMNMX, FSETP, PLOP3 or SEL
-// the shared one for two -- and a packed FFMA2 both for two, so packing buys issue slots, not datapath cycles.
-// The step is therefore written to minimise (FMA-pipe instructions + 2 x ALU-pipe instructions):
-//   * no `alive` predicate: a stopped pixel carries its final transmittance NEGATED (T < 0). Then T' = T (1 - alpha)
-//     < 0 fails `T' >= 1e-4` by itself, nothing is ever composited again, and the stop is idempotent: two FSETP
-//     (listed, composite) instead of two FSETP + PLOP3 + predicated FSETP;
-//   * the contribution and the T update are predicated FFMAs (FMA pipe), not selects;
+// ---- packed fp32 (sm_100: add / sub / mul / fma .f32x2 on 64-bit register pairs) -------------------------------
+// The kernel is ISSUE-bound (ncu, round 1: issue-active 84 %, 18 instructions per (pixel, entry) evaluation; round 2
+// confirmed it: trading ALU-pipe instructions for FMA-pipe ones one for one left the time unchanged). A packed
+// instruction performs the fp32 operation on both halves of a register pair -- the SAME IEEE operation per half,
+// so results are bit-identical to the scalar form -- for ONE issue slot. pvg_calibrate_fp32 measures what it buys:
+// FFMA2 issues at half the FFMA rate, i.e. the same FMAs per second, but leaves every other slot to the compares,
+// selects, MUFU and shared-memory loads that make up the rest of this loop. A thread's four pixels form two pairs.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+  f32x2 v;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi));
+  return v;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+
+// Compositing state of a PAIR of horizontally adjacent pixels and one front-to-back step.
+//   * no `alive` predicate: a stopped pixel carries its final transmittance NEGATED (T < 0). Then T' = T - alpha T
+//     < 0 fails `T' >= 1e-4` by itself, nothing is ever composited again, and the stop is idempotent;
+//   * the contribution is added unconditionally with a weight that is 0 unless the entry is composited
+//     (fma(c, 0, C) = C exactly: colours and depths are finite), so that the five accumulations are packed;
 //   * the two clamps -- w <= log2 o~ (S16': the exact quadratic form is <= 0) and alpha <= 0.99 -- are applied only to
-//     entries that can need them (o~ > 0.98, or a conic that is not safely positive definite in fp32: the staging
-//     code decides per entry, below); for every other entry w <= log2 o~ + rounding < log2 0.99 holds by itself.
-// 11 FMA-pipe + 2 ALU-pipe + 1 MUFU instructions per (pixel, entry) evaluation = 15 cycles of the shared datapath,
-// against 9 + 7 (23 cycles) before.
-struct BlendPixel {
-  float T = -1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f, D = 0.f;   // T > 0: live; T < 0: stopped, |T| final (outside the image: -1)
-  __device__ __forceinline__ bool alive() const { return T > 0.f; }
-  // alpha: opacity of this entry at this pixel, clamps already applied.
-  // T' = T - alpha T as ONE fma (tested and, if it passes, stored: the same expression twice, so the same bits).
-  // The T logic stays on the FMA pipe: "@listed T = -|T|" (as |T| * -2 + |T|, exact), then "@composite T = T'"
-  // rebuilt from the negated value (alpha * (-T) + T) -- ptxas turns a predicated MOV into an FSEL (ALU pipe, two
-  // cycles) but leaves a predicated FFMA alone.
+//     entries that can need them (decided per entry by the staging code, below).
+struct BlendPair {
+  f32x2 T, Cr, Cg, Cb, D;   // T > 0: live; T < 0: stopped, |T| final (outside the image: -1)
+  // alpha of the entry at the two pixels (clamps applied); r2 .. z2: the entry's colour and depth, each duplicated
   template <bool WANT_FLAG>
-  __device__ __forceinline__ uint32_t step(float alpha, float r, float g, float b, float z) {
-    const float wgt = alpha * T;
-    uint32_t used = 0;
-    asm("{\n\t"
-        ".reg .pred pa, pu;\n\t"
-        ".reg .f32 ta, nt, tn;\n\t"
-        "abs.f32 ta, %4;\n\t"
-        "neg.f32 nt, %4;\n\t"
-        "fma.rn.f32 tn, %6, nt, %4;\n\t"                  // T' = T (1 - alpha)
-        "setp.ge.f32 pa, %6, 0f3B808081;\n\t"             // listed: alpha >= 1/255 (false for NaN)
-        "setp.ge.and.f32 pu, tn, 0f38D1B717, pa;\n\t"     // composite: T' >= 1e-4; listed and not composite = stop (S10)
-        "@pu fma.rn.f32 %0, %7, %11, %0;\n\t"
-        "@pu fma.rn.f32 %1, %8, %11, %1;\n\t"
-        "@pu fma.rn.f32 %2, %9, %11, %2;\n\t"
-        "@pu fma.rn.f32 %3, %10, %11, %3;\n\t"
-        "@pa fma.rn.f32 %4, ta, 0fC0000000, ta;\n\t"      // T = -|T| (a stopped pixel keeps its value)
-        "neg.f32 nt, %4;\n\t"
-        "@pu fma.rn.f32 %4, %6, %4, nt;\n\t"              // T = alpha (-T0) + T0 = T'
-        "selp.u32 %5, 1, 0, pu;\n\t"
-        "}"
-        : "+f"(Cr), "+f"(Cg), "+f"(Cb), "+f"(D), "+f"(T), "=r"(used)
-        : "f"(alpha), "f"(r), "f"(g), "f"(b), "f"(z), "f"(wgt));
-    return WANT_FLAG ? used : 0u;
+  __device__ __forceinline__ uint32_t step(float a0, float a1, f32x2 r2, f32x2 g2, f32x2 b2, f32x2 z2) {
+    // T' = T (1 - alpha) with 1 - alpha formed off the T -> T' recurrence: the loop-carried chain of a pixel is
+    // FMUL2 -> FSETP -> FSEL (the profile of the T - alpha T form showed its FMUL2 -> FADD2 pair as the top stall)
+    const f32x2 al = pack2(a0, a1);
+    const f32x2 wg = mul2(al, T);                                     // alpha T: the weight of the contribution
+    const f32x2 tn = mul2(T, sub2(0x3f8000003f800000ull, al));        // (1.0f, 1.0f) - alpha
+    float t0, t1, g0, g1, n0, n1;
+    unpack2(T, t0, t1);
+    unpack2(wg, g0, g1);
+    unpack2(tn, n0, n1);
+    const bool pa0 = a0 >= PVG_ALPHA_MIN, pa1 = a1 >= PVG_ALPHA_MIN;      // listed (false for NaN)
+    const bool pu0 = pa0 && n0 >= PVG_T_STOP, pu1 = pa1 && n1 >= PVG_T_STOP;   // composited; listed and not composited: stop (S10)
+    const f32x2 we = pack2(pu0 ? g0 : 0.f, pu1 ? g1 : 0.f);
+    Cr = fma2(r2, we, Cr);
+    Cg = fma2(g2, we, Cg);
+    Cb = fma2(b2, we, Cb);
+    D = fma2(z2, we, D);
+    T = pack2(pa0 ? (pu0 ? n0 : -fabsf(t0)) : t0, pa1 ? (pu1 ? n1 : -fabsf(t1)) : t1);
+    return WANT_FLAG ? (pu0 ? 1u : 0u) + (pu1 ? 1u : 0u) : 0u;
   }
 };
 
@@ -201,9 +224,14 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
            const uint32_t* __restrict__ vals, const float4* __restrict__ record,
            float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
            unsigned long long* __restrict__ counters, const float* __restrict__ featw, const BlendLazy& Z) {
-  __shared__ float4 s_geo[BLEND_BATCH];   // mx, my, a', b'
-  __shared__ float4 s_col[BLEND_BATCH];   // c', log2 o~, r, g
-  __shared__ float4 s_bz[BLEND_BATCH];    // b, z, upper clamp of w (+inf: none), upper clamp of alpha (+inf: none)
+  // every per-entry operand of a packed instruction is stored DUPLICATED, so that one 128-bit shared-memory load
+  // fills two register pairs and no instruction is spent on broadcasting
+  __shared__ float4 s_xa[BLEND_BATCH];    // mx, mx, a', a'
+  __shared__ float4 s_yb[BLEND_BATCH];    // my, my, b', b'
+  __shared__ float4 s_cl[BLEND_BATCH];    // c', c', log2 o~, log2 o~
+  __shared__ float4 s_rg[BLEND_BATCH];    // r, r, g, g
+  __shared__ float4 s_bz[BLEND_BATCH];    // b, b, z, z
+  __shared__ float2 s_clamp[BLEND_BATCH]; // upper clamp of w (+inf: none), upper clamp of alpha (+inf: none)
   __shared__ uint32_t s_kept[BLEND_THREADS / 32];
   __shared__ uint32_t s_plain[BLEND_BATCH / BLEND_UNROLL];   // per group of BLEND_UNROLL staged entries: none of them is clamped
 
@@ -221,29 +249,40 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     if (PHASE == 1) range.y = lim; else range.x = lim;
   }
 
-  BlendPixel X[BLEND_NPX];
-#pragma unroll
-  for (int k = 0; k < BLEND_NPX; ++k) X[k].T = (px + k < (uint32_t)P.width && py < (uint32_t)P.height) ? 1.f : -1.f;
-  if (PHASE == 2) {
-    const size_t HW = (size_t)P.width * P.height;
-    const size_t pi = (size_t)py * P.width + px;
+  static_assert(BLEND_NPX == 4, "two pixel pairs per thread");
+  constexpr int NPAIR = BLEND_NPX / 2;
+  BlendPair X[NPAIR];
+  {
+    float st[BLEND_NPX][5];
 #pragma unroll
     for (int k = 0; k < BLEND_NPX; ++k) {
-      if (!(px + k < (uint32_t)P.width && py < (uint32_t)P.height)) continue;
-      X[k].T = Z.state[pi + k];
-      X[k].Cr = Z.state[HW + pi + k];
-      X[k].Cg = Z.state[2 * HW + pi + k];
-      X[k].Cb = Z.state[3 * HW + pi + k];
-      X[k].D = Z.state[4 * HW + pi + k];
+      const bool in = px + k < (uint32_t)P.width && py < (uint32_t)P.height;
+      st[k][0] = in ? 1.f : -1.f;
+      st[k][1] = st[k][2] = st[k][3] = st[k][4] = 0.f;
+      if (PHASE == 2 && in) {
+        const size_t HW = (size_t)P.width * P.height;
+        const size_t pi = (size_t)py * P.width + px;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) st[k][c] = Z.state[c * HW + pi + k];
+      }
+    }
+#pragma unroll
+    for (int p = 0; p < NPAIR; ++p) {
+      X[p].T = pack2(st[2 * p][0], st[2 * p + 1][0]);
+      X[p].Cr = pack2(st[2 * p][1], st[2 * p + 1][1]);
+      X[p].Cg = pack2(st[2 * p][2], st[2 * p + 1][2]);
+      X[p].Cb = pack2(st[2 * p][3], st[2 * p + 1][3]);
+      X[p].D = pack2(st[2 * p][4], st[2 * p + 1][4]);
     }
   }
-  // a pixel is live while its T is positive: some pixel of the thread is live iff the AND of the sign bits is clear
+  // a pixel is live while its T is positive: some pixel of the thread is live iff the AND of the four sign bits is clear
   auto any_alive = [&]() {
-    uint32_t m = __float_as_uint(X[0].T);
-#pragma unroll
-    for (int k = 1; k < BLEND_NPX; ++k) m &= __float_as_uint(X[k].T);
-    return (int)m >= 0;
+    const f32x2 m = X[0].T & X[1].T;
+    return (m & 0x8000000080000000ull) != 0x8000000080000000ull;
   };
+  // the pixel centres of the two pairs, and the row, as packed operands
+  const f32x2 pxp[NPAIR] = {pack2(pxf, pxf + 1.0f), pack2(pxf + 2.0f, pxf + 3.0f)};
+  const f32x2 pyp = pack2(pyf, pyf);
   uint32_t n_eval = 0, n_contrib = 0;
 
   // The tile's box of pixel centres, for the staging-time test below.
@@ -252,6 +291,43 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   const uint32_t lane = tid & 31u, wid = tid >> 5;
   constexpr uint32_t WARPS = BLEND_THREADS / 32;
   const float kInf = __int_as_float(0x7f800000);
+
+  // One group of BLEND_UNROLL staged entries (slots j .. j + 3, of which the first `real` are list entries and the
+  // rest padding) against the thread's two pixel pairs. PLAIN: no entry of the group is clamped; otherwise the plain
+  // evaluation plus two FMNMX per pixel, which are no-ops on the group's unclamped entries (their clamps are +inf).
+  auto group = [&]<bool PLAIN>(uint32_t j, uint32_t real) {
+#pragma unroll
+    for (int u = 0; u < BLEND_UNROLL; ++u) {
+      const ulonglong2 xa = *reinterpret_cast<const ulonglong2*>(&s_xa[j + u]);
+      const ulonglong2 yb = *reinterpret_cast<const ulonglong2*>(&s_yb[j + u]);
+      const ulonglong2 cl = *reinterpret_cast<const ulonglong2*>(&s_cl[j + u]);
+      const ulonglong2 rg = *reinterpret_cast<const ulonglong2*>(&s_rg[j + u]);
+      const ulonglong2 bz = *reinterpret_cast<const ulonglong2*>(&s_bz[j + u]);
+      // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~); both halves
+      // of every row term hold the same value
+      const f32x2 dy = sub2(yb.x, pyp);
+      const f32x2 q = mul2(yb.y, dy);
+      const f32x2 rr = fma2(mul2(cl.x, dy), dy, cl.y);
+      float2 clamp = make_float2(0.f, 0.f);
+      if (!PLAIN) clamp = s_clamp[j + u];
+#pragma unroll
+      for (int p = 0; p < NPAIR; ++p) {
+        if (COUNT) {
+          float t0, t1;
+          unpack2(X[p].T, t0, t1);
+          n_eval += ((uint32_t)u < real ? 1u : 0u) * ((t0 > 0.f ? 1u : 0u) + (t1 > 0.f ? 1u : 0u));
+        }
+        const f32x2 dx = sub2(xa.x, pxp[p]);
+        float w0, w1;
+        unpack2(fma2(fma2(xa.y, dx, q), dx, rr), w0, w1);
+        if (!PLAIN) { w0 = fminf(w0, clamp.x); w1 = fminf(w1, clamp.x); }   // S16'
+        float a0 = ex2_approx(w0), a1 = ex2_approx(w1);
+        if (!PLAIN) { a0 = fminf(a0, clamp.y); a1 = fminf(a1, clamp.y); }   // S9
+        const uint32_t used = X[p].template step<COUNT>(a0, a1, rg.x, rg.y, bz.x, bz.y);
+        if (COUNT) n_contrib += used;
+      }
+    }
+  };
 
   // batches grow 64 -> 128 -> 256: at config 3 a tile consumes ~90 entries on average before it
   // saturates, so a fixed 256-entry first batch gathers mostly records that are never used
@@ -270,7 +346,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     for (uint32_t r = 0; r < seg; r += 32) {
       const uint32_t idx = base + seg0 + r + lane;
       bool keep = false;
-      float4 ge, co, bz;
+      float4 ge, co, bz;   // (mx, my, a', b'), (c', log2 o~, r, g), (b, z, clamp of w, clamp of alpha)
       if (idx < range.y) {
         const uint32_t g = __ldg(vals + idx);
         const float4 r0 = __ldg(record + 3 * (size_t)g);
@@ -291,17 +367,24 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
       const uint32_t m = __ballot_sync(0xffffffffu, keep);
       if (keep) {
         const uint32_t slot = seg0 + kept + __popc(m & ((1u << lane) - 1u));
-        s_geo[slot] = ge;
-        s_col[slot] = co;
-        s_bz[slot] = bz;
+        s_xa[slot] = make_float4(ge.x, ge.x, ge.z, ge.z);
+        s_yb[slot] = make_float4(ge.y, ge.y, ge.w, ge.w);
+        s_cl[slot] = make_float4(co.x, co.x, co.y, co.y);
+        s_rg[slot] = make_float4(co.z, co.z, co.w, co.w);
+        s_bz[slot] = make_float4(bz.x, bz.x, bz.y, bz.y);
+        s_clamp[slot] = make_float2(bz.z, bz.w);
       }
       kept += __popc(m);
     }
     // padding up to the unroll factor: log2 o~ = -inf gives alpha = 0 (kept < seg leaves room: seg % 4 == 0)
     if (lane < ((0u - kept) & (BLEND_UNROLL - 1u))) {
-      s_geo[seg0 + kept + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_col[seg0 + kept + lane] = make_float4(0.f, __int_as_float(0xff800000), 0.f, 0.f);
-      s_bz[seg0 + kept + lane] = make_float4(0.f, 0.f, kInf, kInf);
+      const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_xa[seg0 + kept + lane] = zero;
+      s_yb[seg0 + kept + lane] = zero;
+      s_cl[seg0 + kept + lane] = make_float4(0.f, 0.f, __int_as_float(0xff800000), __int_as_float(0xff800000));
+      s_rg[seg0 + kept + lane] = zero;
+      s_bz[seg0 + kept + lane] = zero;
+      s_clamp[seg0 + kept + lane] = make_float2(kInf, kInf);
     }
     if (lane == 0) s_kept[wid] = kept;
     __syncwarp();
@@ -309,7 +392,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     for (uint32_t gq = lane; BLEND_UNROLL * gq < kept; gq += 32) {
       uint32_t m = 0x7f800000u;
 #pragma unroll
-      for (int u = 0; u < BLEND_UNROLL; ++u) m &= __float_as_uint(s_bz[seg0 + BLEND_UNROLL * gq + u].z);
+      for (int u = 0; u < BLEND_UNROLL; ++u) m &= __float_as_uint(s_clamp[seg0 + BLEND_UNROLL * gq + u].x);
       s_plain[seg0 / BLEND_UNROLL + gq] = m == 0x7f800000u ? 1u : 0u;   // +inf's bit pattern survives the AND iff all four are +inf
     }
     __syncthreads();
@@ -320,47 +403,10 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
         for (uint32_t j0 = 0; j0 < nb; j0 += BLEND_UNROLL) {
           // warp-uniform (every lane looks at the same entries): the clamped evaluation is the plain one plus two
           // FMNMX per (pixel, entry), and a no-op on the group's unclamped entries (their clamps are +inf)
-          if (s_plain[(j00 + j0) / BLEND_UNROLL]) {
-#pragma unroll
-            for (int u = 0; u < BLEND_UNROLL; ++u) {
-              const uint32_t j = j00 + j0 + u;
-              const float4 ge = s_geo[j];
-              const float4 co = s_col[j];
-              const float2 bz = *reinterpret_cast<const float2*>(&s_bz[j]);
-              // log2 of o~ exp(-1/2 (a dx^2 + c dy^2) - b dx dy) = dx (a' dx + b' dy) + (c' dy^2 + log2 o~)
-              const float dy = ge.y - pyf;
-              const float q = ge.w * dy;
-              const float rr = fmaf(co.x * dy, dy, co.y);
-#pragma unroll
-              for (int k = 0; k < BLEND_NPX; ++k) {
-                if (COUNT) n_eval += (j0 + u < nb && X[k].alive()) ? 1u : 0u;
-                const float dx = ge.x - (pxf + (float)k);
-                const float alpha = ex2_approx(fmaf(fmaf(ge.z, dx, q), dx, rr));
-                const uint32_t used = X[k].template step<COUNT>(alpha, co.z, co.w, bz.x, bz.y);
-                if (COUNT) n_contrib += used;
-              }
-            }
-          } else {
-#pragma unroll
-            for (int u = 0; u < BLEND_UNROLL; ++u) {
-              const uint32_t j = j00 + j0 + u;
-              const float4 ge = s_geo[j];
-              const float4 co = s_col[j];
-              const float4 bz = s_bz[j];
-              const float dy = ge.y - pyf;
-              const float q = ge.w * dy;
-              const float rr = fmaf(co.x * dy, dy, co.y);
-#pragma unroll
-              for (int k = 0; k < BLEND_NPX; ++k) {
-                if (COUNT) n_eval += (j0 + u < nb && X[k].alive()) ? 1u : 0u;
-                const float dx = ge.x - (pxf + (float)k);
-                const float w = fminf(fmaf(fmaf(ge.z, dx, q), dx, rr), bz.z);   // S16'
-                const float alpha = fminf(ex2_approx(w), bz.w);                 // S9
-                const uint32_t used = X[k].template step<COUNT>(alpha, co.z, co.w, bz.x, bz.y);
-                if (COUNT) n_contrib += used;
-              }
-            }
-          }
+          // warp-uniform (every lane looks at the same entries): two copies of the group's code, so that the
+          // common one carries no clamp instructions at all
+          if (s_plain[(j00 + j0) / BLEND_UNROLL]) group.template operator()<true>(j00 + j0, nb - j0);
+          else group.template operator()<false>(j00 + j0, nb - j0);
           if (!__any_sync(0xffffffffu, any_alive())) { stop = true; break; }
         }
         if (stop) break;
@@ -380,9 +426,12 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     if (__syncthreads_or(any_alive())) {
       float st[BLEND_NPX][5];
 #pragma unroll
-      for (int k = 0; k < BLEND_NPX; ++k) {
-        st[k][0] = X[k].T;
-        st[k][1] = X[k].Cr; st[k][2] = X[k].Cg; st[k][3] = X[k].Cb; st[k][4] = X[k].D;
+      for (int p = 0; p < NPAIR; ++p) {
+        unpack2(X[p].T, st[2 * p][0], st[2 * p + 1][0]);
+        unpack2(X[p].Cr, st[2 * p][1], st[2 * p + 1][1]);
+        unpack2(X[p].Cg, st[2 * p][2], st[2 * p + 1][2]);
+        unpack2(X[p].Cb, st[2 * p][3], st[2 * p + 1][3]);
+        unpack2(X[p].D, st[2 * p][4], st[2 * p + 1][4]);
       }
       uint32_t inmask = 0;
 #pragma unroll
@@ -391,10 +440,19 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
       return;
     }
   }
+  float fin[BLEND_NPX][5];
+#pragma unroll
+  for (int p = 0; p < NPAIR; ++p) {
+    unpack2(X[p].T, fin[2 * p][0], fin[2 * p + 1][0]);
+    unpack2(X[p].Cr, fin[2 * p][1], fin[2 * p + 1][1]);
+    unpack2(X[p].Cg, fin[2 * p][2], fin[2 * p + 1][2]);
+    unpack2(X[p].Cb, fin[2 * p][3], fin[2 * p + 1][3]);
+    unpack2(X[p].D, fin[2 * p][4], fin[2 * p + 1][4]);
+  }
 #pragma unroll
   for (int k = 0; k < BLEND_NPX; ++k) {
     if (!(px + k < (uint32_t)P.width && py < (uint32_t)P.height)) continue;   // recomputed: not kept live through the loop
-    const float Tk = fabsf(X[k].T);
+    const float Tk = fabsf(fin[k][0]);
     const float Al = 1.0f - Tk;
     if (out_rgb) {
       float bg[3] = {P.bg[0], P.bg[1], P.bg[2]};
@@ -405,17 +463,17 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
         sky_sample(P.sky, P.sky_res, fmaf(P.R[0], cxr, fmaf(P.R[3], cyr, P.R[6])),
                    fmaf(P.R[1], cxr, fmaf(P.R[4], cyr, P.R[7])), fmaf(P.R[2], cxr, fmaf(P.R[5], cyr, P.R[8])), bg);
       }
-      out_rgb[pi + k] = fmaf(Tk, bg[0], X[k].Cr);
-      out_rgb[HW + pi + k] = fmaf(Tk, bg[1], X[k].Cg);
-      out_rgb[2 * HW + pi + k] = fmaf(Tk, bg[2], X[k].Cb);
+      out_rgb[pi + k] = fmaf(Tk, bg[0], fin[k][1]);
+      out_rgb[HW + pi + k] = fmaf(Tk, bg[1], fin[k][2]);
+      out_rgb[2 * HW + pi + k] = fmaf(Tk, bg[2], fin[k][3]);
     }
-    if (out_depth) out_depth[pi + k] = MODE == BLEND_FEATURE ? X[k].D : (Al > 0.f ? X[k].D / Al : 0.f);
+    if (out_depth) out_depth[pi + k] = MODE == BLEND_FEATURE ? fin[k][4] : (Al > 0.f ? fin[k][4] / Al : 0.f);
     if (out_alpha) out_alpha[pi + k] = Al;
   }
 }
 
 template <bool COUNT, int MODE, int PHASE>
-__global__ void __launch_bounds__(BLEND_THREADS)
+__global__ void __launch_bounds__(BLEND_THREADS, PVG_BLEND_MINB)
 blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ranges,
              const uint32_t* __restrict__ vals, const float4* __restrict__ record,
              float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
