@@ -267,7 +267,9 @@ def algorithmic_bytes(agg, K, N, S, Msum, Mbsum, chunks, lazy):
     for key in (("onesweep_pass", "sort"), ("onesweep_pass", "depth_sort")):
         if key in agg:
             per_frame = agg[key][1] / K
-            alg[key] = 24.0 * (Msum if key[1] == "sort" else K * N) * per_frame
+            # depth sort (9 + 9 + 9 + 4 bits): pass 0 reads the n pairs and writes the S survivors, passes 1 and 2 move
+            # the S survivors, the top-digit pass is the identity and exits (12 B per pair each way)
+            alg[key] = 24.0 * Msum * per_frame if key[1] == "sort" else K * (12.0 * N + 60.0 * S)
     return alg
 
 

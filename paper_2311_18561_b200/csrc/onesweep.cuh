@@ -157,13 +157,17 @@ struct RadixCore {
   static constexpr int TILE = THREADS * ITEMS;
   static constexpr int RADIX = 1 << BITS;
   static constexpr int DWARPS = (RADIX + 31) / 32;  // warps that hold the digit threads
-  static_assert(THREADS >= RADIX && TILE < 65536, "digit threads / u16 positions");
+  static constexpr int DSHIFT = BITS <= 8 ? 8 : BITS;   // dp = digit | position << DSHIFT
+  static constexpr uint32_t DMASK = (1u << DSHIFT) - 1u;
+  static constexpr uint32_t INVALID = 0xFFFFFFFFu;      // SPARSE: "no element here"
+  static_assert(THREADS >= RADIX && TILE < 65536 && DSHIFT + 16 <= 32, "digit threads / u16 positions");
 
   struct Smem {
     uint32_t warp_off[WARPS * RADIX];  // per-warp digit counts -> tile-local start of (warp, digit)
     uint32_t out_base[RADIX];          // output index of the digit's run MINUS its tile-local start
     uint32_t warp_sums[DWARPS];
     uint32_t tile;
+    uint32_t total;                    // elements of the tile that take part (SPARSE: the valid ones)
   };
 
   __device__ static __forceinline__ uint32_t take_ticket(Smem& s, uint32_t* ticket) {
@@ -174,9 +178,12 @@ struct RadixCore {
   }
 
   // In: dp[j] = digit of the thread's j-th element (padding elements carry RADIX-1 and must
-  // be the last elements of the tile). Out: dp[j] = digit | tile-local sorted position << 8
+  // be the last elements of the tile). Out: dp[j] = digit | tile-local sorted position << DSHIFT
   // (packed to save registers). Ends with a __syncthreads(); afterwards
   // s.out_base[digit] + position is the element's output index.
+  // SPARSE: elements with dp[j] == INVALID take no part (anywhere in the tile): they are not counted, get no
+  // position and keep dp[j] == INVALID; s.total is the number of elements that do take part.
+  template <bool SPARSE = false>
   __device__ static __forceinline__ void rank(Smem& s, uint32_t tile, uint32_t (&dp)[ITEMS],
                                               const uint32_t* __restrict__ hist_excl,
                                               uint64_t* __restrict__ lookback) {
@@ -185,13 +192,15 @@ struct RadixCore {
     const uint32_t lt = lanemask_lt();
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
-      const uint32_t d = dp[j];
-      const uint32_t peers = digit_peers<BITS>(d);
+      const bool ok = !SPARSE || dp[j] != INVALID;
+      const uint32_t d = ok ? dp[j] : 0u;
+      uint32_t peers = digit_peers<BITS>(d);
+      if (SPARSE) peers &= __ballot_sync(0xffffffffu, ok);
       const uint32_t before = wh[d];
       __syncwarp();
-      if ((peers & lt) == 0) wh[d] = before + __popc(peers);
+      if (ok && (peers & lt) == 0) wh[d] = before + __popc(peers);
       __syncwarp();
-      dp[j] = d | ((before + __popc(peers & lt)) << 8);
+      dp[j] = ok ? (d | ((before + __popc(peers & lt)) << DSHIFT)) : INVALID;
     }
     __syncthreads();
 
@@ -219,6 +228,7 @@ struct RadixCore {
 #pragma unroll
       for (int w = 0; w < DWARPS; ++w)
         if (w < (int)warp) start += s.warp_sums[w];
+      if (tid == RADIX - 1) s.total = start + tile_count;
       if (live) {
         uint32_t run = start;
 #pragma unroll
@@ -232,7 +242,10 @@ struct RadixCore {
         if (tile != 0) {
           // windowed: the status words of the next LB_WINDOW predecessors are fetched together (one L2
           // round trip), then consumed in order up to the first one that is not published yet
-          constexpr int LB_WINDOW = 4;
+#ifndef PVG_LB_WINDOW
+#define PVG_LB_WINDOW 4
+#endif
+          constexpr int LB_WINDOW = PVG_LB_WINDOW;
           uint32_t left = tile;   // predecessors not yet consumed; tile 0 always ends the walk
           const uint64_t* p = lookback + (uint64_t)(tile - 1) * RADIX + tid;
           bool done = false;
@@ -262,7 +275,8 @@ struct RadixCore {
     }
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < ITEMS; ++j) dp[j] += wh[dp[j] & 0xFFu] << 8;
+    for (int j = 0; j < ITEMS; ++j)
+      if (!SPARSE || dp[j] != INVALID) dp[j] += wh[dp[j] & DMASK] << DSHIFT;
   }
 };
 
@@ -327,8 +341,8 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
 
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
-    s.keys[dp[j] >> 8] = key[j];
-    s.vals[dp[j] >> 8] = val[j];
+    s.keys[dp[j] >> Core::DSHIFT] = key[j];
+    s.vals[dp[j] >> Core::DSHIFT] = val[j];
   }
   __syncthreads();
 
@@ -337,6 +351,91 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
     const uint64_t k = s.keys[p];
     const uint32_t w = HI ? (uint32_t)(k >> 32) : (uint32_t)k;
     const uint32_t o = s.core.out_base[(w >> shift32) & MASK] + p;
+    keys_out[o] = k;
+    vals_out[o] = s.vals[p];
+  }
+}
+
+// ---- the depth sort of the Gaussians: its own plan and pass kernel ------------------------------
+// Keys are the n depth pairs preprocess writes: low half = fp32 bits of z MINUS the fp32 bits of znear (z > znear > 0,
+// so the difference is positive and order-preserving; for z up to 65536 znear it is below 2^27), or 0xFFFFFFFF for a
+// culled Gaussian; upper half = the packed tile rectangle (payload). 31 key bits in digits of 9 + 9 + 9 + 4:
+//   * pass 0 reads all n pairs and DROPS the culled ones (they take no part in its ranking, RadixCore SPARSE), so the
+//     later passes, the scan and the list building see the S survivors only (75 % of n at config 3);
+//   * a pass whose digit is the same for every key is the identity and exits at once -- the 4-bit top digit of any
+//     scene whose far plane is below 65536 znear: three passes instead of the four of an 8-bit plan;
+//   * S, which passes run and which buffer each reads are decided on the device by the last CTA of preprocess, which
+//     holds the digit histograms (DepthCtl); every pass is launched for the worst case and reads the block.
+constexpr int DS_PASSES = 4;
+constexpr int DS_BITS = 9;
+constexpr int DS_RADIX = 1 << DS_BITS;
+constexpr int DS_TOP_BITS = 31 - 3 * DS_BITS;   // 4
+__host__ __device__ constexpr int ds_shift(int p) { return p * DS_BITS; }
+__host__ __device__ constexpr int ds_bits(int p) { return p < 3 ? DS_BITS : DS_TOP_BITS; }
+
+// control block in device memory, written by preprocess's last CTA (preprocess.cuh)
+struct DepthCtl {
+  uint32_t survivors;          // S
+  uint32_t final_side;         // which buffer pair holds the sorted pairs
+  uint32_t skip[DS_PASSES];    // 1: the pass is the identity
+  uint32_t in_side[DS_PASSES]; // buffer pair the pass reads (it writes the other one)
+};
+
+template <int THREADS, int ITEMS, int BITS, int MINB, bool FIRST>
+__global__ void __launch_bounds__(THREADS, MINB)
+depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, uint64_t* __restrict__ keys_b,
+                  uint32_t* __restrict__ vals_b, uint32_t n /* pairs in buffer a (FIRST) */, int pass, int shift,
+                  const DepthCtl* __restrict__ ctl, const uint32_t* __restrict__ hist_excl /* [512] this pass */,
+                  uint64_t* __restrict__ lookback /* [tiles][1 << BITS], zeroed */, uint32_t* __restrict__ ticket /* zeroed */) {
+  using Core = RadixCore<THREADS, ITEMS, BITS>;
+  constexpr int TILE = Core::TILE;
+  constexpr uint32_t MASK = (1u << BITS) - 1u;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  OnesweepSmem<THREADS, ITEMS, BITS>& s = *reinterpret_cast<OnesweepSmem<THREADS, ITEMS, BITS>*>(smem_raw);
+  if (!FIRST) {
+    if (ctl->skip[pass]) return;
+    n = ctl->survivors;
+  }
+  const bool from_a = FIRST || ctl->in_side[pass] == 0u;
+  const uint64_t* keys_in = from_a ? keys_a : keys_b;
+  const uint32_t* vals_in = from_a ? vals_a : vals_b;
+  uint64_t* keys_out = from_a ? keys_b : keys_a;
+  uint32_t* vals_out = from_a ? vals_b : vals_a;
+
+  const uint32_t tile = Core::take_ticket(s.core, ticket);
+  const uint32_t tile_base = tile * TILE;
+  if (tile_base >= n) return;   // launched for n pairs, S are left: nobody looks back at a tile past the end
+  const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
+  const uint32_t tid = threadIdx.x;
+  const uint32_t wbase = (tid >> 5) * (ITEMS * 32) + (tid & 31u);
+  const uint64_t* kp = keys_in + tile_base + wbase;
+  const uint32_t* vp = vals_in + tile_base + wbase;
+  uint64_t key[ITEMS];
+  uint32_t val[ITEMS], dp[ITEMS];
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const bool ok = wbase + j * 32 < tile_n;
+    key[j] = ok ? __ldcg(kp + j * 32) : ~0ull;
+    val[j] = ok ? __ldcg(vp + j * 32) : 0u;
+  }
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const uint32_t w = (uint32_t)key[j];
+    // the culled Gaussians (and the padding of the last tile) carry 0xFFFFFFFF: no element
+    dp[j] = w == 0xFFFFFFFFu ? Core::INVALID : ((w >> shift) & MASK);
+  }
+  Core::template rank<true>(s.core, tile, dp, hist_excl, lookback);
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j)
+    if (dp[j] != Core::INVALID) {
+      s.keys[dp[j] >> Core::DSHIFT] = key[j];
+      s.vals[dp[j] >> Core::DSHIFT] = val[j];
+    }
+  __syncthreads();
+  const uint32_t total = s.core.total;
+  for (uint32_t p = tid; p < total; p += THREADS) {
+    const uint64_t k = s.keys[p];
+    const uint32_t o = s.core.out_base[((uint32_t)k >> shift) & MASK] + p;
     keys_out[o] = k;
     vals_out[o] = s.vals[p];
   }

@@ -10,6 +10,7 @@
 #pragma once
 
 #include "common.cuh"
+#include "onesweep.cuh"
 
 namespace pvg {
 
@@ -53,8 +54,9 @@ __device__ __forceinline__ double sinpi_reduced(double x) {
 //                           colour slot holds vbar in camera axes and featw[i] = clamp(rho, 0, 2)
 //   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
-//   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | fp32 bits of z, or 0xFFFFFFFF if culled), i
-// Returns the low half of the depth-sort key: the fp32 bits of z, 0xFFFFFFFF if culled.
+//   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | depth key, or 0xFFFFFFFF if culled), i
+//                           depth key = fp32 bits of z - fp32 bits of znear (z > znear > 0: positive, same order as z)
+// Returns the depth key, 0xFFFFFFFF if culled.
 // PART: PRE_ALL -- everything. PRE_GEO -- what the list building needs (tile info, counts, depth pair) without the
 // record: the 192 B of SH coefficients are not read (lazy lists: most Gaussians are never composited). Whether a
 // Gaussian survives depends on its colour only through the non-finite-colour cull, which needs non-finite or
@@ -289,20 +291,27 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
       const uint32_t x0 = ti.x & 0xFFFFu, y0 = ti.x >> 16;
       rect = x0 | (y0 << 8) | ((x0 + (ti.y & 0xFFFFu) - 1u) << 16) | ((y0 + (ti.y >> 16) - 1u) << 24);
     }
-    dkeys[i] = valid ? (((uint64_t)rect << 32) | ti.z) : 0xFFFFFFFFull;
+    dkeys[i] = valid ? (((uint64_t)rect << 32) | (ti.z - __float_as_uint(P.znear))) : 0xFFFFFFFFull;
     dvals[i] = i;
   }
-  return valid ? ti.z : 0xFFFFFFFFu;
+  return valid ? ti.z - __float_as_uint(P.znear) : 0xFFFFFFFFu;
 }
 
-// PRE_CHUNKS consecutive groups of 256 Gaussians per CTA. With dhist != nullptr the CTA also counts the four
-// 8-bit digits of its depth keys in shared memory, adds them to dhist[4][256] (zeroed) and the last CTA to
-// finish (dhist[1024] counts them) turns the counts into the exclusive prefixes the onesweep passes of the
-// depth sort start from -- the keys are in registers here; a histogram kernel would read them back from HBM.
+// PRE_CHUNKS consecutive groups of 256 Gaussians per CTA. With dhist != nullptr the CTA also counts the four digits
+// (9 + 9 + 9 + 4 bits, onesweep.cuh "depth sort") of its survivors' depth keys in shared memory, adds them to
+// dhist[4][512] (zeroed) and the last CTA to finish (dhist[DH_COUNTER] counts them) turns the counts into the
+// exclusive prefixes the passes of the depth sort start from, and writes the sort's control block: the number of
+// survivors S, which passes are the identity (one non-empty bin) and which buffer each pass reads -- the keys are in
+// registers here; a histogram kernel would read them back from HBM.
 #ifndef PVG_PRE_CHUNKS
 #define PVG_PRE_CHUNKS 4
 #endif
 constexpr int PRE_CHUNKS = PVG_PRE_CHUNKS;
+constexpr int DH_COUNTER = DS_PASSES * DS_RADIX;   // u32 index of the CTA counter inside a dhist half
+constexpr int DH_CTL = DH_COUNTER + 8;             // u32 index of the DepthCtl block (8-byte aligned)
+constexpr int DH_WORDS = DH_CTL + 16;              // words per dhist half (a multiple of 4)
+static_assert(sizeof(DepthCtl) <= 16 * 4, "DepthCtl fits its slot");
+
 template <int PART>
 __global__ void __launch_bounds__(256)
 preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8_t* __restrict__ shflag,
@@ -311,11 +320,11 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
                   const float4* __restrict__ SH, float4* __restrict__ record,
                   uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
                   uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, float* __restrict__ featw,
-                  uint32_t* __restrict__ dhist) {
-  __shared__ uint32_t s_hist[4 * 256];
+                  uint32_t* __restrict__ dhist, volatile uint64_t* __restrict__ host_words /* mapped: [4] = S, [5] = final side, [6] = skipped passes (bit p) */) {
+  __shared__ uint32_t s_hist[DS_PASSES * DS_RADIX];
   if (dhist) {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) s_hist[k * 256 + threadIdx.x] = 0;
+    for (int k = 0; k < DS_PASSES * DS_RADIX / 256; ++k) s_hist[k * 256 + threadIdx.x] = 0;
     __syncthreads();
   }
 #pragma unroll 1
@@ -323,65 +332,103 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
     const uint32_t i = (blockIdx.x * PRE_CHUNKS + c) * 256u + threadIdx.x;
     if (i >= n) break;
     const uint32_t z = preprocess_point<PART>(P, n, i, shflag, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
-    if (dhist) {
+    if (dhist && z != 0xFFFFFFFFu) {
 #pragma unroll
-      for (int k = 0; k < 4; ++k) atomicAdd(&s_hist[k * 256 + ((z >> (8 * k)) & 0xFFu)], 1u);
+      for (int k = 0; k < DS_PASSES; ++k) atomicAdd(&s_hist[k * DS_RADIX + ((z >> ds_shift(k)) & ((1u << ds_bits(k)) - 1u))], 1u);
     }
   }
   if (!dhist) return;
   __syncthreads();
 #pragma unroll
-  for (int k = 0; k < 4; ++k) {
+  for (int k = 0; k < DS_PASSES * DS_RADIX / 256; ++k) {
     const uint32_t v = s_hist[k * 256 + threadIdx.x];
     if (v) atomicAdd(&dhist[k * 256 + threadIdx.x], v);
   }
   __shared__ bool s_last;
-  __shared__ uint32_t s_warp[8];
+  __shared__ uint32_t s_warp[8], s_bins[8];
   __threadfence();
   __syncthreads();
-  if (threadIdx.x == 0) s_last = atomicAdd(dhist + 1024, 1u) == gridDim.x - 1;
+  if (threadIdx.x == 0) s_last = atomicAdd(dhist + DH_COUNTER, 1u) == gridDim.x - 1;
   __syncthreads();
   if (!s_last) return;
   __threadfence();
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  for (int k = 0; k < 4; ++k) {
-    const uint32_t v = __ldcg(dhist + k * 256 + threadIdx.x);
+  uint32_t nonempty[DS_PASSES], total = 0;
+  for (int k = 0; k < DS_PASSES; ++k) {
+    // thread t owns bins 2 t, 2 t + 1 of the digit's 512
+    const uint32_t v0 = __ldcg(dhist + k * DS_RADIX + 2 * threadIdx.x), v1 = __ldcg(dhist + k * DS_RADIX + 2 * threadIdx.x + 1);
+    const uint32_t v = v0 + v1;
     uint32_t incl = v;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
       const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
       if (lane >= d) incl += t;
     }
-    if (lane == 31) s_warp[warp] = incl;
+    const uint32_t ne = __reduce_add_sync(0xffffffffu, (v0 ? 1u : 0u) + (v1 ? 1u : 0u));
+    if (lane == 31) { s_warp[warp] = incl; s_bins[warp] = ne; }
     __syncthreads();
-    uint32_t wex = 0;
-    for (uint32_t w = 0; w < warp; ++w) wex += s_warp[w];
-    dhist[k * 256 + threadIdx.x] = wex + incl - v;
+    uint32_t wex = 0, bins = 0, all = 0;
+    for (uint32_t w = 0; w < 8; ++w) {
+      if (w < warp) wex += s_warp[w];
+      all += s_warp[w];
+      bins += s_bins[w];
+    }
+    const uint32_t ex = wex + incl - v;
+    dhist[k * DS_RADIX + 2 * threadIdx.x] = ex;
+    dhist[k * DS_RADIX + 2 * threadIdx.x + 1] = ex + v0;
+    nonempty[k] = bins;
+    total = all;
     __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    DepthCtl* ctl = reinterpret_cast<DepthCtl*>(dhist + DH_CTL);
+    ctl->survivors = total;
+    uint32_t side = 0;
+    for (int k = 0; k < DS_PASSES; ++k) {
+      const uint32_t skip = (k > 0 && nonempty[k] <= 1u) ? 1u : 0u;   // pass 0 always runs: it drops the culled pairs
+      ctl->skip[k] = skip;
+      ctl->in_side[k] = side;
+      side ^= skip ^ 1u;
+    }
+    ctl->final_side = side;
+    if (host_words) {
+      uint32_t skips = 0;
+      for (int k = 0; k < DS_PASSES; ++k) skips |= ctl->skip[k] << k;
+      host_words[4] = total; host_words[5] = side; host_words[6] = skips;
+    }
   }
 }
 
-// The records PRE_GEO left out, for the Gaussians at depth ranks [*r_lo (or 0), *r_hi + 1 (or n)) of the sorted
-// order: the same arithmetic as preprocess_kernel<PRE_ALL>, so the records are bit-identical to an eager frame.
-// only_if: nothing to do when *only_if == 0 (lazy lists: the second round runs only if a tile was parked).
+// The records PRE_GEO left out, for the survivors at depth ranks [*r_lo + 1 (or 0), *r_hi + 1 (or nv)) of the sorted
+// order (nv = S survivors): the same arithmetic as preprocess_kernel<PRE_ALL>, so the records are bit-identical to an
+// eager frame. only_if: nothing to do when *only_if == 0 (lazy lists: the second round runs only if a tile was parked).
 __global__ void __launch_bounds__(256)
-shade_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit,
+shade_kernel(const __grid_constant__ FrameParams P, uint32_t n, uint32_t nv, const uint32_t* __restrict__ visit,
              const uint32_t* __restrict__ r_lo, const uint32_t* __restrict__ r_hi, const uint32_t* __restrict__ only_if,
              const float4* __restrict__ A0, const float4* __restrict__ A1, const float4* __restrict__ A2,
-             const float4* __restrict__ A3, const float4* __restrict__ SH, float4* __restrict__ record, float* __restrict__ featw,
-             int zero_culled /* pvg_debug_view: the culled Gaussians' records read as zero */) {
+             const float4* __restrict__ A3, const float4* __restrict__ SH, float4* __restrict__ record, float* __restrict__ featw) {
   if (only_if && *only_if == 0u) return;
-  const uint32_t lo = r_lo ? *r_lo + 1u : 0u, hi = r_hi ? min(*r_hi + 1u, n) : n;
+  const uint32_t lo = r_lo ? *r_lo + 1u : 0u, hi = r_hi ? min(*r_hi + 1u, nv) : nv;
   const uint32_t r = lo + blockIdx.x * 256u + threadIdx.x;
   if (r >= hi) return;
-  if ((uint32_t)keys[r] == 0xFFFFFFFFu) {   // culled (they sort last): nobody composites them
-    if (zero_culled) {
-      const size_t g = visit[r];
-      record[3 * g] = record[3 * g + 1] = record[3 * g + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
+  preprocess_point<PRE_REC>(P, n, visit[r], nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
+}
+
+// The records of ALL Gaussians in index order (coalesced model reads: 4 x faster than the gather by depth rank when
+// most of the scene has to be shaded anyway -- the second round of a frame whose tiles parked, pvg_debug_view):
+// survivors (counts[i] != 0) get their record, culled Gaussians zeros.
+__global__ void __launch_bounds__(256)
+shade_all_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint32_t* __restrict__ counts, const uint32_t* __restrict__ only_if,
+                 const float4* __restrict__ A0, const float4* __restrict__ A1, const float4* __restrict__ A2,
+                 const float4* __restrict__ A3, const float4* __restrict__ SH, float4* __restrict__ record, float* __restrict__ featw) {
+  if (only_if && *only_if == 0u) return;
+  const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+  if (i >= n) return;
+  if (counts[i] == 0u) {
+    record[3 * (size_t)i] = record[3 * (size_t)i + 1] = record[3 * (size_t)i + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
     return;
   }
-  preprocess_point<PRE_REC>(P, n, visit[r], nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
+  preprocess_point<PRE_REC>(P, n, i, nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
 }
 
 // One-off re-layout of the caller's arrays into the SoA float4 model (pvg_create_scene).

@@ -148,7 +148,7 @@ constexpr uint64_t OS_SMALL_BELOW = PVG_OS_SMALL_BELOW;
 // scratch of one sort call
 // layout of pvg_scene::unf: [256] u64 block masks | u32 parked count (+ pad) | [tiles] u32 lim | [tiles] u32 parked list
 constexpr size_t kUnfHead = 2048 + 64;
-constexpr size_t kDhistWords = 1032;   // 4 x 256 counts + the CTA counter, padded to 16 B
+constexpr size_t kDhistWords = DH_WORDS;   // 4 x 512 digit counts, the CTA counter and the depth sort's control block
 
 struct SortScratch {
   Buf hist;      // [passes][256] u32
@@ -298,6 +298,63 @@ int run_onesweep(const Dev& dv, uint64_t n, uint64_t* ka, uint32_t* va, uint64_t
   return PVG_OK;
 }
 
+// ---- the depth sort of the Gaussians (onesweep.cuh: 9 + 9 + 9 + 4 bits, pass 0 drops the culled pairs) ----------
+#ifndef PVG_DS_THREADS
+#define PVG_DS_THREADS 512
+#define PVG_DS_ITEMS 8
+#define PVG_DS_MINB 2
+#endif
+struct DsCfg { static constexpr int THREADS = PVG_DS_THREADS, ITEMS = PVG_DS_ITEMS, MINB = PVG_DS_MINB; };
+constexpr uint32_t kDsTile = DsCfg::THREADS * DsCfg::ITEMS;
+
+inline size_t depth_lookback_words(uint32_t n) {
+  const size_t tiles = (n + kDsTile - 1) / kDsTile;
+  return tiles * (size_t)(3 * DS_RADIX + (1 << DS_TOP_BITS));
+}
+
+// sizes and zeroes the tickets and look-back words of the four passes on stream zs
+int prep_depth_sort(uint32_t n, cudaStream_t alloc_st, cudaStream_t zs, SortScratch& sc) {
+  TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, alloc_st));
+  TRY(sc.lookback.reserve(depth_lookback_words(n) * 8, alloc_st, 1.25));
+  CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, zs));
+  CU(cudaMemsetAsync(sc.lookback.p, 0, depth_lookback_words(n) * 8, zs));
+  return PVG_OK;
+}
+
+template <int BITS, bool FIRST>
+int launch_depth_pass(uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, uint32_t n, int pass, const DepthCtl* ctl,
+                      const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev) {
+  using Smem = OnesweepSmem<DsCfg::THREADS, DsCfg::ITEMS, BITS>;
+  auto kern = depth_pass_kernel<DsCfg::THREADS, DsCfg::ITEMS, BITS, DsCfg::MINB, FIRST>;
+  PVG_ENSURE_SMEM(kern, sizeof(Smem), dev);
+  kern<<<(n + kDsTile - 1) / kDsTile, DsCfg::THREADS, sizeof(Smem), st>>>(ka, va, kb, vb, n, pass, ds_shift(pass), ctl, hist, lookback, ticket);
+  return PVG_OK;
+}
+
+// dh: this frame's dhist half (exclusive digit prefixes + DepthCtl, written by preprocess). Every pass is launched
+// for n pairs; passes 1..3 read S and their input side from the control block and exit at once if they are the identity.
+// Launches passes [p0, p1). The frame launches 0..2 at once and the top-digit pass after its host wait, only if
+// preprocess found it to be needed (it is the identity unless the far plane is beyond 65536 znear).
+int run_depth_sort(const Dev& dv, uint32_t n, uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, const uint32_t* dh,
+                   cudaStream_t st, SortScratch& sc, Timer* tm, int p0 = 0, int p1 = DS_PASSES) {
+  const DepthCtl* ctl = reinterpret_cast<const DepthCtl*>(dh + DH_CTL);
+  const size_t tiles = (n + kDsTile - 1) / kDsTile;
+  uint64_t* lb = sc.lookback.as<uint64_t>();
+  uint32_t* tk = sc.tickets.as<uint32_t>();
+  for (int p = 0; p < p0; ++p) lb += tiles * (size_t)(1 << ds_bits(p));
+  for (int p = p0; p < p1; ++p) {
+    if (tm) TRY(tm->begin("onesweep_pass", PVG_STAGE_DEPTH_SORT, st));
+    const uint32_t* hist = dh + p * DS_RADIX;
+    if (p == 0) TRY((launch_depth_pass<DS_BITS, true>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal)));
+    else if (p < 3) TRY((launch_depth_pass<DS_BITS, false>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal)));
+    else TRY((launch_depth_pass<DS_TOP_BITS, false>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal)));
+    if (tm) TRY(tm->end(st));
+    lb += tiles * (size_t)(1 << ds_bits(p));
+  }
+  CU(cudaGetLastError());
+  return PVG_OK;
+}
+
 #ifndef PVG_CP_THREADS
 #define PVG_CP_THREADS 384
 #define PVG_CP_ITEMS 16
@@ -369,6 +426,7 @@ struct Model {
 
 struct pvg_scene {
   uint32_t n = 0;
+  uint32_t nv = 0;   // pairs in visiting order that take part in the last frame: the S survivors (PRESORT_DEPTH) or n
   float cycle = 0.2f;
   int sh_degree = 3;
   cudaStream_t stream = nullptr;
@@ -381,6 +439,7 @@ struct pvg_scene {
   int lazy_slab = 8;                  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front
   uint32_t emit_first = 0, emit_tiles = 0, emit_radix = 256;   // bin_emit tiles in the first launch / in all; its look-back row length
   const uint32_t* visit_last = nullptr;
+  bool visit_tail_done = false;       // pvg_debug_view has appended the culled Gaussians to the visiting order
   bool light = false;                 // this frame's preprocess left the records to shade_kernel
   bool records_complete = true;       // record[] holds every Gaussian's record (pvg_debug_view completes them on demand)
   float* featw_last = nullptr;
@@ -399,7 +458,7 @@ struct pvg_scene {
   // block-entry workspace (blockbin.cuh)
   Buf boffsets, chunk_owner, e_bin, e_g, e_mask, s_g, s_mask, bin_tables, chunk_cnt;
   Buf lazy_state, unf;   // blend state of parked tiles [5][H W]; unfinished flags: [256] u64 block masks, then [tiles] u32
-  Buf dhist;          // 2 x (4 x 256 digit counts + 1 CTA counter) u32: the depth histogram preprocess accumulates, double-buffered
+  Buf dhist;          // 2 x DH_WORDS u32 (preprocess.cuh): digit histograms + control block of the depth sort, double-buffered
   int dhist_side = 0;
   Buf ranges, tilegrid;
   Buf featw;   // clamp(rho, 0, 2) per Gaussian (dynamics target)
@@ -609,9 +668,11 @@ int prep_scan(pvg_scene* s, cudaStream_t zs) {
   return PVG_OK;
 }
 
-int run_scan(pvg_scene* s, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm, bool scratch_ready = false) {
+// nv: the first nv visiting positions are scanned (the survivors after the depth sort; n otherwise)
+int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm, bool scratch_ready = false) {
   cudaStream_t st = s->stream;
-  const uint32_t n = s->n;
+  const uint32_t n = nv;
+  if (n == 0) return PVG_OK;
   const uint32_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
   if (!scratch_ready) {
     TRY(prep_scan(s, st));
@@ -648,7 +709,7 @@ int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t b
   auto kern = bin_emit_kernel<BITS>;
   PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
   kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
-      s->n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
+      s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
       blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if);
   return PVG_OK;
 }
@@ -705,14 +766,24 @@ int run_bin_emit(pvg_scene* s, const FrameParams& P, const uint32_t* visit, uint
 }
 #endif
 
-// shade_kernel over the depth ranks (r_lo, r_hi] given by device words (nullptr: from the start / to the end)
-int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const uint32_t* r_hi, const uint32_t* only_if, int zero_culled,
+// shade_kernel over the depth ranks (r_lo, r_hi] given by device words (nullptr: from the start / to the last survivor)
+int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const uint32_t* r_hi, const uint32_t* only_if,
               cudaStream_t on = nullptr) {
   const Model* m = s->model;
-  shade_kernel<<<(s->n + 255) / 256, 256, 0, on ? on : s->stream>>>(P, s->n, s->dkeys[s->visit_side].as<uint64_t>(), s->visit_last, r_lo, r_hi,
-                                                          only_if, m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(),
-                                                          m->A3.as<float4>(), m->SH.as<float4>(), s->record.as<float4>(),
-                                                          s->featw_last, zero_culled);
+  if (s->nv == 0) return PVG_OK;
+  shade_kernel<<<(s->nv + 255) / 256, 256, 0, on ? on : s->stream>>>(P, s->n, s->nv, s->visit_last, r_lo, r_hi, only_if,
+                                                                      m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(),
+                                                                      m->A3.as<float4>(), m->SH.as<float4>(), s->record.as<float4>(),
+                                                                      s->featw_last);
+  return PVG_OK;
+}
+
+// every Gaussian's record, in index order (zeros for the culled ones)
+int run_shade_all(pvg_scene* s, const FrameParams& P, const uint32_t* only_if) {
+  const Model* m = s->model;
+  shade_all_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(P, s->n, s->counts.as<uint32_t>(), only_if, m->A0.as<float4>(),
+                                                               m->A1.as<float4>(), m->A2.as<float4>(), m->A3.as<float4>(),
+                                                               m->SH.as<float4>(), s->record.as<float4>(), s->featw_last);
   return PVG_OK;
 }
 
@@ -765,7 +836,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
     CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
     tm->cut();
     TRY(tm->begin("shade", PVG_STAGE_PREPROCESS, sd));
-    TRY(run_shade(s, P, nullptr, s->emit_first < s->emit_tiles ? s->chunk_owner.as<uint32_t>() + s->emit_first : nullptr, nullptr, 0, sd));
+    TRY(run_shade(s, P, nullptr, s->emit_first < s->emit_tiles ? s->chunk_owner.as<uint32_t>() + s->emit_first : nullptr, nullptr, sd));
     TRY(tm->end(sd));
     CU(cudaEventRecord(s->ev_join, sd));
   }
@@ -775,7 +846,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
-      s->n, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x,
+      s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit, blocks_x,
       s->e_bin.as<uint8_t>(),
       s->e_g.as<uint32_t>(), s->e_mask.as<uint64_t>());
   TRY(tm->end(st));
@@ -825,6 +896,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   const uint32_t tiles = (uint32_t)P.tiles_x * (uint32_t)P.tiles_y;
   s->tiles_x = P.tiles_x; s->tiles_y = P.tiles_y;
   s->rendered = false;
+  s->visit_tail_done = false;
   TRY(s->ranges.reserve((size_t)tiles * 8, st));
 
   const int tile_bits = std::max(1, ceil_log2(tiles));
@@ -843,7 +915,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     CU(cudaStreamWaitEvent(st, s->ev_zero, 0));   // normally long past; matters only after a frame that stopped early
     CU(cudaEventRecord(s->ev_start, st));
     CU(cudaStreamWaitEvent(sd, s->ev_start, 0));
-    TRY(prep_onesweep(n, 0, 32, st, sd, s->sort_n, true));
+    TRY(prep_depth_sort(n, st, sd, s->sort_n));
     // the depth histogram is accumulated by preprocess into one half of dhist; the other half is zeroed here for
     // the next frame (its last readers, the previous frame's passes, are behind ev_start)
     s->dhist_side ^= 1;
@@ -874,12 +946,12 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       preprocess_kernel<PRE_GEO><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
                                                           m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
                                                           s->record.as<float4>(), s->tileinfo.as<uint4>(),
-                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh);
+                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh, s->d_total);
     else
       preprocess_kernel<PRE_ALL><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
                                                           m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
                                                           s->record.as<float4>(), s->tileinfo.as<uint4>(),
-                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh);
+                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh, s->d_total);
   }
   TRY(tm.end(st));
 
@@ -922,21 +994,24 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     CU(cudaEventRecord(s->ev_join, sd));
     tm.cut();
 
-    // a3 (n-key part): depth order of the Gaussians
-    int side = 0;
-    TRY(run_onesweep(s->dev, n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
-                     s->dvals[1].as<uint32_t>(), 0, 32, st, s->sort_n, &tm, PVG_STAGE_DEPTH_SORT, &side, true, true,
-                     s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords));
-    s->visit_side = side;
-    visit = s->dvals[side].as<uint32_t>();
+    // a3 (n-key part): depth order of the survivors
+    TRY(run_depth_sort(s->dev, n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
+                       s->dvals[1].as<uint32_t>(), s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords, st, s->sort_n, &tm, 0, 3));
 
-    // the one host wait of the frame, hidden behind the depth sort
+    // the one host wait of the frame, hidden behind the depth sort: the totals of the tile grid, and what preprocess's
+    // last CTA decided for the depth sort (S, and which buffer the sorted pairs end in)
     CU(cudaEventSynchronize(s->ev_join));
     CU(cudaStreamWaitEvent(st, s->ev_join, 0));
     tm.cut();
     M = s->h_total[0];
     s->Mb = block ? s->h_total[1] : 0;
-    s->survivors = s->h_total[2];
+    s->survivors = s->h_total[4];
+    s->nv = (uint32_t)s->h_total[4];
+    s->visit_side = (int)s->h_total[5];
+    visit = s->dvals[s->visit_side].as<uint32_t>();
+    if (!(s->h_total[6] & 8u))   // the top digit is not constant: its pass is needed
+      TRY(run_depth_sort(s->dev, n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
+                         s->dvals[1].as<uint32_t>(), s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords, st, s->sort_n, &tm, 3, 4));
     if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
     s->M = M;
     if (block && M > 0) {   // the side stream is idle now: size and zero the block path's scratch beside the depth sort
@@ -944,9 +1019,10 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       CU(cudaEventRecord(s->ev_zero, sd));
     }
     // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
-    TRY(run_scan(s, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm, true));
+    TRY(run_scan(s, s->nv, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm, true));
   } else {
-    TRY(run_scan(s, false, s->offsets.as<uint32_t>(), nullptr, &tm));
+    s->nv = n;
+    TRY(run_scan(s, n, false, s->offsets.as<uint32_t>(), nullptr, &tm));
     CU(cudaMemcpyAsync(s->h_total, s->small.as<unsigned char>() + 8, 8, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));   // index-order path: M is only known after the scan
     tm.cut();
@@ -974,7 +1050,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     }
     TRY(tm.begin("duplicate", PVG_STAGE_DUPLICATE, st));
     expand_kernel<true><<<(unsigned)((M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
-        n, (uint32_t)M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x, nullptr,
+        s->nv, (uint32_t)M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x, nullptr,
         s->tiles16[0].as<uint16_t>(), s->vals[0].as<uint32_t>());
     TRY(tm.end(st));
     if (s->keep_unsorted) {
@@ -996,7 +1072,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     // a2 emit
     TRY(tm.begin("duplicate", PVG_STAGE_DUPLICATE, st));
     expand_kernel<false><<<(unsigned)((M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
-        n, (uint32_t)M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x,
+        s->nv, (uint32_t)M, s->offsets.as<uint32_t>(), visit, s->tileinfo.as<uint4>(), (uint32_t)P.tiles_x,
         s->keys[0].as<uint64_t>(), nullptr, s->vals[0].as<uint32_t>());
     TRY(tm.end(st));
     if (s->keep_unsorted) {
@@ -1074,7 +1150,9 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
         TRY(tm.end(st));
         if (s->light) {
           TRY(tm.begin("shade", PVG_STAGE_PREPROCESS, st));
-          TRY(run_shade(s, P, s->chunk_owner.as<uint32_t>() + s->emit_first, nullptr, Z.unf_count, 0));
+          // the rest of the scene: in index order (sequential model reads; the first slab's records are rewritten
+          // with the same values)
+          TRY(run_shade_all(s, P, Z.unf_count));
           TRY(tm.end(st));
         }
       }
@@ -1343,9 +1421,26 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->counts = s->counts.as<uint32_t>();
   out->visit_order = s->presort_used ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
+  if (s->presort_used && s->nv < s->n && !s->visit_tail_done) {
+    // The depth sort drops the culled Gaussians in its first pass: the frame's visiting order holds the S survivors.
+    // The view documents all n positions (the culled ones follow, in index order): append them here, on the host --
+    // a debugging call.
+    std::vector<uint32_t> cnt(s->n), tail;
+    CU(cudaStreamSynchronize(s->stream));
+    CU(cudaMemcpy(cnt.data(), s->counts.p, (size_t)s->n * 4, cudaMemcpyDeviceToHost));
+    tail.reserve(s->n - s->nv);
+    for (uint32_t i = 0; i < s->n; ++i)
+      if (cnt[i] == 0u) tail.push_back(i);
+    if (tail.size() != (size_t)(s->n - s->nv)) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "debug view: %zu culled Gaussians, %u expected", tail.size(), s->n - s->nv);
+      return PVG_ERR_CUDA;
+    }
+    CU(cudaMemcpy(s->dvals[s->visit_side].as<uint32_t>() + s->nv, tail.data(), tail.size() * 4, cudaMemcpyHostToDevice));
+    s->visit_tail_done = true;
+  }
   if (s->block_used && s->light && !s->records_complete && s->M) {
     // lazy lists: the records the frame never needed (and zeros for the culled Gaussians)
-    TRY(run_shade(s, s->last_P, nullptr, nullptr, nullptr, 1));
+    TRY(run_shade_all(s, s->last_P, nullptr));
     CU(cudaGetLastError());
     s->records_complete = true;
   }
@@ -1370,7 +1465,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     // the block path never forms per-instance offsets or the unsorted list: produce them here
     cudaStream_t st = s->stream;
     const uint32_t* visit = s->dvals[s->visit_side].as<uint32_t>();
-    TRY(run_scan(s, false, s->offsets.as<uint32_t>(), visit, nullptr));
+    TRY(run_scan(s, s->n, false, s->offsets.as<uint32_t>(), visit, nullptr));
     if (s->M) {
       TRY(s->keys[0].reserve((size_t)s->M * 8, st));
       keys_from_ranges_kernel<<<s->tiles_x * s->tiles_y, 256, 0, st>>>(s->ranges.as<uint2>(), s->vals[0].as<uint32_t>(),
