@@ -35,6 +35,8 @@ def lib():
         L = C.CDLL(_build.build())
         L.oracle_tile_counts.restype = C.c_uint64
         L.oracle_tile_list.restype = C.c_uint64
+        L.oracle_tile_counts_ex.restype = C.c_uint64
+        L.oracle_tile_list_ex.restype = C.c_uint64
         L.oracle_record_stride.restype = C.c_int
         L.oracle_num_threads.restype = C.c_int
         _lib = L
@@ -103,47 +105,49 @@ def sh_basis(d: Sequence[float]) -> np.ndarray:
     return Y
 
 
-def tile_counts(rec, width, height):
-    """Integer chain step 1. Returns (rects [n,4] int32 inclusive, counts [n] uint32, M)."""
+def tile_counts(rec, width, height, exact: bool = False):
+    """Integer chain step 1. Returns (rects [n,4] int32 inclusive, counts [n] uint32, M). exact: count only the tiles
+    of the rectangle that pass the ellipse-versus-tile test P13."""
     rec = np.ascontiguousarray(rec, dtype=np.float32)
     n = rec.shape[0]
     assert rec.shape == (n, 12)
     rects = np.empty((n, 4), dtype=np.int32)
     counts = np.empty(n, dtype=np.uint32)
-    M = lib().oracle_tile_counts(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), _p(rects),
-                                 _p(counts))
+    M = lib().oracle_tile_counts_ex(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_int(1 if exact else 0),
+                                    _p(rects), _p(counts))
     return rects, counts, int(M)
 
 
-def keys(rec, width, height, order_mode=0):
+def keys(rec, width, height, order_mode=0, exact: bool = False):
     """Integer chain step 2 (offsets, unsorted list, std::stable_sort, ranges)."""
     rec = np.ascontiguousarray(rec, dtype=np.float32)
     n = rec.shape[0]
-    _, _, M = tile_counts(rec, width, height)
+    _, _, M = tile_counts(rec, width, height, exact)
     ntiles = ((width + 15) // 16) * ((height + 15) // 16)
     out = dict(M=M,
                offsets=np.zeros(n, dtype=np.uint64),
                keys_unsorted=np.zeros(M, dtype=np.uint64), vals_unsorted=np.zeros(M, dtype=np.uint32),
                keys_sorted=np.zeros(M, dtype=np.uint64), vals_sorted=np.zeros(M, dtype=np.uint32),
                ranges=np.zeros((ntiles, 2), dtype=np.uint32))
-    lib().oracle_keys(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_int(order_mode),
-                      _p(out["offsets"]), _p(out["keys_unsorted"]), _p(out["vals_unsorted"]),
+    lib().oracle_keys_ex(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_int(order_mode),
+                         C.c_int(1 if exact else 0), _p(out["offsets"]), _p(out["keys_unsorted"]), _p(out["vals_unsorted"]),
                       _p(out["keys_sorted"]), _p(out["vals_sorted"]), _p(out["ranges"]))
     return out
 
 
-def tile_list(rec, width, height, tile):
+def tile_list(rec, width, height, tile, exact: bool = False):
     """Sorted instance list of one tile, computed directly. Returns (keys u64, vals u32)."""
     rec = np.ascontiguousarray(rec, dtype=np.float32)
     n = rec.shape[0]
     L = lib()
-    cnt = int(L.oracle_tile_list(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height),
-                                 C.c_uint32(tile), C.c_uint64(0), None, None))
+    ex = C.c_int(1 if exact else 0)
+    cnt = int(L.oracle_tile_list_ex(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height),
+                                    C.c_uint32(tile), ex, C.c_uint64(0), None, None))
     k = np.zeros(cnt, dtype=np.uint64)
     v = np.zeros(cnt, dtype=np.uint32)
     if cnt:
-        L.oracle_tile_list(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_uint32(tile),
-                           C.c_uint64(cnt), _p(k), _p(v))
+        L.oracle_tile_list_ex(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_uint32(tile), ex,
+                              C.c_uint64(cnt), _p(k), _p(v))
     return k, v
 
 
@@ -171,7 +175,7 @@ def render(rec, width, height, bg=(0.0, 0.0, 0.0), mode="binned", tiles: Optiona
         tl_arr = np.ascontiguousarray(tiles, dtype=np.uint32)
         tl, ntl = _p(tl_arr), tl_arr.shape[0]
     lib().oracle_render(C.c_uint64(n), _p(rec), C.c_int(W), C.c_int(H), _p(bg),
-                        C.c_int({"brute": 0, "binned": 1}[mode]), tl, C.c_uint64(ntl),
+                        C.c_int({"brute": 0, "binned": 1, "binned_exact": 2}[mode]), tl, C.c_uint64(ntl),
                         C.c_int(1 if tie_budget else 0), _p(rgb), _p(depth), _p(alpha), _p(budget),
                         _p(cond), _p(stats), _p(sl) if sl is not None else None, _p(derived))
     # c_max: the colour scale of budget and cond (largest colour of a non-culled Gaussian or of the background)

@@ -129,6 +129,60 @@ inline uint32_t rect_of(const float* r, int TX, int TY, int rect[4]) {
   return (uint32_t)(tx1 - tx0 + 1) * (uint32_t)(ty1 - ty0 + 1);
 }
 
+// P13: which tiles of its rectangle can a Gaussian reach at all?
+// The rectangle (P10) is the bounding box of the region R = { x : alpha(x) >= 1/255 } = { d : a dx^2 + 2 b dx dy + c dy^2
+// <= k }, k = 2 ln(255 o~); towards its corners it holds tiles R does not touch. A tile is KEPT iff the box of its pixel
+// centres, [16 tx + 0.5, 16 tx + 15.5] x [16 ty + 0.5, 16 ty + 15.5], intersects a slightly enlarged R. For one tile row
+// (a band of dy) the x-projection of R within the band is an interval: its right end is the ellipse's right boundary
+// xr(dy) = (-b dy + sqrt(a k - det dy^2)) / a at the dy of the band closest to where xr peaks (dy = -(b/c) dxm, dxm =
+// sqrt(k c / det) the half-width of R), and mirrored for the left end. The decision is integer work: like P10 it is
+// taken in fp32 from the fp32 record by INDIVIDUALLY ROUNDED operations (+, -, *, /, sqrt, min, max, floor, ceil), so
+// that the CUDA path and this oracle decide identically. k is recovered without a logarithm from the record's
+// extent, hx^2 = k Sigma'xx = k c / det. Margins (k (1 + 2e-4) + 2e-5, 1e-3 px) keep the test on the safe side of every
+// rounding: a dropped tile has no pixel centre with alpha >= 1/255 (pinned by brute force in double).
+struct ExactTile {
+  bool refine;   // false: keep the whole rectangle (degenerate or non-finite conic)
+  float mx, my, a, b, det, akk, dyr, ia;
+};
+inline ExactTile exact_tile_params(const float* r) {
+  ExactTile e{};
+  const float a = r[4], b = r[5], c = r[6], hx = r[7];
+  const float det = a * c - b * b;
+  const float k = ((hx * hx) * det) / c;
+  const float kk = k * 1.0002f + 2e-5f;
+  const float dxm = std::sqrt((kk * c) / det);
+  const float dyr = -((b / c) * dxm);
+  const float ia = 1.0f / a;
+  e.mx = r[0]; e.my = r[1]; e.a = a; e.b = b; e.det = det; e.akk = a * kk; e.dyr = dyr; e.ia = ia;
+  e.refine = (det > 0.0f) && (a > 0.0f) && (c > 0.0f) && std::isfinite(kk) && std::isfinite(dxm) && std::isfinite(ia) &&
+             std::isfinite(dyr) && (kk > 0.0f);
+  return e;
+}
+// kept tiles [lo, hi] of tile row ty inside the rectangle's columns [tx0, tx1] (empty if lo > hi)
+inline void exact_row_span(const ExactTile& e, int ty, int tx0, int tx1, int& lo, int& hi) {
+  lo = tx0; hi = tx1;
+  if (!e.refine) return;
+  const float y0 = ((float)(16 * ty) + 0.5f) - e.my, y1 = y0 + 15.0f;
+  // the band of pixel-centre rows lies wholly above or below R (|dy| > sqrt(a k / det) on its near side): no tile
+  if ((y0 > 0.0f && e.akk - (e.det * y0) * y0 < 0.0f) || (y1 < 0.0f && e.akk - (e.det * y1) * y1 < 0.0f)) {
+    hi = tx0 - 1;
+    return;
+  }
+  const float tr = std::fmin(std::fmax(e.dyr, y0), y1);      // where the right boundary peaks inside the band
+  const float tl = std::fmin(std::fmax(-e.dyr, y0), y1);     // and the left one
+  const float dr = std::fmax(e.akk - (e.det * tr) * tr, 0.0f);
+  const float dl = std::fmax(e.akk - (e.det * tl) * tl, 0.0f);
+  const float xr = (std::sqrt(dr) - e.b * tr) * e.ia;
+  const float xl = (-std::sqrt(dl) - e.b * tl) * e.ia;
+  const float XR = (e.mx + xr) + 1e-3f, XL = (e.mx + xl) - 1e-3f;
+  if (!std::isfinite(XR) || !std::isfinite(XL)) return;
+  const float fh = std::floor((XR - 0.5f) * 0.0625f), fl = std::ceil((XL - 15.5f) * 0.0625f);
+  // clamp in float before the conversion (|values| may exceed the int range)
+  const int h = (int)std::fmin(std::fmax(fh, -2.0f), 1.0e6f), l = (int)std::fmin(std::fmax(fl, -2.0f), 1.0e6f);
+  if (l > lo) lo = l;
+  if (h < hi) hi = h;
+}
+
 // Depth order shared by every pixel (S11): ascending
 // (fp32 bit pattern of z, Gaussian index) over the non-culled rows.
 std::vector<uint32_t> depth_order(uint64_t n, const float* rec) {
@@ -397,18 +451,31 @@ void oracle_sh_basis(const double* d, double* Y) { sh_basis(d, Y); }
 
 // Integer chain, step 1: per-Gaussian tile rectangle + count from an fp32 record.
 // Returns M = sum of counts.
-uint64_t oracle_tile_counts(uint64_t n, const float* rec, int width, int height, int32_t* rects,
-                            uint32_t* counts) {
+// exact != 0: only the tiles of the rectangle that pass the P13 test are counted.
+uint64_t oracle_tile_counts_ex(uint64_t n, const float* rec, int width, int height, int exact, int32_t* rects,
+                               uint32_t* counts) {
   const int TX = (width + kTile - 1) / kTile, TY = (height + kTile - 1) / kTile;
   uint64_t M = 0;
   for (uint64_t i = 0; i < n; ++i) {
     int rc[4];
-    const uint32_t c = rect_of(rec + i * 12, TX, TY, rc);
+    uint32_t c = rect_of(rec + i * 12, TX, TY, rc);
+    if (c && exact) {
+      const ExactTile e = exact_tile_params(rec + i * 12);
+      c = 0;
+      for (int ty = rc[1]; ty <= rc[3]; ++ty) {
+        int lo, hi;
+        exact_row_span(e, ty, rc[0], rc[2], lo, hi);
+        if (hi >= lo) c += (uint32_t)(hi - lo + 1);
+      }
+    }
     if (rects) for (int k = 0; k < 4; ++k) rects[i * 4 + k] = rc[k];
     if (counts) counts[i] = c;
     M += c;
   }
   return M;
+}
+uint64_t oracle_tile_counts(uint64_t n, const float* rec, int width, int height, int32_t* rects, uint32_t* counts) {
+  return oracle_tile_counts_ex(n, rec, width, height, 0, rects, counts);
 }
 
 // Integer chain, step 2: emission order -> exclusive offsets -> unsorted
@@ -419,9 +486,9 @@ uint64_t oracle_tile_counts(uint64_t n, const float* rec, int width, int height,
 // Gaussian are emitted row-major (ty outer, tx inner).
 // offsets[n]: exclusive offset of Gaussian i's first instance (0-count rows get
 // the running offset at their position in the visiting order).
-void oracle_keys(uint64_t n, const float* rec, int width, int height, int order_mode,
-                 uint64_t* offsets, uint64_t* keys_unsorted, uint32_t* vals_unsorted,
-                 uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* ranges) {
+void oracle_keys_ex(uint64_t n, const float* rec, int width, int height, int order_mode, int exact,
+                    uint64_t* offsets, uint64_t* keys_unsorted, uint32_t* vals_unsorted,
+                    uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* ranges) {
   const int TX = (width + kTile - 1) / kTile, TY = (height + kTile - 1) / kTile;
   std::vector<uint32_t> visit;
   if (order_mode == 0) {
@@ -441,14 +508,19 @@ void oracle_keys(uint64_t n, const float* rec, int width, int height, int order_
     if (offsets) offsets[g] = off;
     const uint64_t zb = f32_bits(rec[(uint64_t)g * 12 + 2]);
     uint64_t o = off;
-    if (c)
-      for (int ty = rc[1]; ty <= rc[3]; ++ty)
-        for (int tx = rc[0]; tx <= rc[2]; ++tx) {
+    if (c) {
+      const ExactTile e = exact_tile_params(rec + (uint64_t)g * 12);
+      for (int ty = rc[1]; ty <= rc[3]; ++ty) {
+        int lo = rc[0], hi = rc[2];
+        if (exact) exact_row_span(e, ty, rc[0], rc[2], lo, hi);
+        for (int tx = lo; tx <= hi; ++tx) {
           keys_unsorted[o] = ((uint64_t)(ty * TX + tx) << 32) | zb;
           vals_unsorted[o] = g;
           ++o;
         }
-    off += c;
+      }
+    }
+    off = o;
   }
   const uint64_t M = off;
   std::vector<uint64_t> idx(M);
@@ -468,19 +540,31 @@ void oracle_keys(uint64_t n, const float* rec, int width, int height, int order_
   }
 }
 
+void oracle_keys(uint64_t n, const float* rec, int width, int height, int order_mode,
+                 uint64_t* offsets, uint64_t* keys_unsorted, uint32_t* vals_unsorted,
+                 uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* ranges) {
+  oracle_keys_ex(n, rec, width, height, order_mode, 0, offsets, keys_unsorted, vals_unsorted, keys_sorted, vals_sorted, ranges);
+}
+
 // One tile's sorted instance list computed directly (no global sort): every
 // non-culled Gaussian whose rectangle contains the tile, ascending by
 // (fp32 z bits, index). Used for sampled full-size parity. Returns the length;
 // writes at most `cap` entries.
-uint64_t oracle_tile_list(uint64_t n, const float* rec, int width, int height, uint32_t tile,
-                          uint64_t cap, uint64_t* keys, uint32_t* vals) {
+uint64_t oracle_tile_list_ex(uint64_t n, const float* rec, int width, int height, uint32_t tile, int exact,
+                             uint64_t cap, uint64_t* keys, uint32_t* vals) {
   const int TX = (width + kTile - 1) / kTile, TY = (height + kTile - 1) / kTile;
   const int tx = (int)(tile % TX), ty = (int)(tile / TX);
   std::vector<uint32_t> cand;
   for (uint64_t i = 0; i < n; ++i) {
     int rc[4];
-    if (rect_of(rec + i * 12, TX, TY, rc) && tx >= rc[0] && tx <= rc[2] && ty >= rc[1] && ty <= rc[3])
+    if (rect_of(rec + i * 12, TX, TY, rc) && tx >= rc[0] && tx <= rc[2] && ty >= rc[1] && ty <= rc[3]) {
+      if (exact) {
+        int lo, hi;
+        exact_row_span(exact_tile_params(rec + i * 12), ty, rc[0], rc[2], lo, hi);
+        if (tx < lo || tx > hi) continue;
+      }
       cand.push_back((uint32_t)i);
+    }
   }
   std::stable_sort(cand.begin(), cand.end(), [&](uint32_t a, uint32_t b) {
     return f32_bits(rec[(uint64_t)a * 12 + 2]) < f32_bits(rec[(uint64_t)b * 12 + 2]);
@@ -490,6 +574,10 @@ uint64_t oracle_tile_list(uint64_t n, const float* rec, int width, int height, u
     vals[k] = cand[k];
   }
   return cand.size();
+}
+uint64_t oracle_tile_list(uint64_t n, const float* rec, int width, int height, uint32_t tile,
+                          uint64_t cap, uint64_t* keys, uint32_t* vals) {
+  return oracle_tile_list_ex(n, rec, width, height, tile, 0, cap, keys, vals);
 }
 
 // Oracle-R. mode 0 = brute force (every pixel visits every non-culled Gaussian in
@@ -522,18 +610,22 @@ void oracle_render(uint64_t n, const float* rec, int width, int height, const do
 
   // binned: per selected tile, the Gaussians whose rectangle contains it, in depth order
   std::vector<std::vector<uint32_t>> lists;
-  if (mode == 1) {
+  if (mode >= 1) {   // 1: binned by the P10 rectangle; 2: binned by the tiles that pass the P13 test (f-4)
     lists.resize(sel.size());
     std::vector<int32_t> slot((size_t)TX * TY, -1);
     for (size_t s = 0; s < sel.size(); ++s) slot[sel[s]] = (int32_t)s;
     for (uint32_t g : order) {
       int rc[4];
       if (!rect_of(rec + (uint64_t)g * 12, TX, TY, rc)) continue;
-      for (int ty = rc[1]; ty <= rc[3]; ++ty)
-        for (int tx = rc[0]; tx <= rc[2]; ++tx) {
+      const ExactTile e = exact_tile_params(rec + (uint64_t)g * 12);
+      for (int ty = rc[1]; ty <= rc[3]; ++ty) {
+        int lo = rc[0], hi = rc[2];
+        if (mode == 2) exact_row_span(e, ty, rc[0], rc[2], lo, hi);
+        for (int tx = lo; tx <= hi; ++tx) {
           const int32_t s = slot[(size_t)ty * TX + tx];
           if (s >= 0) lists[s].push_back(g);
         }
+      }
     }
   }
   uint64_t visited = 0, contributed = 0;
@@ -542,7 +634,7 @@ void oracle_render(uint64_t n, const float* rec, int width, int height, const do
     const int tx = (int)(sel[s] % TX), ty = (int)(sel[s] / TX);
     const uint32_t* cand = order.data();
     size_t ncand = order.size();
-    if (mode == 1) {
+    if (mode >= 1) {
       cand = lists[s].data();
       ncand = lists[s].size();
     }

@@ -906,3 +906,154 @@ class TestEndToEndAllowance:
                 swapped[0, 2], swapped[1, 2] = rows[1, 2], rows[0, 2]      # the other depth order
                 sw = oracle.render(swapped, 16, 16)
                 assert np.isclose(np.abs(sw["rgb"][:, 8, 8] - o["rgb"][:, 8, 8]).max(), 0.25)
+
+
+# ----------------------------------------------------------------------------- exact tile lists (f-4)
+class TestExactTiles:
+    """P13: only the tiles of a Gaussian's rectangle whose box of pixel centres its region
+    { alpha >= 1/255 } can reach are listed. Pinned against brute force in double on the fp32 record:
+    safety (no dropped tile has a pixel centre with alpha >= 1/255), kept subset of the rectangle, and tightness
+    (kept == 'the box intersects the region', by an independent box-minimum of the quadratic form)."""
+
+    @staticmethod
+    def _scenes():
+        out = []
+        for seed, scale, n in ((0, 1.0, 1500), (5, 4.0, 600), (7, 12.0, 300)):
+            wl = make_config(0, n=n, seed=seed)
+            s = wl.scene
+            sc = one_scene(mu=s.mu, quat=s.quat, scale=s.scale * scale, opacity=s.opacity, sh=s.sh, tau=s.tau, beta=s.beta, vel=s.vel)
+            out.append((sc, wl.cameras[0]))
+        # needles: one long axis, thin others, random orientations
+        rng = np.random.default_rng(3)
+        n = 400
+        mu = np.stack([rng.uniform(-3, 3, n), rng.uniform(-2, 2, n), rng.uniform(2, 12, n)], 1)
+        sc = one_scene(mu=mu, quat=rng.normal(size=(n, 4)), scale=np.stack([rng.uniform(0.5, 3, n), np.full(n, 0.01), np.full(n, 0.01)], 1),
+                       opacity=rng.uniform(0.004, 1.0, n))
+        out.append((sc, cam_simple(160, 112, 120.0)))
+        return out
+
+    @staticmethod
+    def _pairs(rec, W, H):
+        """(g, tile) pairs of the rectangle list and of the exact list, as sets of g * ntiles + tile."""
+        TX, TY = (W + 15) // 16, (H + 15) // 16
+        a = oracle.keys(rec, W, H, 0, exact=False)
+        b = oracle.keys(rec, W, H, 0, exact=True)
+        pa = a["vals_unsorted"].astype(np.int64) * (TX * TY) + (a["keys_unsorted"] >> np.uint64(32)).astype(np.int64)
+        pb = b["vals_unsorted"].astype(np.int64) * (TX * TY) + (b["keys_unsorted"] >> np.uint64(32)).astype(np.int64)
+        return pa, pb, TX, TY
+
+    @staticmethod
+    def _alpha_max_over_pixel_centres(rec, g, tile, TX, W, H):
+        r = rec[g].astype(np.float64)
+        tx, ty = tile % TX, tile // TX
+        xs = np.arange(tx * 16, min(tx * 16 + 16, W)) + 0.5
+        ys = np.arange(ty * 16, min(ty * 16 + 16, H)) + 0.5
+        dx, dy = np.meshgrid(r[0] - xs, r[1] - ys)
+        w = -0.5 * (r[4] * dx * dx + r[6] * dy * dy) - r[5] * dx * dy
+        return float((r[3] * np.exp(np.minimum(w, 0.0))).max())
+
+    def test_kept_is_a_subset_and_safe(self):
+        dropped_total = 0
+        for sc, cam in self._scenes():
+            _, rec = P(sc, cam, 0.37)
+            pa, pb, TX, TY = self._pairs(rec, cam.width, cam.height)
+            sa, sb = set(pa.tolist()), set(pb.tolist())
+            assert sb <= sa and len(pb) == len(sb)
+            _, c0, M0 = oracle.tile_counts(rec, cam.width, cam.height)
+            _, c1, M1 = oracle.tile_counts(rec, cam.width, cam.height, exact=True)
+            assert M1 == len(pb) and M0 == len(pa) and np.all(c1 <= c0)
+            # (a Gaussian whose region falls between the pixel centres of neighbouring tiles keeps no tile at all)
+            for pr in sa - sb:
+                g, tile = divmod(pr, TX * TY)
+                assert self._alpha_max_over_pixel_centres(rec, g, tile, TX, cam.width, cam.height) < 1.0 / 255.0, (g, tile)
+            dropped_total += len(sa - sb)
+        assert dropped_total > 500       # the pin bites: many pairs are dropped
+
+    def test_kept_equals_box_intersects_region(self):
+        """Independent characterisation: the minimum of q(d) = a dx^2 + 2 b dx dy + c dy^2 over the tile's box of pixel
+        centres (0 if the centre is inside, else the least over the four edges of the 1-D quadratic at its clamped
+        stationary point), against k = 2 ln(255 o~)."""
+        def qmin(r, x0, x1, y0, y1):
+            a, b, c = r[4], r[5], r[6]
+            dx0, dx1, dy0, dy1 = x0 - r[0], x1 - r[0], y0 - r[1], y1 - r[1]
+            if dx0 <= 0 <= dx1 and dy0 <= 0 <= dy1:
+                return 0.0
+            best = np.inf
+            for dx in (dx0, dx1):
+                dy = min(max(-b * dx / c, dy0), dy1)
+                best = min(best, a * dx * dx + 2 * b * dx * dy + c * dy * dy)
+            for dy in (dy0, dy1):
+                dx = min(max(-b * dy / a, dx0), dx1)
+                best = min(best, a * dx * dx + 2 * b * dx * dy + c * dy * dy)
+            return best
+        checked = fragile = 0
+        for sc, cam in self._scenes():
+            _, rec = P(sc, cam, 0.37)
+            pa, pb, TX, TY = self._pairs(rec, cam.width, cam.height)
+            sb = set(pb.tolist())
+            for pr in pa.tolist()[::3]:
+                g, tile = divmod(pr, TX * TY)
+                r = rec[g].astype(np.float64)
+                k = 2.0 * math.log(255.0 * r[3])
+                tx, ty = tile % TX, tile // TX
+                q = qmin(r, tx * 16 + 0.5, tx * 16 + 15.5, ty * 16 + 0.5, ty * 16 + 15.5)
+                # the fp32 test keeps a margin (k (1 + 2e-4) + 2e-5, 1e-3 px); pairs inside that band may go either way
+                if abs(q - k) <= 1e-3 * k + 1e-3 + 0.05 * math.sqrt(max(q, k) * max(r[4], r[6])):
+                    fragile += 1
+                    continue
+                assert (pr in sb) == (q <= k), (g, tile, q, k)
+                checked += 1
+        assert checked > 3000 and fragile < 0.05 * checked
+
+    def test_binned_by_exact_tiles_equals_brute_force(self):
+        """The image is the tile-free definition: compositing a pixel over the exact lists must equal compositing it
+        over ALL Gaussians, bit for bit in double."""
+        for sc, cam in self._scenes()[:2] + self._scenes()[3:]:
+            _, rec = P(sc, cam, 0.37)
+            a = oracle.render(rec, cam.width, cam.height, mode="brute")
+            b = oracle.render(rec, cam.width, cam.height, mode="binned_exact")
+            for k in ("rgb", "depth", "alpha"):
+                assert np.array_equal(a[k], b[k]), k
+            assert b["visited"] < oracle.render(rec, cam.width, cam.height, mode="binned")["visited"]
+
+    def test_lists_ranges_and_single_tile_lists_are_consistent(self):
+        sc, cam = self._scenes()[1]
+        _, rec = P(sc, cam, 0.37)
+        k = oracle.keys(rec, cam.width, cam.height, 1, exact=True)
+        assert np.all(np.diff(k["keys_sorted"].astype(np.int64)) >= 0)
+        TX, TY = (cam.width + 15) // 16, (cam.height + 15) // 16
+        for tile in (0, TX - 1, TX * TY // 2, TX * TY - 1):
+            kk, vv = oracle.tile_list(rec, cam.width, cam.height, tile, exact=True)
+            b, e = k["ranges"][tile]
+            assert np.array_equal(k["vals_sorted"][b:e], vv) and np.array_equal(k["keys_sorted"][b:e], kk)
+
+    def test_special_cases(self):
+        cam = cam_simple(128, 96, 100.0)
+        # a Gaussian covering the whole image keeps every tile; an isotropic blob keeps a disc, not its square
+        big = record_row(64.0, 48.0, 3.0, 0.9, 1e-6, 0.0, 1e-6, hx=float(np.sqrt(2 * math.log(255 * 0.9) / 1e-6)), hy=float(np.sqrt(2 * math.log(255 * 0.9) / 1e-6)))
+        _, c0, _ = oracle.tile_counts(big[None], 128, 96)
+        _, c1, _ = oracle.tile_counts(big[None], 128, 96, exact=True)
+        assert c0[0] == c1[0] == 48
+        sig = 12.0
+        kq = 2 * math.log(255 * 0.9)
+        blob = record_row(64.3, 47.8, 3.0, 0.9, 1 / sig ** 2, 0.0, 1 / sig ** 2, hx=float(sig * math.sqrt(kq)), hy=float(sig * math.sqrt(kq)))
+        _, c0, _ = oracle.tile_counts(blob[None], 128, 96)
+        _, c1, _ = oracle.tile_counts(blob[None], 128, 96, exact=True)
+        assert c1[0] < c0[0]                                  # the corners of the square go
+        # at the opacity cutoff (k ~ 0) the region is a point: the Gaussian keeps the tile of its centre
+        dot = record_row(40.2, 40.7, 3.0, (1 / 255) * (1 + 1e-6), 0.5, 0.1, 0.5, hx=1e-3, hy=1e-3)
+        _, c1, _ = oracle.tile_counts(dot[None], 128, 96, exact=True)
+        assert c1[0] == 1
+        # a degenerate conic (det <= 0, NaN) keeps the whole rectangle
+        for bad in (record_row(60, 40, 3, 0.5, 1e-3, 1e-2, 1e-3, hx=30, hy=30), record_row(60, 40, 3, 0.5, np.nan, 0.0, 1e-3, hx=30, hy=30)):
+            _, c0, _ = oracle.tile_counts(bad[None], 128, 96)
+            _, c1, _ = oracle.tile_counts(bad[None], 128, 96, exact=True)
+            assert c0[0] == c1[0] > 1
+
+    def test_reduction_on_an_urban_shaped_scene(self):
+        wl = make_config(2, n=20_000)
+        cam = wl.cameras[0]
+        _, rec = P(wl.scene, cam, 0.5)
+        _, _, M0 = oracle.tile_counts(rec, cam.width, cam.height)
+        _, _, M1 = oracle.tile_counts(rec, cam.width, cam.height, exact=True)
+        assert M1 < 0.8 * M0, (M0, M1)
