@@ -534,6 +534,19 @@ def run_ours(args):
                         for k, v in t1["kernels"].items()},
             "note": "PVG_OPT_LAZY_CHUNKS=0: full preprocess (records, SH), every block entry emitted and split, every tile list "
                     "written whole; same frames, same images bit for bit"}
+        # (1b) exact tile lists on top of the complete lists (PVG_OPT_EXACT_TILES; SURVEY 8(f-4) at list-build time)
+        scene.set_option(pvg.OPT_EXACT_TILES, 1)
+        warm_up(scene)
+        run1b = timed_frames(pvg, torch, dist, scene, sched, cams, out_by_cam, local_rank, dev, stride)
+        t1b = kernel_table(run1b, stride, N, S, False, hbm_peak, alu_peak)
+        legs["exact_tiles"] = {
+            "value": total_frames / run1b["elapsed_s"], "unit": UNIT, "ms_per_step": run1b["elapsed_s"] * 1e3 / args.steps,
+            "instances_rectangles": int(run1b["Ms"][-1]), "instances_exact": int(scene.frame_stats()["M_exact"]),
+            "stage_ms_per_frame": t1b["stage_ms"],
+            "kernels": {k: {"ms_per_frame": v["ms_per_frame"], "launches": v["launches"]} for k, v in t1b["kernels"].items()},
+            "note": "complete lists of only the tiles each Gaussian's ellipse can reach (P13): masks refined in bin_emit, tile "
+                    "counts counted, ranges rebuilt; images bit-identical. Compare with complete_lists (the rectangle lists)"}
+        scene.set_option(pvg.OPT_EXACT_TILES, 0)
         scene.set_option(pvg.OPT_LAZY_CHUNKS, args.lazy_chunks if args.lazy_chunks >= 0 else 2)
 
         # (2) a scene whose tiles do NOT saturate inside the list prefixes: opacity x 0.05 -> tiles park, the second

@@ -220,7 +220,18 @@ typedef enum pvg_option {
    *    (whole tiles of 4096), is formed and split by block before the first blend phase; a block's chunk counts for
    *    that phase only if all of its 512 entries exist. The entries behind the slab are formed only if a tile was
    *    parked (the launch checks the count on the device). 1: form all entries up front. */
-  PVG_OPT_LAZY_SLAB = 12
+  PVG_OPT_LAZY_SLAB = 12,
+  /* 1 (default 0), BLOCK_BINS mode: exact tile lists. A Gaussian's tile rectangle is the bounding box
+   *    of the region where its alpha can reach 1/255; towards the corners it holds tiles the region does not touch
+   *    (a quarter of all instances at config 3, half at config 4). With this option a Gaussian is listed only in the
+   *    tiles whose box of pixel centres the region can reach: every block entry's tile mask is refined by an fp32 test
+   *    taken with individually rounded operations (the oracle takes the same ones), the per-tile counts are counted
+   *    from the refined masks and the ranges rebuilt from them. A dropped (Gaussian, tile) pair contributes to no
+   *    pixel, so the images are bit-identical; counts, M, the sorted list and the ranges are those of the exact lists
+   *    (pvg_debug_view; no unsorted list in this mode). Implies complete lists and eager records (LAZY_CHUNKS is
+   *    ignored): with lazy lists the same test already runs inside the blend on the few entries a tile consumes
+   *    (BLEND_CULL), which is cheaper by two orders of magnitude -- this mode is for consumers of the lists themselves. */
+  PVG_OPT_EXACT_TILES = 13
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 
@@ -267,11 +278,12 @@ int pvg_kernel_times_ms(pvg_scene *scene, int cap, const char **names, int *stag
  * launch order, so that gaps and the overlap of the side stream are visible. Same return convention. */
 int pvg_kernel_timeline_ms(pvg_scene *scene, int cap, const char **names, float *start_ms, float *dur_ms);
 
-/* Sizes of the last render, no device work: out = {points n, tile instances M, tiles_x, tiles_y,
- * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries,
- * surviving Gaussians S (PRESORT_DEPTH=1, else 0), tiles the first blend phase of the lazy lists parked (LAZY_CHUNKS;
- * valid once the frame has completed on the stream)}. */
-int pvg_frame_stats(pvg_scene *scene, uint64_t out[8]);
+/* Sizes of the last render, no device work: out = {points n, tile instances M (of the rectangles), tiles_x, tiles_y,
+ * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries, 3 = block
+ * entries with exact tile lists, surviving Gaussians S (PRESORT_DEPTH=1, else 0), tiles the first blend phase of the
+ * lazy lists parked (LAZY_CHUNKS; valid once the frame has completed on the stream), instances of the exact lists
+ * (EXACT_TILES; valid once the frame has completed), 0}. */
+int pvg_frame_stats(pvg_scene *scene, uint64_t out[10]);
 
 /* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs
  * evaluated before the pixel stopped, out[1] = pairs that contributed (alpha >= 1/255). */

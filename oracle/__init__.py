@@ -118,6 +118,16 @@ def tile_counts(rec, width, height, exact: bool = False):
     return rects, counts, int(M)
 
 
+def tile_hist(rec, width, height, exact: bool = False) -> np.ndarray:
+    """List length of every tile [tiles] uint64 (row-major), from the per-Gaussian tile sets (no sort)."""
+    rec = np.ascontiguousarray(rec, dtype=np.float32)
+    n = rec.shape[0]
+    ntiles = ((width + 15) // 16) * ((height + 15) // 16)
+    out = np.zeros(ntiles, dtype=np.uint64)
+    lib().oracle_tile_hist_ex(C.c_uint64(n), _p(rec), C.c_int(width), C.c_int(height), C.c_int(1 if exact else 0), _p(out))
+    return out
+
+
 def keys(rec, width, height, order_mode=0, exact: bool = False):
     """Integer chain step 2 (offsets, unsorted list, std::stable_sort, ranges)."""
     rec = np.ascontiguousarray(rec, dtype=np.float32)

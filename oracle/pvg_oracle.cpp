@@ -154,8 +154,9 @@ inline ExactTile exact_tile_params(const float* r) {
   const float dyr = -((b / c) * dxm);
   const float ia = 1.0f / a;
   e.mx = r[0]; e.my = r[1]; e.a = a; e.b = b; e.det = det; e.akk = a * kk; e.dyr = dyr; e.ia = ia;
-  e.refine = (det > 0.0f) && (a > 0.0f) && (c > 0.0f) && std::isfinite(kk) && std::isfinite(dxm) && std::isfinite(ia) &&
-             std::isfinite(dyr) && (kk > 0.0f);
+  const float big = 3.0e38f;   // "finite" as the kernels test it: |x| <= 3e38 (false for NaN)
+  e.refine = (det > 0.0f) && (a > 0.0f) && (c > 0.0f) && (std::fabs(kk) <= big) && (std::fabs(dxm) <= big) &&
+             (std::fabs(ia) <= big) && (std::fabs(dyr) <= big) && (kk > 0.0f);
   return e;
 }
 // kept tiles [lo, hi] of tile row ty inside the rectangle's columns [tx0, tx1] (empty if lo > hi)
@@ -175,7 +176,7 @@ inline void exact_row_span(const ExactTile& e, int ty, int tx0, int tx1, int& lo
   const float xr = (std::sqrt(dr) - e.b * tr) * e.ia;
   const float xl = (-std::sqrt(dl) - e.b * tl) * e.ia;
   const float XR = (e.mx + xr) + 1e-3f, XL = (e.mx + xl) - 1e-3f;
-  if (!std::isfinite(XR) || !std::isfinite(XL)) return;
+  if (!(std::fabs(XR) <= 3.0e38f) || !(std::fabs(XL) <= 3.0e38f)) return;
   const float fh = std::floor((XR - 0.5f) * 0.0625f), fl = std::ceil((XL - 15.5f) * 0.0625f);
   // clamp in float before the conversion (|values| may exceed the int range)
   const int h = (int)std::fmin(std::fmax(fh, -2.0f), 1.0e6f), l = (int)std::fmin(std::fmax(fl, -2.0f), 1.0e6f);
@@ -473,6 +474,23 @@ uint64_t oracle_tile_counts_ex(uint64_t n, const float* rec, int width, int heig
     M += c;
   }
   return M;
+}
+// Per-tile list lengths (how many Gaussians list the tile), directly from the per-Gaussian tile sets: the ranges of the
+// sorted list are their exclusive scan in row-major tile order. For full-size checks, where the M instances cannot be
+// sorted in seconds.
+void oracle_tile_hist_ex(uint64_t n, const float* rec, int width, int height, int exact, uint64_t* per_tile) {
+  const int TX = (width + kTile - 1) / kTile, TY = (height + kTile - 1) / kTile;
+  for (int64_t t = 0; t < (int64_t)TX * TY; ++t) per_tile[t] = 0;
+  for (uint64_t i = 0; i < n; ++i) {
+    int rc[4];
+    if (!rect_of(rec + i * 12, TX, TY, rc)) continue;
+    const ExactTile e = exact_tile_params(rec + i * 12);
+    for (int ty = rc[1]; ty <= rc[3]; ++ty) {
+      int lo = rc[0], hi = rc[2];
+      if (exact) exact_row_span(e, ty, rc[0], rc[2], lo, hi);
+      for (int tx = lo; tx <= hi; ++tx) ++per_tile[(size_t)ty * TX + tx];
+    }
+  }
 }
 uint64_t oracle_tile_counts(uint64_t n, const float* rec, int width, int height, int32_t* rects, uint32_t* counts) {
   return oracle_tile_counts_ex(n, rec, width, height, 0, rects, counts);

@@ -67,6 +67,55 @@ __device__ __forceinline__ void bb_entry(uint32_t xy0, uint32_t xy1, uint32_t j,
   mask = ((uint64_t)rowmask * 0x0101010101010101ull) & rows;    // bit (ty & 7) * 8 + (tx & 7)
 }
 
+// P13: clears from an entry's mask the tiles of the block that the
+// Gaussian's region { alpha >= 1/255 } cannot reach. Per tile row the region's x-extent inside the band of pixel-centre
+// rows is an interval (the ellipse's right / left boundary at the dy of the band nearest to where it peaks); tiles whose
+// box of pixel centres misses it go. Integer work: every float operation is an individually rounded fp32 one
+// (__f*_rn: no contraction), in the order the oracle's exact_row_span takes them, so both sides decide identically.
+// r0 = (mx, my, z, o~), r1 = (a, b, c, hx) of the fp32 record.
+__device__ __noinline__ uint64_t bb_refine_mask(uint64_t mask, uint32_t bx, uint32_t by, float4 r0, float4 r1) {
+  const float a = r1.x, b = r1.y, c = r1.z, hx = r1.w;
+  const float det = __fsub_rn(__fmul_rn(a, c), __fmul_rn(b, b));
+  const float k = __fdiv_rn(__fmul_rn(__fmul_rn(hx, hx), det), c);
+  const float kk = __fadd_rn(__fmul_rn(k, 1.0002f), 2e-5f);
+  const float dxm = __fsqrt_rn(__fdiv_rn(__fmul_rn(kk, c), det));
+  const float dyr = -__fmul_rn(__fdiv_rn(b, c), dxm);
+  const float ia = __fdiv_rn(1.0f, a);
+  const float akk = __fmul_rn(a, kk);
+  const float big = 3.0e38f;
+  const bool refine = (det > 0.0f) && (a > 0.0f) && (c > 0.0f) && (fabsf(kk) <= big) && (fabsf(dxm) <= big) && (fabsf(ia) <= big) &&
+                      (fabsf(dyr) <= big) && (kk > 0.0f);
+  if (!refine) return mask;
+#pragma unroll 1
+  for (uint32_t ly = 0; ly < 8u; ++ly) {
+    const uint32_t row = (uint32_t)(mask >> (8u * ly)) & 0xFFu;
+    if (!row) continue;
+    const int ty = (int)(by * 8u + ly);
+    const float y0 = __fsub_rn(__fadd_rn((float)(16 * ty), 0.5f), r0.y), y1 = __fadd_rn(y0, 15.0f);
+    uint32_t keep = row;
+    if ((y0 > 0.0f && __fsub_rn(akk, __fmul_rn(__fmul_rn(det, y0), y0)) < 0.0f) ||
+        (y1 < 0.0f && __fsub_rn(akk, __fmul_rn(__fmul_rn(det, y1), y1)) < 0.0f)) {
+      keep = 0u;
+    } else {
+      const float tr = fminf(fmaxf(dyr, y0), y1), tl = fminf(fmaxf(-dyr, y0), y1);
+      const float dr = fmaxf(__fsub_rn(akk, __fmul_rn(__fmul_rn(det, tr), tr)), 0.0f);
+      const float dl = fmaxf(__fsub_rn(akk, __fmul_rn(__fmul_rn(det, tl), tl)), 0.0f);
+      const float xr = __fmul_rn(__fsub_rn(__fsqrt_rn(dr), __fmul_rn(b, tr)), ia);
+      const float xl = __fmul_rn(__fsub_rn(-__fsqrt_rn(dl), __fmul_rn(b, tl)), ia);
+      const float XR = __fadd_rn(__fadd_rn(r0.x, xr), 1e-3f), XL = __fsub_rn(__fadd_rn(r0.x, xl), 1e-3f);
+      if (fabsf(XR) <= big && fabsf(XL) <= big) {
+        const float fh = floorf(__fmul_rn(__fsub_rn(XR, 0.5f), 0.0625f)), fl = ceilf(__fmul_rn(__fsub_rn(XL, 15.5f), 0.0625f));
+        const int h = (int)fminf(fmaxf(fh, -2.0f), 1.0e6f), l = (int)fminf(fmaxf(fl, -2.0f), 1.0e6f);
+        // columns [l, h] of the image -> bits of this block's row
+        const int lo = max(l - (int)(bx * 8u), 0), hi = min(h - (int)(bx * 8u), 7);
+        keep = lo <= hi ? (row & (((2u << hi) - 1u) & ~((1u << lo) - 1u))) : 0u;
+      }
+    }
+    mask &= ~((uint64_t)(row & ~keep) << (8u * ly));
+  }
+  return mask;
+}
+
 // One CTA owns BE_CHUNK consecutive entries. The owners of the chunk are staged in shared
 // memory, each marks its first entry, and a max-scan spreads the owner slot over the chunk
 // (same scheme as expand.cuh). keys/visit: the depth-sorted (rect | depth, Gaussian) pairs;
@@ -251,13 +300,14 @@ struct BinEmitSmem {
   };
 };
 
-template <int BITS>
+template <int BITS, bool EXACT>
 __global__ void __launch_bounds__(BP_THREADS, PVG_BP_MINB)
 bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
                 const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x,
                 uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, const uint32_t* __restrict__ bin_start,
                 uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket,
-                const uint32_t* __restrict__ only_if /* nullptr, or: do nothing when *only_if == 0 */) {
+                const uint32_t* __restrict__ only_if /* nullptr, or: do nothing when *only_if == 0 */,
+                const float4* __restrict__ record /* EXACT (exact tile lists): every mask is refined by P13 */) {
   using Core = RadixCore<BP_THREADS, BP_ITEMS, BITS>;
   constexpr uint32_t MASK = (1u << BITS) - 1u;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -356,6 +406,14 @@ bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, 
         g[j] = visit[r];
       }
     }
+  }
+  if (EXACT) {
+#pragma unroll
+    for (int j = 0; j < BP_ITEMS; ++j)
+      if (mk[j]) {
+        const float4 r0 = __ldg(record + 3 * (size_t)g[j]), r1 = __ldg(record + 3 * (size_t)g[j] + 1);
+        mk[j] = bb_refine_mask(mk[j], dp[j] % blocks_x, dp[j] / blocks_x, r0, r1);
+      }
   }
   __syncthreads();   // the owner table is dead: s.b reuses it
   Core::rank(s.core, tile, dp, bin_start, lookback);
@@ -505,6 +563,70 @@ __device__ __forceinline__ void bin_write_tiles(const uint32_t (&m)[BB_CHUNK / 3
       }
     }
   }
+}
+
+// ---- exact tile lists (P13): per-tile and per-Gaussian counts of the refined masks, then the ranges ----------------
+// With refined masks a tile's count is no longer the number of rectangles over it (tilebin.cuh's difference array):
+// it is counted. A warp owns (chunk, half of the block's tiles) exactly as in bin_write_kernel below: the counts per tile
+// come from the bit-matrix transpose + popcount, one atomicAdd per (chunk, tile); each lane also adds its entries'
+// popcounts to its Gaussians' exact counts. Integer adds commute: deterministic.
+__global__ void __launch_bounds__(BW_THREADS, 4)
+exact_count_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
+                   const uint32_t* __restrict__ chunk_start, uint32_t tiles_x, uint32_t tiles_y, uint32_t blocks_x,
+                   uint32_t* __restrict__ ticket, uint32_t* __restrict__ tile_count /* [tiles], zeroed */,
+                   uint32_t* __restrict__ gauss_count /* [n], zeroed */) {
+  __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
+  BinWalk w;
+  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w, 0u, 0xFFFFFFFFu, nullptr)) return;
+  const uint32_t lane = threadIdx.x & 31u;
+  constexpr int NB = BB_CHUNK / 32;
+  const uint32_t* mp = reinterpret_cast<const uint32_t*>(masks) + w.half;   // this half's 32 mask bits
+  uint32_t cnt = 0;
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    const uint32_t e = w.e0 + b * 32 + lane;
+    const bool ok = e < w.e1;
+    const uint32_t m = ok ? __ldcs(mp + 2 * (size_t)e) : 0u;
+    if (m) atomicAdd(gauss_count + __ldcs(gs + e), (uint32_t)__popc(m));
+    cnt += __popc(transpose32(m, lane));
+  }
+  const uint32_t ltile = w.half * 32u + lane;
+  const uint32_t tx = (w.bin % blocks_x) * 8u + (ltile & 7u), ty = (w.bin / blocks_x) * 8u + (ltile >> 3);
+  if (cnt && tx < tiles_x && ty < tiles_y) atomicAdd(tile_count + ty * tiles_x + tx, cnt);
+}
+
+// ranges[tile] = exclusive scan of the exact counts in row-major tile order; one CTA. total -> totals[0] (device) and
+// totals_host[7] (mapped).
+__global__ void __launch_bounds__(1024)
+exact_ranges_kernel(const uint32_t* __restrict__ tile_count, uint32_t tiles, uint2* __restrict__ ranges,
+                    uint64_t* __restrict__ total_dev, volatile uint64_t* __restrict__ totals_host) {
+  __shared__ uint64_t s_part[32];
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t per = (tiles + 1023u) / 1024u;
+  const uint32_t t0 = min(tiles, tid * per), t1 = min(tiles, t0 + per);
+  uint64_t sum = 0;
+  for (uint32_t t = t0; t < t1; ++t) sum += tile_count[t];
+  uint64_t incl = sum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint64_t v = __shfl_up_sync(0xffffffffu, incl, d);
+    if (lane >= d) incl += v;
+  }
+  if (lane == 31) s_part[warp] = incl;
+  __syncthreads();
+  uint64_t wex = 0, all = 0;
+  for (uint32_t wv = 0; wv < 32; ++wv) {
+    const uint64_t v = s_part[wv];
+    if (wv < warp) wex += v;
+    all += v;
+  }
+  uint64_t run = wex + incl - sum;
+  for (uint32_t t = t0; t < t1; ++t) {
+    const uint32_t c = tile_count[t];
+    ranges[t] = make_uint2((uint32_t)run, (uint32_t)(run + c));
+    run += c;
+  }
+  if (tid == 0) { *total_dev = all; totals_host[7] = all; }
 }
 
 // status[chunk][64]: 64-bit look-back words (flag | position), zeroed. A chunk first counts, per tile,

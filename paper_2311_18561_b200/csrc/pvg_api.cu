@@ -437,6 +437,9 @@ struct pvg_scene {
   int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
   int lazy_chunks = 2;                // PVG_OPT_LAZY_CHUNKS (0: always write the complete lists)
   int lazy_slab = 8;                  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front
+  int exact_tiles = 0;                // PVG_OPT_EXACT_TILES: list a Gaussian only in the tiles its ellipse can reach (P13)
+  bool exact_used = false;            // the last frame built exact lists
+  Buf tile_count, counts_exact;       // exact lists: per-tile and per-Gaussian counts of the refined masks
   uint32_t emit_first = 0, emit_tiles = 0, emit_radix = 256;   // bin_emit tiles in the first launch / in all; its look-back row length
   const uint32_t* visit_last = nullptr;
   bool visit_tail_done = false;       // pvg_debug_view has appended the culled Gaussians to the visiting order
@@ -503,7 +506,7 @@ void release_all(pvg_scene* s) {
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->lazy_state, &s->unf, &s->dhist, &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
-                 &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->tile_count, &s->counts_exact, &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
@@ -669,7 +672,8 @@ int prep_scan(pvg_scene* s, cudaStream_t zs) {
 }
 
 // nv: the first nv visiting positions are scanned (the survivors after the depth sort; n otherwise)
-int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm, bool scratch_ready = false) {
+int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm, bool scratch_ready = false,
+             const uint32_t* counts = nullptr /* default: the rectangle counts */) {
   cudaStream_t st = s->stream;
   const uint32_t n = nv;
   if (n == 0) return PVG_OK;
@@ -686,7 +690,7 @@ int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32
                                                                   visit, out, total, s->scan_status.as<uint64_t>(), ticket,
                                                                   s->chunk_owner.as<uint32_t>(), kOwnerChunk);
   else
-    scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), nullptr, visit, out, total,
+    scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, counts ? counts : s->counts.as<uint32_t>(), nullptr, visit, out, total,
                                                                    s->scan_status.as<uint64_t>(), ticket, nullptr, 0u);
   if (tm) TRY(tm->end(st));
   return PVG_OK;
@@ -706,11 +710,19 @@ int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64
 template <int BITS>
 int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t blocks_x, const uint32_t* bin_start,
                     uint64_t* lookback, uint32_t* ticket, uint32_t grid, const uint32_t* only_if) {
-  auto kern = bin_emit_kernel<BITS>;
-  PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
-  kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
-      s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
-      blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if);
+  if (s->exact_used) {
+    auto kern = bin_emit_kernel<BITS, true>;
+    PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
+    kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
+        s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
+        blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, s->record.as<float4>());
+  } else {
+    auto kern = bin_emit_kernel<BITS, false>;
+    PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
+    kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
+        s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
+        blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, nullptr);
+  }
   return PVG_OK;
 }
 
@@ -737,9 +749,16 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
   TRY(s->sort_m.lookback.reserve((size_t)pass_tiles * OS_RADIX * 8, st, 1.25));
   TRY(s->sort_m.tickets.reserve((size_t)OS_MAX_PASSES * 4, st));
   TRY(s->chunk_owner.reserve(((size_t)Mb / kOwnerChunk + 2) * 4, st, 1.125));
-  CU(cudaMemsetAsync(s->sort_m.tickets.p, 0, 16, zs));   // emit, write (round 0), write (round 1), write (completion)
+  CU(cudaMemsetAsync(s->sort_m.tickets.p, 0, 32, zs));   // emit, write (round 0), write (round 1), write (completion), exact count
+  if (s->exact_used) {
+    const size_t tiles = (size_t)P.tiles_x * P.tiles_y;
+    TRY(s->tile_count.reserve(tiles * 4, st));
+    TRY(s->counts_exact.reserve((size_t)s->n * 4, st));
+    CU(cudaMemsetAsync(s->tile_count.p, 0, tiles * 4, zs));
+    CU(cudaMemsetAsync(s->counts_exact.p, 0, (size_t)s->n * 4, zs));
+  }
   CU(cudaMemsetAsync(s->chunk_cnt.p, 0, (size_t)max_chunks * 64 * 8, zs));
-  if (s->lazy_chunks > 0) {
+  if (s->lazy_chunks > 0 && !s->exact_used) {
     const size_t tiles = (size_t)P.tiles_x * P.tiles_y;
     TRY(s->unf.reserve(kUnfHead + tiles * 8, st));
     TRY(s->lazy_state.reserve((size_t)5 * P.width * P.height * 4, st));
@@ -822,7 +841,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 #if PVG_BIN_FUSED
   // lazy lists: only the first slab of the entries (in depth order) is formed now; render_impl emits the rest if
   // the first blend phase parks a tile
-  s->lazy_used = s->lazy_chunks > 0;
+  s->lazy_used = s->lazy_chunks > 0 && !s->exact_used;   // exact lists are counted: every entry is formed and refined
   const uint32_t emit_tiles = (Mb + BF_TILE - 1) / BF_TILE;
   s->emit_first = s->lazy_used ? std::min(emit_tiles, std::max(1u, (emit_tiles + (uint32_t)s->lazy_slab - 1) / (uint32_t)s->lazy_slab)) : emit_tiles;
   s->emit_tiles = emit_tiles;
@@ -843,6 +862,23 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(tm->begin("bin_emit", PVG_STAGE_SORT, st));
   TRY(run_bin_emit(s, P, visit, s->emit_first, nullptr));
   TRY(tm->end(st));
+  if (s->exact_used) {
+    // exact lists: the masks are refined, so the tile counts are counted (not taken from the rectangles) and the
+    // ranges rebuilt from them before the lists are written
+    const uint32_t nb = blocks_x * bb_blocks(P.tiles_y);
+    const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nb;
+    uint32_t* bin_start = s->bin_tables.as<uint32_t>();
+    TRY(tm->begin("exact_count", PVG_STAGE_RANGES, st));
+    exact_count_kernel<<<(max_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA, BW_THREADS, 0, st>>>(
+        s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, bin_start + 257, (uint32_t)P.tiles_x, (uint32_t)P.tiles_y,
+        blocks_x, s->sort_m.tickets.as<uint32_t>() + 4, s->tile_count.as<uint32_t>(), s->counts_exact.as<uint32_t>());
+    TRY(tm->end(st));
+    TRY(tm->begin("exact_ranges", PVG_STAGE_RANGES, st));
+    exact_ranges_kernel<<<1, 1024, 0, st>>>(s->tile_count.as<uint32_t>(), (uint32_t)P.tiles_x * (uint32_t)P.tiles_y,
+                                            s->ranges.as<uint2>(), reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 40),
+                                            s->d_total);
+    TRY(tm->end(st));
+  }
 #else
   TRY(tm->begin("bin_expand", PVG_STAGE_DUPLICATE, st));
   bin_expand_kernel<<<(Mb + BE_CHUNK - 1) / BE_CHUNK, BE_THREADS, 0, st>>>(
@@ -865,7 +901,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   // the tile lists: all of them, or (lazy) only as far as the first lazy_chunks chunks of every block reach --
   // render_impl runs the second round after the first blend phase
 #if !PVG_BIN_FUSED
-  s->lazy_used = s->lazy_chunks > 0;
+  s->lazy_used = s->lazy_chunks > 0 && !s->exact_used;
   s->emit_first = s->emit_tiles = 0;
 #endif
   s->lists_complete = !s->lazy_used;
@@ -936,7 +972,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
   // lazy lists: the records (conic, colour: 48 B written, 192 B of SH read per survivor) are left to shade_kernel,
   // which forms them for the Gaussians in front only -- unless a tile parks
-  s->light = block && s->lazy_chunks > 0 && PVG_BIN_FUSED;
+  s->exact_used = block && s->exact_tiles && PVG_BIN_FUSED;
+  s->light = block && s->lazy_chunks > 0 && PVG_BIN_FUSED && !s->exact_used;
   s->records_complete = !s->light;
   {
     const unsigned pgrid = (n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS);
@@ -1252,7 +1289,7 @@ int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
   s->dev = scene->dev;
   s->presort = scene->presort; s->keep_unsorted = scene->keep_unsorted; s->count_pairs = scene->count_pairs;
   s->compact = scene->compact; s->block = scene->block; s->blend_cull = scene->blend_cull;
-  s->lazy_chunks = scene->lazy_chunks; s->lazy_slab = scene->lazy_slab;
+  s->lazy_chunks = scene->lazy_chunks; s->lazy_slab = scene->lazy_slab; s->exact_tiles = scene->exact_tiles;
   s->band_begin = scene->band_begin; s->band_end = scene->band_end;
   s->timer.enabled = scene->timer.enabled; s->timer.accumulate = scene->timer.accumulate; s->timer.stride = scene->timer.stride;
   s->model = scene->model;
@@ -1322,6 +1359,7 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
       if (value < 1 || value > 4096) return PVG_ERR_BAD_OPTION;
       scene->lazy_slab = (int)value;
       return PVG_OK;
+    case PVG_OPT_EXACT_TILES: scene->exact_tiles = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_TILE_ROW_BEGIN:
       if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
       scene->band_begin = (int)value;
@@ -1465,12 +1503,13 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     // the block path never forms per-instance offsets or the unsorted list: produce them here
     cudaStream_t st = s->stream;
     const uint32_t* visit = s->dvals[s->visit_side].as<uint32_t>();
-    TRY(run_scan(s, s->n, false, s->offsets.as<uint32_t>(), visit, nullptr));
+    TRY(run_scan(s, s->n, false, s->offsets.as<uint32_t>(), visit, nullptr, false,
+                 s->exact_used ? s->counts_exact.as<uint32_t>() : nullptr));
     if (s->M) {
       TRY(s->keys[0].reserve((size_t)s->M * 8, st));
       keys_from_ranges_kernel<<<s->tiles_x * s->tiles_y, 256, 0, st>>>(s->ranges.as<uint2>(), s->vals[0].as<uint32_t>(),
                                                                         s->tileinfo.as<uint4>(), s->keys[0].as<uint64_t>());
-      if (s->keep_unsorted_used) {
+      if (s->keep_unsorted_used && !s->exact_used) {   // (the exact lists have no unsorted form: their masks are refined after the split)
         TRY(s->keys_unsorted.reserve((size_t)s->M * 8, st));
         TRY(s->vals_unsorted.reserve((size_t)s->M * 4, st));
         expand_kernel<false><<<(unsigned)((s->M + EXP_CHUNK - 1) / EXP_CHUNK), EXP_THREADS, 0, st>>>(
@@ -1498,7 +1537,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(st));
   }
-  if (s->keep_unsorted_used && s->M) {
+  if (s->keep_unsorted_used && s->M && !s->exact_used) {
     out->keys_unsorted = s->keys_unsorted.as<uint64_t>();
     out->vals_unsorted = s->vals_unsorted.as<uint32_t>();
   }
@@ -1507,6 +1546,10 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
     out->vals_sorted = s->vals[s->sorted_side].as<uint32_t>();
   }
   out->ranges = s->ranges.as<uint32_t>();
+  if (s->exact_used) {   // the exact lists: their own counts and total (the stream was synchronised above)
+    out->counts = s->counts_exact.as<uint32_t>();
+    out->num_instances = s->M ? s->h_total[7] : 0;
+  }
   return PVG_OK;
 }
 
@@ -1561,18 +1604,22 @@ int pvg_stage_times_ms(pvg_scene* s, float ms[PVG_NUM_STAGES]) {
   return PVG_OK;
 }
 
-int pvg_frame_stats(pvg_scene* s, uint64_t out[8]) {
+int pvg_frame_stats(pvg_scene* s, uint64_t out[10]) {
   if (!s || !out) return PVG_ERR_NULL;
   out[0] = s->n;
   out[1] = s->rendered ? s->M : 0;
   out[2] = s->tiles_x;
   out[3] = s->tiles_y;
   out[4] = s->rendered ? s->Mb : 0;
-  out[5] = s->block_used ? 2 : (s->compact_used ? 1 : 0);
+  out[5] = s->block_used ? (s->exact_used ? 3 : 2) : (s->compact_used ? 1 : 0);
   out[6] = (s->rendered && s->presort_used) ? s->survivors : 0;
   // tiles the lazy lists' first blend phase parked (stored by the second phase through mapped host memory: it is
   // the last frame's figure once that frame has completed on the stream; the word is only read here)
   out[7] = (s->rendered && s->block_used && s->lazy_used && s->M) ? s->h_total[3] : 0;
+  // exact lists: the instances actually listed (stored by exact_ranges_kernel through mapped host memory: the last
+  // frame's figure once that frame has completed on the stream)
+  out[8] = (s->rendered && s->exact_used && s->M) ? s->h_total[7] : 0;
+  out[9] = 0;
   return PVG_OK;
 }
 

@@ -165,20 +165,22 @@ def check_record(gpu_rec: np.ndarray, wide: np.ndarray, cam, scene):
     return stats
 
 
-def check_integer_chain(dbg: dict, width: int, height: int, presort: bool):
-    """(I): bit-exact. dbg = Scene.debug() of a render with KEEP_UNSORTED=1."""
+def check_integer_chain(dbg: dict, width: int, height: int, presort: bool, exact: bool = False):
+    """(I): bit-exact. dbg = Scene.debug() of a render with KEEP_UNSORTED=1. exact: the exact tile lists (P13,
+    PVG_OPT_EXACT_TILES): counts, offsets, sorted list and ranges of the refined tile sets; no unsorted list."""
     rec = dbg["record"]
-    rects, counts, M = oracle.tile_counts(rec, width, height)
+    rects, counts, M = oracle.tile_counts(rec, width, height, exact)
     assert dbg["M"] == M, (dbg["M"], M)
     assert np.array_equal(dbg["counts"], counts), "per-Gaussian tile counts"
-    k = oracle.keys(rec, width, height, 1 if presort else 0)
+    k = oracle.keys(rec, width, height, 1 if presort else 0, exact=exact)
     n = rec.shape[0]
     if presort:
         visit = dbg["visit_order"]
         # survivors come first in (z bits, index) order; the culled tail is in index order
-        surv = np.nonzero(counts)[0]
+        rect_counts = oracle.tile_counts(rec, width, height)[1] if exact else counts   # survival is decided by the rectangle
+        surv = np.nonzero(rect_counts)[0]
         exp = surv[np.lexsort((surv, rec[surv, 2].view(np.uint32)))]
-        culled = np.nonzero(counts == 0)[0]
+        culled = np.nonzero(rect_counts == 0)[0]
         assert np.array_equal(visit, np.concatenate([exp, culled]).astype(np.uint32)), "depth visit order"
         off_by_g = np.empty(n, dtype=np.uint64)
         off_by_g[visit] = dbg["offsets"].astype(np.uint64)

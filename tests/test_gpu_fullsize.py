@@ -154,3 +154,44 @@ def test_cfg4_full_size_all_cameras_and_timestamps():
                 assert st["M"] > 100_000_000, (cam.name, t)
     finally:
         sc.close()
+
+
+def test_cfg3_full_size_exact_tile_lists():
+    """SURVEY 8(f-4) at full size (config 3, frame 24, PVG_OPT_EXACT_TILES): the images equal the default mode's bit for
+    bit; the per-Gaussian counts of ALL Gaussians, M, EVERY tile range and the sorted lists of sampled tiles are bit-exact
+    against the oracle's exact lists (P13); M falls by at least a quarter."""
+    import torch
+    wl = make_config(3)
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    try:
+        cam, t = list(wl.frames())[24]
+        ref = [x.clone() for x in sc.render(cam, t)]
+        M_rect = sc.frame_stats()["M"]
+        sc.set_option(pvg.OPT_EXACT_TILES, 1)
+        out = sc.render(cam, t)
+        assert all(torch.equal(a, b) for a, b in zip(ref, out)), "EXACT_TILES changed the image"
+        d = sc.debug_info()
+        n, M = int(d.n), int(d.num_instances)
+        TX, TY = int(d.tiles_x), int(d.tiles_y)
+        W, H = cam.width, cam.height
+        assert sc.frame_stats()["list_mode"] == "blocks_exact" and sc.frame_stats()["M_exact"] == M
+        grec = _d2h(sc, d.record, 0, (n, 12), np.float32)
+        gcounts = _d2h(sc, d.counts, 0, (n,), np.uint32)
+        granges = _d2h(sc, d.ranges, 0, (TX * TY, 2), np.uint32)
+        _, counts_o, M_o = oracle.tile_counts(grec, W, H, exact=True)
+        assert M == M_o and np.array_equal(gcounts, counts_o)
+        assert M <= 0.75 * M_rect, (M, M_rect)
+        per_tile = oracle.tile_hist(grec, W, H, exact=True)
+        end = per_tile.cumsum()
+        assert np.array_equal(granges, np.stack([end - per_tile, end], 1).astype(np.uint32)), "tile ranges"
+        rng = np.random.default_rng(1)
+        sel = sorted({0, TX - 1, (TY - 1) * TX, TX * TY - 1, (TY // 2) * TX + TX // 2, int(per_tile.argmax())} |
+                     set(int(x) for x in rng.choice(np.nonzero(per_tile)[0], size=8, replace=False)))
+        for tl in sel:
+            b, e = int(granges[tl, 0]), int(granges[tl, 1])
+            gv = _d2h(sc, d.vals_sorted, 4 * b, (e - b,), np.uint32)
+            _, v_o = oracle.tile_list(grec, W, H, tl, exact=True)
+            assert np.array_equal(gv, v_o), f"sorted list of tile {tl}"
+        print(json.dumps(dict(M_rect=M_rect, M_exact=M, ratio=M / M_rect, tiles=len(sel))))
+    finally:
+        sc.close()

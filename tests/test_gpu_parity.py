@@ -597,3 +597,37 @@ def test_depth_sort_key_range(znear, top_pass):
     if znear == 50.0:
         assert sc.frame_stats()["survivors"] < 0.5 * wl.scene.n
     sc.close()
+
+
+@pytest.mark.parametrize("cfg,n,cam_i", [(0, None, 0), (1, None, 0), (2, 30_000, 0), (4, 30_000, 1), (4, 30_000, 4)])
+def test_exact_tile_lists(cfg, n, cam_i):
+    """SURVEY 8(f-4) at list-build time (PVG_OPT_EXACT_TILES): every block entry's mask is refined by the ellipse-versus-
+    tile test P13; counts, M, visiting order, offsets, the sorted list and the ranges are bit-exact against the
+    oracle's exact lists; the images do not change by one bit (a dropped pair contributes to no pixel)."""
+    import torch
+    wl = make_config(cfg, n=n)
+    cam = wl.cameras[cam_i]
+    sc = pvg.Scene.from_workload_scene(wl.scene)
+    ref = [x.clone() for x in sc.render(cam, 0.25)]
+    M_rect = sc.frame_stats()["M"]
+    sc.set_option(pvg.OPT_EXACT_TILES, 1)
+    sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
+    out = sc.render(cam, 0.25)
+    torch.cuda.synchronize()
+    fs = sc.frame_stats()
+    assert fs["list_mode"] == "blocks_exact" and fs["M"] == M_rect
+    for a, b in zip(ref, out):
+        assert torch.equal(a, b)
+    dbg = sc.debug()
+    st = check_integer_chain(dbg, cam.width, cam.height, True, exact=True)
+    assert dbg["keys_unsorted"] is None
+    assert st["M"] == fs["M_exact"] < M_rect
+    print(cfg, cam_i, "M", M_rect, "->", st["M"], f"({st['M'] / M_rect:.3f})")
+    # back to the rectangle lists
+    sc.set_option(pvg.OPT_EXACT_TILES, 0)
+    again = sc.render(cam, 0.25)
+    for a, b in zip(ref, again):
+        assert torch.equal(a, b)
+    assert sc.frame_stats()["list_mode"] == "blocks"
+    check_integer_chain(sc.debug(), cam.width, cam.height, True)
+    sc.close()
