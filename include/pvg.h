@@ -304,6 +304,13 @@ int pvg_sort_pairs(uint64_t n, uint64_t *keys_in, uint32_t *vals_in, uint64_t *k
  *   counted once). sm_count (may be NULL) receives cudaDevAttrMultiProcessorCount. Synchronises `cuda_stream`. */
 int pvg_calibrate_fp32(int mode, void *cuda_stream, double *thread_instr_per_s, int *sm_count);
 
+/* Test hook: guard bands. After pvg_guard_bands(1) every device allocation the library makes (model, workspace) carries
+ * 4096 bytes of a known pattern in front and behind; pvg_check_guards synchronises the device and reports how many live
+ * allocations have a damaged band (a kernel wrote out of bounds) and how many were checked. A stand-in for
+ * compute-sanitizer's memcheck where that tool is not available; off by default, process-wide. */
+int pvg_guard_bands(int enable);
+int pvg_check_guards(uint64_t *damaged_allocations, uint64_t *checked_allocations);
+
 /* Debug helper so that bindings need no CUDA runtime of their own: synchronous copy of `bytes`
  * from a device pointer (e.g. a pvg_debug view) into host memory. */
 int pvg_memcpy_d2h(void *host_dst, const void *device_src, size_t bytes);

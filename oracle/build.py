@@ -13,6 +13,10 @@ LIB = os.path.join(HERE, "libpvg_oracle.so")
 
 
 def build(force: bool = False) -> str:
+    """PVG_ORACLE_LIB names an alternative library to load instead (the sanitizer build below)."""
+    alt = os.environ.get("PVG_ORACLE_LIB")
+    if alt:
+        return alt
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB
@@ -24,5 +28,22 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+def build_sanitized(out: str) -> str:
+    """AddressSanitizer + UndefinedBehaviorSanitizer build of the oracle. Run the CPU pins on it:
+        python -m oracle.build sanitize /tmp/libpvg_oracle_asan.so
+        LD_PRELOAD=$(g++ -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 PVG_ORACLE_LIB=/tmp/libpvg_oracle_asan.so \
+            python -m pytest tests/test_oracle_pins.py tests/test_oracle_golden.py -q
+    (the interpreter is not instrumented, so the runtime is preloaded and leak checking, which would report CPython's
+    own allocations, is off)."""
+    cmd = ["g++", "-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+           "-ffp-contract=off", "-fopenmp", "-std=c++17", "-shared", "-fPIC", "-Wall", "-Wextra", "-o", out, SRC]
+    subprocess.run(cmd, check=True)
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force=True))
+    import sys
+    if len(sys.argv) == 3 and sys.argv[1] == "sanitize":
+        print(build_sanitized(sys.argv[2]))
+    else:
+        print(build(force=True))

@@ -30,7 +30,7 @@ NUM_STAGES = len(STAGES)
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
            "pvg_render_host_async", "pvg_wait_host", "pvg_render_state", "pvg_set_sky",
            "pvg_destroy", "pvg_fork_scene", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms", "pvg_kernel_timeline_ms",
-           "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_calibrate_fp32", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
+           "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_calibrate_fp32", "pvg_guard_bands", "pvg_check_guards", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
 
 class PvgError(RuntimeError):
@@ -108,6 +108,8 @@ def load_library(path: Optional[str] = None):
     L.pvg_memcpy_d2h.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
     L.pvg_set_allocator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.pvg_calibrate_fp32.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    L.pvg_guard_bands.argtypes = [C.c_int]
+    L.pvg_check_guards.argtypes = [C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     if path is None:
         _lib = L
     return L
@@ -425,3 +427,15 @@ def calibrate_fp32(mode: int = 1):
     rate, sms = C.c_double(0.0), C.c_int(0)
     _check(L.pvg_calibrate_fp32(int(mode), torch.cuda.current_stream().cuda_stream, C.byref(rate), C.byref(sms)))
     return float(rate.value), int(sms.value)
+
+
+def guard_bands(enable: bool = True) -> None:
+    """Test hook (include/pvg.h pvg_guard_bands): allocations made from now on carry guard bands."""
+    _check(load_library().pvg_guard_bands(1 if enable else 0))
+
+
+def check_guards():
+    """(damaged, checked) live guarded allocations (include/pvg.h pvg_check_guards)."""
+    bad, n = C.c_uint64(0), C.c_uint64(0)
+    _check(load_library().pvg_check_guards(C.byref(bad), C.byref(n)))
+    return int(bad.value), int(n.value)

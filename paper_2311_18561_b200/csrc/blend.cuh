@@ -479,6 +479,8 @@ blend_kernel(const __grid_constant__ FrameParams P, const uint2* __restrict__ ra
              float* __restrict__ out_rgb, float* __restrict__ out_depth, float* __restrict__ out_alpha,
              unsigned long long* __restrict__ counters, const float* __restrict__ featw,
              const __grid_constant__ BlendLazy Z) {
+  pdl_launch_dependents();
+  pdl_wait();
   if (PHASE != 2) {
     // one CTA per tile; only the band's tiles are launched
     blend_tile<COUNT, MODE, PHASE>(P, blockIdx.x + (uint32_t)P.band_y0 * (uint32_t)P.tiles_x, ranges, vals, record, out_rgb,

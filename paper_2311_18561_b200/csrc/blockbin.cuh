@@ -308,6 +308,8 @@ bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, 
                 uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket,
                 const uint32_t* __restrict__ only_if /* nullptr, or: do nothing when *only_if == 0 */,
                 const float4* __restrict__ record /* EXACT (exact tile lists): every mask is refined by P13 */) {
+  pdl_launch_dependents();
+  pdl_wait();
   using Core = RadixCore<BP_THREADS, BP_ITEMS, BITS>;
   constexpr uint32_t MASK = (1u << BITS) - 1u;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -642,6 +644,8 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
                  const uint32_t* __restrict__ want_count /* with want_mask: nothing to do at all if 0 */,
                  uint32_t* __restrict__ lim /* [tiles] or nullptr: where each tile's list stands after this round */,
                  const uint64_t* __restrict__ avail /* [blocks] or nullptr: entries emitted so far (bin_round0_chunks) */) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
   // the base pointer round-trips through shared memory so that it lives in registers; taken from the
   // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)

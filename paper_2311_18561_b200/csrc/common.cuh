@@ -61,6 +61,14 @@ __device__ __forceinline__ uint32_t lanemask_lt() {
   return r;
 }
 
+// Programmatic dependent launch (sm_90+): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may
+// start -- its CTAs become resident and run up to pdl_wait() -- while the kernel before it in the stream is still
+// draining; pdl_wait() returns when that kernel has completed and its writes are visible. pdl_launch_dependents()
+// lets the NEXT kernel of the stream do the same with respect to this one. Both are no-ops in a plain launch.
+// Every kernel of a chain waits before its first global read (transitively, everything earlier has then completed).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // 64-bit status words of the decoupled look-back (flag in the top 2 bits, value
 // below): one aligned 64-bit access carries flag and payload together, so relaxed
 // gpu-scope accesses are sufficient.

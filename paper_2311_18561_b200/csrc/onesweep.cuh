@@ -387,6 +387,8 @@ depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, 
                   uint32_t* __restrict__ vals_b, uint32_t n /* pairs in buffer a (FIRST) */, int pass, int shift,
                   const DepthCtl* __restrict__ ctl, const uint32_t* __restrict__ hist_excl /* [512] this pass */,
                   uint64_t* __restrict__ lookback /* [tiles][1 << BITS], zeroed */, uint32_t* __restrict__ ticket /* zeroed */) {
+  pdl_launch_dependents();
+  pdl_wait();
   using Core = RadixCore<THREADS, ITEMS, BITS>;
   constexpr int TILE = Core::TILE;
   constexpr uint32_t MASK = (1u << BITS) - 1u;

@@ -421,6 +421,8 @@ __global__ void __launch_bounds__(256)
 shade_all_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint32_t* __restrict__ counts, const uint32_t* __restrict__ only_if,
                  const float4* __restrict__ A0, const float4* __restrict__ A1, const float4* __restrict__ A2,
                  const float4* __restrict__ A3, const float4* __restrict__ SH, float4* __restrict__ record, float* __restrict__ featw) {
+  pdl_launch_dependents();
+  pdl_wait();
   if (only_if && *only_if == 0u) return;
   const uint32_t i = blockIdx.x * 256u + threadIdx.x;
   if (i >= n) return;

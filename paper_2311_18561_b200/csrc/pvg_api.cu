@@ -6,6 +6,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -77,8 +79,16 @@ struct Dev {
   }
 };
 
-void* dev_alloc(size_t bytes, cudaStream_t st) {
-  if (bytes == 0) bytes = 256;
+// Guard bands (pvg_guard_bands / pvg_check_guards; a test hook: compute-sanitizer is not available on every pool): every
+// device allocation of the library gets kGuard bytes of a known pattern in front and behind; a kernel that writes out
+// of bounds of a workspace buffer by less than that damages a band, which pvg_check_guards finds.
+constexpr size_t kGuard = 4096;
+constexpr int kGuardByte = 0xA5;
+std::atomic<bool> g_guards{false};
+std::mutex g_guard_mu;
+std::map<void*, size_t> g_guarded;   // user pointer -> user bytes
+
+void* raw_alloc(size_t bytes, cudaStream_t st) {
   if (g_alloc) return g_alloc(bytes, (void*)st, g_alloc_user);
   void* p = nullptr;
   if (cudaMalloc(&p, bytes) != cudaSuccess) {
@@ -87,10 +97,36 @@ void* dev_alloc(size_t bytes, cudaStream_t st) {
   }
   return p;
 }
-void dev_free(void* p) {
-  if (!p) return;
+void raw_free(void* p) {
   if (g_free) g_free(p, g_alloc_user);
   else cudaFree(p);
+}
+void* dev_alloc(size_t bytes, cudaStream_t st) {
+  if (bytes == 0) bytes = 256;
+  if (!g_guards.load()) return raw_alloc(bytes, st);
+  bytes = (bytes + 255) & ~(size_t)255;
+  unsigned char* base = static_cast<unsigned char*>(raw_alloc(bytes + 2 * kGuard, st));
+  if (!base) return nullptr;
+  if (cudaMemset(base, kGuardByte, kGuard) != cudaSuccess || cudaMemset(base + kGuard + bytes, kGuardByte, kGuard) != cudaSuccess) {
+    cudaGetLastError();
+    raw_free(base);
+    return nullptr;
+  }
+  std::lock_guard<std::mutex> lk(g_guard_mu);
+  g_guarded[base + kGuard] = bytes;
+  return base + kGuard;
+}
+void dev_free(void* p) {
+  if (!p) return;
+  {
+    std::lock_guard<std::mutex> lk(g_guard_mu);
+    auto it = g_guarded.find(p);
+    if (it != g_guarded.end()) {
+      g_guarded.erase(it);
+      p = static_cast<unsigned char*>(p) - kGuard;
+    }
+  }
+  raw_free(p);
 }
 
 // growable device buffer
@@ -181,11 +217,16 @@ struct Timer {
   // stream (a wait on another stream, a memset, a copy) must call cut() so that it is not billed to a kernel.
   cudaStream_t chain_stream = nullptr;
   cudaEvent_t chain_event = nullptr;
-  void cut() { chain_event = nullptr; }
+  // programmatic dependent launch: the last operation enqueued on pdl_stream was a kernel of the chain (launch_chain);
+  // anything else -- a memset, an event, a wait, a copy: whatever calls cut(), or an event record of this timer -- breaks it
+  cudaStream_t pdl_stream = nullptr;
+  bool pdl_open = false;
+  void cut() { chain_event = nullptr; pdl_open = false; }
   void reset() { recs.clear(); used = 0; cut(); }
   int begin(const char* name, int stage, cudaStream_t st) {
     if (!frame_on) return PVG_OK;
     KernelRec r{name, stage, nullptr, nullptr};
+    pdl_open = false;
     if (chain_event && chain_stream == st) {
       r.e0 = chain_event;
     } else {
@@ -199,6 +240,7 @@ struct Timer {
   int end(cudaStream_t st) {
     if (!frame_on) return PVG_OK;
     CU(cudaEventRecord(recs.back().e1, st));
+    pdl_open = false;
     chain_stream = st;
     chain_event = recs.back().e1;
     return PVG_OK;
@@ -210,6 +252,26 @@ struct Timer {
     used = 0;
   }
 };
+
+// Launch of a kernel of the frame's main chain (they all begin with pdl_launch_dependents(); pdl_wait();): as a
+// programmatic dependent of the previous kernel when that one was the last thing enqueued on the stream, so that its
+// launch latency and its CTAs' start overlap the previous kernel's tail (PVG_PDL=0: always plain launches).
+#ifndef PVG_PDL
+#define PVG_PDL 1
+#endif
+template <class... KArgs, class... Args>
+int launch_chain(Timer* tm, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = (PVG_PDL && tm && tm->pdl_open && tm->pdl_stream == st) ? 1 : 0;
+  CU(cudaLaunchKernelEx(&cfg, kern, KArgs(args)...));
+  if (tm) { tm->pdl_open = true; tm->pdl_stream = st; }
+  return PVG_OK;
+}
 
 template <class Cfg, int BITS, int HI>
 int launch_pass_bits(const uint64_t* kin, const uint32_t* vin, uint64_t* kout, uint32_t* vout, uint32_t n, int shift,
@@ -323,12 +385,12 @@ int prep_depth_sort(uint32_t n, cudaStream_t alloc_st, cudaStream_t zs, SortScra
 
 template <int BITS, bool FIRST>
 int launch_depth_pass(uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, uint32_t n, int pass, const DepthCtl* ctl,
-                      const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev) {
+                      const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev, Timer* tm) {
   using Smem = OnesweepSmem<DsCfg::THREADS, DsCfg::ITEMS, BITS>;
   auto kern = depth_pass_kernel<DsCfg::THREADS, DsCfg::ITEMS, BITS, DsCfg::MINB, FIRST>;
   PVG_ENSURE_SMEM(kern, sizeof(Smem), dev);
-  kern<<<(n + kDsTile - 1) / kDsTile, DsCfg::THREADS, sizeof(Smem), st>>>(ka, va, kb, vb, n, pass, ds_shift(pass), ctl, hist, lookback, ticket);
-  return PVG_OK;
+  return launch_chain(tm, kern, dim3((n + kDsTile - 1) / kDsTile), dim3(DsCfg::THREADS), sizeof(Smem), st, ka, va, kb, vb, n, pass,
+                      ds_shift(pass), ctl, hist, lookback, ticket);
 }
 
 // dh: this frame's dhist half (exclusive digit prefixes + DepthCtl, written by preprocess). Every pass is launched
@@ -345,9 +407,9 @@ int run_depth_sort(const Dev& dv, uint32_t n, uint64_t* ka, uint32_t* va, uint64
   for (int p = p0; p < p1; ++p) {
     if (tm) TRY(tm->begin("onesweep_pass", PVG_STAGE_DEPTH_SORT, st));
     const uint32_t* hist = dh + p * DS_RADIX;
-    if (p == 0) TRY((launch_depth_pass<DS_BITS, true>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal)));
-    else if (p < 3) TRY((launch_depth_pass<DS_BITS, false>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal)));
-    else TRY((launch_depth_pass<DS_TOP_BITS, false>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal)));
+    if (p == 0) TRY((launch_depth_pass<DS_BITS, true>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal, tm)));
+    else if (p < 3) TRY((launch_depth_pass<DS_BITS, false>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal, tm)));
+    else TRY((launch_depth_pass<DS_TOP_BITS, false>(ka, va, kb, vb, n, p, ctl, hist, lb, tk + p, st, dv.ordinal, tm)));
     if (tm) TRY(tm->end(st));
     lb += tiles * (size_t)(1 << ds_bits(p));
   }
@@ -686,12 +748,13 @@ int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32
   uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
   if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
   if (blocks)
-    scan_counts_kernel<true><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, s->counts.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(),
-                                                                  visit, out, total, s->scan_status.as<uint64_t>(), ticket,
-                                                                  s->chunk_owner.as<uint32_t>(), kOwnerChunk);
+    TRY(launch_chain(tm, scan_counts_kernel<true>, dim3(scan_tiles), dim3(SCAN_THREADS), 0, st, n, s->counts.as<uint32_t>(),
+                     s->dkeys[s->visit_side].as<uint64_t>(), visit, out, total, s->scan_status.as<uint64_t>(), ticket,
+                     s->chunk_owner.as<uint32_t>(), kOwnerChunk));
   else
-    scan_counts_kernel<false><<<scan_tiles, SCAN_THREADS, 0, st>>>(n, counts ? counts : s->counts.as<uint32_t>(), nullptr, visit, out, total,
-                                                                   s->scan_status.as<uint64_t>(), ticket, nullptr, 0u);
+    TRY(launch_chain(tm, scan_counts_kernel<false>, dim3(scan_tiles), dim3(SCAN_THREADS), 0, st, n,
+                     counts ? counts : s->counts.as<uint32_t>(), (const uint64_t*)nullptr, visit, out, total,
+                     s->scan_status.as<uint64_t>(), ticket, (uint32_t*)nullptr, 0u));
   if (tm) TRY(tm->end(st));
   return PVG_OK;
 }
@@ -713,15 +776,15 @@ int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t b
   if (s->exact_used) {
     auto kern = bin_emit_kernel<BITS, true>;
     PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
-    kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
-        s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
-        blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, s->record.as<float4>());
+    TRY(launch_chain(&s->timer, kern, dim3(grid), dim3(BP_THREADS), sizeof(BinEmitSmem<BITS>), s->stream,
+                     s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
+                     blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, s->record.as<float4>()));
   } else {
     auto kern = bin_emit_kernel<BITS, false>;
     PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
-    kern<<<grid, BP_THREADS, sizeof(BinEmitSmem<BITS>), s->stream>>>(
-        s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
-        blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, nullptr);
+    TRY(launch_chain(&s->timer, kern, dim3(grid), dim3(BP_THREADS), sizeof(BinEmitSmem<BITS>), s->stream,
+                     s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
+                     blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, (const float4*)nullptr));
   }
   return PVG_OK;
 }
@@ -800,10 +863,9 @@ int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const ui
 // every Gaussian's record, in index order (zeros for the culled ones)
 int run_shade_all(pvg_scene* s, const FrameParams& P, const uint32_t* only_if) {
   const Model* m = s->model;
-  shade_all_kernel<<<(s->n + 255) / 256, 256, 0, s->stream>>>(P, s->n, s->counts.as<uint32_t>(), only_if, m->A0.as<float4>(),
-                                                               m->A1.as<float4>(), m->A2.as<float4>(), m->A3.as<float4>(),
-                                                               m->SH.as<float4>(), s->record.as<float4>(), s->featw_last);
-  return PVG_OK;
+  return launch_chain(&s->timer, shade_all_kernel, dim3((s->n + 255) / 256), dim3(256), 0, s->stream, P, s->n, s->counts.as<uint32_t>(),
+                      only_if, m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
+                      s->record.as<float4>(), s->featw_last);
 }
 
 // bin_write over the chunks kin_lo <= kin < kin_hi of every block; only_unfinished: the tiles the first blend
@@ -815,15 +877,14 @@ int launch_bin_write(pvg_scene* s, const FrameParams& P, uint32_t kin_lo, uint32
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
   const uint32_t launch_chunks = (kin_lo == 0 && kin_hi < (1u << 30)) ? std::min<uint64_t>((uint64_t)nbins * kin_hi, 0x7FFFFFFFull) : max_chunks;
   const unsigned grid = (launch_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
-  bin_write_kernel<<<grid, BW_THREADS, 0, s->stream>>>(
+  return launch_chain(&s->timer, bin_write_kernel, dim3(grid), dim3(BW_THREADS), 0, s->stream,
       s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, bin_start + 257, s->ranges.as<uint2>(), (uint32_t)P.tiles_x,
       (uint32_t)P.tiles_y, blocks_x, s->chunk_cnt.as<uint64_t>(), s->sort_m.tickets.as<uint32_t>() + ticket_slot,
-      s->vals[0].as<uint32_t>(), kin_lo, kin_hi, only_unfinished ? s->unf.as<unsigned long long>() : nullptr,
+      s->vals[0].as<uint32_t>(), kin_lo, kin_hi, only_unfinished ? s->unf.as<unsigned long long>() : (unsigned long long*)nullptr,
       reinterpret_cast<const uint32_t*>(s->unf.as<unsigned char>() + 2048),
-      (kin_lo == 0 && kin_hi < (1u << 30)) ? reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) : nullptr,
+      (kin_lo == 0 && kin_hi < (1u << 30)) ? reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) : (uint32_t*)nullptr,
       (s->lazy_used && s->emit_first && s->emit_first < s->emit_tiles)
-          ? s->sort_m.lookback.as<uint64_t>() + (size_t)(s->emit_first - 1) * s->emit_radix : nullptr);
-  return PVG_OK;
+          ? s->sort_m.lookback.as<uint64_t>() + (size_t)(s->emit_first - 1) * s->emit_radix : (uint64_t*)nullptr);
 }
 
 // a2 + a3 (instance part) through 8x8-tile block entries (blockbin.cuh), after prep_block_bins: the sorted value
@@ -925,6 +986,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   DeviceGuard guard(s->dev.ordinal);
   cudaStream_t st = s->stream;
   Timer& tm = s->timer;
+  tm.cut();
   s->presort_used = s->presort; s->keep_unsorted_used = s->keep_unsorted; s->lazy_chunks_used = s->lazy_chunks;
   tm.next_frame();
   if (!tm.accumulate) { if (tm.frame_on) tm.reset(); } else tm.cut();
@@ -1163,7 +1225,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       Z.parked_host = s->d_total + 3;
       Z.blocks_x = bb_blocks(P.tiles_x);
     }
-#define PVG_BLEND(C, M, PH) blend_kernel<C, M, PH><<<(PH) == 2 ? std::min(band_tiles, (uint32_t)s->dev.sms * 8u) : band_tiles, BLEND_THREADS, 0, st>>>(P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, featw, Z)
+#define PVG_BLEND(C, M, PH) TRY(launch_chain(&tm, blend_kernel<C, M, PH>, dim3((PH) == 2 ? std::min(band_tiles, (uint32_t)s->dev.sms * 8u) : band_tiles), dim3(BLEND_THREADS), 0, st, P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, (const float*)featw, Z))
 #define PVG_BLEND_ALL(PH)                                        \
     if (s->count_pairs) {                                        \
       if (mode == BLEND_FEATURE) PVG_BLEND(true, BLEND_FEATURE, PH); \
@@ -1449,6 +1511,7 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   memset(out, 0, sizeof(*out));
   if (!s->rendered) return PVG_OK;
   DeviceGuard guard(s->dev.ordinal);
+  s->timer.cut();
   out->n = s->n;
   out->num_instances = s->M;
   out->tiles_x = s->tiles_x;
@@ -1665,6 +1728,31 @@ int pvg_calibrate_fp32(int mode, void* cuda_stream, double* thread_instr_per_s, 
   cudaFree(sink);
   if (rc == PVG_OK) *thread_instr_per_s = best > 0.f ? calib_instructions(mode, grid, trips) / ((double)best * 1e-3) : 0.0;
   return rc;
+}
+
+int pvg_guard_bands(int enable) {
+  g_guards.store(enable != 0);
+  return PVG_OK;
+}
+
+int pvg_check_guards(uint64_t* damaged_allocations, uint64_t* checked_allocations) {
+  CU(cudaDeviceSynchronize());
+  std::lock_guard<std::mutex> lk(g_guard_mu);
+  std::vector<unsigned char> h(kGuard);
+  uint64_t bad = 0;
+  for (const auto& kv : g_guarded) {
+    const unsigned char* user = static_cast<const unsigned char*>(kv.first);
+    bool ok = true;
+    for (int side = 0; side < 2 && ok; ++side) {
+      CU(cudaMemcpy(h.data(), side ? user + kv.second : user - kGuard, kGuard, cudaMemcpyDeviceToHost));
+      for (size_t i = 0; i < kGuard; ++i)
+        if (h[i] != (unsigned char)kGuardByte) { ok = false; break; }
+    }
+    if (!ok) ++bad;
+  }
+  if (damaged_allocations) *damaged_allocations = bad;
+  if (checked_allocations) *checked_allocations = g_guarded.size();
+  return PVG_OK;
 }
 
 int pvg_memcpy_d2h(void* host_dst, const void* device_src, size_t bytes) {

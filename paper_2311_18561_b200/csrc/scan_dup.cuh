@@ -45,6 +45,8 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
                    uint32_t* __restrict__ offsets, uint64_t* __restrict__ total,
                    uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
                    uint32_t* __restrict__ chunk_owner, uint32_t chunk) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ uint32_t s_tile;
   __shared__ uint64_t s_warp[SCAN_THREADS / 32];
   __shared__ uint64_t s_prefix;
