@@ -424,13 +424,14 @@ shade_all_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint32
   pdl_launch_dependents();
   pdl_wait();
   if (only_if && *only_if == 0u) return;
-  const uint32_t i = blockIdx.x * 256u + threadIdx.x;
-  if (i >= n) return;
-  if (counts[i] == 0u) {
-    record[3 * (size_t)i] = record[3 * (size_t)i + 1] = record[3 * (size_t)i + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
-    return;
+  // grid-stride: the launch that finds nothing to do (no tile parked) should cost a few hundred CTAs, not n / 256
+  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
+    if (counts[i] == 0u) {
+      record[3 * (size_t)i] = record[3 * (size_t)i + 1] = record[3 * (size_t)i + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+      continue;
+    }
+    preprocess_point<PRE_REC>(P, n, i, nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
   }
-  preprocess_point<PRE_REC>(P, n, i, nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
 }
 
 // One-off re-layout of the caller's arrays into the SoA float4 model (pvg_create_scene).

@@ -863,7 +863,8 @@ int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const ui
 // every Gaussian's record, in index order (zeros for the culled ones)
 int run_shade_all(pvg_scene* s, const FrameParams& P, const uint32_t* only_if) {
   const Model* m = s->model;
-  return launch_chain(&s->timer, shade_all_kernel, dim3((s->n + 255) / 256), dim3(256), 0, s->stream, P, s->n, s->counts.as<uint32_t>(),
+  const unsigned grid = std::min<unsigned>((s->n + 255) / 256, (unsigned)s->dev.sms * 8u);
+  return launch_chain(&s->timer, shade_all_kernel, dim3(grid), dim3(256), 0, s->stream, P, s->n, s->counts.as<uint32_t>(),
                       only_if, m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
                       s->record.as<float4>(), s->featw_last);
 }
