@@ -300,25 +300,18 @@ struct BinEmitSmem {
   };
 };
 
+// One tile of BF_TILE entries (the next ticket). Returns false, doing nothing, when the ticket is at or beyond
+// tile_end (tile_end != 0 only in a launch whose CTAs loop over tickets).
 template <int BITS, bool EXACT>
-__global__ void __launch_bounds__(BP_THREADS, PVG_BP_MINB)
-bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
-                const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x,
-                uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, const uint32_t* __restrict__ bin_start,
-                uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket,
-                const uint32_t* __restrict__ only_if /* nullptr, or: do nothing when *only_if == 0 */,
-                const float4* __restrict__ record /* EXACT (exact tile lists): every mask is refined by P13 */) {
-  pdl_launch_dependents();
-  pdl_wait();
+__device__ __forceinline__ bool
+bin_emit_tile(BinEmitSmem<BITS>& s, uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
+              const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x,
+              uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, const uint32_t* __restrict__ bin_start,
+              uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket, const float4* __restrict__ record, uint32_t tile_end) {
   using Core = RadixCore<BP_THREADS, BP_ITEMS, BITS>;
   constexpr uint32_t MASK = (1u << BITS) - 1u;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  BinEmitSmem<BITS>& s = *reinterpret_cast<BinEmitSmem<BITS>*>(smem_raw);
-  // lazy lists: the launch that emits the entries behind the first slab runs only if a tile was parked. The
-  // tiles are handed out by the ticket, which simply goes on counting from the first launch.
-  if (only_if && *only_if == 0u) return;
-
   const uint32_t tile = Core::take_ticket(s.core, ticket);
+  if (tile_end && tile >= tile_end) return false;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t i0 = tile * BF_TILE;
   const uint32_t tile_n = min((uint32_t)BF_TILE, Mb - i0);
@@ -431,6 +424,34 @@ bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, 
     g_out[o] = s.b.g[p];
     mask_out[o] = s.b.mask[p];
   }
+  return true;
+}
+
+// tile_end == 0: one tile per CTA (the grid is the number of tiles of the launch). tile_end != 0: the CTAs loop over
+// tickets until they reach tile_end -- the second-round launch of the lazy lists, which usually finds nothing to do
+// (*only_if == 0) and should then cost a few hundred CTAs, not thousands.
+template <int BITS, bool EXACT>
+__global__ void __launch_bounds__(BP_THREADS, PVG_BP_MINB)
+bin_emit_kernel(uint32_t n, uint32_t Mb, const uint32_t* __restrict__ boffsets, const uint32_t* __restrict__ chunk_owner,
+                const uint64_t* __restrict__ keys, const uint32_t* __restrict__ visit, uint32_t blocks_x,
+                uint32_t* __restrict__ g_out, uint64_t* __restrict__ mask_out, const uint32_t* __restrict__ bin_start,
+                uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket,
+                const uint32_t* __restrict__ only_if /* nullptr, or: do nothing when *only_if == 0 */,
+                const float4* __restrict__ record /* EXACT (exact tile lists): every mask is refined by P13 */,
+                uint32_t tile_end) {
+  pdl_launch_dependents();
+  pdl_wait();
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  BinEmitSmem<BITS>& s = *reinterpret_cast<BinEmitSmem<BITS>*>(smem_raw);
+  // lazy lists: the launch that emits the entries behind the first slab runs only if a tile was parked. The
+  // tiles are handed out by the ticket, which simply goes on counting from the first launch.
+  if (only_if && *only_if == 0u) return;
+  do {
+    if (!bin_emit_tile<BITS, EXACT>(s, n, Mb, boffsets, chunk_owner, keys, visit, blocks_x, g_out, mask_out, bin_start, lookback,
+                                    ticket, record, tile_end))
+      return;
+    __syncthreads();   // the next tile reuses the shared memory
+  } while (tile_end);
 }
 
 // ---- 3./4. the walks over a block's entries --------------------------------------------------
@@ -635,31 +656,26 @@ exact_ranges_kernel(const uint32_t* __restrict__ tile_count, uint32_t tiles, uin
 // how many of its entries cover it (bit-matrix transpose + popcount), publishes the counts, resolves
 // where it starts in every tile list by looking back over the earlier chunks of its block (the block's
 // first chunk starts at the tile's range begin), and then writes.
-__global__ void __launch_bounds__(BW_THREADS, 4)
-bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
+// One ticket's BW_CHUNKS_PER_CTA chunks. *past_end (block-uniform): the ticket lies beyond the launch's last chunk.
+__device__ __forceinline__ void
+bin_write_ticket(uint32_t* s_cs, uint32_t* const* s_vals, ulonglong2 (*s_ptr)[32 * BW_PTR_ROW], bool* past_end,
+                 const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
                  const uint32_t* __restrict__ chunk_start, const uint2* __restrict__ ranges, uint32_t tiles_x,
                  uint32_t tiles_y, uint32_t blocks_x, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
-                 uint32_t* __restrict__ vals, uint32_t kin_lo, uint32_t kin_hi,
-                 const unsigned long long* __restrict__ want_mask /* [blocks] tiles still wanted, or nullptr: all */,
-                 const uint32_t* __restrict__ want_count /* with want_mask: nothing to do at all if 0 */,
-                 uint32_t* __restrict__ lim /* [tiles] or nullptr: where each tile's list stands after this round */,
-                 const uint64_t* __restrict__ avail /* [blocks] or nullptr: entries emitted so far (bin_round0_chunks) */) {
-  pdl_launch_dependents();
-  pdl_wait();
-  __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
-  // the base pointer round-trips through shared memory so that it lives in registers; taken from the
-  // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
-  __shared__ uint32_t* s_vals;
-  __shared__ ulonglong2 s_ptr[BW_THREADS / 32][32 * BW_PTR_ROW];
-  if (want_mask && *want_count == 0u) return;   // lazy lists: no tile was parked
-  if (threadIdx.x == 0) s_vals = vals;
+                 uint32_t kin_lo, uint32_t kin_hi, const unsigned long long* __restrict__ want_mask, uint32_t* __restrict__ lim,
+                 const uint64_t* __restrict__ avail) {
   BinWalk w;
-  if (!bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w, kin_lo, kin_hi, avail)) return;   // (contains the barrier)
+  const bool mine = bin_walk_setup(bin_start, chunk_start, s_cs, ticket, w, kin_lo, kin_hi, avail);   // (contains the barrier)
+  {
+    const uint32_t first = s_cs[BB_MAX_BINS + 1] * BW_CHUNKS_PER_CTA;
+    *past_end = (kin_lo == 0 && kin_hi < (1u << 30)) ? first / kin_hi >= (uint32_t)BB_MAX_BINS : first >= s_cs[BB_MAX_BINS];
+  }
+  if (!mine) return;
   // lazy lists, second round: only the tiles the blend has not finished; a block without any is skipped by all of
   // its chunks alike (the mask is fixed for the whole launch), so nobody waits for a skipped chunk's look-back word
   const uint32_t want = want_mask ? (uint32_t)(want_mask[w.bin] >> (32u * w.half)) : 0xFFFFFFFFu;
   if (want_mask && want_mask[w.bin] == 0ull) return;
-  uint32_t* const vp = s_vals;
+  uint32_t* const vp = *s_vals;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t lt = lanemask_lt();
   constexpr int NB = BB_CHUNK / 32;
@@ -739,6 +755,38 @@ bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ m
   const uint32_t nb = (w.e1 - w.e0 + 31u) >> 5;
   if (nb == NB) bin_write_tiles<true>(m, g, sp, nb, lt, want);
   else bin_write_tiles<false>(m, g, sp, nb, lt, want);
+}
+
+// loop == 0: one ticket per CTA (the grid covers the launch's chunks). loop != 0: the CTAs loop over tickets to the
+// launch's last chunk -- the second round of the lazy lists, which usually finds nothing to do (*want_count == 0) and
+// should then cost a few hundred CTAs. Tickets are taken in order by running CTAs, so a chunk still only ever waits
+// (look-back) on chunks that are done or being worked on.
+__global__ void __launch_bounds__(BW_THREADS, 4)
+bin_write_kernel(const uint32_t* __restrict__ gs, const uint64_t* __restrict__ masks, const uint32_t* __restrict__ bin_start,
+                 const uint32_t* __restrict__ chunk_start, const uint2* __restrict__ ranges, uint32_t tiles_x,
+                 uint32_t tiles_y, uint32_t blocks_x, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
+                 uint32_t* __restrict__ vals, uint32_t kin_lo, uint32_t kin_hi,
+                 const unsigned long long* __restrict__ want_mask /* [blocks] tiles still wanted, or nullptr: all */,
+                 const uint32_t* __restrict__ want_count /* with want_mask: nothing to do at all if 0 */,
+                 uint32_t* __restrict__ lim /* [tiles] or nullptr: where each tile's list stands after this round */,
+                 const uint64_t* __restrict__ avail /* [blocks] or nullptr: entries emitted so far (bin_round0_chunks) */,
+                 uint32_t loop) {
+  pdl_launch_dependents();
+  pdl_wait();
+  __shared__ uint32_t s_cs[BB_MAX_BINS + 2];
+  // the base pointer round-trips through shared memory so that it lives in registers; taken from the
+  // kernel parameter it is re-read from the constant bank before every store (one more instruction per step)
+  __shared__ uint32_t* s_vals;
+  __shared__ ulonglong2 s_ptr[BW_THREADS / 32][32 * BW_PTR_ROW];
+  if (want_mask && *want_count == 0u) return;   // lazy lists: no tile was parked
+  if (threadIdx.x == 0) s_vals = vals;
+  do {
+    bool past_end;
+    bin_write_ticket(s_cs, &s_vals, s_ptr, &past_end, gs, masks, bin_start, chunk_start, ranges, tiles_x, tiles_y, blocks_x, status,
+                     ticket, kin_lo, kin_hi, want_mask, lim, avail);
+    if (past_end) return;   // block-uniform
+    __syncthreads();        // the next ticket's setup rewrites s_cs
+  } while (loop);
 }
 
 }  // namespace pvg

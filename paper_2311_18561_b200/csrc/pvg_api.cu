@@ -772,19 +772,19 @@ int launch_bin_pass(pvg_scene* s, uint32_t Mb, const uint32_t* bin_start, uint64
 
 template <int BITS>
 int launch_bin_emit(pvg_scene* s, uint32_t Mb, const uint32_t* visit, uint32_t blocks_x, const uint32_t* bin_start,
-                    uint64_t* lookback, uint32_t* ticket, uint32_t grid, const uint32_t* only_if) {
+                    uint64_t* lookback, uint32_t* ticket, uint32_t grid, const uint32_t* only_if, uint32_t tile_end) {
   if (s->exact_used) {
     auto kern = bin_emit_kernel<BITS, true>;
     PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
     TRY(launch_chain(&s->timer, kern, dim3(grid), dim3(BP_THREADS), sizeof(BinEmitSmem<BITS>), s->stream,
                      s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
-                     blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, s->record.as<float4>()));
+                     blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, s->record.as<float4>(), tile_end));
   } else {
     auto kern = bin_emit_kernel<BITS, false>;
     PVG_ENSURE_SMEM(kern, sizeof(BinEmitSmem<BITS>), s->dev.ordinal);
     TRY(launch_chain(&s->timer, kern, dim3(grid), dim3(BP_THREADS), sizeof(BinEmitSmem<BITS>), s->stream,
                      s->nv, Mb, s->boffsets.as<uint32_t>(), s->chunk_owner.as<uint32_t>(), s->dkeys[s->visit_side].as<uint64_t>(), visit,
-                     blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, (const float4*)nullptr));
+                     blocks_x, s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, lookback, ticket, only_if, (const float4*)nullptr, tile_end));
   }
   return PVG_OK;
 }
@@ -833,13 +833,16 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
 
 #if PVG_BIN_FUSED
 // bin_emit over the next `grid` tiles of 4096 entries (the ticket goes on counting across launches)
-int run_bin_emit(pvg_scene* s, const FrameParams& P, const uint32_t* visit, uint32_t grid, const uint32_t* only_if) {
+// loop: the CTAs of the launch loop over tickets up to the last tile (a grid of at most two CTAs per SM)
+int run_bin_emit(pvg_scene* s, const FrameParams& P, const uint32_t* visit, uint32_t grid, const uint32_t* only_if, bool loop = false) {
+  const uint32_t tile_end = loop ? s->emit_tiles : 0u;
+  if (loop) grid = std::min(grid, (uint32_t)s->dev.sms * (uint32_t)PVG_BP_MINB);
   const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();
   uint32_t* ticket = s->sort_m.tickets.as<uint32_t>();
   int rc = PVG_ERR_BAD_OPTION;
   switch (std::max(1, ceil_log2(nbins))) {
-#define PVG_CASE(B) case B: rc = launch_bin_emit<B>(s, (uint32_t)s->Mb, visit, blocks_x, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket, grid, only_if); break;
+#define PVG_CASE(B) case B: rc = launch_bin_emit<B>(s, (uint32_t)s->Mb, visit, blocks_x, bin_start, s->sort_m.lookback.as<uint64_t>(), ticket, grid, only_if, tile_end); break;
     PVG_CASE(1) PVG_CASE(2) PVG_CASE(3) PVG_CASE(4) PVG_CASE(5) PVG_CASE(6) PVG_CASE(7) PVG_CASE(8)
 #undef PVG_CASE
     default: break;
@@ -861,10 +864,11 @@ int run_shade(pvg_scene* s, const FrameParams& P, const uint32_t* r_lo, const ui
 }
 
 // every Gaussian's record, in index order (zeros for the culled ones)
-int run_shade_all(pvg_scene* s, const FrameParams& P, const uint32_t* only_if) {
+int run_shade_all(pvg_scene* s, const FrameParams& P, const uint32_t* only_if, cudaStream_t on = nullptr) {
   const Model* m = s->model;
+  cudaStream_t st = on ? on : s->stream;
   const unsigned grid = std::min<unsigned>((s->n + 255) / 256, (unsigned)s->dev.sms * 8u);
-  return launch_chain(&s->timer, shade_all_kernel, dim3(grid), dim3(256), 0, s->stream, P, s->n, s->counts.as<uint32_t>(),
+  return launch_chain(&s->timer, shade_all_kernel, dim3(grid), dim3(256), 0, st, P, s->n, s->counts.as<uint32_t>(),
                       only_if, m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
                       s->record.as<float4>(), s->featw_last);
 }
@@ -877,7 +881,10 @@ int launch_bin_write(pvg_scene* s, const FrameParams& P, uint32_t kin_lo, uint32
   const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
   uint32_t* bin_start = s->bin_tables.as<uint32_t>();   // written by tile_prefix_kernel
   const uint32_t launch_chunks = (kin_lo == 0 && kin_hi < (1u << 30)) ? std::min<uint64_t>((uint64_t)nbins * kin_hi, 0x7FFFFFFFull) : max_chunks;
-  const unsigned grid = (launch_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
+  unsigned grid = (launch_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA;
+  // the second round (parked tiles only) usually finds nothing to do: a grid of four CTAs per SM that loops over tickets
+  const uint32_t loop = only_unfinished ? 1u : 0u;
+  if (loop) grid = std::min(grid, (unsigned)s->dev.sms * 4u);
   return launch_chain(&s->timer, bin_write_kernel, dim3(grid), dim3(BW_THREADS), 0, s->stream,
       s->s_g.as<uint32_t>(), s->s_mask.as<uint64_t>(), bin_start, bin_start + 257, s->ranges.as<uint2>(), (uint32_t)P.tiles_x,
       (uint32_t)P.tiles_y, blocks_x, s->chunk_cnt.as<uint64_t>(), s->sort_m.tickets.as<uint32_t>() + ticket_slot,
@@ -885,7 +892,7 @@ int launch_bin_write(pvg_scene* s, const FrameParams& P, uint32_t kin_lo, uint32
       reinterpret_cast<const uint32_t*>(s->unf.as<unsigned char>() + 2048),
       (kin_lo == 0 && kin_hi < (1u << 30)) ? reinterpret_cast<uint32_t*>(s->unf.as<unsigned char>() + kUnfHead) : (uint32_t*)nullptr,
       (s->lazy_used && s->emit_first && s->emit_first < s->emit_tiles)
-          ? s->sort_m.lookback.as<uint64_t>() + (size_t)(s->emit_first - 1) * s->emit_radix : (uint64_t*)nullptr);
+          ? s->sort_m.lookback.as<uint64_t>() + (size_t)(s->emit_first - 1) * s->emit_radix : (uint64_t*)nullptr, loop);
 }
 
 // a2 + a3 (instance part) through 8x8-tile block entries (blockbin.cuh), after prep_block_bins: the sorted value
@@ -1244,22 +1251,33 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       PVG_BLEND_ALL(1)
       TRY(tm.end(st));
 #if PVG_BIN_FUSED
+      bool shading = false;
       if (s->emit_first < s->emit_tiles) {
-        TRY(tm.begin("bin_emit", PVG_STAGE_SORT, st));
-        TRY(run_bin_emit(s, P, s->visit_last, s->emit_tiles - s->emit_first, Z.unf_count));
-        TRY(tm.end(st));
         if (s->light) {
-          TRY(tm.begin("shade", PVG_STAGE_PREPROCESS, st));
-          // the rest of the scene: in index order (sequential model reads; the first slab's records are rewritten
-          // with the same values)
-          TRY(run_shade_all(s, P, Z.unf_count));
-          TRY(tm.end(st));
+          // the rest of the scene's records, in index order (sequential model reads; the first slab's records are
+          // rewritten with the same values), on the side stream: nothing before phase 2 of the blend needs them
+          cudaStream_t sd = s->side;
+          CU(cudaEventRecord(s->ev_fork, st));
+          CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
+          tm.cut();
+          TRY(tm.begin("shade", PVG_STAGE_PREPROCESS, sd));
+          TRY(run_shade_all(s, P, Z.unf_count, sd));
+          TRY(tm.end(sd));
+          CU(cudaEventRecord(s->ev_join, sd));
+          shading = true;
         }
+        TRY(tm.begin("bin_emit", PVG_STAGE_SORT, st));
+        TRY(run_bin_emit(s, P, s->visit_last, s->emit_tiles - s->emit_first, Z.unf_count, true));
+        TRY(tm.end(st));
       }
 #endif
       TRY(tm.begin("bin_write", PVG_STAGE_SORT, st));
       TRY(launch_bin_write(s, P, (uint32_t)s->lazy_chunks, 0xFFFFFFFFu, true, 2));
       TRY(tm.end(st));
+      if (shading) {
+        CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+        tm.cut();
+      }
       TRY(tm.begin("blend", PVG_STAGE_BLEND, st));
       PVG_BLEND_ALL(2)
     }
