@@ -37,6 +37,16 @@ CONFIG_NAMES = {0: "cfg0_tiny_4096g_128x96", 1: "cfg1_mid_200kg_960x640", 2: "cf
 SLOTS_REJECT, SLOTS_ACCEPT_EXTRA = 11, 6
 
 
+def base_config(args, n_gaussians: int, frames, world_size: int) -> dict:
+    """`config` of the JSON line: what is rendered. Identical in both arms (ours / reference) by construction; what is
+    specific to an arm's run goes into `run_details`."""
+    c0 = frames[0][0]
+    return {"workload": CONFIG_NAMES[args.config], "n_gaussians": int(n_gaussians), "resolution": f"{c0.width}x{c0.height}",
+            "frames": "one (camera, t) per step, round-robin over the sweep",
+            "l2_policy": f"inputs larger than L2: the model, {n_gaussians * 256 / 1e6:.0f} MB, is read every frame (126 MB L2)",
+            "parallelism": f"frames sharded over {world_size} rank(s), no collective"}
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -203,8 +213,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": CONFIG_NAMES[args.config], "n_gaussians": wl.scene.n,
-                       "resolution": f"{frames[0][0].width}x{frames[0][0].height}"},
+            "config": base_config(args, wl.scene.n, frames, args.gpus),
             "cpu_baseline": {"value": fps, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                              "sample": (f"every step one whole frame: Oracle-P on all {wl.scene.n} Gaussians + Oracle-R (binned) "
                                         f"on all {det['tiles_total']} tiles; no sampling, no extrapolation")},
@@ -258,8 +267,8 @@ def algorithmic_bytes(agg, K, N, S, Msum, Mbsum, chunks, lazy):
            ("onesweep_histogram", "depth_sort"): K * 8.0 * N,
            ("tile_ranges", "ranges"): 8.0 * Msum}
     if lazy:
-        # deferred records: preprocess reads the 64 B model + 1 B flag and writes tile info, count and depth pair (32 B)
-        alg[("preprocess", "preprocess")] = K * 97.0 * N
+        # deferred records: preprocess reads the 64 B model + 1 B flag and writes tile info, count and depth key (28 B)
+        alg[("preprocess", "preprocess")] = K * 93.0 * N
         # lazy lists: bin_emit forms the first 1/8 of the entries and bin_write the first chunks of every block -- what
         # they move depends on where the tiles saturate, so no algorithmic-byte figure is claimed for them
         alg.pop(("bin_emit", "sort"), None)
@@ -267,9 +276,9 @@ def algorithmic_bytes(agg, K, N, S, Msum, Mbsum, chunks, lazy):
     for key in (("onesweep_pass", "sort"), ("onesweep_pass", "depth_sort")):
         if key in agg:
             per_frame = agg[key][1] / K
-            # depth sort (9 + 9 + 9 + 4 bits): pass 0 reads the n pairs and writes the S survivors, passes 1 and 2 move
-            # the S survivors, the top-digit pass is the identity and exits (12 B per pair each way)
-            alg[key] = 24.0 * Msum * per_frame if key[1] == "sort" else K * (12.0 * N + 60.0 * S)
+            # depth sort (9 + 9 + 9 + 4 bits): pass 0 reads the n keys (8 B; the value of pair i is i) and writes the S
+            # surviving pairs (12 B), passes 1 and 2 move the S pairs, the top-digit pass is the identity and not launched
+            alg[key] = 24.0 * Msum * per_frame if key[1] == "sort" else K * (8.0 * N + 60.0 * S)
     return alg
 
 
@@ -605,18 +614,13 @@ def run_ours(args):
     line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": ws, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": elapsed_s * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload, "n_gaussians": N, "survivors_last_frame": S,
-                       "resolution": f"{frames[0][0].width}x{frames[0][0].height}",
-                       "instances_per_frame_mean": tab["Msum"] / K, "block_entries_per_frame_mean": tab["Mbsum"] / K,
-                       "list_mode": list_mode,
-                       "lists": ("lazy (PVG_OPT_LAZY_CHUNKS/SLAB defaults): list prefixes, the remainder only for parked tiles; "
-                                 f"parked tiles in the last frame: {main['parked']}") if lazy else "complete",
-                       "frames": "one (camera, t) per step, round-robin over the sweep",
-                       "l2_policy": (f"inputs larger than L2: the model, {N * 256 / 1e6:.0f} MB read every frame, vs 126 MB L2" if lazy else
-                                     f"inputs larger than L2: model {N * 256 / 1e6:.0f} MB + sorted list + block entries "
-                                     f"{(4 * tab['Msum'] + 25 * tab['Mbsum']) / K / 1e6:.0f} MB per frame vs 126 MB L2"),
-                       "arithmetic": "fp32; the position chain mu~(t) -> p_cam -> mean2D and the record's conic in fp64 (DESIGN.md 5)",
-                       "parallelism": f"frames sharded over {ws} rank(s), no collective", "presort_depth": args.presort},
+            "config": base_config(args, N, frames, ws),
+            "run_details": {"survivors_last_frame": S, "instances_per_frame_mean": tab["Msum"] / K,
+                            "block_entries_per_frame_mean": tab["Mbsum"] / K, "list_mode": list_mode,
+                            "lists": ("lazy (PVG_OPT_LAZY_CHUNKS/SLAB defaults): list prefixes, the remainder only for parked tiles; "
+                                      f"parked tiles in the last frame: {main['parked']}") if lazy else "complete",
+                            "arithmetic": "fp32; the position chain mu~(t) -> p_cam -> mean2D and the record's conic in fp64 (DESIGN.md 5)",
+                            "presort_depth": args.presort},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "pipelined": pipelined, "clocks": clocks,
             "gpu_launches": int(round(len(main["krecs"]) * Kall / K)),
             "kernel_events": f"recorded on every {stride}th frame of the timed region ({K} of {Kall} frames, {len(main['krecs'])} launches)",

@@ -249,7 +249,7 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
     if (PHASE == 1) range.y = lim; else range.x = lim;
   }
 
-  static_assert(BLEND_NPX == 4, "two pixel pairs per thread");
+  static_assert(BLEND_NPX == 4 || BLEND_NPX == 8, "two or four pixel pairs per thread");
   constexpr int NPAIR = BLEND_NPX / 2;
   BlendPair X[NPAIR];
   {
@@ -277,11 +277,15 @@ blend_tile(const FrameParams& P, const uint32_t tile, const uint2* __restrict__ 
   }
   // a pixel is live while its T is positive: some pixel of the thread is live iff the AND of the four sign bits is clear
   auto any_alive = [&]() {
-    const f32x2 m = X[0].T & X[1].T;
+    f32x2 m = X[0].T;
+#pragma unroll
+    for (int p = 1; p < NPAIR; ++p) m &= X[p].T;
     return (m & 0x8000000080000000ull) != 0x8000000080000000ull;
   };
   // the pixel centres of the two pairs, and the row, as packed operands
-  const f32x2 pxp[NPAIR] = {pack2(pxf, pxf + 1.0f), pack2(pxf + 2.0f, pxf + 3.0f)};
+  f32x2 pxp[NPAIR];
+#pragma unroll
+  for (int p = 0; p < NPAIR; ++p) pxp[p] = pack2(pxf + (float)(2 * p), pxf + (float)(2 * p + 1));
   const f32x2 pyp = pack2(pyf, pyf);
   uint32_t n_eval = 0, n_contrib = 0;
 

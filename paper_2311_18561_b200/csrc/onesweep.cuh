@@ -418,7 +418,8 @@ depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, 
   for (int j = 0; j < ITEMS; ++j) {
     const bool ok = wbase + j * 32 < tile_n;
     key[j] = ok ? __ldcg(kp + j * 32) : ~0ull;
-    val[j] = ok ? __ldcg(vp + j * 32) : 0u;
+    // FIRST: the pairs come from preprocess in index order, the value of pair i is i
+    val[j] = FIRST ? tile_base + wbase + j * 32 : (ok ? __ldcg(vp + j * 32) : 0u);
   }
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {

@@ -54,7 +54,7 @@ __device__ __forceinline__ double sinpi_reduced(double x) {
 //                           colour slot holds vbar in camera axes and featw[i] = clamp(rho, 0, 2)
 //   tileinfo[i] = (x0 | y0 << 16, rect width | height << 16, fp32 bits of z, rect count)
 //   counts[i]   = rect count (0 if culled)
-//   dkeys[i], dvals[i] (optional) = (packed tile rect << 32 | depth key, or 0xFFFFFFFF if culled), i
+//   dkeys[i] (optional) = (packed tile rect << 32 | depth key, or 0xFFFFFFFF if culled); the pair's value is i itself
 //                           depth key = fp32 bits of z - fp32 bits of znear (z > znear > 0: positive, same order as z)
 // Returns the depth key, 0xFFFFFFFF if culled.
 // PART: PRE_ALL -- everything. PRE_GEO -- what the list building needs (tile info, counts, depth pair) without the
@@ -292,7 +292,7 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
       rect = x0 | (y0 << 8) | ((x0 + (ti.y & 0xFFFFu) - 1u) << 16) | ((y0 + (ti.y >> 16) - 1u) << 24);
     }
     dkeys[i] = valid ? (((uint64_t)rect << 32) | (ti.z - __float_as_uint(P.znear))) : 0xFFFFFFFFull;
-    dvals[i] = i;
+    (void)dvals;   // the value of pair i is i: the first pass of the depth sort forms it instead of loading it
   }
   return valid ? ti.z - __float_as_uint(P.znear) : 0xFFFFFFFFu;
 }
@@ -346,9 +346,13 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
   }
   __shared__ bool s_last;
   __shared__ uint32_t s_warp[8], s_bins[8];
-  __threadfence();
+  // release: the barrier orders every thread's histogram atomics before thread 0, whose (cumulative) fence orders them
+  // before its count -- one fence per CTA instead of one per thread (ncu: 1.1 stall cycles per issued instruction)
   __syncthreads();
-  if (threadIdx.x == 0) s_last = atomicAdd(dhist + DH_COUNTER, 1u) == gridDim.x - 1;
+  if (threadIdx.x == 0) {
+    __threadfence();
+    s_last = atomicAdd(dhist + DH_COUNTER, 1u) == gridDim.x - 1;
+  }
   __syncthreads();
   if (!s_last) return;
   __threadfence();
