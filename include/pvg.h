@@ -231,7 +231,17 @@ typedef enum pvg_option {
    *    (pvg_debug_view; no unsorted list in this mode). Implies complete lists and eager records (LAZY_CHUNKS is
    *    ignored): with lazy lists the same test already runs inside the blend on the few entries a tile consumes
    *    (BLEND_CULL), which is cheaper by two orders of magnitude -- this mode is for consumers of the lists themselves. */
-  PVG_OPT_EXACT_TILES = 13
+  PVG_OPT_EXACT_TILES = 13,
+  /* 1 (default), with LAZY_CHUNKS > 0: front-first depth order. The first blend phase consumes the first slab of the
+   *    block entries in depth order, and those belong to the few Gaussians nearest the camera (about 1 % of the
+   *    survivors at config 3: near Gaussians are large on screen). So the frame orders, scans and bins only that front:
+   *    preprocess's last CTA picks a depth-key threshold from a histogram of the entries over the top key bits such
+   *    that the Gaussians below it own more than the slab; the pairs below the threshold are compacted in index
+   *    order (the sort stays stable) and radix-sorted. The pairs at and beyond the threshold are compacted, sorted
+   *    behind the front and scanned only if a tile was parked (or pvg_debug_view asks): a sorted front followed by a
+   *    sorted back is the sorted whole, the threshold being a key value, so the visiting order, the offsets, the
+   *    lists and the images are bit-identical to 0. 0: sort all survivors up front. */
+  PVG_OPT_LAZY_DEPTH = 14
 } pvg_option;
 int pvg_set_option(pvg_scene *scene, int option, int64_t value);
 
@@ -282,7 +292,8 @@ int pvg_kernel_timeline_ms(pvg_scene *scene, int cap, const char **names, float 
  * block entries (BLOCK_BINS mode, else 0), list mode: 0 = 64-bit keys, 1 = compact keys, 2 = block entries, 3 = block
  * entries with exact tile lists, surviving Gaussians S (PRESORT_DEPTH=1, else 0), tiles the first blend phase of the
  * lazy lists parked (LAZY_CHUNKS; valid once the frame has completed on the stream), instances of the exact lists
- * (EXACT_TILES; valid once the frame has completed), 0}. */
+ * (EXACT_TILES; valid once the frame has completed), pairs the front-first depth order sorted up front (LAZY_DEPTH,
+ * else 0)}. */
 int pvg_frame_stats(pvg_scene *scene, uint64_t out[10]);
 
 /* Work done by the last blend when PVG_OPT_COUNT_PAIRS=1: out[0] = (pixel, list entry) pairs

@@ -22,7 +22,7 @@ STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_
 OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
 OPT_BLEND_CULL, OPT_EVENT_STRIDE = 7, 8
 OPT_TILE_ROW_BEGIN, OPT_TILE_ROW_END = 9, 10
-OPT_LAZY_CHUNKS, OPT_LAZY_SLAB, OPT_EXACT_TILES = 11, 12, 13
+OPT_LAZY_CHUNKS, OPT_LAZY_SLAB, OPT_EXACT_TILES, OPT_LAZY_DEPTH = 11, 12, 13, 14
 STAGES = ("preprocess", "depth_sort", "duplicate", "sort", "ranges", "blend")
 NUM_STAGES = len(STAGES)
 
@@ -356,7 +356,7 @@ class Scene:
         _check(self._L.pvg_frame_stats(self._h, out))
         return {"n": int(out[0]), "M": int(out[1]), "tiles_x": int(out[2]), "tiles_y": int(out[3]),
                 "block_entries": int(out[4]), "list_mode": ("keys64", "compact", "blocks", "blocks_exact")[int(out[5])],
-                "survivors": int(out[6]), "parked_tiles": int(out[7]), "M_exact": int(out[8])}
+                "survivors": int(out[6]), "parked_tiles": int(out[7]), "M_exact": int(out[8]), "front": int(out[9])}
 
     def blend_counters(self) -> Tuple[int, int]:
         """(pairs evaluated, pairs contributing) of the last render with OPT_COUNT_PAIRS=1."""

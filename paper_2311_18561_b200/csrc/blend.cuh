@@ -198,6 +198,37 @@ struct BlendLazy {
   uint32_t blocks_x;
 };
 
+// The second round of the lazy lists, launched FROM THE DEVICE (round2.cuh, round2.cu): the launch parameters of its
+// kernels, filled by the host before the first blend phase. After that phase a one-thread gate kernel reads the
+// parked count; if it is not zero it tail-launches the chain (CUDA dynamic parallelism: the kernels run in order once
+// the gate has completed, and whatever the host enqueued next runs after them). A frame in which no tile parked --
+// the normal case -- then pays one small launch for the second round, where nine launches that found nothing to do
+// cost 25-35 us.
+struct FrontCtl;   // onesweep.cuh
+struct R2Chain {
+  uint32_t enabled;      // 0: the host launches the second round itself (PVG_R2_TAIL=0)
+  // the back of the depth order (front-first, onesweep.cuh): select, passes, scan
+  uint32_t back;
+  const uint64_t* okeys; uint32_t n; const FrontCtl* fc;
+  uint64_t* sel_keys; uint32_t* sel_vals; uint32_t* sel_region; uint64_t* sel_status; uint32_t* sel_ticket;
+  uint32_t sel_side, sel_grid;
+  uint64_t* lb; uint32_t lb_rows, lb_tile;
+  uint64_t *ka, *kb; uint32_t *va, *vb;
+  uint32_t back_count, passes, pass_grid; uint32_t* pass_tickets;
+  uint32_t scan_grid; const uint64_t* scan_keys; const uint32_t* visit; uint32_t* boffsets; uint64_t* scan_total;
+  uint64_t* scan_status; uint32_t* scan_ticket; uint32_t* chunk_owner; uint32_t owner_chunk, rank0; const uint64_t* scan_init;
+  const uint32_t* counts;
+  // the records of the whole scene
+  uint32_t shade, shade_grid; const float4 *A0, *A1, *A2, *A3, *SH; float4* record; float* featw;
+  // the entries behind the first slab
+  uint32_t emit, emit_grid, emit_bits, nv, Mb, blocks_x, emit_tiles;
+  uint32_t* s_g; uint64_t* s_mask; const uint32_t* bin_start; uint64_t* emit_lookback; uint32_t* emit_ticket;
+  // the rest of the parked tiles' lists
+  uint32_t write_grid; const uint2* ranges; uint32_t tiles_x, tiles_y; uint64_t* chunk_cnt; uint32_t* write_ticket;
+  uint32_t* vals; uint32_t kin_lo; const unsigned long long* want_mask; const uint32_t* want_count; const uint64_t* avail;
+  // the second blend phase
+  uint32_t blend_grid;
+};
 // Parks a tile (first blend phase of the lazy lists): out of line, so that the rare path costs the common one nothing.
 // st[k] = (T signed: negative = stopped, Cr, Cg, Cb, D).
 __device__ __noinline__ void blend_park(const BlendLazy& Z, uint32_t tile, uint32_t bin, uint32_t ltile, size_t HW, size_t pi,

@@ -73,7 +73,7 @@ __device__ __forceinline__ void bb_entry(uint32_t xy0, uint32_t xy1, uint32_t j,
 // box of pixel centres misses it go. Integer work: every float operation is an individually rounded fp32 one
 // (__f*_rn: no contraction), in the order the oracle's exact_row_span takes them, so both sides decide identically.
 // r0 = (mx, my, z, o~), r1 = (a, b, c, hx) of the fp32 record.
-__device__ __noinline__ uint64_t bb_refine_mask(uint64_t mask, uint32_t bx, uint32_t by, float4 r0, float4 r1) {
+static __device__ __noinline__ uint64_t bb_refine_mask(uint64_t mask, uint32_t bx, uint32_t by, float4 r0, float4 r1) {
   const float a = r1.x, b = r1.y, c = r1.z, hx = r1.w;
   const float det = __fsub_rn(__fmul_rn(a, c), __fmul_rn(b, b));
   const float k = __fdiv_rn(__fmul_rn(__fmul_rn(hx, hx), det), c);
@@ -280,6 +280,7 @@ bin_pass_kernel(const uint8_t* __restrict__ bin_in, const uint32_t* __restrict__
 // thread derives its BP_ITEMS entries (warp-striped, the order RadixCore ranks in), and the staging arrays of
 // the split then reuse the shared memory of the owner table.
 constexpr int BF_TILE = BP_THREADS * BP_ITEMS;
+static_assert(BF_TILE == PVG_EMIT_TILE, "lazy_emit_first (common.cuh) counts bin_emit tiles");
 constexpr int BF_SPAN = BF_TILE + 64;
 
 template <int BITS>

@@ -48,7 +48,18 @@ struct FrameParams {
   float bg[3];
   const float* sky;   // cube map [6][res][res][3] or nullptr: rgb = C + (1 - O) f_sky(d)
   int sky_res;
+  int lazy_slab;      // PVG_OPT_LAZY_SLAB (front-first depth order: preprocess sizes the front from it)
 };
+
+// Lazy lists: bin_emit forms the block entries in tiles of PVG_EMIT_TILE (== BF_TILE, blockbin.cuh); its first launch
+// takes the first 1 / lazy_slab of the tiles (at least one). One formula for the host and for preprocess's last CTA.
+#define PVG_EMIT_TILE 4096
+__host__ __device__ inline uint32_t lazy_emit_first(unsigned long long Mb, int lazy_slab) {
+  const uint32_t tiles = (uint32_t)((Mb + PVG_EMIT_TILE - 1) / PVG_EMIT_TILE);
+  const uint32_t slab = lazy_slab > 0 ? (uint32_t)lazy_slab : 1u;
+  const uint32_t first = (tiles + slab - 1u) / slab;
+  return tiles < (first > 1u ? first : 1u) ? tiles : (first > 1u ? first : 1u);
+}
 
 __device__ __forceinline__ uint32_t lane_id() {
   uint32_t r;
@@ -66,8 +77,15 @@ __device__ __forceinline__ uint32_t lanemask_lt() {
 // draining; pdl_wait() returns when that kernel has completed and its writes are visible. pdl_launch_dependents()
 // lets the NEXT kernel of the stream do the same with respect to this one. Both are no-ops in a plain launch.
 // Every kernel of a chain waits before its first global read (transitively, everything earlier has then completed).
+// PVG_NO_GRIDDEP (round2.cu: the copies of the kernels that are launched from the device, never as programmatic
+// dependents): both are empty.
+#ifdef PVG_NO_GRIDDEP
+__device__ __forceinline__ void pdl_wait() {}
+__device__ __forceinline__ void pdl_launch_dependents() {}
+#else
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
 
 // 64-bit status words of the decoupled look-back (flag in the top 2 bits, value
 // below): one aligned 64-bit access carries flag and payload together, so relaxed

@@ -151,6 +151,9 @@ onesweep_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n, const _
 // elements). rank() turns the per-element digits into tile-local sorted positions and
 // resolves, by decoupled look-back over earlier tiles, where each digit's run starts in the
 // output. Stable: earlier rows, lower lanes, lower warps, earlier tiles come first.
+#ifndef PVG_LB_WINDOW
+#define PVG_LB_WINDOW 4
+#endif
 template <int THREADS, int ITEMS, int BITS>
 struct RadixCore {
   static constexpr int WARPS = THREADS / 32;
@@ -183,7 +186,9 @@ struct RadixCore {
   // s.out_base[digit] + position is the element's output index.
   // SPARSE: elements with dp[j] == INVALID take no part (anywhere in the tile): they are not counted, get no
   // position and keep dp[j] == INVALID; s.total is the number of elements that do take part.
-  template <bool SPARSE = false>
+  // WINDOW: look-back words fetched per round trip. Large sorts run in waves and find a published prefix nearby (4 is
+  // enough); a small sort's tiles all start together, and a tile walks back over all of them.
+  template <bool SPARSE = false, int WINDOW = PVG_LB_WINDOW>
   __device__ static __forceinline__ void rank(Smem& s, uint32_t tile, uint32_t (&dp)[ITEMS],
                                               const uint32_t* __restrict__ hist_excl,
                                               uint64_t* __restrict__ lookback) {
@@ -242,10 +247,7 @@ struct RadixCore {
         if (tile != 0) {
           // windowed: the status words of the next LB_WINDOW predecessors are fetched together (one L2
           // round trip), then consumed in order up to the first one that is not published yet
-#ifndef PVG_LB_WINDOW
-#define PVG_LB_WINDOW 4
-#endif
-          constexpr int LB_WINDOW = PVG_LB_WINDOW;
+          constexpr int LB_WINDOW = WINDOW;
           uint32_t left = tile;   // predecessors not yet consumed; tile 0 always ends the walk
           const uint64_t* p = lookback + (uint64_t)(tile - 1) * RADIX + tid;
           bool done = false;
@@ -366,6 +368,11 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __res
 //     scene whose far plane is below 65536 znear: three passes instead of the four of an 8-bit plan;
 //   * S, which passes run and which buffer each reads are decided on the device by the last CTA of preprocess, which
 //     holds the digit histograms (DepthCtl); every pass is launched for the worst case and reads the block.
+#ifndef PVG_DS_THREADS
+#define PVG_DS_THREADS 512   // tile shape of the depth passes (the launch configuration lives in pvg_api.cu: DsCfg)
+#define PVG_DS_ITEMS 8
+#define PVG_DS_MINB 2
+#endif
 constexpr int DS_PASSES = 4;
 constexpr int DS_BITS = 9;
 constexpr int DS_RADIX = 1 << DS_BITS;
@@ -381,14 +388,224 @@ struct DepthCtl {
   uint32_t in_side[DS_PASSES]; // buffer pair the pass reads (it writes the other one)
 };
 
-template <int THREADS, int ITEMS, int BITS, int MINB, bool FIRST>
+// Layout of a histogram region (u32 words) of the depth sort: [4][512] digit counts, turned into exclusive prefixes by
+// the last CTA of the kernel that counts them, a CTA counter, the control block.
+constexpr int DH_COUNTER = DS_PASSES * DS_RADIX;   // u32 index of the CTA counter (the two words after it: a 64-bit sum)
+constexpr int DH_CTL = DH_COUNTER + 8;             // u32 index of the control block (8-byte aligned)
+constexpr int DH_WORDS = DH_CTL + 16;              // words per region (a multiple of 4)
+static_assert(sizeof(DepthCtl) <= 16 * 4, "DepthCtl fits its slot");
+
+// ---- front-first depth order (lazy lists) -------------------------------------------------------------------------
+// The first round of the lazy lists consumes the first slab of the block entries in depth order, and those belong to
+// the few Gaussians nearest the camera (they are the large ones: about 1 % of the survivors own the first eighth of
+// the entries at config 3). So the frame orders only those: preprocess's last CTA picks a key threshold from a
+// histogram of the entries over the top key bits (FrontCtl), depth_select_kernel<false> compacts the pairs below it
+// (index order: the sort stays stable) and counts their digits, and the ordinary passes run over that front alone.
+// The pairs at and beyond the threshold are selected and ordered behind the front -- a sorted front followed by a sorted
+// back IS the sorted whole, the threshold being a key value -- only if a tile parks (second round) or a debug view asks.
+constexpr int FR_SHIFT = 18;                       // bucket = key >> 18: 32 buckets per binade of z
+constexpr int FR_BUCKETS = 1024;                   // the last one takes every key beyond 1023 << 18
+constexpr int FR_TOP = 1 << (3 * DS_BITS - FR_SHIFT);   // buckets below it hold keys below 2^27: top digit 0
+struct FrontCtl {
+  uint32_t survivors;   // S
+  uint32_t front;       // F: pairs with key < thr
+  uint32_t thr;         // 0xFFFFFFFF: every survivor is in front
+  uint32_t top_front;   // 1: the front has keys of 2^27 and beyond (its top-digit pass is needed)
+  uint32_t top_back;    // 1: the back has
+};
+
+// One wave: 1024 threads x 24 pairs = 24576 pairs per CTA, 123 CTAs for 3 M pairs. A pass like this is a chain of
+// latencies (ticket, loads, look-back, writes, last-CTA count) -- with tiles of 4096 it ran in three waves and took
+// three chains (ncu: 36 us, warps waiting at barriers).
+constexpr int SEL_THREADS = 1024;
+constexpr int SEL_ITEMS = 24;
+constexpr int SEL_TILE = SEL_THREADS * SEL_ITEMS;
+
+// Ordered selection of one class of pairs. keys: the n pairs of preprocess in index order (never overwritten).
+// Output: the selected pairs (key, index) in index order at keys_out / vals_out [base, base + count), base = 0 (front)
+// or F (back), the indices once more in list_out (optional: shade_list_kernel reads them while the passes already
+// overwrite vals_out); region: the class's histogram region (zeroed): digit prefixes + DepthCtl for the passes, which
+// read buffer `out_side` first. status [tiles] and ticket: zeroed. only_if: nothing to do when *only_if == 0.
+// The kernel also zeroes the look-back words its class's passes will use (lb: [4 passes][lb_rows][radix], tiles of
+// lb_tile pairs): the class's size is known here (FrontCtl), so no memset sized by n is needed.
+// A warp owns 32 x 24 consecutive pairs, element (j, lane) at j * 32 + lane: coalesced loads, and the rank of a
+// selected element inside the warp's run is popc of the ballots before it. Only the ballots stay in registers; the
+// selected keys are loaded again (few of them in front; all of them, coalesced, behind).
+template <bool BACK>
+__global__ void __launch_bounds__(SEL_THREADS)
+depth_select_kernel(const uint64_t* __restrict__ keys, uint32_t n, const FrontCtl* __restrict__ fc,
+                    uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint32_t* __restrict__ list_out,
+                    uint32_t* __restrict__ region, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
+                    uint32_t out_side, uint64_t* __restrict__ lb, uint32_t lb_rows, uint32_t lb_tile,
+                    const uint32_t* __restrict__ only_if) {
+  pdl_launch_dependents();
+  pdl_wait();
+  if (only_if && *only_if == 0u) return;
+  __shared__ uint32_t s_hist[DS_PASSES * DS_RADIX];
+  __shared__ uint32_t s_tile, s_warp[SEL_THREADS / 32], s_first[SEL_THREADS / 32];
+  __shared__ uint64_t s_sum[SEL_THREADS / 32];
+  __shared__ bool s_last;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+#pragma unroll
+  for (int k = 0; k < DS_PASSES * DS_RADIX / SEL_THREADS; ++k) s_hist[k * SEL_THREADS + tid] = 0;
+  if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+  const uint32_t thr = fc->thr;
+  const uint32_t out0 = BACK ? fc->front : 0u;
+  {
+    const uint32_t cnt = BACK ? fc->survivors - fc->front : fc->front;
+    const uint32_t rows = min(lb_rows, (cnt + lb_tile - 1u) / lb_tile);
+    uint64_t* q = lb;
+    for (int d = 0; d < DS_PASSES; ++d) {
+      const uint32_t words = rows << ds_bits(d);
+      for (uint32_t i = blockIdx.x * SEL_THREADS + tid; i < words; i += gridDim.x * SEL_THREADS) q[i] = 0ull;
+      q += (size_t)lb_rows << ds_bits(d);
+    }
+  }
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const uint32_t wbase = tile * SEL_TILE + warp * (32 * SEL_ITEMS) + lane;
+  const uint32_t* lo32 = reinterpret_cast<const uint32_t*>(keys);   // the depth key: the low word of the pair
+  uint32_t bal[SEL_ITEMS];
+  uint32_t wcount = 0;
+  constexpr int HALF = SEL_ITEMS / 2;   // the loads of a half are all in flight before the first ballot
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t w[HALF];
+#pragma unroll
+    for (int j = 0; j < HALF; ++j) {
+      const uint32_t i = wbase + (h * HALF + j) * 32;
+      w[j] = i < n ? __ldcg(lo32 + 2 * (size_t)i) : 0xFFFFFFFFu;
+    }
+#pragma unroll
+    for (int j = 0; j < HALF; ++j) {
+      const bool in = BACK ? (w[j] >= thr && w[j] != 0xFFFFFFFFu) : (w[j] < thr);
+      bal[h * HALF + j] = __ballot_sync(0xffffffffu, in);
+      wcount += __popc(bal[h * HALF + j]);
+    }
+  }
+  if (lane == 0) s_warp[warp] = wcount;
+  __syncthreads();
+  uint32_t warp_excl = 0, block_sum = 0;
+#pragma unroll
+  for (int w = 0; w < SEL_THREADS / 32; ++w) {
+    const uint32_t v = s_warp[w];
+    if (w < (int)warp) warp_excl += v;
+    block_sum += v;
+  }
+  // Look-back over the tiles' counts, the whole CTA wide: thread t waits for the word of tile - 1 - t (it holds an
+  // earlier ticket: its CTA is running), the CTA adds the counts up to the nearest published prefix.
+  uint64_t excl = 0;
+  if (tile == 0) {
+    if (tid == 0) st_relaxed_u64(status, LB_FLAG_PREFIX | block_sum);
+  } else {
+    if (tid == 0) st_relaxed_u64(status + tile, LB_FLAG_AGG | block_sum);
+    int64_t p = (int64_t)tile - 1 - (int64_t)tid;
+    while (true) {
+      uint64_t sv = LB_FLAG_PREFIX;
+      if (p >= 0) do { sv = ld_relaxed_u64(status + p); } while ((sv & LB_FLAG_MASK) == 0ull);
+      const uint32_t pref = __ballot_sync(0xffffffffu, (sv & LB_FLAG_MASK) == LB_FLAG_PREFIX);
+      if (lane == 0) s_first[warp] = pref ? warp * 32u + (uint32_t)(__ffs(pref) - 1) : 0xFFFFFFFFu;
+      __syncthreads();
+      uint32_t first = 0xFFFFFFFFu;
+#pragma unroll
+      for (int w = 0; w < SEL_THREADS / 32; ++w) first = min(first, s_first[w]);
+      uint64_t v = tid <= first ? (sv & LB_VALUE_MASK) : 0ull;
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+      if (lane == 0) s_sum[warp] = v;
+      __syncthreads();
+#pragma unroll
+      for (int w = 0; w < SEL_THREADS / 32; ++w) excl += s_sum[w];
+      __syncthreads();
+      if (first != 0xFFFFFFFFu) break;
+      p -= SEL_THREADS;
+    }
+    if (tid == 0) st_relaxed_u64(status + tile, LB_FLAG_PREFIX | (excl + block_sum));
+  }
+  if (wcount) {
+    uint32_t o = out0 + (uint32_t)excl + warp_excl;
+    const uint32_t lt = lanemask_lt();
+#pragma unroll
+    for (int j = 0; j < SEL_ITEMS; ++j) {
+      if ((bal[j] >> lane) & 1u) {
+        const uint32_t i = wbase + j * 32;
+        const uint64_t key = __ldcg(keys + i);
+        const uint32_t at = o + __popc(bal[j] & lt);
+        keys_out[at] = key;
+        vals_out[at] = i;
+        if (list_out) list_out[at] = i;
+        const uint32_t w = (uint32_t)key;
+#pragma unroll
+        for (int d = 0; d < DS_PASSES; ++d) atomicAdd(&s_hist[d * DS_RADIX + ((w >> ds_shift(d)) & ((1u << ds_bits(d)) - 1u))], 1u);
+      }
+      o += __popc(bal[j]);
+    }
+  }
+  __syncthreads();
+  if (block_sum) {
+#pragma unroll
+    for (int k = 0; k < DS_PASSES * DS_RADIX / SEL_THREADS; ++k) {
+      const uint32_t v = s_hist[k * SEL_THREADS + tid];
+      if (v) atomicAdd(&region[k * SEL_THREADS + tid], v);
+    }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_last = atomicAdd(region + DH_COUNTER, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  // the last CTA: exclusive digit prefixes (thread t owns bin t) and the control block of the class's passes
+  uint32_t total = 0;
+  for (int d = 0; d < DS_PASSES; ++d) {
+    const uint32_t v = tid < (1u << ds_bits(d)) ? __ldcg(region + d * DS_RADIX + tid) : 0u;
+    uint32_t in2 = v;
+#pragma unroll
+    for (int q = 1; q < 32; q <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, in2, q);
+      if (lane >= q) in2 += t;
+    }
+    if (lane == 31) s_warp[warp] = in2;
+    __syncthreads();
+    uint32_t wex = 0, all = 0;
+    for (uint32_t w = 0; w < SEL_THREADS / 32; ++w) {
+      if (w < warp) wex += s_warp[w];
+      all += s_warp[w];
+    }
+    if (tid < (1u << ds_bits(d))) region[d * DS_RADIX + tid] = wex + in2 - v;
+    total = all;
+    __syncthreads();
+  }
+  if (tid == 0) {
+    DepthCtl* ctl = reinterpret_cast<DepthCtl*>(region + DH_CTL);
+    ctl->survivors = total;
+    uint32_t side = out_side;
+    for (int d = 0; d < DS_PASSES; ++d) {
+      // the three 9-bit passes always run (the host fixes the final buffer before it knows the digits); the top digit's
+      // only if preprocess saw a key of 2^27 or beyond in the class
+      const uint32_t skip = d < 3 ? 0u : ((BACK ? fc->top_back : fc->top_front) ? 0u : 1u);
+      ctl->skip[d] = skip;
+      ctl->in_side[d] = side;
+      side ^= skip ^ 1u;
+    }
+    ctl->final_side = side;
+  }
+}
+
+// LOOP: the launch is smaller than the number of tiles (which only the device knows: ctl->survivors); its CTAs take
+// tickets until the pairs run out. only_if (LOOP): nothing to do when *only_if == 0.
+template <int THREADS, int ITEMS, int BITS, int MINB, bool FIRST, bool LOOP>
 __global__ void __launch_bounds__(THREADS, MINB)
 depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, uint64_t* __restrict__ keys_b,
                   uint32_t* __restrict__ vals_b, uint32_t n /* pairs in buffer a (FIRST) */, int pass, int shift,
                   const DepthCtl* __restrict__ ctl, const uint32_t* __restrict__ hist_excl /* [512] this pass */,
-                  uint64_t* __restrict__ lookback /* [tiles][1 << BITS], zeroed */, uint32_t* __restrict__ ticket /* zeroed */) {
+                  uint64_t* __restrict__ lookback /* [tiles][1 << BITS], zeroed */, uint32_t* __restrict__ ticket /* zeroed */,
+                  const uint32_t* __restrict__ only_if) {
   pdl_launch_dependents();
   pdl_wait();
+  if (LOOP && only_if && *only_if == 0u) return;
   using Core = RadixCore<THREADS, ITEMS, BITS>;
   constexpr int TILE = Core::TILE;
   constexpr uint32_t MASK = (1u << BITS) - 1u;
@@ -404,6 +621,7 @@ depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, 
   uint64_t* keys_out = from_a ? keys_b : keys_a;
   uint32_t* vals_out = from_a ? vals_b : vals_a;
 
+  do {
   const uint32_t tile = Core::take_ticket(s.core, ticket);
   const uint32_t tile_base = tile * TILE;
   if (tile_base >= n) return;   // launched for n pairs, S are left: nobody looks back at a tile past the end
@@ -427,7 +645,7 @@ depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, 
     // the culled Gaussians (and the padding of the last tile) carry 0xFFFFFFFF: no element
     dp[j] = w == 0xFFFFFFFFu ? Core::INVALID : ((w >> shift) & MASK);
   }
-  Core::template rank<true>(s.core, tile, dp, hist_excl, lookback);
+  Core::template rank<true, (LOOP && ITEMS <= 4) ? 16 : PVG_LB_WINDOW>(s.core, tile, dp, hist_excl, lookback);
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j)
     if (dp[j] != Core::INVALID) {
@@ -442,6 +660,8 @@ depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, 
     keys_out[o] = k;
     vals_out[o] = s.vals[p];
   }
+  if (LOOP) __syncthreads();   // the next tile reuses the shared memory
+  } while (LOOP);
 }
 
 // ---- digit pass over the compact instance payload -----------------------------------------

@@ -64,7 +64,7 @@ __device__ __forceinline__ double sinpi_reduced(double x) {
 // colour here. PRE_REC -- recompute the same values and write the record only (shade_kernel).
 enum { PRE_ALL = 0, PRE_GEO = 1, PRE_REC = 2 };
 template <int PART>
-__device__ __forceinline__ uint32_t
+__device__ __forceinline__ uint64_t
 preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __restrict__ shflag,
                  const float4* __restrict__ A0, const float4* __restrict__ A1,
                  const float4* __restrict__ A2, const float4* __restrict__ A3,
@@ -280,7 +280,7 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
     record[3 * (size_t)i + 1] = r1;
     record[3 * (size_t)i + 2] = r2;
   }
-  if (PART == PRE_REC) return valid ? ti.z : 0xFFFFFFFFu;
+  if (PART == PRE_REC) return valid ? (uint64_t)ti.z : 0xFFFFFFFFull;
   tileinfo[i] = ti;
   counts[i] = ti.w;
   if (dkeys) {
@@ -291,10 +291,12 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
       const uint32_t x0 = ti.x & 0xFFFFu, y0 = ti.x >> 16;
       rect = x0 | (y0 << 8) | ((x0 + (ti.y & 0xFFFFu) - 1u) << 16) | ((y0 + (ti.y >> 16) - 1u) << 24);
     }
-    dkeys[i] = valid ? (((uint64_t)rect << 32) | (ti.z - __float_as_uint(P.znear))) : 0xFFFFFFFFull;
+    const uint64_t key = valid ? (((uint64_t)rect << 32) | (ti.z - __float_as_uint(P.znear))) : 0xFFFFFFFFull;
+    dkeys[i] = key;
     (void)dvals;   // the value of pair i is i: the first pass of the depth sort forms it instead of loading it
+    return key;
   }
-  return valid ? ti.z - __float_as_uint(P.znear) : 0xFFFFFFFFu;
+  return valid ? (uint64_t)(ti.z - __float_as_uint(P.znear)) : 0xFFFFFFFFull;
 }
 
 // PRE_CHUNKS consecutive groups of 256 Gaussians per CTA. With dhist != nullptr the CTA also counts the four digits
@@ -307,12 +309,12 @@ preprocess_point(const FrameParams& P, uint32_t n, uint32_t i, const uint8_t* __
 #define PVG_PRE_CHUNKS 4
 #endif
 constexpr int PRE_CHUNKS = PVG_PRE_CHUNKS;
-constexpr int DH_COUNTER = DS_PASSES * DS_RADIX;   // u32 index of the CTA counter inside a dhist half
-constexpr int DH_CTL = DH_COUNTER + 8;             // u32 index of the DepthCtl block (8-byte aligned)
-constexpr int DH_WORDS = DH_CTL + 16;              // words per dhist half (a multiple of 4)
-static_assert(sizeof(DepthCtl) <= 16 * 4, "DepthCtl fits its slot");
 
-template <int PART>
+// FRONT (lazy lists with the front-first depth order, onesweep.cuh): instead of the digits the CTA counts, per bucket
+// of the top key bits (key >> FR_SHIFT), its survivors and their block entries, and sums their tile instances; the last
+// CTA picks the key threshold below which the first slab's owners lie (FrontCtl) and hands the frame's totals to the
+// host: M, Mb, S, F -- all the host waits for.
+template <int PART, bool FRONT>
 __global__ void __launch_bounds__(256)
 preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8_t* __restrict__ shflag,
                   const float4* __restrict__ A0, const float4* __restrict__ A1,
@@ -320,21 +322,33 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
                   const float4* __restrict__ SH, float4* __restrict__ record,
                   uint4* __restrict__ tileinfo, uint32_t* __restrict__ counts,
                   uint64_t* __restrict__ dkeys, uint32_t* __restrict__ dvals, float* __restrict__ featw,
-                  uint32_t* __restrict__ dhist, volatile uint64_t* __restrict__ host_words /* mapped: [4] = S, [5] = final side, [6] = skipped passes (bit p) */) {
+                  uint32_t* __restrict__ dhist, volatile uint64_t* __restrict__ host_words /* mapped: [4] = S, [5] = final side, [6] = skipped passes (bit p); FRONT: [0] = M, [1] = Mb, [4] = S, [8] = F, [9] = top-digit flags */) {
   __shared__ uint32_t s_hist[DS_PASSES * DS_RADIX];
+  static_assert(2 * FR_BUCKETS == DS_PASSES * DS_RADIX, "the bucket histograms reuse the digit histograms' words");
   if (dhist) {
 #pragma unroll
     for (int k = 0; k < DS_PASSES * DS_RADIX / 256; ++k) s_hist[k * 256 + threadIdx.x] = 0;
     __syncthreads();
   }
+  uint32_t inst = 0;   // FRONT: tile instances of this thread's survivors
 #pragma unroll 1
   for (int c = 0; c < PRE_CHUNKS; ++c) {
     const uint32_t i = (blockIdx.x * PRE_CHUNKS + c) * 256u + threadIdx.x;
     if (i >= n) break;
-    const uint32_t z = preprocess_point<PART>(P, n, i, shflag, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
+    const uint64_t key = preprocess_point<PART>(P, n, i, shflag, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
+    const uint32_t z = (uint32_t)key;
     if (dhist && z != 0xFFFFFFFFu) {
+      if (FRONT) {
+        const uint32_t r = (uint32_t)(key >> 32);
+        const uint32_t x0 = r & 0xFFu, y0 = (r >> 8) & 0xFFu, x1 = (r >> 16) & 0xFFu, y1 = r >> 24;
+        const uint32_t b = min(z >> FR_SHIFT, (uint32_t)FR_BUCKETS - 1u);
+        atomicAdd(&s_hist[b], 1u);
+        atomicAdd(&s_hist[FR_BUCKETS + b], ((x1 >> 3) - (x0 >> 3) + 1u) * ((y1 >> 3) - (y0 >> 3) + 1u));
+        inst += (x1 - x0 + 1u) * (y1 - y0 + 1u);
+      } else {
 #pragma unroll
-      for (int k = 0; k < DS_PASSES; ++k) atomicAdd(&s_hist[k * DS_RADIX + ((z >> ds_shift(k)) & ((1u << ds_bits(k)) - 1u))], 1u);
+        for (int k = 0; k < DS_PASSES; ++k) atomicAdd(&s_hist[k * DS_RADIX + ((z >> ds_shift(k)) & ((1u << ds_bits(k)) - 1u))], 1u);
+      }
     }
   }
   if (!dhist) return;
@@ -346,6 +360,10 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
   }
   __shared__ bool s_last;
   __shared__ uint32_t s_warp[8], s_bins[8];
+  if (FRONT) {
+    inst = __reduce_add_sync(0xffffffffu, inst);   // < 2^32: 32 Gaussians of at most 2^16 tiles each
+    if ((threadIdx.x & 31u) == 0 && inst) atomicAdd(reinterpret_cast<unsigned long long*>(dhist + DH_COUNTER + 2), (unsigned long long)inst);
+  }
   // release: the barrier orders every thread's histogram atomics before thread 0, whose (cumulative) fence orders them
   // before its count -- one fence per CTA instead of one per thread (ncu: 1.1 stall cycles per issued instruction)
   __syncthreads();
@@ -357,6 +375,72 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
   if (!s_last) return;
   __threadfence();
   const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  if (FRONT) {
+    // thread t owns buckets 4 t .. 4 t + 3; inclusive sums of the survivors and of their block entries over the buckets
+    __shared__ unsigned long long s_ent[8];
+    uint32_t c[4], e[4];
+    uint32_t csum = 0;
+    unsigned long long esum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      c[k] = __ldcg(dhist + 4 * threadIdx.x + k);
+      e[k] = __ldcg(dhist + FR_BUCKETS + 4 * threadIdx.x + k);
+      csum += c[k]; esum += e[k];
+    }
+    uint32_t cin = csum;
+    unsigned long long ein = esum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t tc = __shfl_up_sync(0xffffffffu, cin, d);
+      const unsigned long long te = __shfl_up_sync(0xffffffffu, ein, d);
+      if (lane >= d) { cin += tc; ein += te; }
+    }
+    if (lane == 31) { s_warp[warp] = cin; s_ent[warp] = ein; }
+    __syncthreads();
+    uint32_t cex = 0, S = 0;
+    unsigned long long eex = 0, Mb = 0;
+    for (uint32_t w = 0; w < 8; ++w) {
+      if (w < warp) { cex += s_warp[w]; eex += s_ent[w]; }
+      S += s_warp[w]; Mb += s_ent[w];
+    }
+    cex += cin - csum; eex += ein - esum;   // exclusive of this thread's four buckets
+    // the first slab: bin_emit's first launch forms the entries [0, emit_first * BF_TILE), and shade_kernel asks for
+    // the owner of entry emit_first * BF_TILE: the front must hold more entries than that
+    const unsigned long long target = ((unsigned long long)lazy_emit_first(Mb, P.lazy_slab) + 1ull) * (unsigned long long)PVG_EMIT_TILE;
+    __shared__ uint32_t s_thr, s_front;
+    if (threadIdx.x == 0) { s_thr = 0xFFFFFFFFu; s_front = S; }
+    __syncthreads();
+    if (Mb > target) {
+      // the one bucket at which the inclusive entry sum first reaches the target
+      unsigned long long run = eex;
+      uint32_t crun = cex;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const unsigned long long before = run;
+        run += e[k]; crun += c[k];
+        const uint32_t b = 4 * threadIdx.x + k;
+        if (before < target && run >= target && b + 1 < (uint32_t)FR_TOP) { s_thr = (b + 1u) << FR_SHIFT; s_front = crun; }
+      }
+    }
+    // keys of 2^27 and beyond (buckets FR_TOP ..): which class has them decides its top-digit pass
+    uint32_t far = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) if (4 * threadIdx.x + k >= (uint32_t)FR_TOP) far += c[k];
+    far = __syncthreads_or(far != 0u);
+    if (threadIdx.x == 0) {
+      FrontCtl* fc = reinterpret_cast<FrontCtl*>(dhist + DH_CTL);
+      const uint32_t thr = s_thr, F = s_front;
+      fc->survivors = S; fc->front = F; fc->thr = thr;
+      fc->top_front = (thr == 0xFFFFFFFFu && far) ? 1u : 0u;
+      fc->top_back = (thr != 0xFFFFFFFFu && far) ? 1u : 0u;
+      const unsigned long long M = *reinterpret_cast<const volatile unsigned long long*>(dhist + DH_COUNTER + 2);
+      if (host_words) {
+        host_words[0] = M; host_words[1] = Mb; host_words[4] = S; host_words[8] = F;
+        host_words[9] = fc->top_front | (fc->top_back << 1);
+      }
+    }
+    return;
+  }
   uint32_t nonempty[DS_PASSES], total = 0;
   for (int k = 0; k < DS_PASSES; ++k) {
     // thread t owns bins 2 t, 2 t + 1 of the digit's 512
@@ -416,6 +500,18 @@ shade_kernel(const __grid_constant__ FrameParams P, uint32_t n, uint32_t nv, con
   const uint32_t r = lo + blockIdx.x * 256u + threadIdx.x;
   if (r >= hi) return;
   preprocess_point<PRE_REC>(P, n, visit[r], nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
+}
+
+// The records of the Gaussians in a device-side list (front-first depth order: the front, as depth_select_kernel
+// compacted it -- in index order, before it is sorted: the records do not depend on the order, so this runs beside
+// the sort on a stream of its own). *count entries; grid-stride, the launch does not know the count.
+__global__ void __launch_bounds__(256)
+shade_list_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint32_t* __restrict__ count, const uint32_t* __restrict__ list,
+                  const float4* __restrict__ A0, const float4* __restrict__ A1, const float4* __restrict__ A2,
+                  const float4* __restrict__ A3, const float4* __restrict__ SH, float4* __restrict__ record, float* __restrict__ featw) {
+  const uint32_t c = *count;
+  for (uint32_t r = blockIdx.x * 256u + threadIdx.x; r < c; r += gridDim.x * 256u)
+    preprocess_point<PRE_REC>(P, n, list[r], nullptr, A0, A1, A2, A3, SH, record, nullptr, nullptr, nullptr, nullptr, featw);
 }
 
 // The records of ALL Gaussians in index order (coalesced model reads: 4 x faster than the gather by depth rank when

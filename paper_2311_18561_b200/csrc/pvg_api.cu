@@ -361,11 +361,6 @@ int run_onesweep(const Dev& dv, uint64_t n, uint64_t* ka, uint32_t* va, uint64_t
 }
 
 // ---- the depth sort of the Gaussians (onesweep.cuh: 9 + 9 + 9 + 4 bits, pass 0 drops the culled pairs) ----------
-#ifndef PVG_DS_THREADS
-#define PVG_DS_THREADS 512
-#define PVG_DS_ITEMS 8
-#define PVG_DS_MINB 2
-#endif
 struct DsCfg { static constexpr int THREADS = PVG_DS_THREADS, ITEMS = PVG_DS_ITEMS, MINB = PVG_DS_MINB; };
 constexpr uint32_t kDsTile = DsCfg::THREADS * DsCfg::ITEMS;
 
@@ -374,23 +369,47 @@ inline size_t depth_lookback_words(uint32_t n) {
   return tiles * (size_t)(3 * DS_RADIX + (1 << DS_TOP_BITS));
 }
 
+// The front of a front-first frame is small (tens of thousands of pairs): its passes run on small tiles, so that the
+// few tiles spread over many SMs and a tile's latency -- which is all a pass costs at that size -- is short.
+#ifndef PVG_DSF_THREADS
+#define PVG_DSF_THREADS 512
+#define PVG_DSF_ITEMS 2
+#define PVG_DSF_MINB 2
+#endif
+struct DsFrontCfg { static constexpr int THREADS = PVG_DSF_THREADS, ITEMS = PVG_DSF_ITEMS, MINB = PVG_DSF_MINB; };
+constexpr uint32_t kDsFrontTile = DsFrontCfg::THREADS * DsFrontCfg::ITEMS;
+inline size_t class_lookback_rows(uint32_t n, int cls) { const uint32_t t = cls ? kDsTile : kDsFrontTile; return (n + t - 1) / t; }
+inline size_t class_lookback_words(uint32_t n, int cls) { return class_lookback_rows(n, cls) * (size_t)(3 * DS_RADIX + (1 << DS_TOP_BITS)); }
+
 // sizes and zeroes the tickets and look-back words of the four passes on stream zs
-int prep_depth_sort(uint32_t n, cudaStream_t alloc_st, cudaStream_t zs, SortScratch& sc) {
+// front_first: the front's passes and the back's have their own tickets (0..3 / 4..7) and look-back words, and
+// depth_select_kernel zeroes the words its class will use (it knows how many pairs there are)
+int prep_depth_sort(uint32_t n, cudaStream_t alloc_st, cudaStream_t zs, SortScratch& sc, bool front_first = false) {
+  static_assert(OS_MAX_PASSES >= 2 * DS_PASSES, "tickets of two classes");
   TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, alloc_st));
-  TRY(sc.lookback.reserve(depth_lookback_words(n) * 8, alloc_st, 1.25));
   CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, zs));
-  CU(cudaMemsetAsync(sc.lookback.p, 0, depth_lookback_words(n) * 8, zs));
+  if (front_first) {
+    TRY(sc.lookback.reserve((class_lookback_words(n, 0) + class_lookback_words(n, 1)) * 8, alloc_st, 1.25));
+  } else {
+    TRY(sc.lookback.reserve(depth_lookback_words(n) * 8, alloc_st, 1.25));
+    CU(cudaMemsetAsync(sc.lookback.p, 0, depth_lookback_words(n) * 8, zs));
+  }
   return PVG_OK;
 }
 
-template <int BITS, bool FIRST>
+// loop_ctas > 0: a launch of at most that many CTAs that loop over tickets (the number of pairs is on the device)
+template <int BITS, bool FIRST, bool LOOP = false, class Cfg = DsCfg>
 int launch_depth_pass(uint64_t* ka, uint32_t* va, uint64_t* kb, uint32_t* vb, uint32_t n, int pass, const DepthCtl* ctl,
-                      const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev, Timer* tm) {
-  using Smem = OnesweepSmem<DsCfg::THREADS, DsCfg::ITEMS, BITS>;
-  auto kern = depth_pass_kernel<DsCfg::THREADS, DsCfg::ITEMS, BITS, DsCfg::MINB, FIRST>;
+                      const uint32_t* hist, uint64_t* lookback, uint32_t* ticket, cudaStream_t st, int dev, Timer* tm,
+                      unsigned loop_ctas = 0, const uint32_t* only_if = nullptr) {
+  using Smem = OnesweepSmem<Cfg::THREADS, Cfg::ITEMS, BITS>;
+  auto kern = depth_pass_kernel<Cfg::THREADS, Cfg::ITEMS, BITS, Cfg::MINB, FIRST, LOOP>;
   PVG_ENSURE_SMEM(kern, sizeof(Smem), dev);
-  return launch_chain(tm, kern, dim3((n + kDsTile - 1) / kDsTile), dim3(DsCfg::THREADS), sizeof(Smem), st, ka, va, kb, vb, n, pass,
-                      ds_shift(pass), ctl, hist, lookback, ticket);
+  constexpr uint32_t TILE = Cfg::THREADS * Cfg::ITEMS;
+  unsigned grid = (n + TILE - 1) / TILE;
+  if (LOOP) grid = std::max(1u, std::min(grid, loop_ctas));
+  return launch_chain(tm, kern, dim3(grid), dim3(Cfg::THREADS), sizeof(Smem), st, ka, va, kb, vb, n, pass,
+                      ds_shift(pass), ctl, hist, lookback, ticket, only_if);
 }
 
 // dh: this frame's dhist half (exclusive digit prefixes + DepthCtl, written by preprocess). Every pass is launched
@@ -500,6 +519,15 @@ struct pvg_scene {
   int lazy_chunks = 2;                // PVG_OPT_LAZY_CHUNKS (0: always write the complete lists)
   int lazy_slab = 8;                  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front
   int exact_tiles = 0;                // PVG_OPT_EXACT_TILES: list a Gaussian only in the tiles its ellipse can reach (P13)
+  int lazy_depth = 1;                 // PVG_OPT_LAZY_DEPTH: with lazy lists, order the front of the scene first (onesweep.cuh)
+  bool front_used = false;            // the last frame ordered its front first
+  bool depth_complete = true;         // dvals[visit_side] holds all S survivors in depth order (pvg_debug_view completes it)
+  uint32_t front = 0;                 // F: the pairs in front of the threshold
+  int top_front = 0, top_back = 0;    // the class has keys of 2^27 and beyond
+  Buf front_idx;                      // front-first: the front's Gaussian indices once more, for shade_list_kernel
+  Buf okeys;                          // front-first: the n depth pairs of preprocess, index order (the sort's buffers ping-pong)
+  Buf dsel;                           // front-first: 2 histogram regions (front, back) + 2 tickets
+  Buf sel_status;                     // front-first: 2 x [tiles] look-back words of depth_select_kernel
   bool exact_used = false;            // the last frame built exact lists
   Buf tile_count, counts_exact;       // exact lists: per-tile and per-Gaussian counts of the refined masks
   uint32_t emit_first = 0, emit_tiles = 0, emit_radix = 256;   // bin_emit tiles in the first launch / in all; its look-back row length
@@ -538,7 +566,9 @@ struct pvg_scene {
   uint64_t* h_total = nullptr;  // pinned, mapped
   uint64_t* d_total = nullptr;  // device alias of h_total (tile_prefix_kernel stores the totals through it)
   cudaStream_t side = nullptr;  // tile grid + prefix run here, beside the depth sort
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_start = nullptr, ev_zero = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_start = nullptr, ev_zero = nullptr, ev_pre = nullptr;
+  cudaStream_t aux = nullptr;   // front-first: the front's records are formed here, beside the sort and the tile grid
+  cudaEvent_t ev_sel = nullptr, ev_aux = nullptr;
   Timer timer;
   // last frame
   uint64_t M = 0, Mb = 0, survivors = 0;
@@ -568,7 +598,7 @@ void release_all(pvg_scene* s) {
                  &s->dkeys[0], &s->dkeys[1], &s->dvals[0], &s->dvals[1], &s->scan_status, &s->small,
                  &s->keys[0], &s->keys[1], &s->vals[0], &s->vals[1], &s->keys_unsorted, &s->vals_unsorted, &s->tiles16[0], &s->tiles16[1], &s->tiles16_unsorted,
                  &s->lazy_state, &s->unf, &s->dhist, &s->boffsets, &s->chunk_owner, &s->e_bin, &s->e_g, &s->e_mask, &s->s_g, &s->s_mask, &s->bin_tables, &s->chunk_cnt,
-                 &s->tile_count, &s->counts_exact, &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
+                 &s->tile_count, &s->counts_exact, &s->okeys, &s->front_idx, &s->dsel, &s->sel_status, &s->ranges, &s->tilegrid, &s->featw, &s->sky, &s->img[0], &s->img[1], &s->sort_n.hist, &s->sort_n.lookback, &s->sort_n.tickets,
                  &s->sort_m.hist, &s->sort_m.lookback, &s->sort_m.tickets};
   for (Buf* b : bufs) b->release();
   if (s->h_total) cudaFreeHost(s->h_total);
@@ -579,6 +609,13 @@ void release_all(pvg_scene* s) {
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->ev_start) cudaEventDestroy(s->ev_start);
   if (s->ev_zero) cudaEventDestroy(s->ev_zero);
+  if (s->ev_pre) cudaEventDestroy(s->ev_pre);
+  s->ev_pre = nullptr;
+  if (s->ev_sel) cudaEventDestroy(s->ev_sel);
+  if (s->ev_aux) cudaEventDestroy(s->ev_aux);
+  s->ev_sel = s->ev_aux = nullptr;
+  if (s->aux) cudaStreamDestroy(s->aux);
+  s->aux = nullptr;
   s->ev_start = s->ev_zero = nullptr;
   if (s->side) cudaStreamDestroy(s->side);
   if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
@@ -650,19 +687,23 @@ int init_workspace(pvg_scene* s) {
   auto rs = [&](Buf& b, size_t bytes) { if (rc == PVG_OK) rc = b.reserve(bytes, st); };
   rs(s->record, n * 48); rs(s->tileinfo, n * 16); rs(s->counts, n * 4); rs(s->offsets, n * 4); rs(s->boffsets, n * 4);
   rs(s->dkeys[0], n * 8); rs(s->dkeys[1], n * 8); rs(s->dvals[0], n * 4); rs(s->dvals[1], n * 4);
-  rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 8); rs(s->small, 256);
+  rs(s->scan_status, ((n + SCAN_TILE - 1) / SCAN_TILE) * 16); rs(s->small, 256);
   rs(s->dhist, 2 * kDhistWords * 4);
   if (rc != PVG_OK) return rc;
   CU(cudaMemsetAsync(s->dhist.p, 0, 2 * kDhistWords * 4, st));
   CU(cudaStreamSynchronize(st));   // the first render may run on another stream: the zeroes must have landed
   CU(cudaEventCreateWithFlags(&s->ev_switch, cudaEventDisableTiming));
-  CU(cudaHostAlloc((void**)&s->h_total, 64, cudaHostAllocMapped));
+  CU(cudaHostAlloc((void**)&s->h_total, 128, cudaHostAllocMapped));
   CU(cudaHostGetDevicePointer((void**)&s->d_total, s->h_total, 0));
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_start, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_zero, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_pre, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_sel, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_aux, cudaEventDisableTiming));
+  CU(cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking));
   CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_rendered, cudaEventDisableTiming));
   for (int k = 0; k < 2; ++k) CU(cudaEventCreateWithFlags(&s->ev_copied[k], cudaEventDisableTiming));
@@ -715,6 +756,7 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   for (int j = 0; j < 3; ++j) P->bg[j] = cam->bg[j];
   P->sky = s->sky_res > 0 ? s->sky.as<float>() : nullptr;
   P->sky_res = s->sky_res;
+  P->lazy_slab = s->lazy_slab;
   return PVG_OK;
 }
 
@@ -726,16 +768,21 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
 constexpr uint32_t kOwnerChunk = PVG_BIN_FUSED ? (uint32_t)BF_TILE : (uint32_t)BE_CHUNK;   // granularity of chunk_owner[]
 
 // a2 scan of the per-Gaussian item counts in visiting order; the total lands in small @8.
+// (the status words are there twice, and a second ticket and total at small @96 / @104: the front-first depth order
+// scans the back of the visiting order in a launch of its own)
 int prep_scan(pvg_scene* s, cudaStream_t zs) {
   const uint32_t scan_tiles = (s->n + SCAN_TILE - 1) / SCAN_TILE;
-  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 8, zs));
+  CU(cudaMemsetAsync(s->scan_status.p, 0, (size_t)scan_tiles * 16, zs));
   CU(cudaMemsetAsync(s->small.p, 0, 16, zs));
+  CU(cudaMemsetAsync(s->small.as<unsigned char>() + 96, 0, 16, zs));
   return PVG_OK;
 }
 
 // nv: the first nv visiting positions are scanned (the survivors after the depth sort; n otherwise)
+// rank0 > 0 (blocks only): the second part of a front-first frame -- positions [rank0, rank0 + nv), continuing from the
+// total the first part left; only_if: a device word, nothing happens when it is 0
 int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32_t* visit, Timer* tm, bool scratch_ready = false,
-             const uint32_t* counts = nullptr /* default: the rectangle counts */) {
+             const uint32_t* counts = nullptr /* default: the rectangle counts */, uint32_t rank0 = 0, const uint32_t* only_if = nullptr) {
   cudaStream_t st = s->stream;
   const uint32_t n = nv;
   if (n == 0) return PVG_OK;
@@ -744,18 +791,106 @@ int run_scan(pvg_scene* s, uint32_t nv, bool blocks, uint32_t* out, const uint32
     TRY(prep_scan(s, st));
     if (tm) tm->cut();
   }
-  uint32_t* ticket = s->small.as<uint32_t>();
+  const bool second = rank0 > 0;
+  uint32_t* ticket = reinterpret_cast<uint32_t*>(s->small.as<unsigned char>() + (second ? 96 : 0));
   uint64_t* total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8);
+  uint64_t* total_out = second ? reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 104) : total;
+  uint64_t* status = s->scan_status.as<uint64_t>() + (second ? (s->n + SCAN_TILE - 1) / SCAN_TILE : 0);
   if (tm) TRY(tm->begin("scan_counts", PVG_STAGE_DUPLICATE, st));
   if (blocks)
     TRY(launch_chain(tm, scan_counts_kernel<true>, dim3(scan_tiles), dim3(SCAN_THREADS), 0, st, n, s->counts.as<uint32_t>(),
-                     s->dkeys[s->visit_side].as<uint64_t>(), visit, out, total, s->scan_status.as<uint64_t>(), ticket,
-                     s->chunk_owner.as<uint32_t>(), kOwnerChunk));
+                     s->dkeys[s->visit_side].as<uint64_t>(), visit, out, total_out, status, ticket,
+                     s->chunk_owner.as<uint32_t>(), kOwnerChunk, rank0, second ? total : (uint64_t*)nullptr, only_if));
   else
     TRY(launch_chain(tm, scan_counts_kernel<false>, dim3(scan_tiles), dim3(SCAN_THREADS), 0, st, n,
                      counts ? counts : s->counts.as<uint32_t>(), (const uint64_t*)nullptr, visit, out, total,
-                     s->scan_status.as<uint64_t>(), ticket, (uint32_t*)nullptr, 0u));
+                     s->scan_status.as<uint64_t>(), ticket, (uint32_t*)nullptr, 0u, 0u, (const uint64_t*)nullptr, (const uint32_t*)nullptr));
   if (tm) TRY(tm->end(st));
+  return PVG_OK;
+}
+
+// ---- front-first depth order (onesweep.cuh, PVG_OPT_LAZY_DEPTH) ---------------------------------------------------
+// dsel (u32 words): the front's histogram region, the back's, two tickets of depth_select_kernel
+constexpr size_t kDselWords = 2 * (size_t)DH_WORDS + 4;
+inline uint32_t sel_tiles(uint32_t n) { return (n + SEL_TILE - 1) / SEL_TILE; }
+
+// sizes the scratch of a front-first frame and zeroes it on stream zs
+int prep_front(pvg_scene* s, cudaStream_t zs) {
+  cudaStream_t st = s->stream;
+  TRY(s->okeys.reserve((size_t)s->n * 8, st));
+  TRY(s->front_idx.reserve((size_t)s->n * 4, st));
+  TRY(s->dsel.reserve(kDselWords * 4, st));
+  TRY(s->sel_status.reserve((size_t)2 * sel_tiles(s->n) * 8, st));
+  CU(cudaMemsetAsync(s->dsel.p, 0, kDselWords * 4, zs));
+  CU(cudaMemsetAsync(s->sel_status.p, 0, (size_t)2 * sel_tiles(s->n) * 8, zs));
+  return PVG_OK;
+}
+
+// cls 0: the pairs below the threshold, to positions [0, F) of buffer pair 1; cls 1: the others, to [F, S) of the pair
+// from which the back's passes end in the buffer the front ended in.
+int back_out_side(const pvg_scene* s) { return s->visit_side ^ ((3 + s->top_back) & 1); }
+int run_depth_select(pvg_scene* s, int cls, const uint32_t* only_if, Timer* tm) {
+  cudaStream_t st = s->stream;
+  const uint32_t* dh = s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords;
+  const FrontCtl* fc = reinterpret_cast<const FrontCtl*>(dh + DH_CTL);
+  uint32_t* region = s->dsel.as<uint32_t>() + (size_t)cls * DH_WORDS;
+  uint64_t* status = s->sel_status.as<uint64_t>() + (size_t)cls * sel_tiles(s->n);
+  uint32_t* ticket = s->dsel.as<uint32_t>() + 2 * (size_t)DH_WORDS + cls;
+  const int out_side = cls ? back_out_side(s) : 1;
+  uint64_t* lb = s->sort_n.lookback.as<uint64_t>() + (cls ? class_lookback_words(s->n, 0) : 0);
+  const uint32_t lb_rows = (uint32_t)class_lookback_rows(s->n, cls), lb_tile = cls ? kDsTile : kDsFrontTile;
+  if (tm) TRY(tm->begin("depth_select", PVG_STAGE_DEPTH_SORT, st));
+  if (cls)
+    TRY(launch_chain(tm, depth_select_kernel<true>, dim3(sel_tiles(s->n)), dim3(SEL_THREADS), 0, st, s->okeys.as<uint64_t>(), s->n, fc,
+                     s->dkeys[out_side].as<uint64_t>(), s->dvals[out_side].as<uint32_t>(), (uint32_t*)nullptr, region, status, ticket,
+                     (uint32_t)out_side, lb, lb_rows, lb_tile, only_if));
+  else
+    TRY(launch_chain(tm, depth_select_kernel<false>, dim3(sel_tiles(s->n)), dim3(SEL_THREADS), 0, st, s->okeys.as<uint64_t>(), s->n, fc,
+                     s->dkeys[out_side].as<uint64_t>(), s->dvals[out_side].as<uint32_t>(), s->front_idx.as<uint32_t>(), region, status, ticket,
+                     (uint32_t)out_side, lb, lb_rows, lb_tile, only_if));
+  if (tm) TRY(tm->end(st));
+  return PVG_OK;
+}
+
+// passes [p0, p1) over one class: small launches whose CTAs loop over tickets (the class's size is in its control block)
+// count: an upper bound of the class's pairs known to the host (n before it has read F)
+int run_class_passes(pvg_scene* s, int cls, uint32_t count, int p0, int p1, const uint32_t* only_if, Timer* tm) {
+  cudaStream_t st = s->stream;
+  const uint32_t* region = s->dsel.as<uint32_t>() + (size_t)cls * DH_WORDS;
+  const DepthCtl* ctl = reinterpret_cast<const DepthCtl*>(region + DH_CTL);
+  const size_t base = cls ? s->front : 0u;
+  const size_t tiles = class_lookback_rows(s->n, cls);
+  uint64_t* lb = s->sort_n.lookback.as<uint64_t>() + (cls ? class_lookback_words(s->n, 0) : 0);
+  uint32_t* tk = s->sort_n.tickets.as<uint32_t>() + cls * DS_PASSES;
+  uint64_t* ka = s->dkeys[0].as<uint64_t>() + base; uint32_t* va = s->dvals[0].as<uint32_t>() + base;
+  uint64_t* kb = s->dkeys[1].as<uint64_t>() + base; uint32_t* vb = s->dvals[1].as<uint32_t>() + base;
+  const unsigned ctas = (unsigned)s->dev.sms * (unsigned)DsCfg::MINB;
+  for (int p = 0; p < p0; ++p) lb += tiles * (size_t)(1 << ds_bits(p));
+  for (int p = p0; p < p1; ++p) {
+    if (tm) TRY(tm->begin("onesweep_pass", PVG_STAGE_DEPTH_SORT, st));
+    const uint32_t* hist = region + p * DS_RADIX;
+    if (cls == 0) {
+      const unsigned fctas = (unsigned)s->dev.sms * (unsigned)DsFrontCfg::MINB;
+      if (p < 3) TRY((launch_depth_pass<DS_BITS, false, true, DsFrontCfg>(ka, va, kb, vb, count, p, ctl, hist, lb, tk + p, st, s->dev.ordinal, tm, fctas, only_if)));
+      else TRY((launch_depth_pass<DS_TOP_BITS, false, true, DsFrontCfg>(ka, va, kb, vb, count, p, ctl, hist, lb, tk + p, st, s->dev.ordinal, tm, fctas, only_if)));
+    } else if (p < 3) TRY((launch_depth_pass<DS_BITS, false, true>(ka, va, kb, vb, count, p, ctl, hist, lb, tk + p, st, s->dev.ordinal, tm, ctas, only_if)));
+    else TRY((launch_depth_pass<DS_TOP_BITS, false, true>(ka, va, kb, vb, count, p, ctl, hist, lb, tk + p, st, s->dev.ordinal, tm, ctas, only_if)));
+    if (tm) TRY(tm->end(st));
+    lb += tiles * (size_t)(1 << ds_bits(p));
+  }
+  CU(cudaGetLastError());
+  return PVG_OK;
+}
+
+// The back of a front-first frame: the pairs at and beyond the threshold, selected, ordered behind the front and
+// scanned (block entries, continuing the front's offsets). only_if: the parked-tile count (second round) or nullptr.
+int run_depth_back(pvg_scene* s, const uint32_t* only_if, Timer* tm) {
+  const uint32_t S = (uint32_t)s->survivors, F = s->front;
+  if (F >= S) return PVG_OK;
+  TRY(run_depth_select(s, 1, only_if, tm));
+  TRY(run_class_passes(s, 1, S - F, 0, s->top_back ? 4 : 3, only_if, tm));
+  const uint32_t* visit = s->dvals[s->visit_side].as<uint32_t>();
+  TRY(run_scan(s, S - F, true, s->boffsets.as<uint32_t>(), visit, tm, true, nullptr, F, only_if));
   return PVG_OK;
 }
 
@@ -912,11 +1047,11 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   // the first blend phase parks a tile
   s->lazy_used = s->lazy_chunks > 0 && !s->exact_used;   // exact lists are counted: every entry is formed and refined
   const uint32_t emit_tiles = (Mb + BF_TILE - 1) / BF_TILE;
-  s->emit_first = s->lazy_used ? std::min(emit_tiles, std::max(1u, (emit_tiles + (uint32_t)s->lazy_slab - 1) / (uint32_t)s->lazy_slab)) : emit_tiles;
+  s->emit_first = s->lazy_used ? lazy_emit_first(Mb, s->lazy_slab) : emit_tiles;
   s->emit_tiles = emit_tiles;
   s->emit_radix = 1u << bits;
   s->visit_last = visit;
-  if (s->light) {
+  if (s->light && !s->front_used) {
     // the records of the Gaussians that own the first slab's entries (depth ranks 0 .. owner of the slab's end), on
     // the side stream: a latency-bound gather that overlaps the equally latency-bound bin_emit and bin_write
     cudaStream_t sd = s->side;
@@ -979,11 +1114,86 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(launch_bin_write(s, P, 0u, s->lazy_used ? (uint32_t)s->lazy_chunks : 0xFFFFFFFFu, false, 1));
   TRY(tm->end(st));
   if (s->light) {   // the blend reads the records
-    CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+    CU(cudaStreamWaitEvent(st, s->front_used ? s->ev_aux : s->ev_join, 0));
     tm->cut();
   }
   CU(cudaGetLastError());
   s->sorted_side = 0;
+  return PVG_OK;
+}
+
+// PVG_R2_TAIL=1: the second round of the lazy lists is launched from the device, by a one-thread gate kernel after the
+// first blend phase, only if a tile parked (round2.cu); 0: the host launches it every frame and each kernel looks at
+// the parked count.
+#ifndef PVG_R2_TAIL
+#define PVG_R2_TAIL 1
+#endif
+extern "C" int pvg_r2_gate(int device, void* stream, const void* params, const void* chain, const void* lazy, int which,
+                           const void* ranges, const void* vals, const void* record, float* out_rgb, float* out_depth,
+                           float* out_alpha, unsigned long long* counters, const float* featw);
+
+// The launches of the second round, described for r2_tail_launch: the same kernels, grids and arguments as the host
+// path further down (run_depth_back, run_shade_all, run_bin_emit, launch_bin_write, the second blend phase).
+int fill_r2(pvg_scene* s, const FrameParams& P, uint32_t band_tiles, R2Chain* out) {
+  R2Chain c = {};
+  const uint32_t S = (uint32_t)s->survivors, F = s->front, n = s->n;
+  const uint32_t sms = (uint32_t)s->dev.sms;
+  const bool more = s->emit_first < s->emit_tiles;
+  c.enabled = 1;
+  c.n = n;
+  c.counts = s->counts.as<uint32_t>();
+  c.visit = s->dvals[s->visit_side].as<uint32_t>();
+  c.scan_keys = s->dkeys[s->visit_side].as<uint64_t>();
+  c.boffsets = s->boffsets.as<uint32_t>();
+  c.chunk_owner = s->chunk_owner.as<uint32_t>();
+  c.back = (more && s->front_used && F < S) ? 1u : 0u;
+  if (c.back) {
+    const int side = back_out_side(s);
+    c.okeys = s->okeys.as<uint64_t>();
+    c.fc = reinterpret_cast<const FrontCtl*>(s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords + DH_CTL);
+    c.sel_keys = s->dkeys[side].as<uint64_t>(); c.sel_vals = s->dvals[side].as<uint32_t>();
+    c.sel_region = s->dsel.as<uint32_t>() + DH_WORDS;
+    c.sel_status = s->sel_status.as<uint64_t>() + sel_tiles(n);
+    c.sel_ticket = s->dsel.as<uint32_t>() + 2 * (size_t)DH_WORDS + 1;
+    c.sel_side = (uint32_t)side; c.sel_grid = sel_tiles(n);
+    c.lb = s->sort_n.lookback.as<uint64_t>() + class_lookback_words(n, 0);
+    c.lb_rows = (uint32_t)class_lookback_rows(n, 1); c.lb_tile = kDsTile;
+    c.ka = s->dkeys[0].as<uint64_t>() + F; c.va = s->dvals[0].as<uint32_t>() + F;
+    c.kb = s->dkeys[1].as<uint64_t>() + F; c.vb = s->dvals[1].as<uint32_t>() + F;
+    c.back_count = S - F; c.passes = s->top_back ? 4u : 3u;
+    c.pass_grid = std::max(1u, std::min((S - F + kDsTile - 1) / kDsTile, sms * (uint32_t)DsCfg::MINB));
+    c.pass_tickets = s->sort_n.tickets.as<uint32_t>() + DS_PASSES;
+    c.scan_grid = (S - F + SCAN_TILE - 1) / SCAN_TILE;
+    c.scan_total = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 104);
+    c.scan_init = reinterpret_cast<const uint64_t*>(s->small.as<unsigned char>() + 8);
+    c.scan_status = s->scan_status.as<uint64_t>() + (n + SCAN_TILE - 1) / SCAN_TILE;
+    c.scan_ticket = reinterpret_cast<uint32_t*>(s->small.as<unsigned char>() + 96);
+    c.owner_chunk = kOwnerChunk; c.rank0 = F;
+  }
+  const Model* m = s->model;
+  c.shade = (more && s->light) ? 1u : 0u;
+  c.shade_grid = std::min<uint32_t>((n + 255) / 256, sms * 8u);
+  c.A0 = m->A0.as<float4>(); c.A1 = m->A1.as<float4>(); c.A2 = m->A2.as<float4>(); c.A3 = m->A3.as<float4>(); c.SH = m->SH.as<float4>();
+  c.record = s->record.as<float4>(); c.featw = s->featw_last;
+  const uint32_t blocks_x = bb_blocks(P.tiles_x), nbins = blocks_x * bb_blocks(P.tiles_y);
+  const uint32_t Mb = (uint32_t)s->Mb;
+  c.emit = more ? 1u : 0u;
+  c.emit_grid = std::max(1u, std::min(s->emit_tiles - std::min(s->emit_tiles, s->emit_first), sms * (uint32_t)PVG_BP_MINB));
+  c.emit_bits = (uint32_t)std::max(1, ceil_log2(nbins));
+  c.nv = c.back ? S : s->nv; c.Mb = Mb; c.blocks_x = blocks_x; c.emit_tiles = s->emit_tiles;
+  c.s_g = s->s_g.as<uint32_t>(); c.s_mask = s->s_mask.as<uint64_t>(); c.bin_start = s->bin_tables.as<uint32_t>();
+  c.emit_lookback = s->sort_m.lookback.as<uint64_t>(); c.emit_ticket = s->sort_m.tickets.as<uint32_t>();
+  const uint32_t max_chunks = (Mb + BB_CHUNK - 1) / BB_CHUNK + nbins;
+  c.write_grid = std::max(1u, std::min((max_chunks + BW_CHUNKS_PER_CTA - 1) / BW_CHUNKS_PER_CTA, sms * 4u));
+  c.ranges = s->ranges.as<uint2>(); c.tiles_x = (uint32_t)P.tiles_x; c.tiles_y = (uint32_t)P.tiles_y;
+  c.chunk_cnt = s->chunk_cnt.as<uint64_t>(); c.write_ticket = s->sort_m.tickets.as<uint32_t>() + 2;
+  c.vals = s->vals[0].as<uint32_t>(); c.kin_lo = (uint32_t)s->lazy_chunks;
+  c.want_mask = s->unf.as<unsigned long long>();
+  c.want_count = reinterpret_cast<const uint32_t*>(s->unf.as<unsigned char>() + 2048);
+  c.avail = (s->lazy_used && s->emit_first && s->emit_first < s->emit_tiles)
+                ? s->sort_m.lookback.as<uint64_t>() + (size_t)(s->emit_first - 1) * s->emit_radix : (const uint64_t*)nullptr;
+  c.blend_grid = std::max(1u, std::min(band_tiles, sms * 8u));
+  *out = c;
   return PVG_OK;
 }
 
@@ -1015,13 +1225,22 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   s->block_used = block;
   s->last_P = P;
 
+  // lazy lists: the records (conic, colour: 48 B written, 192 B of SH read per survivor) are left to shade_kernel,
+  // which forms them for the Gaussians in front only -- unless a tile parks; and only that front is ordered
+  s->exact_used = block && s->exact_tiles && PVG_BIN_FUSED;
+  s->light = block && s->lazy_chunks > 0 && PVG_BIN_FUSED && !s->exact_used;
+  s->front_used = s->light && s->lazy_depth;
+  s->depth_complete = !s->front_used;
+  s->records_complete = !s->light;
+
   // scratch of the depth sort and of the scan: sized by n, zeroed on the side stream while preprocess runs
   if (s->presort) {
     cudaStream_t sd = s->side;
     CU(cudaStreamWaitEvent(st, s->ev_zero, 0));   // normally long past; matters only after a frame that stopped early
     CU(cudaEventRecord(s->ev_start, st));
     CU(cudaStreamWaitEvent(sd, s->ev_start, 0));
-    TRY(prep_depth_sort(n, st, sd, s->sort_n));
+    TRY(prep_depth_sort(n, st, sd, s->sort_n, s->front_used));
+    if (s->front_used) TRY(prep_front(s, sd));
     // the depth histogram is accumulated by preprocess into one half of dhist; the other half is zeroed here for
     // the next frame (its last readers, the previous frame's passes, are behind ev_start)
     s->dhist_side ^= 1;
@@ -1031,7 +1250,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   }
 
   // a1 preprocess
-  uint64_t* dk = s->presort ? s->dkeys[0].as<uint64_t>() : nullptr;
+  uint64_t* dk = s->presort ? (s->front_used ? s->okeys.as<uint64_t>() : s->dkeys[0].as<uint64_t>()) : nullptr;
   uint32_t* dv = s->presort ? s->dvals[0].as<uint32_t>() : nullptr;
   float* featw = nullptr;
   if (P.target == 1) {
@@ -1040,27 +1259,31 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   }
   s->featw_last = featw;
   TRY(tm.begin("preprocess", PVG_STAGE_PREPROCESS, st));
-  // lazy lists: the records (conic, colour: 48 B written, 192 B of SH read per survivor) are left to shade_kernel,
-  // which forms them for the Gaussians in front only -- unless a tile parks
-  s->exact_used = block && s->exact_tiles && PVG_BIN_FUSED;
-  s->light = block && s->lazy_chunks > 0 && PVG_BIN_FUSED && !s->exact_used;
-  s->records_complete = !s->light;
   {
     const unsigned pgrid = (n + 256 * PRE_CHUNKS - 1) / (256 * PRE_CHUNKS);
     uint32_t* dh = s->presort ? s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords : nullptr;
     const Model* m = s->model;
-    if (s->light)
-      preprocess_kernel<PRE_GEO><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
+    if (s->front_used)
+      preprocess_kernel<PRE_GEO, true><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
+                                                          m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
+                                                          s->record.as<float4>(), s->tileinfo.as<uint4>(),
+                                                          s->counts.as<uint32_t>(), dk, dv, featw, dh, s->d_total);
+    else if (s->light)
+      preprocess_kernel<PRE_GEO, false><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
                                                           m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
                                                           s->record.as<float4>(), s->tileinfo.as<uint4>(),
                                                           s->counts.as<uint32_t>(), dk, dv, featw, dh, s->d_total);
     else
-      preprocess_kernel<PRE_ALL><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
+      preprocess_kernel<PRE_ALL, false><<<pgrid, 256, 0, st>>>(P, n, m->shflag.as<uint8_t>(), m->A0.as<float4>(), m->A1.as<float4>(),
                                                           m->A2.as<float4>(), m->A3.as<float4>(), m->SH.as<float4>(),
                                                           s->record.as<float4>(), s->tileinfo.as<uint4>(),
                                                           s->counts.as<uint32_t>(), dk, dv, featw, dh, s->d_total);
   }
   TRY(tm.end(st));
+  if (s->front_used) {
+    CU(cudaEventRecord(s->ev_pre, st));   // the host waits for preprocess alone: its last CTA hands over M, Mb, S and F
+    tm.cut();
+  }
 
   const uint32_t* visit = nullptr;
   s->visit_side = 0;
@@ -1101,6 +1324,47 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     CU(cudaEventRecord(s->ev_join, sd));
     tm.cut();
 
+    if (s->front_used) {
+      // a3 (n-key part), front first: the pairs below preprocess's threshold are compacted and ordered -- launched
+      // before the host wait (launches that loop over tickets: the front's size is still on the device)
+      TRY(run_depth_select(s, 0, nullptr, &tm));
+      {
+        // the records of the front, from the compacted list (they do not depend on the order), on a stream of their own
+        cudaStream_t ax = s->aux;
+        const Model* m = s->model;
+        const FrontCtl* fc = reinterpret_cast<const FrontCtl*>(s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords + DH_CTL);
+        CU(cudaEventRecord(s->ev_sel, st));
+        CU(cudaStreamWaitEvent(ax, s->ev_sel, 0));
+        tm.cut();
+        TRY(tm.begin("shade", PVG_STAGE_PREPROCESS, ax));
+        shade_list_kernel<<<std::min<unsigned>((n + 255) / 256, (unsigned)s->dev.sms * 8u), 256, 0, ax>>>(
+            P, n, &fc->front, s->front_idx.as<uint32_t>(), m->A0.as<float4>(), m->A1.as<float4>(), m->A2.as<float4>(),
+            m->A3.as<float4>(), m->SH.as<float4>(), s->record.as<float4>(), featw);
+        TRY(tm.end(ax));
+        CU(cudaEventRecord(s->ev_aux, ax));
+      }
+      TRY(run_class_passes(s, 0, n, 0, 3, nullptr, &tm));
+      CU(cudaEventSynchronize(s->ev_pre));
+      M = s->h_total[0];
+      s->Mb = s->h_total[1];
+      s->survivors = s->h_total[4];
+      s->front = (uint32_t)s->h_total[8];
+      s->top_front = (int)(s->h_total[9] & 1u);
+      s->top_back = (int)((s->h_total[9] >> 1) & 1u);
+      s->nv = s->front;
+      s->visit_side = s->top_front ? 1 : 0;
+      visit = s->dvals[s->visit_side].as<uint32_t>();
+      if (s->top_front) TRY(run_class_passes(s, 0, s->front, 3, 4, nullptr, &tm));
+      if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
+      s->M = M;
+      if (M > 0) {   // the block path's scratch, sized and zeroed on the main stream: it has time, the tile grid is the longer branch
+        TRY(prep_block_bins(s, P, st));
+        tm.cut();
+      }
+      TRY(run_scan(s, s->nv, true, s->boffsets.as<uint32_t>(), visit, &tm, true));
+      CU(cudaStreamWaitEvent(st, s->ev_join, 0));   // ranges, bin_start, chunk_start (tile_prefix_kernel)
+      tm.cut();
+    } else {
     // a3 (n-key part): depth order of the survivors
     TRY(run_depth_sort(s->dev, n, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(),
                        s->dvals[1].as<uint32_t>(), s->dhist.as<uint32_t>() + s->dhist_side * kDhistWords, st, s->sort_n, &tm, 0, 3));
@@ -1127,6 +1391,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     }
     // a2 scan: items per Gaussian = tiles (instances), or 8x8-tile blocks touched (block entries)
     TRY(run_scan(s, s->nv, block, block ? s->boffsets.as<uint32_t>() : s->offsets.as<uint32_t>(), visit, &tm, true));
+    }
   } else {
     s->nv = n;
     TRY(run_scan(s, n, false, s->offsets.as<uint32_t>(), nullptr, &tm));
@@ -1233,6 +1498,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       Z.parked_host = s->d_total + 3;
       Z.blocks_x = bb_blocks(P.tiles_x);
     }
+    R2Chain R2 = {};
+    if (lazy && PVG_R2_TAIL && PVG_BIN_FUSED) TRY(fill_r2(s, P, band_tiles, &R2));
 #define PVG_BLEND(C, M, PH) TRY(launch_chain(&tm, blend_kernel<C, M, PH>, dim3((PH) == 2 ? std::min(band_tiles, (uint32_t)s->dev.sms * 8u) : band_tiles), dim3(BLEND_THREADS), 0, st, P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, (const float*)featw, Z))
 #define PVG_BLEND_ALL(PH)                                        \
     if (s->count_pairs) {                                        \
@@ -1246,6 +1513,20 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     }
     if (!lazy) {
       PVG_BLEND_ALL(0)
+    } else if (R2.enabled) {
+      // the second round is launched from the device, by the gate, if a tile parked (round2.cu)
+      PVG_BLEND_ALL(1)
+      TRY(tm.end(st));
+      TRY(tm.begin("round2_gate", PVG_STAGE_BLEND, st));
+      const int which = (s->count_pairs ? 3 : 0) + mode;
+      const int e = pvg_r2_gate(s->dev.ordinal, (void*)st, &P, &R2, &Z, which, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr,
+                                (const float*)featw);
+      if (e != 0) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "round2 gate: %s", cudaGetErrorString((cudaError_t)e));
+        return PVG_ERR_CUDA;
+      }
+      tm.pdl_open = false;
+      if (R2.back) s->nv = (uint32_t)s->survivors;
     } else {
       // phase 1 on the list prefixes; the tiles it could not finish get the rest of their lists, then phase 2
       PVG_BLEND_ALL(1)
@@ -1253,6 +1534,11 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
 #if PVG_BIN_FUSED
       bool shading = false;
       if (s->emit_first < s->emit_tiles) {
+        if (s->front_used && s->front < (uint32_t)s->survivors) {
+          // front-first: the rest of the depth order and of the offsets, if a tile parked
+          TRY(run_depth_back(s, Z.unf_count, &tm));
+          s->nv = (uint32_t)s->survivors;
+        }
         if (s->light) {
           // the rest of the scene's records, in index order (sequential model reads; the first slab's records are
           // rewritten with the same values), on the side stream: nothing before phase 2 of the blend needs them
@@ -1370,7 +1656,7 @@ int pvg_fork_scene(pvg_scene* scene, pvg_scene** out) {
   s->dev = scene->dev;
   s->presort = scene->presort; s->keep_unsorted = scene->keep_unsorted; s->count_pairs = scene->count_pairs;
   s->compact = scene->compact; s->block = scene->block; s->blend_cull = scene->blend_cull;
-  s->lazy_chunks = scene->lazy_chunks; s->lazy_slab = scene->lazy_slab; s->exact_tiles = scene->exact_tiles;
+  s->lazy_chunks = scene->lazy_chunks; s->lazy_slab = scene->lazy_slab; s->exact_tiles = scene->exact_tiles; s->lazy_depth = scene->lazy_depth;
   s->band_begin = scene->band_begin; s->band_end = scene->band_end;
   s->timer.enabled = scene->timer.enabled; s->timer.accumulate = scene->timer.accumulate; s->timer.stride = scene->timer.stride;
   s->model = scene->model;
@@ -1441,6 +1727,7 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
       scene->lazy_slab = (int)value;
       return PVG_OK;
     case PVG_OPT_EXACT_TILES: scene->exact_tiles = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_LAZY_DEPTH: scene->lazy_depth = value ? 1 : 0; return PVG_OK;
     case PVG_OPT_TILE_ROW_BEGIN:
       if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
       scene->band_begin = (int)value;
@@ -1541,6 +1828,17 @@ int pvg_debug_view(pvg_scene* s, pvg_debug* out) {
   out->counts = s->counts.as<uint32_t>();
   out->visit_order = s->presort_used ? s->dvals[s->visit_side].as<uint32_t>() : nullptr;
   out->offsets = s->offsets.as<uint32_t>();
+  if (s->front_used && !s->depth_complete) {
+    // front-first depth order: the frame ordered (and scanned) the back only if a tile parked -- the parked count of
+    // the frame is in mapped host memory once the stream has drained
+    CU(cudaStreamSynchronize(s->stream));
+    if (s->M && s->front < (uint32_t)s->survivors && s->h_total[3] == 0) {
+      TRY(run_depth_back(s, nullptr, nullptr));
+      CU(cudaGetLastError());
+    }
+    s->nv = (uint32_t)s->survivors;
+    s->depth_complete = true;
+  }
   if (s->presort_used && s->nv < s->n && !s->visit_tail_done) {
     // The depth sort drops the culled Gaussians in its first pass: the frame's visiting order holds the S survivors.
     // The view documents all n positions (the culled ones follow, in index order): append them here, on the host --
@@ -1701,7 +1999,7 @@ int pvg_frame_stats(pvg_scene* s, uint64_t out[10]) {
   // exact lists: the instances actually listed (stored by exact_ranges_kernel through mapped host memory: the last
   // frame's figure once that frame has completed on the stream)
   out[8] = (s->rendered && s->exact_used && s->M) ? s->h_total[7] : 0;
-  out[9] = 0;
+  out[9] = (s->rendered && s->front_used) ? s->front : 0;   // front-first depth order: the pairs ordered up front
   return PVG_OK;
 }
 

@@ -44,9 +44,15 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
                    const uint32_t* __restrict__ visit,
                    uint32_t* __restrict__ offsets, uint64_t* __restrict__ total,
                    uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
-                   uint32_t* __restrict__ chunk_owner, uint32_t chunk) {
+                   uint32_t* __restrict__ chunk_owner, uint32_t chunk,
+                   uint32_t rank0, const uint64_t* __restrict__ init, const uint32_t* __restrict__ only_if) {
+  // rank0, init (front-first depth order, second part): the scan covers the visiting positions [rank0, rank0 + n) and
+  // starts from *init, the total the scan of the positions before them left; only_if: nothing to do when *only_if == 0
   pdl_launch_dependents();
   pdl_wait();
+  if (only_if && *only_if == 0u) return;
+  keys += rank0;
+  offsets += rank0;
   __shared__ uint32_t s_tile;
   __shared__ uint64_t s_warp[SCAN_THREADS / 32];
   __shared__ uint64_t s_prefix;
@@ -57,7 +63,7 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
 
   uint32_t c[SCAN_ITEMS];
   uint32_t tsum = 0;
-  const bool whole = base + SCAN_ITEMS <= n;   // this thread's items are all inside: 128-bit accesses
+  const bool whole = base + SCAN_ITEMS <= n && (rank0 & 3u) == 0u;   // this thread's items are all inside (and aligned): 128-bit accesses
   if (BLOCKS && whole) {
 #pragma unroll
     for (int k = 0; k < SCAN_ITEMS; k += 2) {
@@ -98,7 +104,8 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
     // that has published its inclusive prefix (tile -1 counts as a prefix of 0)
     uint64_t excl = 0;
     if (tile == 0) {
-      if (lane == 0) st_relaxed_u64(status, LB_FLAG_PREFIX | block_sum);
+      excl = init ? *init : 0ull;
+      if (lane == 0) st_relaxed_u64(status, LB_FLAG_PREFIX | (excl + block_sum));
     } else {
       if (lane == 0) st_relaxed_u64(status + tile, LB_FLAG_AGG | block_sum);
       int64_t p = (int64_t)tile - 1 - (int64_t)lane;
@@ -141,7 +148,7 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
       if (!whole) offsets[r] = (uint32_t)run;
       if (BLOCKS && chunk_owner && c[k]) {
         const uint64_t first = (run + chunk - 1) / chunk;   // first chunk boundary at or after my first item
-        if (first * chunk < run + c[k]) chunk_owner[first] = r;   // c[k] <= 256 < chunk: at most one boundary
+        if (first * chunk < run + c[k]) chunk_owner[first] = rank0 + r;   // c[k] <= 256 < chunk: at most one boundary
       }
     }
     run += c[k];

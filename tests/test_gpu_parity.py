@@ -420,7 +420,9 @@ def test_repeatable_and_stream():
     times = g.stage_times_ms()
     assert set(times) == set(pvg.STAGES) and times["blend"] > 0
     names = [k[0] for k in g.kernel_times_ms()]
-    assert names[0] == "preprocess" and names[-1] == "blend" and "onesweep_pass" in names
+    # the frame ends with the blend, or with the one-thread gate behind it that launches the second round of the lazy
+    # lists from the device if a tile parked (csrc/round2.cu)
+    assert names[0] == "preprocess" and names[-1] in ("blend", "round2_gate") and "blend" in names and "onesweep_pass" in names
     g.close()
 
 
