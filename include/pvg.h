@@ -33,7 +33,8 @@ typedef enum pvg_status {
   PVG_ERR_INSTANCE_OVERFLOW = -5, /* tile instances M >= 2^32 */
   PVG_ERR_CUDA = -6,              /* CUDA runtime error (or no device); see pvg_last_cuda_error */
   PVG_ERR_BAD_OPTION = -7,
-  PVG_ERR_BAD_STATE = -8          /* non-finite t or dt, rho_min < 0, rho_max < rho_min, unknown target */
+  PVG_ERR_BAD_STATE = -8,         /* non-finite t or dt, rho_min < 0, rho_max < rho_min, unknown target */
+  PVG_ERR_TOO_LARGE = -9          /* pvg_sort_pairs_static: more pairs than the static scratch holds; see pvg_last_cuda_error */
 } pvg_status;
 
 typedef struct pvg_scene pvg_scene; /* opaque; owns device copies of the model and a growable workspace */
@@ -306,6 +307,23 @@ int pvg_blend_counters(pvg_scene *scene, uint64_t out[2]);
  * synchronises it. */
 int pvg_sort_pairs(uint64_t n, uint64_t *keys_in, uint32_t *vals_in, uint64_t *keys_out,
                    uint32_t *vals_out, int begin_bit, int end_bit, void *cuda_stream);
+
+/* The same sort for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): its scratch -- digit histograms, tickets, look-back words -- lives in a file-scope device array
+ * of the library, 4.01 MB that every GPU which loads the library holds until the process exits, enough for
+ * n <= PVG_SORT_STATIC_MAX_N pairs and any bit range. Calls no cudaMalloc, cudaFree or allocating library routine.
+ *   - Same arguments, layouts and result as pvg_sort_pairs (DEVICE buffers of n elements owned by the caller; the
+ *     sorted pairs land in keys_out / vals_out, keys_in / vals_in are clobbered), on the current device.
+ *   - n > PVG_SORT_STATIC_MAX_N: returns PVG_ERR_TOO_LARGE, nothing is enqueued, pvg_last_cuda_error() says why.
+ *   - ASYNCHRONOUS: the work is enqueued on `cuda_stream` and the call returns; it does not synchronise (unlike
+ *     pvg_sort_pairs). Errors of the kernels themselves surface at the caller's next synchronisation.
+ *   - Every call on a device shares the one array (it keeps the last call's contents; the call clears what must
+ *     start at zero, on the stream): two calls that overlap on the GPU -- different streams without an ordering
+ *     between them, or different host threads -- RACE on it. Calls on one stream are ordered and safe. */
+#define PVG_SORT_STATIC_MAX_N (1u << 20)
+int pvg_sort_pairs_static(uint64_t n, uint64_t *keys_in, uint32_t *vals_in, uint64_t *keys_out,
+                          uint32_t *vals_out, int begin_bit, int end_bit, void *cuda_stream);
+uint64_t pvg_sort_pairs_static_max_n(void);   /* PVG_SORT_STATIC_MAX_N as the library was built */
 
 /* Measurement hook for the roofline of the ALU-bound blend ("calibrate with an FFMA microbenchmark on
  * the box"): runs a register-only kernel on the current device (8 CTAs of 256 threads per SM, 8 independent chains

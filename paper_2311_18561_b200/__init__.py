@@ -18,7 +18,8 @@ LIB_PATH = os.environ.get("PVG_LIB") or os.path.join(_HERE, "libpvg.so")   # PVG
 
 PVG_OK = 0
 STATUS = {0: "PVG_OK", -1: "PVG_ERR_NULL", -2: "PVG_ERR_BAD_DESC", -3: "PVG_ERR_BAD_CAMERA",
-          -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION", -8: "PVG_ERR_BAD_STATE"}
+          -4: "PVG_ERR_OOM", -5: "PVG_ERR_INSTANCE_OVERFLOW", -6: "PVG_ERR_CUDA", -7: "PVG_ERR_BAD_OPTION", -8: "PVG_ERR_BAD_STATE",
+          -9: "PVG_ERR_TOO_LARGE"}
 OPT_PRESORT_DEPTH, OPT_KEEP_UNSORTED, OPT_KERNEL_EVENTS, OPT_COUNT_PAIRS, OPT_COMPACT_KEYS, OPT_BLOCK_BINS = 1, 2, 3, 4, 5, 6
 OPT_BLEND_CULL, OPT_EVENT_STRIDE = 7, 8
 OPT_TILE_ROW_BEGIN, OPT_TILE_ROW_END = 9, 10
@@ -30,7 +31,7 @@ NUM_STAGES = len(STAGES)
 EXPORTS = ("pvg_set_allocator", "pvg_set_stream", "pvg_create_scene", "pvg_render", "pvg_render_host",
            "pvg_render_host_async", "pvg_wait_host", "pvg_render_state", "pvg_set_sky",
            "pvg_destroy", "pvg_fork_scene", "pvg_set_option", "pvg_debug_view", "pvg_stage_times_ms", "pvg_kernel_times_ms", "pvg_kernel_timeline_ms",
-           "pvg_sort_pairs", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_calibrate_fp32", "pvg_guard_bands", "pvg_check_guards", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
+           "pvg_sort_pairs", "pvg_sort_pairs_static", "pvg_sort_pairs_static_max_n", "pvg_frame_stats", "pvg_blend_counters", "pvg_memcpy_d2h", "pvg_calibrate_fp32", "pvg_guard_bands", "pvg_check_guards", "pvg_strerror", "pvg_last_cuda_error", "pvg_version")
 
 
 class PvgError(RuntimeError):
@@ -103,6 +104,10 @@ def load_library(path: Optional[str] = None):
                                          C.POINTER(C.c_float)]
     L.pvg_sort_pairs.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                  C.c_void_p]
+    L.pvg_sort_pairs_static.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                        C.c_void_p]
+    L.pvg_sort_pairs_static_max_n.restype = C.c_uint64
+    L.pvg_sort_pairs_static_max_n.argtypes = []
     L.pvg_frame_stats.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
     L.pvg_blend_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
     L.pvg_memcpy_d2h.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
@@ -119,7 +124,7 @@ def _check(rc: int):
     if rc != PVG_OK:
         L = load_library()
         detail = L.pvg_strerror(rc).decode()
-        if rc == -6:
+        if rc in (-6, -9):
             detail += " | " + L.pvg_last_cuda_error().decode()
         raise PvgError(rc, detail)
 
@@ -417,6 +422,27 @@ def sort_pairs(keys, vals, begin_bit: int = 0, end_bit: int = 64):
     _check(L.pvg_sort_pairs(n, keys.data_ptr(), vals.data_ptr(), ko.data_ptr(), vo.data_ptr(), int(begin_bit),
                             int(end_bit), torch.cuda.current_stream().cuda_stream))
     return ko, vo
+
+
+def sort_pairs_static_max_n() -> int:
+    """Largest n pvg_sort_pairs_static accepts (PVG_SORT_STATIC_MAX_N of the built library)."""
+    return int(load_library().pvg_sort_pairs_static_max_n())
+
+
+def sort_pairs_static(keys, vals, keys_out, vals_out, begin_bit: int = 0, end_bit: int = 64) -> None:
+    """pvg_sort_pairs_static (include/pvg.h): the same sort with its scratch in a static device array of the library
+    -- no allocation anywhere in the call, which is why the caller passes the outputs too. At most
+    sort_pairs_static_max_n() pairs (PvgError PVG_ERR_TOO_LARGE beyond). Asynchronous on torch's current stream; calls
+    that overlap on the GPU race on the shared scratch. Inputs are clobbered."""
+    import torch
+    L = load_library()
+    for x in (keys, vals, keys_out, vals_out):
+        assert x.is_cuda and x.is_contiguous()
+    assert keys.dtype == keys_out.dtype == torch.int64 and vals.dtype == vals_out.dtype == torch.int32
+    n = keys.numel()
+    assert vals.numel() == n and keys_out.numel() == n and vals_out.numel() == n
+    _check(L.pvg_sort_pairs_static(n, keys.data_ptr(), vals.data_ptr(), keys_out.data_ptr(), vals_out.data_ptr(),
+                                   int(begin_bit), int(end_bit), torch.cuda.current_stream().cuda_stream))
 
 
 def calibrate_fp32(mode: int = 1):

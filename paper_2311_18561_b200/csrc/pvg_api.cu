@@ -1593,6 +1593,7 @@ const char* pvg_strerror(int code) {
     case PVG_ERR_CUDA: return "CUDA error";
     case PVG_ERR_BAD_OPTION: return "bad option";
     case PVG_ERR_BAD_STATE: return "bad state (non-finite t or dt, negative rho_min, rho_max < rho_min)";
+    case PVG_ERR_TOO_LARGE: return "too many pairs for the static scratch of pvg_sort_pairs_static";
     default: return "unknown error";
   }
 }
@@ -2098,6 +2099,87 @@ int pvg_sort_pairs(uint64_t n, uint64_t* keys_in, uint32_t* vals_in, uint64_t* k
   if (rc == PVG_OK && e != cudaSuccess) { snprintf(g_cuda_err, sizeof(g_cuda_err), "sort: %s", cudaGetErrorString(e)); rc = PVG_ERR_CUDA; }
   sc.hist.release(); sc.lookback.release(); sc.tickets.release();
   return rc;
+}
+
+}  // extern "C"
+
+// ---- the sort primitive without any allocation ---------------------------------------------------------------------
+// pvg_sort_pairs sizes its scratch (digit histograms, tickets, look-back words) with the device allocator on every
+// call. Callers that may not allocate -- code under CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc -- get the same sort with that scratch in a file-scope device array of a fixed, modest size: every GPU that
+// loads the library holds these 4.01 MB until the process exits. The array's name is a host-side stand-in in host
+// code, not a device address: the address is looked up once per device (cudaGetSymbolAddress, with that device current).
+constexpr uint64_t kSortStaticMaxN = PVG_SORT_STATIC_MAX_N;
+constexpr size_t kSsTile = (size_t)OsSmall::THREADS * OsSmall::ITEMS;
+constexpr size_t kSsTiles = (kSortStaticMaxN + kSsTile - 1) / kSsTile;
+constexpr size_t kSsHistBytes = (size_t)OS_MAX_PASSES * OS_RADIX * 4;                  // 10 KB
+constexpr size_t kSsTicketBytes = 256;                                                  // OS_MAX_PASSES u32, padded
+constexpr size_t kSsLookbackBytes = (size_t)8 * kSsTiles * OS_RADIX * 8;                // at most 8 passes of 8 bits for 64 key bits
+constexpr size_t kSsBytes = kSsHistBytes + kSsTicketBytes + kSsLookbackBytes;
+static_assert(kSortStaticMaxN < OS_SMALL_BELOW, "the static scratch is laid out for the small tile shape");
+static_assert(kSsHistBytes % 256 == 0 && OS_MAX_PASSES * 4 <= kSsTicketBytes, "aligned sections");
+static __device__ __align__(256) unsigned char g_sort_static_scratch[kSsBytes];
+
+namespace {
+std::mutex g_ss_mu;
+void* g_ss_ptr[64] = {};   // device address of g_sort_static_scratch, per device ordinal
+
+int sort_static_scratch(int device, unsigned char** out) {
+  if (device < 0 || device >= 64) return PVG_ERR_BAD_OPTION;
+  std::lock_guard<std::mutex> lk(g_ss_mu);
+  if (!g_ss_ptr[device]) {
+    void* ptr = nullptr;
+    CU(cudaGetSymbolAddress(&ptr, g_sort_static_scratch));   // the current device's copy (Dev::query read the ordinal just now)
+    if (!ptr) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "sort scratch: cudaGetSymbolAddress returned a null address");
+      return PVG_ERR_CUDA;
+    }
+    g_ss_ptr[device] = ptr;
+  }
+  *out = static_cast<unsigned char*>(g_ss_ptr[device]);
+  return PVG_OK;
+}
+}  // namespace
+
+extern "C" {
+
+uint64_t pvg_sort_pairs_static_max_n(void) { return kSortStaticMaxN; }
+
+int pvg_sort_pairs_static(uint64_t n, uint64_t* keys_in, uint32_t* vals_in, uint64_t* keys_out, uint32_t* vals_out,
+                          int begin_bit, int end_bit, void* cuda_stream) {
+  if (n && (!keys_in || !vals_in || !keys_out || !vals_out)) return PVG_ERR_NULL;
+  if (begin_bit < 0 || end_bit > 64 || begin_bit > end_bit) return PVG_ERR_BAD_OPTION;
+  if (n > kSortStaticMaxN) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "pvg_sort_pairs_static: n = %llu exceeds the static scratch (at most %llu pairs)",
+             (unsigned long long)n, (unsigned long long)kSortStaticMaxN);
+    return PVG_ERR_TOO_LARGE;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Dev dv;
+  TRY(dv.query());
+  unsigned char* base = nullptr;
+  TRY(sort_static_scratch(dv.ordinal, &base));
+  // views of the static array: never reserved, grown or released (cap is what the array holds)
+  SortScratch sc;
+  sc.hist.p = base;                                   sc.hist.cap = kSsHistBytes;
+  sc.tickets.p = base + kSsHistBytes;                 sc.tickets.cap = kSsTicketBytes;
+  sc.lookback.p = base + kSsHistBytes + kSsTicketBytes; sc.lookback.cap = kSsLookbackBytes;
+  int side = 0;
+  if (n && end_bit > begin_bit) {
+    // the array keeps the last call's contents: what must start at zero is cleared here, on the caller's stream
+    const SortPlan plan = make_sort_plan(begin_bit, end_bit);
+    const size_t tiles = ((size_t)n + kSsTile - 1) / kSsTile;
+    const size_t lb_bytes = (size_t)plan.num_passes * tiles * OS_RADIX * 8;
+    if (plan.num_passes > 8 || lb_bytes > kSsLookbackBytes) return PVG_ERR_TOO_LARGE;
+    CU(cudaMemsetAsync(sc.hist.p, 0, kSsHistBytes + kSsTicketBytes, st));
+    CU(cudaMemsetAsync(sc.lookback.p, 0, lb_bytes, st));
+    TRY(run_onesweep(dv, n, keys_in, vals_in, keys_out, vals_out, begin_bit, end_bit, st, sc, nullptr, 0, &side, false, true));
+  }
+  if (n && side == 0) {   // result landed in the input buffers (an even number of passes, or none)
+    CU(cudaMemcpyAsync(keys_out, keys_in, n * 8, cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemcpyAsync(vals_out, vals_in, n * 4, cudaMemcpyDeviceToDevice, st));
+  }
+  return PVG_OK;
 }
 
 }  // extern "C"
