@@ -217,7 +217,7 @@ typedef enum pvg_option {
    *    the complete list holds there. pvg_debug_view writes the remainder on demand, so vals_sorted is always
    *    every tile's whole list. 0: write the complete lists before the blend. */
   PVG_OPT_LAZY_CHUNKS = 11,
-  /* d >= 1 (default 8), with LAZY_CHUNKS > 0: lazy emission. Only the first 1/d of the block entries, in depth order
+  /* d >= 1 (default 16), with LAZY_CHUNKS > 0: lazy emission. Only the first 1/d of the block entries, in depth order
    *    (whole tiles of 4096), is formed and split by block before the first blend phase; a block's chunk counts for
    *    that phase only if all of its 512 entries exist. The entries behind the slab are formed only if a tile was
    *    parked (the launch checks the count on the device). 1: form all entries up front. */

@@ -517,7 +517,11 @@ struct pvg_scene {
   int presort = 1, keep_unsorted = 0, count_pairs = 0, compact = 1, block = 1, blend_cull = 1;
   int band_begin = 0, band_end = 0;   // PVG_OPT_TILE_ROW_BEGIN / END (0, 0: the whole image)
   int lazy_chunks = 2;                // PVG_OPT_LAZY_CHUNKS (0: always write the complete lists)
-  int lazy_slab = 8;                  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front
+  // PVG_OPT_LAZY_SLAB: the first 1/lazy_slab of the block entries is emitted up front. B200, ms per frame of the config 3
+  // sweep / config 4 (no tile parks at any of these): 4: 0.369 / 0.679, 8: 0.338 / 0.667, 12: 0.304 / 0.659,
+  // 16: 0.300 / 0.659, 24: 0.304 / 0.648, 32: 0.302 / 0.646 -- the front the frame orders, scans and shades shrinks
+  // with the slab (36 k Gaussians at 8, 16 k at 16); beyond 16 nothing is left to gain and parking comes closer
+  int lazy_slab = 16;
   int exact_tiles = 0;                // PVG_OPT_EXACT_TILES: list a Gaussian only in the tiles its ellipse can reach (P13)
   int lazy_depth = 1;                 // PVG_OPT_LAZY_DEPTH: with lazy lists, order the front of the scene first (onesweep.cuh)
   bool front_used = false;            // the last frame ordered its front first
@@ -1130,7 +1134,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 #endif
 extern "C" int pvg_r2_gate(int device, void* stream, const void* params, const void* chain, const void* lazy, int which,
                            const void* ranges, const void* vals, const void* record, float* out_rgb, float* out_depth,
-                           float* out_alpha, unsigned long long* counters, const float* featw);
+                           float* out_alpha, unsigned long long* counters, const float* featw, int pdl);
 
 // The launches of the second round, described for r2_tail_launch: the same kernels, grids and arguments as the host
 // path further down (run_depth_back, run_shade_all, run_bin_emit, launch_bin_write, the second blend phase).
@@ -1295,8 +1299,6 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     // (they size the frame's buffers) while the depth sort is still running
     cudaStream_t sd = s->side;
     CU(cudaStreamWaitEvent(st, s->ev_zero, 0));
-    CU(cudaEventRecord(s->ev_fork, st));
-    CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
     constexpr size_t kMaxDyn = 200 * 1024;
     PVG_ENSURE_SMEM(tile_prefix_kernel, kMaxDyn, s->dev.ordinal);
     PVG_ENSURE_SMEM(tile_grid_kernel, kMaxDyn, s->dev.ordinal);
@@ -1307,7 +1309,9 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     TRY(s->sort_m.hist.reserve((size_t)OS_MAX_PASSES * OS_RADIX * 4, st));
     TRY(s->bin_tables.reserve(4096, st));   // bin_start[257] | chunk_start[257]
     int* grid = s->tilegrid.as<int>();
-    CU(cudaMemsetAsync(grid, 0, grid_bytes + 4, sd));
+    CU(cudaMemsetAsync(grid, 0, grid_bytes + 4, sd));   // beside preprocess: the side stream waits for it only now
+    CU(cudaEventRecord(s->ev_fork, st));
+    CU(cudaStreamWaitEvent(sd, s->ev_fork, 0));
     tm.cut();
     TRY(tm.begin("tile_grid", PVG_STAGE_RANGES, sd));
     tile_grid_kernel<<<std::min<unsigned>((n + TG_THREADS - 1) / TG_THREADS, (unsigned)s->dev.sms), TG_THREADS,
@@ -1357,9 +1361,11 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       if (s->top_front) TRY(run_class_passes(s, 0, s->front, 3, 4, nullptr, &tm));
       if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
       s->M = M;
-      if (M > 0) {   // the block path's scratch, sized and zeroed on the main stream: it has time, the tile grid is the longer branch
-        TRY(prep_block_bins(s, P, st));
-        tm.cut();
+      if (M > 0) {
+        // the block path's scratch, sized here and zeroed on the aux stream behind shade_list_kernel, beside the passes
+        // (on the main stream the five memsets sat between the last pass and the scan: 15 us of the critical path)
+        TRY(prep_block_bins(s, P, s->aux));
+        CU(cudaEventRecord(s->ev_zero, s->aux));
       }
       TRY(run_scan(s, s->nv, true, s->boffsets.as<uint32_t>(), visit, &tm, true));
       CU(cudaStreamWaitEvent(st, s->ev_join, 0));   // ranges, bin_start, chunk_start (tile_prefix_kernel)
@@ -1516,11 +1522,13 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     } else if (R2.enabled) {
       // the second round is launched from the device, by the gate, if a tile parked (round2.cu)
       PVG_BLEND_ALL(1)
+      // with the timing hook on, an event record sits between the two kernels: a plain launch then
+      const int pdl = (PVG_PDL && tm.pdl_open && tm.pdl_stream == st && !tm.frame_on) ? 1 : 0;
       TRY(tm.end(st));
       TRY(tm.begin("round2_gate", PVG_STAGE_BLEND, st));
       const int which = (s->count_pairs ? 3 : 0) + mode;
       const int e = pvg_r2_gate(s->dev.ordinal, (void*)st, &P, &R2, &Z, which, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr,
-                                (const float*)featw);
+                                (const float*)featw, pdl);
       if (e != 0) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "round2 gate: %s", cudaGetErrorString((cudaError_t)e));
         return PVG_ERR_CUDA;

@@ -44,19 +44,26 @@ cudaError_t ensure_all() {
 
 // Enqueues the gate on `stream` (after the first blend phase). params / chain / lazy: FrameParams, R2Chain, BlendLazy
 // of the frame, by address (copied into the launch). which = COUNT * 3 + MODE of the frame's blend kernels.
-// Returns a cudaError_t.
+// pdl: launch as a programmatic dependent of the kernel enqueued just before (the first blend phase). Returns a cudaError_t.
 extern "C" int pvg_r2_gate(int device, void* stream, const void* params, const void* chain, const void* lazy, int which,
                            const void* ranges, const void* vals, const void* record, float* out_rgb, float* out_depth,
-                           float* out_alpha, unsigned long long* counters, const float* featw) {
+                           float* out_alpha, unsigned long long* counters, const float* featw, int pdl) {
   const unsigned bit = 1u << (device & 31);
   if (!(g_ready.load(std::memory_order_acquire) & bit)) {
     cudaError_t e = ensure_all();
     if (e != cudaSuccess) return (int)e;
     g_ready.fetch_or(bit, std::memory_order_release);
   }
-  pvg::r2_gate_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(
-      *static_cast<const pvg::FrameParams*>(params), *static_cast<const pvg::R2Chain*>(chain), which,
-      static_cast<const uint2*>(ranges), static_cast<const uint32_t*>(vals), static_cast<const float4*>(record), out_rgb,
-      out_depth, out_alpha, counters, featw, *static_cast<const pvg::BlendLazy*>(lazy));
-  return (int)cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1); cfg.blockDim = dim3(1); cfg.dynamicSmemBytes = 0; cfg.stream = (cudaStream_t)stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;   // only when the operation before it on the stream is the blend kernel
+  cudaError_t e = cudaLaunchKernelEx(&cfg, pvg::r2_gate_kernel, *static_cast<const pvg::FrameParams*>(params),
+                                     *static_cast<const pvg::R2Chain*>(chain), which, static_cast<const uint2*>(ranges),
+                                     static_cast<const uint32_t*>(vals), static_cast<const float4*>(record), out_rgb, out_depth,
+                                     out_alpha, counters, featw, *static_cast<const pvg::BlendLazy*>(lazy));
+  return (int)(e != cudaSuccess ? e : cudaGetLastError());
 }

@@ -78,6 +78,9 @@ __global__ void r2_gate_kernel(const __grid_constant__ FrameParams P, const __gr
                                const uint2* ranges, const uint32_t* vals, const float4* record, float* out_rgb, float* out_depth,
                                float* out_alpha, unsigned long long* counters, const float* featw,
                                const __grid_constant__ BlendLazy Z) {
+  // launched as a programmatic dependent of the first blend phase (pvg_r2_gate): the thread is resident before that
+  // kernel ends and waits here for its completion, so the launch latency of the gate is off the frame's critical path
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   const uint32_t parked = *Z.unf_count;
   *Z.parked_host = parked;
   if (!parked) return;

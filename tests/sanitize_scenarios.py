@@ -58,8 +58,8 @@ def main():
         sc.set_option(pvg.OPT_LAZY_CHUNKS, 0); same("complete lists")
         sc.set_option(pvg.OPT_EXACT_TILES, 1); same("exact tile lists")
         sc.set_option(pvg.OPT_EXACT_TILES, 0)
-        sc.set_option(pvg.OPT_LAZY_CHUNKS, 1); sc.set_option(pvg.OPT_LAZY_SLAB, 16); same("lazy, one chunk, small slab")
-        sc.set_option(pvg.OPT_LAZY_CHUNKS, 2); sc.set_option(pvg.OPT_LAZY_SLAB, 8)
+        sc.set_option(pvg.OPT_LAZY_CHUNKS, 1); sc.set_option(pvg.OPT_LAZY_SLAB, 48); same("lazy, one chunk, small slab")
+        sc.set_option(pvg.OPT_LAZY_CHUNKS, 2); sc.set_option(pvg.OPT_LAZY_SLAB, 16)
         sc.set_option(pvg.OPT_BLOCK_BINS, 0); same("compact keys")
         sc.set_option(pvg.OPT_COMPACT_KEYS, 0); same("64-bit keys, depth presort")
         sc.set_option(pvg.OPT_PRESORT_DEPTH, 0); same("64-bit keys, index order")

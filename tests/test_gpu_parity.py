@@ -580,20 +580,28 @@ def test_debug_view_follows_the_options_of_the_last_render():
     g.close()
 
 
+@pytest.mark.parametrize("lazy_depth", [0, 1])
 @pytest.mark.parametrize("znear,top_pass", [(1e-4, True), (0.2, False), (50.0, False)])
-def test_depth_sort_key_range(znear, top_pass):
+def test_depth_sort_key_range(znear, top_pass, lazy_depth):
     """The depth key is bits(z) - bits(znear) in digits of 9 + 9 + 9 + 4: with a tiny near plane the keys span more than
     27 bits and the top-digit pass must run; with the default one it is the identity and is not launched; with a
-    near plane inside the scene most Gaussians are culled and dropped by the first pass. All bit-exact."""
+    near plane inside the scene most Gaussians are culled and dropped by the first pass. All bit-exact.
+    lazy_depth = 1 (front-first order): the frame sorts the front alone, whose keys may all lie below 2^27 even then
+    (three passes; the back, ordered for the debug view, takes the fourth) -- or the whole scene is the front (four)."""
     wl = make_config(1, n=80_000)
     cam = wl.cameras[0]
     cam.znear = znear
     sc = pvg.Scene.from_workload_scene(wl.scene)
+    sc.set_option(pvg.OPT_LAZY_DEPTH, lazy_depth)
     sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
     sc.set_option(pvg.OPT_KERNEL_EVENTS, 1)
     sc.render(cam, 0.5)
     passes = [k for k in sc.kernel_times_ms() if k[0] == "onesweep_pass" and k[1] == "depth_sort"]
-    assert len(passes) == (4 if top_pass else 3)
+    if lazy_depth == 0 or not top_pass:
+        assert len(passes) == (4 if top_pass else 3)
+    else:
+        fs = sc.frame_stats()
+        assert len(passes) == (4 if fs["front"] == fs["survivors"] else 3)
     st = check_integer_chain(sc.debug(), cam.width, cam.height, True)
     assert st["M"] > 10_000
     if znear == 50.0:
