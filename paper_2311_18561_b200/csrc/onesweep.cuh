@@ -596,6 +596,12 @@ depth_select_kernel(const uint64_t* __restrict__ keys, uint32_t n, const FrontCt
 
 // LOOP: the launch is smaller than the number of tiles (which only the device knows: ctl->survivors); its CTAs take
 // tickets until the pairs run out. only_if (LOOP): nothing to do when *only_if == 0.
+template <int THREADS, int ITEMS, int BITS, bool FIRST, bool LOOP>
+__device__ __forceinline__ void
+depth_pass_body(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, uint64_t* __restrict__ keys_b,
+                uint32_t* __restrict__ vals_b, uint32_t n, int pass, int shift, const DepthCtl* __restrict__ ctl,
+                const uint32_t* __restrict__ hist_excl, uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket);
+
 template <int THREADS, int ITEMS, int BITS, int MINB, bool FIRST, bool LOOP>
 __global__ void __launch_bounds__(THREADS, MINB)
 depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, uint64_t* __restrict__ keys_b,
@@ -606,6 +612,14 @@ depth_pass_kernel(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, 
   pdl_launch_dependents();
   pdl_wait();
   if (LOOP && only_if && *only_if == 0u) return;
+  depth_pass_body<THREADS, ITEMS, BITS, FIRST, LOOP>(keys_a, vals_a, keys_b, vals_b, n, pass, shift, ctl, hist_excl, lookback, ticket);
+}
+
+template <int THREADS, int ITEMS, int BITS, bool FIRST, bool LOOP>
+__device__ __forceinline__ void
+depth_pass_body(uint64_t* __restrict__ keys_a, uint32_t* __restrict__ vals_a, uint64_t* __restrict__ keys_b,
+                uint32_t* __restrict__ vals_b, uint32_t n, int pass, int shift, const DepthCtl* __restrict__ ctl,
+                const uint32_t* __restrict__ hist_excl, uint64_t* __restrict__ lookback, uint32_t* __restrict__ ticket) {
   using Core = RadixCore<THREADS, ITEMS, BITS>;
   constexpr int TILE = Core::TILE;
   constexpr uint32_t MASK = (1u << BITS) - 1u;

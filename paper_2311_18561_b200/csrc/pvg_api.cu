@@ -17,6 +17,7 @@
 #include "calib.cuh"
 #include "common.cuh"
 #include "expand.cuh"
+#include "front_sort.cuh"
 #include "onesweep.cuh"
 #include "preprocess.cuh"
 #include "ranges.cuh"
@@ -385,7 +386,7 @@ inline size_t class_lookback_words(uint32_t n, int cls) { return class_lookback_
 // front_first: the front's passes and the back's have their own tickets (0..3 / 4..7) and look-back words, and
 // depth_select_kernel zeroes the words its class will use (it knows how many pairs there are)
 int prep_depth_sort(uint32_t n, cudaStream_t alloc_st, cudaStream_t zs, SortScratch& sc, bool front_first = false) {
-  static_assert(OS_MAX_PASSES >= 2 * DS_PASSES, "tickets of two classes");
+  static_assert(OS_MAX_PASSES >= 2 * DS_PASSES + 1, "tickets of two classes and the barrier word of front_sort_kernel");
   TRY(sc.tickets.reserve((size_t)OS_MAX_PASSES * 4, alloc_st));
   CU(cudaMemsetAsync(sc.tickets.p, 0, (size_t)OS_MAX_PASSES * 4, zs));
   if (front_first) {
@@ -572,7 +573,7 @@ struct pvg_scene {
   cudaStream_t side = nullptr;  // tile grid + prefix run here, beside the depth sort
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_start = nullptr, ev_zero = nullptr, ev_pre = nullptr;
   cudaStream_t aux = nullptr;   // front-first: the front's records are formed here, beside the sort and the tile grid
-  cudaEvent_t ev_sel = nullptr, ev_aux = nullptr;
+  cudaEvent_t ev_sel = nullptr, ev_aux = nullptr, ev_blocks = nullptr;
   Timer timer;
   // last frame
   uint64_t M = 0, Mb = 0, survivors = 0;
@@ -617,7 +618,8 @@ void release_all(pvg_scene* s) {
   s->ev_pre = nullptr;
   if (s->ev_sel) cudaEventDestroy(s->ev_sel);
   if (s->ev_aux) cudaEventDestroy(s->ev_aux);
-  s->ev_sel = s->ev_aux = nullptr;
+  if (s->ev_blocks) cudaEventDestroy(s->ev_blocks);
+  s->ev_sel = s->ev_aux = s->ev_blocks = nullptr;
   if (s->aux) cudaStreamDestroy(s->aux);
   s->aux = nullptr;
   s->ev_start = s->ev_zero = nullptr;
@@ -707,6 +709,7 @@ int init_workspace(pvg_scene* s) {
   CU(cudaEventCreateWithFlags(&s->ev_pre, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_sel, cudaEventDisableTiming));
   CU(cudaEventCreateWithFlags(&s->ev_aux, cudaEventDisableTiming));
+  CU(cudaEventCreateWithFlags(&s->ev_blocks, cudaEventDisableTiming));
   CU(cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking));
   CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_rendered, cudaEventDisableTiming));
@@ -1114,6 +1117,10 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 #endif
   s->lists_complete = !s->lazy_used;
   s->visit_last = visit;
+  if (s->front_used) {   // the ranges (tile_prefix_kernel, tile level): bin_write is their first reader
+    CU(cudaStreamWaitEvent(st, s->ev_join, 0));
+    tm->cut();
+  }
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
   TRY(launch_bin_write(s, P, 0u, s->lazy_used ? (uint32_t)s->lazy_chunks : 0xFFFFFFFFu, false, 1));
   TRY(tm->end(st));
@@ -1131,6 +1138,9 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 // the parked count.
 #ifndef PVG_R2_TAIL
 #define PVG_R2_TAIL 1
+#endif
+#ifndef PVG_FRONT_FUSED
+#define PVG_FRONT_FUSED 1
 #endif
 extern "C" int pvg_r2_gate(int device, void* stream, const void* params, const void* chain, const void* lazy, int which,
                            const void* ranges, const void* vals, const void* record, float* out_rgb, float* out_depth,
@@ -1319,12 +1329,17 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
                                                         block ? 1 : 0, grid);
     TRY(tm.end(sd));
     uint64_t* totals = reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 16);
-    TRY(tm.begin("tile_prefix", PVG_STAGE_RANGES, sd));
-    tile_prefix_kernel<<<1, TB_THREADS, use_smem ? grid_bytes : 0, sd>>>(
-        grid, P.tiles_x, P.tiles_y, use_smem, block ? 1 : 0, make_sort_plan(s->sort_begin, s->sort_end),
-        s->ranges.as<uint2>(), s->sort_m.hist.as<uint32_t>(), totals, s->bin_tables.as<uint32_t>(),
-        s->bin_tables.as<uint32_t>() + 257, s->d_total);
-    TRY(tm.end(sd));
+    // front-first frames: the block level first, in a launch of its own -- it is all bin_emit waits for
+    for (int parts : {s->front_used ? 2 : 3, s->front_used ? 1 : 0}) {
+      if (!parts) break;
+      TRY(tm.begin(parts == 2 ? "block_prefix" : "tile_prefix", PVG_STAGE_RANGES, sd));
+      tile_prefix_kernel<<<1, TB_THREADS, use_smem ? grid_bytes : 0, sd>>>(
+          grid, P.tiles_x, P.tiles_y, use_smem, block ? 1 : 0, parts, make_sort_plan(s->sort_begin, s->sort_end),
+          s->ranges.as<uint2>(), s->sort_m.hist.as<uint32_t>(), totals, s->bin_tables.as<uint32_t>(),
+          s->bin_tables.as<uint32_t>() + 257, s->d_total);
+      TRY(tm.end(sd));
+      if (parts == 2) CU(cudaEventRecord(s->ev_blocks, sd));
+    }
     CU(cudaEventRecord(s->ev_join, sd));
     tm.cut();
 
@@ -1347,7 +1362,10 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
         TRY(tm.end(ax));
         CU(cudaEventRecord(s->ev_aux, ax));
       }
-      TRY(run_class_passes(s, 0, n, 0, 3, nullptr, &tm));
+      // PVG_FRONT_FUSED=1: the front's passes and scan are launched after the host wait, when its size is known -- as
+      // one grid when its tiles fit the GPU at once (front_sort.cuh); the selection covers the host's latency.
+      // 0: the passes are launched here, before the wait, as launches that loop over tickets.
+      if (!PVG_FRONT_FUSED) TRY(run_class_passes(s, 0, n, 0, 3, nullptr, &tm));
       CU(cudaEventSynchronize(s->ev_pre));
       M = s->h_total[0];
       s->Mb = s->h_total[1];
@@ -1358,17 +1376,36 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       s->nv = s->front;
       s->visit_side = s->top_front ? 1 : 0;
       visit = s->dvals[s->visit_side].as<uint32_t>();
-      if (s->top_front) TRY(run_class_passes(s, 0, s->front, 3, 4, nullptr, &tm));
+      const uint32_t ftiles = (s->front + kDsFrontTile - 1) / kDsFrontTile;
+      const bool fused = PVG_FRONT_FUSED && s->front > 0 && ftiles <= (uint32_t)s->dev.sms * 2u;
+      if (PVG_FRONT_FUSED && !fused) TRY(run_class_passes(s, 0, s->front, 0, 3, nullptr, &tm));
+      if (!fused && s->top_front) TRY(run_class_passes(s, 0, s->front, 3, 4, nullptr, &tm));
       if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
       s->M = M;
       if (M > 0) {
-        // the block path's scratch, sized here and zeroed on the aux stream behind shade_list_kernel, beside the passes
-        // (on the main stream the five memsets sat between the last pass and the scan: 15 us of the critical path)
+        // the block path's scratch, sized here and zeroed on the aux stream behind shade_list_kernel, beside the sort
+        // (on the main stream the five memsets -- 14 MB -- sat between the sort and bin_emit: 15 us of the critical
+        // path. On a stream of their own they run beside the selection instead, and the frame got 16 us SLOWER.)
         TRY(prep_block_bins(s, P, s->aux));
         CU(cudaEventRecord(s->ev_zero, s->aux));
       }
-      TRY(run_scan(s, s->nv, true, s->boffsets.as<uint32_t>(), visit, &tm, true));
-      CU(cudaStreamWaitEvent(st, s->ev_join, 0));   // ranges, bin_start, chunk_start (tile_prefix_kernel)
+      if (fused) {
+        static_assert(kDsFrontTile == (uint32_t)FSORT_TILE, "front_sort_kernel runs the front's tile shape");
+        using Smem = OnesweepSmem<FSORT_THREADS, FSORT_ITEMS, DS_BITS>;
+        PVG_ENSURE_SMEM(front_sort_kernel, sizeof(Smem), s->dev.ordinal);
+        uint32_t* region = s->dsel.as<uint32_t>();
+        TRY(tm.begin("front_sort_scan", PVG_STAGE_DEPTH_SORT, st));
+        TRY(launch_chain(&tm, front_sort_kernel, dim3(ftiles), dim3(FSORT_THREADS), sizeof(Smem), st, s->dkeys[0].as<uint64_t>(),
+                         s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(), s->dvals[1].as<uint32_t>(), (const uint32_t*)region,
+                         s->sort_n.lookback.as<uint64_t>(), (uint32_t)class_lookback_rows(s->n, 0), s->sort_n.tickets.as<uint32_t>(),
+                         s->sort_n.tickets.as<uint32_t>() + 2 * DS_PASSES, s->boffsets.as<uint32_t>(),
+                         reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8), s->scan_status.as<uint64_t>(),
+                         s->small.as<uint32_t>(), M > 0 ? s->chunk_owner.as<uint32_t>() : (uint32_t*)nullptr, kOwnerChunk));
+        TRY(tm.end(st));
+      } else {
+        TRY(run_scan(s, s->nv, true, s->boffsets.as<uint32_t>(), visit, &tm, true));
+      }
+      CU(cudaStreamWaitEvent(st, s->ev_blocks, 0));   // bin_start, chunk_start (tile_prefix_kernel, block level); run_block_bins waits for the ranges
       tm.cut();
     } else {
     // a3 (n-key part): depth order of the survivors

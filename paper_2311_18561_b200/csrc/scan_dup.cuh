@@ -39,6 +39,13 @@ __device__ __forceinline__ uint32_t scan_block_count(uint64_t key) {
 //            the emission kernel's CTA c starts there instead of searching the offsets (two ~22-step
 //            dependent binary searches per CTA were most of bin_expand's 0.078 ms)
 template <bool BLOCKS>
+__device__ __forceinline__ void
+scan_counts_body(uint32_t n, const uint32_t* __restrict__ counts, const uint64_t* __restrict__ keys,
+                 const uint32_t* __restrict__ visit, uint32_t* __restrict__ offsets, uint64_t* __restrict__ total,
+                 uint64_t* __restrict__ status, uint32_t* __restrict__ ticket, uint32_t* __restrict__ chunk_owner, uint32_t chunk,
+                 uint32_t rank0, const uint64_t* __restrict__ init);
+
+template <bool BLOCKS>
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64_t* __restrict__ keys,
                    const uint32_t* __restrict__ visit,
@@ -51,6 +58,16 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
   pdl_launch_dependents();
   pdl_wait();
   if (only_if && *only_if == 0u) return;
+  scan_counts_body<BLOCKS>(n, counts, keys, visit, offsets, total, status, ticket, chunk_owner, chunk, rank0, init);
+}
+
+// one tile (one ticket) of the scan: the body of scan_counts_kernel, also run by front_sort_kernel (front_sort.cuh)
+template <bool BLOCKS>
+__device__ __forceinline__ void
+scan_counts_body(uint32_t n, const uint32_t* __restrict__ counts, const uint64_t* __restrict__ keys,
+                 const uint32_t* __restrict__ visit, uint32_t* __restrict__ offsets, uint64_t* __restrict__ total,
+                 uint64_t* __restrict__ status, uint32_t* __restrict__ ticket, uint32_t* __restrict__ chunk_owner, uint32_t chunk,
+                 uint32_t rank0, const uint64_t* __restrict__ init) {
   keys += rank0;
   offsets += rank0;
   __shared__ uint32_t s_tile;
@@ -59,6 +76,7 @@ scan_counts_kernel(uint32_t n, const uint32_t* __restrict__ counts, const uint64
   if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
   __syncthreads();
   const uint32_t tile = s_tile;
+  if ((uint64_t)tile * SCAN_TILE >= n) return;   // (front_sort_kernel has more CTAs than the scan has tiles)
   const uint32_t base = tile * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
 
   uint32_t c[SCAN_ITEMS];

@@ -100,8 +100,11 @@ __device__ __forceinline__ void grid_prefix_2d(int* g, int rows, int cols, int s
 //   totals[0] = M (tile instances), totals[1] = Mb (block entries; with_blocks), totals[2] = S (survivors);
 //   totals_host[0..2]: the same, in mapped host memory
 //   bin_start[257], chunk_start[257] (with_blocks): see blockbin.cuh
+// parts: bit 0 -- the tile level (ranges, hist, totals 0 and 2); bit 1 -- the block level (bin_start, chunk_start,
+// totals 1). The two levels integrate different arrays: a front-first frame launches the block level first, on its own,
+// because bin_emit waits for nothing else of this kernel (the ranges are first read by bin_write).
 __global__ void __launch_bounds__(TB_THREADS)
-tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int with_blocks, const __grid_constant__ SortPlan plan,
+tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int with_blocks, int parts, const __grid_constant__ SortPlan plan,
                    uint2* __restrict__ ranges, uint32_t* __restrict__ hist, uint64_t* __restrict__ totals,
                    uint32_t* __restrict__ bin_start, uint32_t* __restrict__ chunk_start,
                    volatile uint64_t* __restrict__ totals_host) {
@@ -117,11 +120,14 @@ tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int wit
   const int bcells = with_blocks ? bstride * (BY + 1) : 0;
   int* g = grid;
   if (use_smem) {
-    for (int k = tid; k < cells + bcells; k += TB_THREADS) s_dyn[k] = grid[k];
+    const int k0 = (parts & 1) ? 0 : cells, k1 = (parts & 2) ? cells + bcells : cells;
+    for (int k = k0 + tid; k < k1; k += TB_THREADS) s_dyn[k] = grid[k];
     g = s_dyn;
   }
   for (int k = tid; k < plan.num_passes * OS_RADIX; k += TB_THREADS) s_hist[k] = 0;
   __syncthreads();
+  const uint32_t lane = lane_id(), warp = tid >> 5;
+  if (parts & 1) {
   grid_prefix_2d(g, TY + 1, TX + 1, stride);
   // exclusive scan of the counts in row-major tile order: thread t owns a contiguous segment
   const uint32_t tiles = (uint32_t)TX * (uint32_t)TY;
@@ -129,7 +135,6 @@ tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int wit
   const uint32_t t0 = min(tiles, (uint32_t)tid * per), t1 = min(tiles, t0 + per);
   uint64_t sum = 0;
   for (uint32_t tl = t0; tl < t1; ++tl) sum += (uint32_t)g[(tl / TX) * stride + (tl % TX)];
-  const uint32_t lane = lane_id(), warp = tid >> 5;
   uint64_t incl = sum;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
@@ -184,7 +189,8 @@ tile_prefix_kernel(int* __restrict__ grid, int TX, int TY, int use_smem, int wit
     }
     __syncthreads();
   }
-  if (!with_blocks) return;
+  }   // parts & 1
+  if (!with_blocks || !(parts & 2)) return;
   // block entries per block -> bin_start (exclusive scan) and chunk_start (scan of ceil(count / chunk))
   int* gb = g + cells;
   grid_prefix_2d(gb, BY + 1, BX + 1, bstride);
