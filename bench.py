@@ -273,7 +273,15 @@ def algorithmic_bytes(agg, K, N, S, Msum, Mbsum, chunks, lazy):
         # they move depends on where the tiles saturate, so no algorithmic-byte figure is claimed for them
         alg.pop(("bin_emit", "sort"), None)
         alg.pop(("bin_write", "sort"), None)
+    if ("depth_select", "depth_sort") in agg:
+        # front-first depth order (PVG_OPT_LAZY_DEPTH): the selection reads the n depth pairs (8 B) and writes the few
+        # pairs in front; the front's passes and scan (front_sort_scan, or onesweep_pass + scan_counts for a large
+        # front) move some ten thousand pairs -- latency, no byte figure claimed
+        alg[("depth_select", "depth_sort")] = agg[("depth_select", "depth_sort")][1] * 8.0 * N
+        alg.pop(("scan_counts", "duplicate"), None)
     for key in (("onesweep_pass", "sort"), ("onesweep_pass", "depth_sort")):
+        if key == ("onesweep_pass", "depth_sort") and ("depth_select", "depth_sort") in agg:
+            continue
         if key in agg:
             per_frame = agg[key][1] / K
             # depth sort (9 + 9 + 9 + 4 bits): pass 0 reads the n keys (8 B; the value of pair i is i) and writes the S

@@ -417,8 +417,12 @@ struct FrontCtl {
 // One wave: 1024 threads x 24 pairs = 24576 pairs per CTA, 123 CTAs for 3 M pairs. A pass like this is a chain of
 // latencies (ticket, loads, look-back, writes, last-CTA count) -- with tiles of 4096 it ran in three waves and took
 // three chains (ncu: 36 us, warps waiting at barriers).
-constexpr int SEL_THREADS = 1024;
-constexpr int SEL_ITEMS = 24;
+#ifndef PVG_SEL_THREADS
+#define PVG_SEL_THREADS 1024
+#define PVG_SEL_ITEMS 24
+#endif
+constexpr int SEL_THREADS = PVG_SEL_THREADS;
+constexpr int SEL_ITEMS = PVG_SEL_ITEMS;
 constexpr int SEL_TILE = SEL_THREADS * SEL_ITEMS;
 
 // Ordered selection of one class of pairs. keys: the n pairs of preprocess in index order (never overwritten).

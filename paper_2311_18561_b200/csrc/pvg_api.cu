@@ -527,6 +527,7 @@ struct pvg_scene {
   int lazy_depth = 1;                 // PVG_OPT_LAZY_DEPTH: with lazy lists, order the front of the scene first (onesweep.cuh)
   bool front_used = false;            // the last frame ordered its front first
   bool depth_complete = true;         // dvals[visit_side] holds all S survivors in depth order (pvg_debug_view completes it)
+  uint64_t prev_parked = 0;           // tiles the frame before this one parked (read at this frame's host wait)
   uint32_t front = 0;                 // F: the pairs in front of the threshold
   int top_front = 0, top_back = 0;    // the class has keys of 2^27 and beyond
   Buf front_idx;                      // front-first: the front's Gaussian indices once more, for shade_list_kernel
@@ -700,6 +701,7 @@ int init_workspace(pvg_scene* s) {
   CU(cudaStreamSynchronize(st));   // the first render may run on another stream: the zeroes must have landed
   CU(cudaEventCreateWithFlags(&s->ev_switch, cudaEventDisableTiming));
   CU(cudaHostAlloc((void**)&s->h_total, 128, cudaHostAllocMapped));
+  memset(s->h_total, 0, 128);
   CU(cudaHostGetDevicePointer((void**)&s->d_total, s->h_total, 0));
   CU(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
   CU(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
@@ -1367,6 +1369,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       // 0: the passes are launched here, before the wait, as launches that loop over tickets.
       if (!PVG_FRONT_FUSED) TRY(run_class_passes(s, 0, n, 0, 3, nullptr, &tm));
       CU(cudaEventSynchronize(s->ev_pre));
+      s->prev_parked = s->h_total[3];   // the frame before has completed (same stream): its parked count
       M = s->h_total[0];
       s->Mb = s->h_total[1];
       s->survivors = s->h_total[4];
@@ -1417,6 +1420,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
     CU(cudaEventSynchronize(s->ev_join));
     CU(cudaStreamWaitEvent(st, s->ev_join, 0));
     tm.cut();
+    s->prev_parked = s->h_total[3];
     M = s->h_total[0];
     s->Mb = block ? s->h_total[1] : 0;
     s->survivors = s->h_total[4];
@@ -1542,7 +1546,15 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       Z.blocks_x = bb_blocks(P.tiles_x);
     }
     R2Chain R2 = {};
-    if (lazy && PVG_R2_TAIL && PVG_BIN_FUSED) TRY(fill_r2(s, P, band_tiles, &R2));
+    // Who launches the second round? The device, when the frame before parked nothing: then this one most likely parks
+    // nothing either, and all the round costs is the one-thread gate. The host, when the frame before did park: grids
+    // launched from the device ran far slower than the same kernels launched from the host (the second blend phase of
+    // a frame whose 9600 tiles all park: 2.36 ms against 0.57 ms, the rest of the chain alike; a larger shared-memory
+    // carve-out for the gate, whose configuration its children inherit, changed nothing), so a scene that does park
+    // is better served by the host's launches, each of which looks at the parked count. Either way the frame is
+    // complete and bit-identical; a wrong guess costs time only (4.3 ms instead of 2.2 ms for the all-parked frame,
+    // 30 us of empty launches for a frame that parks nothing).
+    if (lazy && PVG_R2_TAIL && PVG_BIN_FUSED && s->prev_parked == 0) TRY(fill_r2(s, P, band_tiles, &R2));
 #define PVG_BLEND(C, M, PH) TRY(launch_chain(&tm, blend_kernel<C, M, PH>, dim3((PH) == 2 ? std::min(band_tiles, (uint32_t)s->dev.sms * 8u) : band_tiles), dim3(BLEND_THREADS), 0, st, P, rg, vl, rec, out_rgb, out_depth, out_alpha, ctr, (const float*)featw, Z))
 #define PVG_BLEND_ALL(PH)                                        \
     if (s->count_pairs) {                                        \
