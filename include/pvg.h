@@ -218,7 +218,8 @@ typedef enum pvg_option {
    *    every tile's whole list. 0: write the complete lists before the blend. */
   PVG_OPT_LAZY_CHUNKS = 11,
   /* d >= 1 (default 16), with LAZY_CHUNKS > 0: lazy emission. Only the first 1/d of the block entries, in depth order
-   *    (whole tiles of 4096), is formed and split by block before the first blend phase; a block's chunk counts for
+   *    (whole tiles of 4096; at least twice what the first LAZY_CHUNKS chunks of every block hold, so that small scenes
+   *    do not park for want of entries), is formed and split by block before the first blend phase; a block's chunk counts for
    *    that phase only if all of its 512 entries exist. The entries behind the slab are formed only if a tile was
    *    parked (the launch checks the count on the device). 1: form all entries up front. */
   PVG_OPT_LAZY_SLAB = 12,
@@ -233,7 +234,8 @@ typedef enum pvg_option {
    *    ignored): with lazy lists the same test already runs inside the blend on the few entries a tile consumes
    *    (BLEND_CULL), which is cheaper by two orders of magnitude -- this mode is for consumers of the lists themselves. */
   PVG_OPT_EXACT_TILES = 13,
-  /* 1 (default), with LAZY_CHUNKS > 0: front-first depth order. The first blend phase consumes the first slab of the
+  /* 0, 1 (default: on for scenes of at least 2^19 Gaussians, where it pays) or 2 (always on), with LAZY_CHUNKS > 0:
+   *    front-first depth order. The first blend phase consumes the first slab of the
    *    block entries in depth order, and those belong to the few Gaussians nearest the camera (about 1 % of the
    *    survivors at config 3: near Gaussians are large on screen). So the frame orders, scans and bins only that front:
    *    preprocess's last CTA picks a depth-key threshold from a histogram of the entries over the top key bits such

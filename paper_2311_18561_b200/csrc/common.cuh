@@ -49,16 +49,22 @@ struct FrameParams {
   const float* sky;   // cube map [6][res][res][3] or nullptr: rgb = C + (1 - O) f_sky(d)
   int sky_res;
   int lazy_slab;      // PVG_OPT_LAZY_SLAB (front-first depth order: preprocess sizes the front from it)
+  uint32_t lazy_min_tiles;   // floor of the first slab in bin_emit tiles (lazy_emit_first)
 };
 
 // Lazy lists: bin_emit forms the block entries in tiles of PVG_EMIT_TILE (== BF_TILE, blockbin.cuh); its first launch
 // takes the first 1 / lazy_slab of the tiles (at least one). One formula for the host and for preprocess's last CTA.
 #define PVG_EMIT_TILE 4096
-__host__ __device__ inline uint32_t lazy_emit_first(unsigned long long Mb, int lazy_slab) {
+// min_tiles: a floor -- twice what the first LAZY_CHUNKS chunks of every block hold (FrameParams::lazy_min_tiles): the
+// first round writes the lists as far as those chunks reach, and only chunks whose entries all exist count. At config 1
+// (40 blocks, 78 tiles of entries) a sixteenth of the entries is half of that, and 800 of the 2400 tiles parked.
+__host__ __device__ inline uint32_t lazy_emit_first(unsigned long long Mb, int lazy_slab, uint32_t min_tiles) {
   const uint32_t tiles = (uint32_t)((Mb + PVG_EMIT_TILE - 1) / PVG_EMIT_TILE);
   const uint32_t slab = lazy_slab > 0 ? (uint32_t)lazy_slab : 1u;
-  const uint32_t first = (tiles + slab - 1u) / slab;
-  return tiles < (first > 1u ? first : 1u) ? tiles : (first > 1u ? first : 1u);
+  uint32_t first = (tiles + slab - 1u) / slab;
+  if (first < min_tiles) first = min_tiles;
+  if (first < 1u) first = 1u;
+  return tiles < first ? tiles : first;
 }
 
 __device__ __forceinline__ uint32_t lane_id() {

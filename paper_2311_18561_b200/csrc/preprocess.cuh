@@ -458,7 +458,7 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
     cex += cin - csum; eex += ein - esum;   // exclusive of this thread's four buckets
     // the first slab: bin_emit's first launch forms the entries [0, emit_first * BF_TILE), and shade_kernel asks for
     // the owner of entry emit_first * BF_TILE: the front must hold more entries than that
-    const unsigned long long target = ((unsigned long long)lazy_emit_first(Mb, P.lazy_slab) + 1ull) * (unsigned long long)PVG_EMIT_TILE;
+    const unsigned long long target = ((unsigned long long)lazy_emit_first(Mb, P.lazy_slab, P.lazy_min_tiles) + 1ull) * (unsigned long long)PVG_EMIT_TILE;
     __shared__ uint32_t s_thr, s_front;
     if (threadIdx.x == 0) { s_thr = 0xFFFFFFFFu; s_front = S; }
     __syncthreads();

@@ -49,6 +49,19 @@ void* g_alloc_user = nullptr;
     if (rc_ != PVG_OK) return rc_; \
   } while (0)
 
+// The first slab of the lazy lists holds at least this many halves of (blocks x LAZY_CHUNKS chunks x 512) entries
+// (lazy_emit_first, common.cuh). Config 1 / config 2, ms per frame: 2 halves 0.2228 / 0.3151, 3: 0.2255 / 0.3107,
+// 4: 0.2489 / 0.3300 (no tile parks with any; without a floor 800 of config 1's 2400 tiles park at a slab of 1/16).
+#ifndef PVG_LAZY_FLOOR_HALVES
+#define PVG_LAZY_FLOOR_HALVES 3
+#endif
+// PVG_OPT_LAZY_DEPTH = 1 (auto): front-first depth order for scenes of at least this many Gaussians. Its fixed costs (the
+// selection's latency chain, one more launch) outweigh the sort it saves on small scenes: config 1 (200 k) 0.2255 ms per
+// frame with it, 0.2046 without; config 2 (1 M) 0.313 / 0.333; config 3 (3 M) 0.292 / 0.380.
+#ifndef PVG_LAZY_DEPTH_MIN_N
+#define PVG_LAZY_DEPTH_MIN_N (1u << 19)
+#endif
+
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: remember per (call site, device), thread-safe.
 #define PVG_ENSURE_SMEM(kern, bytes, dev)                                                              \
   do {                                                                                                 \
@@ -524,7 +537,7 @@ struct pvg_scene {
   // with the slab (36 k Gaussians at 8, 16 k at 16); beyond 16 nothing is left to gain and parking comes closer
   int lazy_slab = 16;
   int exact_tiles = 0;                // PVG_OPT_EXACT_TILES: list a Gaussian only in the tiles its ellipse can reach (P13)
-  int lazy_depth = 1;                 // PVG_OPT_LAZY_DEPTH: with lazy lists, order the front of the scene first (onesweep.cuh)
+  int lazy_depth = 1;                 // PVG_OPT_LAZY_DEPTH: with lazy lists, order the front of the scene first (onesweep.cuh); 1: auto (large scenes), 2: always
   bool front_used = false;            // the last frame ordered its front first
   bool depth_complete = true;         // dvals[visit_side] holds all S survivors in depth order (pvg_debug_view completes it)
   uint64_t prev_parked = 0;           // tiles the frame before this one parked (read at this frame's host wait)
@@ -766,6 +779,10 @@ int fill_frame(const pvg_scene* s, const pvg_camera* cam, const pvg_state* state
   P->sky = s->sky_res > 0 ? s->sky.as<float>() : nullptr;
   P->sky_res = s->sky_res;
   P->lazy_slab = s->lazy_slab;
+  {
+    const uint64_t nb = (uint64_t)bb_blocks(P->tiles_x) * bb_blocks(P->tiles_y);
+    P->lazy_min_tiles = (uint32_t)std::min<uint64_t>(((uint64_t)PVG_LAZY_FLOOR_HALVES * nb / 2 * (uint64_t)std::max(s->lazy_chunks, 0) * BB_CHUNK + PVG_EMIT_TILE - 1) / PVG_EMIT_TILE, 1u << 30);
+  }
   return PVG_OK;
 }
 
@@ -1056,7 +1073,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   // the first blend phase parks a tile
   s->lazy_used = s->lazy_chunks > 0 && !s->exact_used;   // exact lists are counted: every entry is formed and refined
   const uint32_t emit_tiles = (Mb + BF_TILE - 1) / BF_TILE;
-  s->emit_first = s->lazy_used ? lazy_emit_first(Mb, s->lazy_slab) : emit_tiles;
+  s->emit_first = s->lazy_used ? lazy_emit_first(Mb, s->lazy_slab, P.lazy_min_tiles) : emit_tiles;
   s->emit_tiles = emit_tiles;
   s->emit_radix = 1u << bits;
   s->visit_last = visit;
@@ -1141,6 +1158,7 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
 #ifndef PVG_R2_TAIL
 #define PVG_R2_TAIL 1
 #endif
+
 #ifndef PVG_FRONT_FUSED
 #define PVG_FRONT_FUSED 1
 #endif
@@ -1245,7 +1263,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
   // which forms them for the Gaussians in front only -- unless a tile parks; and only that front is ordered
   s->exact_used = block && s->exact_tiles && PVG_BIN_FUSED;
   s->light = block && s->lazy_chunks > 0 && PVG_BIN_FUSED && !s->exact_used;
-  s->front_used = s->light && s->lazy_depth;
+  s->front_used = s->light && (s->lazy_depth >= 2 || (s->lazy_depth == 1 && n >= PVG_LAZY_DEPTH_MIN_N));
   s->depth_complete = !s->front_used;
   s->records_complete = !s->light;
 
@@ -1785,7 +1803,10 @@ int pvg_set_option(pvg_scene* scene, int option, int64_t value) {
       scene->lazy_slab = (int)value;
       return PVG_OK;
     case PVG_OPT_EXACT_TILES: scene->exact_tiles = value ? 1 : 0; return PVG_OK;
-    case PVG_OPT_LAZY_DEPTH: scene->lazy_depth = value ? 1 : 0; return PVG_OK;
+    case PVG_OPT_LAZY_DEPTH:
+      if (value < 0 || value > 2) return PVG_ERR_BAD_OPTION;
+      scene->lazy_depth = (int)value;
+      return PVG_OK;
     case PVG_OPT_TILE_ROW_BEGIN:
       if (value < 0 || value > 2048) return PVG_ERR_BAD_OPTION;
       scene->band_begin = (int)value;

@@ -64,6 +64,9 @@ def main():
         sc.set_option(pvg.OPT_COMPACT_KEYS, 0); same("64-bit keys, depth presort")
         sc.set_option(pvg.OPT_PRESORT_DEPTH, 0); same("64-bit keys, index order")
         sc.set_option(pvg.OPT_PRESORT_DEPTH, 1); sc.set_option(pvg.OPT_COMPACT_KEYS, 1); sc.set_option(pvg.OPT_BLOCK_BINS, 1)
+        sc.set_option(pvg.OPT_LAZY_DEPTH, 2); same("front-first depth order")
+        sc.set_option(pvg.OPT_LAZY_SLAB, 64); same("front-first depth order, small slab")
+        sc.set_option(pvg.OPT_LAZY_SLAB, 16); sc.set_option(pvg.OPT_LAZY_DEPTH, 1)
         sc.set_option(pvg.OPT_BLEND_CULL, 0); same("no staging cull")
         sc.set_option(pvg.OPT_BLEND_CULL, 1)
         # sky, dynamics target, temporal-smoothing state, a band of tile rows
@@ -80,13 +83,16 @@ def main():
         thin.set_option(pvg.OPT_LAZY_CHUNKS, 0)
         full = [x.clone() for x in thin.render(cam, 0.37)]
         thin.set_option(pvg.OPT_LAZY_CHUNKS, 1); thin.set_option(pvg.OPT_LAZY_SLAB, 64)
-        lazy = thin.render(cam, 0.37)
-        torch.cuda.synchronize()
-        assert all(torch.equal(a, b) for a, b in zip(full, lazy)), "parked scene"
-        guards("parked scene")
+        for ld in (1, 2, 2):   # front-first order: the first parking frame runs the device-launched second round, the next the host's
+            thin.set_option(pvg.OPT_LAZY_DEPTH, ld)
+            lazy = thin.render(cam, 0.37)
+            torch.cuda.synchronize()
+            assert all(torch.equal(a, b) for a, b in zip(full, lazy)), "parked scene"
+            guards("parked scene")
+            frames += 1
         print(f"config {cfg}: parked tiles {thin.frame_stats()['parked_tiles']}")
         thin.close()
-        frames += 2
+        frames += 1
     # the sort primitive on its own
     keys = torch.randint(0, 2 ** 62, (300_003,), dtype=torch.int64, device="cuda")
     vals = torch.arange(300_003, dtype=torch.int32, device="cuda")

@@ -593,7 +593,7 @@ def test_depth_sort_key_range(znear, top_pass, lazy_depth):
     cam = wl.cameras[0]
     cam.znear = znear
     sc = pvg.Scene.from_workload_scene(wl.scene)
-    sc.set_option(pvg.OPT_LAZY_DEPTH, lazy_depth)
+    sc.set_option(pvg.OPT_LAZY_DEPTH, 2 * lazy_depth)   # 2: always (80 k Gaussians are below the automatic threshold)
     sc.set_option(pvg.OPT_KEEP_UNSORTED, 1)
     sc.set_option(pvg.OPT_KERNEL_EVENTS, 1)
     sc.render(cam, 0.5)
@@ -671,7 +671,7 @@ def test_front_first_depth_order(cfg, n, thin, slab):
     st0 = sc.frame_stats()
     d0 = sc.debug(["visit_order", "offsets", "vals_sorted", "ranges", "counts", "record"])
     assert st0["front"] == 0
-    sc.set_option(pvg.OPT_LAZY_DEPTH, 1)
+    sc.set_option(pvg.OPT_LAZY_DEPTH, 2)   # always (1, the default, turns it on for large scenes only)
     for rep in range(2):   # twice: the second frame runs on the scratch the first one left
         out = sc.render(cam, 0.37)
         torch.cuda.synchronize()
