@@ -22,9 +22,9 @@ constexpr int FSORT_TILE = FSORT_THREADS * FSORT_ITEMS;
 static_assert(FSORT_THREADS == SCAN_THREADS, "the scan tiles are run by the same thread blocks");
 static_assert(SCAN_TILE >= FSORT_TILE, "a grid of one CTA per sort tile covers the scan's tiles");
 
-// All CTAs of the grid are resident (the host launches at most as many as fit beside nothing else, and the kernels of
-// the other streams it shares the GPU with -- tile grid, shade -- finish on their own): a CTA that waits here waits for
-// CTAs that are running or will be scheduled without its help. bar: zeroed; target = gridDim.x * (barriers so far).
+// The kernel is launched cooperatively (cudaLaunchAttributeCooperative; the host launches at most 2 CTAs per SM, which
+// its launch bounds let fit): all CTAs of the grid are resident together, so a CTA that waits here waits for CTAs that are
+// running. bar: zeroed; target = gridDim.x * (barriers so far).
 __device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t target) {
   __syncthreads();
   if (threadIdx.x == 0) {

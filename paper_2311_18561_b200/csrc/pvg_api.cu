@@ -85,10 +85,11 @@ struct DeviceGuard {
 
 // device ordinal and SM count, looked up once (pvg_create_scene) instead of on every frame
 struct Dev {
-  int ordinal = 0, sms = 1;
+  int ordinal = 0, sms = 1, coop = 0;   // coop: cooperative launches supported (front_sort_kernel)
   int query() {
     CU(cudaGetDevice(&ordinal));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ordinal));
+    CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ordinal));
     return PVG_OK;
   }
 };
@@ -1398,7 +1399,7 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       s->visit_side = s->top_front ? 1 : 0;
       visit = s->dvals[s->visit_side].as<uint32_t>();
       const uint32_t ftiles = (s->front + kDsFrontTile - 1) / kDsFrontTile;
-      const bool fused = PVG_FRONT_FUSED && s->front > 0 && ftiles <= (uint32_t)s->dev.sms * 2u;
+      const bool fused = PVG_FRONT_FUSED && s->dev.coop && s->front > 0 && ftiles <= (uint32_t)s->dev.sms * 2u;
       if (PVG_FRONT_FUSED && !fused) TRY(run_class_passes(s, 0, s->front, 0, 3, nullptr, &tm));
       if (!fused && s->top_front) TRY(run_class_passes(s, 0, s->front, 3, 4, nullptr, &tm));
       if (M >= (1ull << 32) - 65536 || s->Mb >= (1ull << 32) - 65536) return PVG_ERR_INSTANCE_OVERFLOW;
@@ -1416,12 +1417,26 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
         PVG_ENSURE_SMEM(front_sort_kernel, sizeof(Smem), s->dev.ordinal);
         uint32_t* region = s->dsel.as<uint32_t>();
         TRY(tm.begin("front_sort_scan", PVG_STAGE_DEPTH_SORT, st));
-        TRY(launch_chain(&tm, front_sort_kernel, dim3(ftiles), dim3(FSORT_THREADS), sizeof(Smem), st, s->dkeys[0].as<uint64_t>(),
-                         s->dvals[0].as<uint32_t>(), s->dkeys[1].as<uint64_t>(), s->dvals[1].as<uint32_t>(), (const uint32_t*)region,
-                         s->sort_n.lookback.as<uint64_t>(), (uint32_t)class_lookback_rows(s->n, 0), s->sort_n.tickets.as<uint32_t>(),
-                         s->sort_n.tickets.as<uint32_t>() + 2 * DS_PASSES, s->boffsets.as<uint32_t>(),
-                         reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8), s->scan_status.as<uint64_t>(),
-                         s->small.as<uint32_t>(), M > 0 ? s->chunk_owner.as<uint32_t>() : (uint32_t*)nullptr, kOwnerChunk));
+        {
+          // a COOPERATIVE launch: the grid waits on itself (grid_barrier), so all of its CTAs must be resident together
+          // whatever else shares the device -- a second frame in flight (pvg_fork_scene) runs the same kernel, and two
+          // such grids admitted half each would wait for one another for ever. The attribute makes the co-residency the
+          // driver's guarantee instead of an assumption (no programmatic dependent launch for this kernel then).
+          cudaLaunchConfig_t cfg = {};
+          cfg.gridDim = dim3(ftiles); cfg.blockDim = dim3(FSORT_THREADS); cfg.dynamicSmemBytes = sizeof(Smem); cfg.stream = st;
+          cudaLaunchAttribute at[1];
+          at[0].id = cudaLaunchAttributeCooperative;
+          at[0].val.cooperative = 1;
+          cfg.attrs = at; cfg.numAttrs = 1;
+          CU(cudaLaunchKernelEx(&cfg, front_sort_kernel, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(),
+                                s->dkeys[1].as<uint64_t>(), s->dvals[1].as<uint32_t>(), (const uint32_t*)region,
+                                s->sort_n.lookback.as<uint64_t>(), (uint32_t)class_lookback_rows(s->n, 0),
+                                s->sort_n.tickets.as<uint32_t>(), s->sort_n.tickets.as<uint32_t>() + 2 * DS_PASSES,
+                                s->boffsets.as<uint32_t>(), reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8),
+                                s->scan_status.as<uint64_t>(), s->small.as<uint32_t>(),
+                                M > 0 ? s->chunk_owner.as<uint32_t>() : (uint32_t*)nullptr, (uint32_t)kOwnerChunk));
+          tm.pdl_open = true; tm.pdl_stream = st;   // the next kernel of the chain may still be ITS programmatic dependent
+        }
         TRY(tm.end(st));
       } else {
         TRY(run_scan(s, s->nv, true, s->boffsets.as<uint32_t>(), visit, &tm, true));
