@@ -1428,13 +1428,14 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
           at[0].id = cudaLaunchAttributeCooperative;
           at[0].val.cooperative = 1;
           cfg.attrs = at; cfg.numAttrs = 1;
-          CU(cudaLaunchKernelEx(&cfg, front_sort_kernel, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(),
+          const cudaError_t launched = (cudaLaunchKernelEx(&cfg, front_sort_kernel, s->dkeys[0].as<uint64_t>(), s->dvals[0].as<uint32_t>(),
                                 s->dkeys[1].as<uint64_t>(), s->dvals[1].as<uint32_t>(), (const uint32_t*)region,
                                 s->sort_n.lookback.as<uint64_t>(), (uint32_t)class_lookback_rows(s->n, 0),
                                 s->sort_n.tickets.as<uint32_t>(), s->sort_n.tickets.as<uint32_t>() + 2 * DS_PASSES,
                                 s->boffsets.as<uint32_t>(), reinterpret_cast<uint64_t*>(s->small.as<unsigned char>() + 8),
                                 s->scan_status.as<uint64_t>(), s->small.as<uint32_t>(),
                                 M > 0 ? s->chunk_owner.as<uint32_t>() : (uint32_t*)nullptr, (uint32_t)kOwnerChunk));
+          CU(launched);
           tm.pdl_open = true; tm.pdl_stream = st;   // the next kernel of the chain may still be ITS programmatic dependent
         }
         TRY(tm.end(st));
