@@ -60,6 +60,9 @@ def _check_frame(sc, wl_scene, cam, t, n_random_tiles=10, seed=0, end_to_end=Tru
     rgb, depth, alpha = (x.cpu().numpy() for x in out)
     st = sc.frame_stats()
     assert st["list_mode"] == "blocks"
+    # the launch configuration bench.py times: at these sizes (n >= 2^19) the default options order the front of the scene
+    # only -- everything below is checked on what pvg_debug_view completes from such a frame
+    assert 0 < st["front"] < st["survivors"], st
     d = sc.debug_info()
     n, M = int(d.n), int(d.num_instances)
     TX, TY = int(d.tiles_x), int(d.tiles_y)

@@ -671,6 +671,12 @@ def test_front_first_depth_order(cfg, n, thin, slab):
     st0 = sc.frame_stats()
     d0 = sc.debug(["visit_order", "offsets", "vals_sorted", "ranges", "counts", "record"])
     assert st0["front"] == 0
+    if wl.scene.n < (1 << 19):   # the default (1) leaves small scenes to the whole-scene sort
+        sc.set_option(pvg.OPT_LAZY_DEPTH, 1)
+        sc.render(cam, 0.37)
+        assert sc.frame_stats()["front"] == 0
+    with pytest.raises(pvg.PvgError):
+        sc.set_option(pvg.OPT_LAZY_DEPTH, 3)
     sc.set_option(pvg.OPT_LAZY_DEPTH, 2)   # always (1, the default, turns it on for large scenes only)
     for rep in range(2):   # twice: the second frame runs on the scratch the first one left
         out = sc.render(cam, 0.37)
