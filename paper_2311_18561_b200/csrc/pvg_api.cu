@@ -1165,10 +1165,13 @@ int run_block_bins(pvg_scene* s, const FrameParams& P, const uint32_t* visit, Ti
   TRY(tm->begin("bin_write", PVG_STAGE_SORT, st));
   TRY(launch_bin_write(s, P, 0u, s->lazy_used ? (uint32_t)s->lazy_chunks : 0xFFFFFFFFu, false, 1));
   TRY(tm->end(st));
-  if (s->light) {   // the blend reads the records
-    CU(cudaStreamWaitEvent(st, s->front_used ? s->ev_aux : s->ev_join, 0));
+  if (s->light && !s->front_used) {   // the blend reads the records
+    CU(cudaStreamWaitEvent(st, s->ev_join, 0));
     tm->cut();
   }
+  // (front-first frames: shade_list_kernel ran on the aux stream ahead of the zeroing kernel whose event, ev_zero, the
+  // main stream waited for before bin_emit -- nothing sits between bin_write and the blend, which is launched as its
+  // programmatic dependent)
   CU(cudaGetLastError());
   s->sorted_side = 0;
   return PVG_OK;
