@@ -530,7 +530,7 @@ def run_ours(args):
         roofline = {"bound": "hbm", "achieved": dk.get("GBps"), "peak": hbm_peak, "unit": "GB/s", "frac": dk.get("hbm_frac"),
                     "traffic": ncu_traffic(dom[0], workload), "kernel": f"{dom[0]} ({dom[1]} stage)",
                     "peak_source": peak_src, "avg_launch_ms": dk["ms_avg"],
-                    "algorithmic_bytes_per_launch": alg[dom] / agg[dom][1]}
+                    "algorithmic_bytes_per_launch": (alg[dom] / agg[dom][1]) if dom in alg else None}
 
     # ---- extra legs (1 GPU only): complete lists, a scene whose tiles park, a sustained loop
     legs = {}

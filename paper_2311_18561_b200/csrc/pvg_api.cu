@@ -1009,7 +1009,12 @@ int prep_block_bins(pvg_scene* s, const FrameParams& P, cudaStream_t zs) {
     zl.add(s->unf.p, kUnfHead + tiles * 4);   // masks, count and lim; the list is written before it is read
   }
   zl.add(s->sort_m.lookback.p, (size_t)pass_tiles * OS_RADIX * 8);
+  Timer& tm = s->timer;
+  tm.cut();
+  TRY(tm.begin("zero_scratch", PVG_STAGE_SORT, zs));
   zero_regions_kernel<<<std::max(1, s->dev.sms * 4), 256, 0, zs>>>(zl);
+  TRY(tm.end(zs));
+  tm.cut();
   CU(cudaGetLastError());
   return PVG_OK;
 }
