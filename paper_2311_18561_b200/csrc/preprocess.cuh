@@ -330,9 +330,7 @@ preprocess_loaded(const FrameParams& P, uint32_t n, uint32_t i, const float4 a0,
 #ifndef PVG_PRE_PF
 #define PVG_PRE_PF 1
 #endif
-#ifndef PVG_PRE_PIPE
-#define PVG_PRE_PIPE 0
-#endif
+
 constexpr int PRE_CHUNKS = PVG_PRE_CHUNKS;
 
 // FRONT (lazy lists with the front-first depth order, onesweep.cuh): instead of the digits the CTA counts, per bucket
@@ -356,10 +354,6 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
     __syncthreads();
   }
   uint32_t inst = 0;   // FRONT: tile instances of this thread's survivors
-#if PVG_PRE_PIPE
-  float4 q0, q1, q2, q3;
-  bool qf = false;
-#endif
 #pragma unroll 1
   for (int c = 0; c < PRE_CHUNKS; ++c) {
     const uint32_t i = (blockIdx.x * PRE_CHUNKS + c) * 256u + threadIdx.x;
@@ -372,22 +366,7 @@ preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8
       asm volatile("prefetch.global.L2 [%0];" ::"l"(A3 + i + 256));
     }
 #endif
-#if PVG_PRE_PIPE
-    // software pipeline: the next chunk's model values are in flight while this one is computed
-    if (c == 0) {
-      q0 = ldg_stream_f4(A0 + i); q1 = ldg_stream_f4(A1 + i); q2 = ldg_stream_f4(A2 + i); q3 = ldg_stream_f4(A3 + i);
-      qf = PART != PRE_GEO || (shflag != nullptr && __ldg(shflag + i) != 0);
-    }
-    const float4 c0 = q0, c1 = q1, c2 = q2, c3 = q3;
-    const bool cf = qf;
-    if (c + 1 < PRE_CHUNKS && i + 256u < n) {
-      q0 = ldg_stream_f4(A0 + i + 256); q1 = ldg_stream_f4(A1 + i + 256); q2 = ldg_stream_f4(A2 + i + 256); q3 = ldg_stream_f4(A3 + i + 256);
-      qf = PART != PRE_GEO || (shflag != nullptr && __ldg(shflag + i + 256) != 0);
-    }
-    const uint64_t key = preprocess_loaded<PART>(P, n, i, c0, c1, c2, c3, cf, SH, record, tileinfo, counts, dkeys, dvals, featw);
-#else
     const uint64_t key = preprocess_point<PART>(P, n, i, shflag, A0, A1, A2, A3, SH, record, tileinfo, counts, dkeys, dvals, featw);
-#endif
     const uint32_t z = (uint32_t)key;
     if (dhist && z != 0xFFFFFFFFu) {
       if (FRONT) {
