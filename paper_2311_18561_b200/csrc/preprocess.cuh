@@ -337,8 +337,14 @@ constexpr int PRE_CHUNKS = PVG_PRE_CHUNKS;
 // of the top key bits (key >> FR_SHIFT), its survivors and their block entries, and sums their tile instances; the last
 // CTA picks the key threshold below which the first slab's owners lie (FrontCtl) and hands the frame's totals to the
 // host: M, Mb, S, F -- all the host waits for.
+// The geometry-only pass at 6 CTAs per SM (40 registers, 180 bytes of spills) instead of the 4 (64 registers) the compiler
+// picks on its own: config 3 frame 0.2890 -> 0.2842 ms, config 4 0.6395 -> 0.6310 (5 CTAs: 0.2845; 7 and 8: 0.310 -- 32
+// registers, 340 bytes of spills). The full pass (records with SH colour) keeps the compiler's choice (0: no minimum).
+#ifndef PVG_PRE_MINB
+#define PVG_PRE_MINB 6
+#endif
 template <int PART, bool FRONT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, PART == PRE_GEO ? PVG_PRE_MINB : 0)
 preprocess_kernel(const __grid_constant__ FrameParams P, uint32_t n, const uint8_t* __restrict__ shflag,
                   const float4* __restrict__ A0, const float4* __restrict__ A1,
                   const float4* __restrict__ A2, const float4* __restrict__ A3,
