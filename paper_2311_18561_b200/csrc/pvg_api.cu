@@ -1436,7 +1436,8 @@ int render_impl(pvg_scene* s, const pvg_camera* cam, const pvg_state* state, flo
       if (M > 0) {
         // the block path's scratch, sized here and zeroed on the aux stream behind shade_list_kernel, beside the sort
         // (on the main stream the five memsets -- 14 MB -- sat between the sort and bin_emit: 15 us of the critical
-        // path. On a stream of their own they run beside the selection instead, and the frame got 16 us SLOWER.)
+        // path. On a stream of their own they run beside the selection instead, and the frame got 14-16 us SLOWER: a CTA
+        // of depth_select_kernel takes a whole SM's registers and has to wait for whatever got onto the SMs first.)
         TRY(prep_block_bins(s, P, s->aux));
         CU(cudaEventRecord(s->ev_zero, s->aux));
       }
